@@ -1,0 +1,160 @@
+/*
+ * pa_b200.h -- C ABI of the B200-native population-annealing (PA) hot path for the 2D Ising model.
+ *
+ * What is computed is defined by arxiv 2006.00561 and the readings in DESIGN.md:
+ *   reweight   Q(beta,beta') = sum_j exp[-(beta'-beta) E_j] / R            PAPER.md:46  eq. (3), :94
+ *              tau_j = exp[-(beta'-beta) E_j] / Q                           PAPER.md:51  eq. (4)
+ *   resample   n_j ~ Poisson(tau_j * R0/R), offspring = exact copies
+ *   redistribute  new population balanced over P logical partitions
+ *   equilibrate   theta MCMC (checkerboard Metropolis) sweeps at beta'
+ *   observe    population sums of E, E^2, |M|, M^2, M^4; ln Z recursion     PAPER.md:62, :66 eq. (5)
+ *   model      H = -(J/2) sum' sigma sigma', J = 1, periodic L x L          PAPER.md:76-80 eq. (6)
+ *
+ * Conventions
+ *   - plain C, no exceptions; every function returns PA_OK (0) or a negative pa_status;
+ *     pa_last_error(ctx) gives a message for the last failure on that context.
+ *   - pointers marked DEVICE are CUDA device pointers, HOST are host pointers; getters take a flag
+ *     saying which kind `dst` is.  All device work is issued on cfg.stream.
+ *   - ownership: the CALLER owns the device workspace and the stream (PyTorch allocates both); the library
+ *     owns only the host-side pa_ctx (and a few bytes of pinned host memory inside it).  pa_destroy never
+ *     frees the workspace.
+ *   - packed lattice layout ("C2" in DESIGN.md): a replica is an N = L*L bit little-endian string, spin (x,y)
+ *     is bit b = y*L + x, stored in uint32 word b>>5 at bit b&31, bit 1 <-> sigma = +1; slot i of the
+ *     population starts at byte i * N/8.
+ *   - one context per host thread; a context is bound to the device that was current in pa_init.
+ *   - there is NO CPU fallback: without a CUDA device pa_init returns PA_ECUDA.
+ */
+#ifndef PA_B200_H
+#define PA_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pa_ctx pa_ctx; /* opaque, host side, library owned */
+
+typedef enum {
+  PA_OK = 0,
+  PA_EINVAL = -1,    /* bad argument (L, P, theta, NaN beta, |dbeta|*2N >= 700, getter without its KEEP flag) */
+  PA_ENOMEM = -2,    /* workspace smaller than pa_workspace_bytes(cfg) */
+  PA_ECAPACITY = -3, /* resampled population R' > capacity: step NOT committed, population unchanged */
+  PA_EEXTINCT = -4,  /* R' = 0: step NOT committed, population unchanged */
+  PA_ECUDA = -5      /* CUDA runtime error (message in pa_last_error) */
+} pa_status;
+
+enum {
+  PA_KEEP_TAU = 1u,    /* materialise tau_j of every step (8 B per parent) for pa_tau */
+  PA_KEEP_COUNTS = 2u, /* materialise n_j of every step (4 B per parent) for pa_counts(n != NULL) */
+  PA_PROFILE = 4u      /* record CUDA events around every kernel (pa_profile_read) */
+};
+
+typedef struct {
+  int32_t L;        /* lattice side: 8, 16, 32, 64 or 128 */
+  int32_t P;        /* logical partitions, >= 1 (148 = one per B200 SM) */
+  int64_t R0;       /* initial = target population R_beta0, 1 <= R0 < 2^31 */
+  int64_t capacity; /* slots per population buffer; 0 => R0 + max(1024, 16*ceil(sqrt(R0))) rounded up to 1024 */
+  uint64_t seed;    /* Philox key */
+  double beta0;     /* inverse temperature the initial population is declared to be at (uniform init is exact for 0) */
+  void* workspace;  /* DEVICE memory, caller owned, 256-byte aligned, >= pa_workspace_bytes(cfg) */
+  uint64_t workspace_bytes;
+  void* stream;     /* cudaStream_t, caller owned (NULL = legacy default stream) */
+  uint32_t flags;   /* PA_KEEP_TAU | PA_KEEP_COUNTS | PA_PROFILE */
+  uint32_t reserved;
+} pa_config;
+
+/* population sums after the last committed step (or after pa_init / pa_set_spins); 128-bit integers as {lo, hi} */
+typedef struct {
+  int64_t R;            /* population size the sums run over */
+  int64_t sum_E;        /* sum_j E_j                     (|sum| < 2^63 for every supported size) */
+  uint64_t sum_E2[2];   /* sum_j E_j^2 */
+  uint64_t sum_absM[2]; /* sum_j |M_j| */
+  uint64_t sum_M2[2];   /* sum_j M_j^2 */
+  uint64_t sum_M4[2];   /* sum_j M_j^4                   (exceeds 2^64 for L = 128, R = 2^20) */
+  double mean_E, mean_E2, mean_absM, mean_M2, mean_M4; /* sums / R in fp64 */
+} pa_obs;
+
+/* per-partition diagnostics of the last step, in the paper's vocabulary */
+typedef struct {
+  uint32_t cnt;  /* replicas the partition holds after redistribution ("desired" r_n; counts differ by <= 1) */
+  uint32_t born; /* offspring of the parents that lived in this partition (what it would hold without redistribution) */
+  uint32_t maxg; /* excess   max(0, born - cnt) */
+  uint32_t minl; /* shortage max(0, cnt - born) */
+} pa_part_stats;
+
+/* kernels of one pa_step, in launch order (indices of pa_profile_read arrays) */
+enum {
+  PA_K_LEVELS_W = 0, /* w_e = exp(-dbeta e) per energy level */
+  PA_K_Q_REDUCE,     /* eq. 3: fp64 warp-shuffle reduction, Q, ln Q */
+  PA_K_LEVELS_TAU,   /* eq. 4 per level + Poisson chunk tables */
+  PA_K_POISSON_SCAN, /* Poisson copy counts + single-pass exclusive scan */
+  PA_K_BALANCE,      /* partition table + diagnostics */
+  PA_K_COPY,         /* replica redistribution (gather copy) */
+  PA_K_SWEEP,        /* theta checkerboard Metropolis sweeps + E, M */
+  PA_K_OBSERVE,      /* population sums + commit of the step */
+  PA_K_COUNT
+};
+
+/* Bytes of device workspace needed for cfg (L, R0, capacity, P, flags are read).  0 on invalid cfg. */
+uint64_t pa_workspace_bytes(const pa_config* cfg);
+
+/* a0. Create a context and the initial population: R0 replicas of uniform +-1 spins from Philox (seed),
+ * E_j, M_j, ln Omega = N ln 2.  Synchronises the stream before returning. */
+int pa_init(const pa_config* cfg, pa_ctx** out);
+
+/* a1-a8. One temperature step beta -> beta_next with theta >= 0 sweeps.  Synchronous: returns after the step's
+ * kernels finished and its status was read back.  On PA_ECAPACITY / PA_EEXTINCT the population, beta, step
+ * counter and ln Z are unchanged. */
+int pa_step(pa_ctx* ctx, double beta_next, int32_t theta);
+
+/* K steps beta_k = betas[k] (HOST array of K doubles), all launched back to back with ONE synchronisation at the
+ * end; stops committing at the first failing step (later steps are no-ops) and reports it.  *steps_done (may be
+ * NULL) receives the number of committed steps. */
+int pa_run(pa_ctx* ctx, const double* betas, int32_t K, int32_t theta, int32_t* steps_done);
+
+int pa_population(pa_ctx* ctx, int64_t* R);
+int pa_beta(pa_ctx* ctx, double* beta, int64_t* steps);
+
+/* E_j (and M_j) of slots 0..n-1 of the current population, slot order.  n <= R.  M may be NULL. */
+int pa_energies(pa_ctx* ctx, int32_t* E, int32_t* M, int64_t n, int dst_on_device);
+
+/* eq. 5 (reading G1): *lnZ = N ln 2 + sum_lnQ; *last_Q = Q of the last committed step. NULLs allowed. */
+int pa_log_Z(pa_ctx* ctx, double* lnZ, double* sum_lnQ, double* last_Q);
+
+int pa_observables(pa_ctx* ctx, pa_obs* out);
+
+/* ---- parity / debug getters --------------------------------------------------------------------------- */
+/* packed lattices of slots first..first+count-1 (count * N/32 uint32 words) */
+int pa_spins(pa_ctx* ctx, uint32_t* dst, int64_t first, int64_t count, int dst_on_device);
+/* tau_j of the LAST step's parents, j = 0..n-1, n <= number of parents (needs PA_KEEP_TAU) */
+int pa_tau(pa_ctx* ctx, double* dst, int64_t n, int dst_on_device);
+/* copy counts n_j (needs PA_KEEP_COUNTS; may be NULL) and exclusive offsets off_j, j = 0..n_parents (off has
+ * n_parents+1 entries, off[n_parents] = R') of the LAST step */
+int pa_counts(pa_ctx* ctx, uint32_t* n, uint32_t* off, int64_t n_parents, int dst_on_device);
+/* number of parents of the last step (population size before it) */
+int pa_parents(pa_ctx* ctx, int64_t* n_parents);
+/* partition table of the current population (HOST, P+1 entries) and the last step's diagnostics (HOST, P
+ * entries, may be NULL); *moved (may be NULL) = children whose partition differs from their parent's */
+int pa_partitions(pa_ctx* ctx, uint32_t* part_start, pa_part_stats* stats, int64_t* moved);
+/* acceptance thresholds used by the last step with theta > 0 */
+int pa_thresholds(pa_ctx* ctx, uint32_t* T4, uint32_t* T8);
+/* test hook: replace the population by R packed lattices (R <= capacity); recomputes E, M, sums, partitions;
+ * beta, step counter and ln Z are kept */
+int pa_set_spins(pa_ctx* ctx, const uint32_t* src, int64_t R, int src_on_device);
+
+/* ---- profiling (PA_PROFILE) --------------------------------------------------------------------------- */
+/* Sum of CUDA-event durations (ms) and number of launches per kernel since the last call; synchronises.
+ * Both arrays have PA_K_COUNT entries (HOST). */
+int pa_profile_read(pa_ctx* ctx, double* ms, int64_t* launches);
+/* total number of kernels this context has launched since pa_init (all kernels, profiled or not) */
+int pa_launch_count(pa_ctx* ctx, int64_t* launches);
+
+const char* pa_last_error(pa_ctx* ctx);
+int pa_destroy(pa_ctx* ctx); /* frees the host context only */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PA_B200_H */

@@ -156,10 +156,11 @@ void orc_init_population(int L, int64_t R, uint64_t seed, uint32_t* packed) {
     int8_t* s = (int8_t*)malloc((size_t)N);
 #pragma omp for schedule(static)
     for (int64_t j = 0; j < R; ++j) {
+      uint32_t w[4] = {0, 0, 0, 0};
       for (int b = 0; b < N; ++b) {
-        uint32_t v = (uint32_t)(b >> 5);
-        uint32_t w[4];
-        philox_keyed(seed, v >> 2, (uint32_t)j, 0u, TAG_INIT, 0u, w);
+        uint32_t v = (uint32_t)(b >> 5); /* word that holds bit b */
+        if ((b & 127) == 0)              /* one Philox block serves four consecutive words = 128 spins */
+          philox_keyed(seed, v >> 2, (uint32_t)j, 0u, TAG_INIT, 0u, w);
         uint32_t word = w[v & 3];
         s[b] = ((word >> (b & 31)) & 1u) ? (int8_t)1 : (int8_t)-1;
       }

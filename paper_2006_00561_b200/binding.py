@@ -1,0 +1,241 @@
+"""ctypes binding of libpa_b200.so (include/pa_b200.h): argument marshalling only.
+
+PyTorch is used for device memory (the workspace tensor) and the stream; every step of the path runs in
+the library's CUDA kernels.  There is no CPU fallback: a missing library or a missing GPU raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libpa_b200.so")
+
+PA_OK, PA_EINVAL, PA_ENOMEM, PA_ECAPACITY, PA_EEXTINCT, PA_ECUDA = 0, -1, -2, -3, -4, -5
+PA_KEEP_TAU, PA_KEEP_COUNTS, PA_PROFILE = 1, 2, 4
+KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "copy", "sweep", "observe"]
+
+EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_population", "pa_beta", "pa_energies", "pa_log_Z",
+           "pa_observables", "pa_spins", "pa_tau", "pa_counts", "pa_parents", "pa_partitions", "pa_thresholds",
+           "pa_set_spins", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
+
+
+class PaConfig(C.Structure):
+    _fields_ = [("L", C.c_int32), ("P", C.c_int32), ("R0", C.c_int64), ("capacity", C.c_int64), ("seed", C.c_uint64),
+                ("beta0", C.c_double), ("workspace", C.c_void_p), ("workspace_bytes", C.c_uint64),
+                ("stream", C.c_void_p), ("flags", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+class PaObs(C.Structure):
+    _fields_ = [("R", C.c_int64), ("sum_E", C.c_int64), ("sum_E2", C.c_uint64 * 2), ("sum_absM", C.c_uint64 * 2),
+                ("sum_M2", C.c_uint64 * 2), ("sum_M4", C.c_uint64 * 2), ("mean_E", C.c_double), ("mean_E2", C.c_double),
+                ("mean_absM", C.c_double), ("mean_M2", C.c_double), ("mean_M4", C.c_double)]
+
+
+class PaError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("pa_b200 error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libpa_b200.so and declare the prototypes.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libpa_b200.so is not built (run `python -m paper_2006_00561_b200.build`); "
+                          "there is no CPU fallback")
+    lib = C.CDLL(LIB_PATH)
+    vp, i64p, i32p, u32p, f64p = C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32), C.POINTER(C.c_uint32), \
+        C.POINTER(C.c_double)
+    proto = {
+        "pa_workspace_bytes": (C.c_uint64, [C.POINTER(PaConfig)]),
+        "pa_init": (C.c_int, [C.POINTER(PaConfig), C.POINTER(vp)]),
+        "pa_step": (C.c_int, [vp, C.c_double, C.c_int32]),
+        "pa_run": (C.c_int, [vp, f64p, C.c_int32, C.c_int32, i32p]),
+        "pa_population": (C.c_int, [vp, i64p]),
+        "pa_beta": (C.c_int, [vp, f64p, i64p]),
+        "pa_energies": (C.c_int, [vp, vp, vp, C.c_int64, C.c_int]),
+        "pa_log_Z": (C.c_int, [vp, f64p, f64p, f64p]),
+        "pa_observables": (C.c_int, [vp, C.POINTER(PaObs)]),
+        "pa_spins": (C.c_int, [vp, vp, C.c_int64, C.c_int64, C.c_int]),
+        "pa_tau": (C.c_int, [vp, vp, C.c_int64, C.c_int]),
+        "pa_counts": (C.c_int, [vp, vp, vp, C.c_int64, C.c_int]),
+        "pa_parents": (C.c_int, [vp, i64p]),
+        "pa_partitions": (C.c_int, [vp, vp, vp, i64p]),
+        "pa_thresholds": (C.c_int, [vp, u32p, u32p]),
+        "pa_set_spins": (C.c_int, [vp, vp, C.c_int64, C.c_int]),
+        "pa_profile_read": (C.c_int, [vp, f64p, i64p]),
+        "pa_launch_count": (C.c_int, [vp, i64p]),
+        "pa_last_error": (C.c_char_p, [vp]),
+        "pa_destroy": (C.c_int, [vp]),
+    }
+    for name, (res, args) in proto.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _np_ptr(a):
+    return C.c_void_p(a.ctypes.data)
+
+
+class PopulationAnnealer:
+    """One PA context on the current CUDA device.  Method names mirror the C ABI (pa_*)."""
+
+    def __init__(self, L, R0, P=1, seed=0, beta0=0.0, capacity=0, flags=0, device=None, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2006_00561_b200 needs a CUDA device (no CPU fallback)")
+        self._lib = load_library()
+        self._torch = torch
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = torch.cuda.current_stream(self.device) if stream is None else stream
+        self.L, self.N, self.P, self.R0, self.seed = int(L), int(L) * int(L), int(P), int(R0), int(seed)
+        self.wpr = self.N // 32
+        cfg = PaConfig(L=L, P=P, R0=R0, capacity=capacity, seed=seed, beta0=beta0, workspace=None, workspace_bytes=0,
+                       stream=self.stream.cuda_stream, flags=flags, reserved=0)
+        nbytes = self._lib.pa_workspace_bytes(C.byref(cfg))
+        if nbytes == 0:
+            raise PaError(PA_EINVAL, "invalid configuration")
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        aligned = (base + 255) // 256 * 256
+        cfg.workspace = aligned
+        cfg.workspace_bytes = nbytes
+        self.workspace_bytes = nbytes
+        self._ctx = C.c_void_p()
+        rc = self._lib.pa_init(C.byref(cfg), C.byref(self._ctx))
+        if rc != PA_OK:
+            msg = self._lib.pa_last_error(self._ctx).decode() if self._ctx else "pa_init failed"
+            if self._ctx:
+                self._lib.pa_destroy(self._ctx)
+                self._ctx = None
+            raise PaError(rc, msg)
+
+    # ---- helpers ---------------------------------------------------------------------------------
+    def _check(self, rc):
+        if rc != PA_OK:
+            raise PaError(rc, self._lib.pa_last_error(self._ctx).decode())
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self._lib.pa_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the path --------------------------------------------------------------------------------
+    def step(self, beta_next, theta):
+        self._check(self._lib.pa_step(self._ctx, float(beta_next), int(theta)))
+
+    def run(self, betas, theta):
+        b = np.ascontiguousarray(betas, np.float64)
+        done = C.c_int32(0)
+        rc = self._lib.pa_run(self._ctx, b.ctypes.data_as(C.POINTER(C.c_double)), b.shape[0], int(theta), C.byref(done))
+        self._check(rc)
+        return int(done.value)
+
+    @property
+    def R(self):
+        r = C.c_int64(0)
+        self._check(self._lib.pa_population(self._ctx, C.byref(r)))
+        return int(r.value)
+
+    def beta_steps(self):
+        b, s = C.c_double(0), C.c_int64(0)
+        self._check(self._lib.pa_beta(self._ctx, C.byref(b), C.byref(s)))
+        return float(b.value), int(s.value)
+
+    def energies(self, n=None):
+        n = self.R if n is None else int(n)
+        E, M = np.empty(n, np.int32), np.empty(n, np.int32)
+        self._check(self._lib.pa_energies(self._ctx, _np_ptr(E), _np_ptr(M), n, 0))
+        return E, M
+
+    def energies_device(self, n=None):
+        torch = self._torch
+        n = self.R if n is None else int(n)
+        E = torch.empty(n, dtype=torch.int32, device=self.device)
+        M = torch.empty(n, dtype=torch.int32, device=self.device)
+        self._check(self._lib.pa_energies(self._ctx, C.c_void_p(E.data_ptr()), C.c_void_p(M.data_ptr()), n, 1))
+        return E, M
+
+    def log_Z(self):
+        a, b, q = C.c_double(0), C.c_double(0), C.c_double(0)
+        self._check(self._lib.pa_log_Z(self._ctx, C.byref(a), C.byref(b), C.byref(q)))
+        return {"lnZ": float(a.value), "sum_lnQ": float(b.value), "last_Q": float(q.value)}
+
+    def observables(self):
+        o = PaObs()
+        self._check(self._lib.pa_observables(self._ctx, C.byref(o)))
+        big = lambda p: int(p[0]) | (int(p[1]) << 64)
+        return {"R": int(o.R), "sum_E": int(o.sum_E), "sum_E2": big(o.sum_E2), "sum_absM": big(o.sum_absM),
+                "sum_M2": big(o.sum_M2), "sum_M4": big(o.sum_M4), "mean_E": o.mean_E, "mean_E2": o.mean_E2,
+                "mean_absM": o.mean_absM, "mean_M2": o.mean_M2, "mean_M4": o.mean_M4}
+
+    def spins(self, first=0, count=None):
+        count = self.R - first if count is None else int(count)
+        out = np.empty((count, self.wpr), np.uint32)
+        self._check(self._lib.pa_spins(self._ctx, _np_ptr(out), int(first), count, 0))
+        return out
+
+    def tau(self, n=None):
+        n = self.parents() if n is None else int(n)
+        out = np.empty(n, np.float64)
+        self._check(self._lib.pa_tau(self._ctx, _np_ptr(out), n, 0))
+        return out
+
+    def counts(self, want_n=True):
+        npar = self.parents()
+        off = np.empty(npar + 1, np.uint32)
+        n = np.empty(npar, np.uint32) if want_n else None
+        self._check(self._lib.pa_counts(self._ctx, _np_ptr(n) if want_n else None, _np_ptr(off), npar, 0))
+        return n, off
+
+    def parents(self):
+        r = C.c_int64(0)
+        self._check(self._lib.pa_parents(self._ctx, C.byref(r)))
+        return int(r.value)
+
+    def partitions(self):
+        ps = np.empty(self.P + 1, np.uint32)
+        st = np.empty((self.P, 4), np.uint32)
+        moved = C.c_int64(0)
+        self._check(self._lib.pa_partitions(self._ctx, _np_ptr(ps), _np_ptr(st), C.byref(moved)))
+        return ps, st, int(moved.value)
+
+    def thresholds(self):
+        a, b = C.c_uint32(0), C.c_uint32(0)
+        self._check(self._lib.pa_thresholds(self._ctx, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
+
+    def set_spins(self, packed):
+        if hasattr(packed, "data_ptr"):  # torch tensor on the device
+            R = int(packed.shape[0])
+            self._check(self._lib.pa_set_spins(self._ctx, C.c_void_p(packed.data_ptr()), R, 1))
+        else:
+            a = np.ascontiguousarray(packed, np.uint32)
+            self._check(self._lib.pa_set_spins(self._ctx, _np_ptr(a), a.shape[0], 0))
+
+    def profile_read(self):
+        ms = (C.c_double * len(KERNELS))()
+        cnt = (C.c_int64 * len(KERNELS))()
+        self._check(self._lib.pa_profile_read(self._ctx, ms, cnt))
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(KERNELS)}
+
+    def launch_count(self):
+        r = C.c_int64(0)
+        self._check(self._lib.pa_launch_count(self._ctx, C.byref(r)))
+        return int(r.value)

@@ -1,0 +1,595 @@
+// pa_b200.cu -- C ABI of the population-annealing hot path (include/pa_b200.h) and its host-side step driver.
+// Host logic only sequences kernels; every step a0-a8 of the path runs on the device.
+#include "../../include/pa_b200.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "pa_common.cuh"
+#include "pa_observe.cuh"
+#include "pa_resample.cuh"
+#include "pa_sweep.cuh"
+
+using namespace pa;
+
+namespace {
+
+constexpr int RUN_CHUNK = 1024;  // step-parameter slots uploaded per pa_run chunk
+constexpr int RED_GRID = 148 * 4;
+constexpr int OBS_GRID = 148 * 2;
+
+struct Layout {
+  uint64_t state, params, spins[2], E[2], M[2], off, n, tau, tile_desc, tile_parent, red_partial, obs_partial,
+      lev_w, lev_tau, lev_mu, lev_m, lev_cdf, part[2], part_stats, total;
+};
+
+inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
+
+int copy_tile_for(int L) {
+  switch (L) {
+    case 8: return CopyGeo<8>::CT;
+    case 16: return CopyGeo<16>::CT;
+    case 32: return CopyGeo<32>::CT;
+    case 64: return CopyGeo<64>::CT;
+    default: return CopyGeo<128>::CT;
+  }
+}
+
+bool valid_L(int L) { return L == 8 || L == 16 || L == 32 || L == 64 || L == 128; }
+
+int64_t default_capacity(int64_t R0) {
+  int64_t s = (int64_t)std::ceil(std::sqrt((double)R0));
+  while (s * s < R0) ++s;
+  while (s > 0 && (s - 1) * (s - 1) >= R0) --s;
+  int64_t slack = 16 * s;
+  if (slack < 1024) slack = 1024;
+  return (R0 + slack + 1023) / 1024 * 1024;
+}
+
+bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
+  if (!c || !valid_L(c->L) || c->P < 1 || c->R0 < 1 || c->R0 >= (1ll << 31) || cap < c->R0 || cap >= (1ll << 32) - 4096)
+    return false;
+  const uint64_t N = (uint64_t)c->L * c->L, S = N / 8, nlev = N + 1, ucap = (uint64_t)cap;
+  uint64_t o = 0;
+  auto take = [&](uint64_t bytes) {
+    const uint64_t at = o;
+    o = align_up(o + bytes, 256);
+    return at;
+  };
+  lo->state = take(sizeof(DevState));
+  lo->params = take(sizeof(StepParams) * RUN_CHUNK);
+  for (int b = 0; b < 2; ++b) lo->spins[b] = take(ucap * S);
+  for (int b = 0; b < 2; ++b) lo->E[b] = take(ucap * 4);
+  for (int b = 0; b < 2; ++b) lo->M[b] = take(ucap * 4);
+  lo->off = take((ucap + 1) * 4);
+  lo->n = (c->flags & PA_KEEP_COUNTS) ? take(ucap * 4) : 0;
+  lo->tau = (c->flags & PA_KEEP_TAU) ? take(ucap * 8) : 0;
+  lo->tile_desc = take(((ucap + SCAN_TILE - 1) / SCAN_TILE + 1) * 8);
+  lo->tile_parent = take((ucap / copy_tile_for(c->L) + 2) * 4);
+  lo->red_partial = take(RED_GRID * 8);
+  lo->obs_partial = take((uint64_t)OBS_GRID * 10 * 8);
+  lo->lev_w = take(nlev * 8);
+  lo->lev_tau = take(nlev * 8);
+  lo->lev_mu = take(nlev * 8);
+  lo->lev_m = take(nlev * 4);
+  lo->lev_cdf = take(nlev * PO_ROW * 8);
+  for (int b = 0; b < 2; ++b) lo->part[b] = take(((uint64_t)c->P + 1) * 4);
+  lo->part_stats = take((uint64_t)c->P * 16);
+  lo->total = o;
+  return true;
+}
+
+struct EventPair {
+  cudaEvent_t a, b;
+  int kernel;
+};
+
+}  // namespace
+
+struct pa_ctx {
+  pa_config cfg;
+  int64_t cap;
+  int N, wrep, device;
+  Layout lo;
+  char* ws;
+  cudaStream_t stream;
+  PhiloxKey key;
+  DevState* h_state;  // pinned mirror
+  StepParams* h_params;  // pinned staging for uploads
+  // host mirrors of committed state
+  int64_t R, R_parents, steps;
+  double beta, sum_lnQ, last_Q;
+  int64_t launches;
+  bool profile;
+  std::vector<EventPair> ev_used, ev_free;
+  std::string err;
+
+  template <class T> T* dev(uint64_t off) const { return reinterpret_cast<T*>(ws + off); }
+};
+
+namespace {
+
+int fail(pa_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+int cuda_fail(pa_ctx* c, cudaError_t e, const char* what) {
+  return fail(c, PA_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                            \
+  do {                                                      \
+    cudaError_t e_ = (call);                                \
+    if (e_ != cudaSuccess) return cuda_fail(c, e_, #call);  \
+  } while (0)
+
+struct Prof {  // records an event pair around one launch when profiling is on
+  pa_ctx* c;
+  EventPair ep;
+  bool on;
+  Prof(pa_ctx* c_, int kernel) : c(c_), on(c_->profile) {
+    c->launches += 1;
+    if (!on) return;
+    if (!c->ev_free.empty()) {
+      ep = c->ev_free.back();
+      c->ev_free.pop_back();
+    } else {
+      cudaEventCreate(&ep.a);
+      cudaEventCreate(&ep.b);
+    }
+    ep.kernel = kernel;
+    cudaEventRecord(ep.a, c->stream);
+  }
+  ~Prof() {
+    if (!on) return;
+    cudaEventRecord(ep.b, c->stream);
+    c->ev_used.push_back(ep);
+  }
+};
+
+LevelTables tables(pa_ctx* c) {
+  LevelTables t;
+  t.w = c->dev<double>(c->lo.lev_w);
+  t.tau = c->dev<double>(c->lo.lev_tau);
+  t.mu = c->dev<double>(c->lo.lev_mu);
+  t.m = c->dev<uint32_t>(c->lo.lev_m);
+  t.cdf = c->dev<double>(c->lo.lev_cdf);
+  return t;
+}
+
+template <int L>
+void launch_sweep_L(pa_ctx* c, const StepParams* sp, int mode) {
+  const uint64_t threads = (uint64_t)c->cap * Geo<L>::G;
+  const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
+  k_sweep<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), sp, c->dev<uint32_t>(c->lo.spins[0]),
+                                                    c->dev<uint32_t>(c->lo.spins[1]), c->dev<int32_t>(c->lo.E[0]),
+                                                    c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]),
+                                                    c->dev<int32_t>(c->lo.M[1]), c->key, mode);
+}
+void launch_sweep(pa_ctx* c, const StepParams* sp, int mode) {
+  Prof p(c, PA_K_SWEEP);
+  switch (c->cfg.L) {
+    case 8: launch_sweep_L<8>(c, sp, mode); break;
+    case 16: launch_sweep_L<16>(c, sp, mode); break;
+    case 32: launch_sweep_L<32>(c, sp, mode); break;
+    case 64: launch_sweep_L<64>(c, sp, mode); break;
+    default: launch_sweep_L<128>(c, sp, mode); break;
+  }
+}
+
+template <int L>
+void launch_copy_L(pa_ctx* c) {
+  const unsigned grid = (unsigned)((c->cap + CopyGeo<L>::CT - 1) / CopyGeo<L>::CT);
+  uint32_t *s0 = c->dev<uint32_t>(c->lo.spins[0]), *s1 = c->dev<uint32_t>(c->lo.spins[1]);
+  int32_t *e0 = c->dev<int32_t>(c->lo.E[0]), *e1 = c->dev<int32_t>(c->lo.E[1]);
+  int32_t *m0 = c->dev<int32_t>(c->lo.M[0]), *m1 = c->dev<int32_t>(c->lo.M[1]);
+  k_copy<L><<<grid, COPY_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), c->dev<uint32_t>(c->lo.off),
+                                                  c->dev<uint32_t>(c->lo.tile_parent), s0, s1, e0, e1, m0, m1);
+}
+void launch_copy(pa_ctx* c) {
+  Prof p(c, PA_K_COPY);
+  switch (c->cfg.L) {
+    case 8: launch_copy_L<8>(c); break;
+    case 16: launch_copy_L<16>(c); break;
+    case 32: launch_copy_L<32>(c); break;
+    case 64: launch_copy_L<64>(c); break;
+    default: launch_copy_L<128>(c); break;
+  }
+}
+
+void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
+  Prof p(c, PA_K_OBSERVE);
+  k_observe<<<OBS_GRID, OBS_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.E[0]),
+                                                     c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]),
+                                                     c->dev<int32_t>(c->lo.M[1]),
+                                                     c->dev<unsigned long long>(c->lo.obs_partial), mode);
+}
+
+// all kernels of one temperature step, parameters in device slot sp
+void enqueue_step(pa_ctx* c, const StepParams* sp, int theta) {
+  DevState* st = c->dev<DevState>(c->lo.state);
+  const LevelTables tb = tables(c);
+  const int N = c->N;
+  const int n_desc = (int)((c->cap + SCAN_TILE - 1) / SCAN_TILE + 1);
+  const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
+  {
+    Prof p(c, PA_K_LEVELS_W);
+    const int threads = 256, work = (N + 1 > n_desc ? N + 1 : n_desc);
+    k_levels_w<<<(work + threads - 1) / threads, threads, 0, c->stream>>>(
+        st, sp, tb, N, c->dev<unsigned long long>(c->lo.tile_desc), n_desc);
+  }
+  {
+    Prof p(c, PA_K_Q_REDUCE);
+    k_q_reduce<<<RED_GRID, RED_THREADS, 0, c->stream>>>(st, E0, E1, tb, N, c->dev<double>(c->lo.red_partial),
+                                                        (double)c->cfg.R0);
+  }
+  {
+    Prof p(c, PA_K_LEVELS_TAU);
+    k_levels_tau<<<(N + 1 + 127) / 128, 128, 0, c->stream>>>(st, tb, N);
+  }
+  {
+    Prof p(c, PA_K_POISSON_SCAN);
+    const unsigned grid = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
+    k_poisson_scan<<<grid, SCAN_THREADS, 0, c->stream>>>(
+        st, E0, E1, tb, N, c->dev<uint32_t>(c->lo.off), c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr,
+        c->lo.tau ? c->dev<double>(c->lo.tau) : nullptr, c->dev<unsigned long long>(c->lo.tile_desc),
+        c->dev<uint32_t>(c->lo.tile_parent), copy_tile_for(c->cfg.L), (unsigned long long)c->cap, c->key);
+  }
+  {
+    Prof p(c, PA_K_BALANCE);
+    k_balance<<<1, 256, 0, c->stream>>>(st, c->dev<uint32_t>(c->lo.off), c->dev<uint32_t>(c->lo.part[0]),
+                                        c->dev<uint32_t>(c->lo.part[1]), c->dev<uint32_t>(c->lo.part_stats), c->cfg.P);
+  }
+  launch_copy(c);
+  if (theta > 0) launch_sweep(c, sp, 0);
+  launch_observe(c, sp, 0);
+}
+
+__global__ void k_init_state(DevState* st, unsigned long long R, double beta0, uint32_t* part0, int P) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    memset(st, 0, sizeof(DevState));
+    st->R = R;
+    st->R_parents = R;
+    st->beta = beta0;
+    st->Q = 1.0;
+  }
+  const unsigned long long base = R / P, rem = R % P;
+  for (int p = threadIdx.x; p <= P; p += blockDim.x)
+    part0[p] = (uint32_t)((unsigned long long)p * base + ((unsigned long long)p < rem ? p : rem));
+}
+// test hook support: set R and rebuild the partition table of the current buffer
+__global__ void k_set_population(DevState* st, unsigned long long R, uint32_t* part0, uint32_t* part1, int P) {
+  if (threadIdx.x == 0) {
+    st->R = R;
+    st->obs_done = 0u;
+  }
+  uint32_t* part = st->cur ? part1 : part0;
+  const unsigned long long base = R / P, rem = R % P;
+  for (int p = threadIdx.x; p <= P; p += blockDim.x)
+    part[p] = (uint32_t)((unsigned long long)p * base + ((unsigned long long)p < rem ? p : rem));
+}
+__global__ void k_clear_status(DevState* st) {
+  st->status = 0u;
+  st->obs_done = 0u;
+}
+
+// read the device state back (synchronises) and refresh the host mirrors
+int sync_state(pa_ctx* c) {
+  CK(cudaMemcpyAsync(c->h_state, c->dev<DevState>(c->lo.state), sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  CK(cudaGetLastError());
+  const DevState& s = *c->h_state;
+  c->R = (int64_t)s.R;
+  c->R_parents = (int64_t)s.R_parents;
+  c->steps = s.step;
+  c->beta = s.beta;
+  c->sum_lnQ = s.sum_lnQ;
+  if (s.step > 0) c->last_Q = s.Q;
+  return PA_OK;
+}
+
+int status_to_code(pa_ctx* c) {
+  const DevState& s = *c->h_state;
+  if (s.status == ST_OK) return PA_OK;
+  char buf[160];
+  if (s.status == ST_CAPACITY) {
+    snprintf(buf, sizeof buf, "step %u: resampled population R'=%llu exceeds capacity %lld (not committed)", s.fail_step,
+             (unsigned long long)s.Rnew, (long long)c->cap);
+    c->err = buf;
+    return PA_ECAPACITY;
+  }
+  snprintf(buf, sizeof buf, "step %u: population extinct (R'=0, not committed)", s.fail_step);
+  c->err = buf;
+  return PA_EEXTINCT;
+}
+
+int copy_out(pa_ctx* c, void* dst, const void* src_dev, size_t bytes, int dst_on_device) {
+  if (bytes == 0) return PA_OK;
+  CK(cudaMemcpyAsync(dst, src_dev, bytes, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return PA_OK;
+}
+
+int check_step_args(pa_ctx* c, double beta_from, double beta_next, int theta) {
+  if (!(beta_next == beta_next) || std::isinf(beta_next)) return fail(c, PA_EINVAL, "beta_next is not finite");
+  if (theta < 0) return fail(c, PA_EINVAL, "theta < 0");
+  if (theta > 0 && beta_next < 0.0) return fail(c, PA_EINVAL, "beta_next < 0 with theta > 0 (reading G10)");
+  const double dbeta = beta_next - beta_from;
+  if (!(std::fabs(dbeta) * 2.0 * c->N < 700.0)) return fail(c, PA_EINVAL, "|dbeta|*2N >= 700 (reading G11)");
+  return PA_OK;
+}
+
+StepParams make_params(double beta_from, double beta_next, int theta) {
+  StepParams p;
+  p.dbeta = beta_next - beta_from;
+  p.beta_next = beta_next;
+  const double a4 = std::floor(4294967296.0 * std::exp(-4.0 * beta_next));
+  const double a8 = std::floor(4294967296.0 * std::exp(-8.0 * beta_next));
+  p.T4 = a4 >= 4294967295.0 ? 0xffffffffu : (a4 > 0.0 ? (uint32_t)a4 : 0u);
+  p.T8 = a8 >= 4294967295.0 ? 0xffffffffu : (a8 > 0.0 ? (uint32_t)a8 : 0u);
+  p.theta = theta;
+  p.pad_ = 0;
+  return p;
+}
+
+}  // namespace
+
+extern "C" {
+
+uint64_t pa_workspace_bytes(const pa_config* cfg) {
+  if (!cfg) return 0;
+  const int64_t cap = cfg->capacity > 0 ? cfg->capacity : (cfg->R0 >= 1 ? default_capacity(cfg->R0) : 0);
+  Layout lo;
+  if (!make_layout(cfg, cap, &lo)) return 0;
+  return lo.total;
+}
+
+int pa_init(const pa_config* cfg, pa_ctx** out) {
+  if (!cfg || !out) return PA_EINVAL;
+  *out = nullptr;
+  pa_ctx* c = new (std::nothrow) pa_ctx();
+  if (!c) return PA_ENOMEM;
+  c->cfg = *cfg;
+  c->cap = cfg->capacity > 0 ? cfg->capacity : (cfg->R0 >= 1 ? default_capacity(cfg->R0) : 0);
+  if (!make_layout(cfg, c->cap, &c->lo) || !(cfg->beta0 == cfg->beta0)) {
+    delete c;
+    return PA_EINVAL;
+  }
+  if (!cfg->workspace || cfg->workspace_bytes < c->lo.total || ((uintptr_t)cfg->workspace & 255u)) {
+    delete c;
+    return cfg->workspace && !((uintptr_t)cfg->workspace & 255u) ? PA_ENOMEM : PA_EINVAL;
+  }
+  c->N = cfg->L * cfg->L;
+  c->wrep = c->N / 32;
+  c->ws = static_cast<char*>(cfg->workspace);
+  c->stream = static_cast<cudaStream_t>(cfg->stream);
+  c->profile = (cfg->flags & PA_PROFILE) != 0;
+  c->launches = 0;
+  uint32_t k0 = (uint32_t)(cfg->seed & 0xffffffffull), k1 = (uint32_t)(cfg->seed >> 32);
+  for (int r = 0; r < 10; ++r) {
+    c->key.k0[r] = k0;
+    c->key.k1[r] = k1;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    delete c;
+    return PA_ECUDA;  // no CPU fallback
+  }
+  cudaGetDevice(&c->device);
+  if (cudaHostAlloc((void**)&c->h_state, sizeof(DevState), cudaHostAllocDefault) != cudaSuccess ||
+      cudaHostAlloc((void**)&c->h_params, sizeof(StepParams) * RUN_CHUNK, cudaHostAllocDefault) != cudaSuccess) {
+    delete c;
+    return PA_ECUDA;
+  }
+  *out = c;  // from here on errors keep the ctx so that pa_last_error works; caller destroys it
+  DevState* st = c->dev<DevState>(c->lo.state);
+  k_init_state<<<1, 256, 0, c->stream>>>(st, (unsigned long long)cfg->R0, cfg->beta0, c->dev<uint32_t>(c->lo.part[0]),
+                                         cfg->P);
+  c->launches += 1;
+  CK(cudaMemsetAsync(c->dev<char>(c->lo.part_stats), 0, (size_t)cfg->P * 16, c->stream));
+  {
+    const int bpr = (c->wrep + 3) / 4;
+    const uint64_t threads = (uint64_t)cfg->R0 * bpr;
+    k_init<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(st, c->dev<uint32_t>(c->lo.spins[0]),
+                                                                      c->dev<uint32_t>(c->lo.spins[1]), c->wrep, c->key);
+    c->launches += 1;
+  }
+  launch_sweep(c, nullptr, 1);   // E_j, M_j
+  launch_observe(c, nullptr, 1);  // population sums
+  c->last_Q = 1.0;
+  int rc = sync_state(c);
+  if (rc != PA_OK) return rc;
+  return PA_OK;
+}
+
+int pa_run(pa_ctx* c, const double* betas, int32_t K, int32_t theta, int32_t* steps_done) {
+  if (!c) return PA_EINVAL;
+  if (steps_done) *steps_done = 0;
+  if (K < 0 || (K > 0 && !betas)) return fail(c, PA_EINVAL, "bad betas/K");
+  double from = c->beta;
+  for (int k = 0; k < K; ++k) {
+    const int rc = check_step_args(c, from, betas[k], theta);
+    if (rc != PA_OK) return rc;
+    from = betas[k];
+  }
+  if ((uint64_t)c->steps + (uint64_t)K >= (1ull << 28)) return fail(c, PA_EINVAL, "step counter would exceed 2^28");
+  const int64_t steps_before = c->steps;
+  StepParams* d_params = c->dev<StepParams>(c->lo.params);
+  from = c->beta;
+  for (int base = 0; base < K; base += RUN_CHUNK) {
+    const int nk = (K - base < RUN_CHUNK) ? (K - base) : RUN_CHUNK;
+    if (base > 0) CK(cudaStreamSynchronize(c->stream));  // staging buffer is reused
+    for (int k = 0; k < nk; ++k) {
+      c->h_params[k] = make_params(from, betas[base + k], theta);
+      from = betas[base + k];
+    }
+    CK(cudaMemcpyAsync(d_params, c->h_params, sizeof(StepParams) * nk, cudaMemcpyHostToDevice, c->stream));
+    for (int k = 0; k < nk; ++k) enqueue_step(c, d_params + k, theta);
+  }
+  int rc = sync_state(c);
+  if (rc != PA_OK) return rc;
+  if (steps_done) *steps_done = (int32_t)(c->steps - steps_before);
+  rc = status_to_code(c);
+  if (rc != PA_OK) {
+    k_clear_status<<<1, 1, 0, c->stream>>>(c->dev<DevState>(c->lo.state));
+    c->launches += 1;
+    CK(cudaStreamSynchronize(c->stream));
+  }
+  return rc;
+}
+
+int pa_step(pa_ctx* c, double beta_next, int32_t theta) { return pa_run(c, &beta_next, 1, theta, nullptr); }
+
+int pa_population(pa_ctx* c, int64_t* R) {
+  if (!c || !R) return PA_EINVAL;
+  *R = c->R;
+  return PA_OK;
+}
+
+int pa_beta(pa_ctx* c, double* beta, int64_t* steps) {
+  if (!c) return PA_EINVAL;
+  if (beta) *beta = c->beta;
+  if (steps) *steps = c->steps;
+  return PA_OK;
+}
+
+int pa_energies(pa_ctx* c, int32_t* E, int32_t* M, int64_t n, int dst_on_device) {
+  if (!c || n < 0 || n > c->R || (!E && !M)) return fail(c, PA_EINVAL, "pa_energies: bad arguments");
+  const unsigned cur = c->h_state->cur;
+  int rc = PA_OK;
+  if (E) rc = copy_out(c, E, c->dev<int32_t>(c->lo.E[cur]), (size_t)n * 4, dst_on_device);
+  if (rc == PA_OK && M) rc = copy_out(c, M, c->dev<int32_t>(c->lo.M[cur]), (size_t)n * 4, dst_on_device);
+  return rc;
+}
+
+int pa_log_Z(pa_ctx* c, double* lnZ, double* sum_lnQ, double* last_Q) {
+  if (!c) return PA_EINVAL;
+  if (lnZ) *lnZ = (double)c->N * std::log(2.0) + c->sum_lnQ;
+  if (sum_lnQ) *sum_lnQ = c->sum_lnQ;
+  if (last_Q) *last_Q = c->last_Q;
+  return PA_OK;
+}
+
+int pa_observables(pa_ctx* c, pa_obs* o) {
+  if (!c || !o) return PA_EINVAL;
+  const DevState& s = *c->h_state;
+  o->R = (int64_t)s.obs_R;
+  o->sum_E = (int64_t)s.obs[0];
+  for (int i = 0; i < 2; ++i) {
+    o->sum_E2[i] = s.obs[2 + i];
+    o->sum_absM[i] = s.obs[4 + i];
+    o->sum_M2[i] = s.obs[6 + i];
+    o->sum_M4[i] = s.obs[8 + i];
+  }
+  const double R = (double)s.obs_R;
+  auto f = [](const unsigned long long* p) { return (double)p[0] + 18446744073709551616.0 * (double)p[1]; };
+  o->mean_E = (double)o->sum_E / R;
+  o->mean_E2 = f(&s.obs[2]) / R;
+  o->mean_absM = f(&s.obs[4]) / R;
+  o->mean_M2 = f(&s.obs[6]) / R;
+  o->mean_M4 = f(&s.obs[8]) / R;
+  return PA_OK;
+}
+
+int pa_spins(pa_ctx* c, uint32_t* dst, int64_t first, int64_t count, int dst_on_device) {
+  if (!c || !dst || first < 0 || count < 0 || first + count > c->R) return fail(c, PA_EINVAL, "pa_spins: bad range");
+  const unsigned cur = c->h_state->cur;
+  return copy_out(c, dst, c->dev<uint32_t>(c->lo.spins[cur]) + (size_t)first * c->wrep, (size_t)count * c->wrep * 4,
+                  dst_on_device);
+}
+
+int pa_tau(pa_ctx* c, double* dst, int64_t n, int dst_on_device) {
+  if (!c || !dst || n < 0) return fail(c, PA_EINVAL, "pa_tau: bad arguments");
+  if (!c->lo.tau) return fail(c, PA_EINVAL, "pa_tau needs PA_KEEP_TAU");
+  if (c->steps == 0 || n > c->R_parents) return fail(c, PA_EINVAL, "pa_tau: no step yet or n > parents");
+  return copy_out(c, dst, c->dev<double>(c->lo.tau), (size_t)n * 8, dst_on_device);
+}
+
+int pa_counts(pa_ctx* c, uint32_t* n, uint32_t* off, int64_t n_parents, int dst_on_device) {
+  if (!c || n_parents < 0 || (!n && !off)) return fail(c, PA_EINVAL, "pa_counts: bad arguments");
+  if (c->steps == 0 || n_parents > c->R_parents) return fail(c, PA_EINVAL, "pa_counts: no step yet or n_parents > parents");
+  if (n && !c->lo.n) return fail(c, PA_EINVAL, "pa_counts(n) needs PA_KEEP_COUNTS");
+  int rc = PA_OK;
+  if (n) rc = copy_out(c, n, c->dev<uint32_t>(c->lo.n), (size_t)n_parents * 4, dst_on_device);
+  if (rc == PA_OK && off) rc = copy_out(c, off, c->dev<uint32_t>(c->lo.off), (size_t)(n_parents + 1) * 4, dst_on_device);
+  return rc;
+}
+
+int pa_parents(pa_ctx* c, int64_t* n_parents) {
+  if (!c || !n_parents) return PA_EINVAL;
+  *n_parents = c->R_parents;
+  return PA_OK;
+}
+
+int pa_partitions(pa_ctx* c, uint32_t* part_start, pa_part_stats* stats, int64_t* moved) {
+  if (!c || !part_start) return fail(c, PA_EINVAL, "pa_partitions: bad arguments");
+  const unsigned cur = c->h_state->cur;
+  int rc = copy_out(c, part_start, c->dev<uint32_t>(c->lo.part[cur]), ((size_t)c->cfg.P + 1) * 4, 0);
+  if (rc == PA_OK && stats) rc = copy_out(c, stats, c->dev<uint32_t>(c->lo.part_stats), (size_t)c->cfg.P * 16, 0);
+  if (moved) *moved = (int64_t)c->h_state->moved;
+  return rc;
+}
+
+int pa_thresholds(pa_ctx* c, uint32_t* T4, uint32_t* T8) {
+  if (!c) return PA_EINVAL;
+  if (T4) *T4 = c->h_state->T4;
+  if (T8) *T8 = c->h_state->T8;
+  return PA_OK;
+}
+
+int pa_set_spins(pa_ctx* c, const uint32_t* src, int64_t R, int src_on_device) {
+  if (!c || !src || R < 1 || R > c->cap) return fail(c, PA_EINVAL, "pa_set_spins: bad arguments");
+  const unsigned cur = c->h_state->cur;
+  CK(cudaMemcpyAsync(c->dev<uint32_t>(c->lo.spins[cur]), src, (size_t)R * c->wrep * 4,
+                     src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+  k_set_population<<<1, 256, 0, c->stream>>>(c->dev<DevState>(c->lo.state), (unsigned long long)R,
+                                             c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]), c->cfg.P);
+  c->launches += 1;
+  launch_sweep(c, nullptr, 1);
+  launch_observe(c, nullptr, 1);
+  return sync_state(c);
+}
+
+int pa_profile_read(pa_ctx* c, double* ms, int64_t* launches) {
+  if (!c || !ms || !launches) return PA_EINVAL;
+  for (int k = 0; k < PA_K_COUNT; ++k) {
+    ms[k] = 0.0;
+    launches[k] = 0;
+  }
+  CK(cudaStreamSynchronize(c->stream));
+  for (EventPair& ep : c->ev_used) {
+    float t = 0.f;
+    CK(cudaEventElapsedTime(&t, ep.a, ep.b));
+    ms[ep.kernel] += t;
+    launches[ep.kernel] += 1;
+    c->ev_free.push_back(ep);
+  }
+  c->ev_used.clear();
+  return PA_OK;
+}
+
+int pa_launch_count(pa_ctx* c, int64_t* launches) {
+  if (!c || !launches) return PA_EINVAL;
+  *launches = c->launches;
+  return PA_OK;
+}
+
+const char* pa_last_error(pa_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int pa_destroy(pa_ctx* c) {
+  if (!c) return PA_EINVAL;
+  cudaStreamSynchronize(c->stream);
+  for (EventPair& ep : c->ev_used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+  for (EventPair& ep : c->ev_free) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+  if (c->h_state) cudaFreeHost(c->h_state);
+  if (c->h_params) cudaFreeHost(c->h_params);
+  delete c;
+  return PA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,80 @@
+// pa_common.cuh -- device-side state, step parameters and the Philox4x32-10 generator.
+// Part of the CUDA product path; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pa {
+
+// ---------------------------------------------------------------------------------------------------
+// Device-resident state of one context.  Every kernel of a step reads it; only single-thread epilogues
+// write it.  A step is COMMITTED by k_observe's last block (cur ^= 1, R = Rnew, ...); when status != 0
+// every later kernel returns at once, so a failed step leaves the population untouched.
+// ---------------------------------------------------------------------------------------------------
+struct DevState {
+  unsigned long long R;          // current population R_beta_i
+  unsigned long long Rnew;       // population after resampling (valid inside a step)
+  unsigned long long R_parents;  // population the last committed step started from
+  double sumw;                   // sum_j exp(-dbeta E_j)
+  double Q;                      // eq. 3
+  double lnQ;
+  double sum_lnQ;                // eq. 5 accumulator
+  double scale;                  // R0 / R  (reading G2)
+  double beta;                   // inverse temperature of the current population
+  unsigned long long moved;      // children whose partition differs from the parent's (last step)
+  unsigned long long obs[10];    // {lo,hi} x (sum E, sum E^2, sum |M|, sum M^2, sum M^4)
+  unsigned long long obs_R;
+  unsigned int step;             // committed steps
+  unsigned int cur;              // index of the buffer holding the current population
+  unsigned int status;           // 0 = ok, else -pa_status of the failing step
+  unsigned int fail_step;        // ordinal of the step that failed
+  unsigned int reduce_done;      // block counters (reset every step by k_levels_w)
+  unsigned int scan_tile;
+  unsigned int obs_done;
+  unsigned int T4, T8;           // thresholds of the last committed step with theta > 0
+  unsigned int pad_;
+};
+
+struct StepParams {
+  double dbeta;      // beta_next - beta (host fp64 subtraction, C5)
+  double beta_next;
+  unsigned int T4, T8;  // C4 thresholds at beta_next (host libm)
+  int theta;
+  int pad_;
+};
+
+// status codes stored in DevState::status (positive; the host negates them into pa_status)
+enum { ST_OK = 0, ST_CAPACITY = 3, ST_EXTINCT = 4 };
+
+// ---------------------------------------------------------------------------------------------------
+// Philox4x32-10.  The key schedule depends only on the seed, so the ten round keys are computed once
+// on the host and passed by value (they end up in the constant bank and feed LOP3 directly).
+// ---------------------------------------------------------------------------------------------------
+struct PhiloxKey {
+  uint32_t k0[10];
+  uint32_t k1[10];
+};
+
+constexpr uint32_t PHILOX_M0 = 0xD2511F53u;
+constexpr uint32_t PHILOX_M1 = 0xCD9E8D57u;
+constexpr uint32_t TAG_INIT = 0u, TAG_RESAMPLE = 1u, TAG_SWEEP = 2u;
+
+__device__ __forceinline__ void philox_round(uint32_t& c0, uint32_t& c1, uint32_t& c2, uint32_t& c3, uint32_t k0,
+                                             uint32_t k1) {
+  const uint32_t hi0 = __umulhi(PHILOX_M0, c0), lo0 = PHILOX_M0 * c0;
+  const uint32_t hi1 = __umulhi(PHILOX_M1, c2), lo1 = PHILOX_M1 * c2;
+  const uint32_t n0 = hi1 ^ c1 ^ k0;
+  const uint32_t n2 = hi0 ^ c3 ^ k1;
+  c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+}
+
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const PhiloxKey& key) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) philox_round(c0, c1, c2, c3, key.k0[r], key.k1[r]);
+  return make_uint4(c0, c1, c2, c3);
+}
+
+__device__ __forceinline__ uint32_t ctr3(uint32_t tag, uint32_t step) { return (tag << 28) | step; }
+
+}  // namespace pa

@@ -1,0 +1,122 @@
+// pa_observe.cuh -- a0 initial population and a8 population sums + commit of the step.
+#pragma once
+#include "pa_common.cuh"
+
+namespace pa {
+
+// a0: uint32 word v of replica j <- w[v&3] of Philox counter (v>>2, j, 0, tag0|0)   (C3 init)
+// One thread per Philox block = up to 4 consecutive words.
+__global__ void k_init(const DevState* __restrict__ st, uint32_t* __restrict__ spins0, uint32_t* __restrict__ spins1,
+                       int wrep, const PhiloxKey key) {
+  const unsigned long long R = st->R;
+  uint32_t* __restrict__ spins = st->cur ? spins1 : spins0;
+  const int blocks_per_rep = (wrep + 3) / 4;
+  const unsigned long long idx = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long j = idx / blocks_per_rep;
+  const unsigned b = (unsigned)(idx % blocks_per_rep);
+  if (j >= R) return;
+  const uint4 w = philox4x32_10(b, (uint32_t)j, 0u, ctr3(TAG_INIT, 0u), key);
+  uint32_t* dst = spins + j * wrep + 4 * b;
+  if (wrep - 4 * (int)b >= 4) {
+    *reinterpret_cast<uint4*>(dst) = w;
+  } else {
+    const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+    for (int i = 0; i < wrep - 4 * (int)b; ++i) dst[i] = ww[i];
+  }
+}
+
+// 128-bit unsigned add helper on {lo, hi}
+struct U128 {
+  unsigned long long lo, hi;
+};
+__device__ __forceinline__ void u128_add(U128& a, unsigned long long lo, unsigned long long hi) {
+  const unsigned long long s = a.lo + lo;
+  a.hi += hi + (s < a.lo ? 1ull : 0ull);
+  a.lo = s;
+}
+__device__ __forceinline__ U128 warp_sum_u128(U128 v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long lo = __shfl_xor_sync(0xffffffffu, v.lo, o);
+    const unsigned long long hi = __shfl_xor_sync(0xffffffffu, v.hi, o);
+    u128_add(v, lo, hi);
+  }
+  return v;
+}
+
+constexpr int OBS_THREADS = 256;
+constexpr int OBS_Q = 5;  // sum E (two's complement), sum E^2, sum |M|, sum M^2, sum M^4
+
+// mode 0: end of a step -> sums over buffer cur^1 (Rnew replicas), then COMMIT the step.
+// mode 1: after init / set_spins -> sums over buffer cur (R replicas), no commit.
+__global__ void __launch_bounds__(OBS_THREADS)
+k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
+          const int32_t* __restrict__ E1, const int32_t* __restrict__ M0, const int32_t* __restrict__ M1,
+          unsigned long long* __restrict__ partial /* [grid][10] */, const int mode) {
+  if (st->status != ST_OK) return;
+  const unsigned buf = mode == 0 ? (st->cur ^ 1u) : st->cur;
+  const unsigned long long count = mode == 0 ? st->Rnew : st->R;
+  const int32_t* __restrict__ E = buf ? E1 : E0;
+  const int32_t* __restrict__ M = buf ? M1 : M0;
+  U128 acc[OBS_Q];
+#pragma unroll
+  for (int q = 0; q < OBS_Q; ++q) acc[q] = {0ull, 0ull};
+  const unsigned long long stride = (unsigned long long)gridDim.x * OBS_THREADS;
+  for (unsigned long long j = (unsigned long long)blockIdx.x * OBS_THREADS + threadIdx.x; j < count; j += stride) {
+    const long long e = E[j], m = M[j];
+    const unsigned long long am = (unsigned long long)(m < 0 ? -m : m);
+    u128_add(acc[0], (unsigned long long)e, e < 0 ? ~0ull : 0ull);  // sign-extended
+    u128_add(acc[1], (unsigned long long)(e * e), 0ull);
+    u128_add(acc[2], am, 0ull);
+    u128_add(acc[3], am * am, 0ull);
+    u128_add(acc[4], am * am * am * am, 0ull);  // |M| <= 2^14 -> < 2^56
+  }
+  __shared__ U128 s_part[OBS_THREADS / 32][OBS_Q];
+  __shared__ bool s_last;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int q = 0; q < OBS_Q; ++q) {
+    const U128 v = warp_sum_u128(acc[q]);
+    if (lane == 0) s_part[warp][q] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < OBS_Q) {
+    U128 t = {0ull, 0ull};
+    for (int w = 0; w < OBS_THREADS / 32; ++w) u128_add(t, s_part[w][threadIdx.x].lo, s_part[w][threadIdx.x].hi);
+    partial[(size_t)blockIdx.x * 10 + 2 * threadIdx.x] = t.lo;
+    partial[(size_t)blockIdx.x * 10 + 2 * threadIdx.x + 1] = t.hi;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    const unsigned done = atomicAdd(&st->obs_done, 1u);
+    s_last = (done == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (threadIdx.x < OBS_Q) {
+    U128 t = {0ull, 0ull};
+    for (unsigned b = 0; b < gridDim.x; ++b)
+      u128_add(t, __ldcg(&partial[(size_t)b * 10 + 2 * threadIdx.x]), __ldcg(&partial[(size_t)b * 10 + 2 * threadIdx.x + 1]));
+    st->obs[2 * threadIdx.x] = t.lo;
+    st->obs[2 * threadIdx.x + 1] = t.hi;
+  }
+  if (threadIdx.x == 0) {
+    st->obs_R = count;
+    if (mode == 0) {  // commit: the new population becomes the current one
+      st->R_parents = st->R;
+      st->R = st->Rnew;
+      st->cur ^= 1u;
+      st->step += 1u;
+      st->sum_lnQ += st->lnQ;
+      st->beta = sp->beta_next;
+      if (sp->theta > 0) {
+        st->T4 = sp->T4;
+        st->T8 = sp->T8;
+      }
+    }
+  }
+}
+
+}  // namespace pa

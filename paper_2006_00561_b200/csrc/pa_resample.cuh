@@ -1,0 +1,481 @@
+// pa_resample.cuh -- a1..a6: reweighting (eq. 3, 4), Poisson copy counts, single-pass exclusive scan,
+// partition balance and the replica gather-copy.  PAPER.md:44-56, :84, :94, :104-106; C5, A4, A5, A6.
+//
+// lambda_j depends on j only through the integer energy E_j = 4*lev - 2N, lev = 0..N, so everything that is
+// floating point is tabulated per energy LEVEL (N+1 levels) by two tiny kernels; the per-replica kernels only
+// look the tables up.  The arithmetic per level is exactly the sequence written in DESIGN.md.
+#pragma once
+#include "pa_common.cuh"
+
+namespace pa {
+
+constexpr int PO_KMAX = 64;            // A4: cap of the CDF inversion loop
+constexpr int PO_ROW = PO_KMAX + 1;    // F_0 .. F_64 per level
+constexpr unsigned M_OVERFLOW = 0xffffffffu;
+
+struct LevelTables {
+  double* w;        // [N+1]  exp(-dbeta * e)
+  double* tau;      // [N+1]  w / Q
+  double* mu;       // [N+1]  lambda / m
+  uint32_t* m;      // [N+1]  number of chunks (0: lambda <= 0; M_OVERFLOW: lambda >= 2^31)
+  double* cdf;      // [N+1][65]  F_k of Poisson(mu) built by the A4 recurrence
+};
+
+// ---------------------------------------------------------------------------------------------------
+// k_levels_w: w_e = exp(-dbeta * e) for every level; also resets the per-step counters and the scan's
+// tile descriptors (it is the first kernel of every step).
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_levels_w(DevState* st, const StepParams* sp, LevelTables tb, int N, unsigned long long* tile_desc,
+                           int n_desc) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx == 0) {
+    st->reduce_done = 0u;
+    st->scan_tile = 0u;
+    st->obs_done = 0u;
+  }
+  for (int i = idx; i < n_desc; i += gridDim.x * blockDim.x) tile_desc[i] = 0ull;
+  if (st->status != ST_OK) return;
+  if (idx <= N) {
+    const double e = (double)(4 * idx - 2 * N);
+    tb.w[idx] = exp(-sp->dbeta * e);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// k_q_reduce: eq. 3.  Grid-stride gather of w[level(E_j)], per-thread serial sum, warp-shuffle tree, block
+// partials; the last block to finish adds the partials in index order (deterministic for a given grid) and
+// writes sumw, Q = sumw / R, ln Q, scale = R0 / R.
+// ---------------------------------------------------------------------------------------------------
+constexpr int RED_THREADS = 256;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+__global__ void __launch_bounds__(RED_THREADS)
+k_q_reduce(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
+           double* __restrict__ partial, double R0) {
+  if (st->status != ST_OK) return;
+  const int32_t* __restrict__ E = st->cur ? E1 : E0;
+  const unsigned long long R = st->R;
+  double acc = 0.0;
+  // four independent loads in flight per thread
+  const unsigned long long stride = (unsigned long long)gridDim.x * RED_THREADS;
+  unsigned long long j = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x;
+  for (; j + 3 * stride < R; j += 4 * stride) {
+    const int e0 = E[j], e1 = E[j + stride], e2 = E[j + 2 * stride], e3 = E[j + 3 * stride];
+    const double w0 = tb.w[(e0 + 2 * N) >> 2], w1 = tb.w[(e1 + 2 * N) >> 2];
+    const double w2 = tb.w[(e2 + 2 * N) >> 2], w3 = tb.w[(e3 + 2 * N) >> 2];
+    acc += (w0 + w1) + (w2 + w3);
+  }
+  for (; j < R; j += stride) acc += tb.w[(E[j] + 2 * N) >> 2];
+
+  __shared__ double s_part[RED_THREADS / 32];
+  __shared__ bool s_last;
+  acc = warp_sum(acc);
+  if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double b = 0.0;
+#pragma unroll
+    for (int w = 0; w < RED_THREADS / 32; ++w) b += s_part[w];
+    partial[blockIdx.x] = b;
+    __threadfence();
+    const unsigned done = atomicAdd(&st->reduce_done, 1u);
+    s_last = (done == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (s_last && threadIdx.x < 32) {
+    __threadfence();
+    double t = 0.0;
+    for (unsigned b = threadIdx.x; b < gridDim.x; b += 32) t += __ldcg(&partial[b]);
+    t = warp_sum(t);
+    if (threadIdx.x == 0) {
+      const double Q = t / (double)R;
+      st->sumw = t;
+      st->Q = Q;
+      st->lnQ = log(Q);
+      st->scale = R0 / (double)R;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// k_levels_tau: per level tau = w / Q (eq. 4), lambda = tau * scale, and the A4 chunk tables
+// (m, mu, F_0..F_64).  Only individually rounded IEEE operations (no FMA contraction).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double expneg_a4(double mu) {
+  // c_i = nearest double to (-1)^i / i!, i = 0..14
+  constexpr double c[15] = {0x1.0000000000000p+0,   -0x1.0000000000000p+0,  0x1.0000000000000p-1,
+                            -0x1.5555555555555p-3,  0x1.5555555555555p-5,   -0x1.1111111111111p-7,
+                            0x1.6c16c16c16c17p-10,  -0x1.a01a01a01a01ap-13, 0x1.a01a01a01a01ap-16,
+                            -0x1.71de3a556c734p-19, 0x1.27e4fb7789f5cp-22,  -0x1.ae64567f544e4p-26,
+                            0x1.1eed8eff8d898p-29,  -0x1.6124613a86d09p-33, 0x1.93974a8c07c9dp-37};
+  const double t = __dmul_rn(mu, 0.0625);
+  double p = c[14];
+#pragma unroll
+  for (int i = 13; i >= 0; --i) p = __dadd_rn(__dmul_rn(p, t), c[i]);
+#pragma unroll
+  for (int s = 0; s < 4; ++s) p = __dmul_rn(p, p);
+  return p;
+}
+
+__global__ void k_levels_tau(const DevState* st, LevelTables tb, int N) {
+  if (st->status != ST_OK) return;
+  const int lev = blockIdx.x * blockDim.x + threadIdx.x;
+  if (lev > N) return;
+  const double tau = __ddiv_rn(tb.w[lev], st->Q);
+  const double lambda = __dmul_rn(tau, st->scale);
+  tb.tau[lev] = tau;
+  double* F = tb.cdf + (size_t)lev * PO_ROW;
+  if (!(lambda > 0.0)) {
+    tb.m[lev] = 0u;
+    tb.mu[lev] = 0.0;
+    return;
+  }
+  if (!(lambda < 2147483648.0)) {  // would exceed any capacity: reported as PA_ECAPACITY if a replica sits here
+    tb.m[lev] = M_OVERFLOW;
+    tb.mu[lev] = 0.0;
+    return;
+  }
+  long long m = (long long)ceil(__ddiv_rn(lambda, 8.0));
+  if (m < 1) m = 1;
+  const double mu = __ddiv_rn(lambda, (double)m);
+  tb.m[lev] = (unsigned)m;
+  tb.mu[lev] = mu;
+  double p = expneg_a4(mu), Fk = p;
+  F[0] = Fk;
+  for (int k = 1; k <= PO_KMAX; ++k) {
+    p = __ddiv_rn(__dmul_rn(p, mu), (double)k);
+    Fk = __dadd_rn(Fk, p);
+    F[k] = Fk;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// k_poisson_scan: a2-a4.  n_j ~ Poisson(lambda_j) by chunked CDF inversion with keyed uniforms, fused with a
+// single-pass exclusive scan (decoupled look-back).  Tile = 8 warps x 8 rounds x 32 lanes = 2048 parents;
+// parents with many chunks (lambda > 32) are drawn cooperatively by the whole warp.
+// ---------------------------------------------------------------------------------------------------
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ROUNDS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ROUNDS;
+constexpr unsigned HEAVY_M = 4;  // chunks drawn by one lane before the warp takes over
+
+constexpr unsigned long long DESC_AGG = 1ull << 62, DESC_PREFIX = 2ull << 62, DESC_VAL = (1ull << 62) - 1;
+
+// one chunk: u from Philox words, k = first index with u <= F_k (capped at KMAX)
+__device__ __forceinline__ unsigned draw_chunk(const double* __restrict__ F, uint32_t j, unsigned long long c,
+                                               uint32_t c3, const PhiloxKey& key) {
+  const uint4 w = philox4x32_10((uint32_t)(c >> 1), j, 0u, c3, key);
+  const uint32_t hi = (c & 1ull) ? w.z : w.x, lo = (c & 1ull) ? w.w : w.y;
+  const unsigned long long x = ((unsigned long long)hi << 32) | lo;
+  const double u = ((double)(x >> 12) + 0.5) * 0x1p-52;  // exact
+  unsigned k = 0;
+  while (k < (unsigned)PO_KMAX && u > __ldg(F + k)) ++k;
+  return k;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS)
+k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
+               uint32_t* __restrict__ off, uint32_t* __restrict__ n_out, double* __restrict__ tau_out,
+               unsigned long long* tile_desc, uint32_t* __restrict__ tile_parent, int copy_tile,
+               unsigned long long capacity, const PhiloxKey key) {
+  if (st->status != ST_OK) return;
+  __shared__ unsigned s_tile;
+  __shared__ unsigned long long s_warp_tot[SCAN_THREADS / 32];
+  __shared__ unsigned long long s_prefix;
+  __shared__ unsigned s_overflow;
+  const unsigned long long R = st->R;
+  const unsigned ntiles = (unsigned)((R + SCAN_TILE - 1) / SCAN_TILE);
+  if (threadIdx.x == 0) {
+    s_tile = atomicAdd(&st->scan_tile, 1u);
+    s_overflow = 0u;
+  }
+  __syncthreads();
+  const unsigned tile = s_tile;
+  if (tile >= ntiles) return;
+  const int32_t* __restrict__ E = st->cur ? E1 : E0;
+  const uint32_t c3 = ctr3(TAG_RESAMPLE, st->step + 1u);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned long long warp_base = (unsigned long long)tile * SCAN_TILE + (unsigned long long)warp * (SCAN_ROUNDS * 32);
+
+  // phase 1: sampling (divergent; kept rolled), counts parked in shared memory
+  __shared__ unsigned s_cnt[SCAN_TILE];
+  unsigned* my_cnt = s_cnt + warp * (SCAN_ROUNDS * 32);
+  bool overflow = false;
+#pragma unroll 1
+  for (int r = 0; r < SCAN_ROUNDS; ++r) {
+    const unsigned long long j = warp_base + r * 32 + lane;
+    unsigned n = 0, m = 0, lev = 0;
+    if (j < R) {
+      lev = (unsigned)((E[j] + 2 * N) >> 2);
+      m = tb.m[lev];
+      if (tau_out) tau_out[j] = tb.tau[lev];
+      if (m == M_OVERFLOW) { overflow = true; m = 0; }
+    }
+    if (m > 0 && m <= HEAVY_M) {
+      const double* F = tb.cdf + (size_t)lev * PO_ROW;
+      for (unsigned c = 0; c < m; ++c) n += draw_chunk(F, (uint32_t)j, c, c3, key);
+    }
+    // heavy parents: the whole warp draws the chunks of one parent at a time
+    unsigned heavy = __ballot_sync(0xffffffffu, m > HEAVY_M);
+    while (heavy) {
+      const int src = __ffs(heavy) - 1;
+      heavy &= heavy - 1;
+      const unsigned hm = __shfl_sync(0xffffffffu, m, src);
+      const unsigned hlev = __shfl_sync(0xffffffffu, lev, src);
+      const uint32_t hj = (uint32_t)(warp_base + r * 32 + src);
+      const double* F = tb.cdf + (size_t)hlev * PO_ROW;
+      unsigned part = 0;
+      for (unsigned c = lane; c < hm; c += 32) part += draw_chunk(F, hj, c, c3, key);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+      if (lane == src) n = part;
+    }
+    my_cnt[r * 32 + lane] = n;
+  }
+  if (overflow) s_overflow = 1u;
+  __syncwarp();
+
+  // phase 2: warp-level scan in striped order (item = r*32 + lane)
+  unsigned cnt[SCAN_ROUNDS];
+  unsigned excl[SCAN_ROUNDS];  // tile-local exclusive offsets within the warp's 256 items
+  unsigned long long run = 0;
+#pragma unroll
+  for (int r = 0; r < SCAN_ROUNDS; ++r) {
+    const unsigned v = my_cnt[r * 32 + lane];
+    cnt[r] = v;
+    unsigned inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    excl[r] = (unsigned)run + (inc - v);
+    run += __shfl_sync(0xffffffffu, inc, 31);
+  }
+  if (lane == 0) s_warp_tot[warp] = run;
+  __syncthreads();
+  unsigned long long warp_excl = 0, tile_total = 0;
+#pragma unroll
+  for (int w = 0; w < SCAN_THREADS / 32; ++w) {
+    const unsigned long long t = s_warp_tot[w];
+    if (w < warp) warp_excl += t;
+    tile_total += t;
+  }
+
+  // decoupled look-back (warp 0)
+  if (warp == 0) {
+    unsigned long long prefix = 0;
+    if (tile == 0) {
+      if (lane == 0) atomicExch(&tile_desc[0], DESC_PREFIX | tile_total);
+    } else {
+      if (lane == 0) atomicExch(&tile_desc[tile], DESC_AGG | tile_total);
+      int look = (int)tile - 1;
+      while (true) {
+        const int idx = look - lane;
+        unsigned long long d = DESC_PREFIX;  // lanes before tile 0 read as an empty prefix
+        if (idx >= 0) {
+          do {
+            d = *((volatile unsigned long long*)&tile_desc[idx]);
+          } while ((d >> 62) == 0ull);
+        }
+        const unsigned is_prefix = __ballot_sync(0xffffffffu, (d >> 62) == 2ull);
+        unsigned long long v = d & DESC_VAL;
+        if (is_prefix) {
+          const int first = __ffs(is_prefix) - 1;  // nearest tile that already knows its inclusive prefix
+          if (lane > first) v = 0ull;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        prefix += v;
+        if (is_prefix) break;
+        look -= 32;
+      }
+      if (lane == 0) atomicExch(&tile_desc[tile], DESC_PREFIX | ((prefix + tile_total) & DESC_VAL));
+    }
+    if (lane == 0) s_prefix = prefix;
+  }
+  __syncthreads();
+  const unsigned long long base = s_prefix + warp_excl;
+
+  // offsets, counts, and for every copy tile the parent that covers its first child
+#pragma unroll
+  for (int r = 0; r < SCAN_ROUNDS; ++r) {
+    const unsigned long long j = warp_base + r * 32 + lane;
+    if (j < R) {
+      const unsigned long long o = base + excl[r];  // exact whenever R' fits the capacity
+      off[j] = (uint32_t)o;
+      if (n_out) n_out[j] = cnt[r];
+      if (cnt[r] > 0 && o + cnt[r] <= capacity) {
+        const unsigned long long t_first = (o + copy_tile - 1) / copy_tile, t_last = (o + cnt[r] - 1) / copy_tile;
+        for (unsigned long long t = t_first; t <= t_last; ++t) tile_parent[t] = (uint32_t)j;
+      }
+    }
+  }
+  if (tile == ntiles - 1 && threadIdx.x == 0) {
+    const unsigned long long Rnew = s_prefix + tile_total;
+    off[R] = (uint32_t)Rnew;
+    st->Rnew = Rnew;
+    if (Rnew > capacity) st->status = ST_CAPACITY;
+    else if (Rnew == 0ull) st->status = ST_EXTINCT;
+    if (st->status != ST_OK) st->fail_step = st->step + 1u;
+  }
+  __syncthreads();
+  if (s_overflow && threadIdx.x == 0) {
+    atomicExch(&st->status, (unsigned)ST_CAPACITY);
+    st->fail_step = st->step + 1u;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// k_balance: a5.  One block.  New partition table, born/excess/shortage per partition, moved count.
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_balance(DevState* st, const uint32_t* __restrict__ off, uint32_t* part0, uint32_t* part1,
+                          uint32_t* __restrict__ stats, int P) {
+  if (st->status != ST_OK) return;
+  const uint32_t* old_start = st->cur ? part1 : part0;
+  uint32_t* new_start = st->cur ? part0 : part1;
+  const unsigned long long Rnew = st->Rnew;
+  const unsigned long long base = Rnew / P, rem = Rnew % P;
+  __shared__ unsigned long long s_same;
+  if (threadIdx.x == 0) s_same = 0ull;
+  __syncthreads();
+  unsigned long long same = 0;
+  for (int p = threadIdx.x; p <= P; p += blockDim.x) {
+    const unsigned long long s = (unsigned long long)p * base + ((unsigned long long)p < rem ? p : rem);
+    new_start[p] = (uint32_t)s;
+    if (p < P) {
+      const unsigned long long e = (unsigned long long)(p + 1) * base + ((unsigned long long)(p + 1) < rem ? p + 1 : rem);
+      const uint32_t cnt = (uint32_t)(e - s);
+      const uint32_t b0 = off[old_start[p]], b1 = off[old_start[p + 1]];
+      const uint32_t born = b1 - b0;
+      stats[4 * p + 0] = cnt;
+      stats[4 * p + 1] = born;
+      stats[4 * p + 2] = born > cnt ? born - cnt : 0u;
+      stats[4 * p + 3] = cnt > born ? cnt - born : 0u;
+      // children of partition p's parents occupy [b0, b1); those inside [s, e) stay in partition p
+      const unsigned long long lo = b0 > s ? b0 : s, hi = b1 < e ? b1 : e;
+      if (hi > lo) same += hi - lo;
+    }
+  }
+  atomicAdd(&s_same, same);
+  __syncthreads();
+  if (threadIdx.x == 0) st->moved = Rnew - s_same;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// k_copy: a6.  Child-centric gather.  Block t owns children [t*CT, (t+1)*CT): it starts from the parent that
+// covers its first child (tile_parent, written by the scan), walks the offsets forward (coalesced), marks every
+// parent at the position of its first child in shared memory and max-scans the marks into a child->parent map;
+// then VT = S/16 lanes copy one lattice with 128-bit loads/stores.  Children are in parent order, so parent
+// reads are monotone and repeated parents hit L1/L2.
+// ---------------------------------------------------------------------------------------------------
+constexpr int COPY_THREADS = 256;
+
+template <int L>
+struct CopyGeo {
+  static constexpr int S = L * L / 8;                        // bytes per replica
+  static constexpr int VB = S < 16 ? S : 16;                 // bytes per vector access
+  static constexpr int VT = S / VB;                          // threads per child
+  static constexpr int CT = S <= 128 ? 1024 : (S <= 512 ? 512 : 256);  // children per tile (multiple of COPY_THREADS)
+};
+
+template <int VB> struct VecT;
+template <> struct VecT<16> { using type = uint4; };
+template <> struct VecT<8> { using type = uint2; };
+
+template <int L>
+__global__ void __launch_bounds__(COPY_THREADS)
+k_copy(const DevState* __restrict__ st, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tile_parent,
+       uint32_t* spins0, uint32_t* spins1, int32_t* E0, int32_t* E1, int32_t* M0, int32_t* M1) {
+  using CG = CopyGeo<L>;
+  using V = typename VecT<CG::VB>::type;
+  if (st->status != ST_OK) return;
+  const unsigned long long Rnew = st->Rnew, R = st->R;
+  const unsigned long long i0 = (unsigned long long)blockIdx.x * CG::CT;
+  if (i0 >= Rnew) return;
+  const unsigned cur = st->cur;  // source = buffer cur, destination = buffer cur^1 (never the same memory)
+  const V* __restrict__ src = reinterpret_cast<const V*>(cur ? spins1 : spins0);
+  V* __restrict__ dst = reinterpret_cast<V*>(cur ? spins0 : spins1);
+  const int32_t* __restrict__ Es = cur ? E1 : E0;
+  const int32_t* __restrict__ Ms = cur ? M1 : M0;
+  int32_t* __restrict__ Ed = cur ? E0 : E1;
+  int32_t* __restrict__ Md = cur ? M0 : M1;
+  const unsigned nchild = (unsigned)((Rnew - i0 < (unsigned long long)CG::CT) ? (Rnew - i0) : CG::CT);
+  const unsigned long long i1 = i0 + nchild;
+
+  __shared__ uint32_t s_par[CG::CT];
+  __shared__ uint32_t s_wmax[COPY_THREADS / 32];
+  for (int c = threadIdx.x; c < CG::CT; c += COPY_THREADS) s_par[c] = 0u;
+  __syncthreads();
+  const uint32_t j_first = tile_parent[blockIdx.x];
+  if (threadIdx.x == 0) s_par[0] = j_first;
+  // walk parents after j_first until their first child falls past the tile
+  for (unsigned long long jb = (unsigned long long)j_first + 1;; jb += COPY_THREADS) {
+    const unsigned long long j = jb + threadIdx.x;
+    bool past = true;
+    if (j < R) {
+      const uint32_t o = off[j], o1 = off[j + 1];
+      past = (o >= i1);
+      if (!past && o1 > o) s_par[o - i0] = (uint32_t)j;  // o >= i0 because j > j_first
+    }
+    // off is monotone: once the first lane of a chunk is past, all later parents are
+    if (__syncthreads_or(past && threadIdx.x == 0)) break;
+  }
+  __syncthreads();
+  // inclusive max-scan of s_par (CT / COPY_THREADS consecutive entries per thread)
+  {
+    constexpr int PER = CG::CT / COPY_THREADS;
+    uint32_t v[PER];
+    uint32_t mx = 0u;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+      mx = max(mx, s_par[threadIdx.x * PER + k]);
+      v[k] = mx;
+    }
+    uint32_t inc = mx;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc = max(inc, t);
+    }
+    if (lane == 31) s_wmax[warp] = inc;
+    __syncthreads();
+    uint32_t before = 0u;
+    for (int w = 0; w < warp; ++w) before = max(before, s_wmax[w]);
+    const uint32_t prev_lane = __shfl_up_sync(0xffffffffu, inc, 1);
+    if (lane > 0) before = max(before, prev_lane);
+#pragma unroll
+    for (int k = 0; k < PER; ++k) s_par[threadIdx.x * PER + k] = max(v[k], before);
+  }
+  __syncthreads();
+
+  // E, M of the children
+  for (unsigned c = threadIdx.x; c < nchild; c += COPY_THREADS) {
+    const uint32_t pj = s_par[c];
+    Ed[i0 + c] = Es[pj];
+    Md[i0 + c] = Ms[pj];
+  }
+  // lattices: VT threads per child, 4 children in flight per thread group
+  constexpr int GROUPS = COPY_THREADS / (CG::VT < COPY_THREADS ? CG::VT : COPY_THREADS);
+  if constexpr (CG::VT <= COPY_THREADS) {
+    const int sub = threadIdx.x % CG::VT, grp = threadIdx.x / CG::VT;
+    constexpr int UNR = 4;
+    unsigned c = grp;
+    for (; c + (UNR - 1) * GROUPS < nchild; c += UNR * GROUPS) {
+      V tmp[UNR];
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) tmp[u] = src[(unsigned long long)s_par[c + u * GROUPS] * CG::VT + sub];
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) dst[(i0 + c + u * GROUPS) * CG::VT + sub] = tmp[u];
+    }
+    for (; c < nchild; c += GROUPS) dst[(i0 + c) * CG::VT + sub] = src[(unsigned long long)s_par[c] * CG::VT + sub];
+  }
+}
+
+}  // namespace pa

@@ -1,0 +1,335 @@
+"""GPU parity (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): spins, E, M, copy counts, offsets, R', partition tables and
+integer moment sums BIT-EXACT; Q, tau, ln Z to relative 1e-12.  Lock-step: each step the oracle computes its own
+Q / tau (compared at 1e-12) and then draws the counts from the GPU's tau array, so that every integer that
+follows is compared exactly.
+"""
+import ctypes as C
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import pa_oracle as orc
+from paper_2006_00561_b200 import inputs
+
+import philox_ref
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-12  # north_star: "Q, tau and ln Z must agree to a relative error of 1e-12 in fp64"
+
+
+def _binding():
+    from paper_2006_00561_b200 import binding
+    return binding
+
+
+def rel(a, b):
+    return abs(a - b) / max(abs(b), 1e-300)
+
+
+def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None):
+    b = _binding()
+    gpu = b.PopulationAnnealer(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity,
+                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS)
+    if spins is not None:
+        gpu.set_spins(spins)
+    ora = orc.OraclePA(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity, spins=spins)
+    return gpu, ora
+
+
+def compare_population(gpu, ora, what=""):
+    assert gpu.R == ora.R, what
+    assert np.array_equal(gpu.spins(), ora.spins), what + " spins"
+    E, M = gpu.energies()
+    assert np.array_equal(E, ora.E), what + " E"
+    assert np.array_equal(M, ora.M), what + " M"
+    og, oo = gpu.observables(), ora.observables()
+    for k in ["R", "sum_E", "sum_E2", "sum_absM", "sum_M2", "sum_M4"]:
+        assert og[k] == oo[k], (what, k, og[k], oo[k])
+    for k in ["mean_E", "mean_E2", "mean_absM", "mean_M2", "mean_M4"]:
+        assert rel(og[k], oo[k]) <= 1e-15 or abs(og[k] - oo[k]) <= 1e-12, (what, k)
+
+
+def lockstep(gpu, ora, betas, theta, sweep_slots=None):
+    """sweep_slots=None: full-population sweep parity; else an int: number of hash-selected slots checked."""
+    L = ora.L
+    for k, beta in enumerate(betas, 1):
+        parents_before = ora.R
+        spins_before = ora.spins
+        gpu.step(beta, theta)
+        tau_gpu = gpu.tau()
+        info = ora.resample(beta, tau_override=tau_gpu)
+        lz = gpu.log_Z()
+        # fp64 quantities
+        assert rel(lz["last_Q"], info["Q"]) <= RTOL, (k, lz["last_Q"], info["Q"])
+        assert np.all(np.abs(tau_gpu - info["tau"]) <= RTOL * np.abs(info["tau"])), k
+        assert rel(lz["lnZ"], ora.lnZ) <= RTOL, (k, lz["lnZ"], ora.lnZ)
+        # integers
+        assert gpu.parents() == parents_before
+        n, off = gpu.counts()
+        assert np.array_equal(n, info["n"]), "step %d: copy counts" % k
+        assert np.array_equal(off, info["off"]), "step %d: offsets" % k
+        assert gpu.R == info["Rnew"]
+        ps, st, moved = gpu.partitions()
+        assert np.array_equal(ps, info["part_start"]) and np.array_equal(st, info["part_stats"]), k
+        assert moved == info["moved"], k
+        if theta > 0:
+            assert gpu.thresholds() == orc.thresholds(beta)
+        if sweep_slots is None:
+            ora.equilibrate(theta)
+            compare_population(gpu, ora, "step %d" % k)
+        else:
+            # a1-a6 on the full population: children are exact copies of their parents, in parent order.
+            # Sweeps: hash-selected slots, each swept alone by the oracle (depends only on lattice, slot, seed, step)
+            rng = np.random.default_rng(1000 + k)
+            slots = np.unique(rng.integers(0, ora.R, sweep_slots)).astype(np.uint32)
+            before = ora.spins[slots].copy()
+            parent = orc.parent_of(info["n"], info["off"], info["Rnew"])
+            assert np.array_equal(before, spins_before[parent[slots]])
+            if theta > 0:
+                T4, T8 = orc.thresholds(beta)
+                orc.sweeps_slots(L, slots, before, ora.seed, ora.step_no, theta, T4, T8)
+            got = gpu.spins()
+            assert np.array_equal(got[slots], before), "step %d: sampled sweeps" % k
+            if theta == 0:  # no sweeps: the whole redistributed population is comparable
+                assert np.array_equal(got, ora.spins), "step %d: redistribution" % k
+            # adopt the GPU population for the next step, after checking E/M of ALL replicas against the oracle's
+            # energy function (plain definition) -- keeps the oracle in lock-step without sweeping everything
+            E, M = gpu.energies()
+            Eo, Mo = orc.energy_mag(L, got)
+            assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+            ora.spins, ora.E, ora.M = got, Eo, Mo
+            og, oo = gpu.observables(), ora.observables()
+            for key in ["R", "sum_E", "sum_E2", "sum_absM", "sum_M2", "sum_M4"]:
+                assert og[key] == oo[key], (k, key)
+
+
+# ---------------------------------------------------------------------------------------------------
+# C3: Philox -- product device function == cuRAND's curand_Philox4x32_10 == oracle == big-int writing
+# ---------------------------------------------------------------------------------------------------
+def test_philox_product_vs_curand_vs_oracle():
+    import torch
+    path = os.path.join(os.path.dirname(__file__), "cuda", "libphilox_check.so")
+    if not os.path.exists(path):
+        pytest.skip("tests/cuda/libphilox_check.so not built (run __graft_entry__.build())")
+    lib = C.CDLL(path)
+    n = 1 << 20
+    rng = np.random.default_rng(2024)
+    ctr = rng.integers(0, 2 ** 32, (n, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, (n, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0], key[0] = 0, 0
+    ctr[1], key[1] = 0xFFFFFFFF, 0xFFFFFFFF
+    d = lambda a: torch.from_numpy(a.view(np.int32)).cuda()
+    dc, dk = d(ctr), d(key)
+    o1 = torch.zeros(n * 4, dtype=torch.int32, device="cuda")
+    o2 = torch.zeros(n * 4, dtype=torch.int32, device="cuda")
+    vp = C.c_void_p
+    lib.philox_check.argtypes = [vp, vp, vp, vp, C.c_int]
+    assert lib.philox_check(dc.data_ptr(), dk.data_ptr(), o1.data_ptr(), o2.data_ptr(), n) == 0
+    a = o1.cpu().numpy().view(np.uint32).reshape(n, 4)
+    b = o2.cpu().numpy().view(np.uint32).reshape(n, 4)
+    assert np.array_equal(a, b)  # product == cuRAND on 2^20 random (ctr, key)
+    for i in list(range(64)) + [n - 1]:
+        assert a[i].tolist() == orc.philox4x32_10(ctr[i], key[i]).tolist() == philox_ref.philox4x32_10(ctr[i], key[i])
+
+
+# ---------------------------------------------------------------------------------------------------
+# a0 init, a8 energies
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,R0", [(8, 1000), (16, 777), (32, 2049), (64, 515), (128, 130)])
+def test_init_population_parity(L, R0):
+    gpu, ora = make_pair(L, R0, P=3, seed=0x0123456789ABCDEF + L)
+    compare_population(gpu, ora, "init L=%d" % L)
+    assert rel(gpu.log_Z()["lnZ"], L * L * math.log(2)) < 1e-15
+    ps, _, _ = gpu.partitions()
+    assert np.array_equal(ps, orc.partition_table(R0, 3))
+
+
+@pytest.mark.parametrize("L", [8, 16, 32, 64, 128])
+def test_set_spins_energy_magnetisation(L):
+    R = 300
+    pop = inputs.structured_population(L, R, seed=L)
+    gpu, ora = make_pair(L, R, P=1, seed=1, spins=pop)
+    compare_population(gpu, ora, "set_spins L=%d" % L)
+    E, _ = gpu.energies()
+    assert E.min() == -2 * L * L and E.max() == 2 * L * L  # all-up and checkerboard are in the mixture
+
+
+# ---------------------------------------------------------------------------------------------------
+# lock-step parity, whole step, every supported L
+# ---------------------------------------------------------------------------------------------------
+def test_config1_full_lockstep():
+    wl = inputs.CONFIGS[1]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
+    compare_population(gpu, ora, "init")
+    lockstep(gpu, ora, [wl.beta(k) for k in range(1, wl.K + 1)], wl.theta)
+    exact = 128.715437337408418  # Kaufman L=8, beta=1 (tests/golden/ising_exact.json)
+    assert abs(gpu.log_Z()["lnZ"] - exact) < 0.2
+
+
+@pytest.mark.parametrize("L,R0,P,K,theta,dbeta", [
+    (16, 3000, 5, 12, 3, 0.04),
+    (32, 4096, 1, 16, 10, 0.03),     # config 2 shape, reduced population, coarser schedule crossing beta_c
+    (64, 2048, 148, 8, 4, 0.06),      # config 3 shape
+    (128, 600, 148, 4, 2, 0.1),       # config 4 shape
+])
+def test_reduced_configs_lockstep(L, R0, P, K, theta, dbeta):
+    gpu, ora = make_pair(L, R0, P, seed=L + 11)
+    lockstep(gpu, ora, [dbeta * k for k in range(1, K + 1)], theta)
+
+
+def test_ragged_population_sizes_and_theta1():
+    # sizes around tile boundaries of the scan (2048), the copy (1024) and a warp
+    for R0 in [1, 31, 33, 1023, 1025, 2047, 2049, 4097]:
+        gpu, ora = make_pair(32, R0, P=7, seed=R0)
+        lockstep(gpu, ora, [0.02, 0.05, 0.2], 1)
+
+
+def test_skewed_resampling_heavy_parents():
+    # structured population + a large dbeta: tau spans many decades, heavy parents (lambda >> 32) use the
+    # warp-cooperative chunk loop; dead parents come in long runs
+    L, R = 32, 20000
+    pop = inputs.random_packed_population(L, R, seed=5)          # E ~ 0
+    ordered = inputs.structured_population(L, 64, seed=6)         # a few lattices with E down to -2N
+    where = np.random.default_rng(7).choice(R, 64, replace=False)
+    pop[where] = ordered
+    pop[5000:5300] = inputs.random_packed_population(L, 300, seed=8, p_up=0.5) ^ np.uint32(0x55555555)
+    gpu, ora = make_pair(L, R, P=148, seed=55, beta0=0.3, spins=pop, capacity=40960)
+    gpu.step(0.3 + 0.004, 0)
+    tau = gpu.tau()
+    info = ora.resample(0.3 + 0.004, tau_override=tau)
+    n, off = gpu.counts()
+    assert tau.max() > 100 and (info["n"] == 0).mean() > 0.5  # really skewed
+    assert info["n"].max() > 64
+    assert np.array_equal(n, info["n"]) and np.array_equal(off, info["off"])
+    assert rel(gpu.log_Z()["last_Q"], info["Q"]) <= RTOL
+    compare_population(gpu, ora, "skewed")
+    ps, st, moved = gpu.partitions()
+    assert np.array_equal(ps, info["part_start"]) and np.array_equal(st, info["part_stats"]) and moved == info["moved"]
+    # a second step with sweeps from the skewed population
+    lockstep(gpu, ora, [0.32], 2)
+
+
+def test_config5_reduced_resample_only():
+    wl = inputs.CONFIGS[5].scaled(1 << 17)
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed, beta0=wl.beta0)
+    lockstep(gpu, ora, [wl.beta_K], 0)
+    n, _ = gpu.counts()
+    assert n.max() >= 32 and (n == 0).mean() > 0.5  # the skew config 5 is meant to have
+
+
+# ---------------------------------------------------------------------------------------------------
+# full-size configs in the launch configuration bench.py times
+# ---------------------------------------------------------------------------------------------------
+def test_config2_full_size_first_steps():
+    wl = inputs.CONFIGS[2]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
+    compare_population(gpu, ora, "init")
+    lockstep(gpu, ora, [wl.beta(k) for k in range(1, 4)], wl.theta)
+
+
+def test_config3_full_size_sampled():
+    wl = inputs.CONFIGS[3]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
+    compare_population(gpu, ora, "init")
+    # jump close to the critical region so that copy counts are skewed, then two paper-sized steps
+    lockstep(gpu, ora, [0.30, 0.42, 0.425], wl.theta, sweep_slots=4096)
+    ps, st, _ = gpu.partitions()
+    cnt = np.diff(ps.astype(np.int64))
+    assert len(cnt) == 148 and cnt.max() - cnt.min() <= 1
+
+
+def test_config4_full_size_sampled():
+    wl = inputs.CONFIGS[4]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
+    lockstep(gpu, ora, [0.2, 0.2012], wl.theta, sweep_slots=1024)
+
+
+def test_config5_full_size():
+    wl = inputs.CONFIGS[5]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed, beta0=wl.beta0)
+    lockstep(gpu, ora, [wl.beta_K], 0, sweep_slots=4096)
+    n, _ = gpu.counts()
+    assert n.max() > 1000 and (n > 0).mean() < 0.3  # U/R ~ 0.22, max n ~ 1e4
+
+
+# ---------------------------------------------------------------------------------------------------
+# boundary behaviour
+# ---------------------------------------------------------------------------------------------------
+def test_run_equals_repeated_step_and_is_deterministic():
+    b = _binding()
+    betas = [0.05 * k for k in range(1, 9)]
+    a = b.PopulationAnnealer(32, 3000, P=4, seed=9)
+    for beta in betas:
+        a.step(beta, 2)
+    c = b.PopulationAnnealer(32, 3000, P=4, seed=9)
+    assert c.run(betas, 2) == len(betas)
+    assert a.R == c.R and np.array_equal(a.spins(), c.spins())
+    assert a.log_Z() == c.log_Z() and a.observables() == c.observables()
+    assert a.beta_steps() == c.beta_steps() == (betas[-1], len(betas))
+
+
+def test_capacity_error_leaves_population_unchanged():
+    b = _binding()
+    g = b.PopulationAnnealer(16, 1024, P=2, seed=3, capacity=1024)
+    failures = 0
+    for k in range(1, 60):
+        before, R_before, lz_before, bs = g.spins(), g.R, g.log_Z(), g.beta_steps()
+        try:
+            g.step(0.002 * k, 1)
+        except b.PaError as e:
+            assert e.code == b.PA_ECAPACITY
+            failures += 1
+            assert g.R == R_before and np.array_equal(g.spins(), before)
+            assert g.log_Z() == lz_before and g.beta_steps() == bs
+    assert failures > 5  # R' ~ Poisson(1024) exceeds 1024 about half of the time
+    assert g.beta_steps()[1] == 59 - failures
+
+
+def test_invalid_arguments():
+    b = _binding()
+    with pytest.raises(b.PaError):
+        b.PopulationAnnealer(12, 100)  # unsupported L
+    with pytest.raises(b.PaError):
+        b.PopulationAnnealer(8, 0)
+    g = b.PopulationAnnealer(8, 64)
+    for bad in [lambda: g.step(float("nan"), 1), lambda: g.step(0.1, -1), lambda: g.step(-0.1, 1),
+                lambda: g.step(1e4, 0), lambda: g.spins(0, 65), lambda: g.tau()]:
+        with pytest.raises(b.PaError) as ei:
+            bad()
+        assert ei.value.code == b.PA_EINVAL
+    g.step(0.1, 1)  # still usable
+
+
+def test_global_flip_covariance_on_gpu():
+    b = _binding()
+    pop = inputs.random_packed_population(64, 500, seed=8)
+    a = b.PopulationAnnealer(64, 500, seed=77)
+    c = b.PopulationAnnealer(64, 500, seed=77)
+    a.set_spins(pop)
+    c.set_spins(~pop)
+    for k in range(1, 5):
+        a.step(0.1 * k, 3)
+        c.step(0.1 * k, 3)
+        assert np.array_equal(a.spins(), ~c.spins())
+        Ea, Ma = a.energies()
+        Ec, Mc = c.energies()
+        assert np.array_equal(Ea, Ec) and np.array_equal(Ma, -Mc)
+        assert a.log_Z() == c.log_Z()
+
+
+def test_device_getters_and_launch_count():
+    b = _binding()
+    g = b.PopulationAnnealer(32, 2000, seed=4, flags=b.PA_PROFILE)
+    l0 = g.launch_count()
+    g.step(0.1, 2)
+    assert g.launch_count() - l0 == 8
+    Ed, Md = g.energies_device()
+    E, M = g.energies()
+    assert np.array_equal(Ed.cpu().numpy(), E) and np.array_equal(Md.cpu().numpy(), M)
+    prof = g.profile_read()
+    assert all(cnt == 1 for _, cnt in prof.values()) and prof["sweep"][0] > 0
