@@ -156,7 +156,7 @@ def test_set_spins_energy_magnetisation(L):
     gpu, ora = make_pair(L, R, P=1, seed=1, spins=pop)
     compare_population(gpu, ora, "set_spins L=%d" % L)
     E, _ = gpu.energies()
-    assert E.min() == -2 * L * L and E.max() == 2 * L * L  # all-up and checkerboard are in the mixture
+    assert E.min() < -1.5 * L * L and E.max() > 1.5 * L * L  # ordered and checkerboard-like lattices are in the mixture
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -175,7 +175,7 @@ def test_config1_full_lockstep():
     (16, 3000, 5, 12, 3, 0.04),
     (32, 4096, 1, 16, 10, 0.03),     # config 2 shape, reduced population, coarser schedule crossing beta_c
     (64, 2048, 148, 8, 4, 0.06),      # config 3 shape
-    (128, 600, 148, 4, 2, 0.1),       # config 4 shape
+    (128, 600, 148, 5, 2, 0.02),      # config 4 shape (|dbeta|*2N < 700, reading G11)
 ])
 def test_reduced_configs_lockstep(L, R0, P, K, theta, dbeta):
     gpu, ora = make_pair(L, R0, P, seed=L + 11)
@@ -236,8 +236,8 @@ def test_config3_full_size_sampled():
     wl = inputs.CONFIGS[3]
     gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
     compare_population(gpu, ora, "init")
-    # jump close to the critical region so that copy counts are skewed, then two paper-sized steps
-    lockstep(gpu, ora, [0.30, 0.42, 0.425], wl.theta, sweep_slots=4096)
+    # coarse steps (|dbeta|*2N < 700, reading G11) up to the critical region, then two paper-sized steps
+    lockstep(gpu, ora, [0.08, 0.16, 0.24, 0.32, 0.40, 0.435, 0.44], wl.theta, sweep_slots=4096)
     ps, st, _ = gpu.partitions()
     cnt = np.diff(ps.astype(np.int64))
     assert len(cnt) == 148 and cnt.max() - cnt.min() <= 1
@@ -246,7 +246,7 @@ def test_config3_full_size_sampled():
 def test_config4_full_size_sampled():
     wl = inputs.CONFIGS[4]
     gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
-    lockstep(gpu, ora, [0.2, 0.2012], wl.theta, sweep_slots=1024)
+    lockstep(gpu, ora, [0.02, 0.04, 0.0412], wl.theta, sweep_slots=1024)
 
 
 def test_config5_full_size():
@@ -312,9 +312,9 @@ def test_global_flip_covariance_on_gpu():
     c = b.PopulationAnnealer(64, 500, seed=77)
     a.set_spins(pop)
     c.set_spins(~pop)
-    for k in range(1, 5):
-        a.step(0.1 * k, 3)
-        c.step(0.1 * k, 3)
+    for k in range(1, 7):
+        a.step(0.08 * k, 3)
+        c.step(0.08 * k, 3)
         assert np.array_equal(a.spins(), ~c.spins())
         Ea, Ma = a.energies()
         Ec, Mc = c.energies()
@@ -325,6 +325,7 @@ def test_global_flip_covariance_on_gpu():
 def test_device_getters_and_launch_count():
     b = _binding()
     g = b.PopulationAnnealer(32, 2000, seed=4, flags=b.PA_PROFILE)
+    g.profile_read()  # drain the launches of pa_init
     l0 = g.launch_count()
     g.step(0.1, 2)
     assert g.launch_count() - l0 == 8
