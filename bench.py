@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- population-annealing hot path on B200 (arxiv 2006.00561), driver contract.
+
+    python bench.py --gpus N --steps K --warmup W            # our CUDA path (default N=1, config 3)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle as it stands (reference arm)
+
+A "step" is one pa_step: Q/tau reduction, Poisson resampling, scan, partition balance, replica copy, theta
+Metropolis sweeps, observables.  Workload: BASELINE.json configs[2] ("config 3": L=64, R0=2^21, dbeta=0.005,
+theta=10, P=148) -- the paper's own workload shape on one GPU; its population (1 GiB)
+is larger than L2.  metric = spin-flip attempts/s over the whole step.  The resampling/redistribution path
+(config 5, theta=0) is measured in the same run and reported under "resample".  N > 1: independent replicas of
+the whole simulation, one per GPU ("replicas only"), no data-path collective.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2006_00561_b200 import inputs  # noqa: E402
+
+I_MIN = 12.0          # algorithmic lane-instructions per flip attempt
+WIDE_PER_ATTEMPT = 4.5  # 32x32->64 multiplies per attempt that cannot be hoisted (18 per Philox block of 4 sites)
+SM_COUNT, SMSP, LANES = 148, 4, 32
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu, self.proc, self.lines = gpu_index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._pump, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                mx.append(float(f[2]))
+                pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def schedule(wl, first_step, count):
+    dbeta = (wl.beta_K - wl.beta0) / wl.K
+    return [wl.beta0 + dbeta * k for k in range(first_step, first_step + count)]
+
+
+# ---------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of our arm; the whole reference arm)
+# ---------------------------------------------------------------------------------------------------
+def oracle_sample_run(wl, R_sample, steps, warmup):
+    """the oracle, as it stands, on a bounded sample of the workload: same L, dbeta, theta, P; R = R_sample"""
+    from oracle import pa_oracle as orc
+    cores = orc.max_threads()
+    small = wl.scaled(R_sample)
+    pa = orc.OraclePA(small.L, small.R0, P=small.P, seed=small.seed, beta0=small.beta0)
+    betas = schedule(wl, 1, warmup + steps)
+    for b in betas[:warmup]:
+        pa.step(b, wl.theta)
+    attempts = 0
+    t0 = time.perf_counter()
+    for b in betas[warmup:]:
+        pa.step(b, wl.theta)
+        attempts += wl.theta * wl.N * pa.R
+    dt = time.perf_counter() - t0
+    return {"attempts": attempts, "seconds": dt, "cores": cores, "R_sample": R_sample, "steps": steps,
+            "lnZ": pa.lnZ}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl = inputs.CONFIGS[args.config]
+    R_sample = 2048
+    r = oracle_sample_run(wl, R_sample, args.steps, args.warmup)
+    value = r["attempts"] / r["seconds"]
+    sample = "oracle on %s at R=%d (same L, dbeta, theta, P), %d steps" % (wl.name, R_sample, args.steps)
+    line = {"impl": "reference", "metric": "spin_flip_attempts_per_s", "value": value, "unit": "attempts/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * r["seconds"] / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32+f64", "data": "synthetic",
+            "config": {"workload": wl.name + " (bounded sample R=%d)" % R_sample, "L": wl.L, "theta": wl.theta, "P": wl.P},
+            "cpu_baseline": {"value": value, "unit": "attempts/s", "cores": r["cores"], "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "attempts/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+def resample_leg(binding, torch, peaks, repeats=5):
+    """config 5: a1-a6 only (theta=0) on R=2^24 L=32 lattices; algorithmic bytes S*(U+R') + 28*R per step"""
+    wl = inputs.CONFIGS[5]
+    S = wl.bytes_per_replica
+    times, res = [], None
+    for rep in range(repeats + 2):  # a fresh context per repeat: same parents, same step (pa_init is deterministic)
+        pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0, flags=binding.PA_PROFILE)
+        pa.profile_read()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(pa.stream)
+        pa.step(wl.beta_K, 0)
+        ev1.record(pa.stream)
+        torch.cuda.synchronize()
+        prof = pa.profile_read()
+        R, Rn = pa.parents(), pa.R
+        off = pa.counts_device()
+        U = int(torch.count_nonzero(off[1:] != off[:-1]).item())
+        k_ms = {k: v[0] for k, v in prof.items()}
+        chain_ms = sum(k_ms[k] for k in ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "copy"])
+        if rep >= 2:
+            times.append((chain_ms, ev0.elapsed_time(ev1), k_ms))
+        res = (R, Rn, U)
+        del pa, off
+    torch.cuda.empty_cache()
+    R, Rn, U = res
+    chain = statistics.median(t[0] for t in times)
+    wall = statistics.median(t[1] for t in times)
+    copy_ms = statistics.median(t[2]["copy"] for t in times)
+    scan_ms = statistics.median(t[2]["poisson_scan"] for t in times)
+    red_ms = statistics.median(t[2]["q_reduce"] for t in times)
+    alg_bytes = S * (U + Rn) + 28 * R
+    copy_bytes = S * (U + Rn) + 4 * R + 8 * Rn + 8 * U  # lattices + offsets read + E,M written/read
+    return {"workload": wl.name, "R": R, "R_new": Rn, "U": U, "algorithmic_bytes": alg_bytes,
+            "ms_a1_a6_kernels": chain, "ms_step_wall": wall, "ms_copy": copy_ms, "ms_poisson_scan": scan_ms,
+            "ms_q_reduce": red_ms, "replicas_per_s": Rn / (chain * 1e-3),
+            "roofline": {"bound": "hbm", "achieved": alg_bytes / (chain * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                         "unit": "GB/s", "frac": alg_bytes / (chain * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                         "peak_src": peaks["src"], "traffic": None,
+                         "copy_kernel_GBps": copy_bytes / (copy_ms * 1e-3) / 1e9,
+                         "frac_vs_8000": alg_bytes / (chain * 1e-3) / 1e9 / 8000.0}}
+
+
+def e2e_leg(pa, torch, wl, first_step, steps):
+    """same metric through the C ABI with HOST buffers: every step uploads the population from pinned host memory
+    (pa_set_spins), runs pa_step, and reads the new population + E, M back to pinned host memory."""
+    cap_words = (pa.R + 65536) * pa.wpr
+    host_pop = torch.empty(cap_words, dtype=torch.int32).pin_memory()
+    host_E = torch.empty(pa.R + 65536, dtype=torch.int32).pin_memory()
+    host_M = torch.empty(pa.R + 65536, dtype=torch.int32).pin_memory()
+    R = pa.R
+    pa.spins_into_host_tensor(host_pop, R)
+    betas = schedule(wl, first_step, steps)
+    h2d = d2h = 0
+    attempts = 0
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for b in betas:
+        pa.set_spins_host_tensor(host_pop, R)            # H2D: R*S bytes
+        h2d += R * pa.wpr * 4
+        pa.step(b, wl.theta)
+        R = pa.R
+        pa.spins_into_host_tensor(host_pop, R)           # D2H: R'*S bytes
+        pa.energies_into_host_tensors(host_E, host_M, R)  # D2H: 8 R' bytes
+        d2h += R * pa.wpr * 4 + 8 * R
+        attempts += wl.theta * wl.N * R
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    return {"attempts": attempts, "seconds": dt, "h2d_bytes_per_step": h2d // steps, "d2h_bytes_per_step": d2h // steps}
+
+
+def run_ours(args):
+    import torch
+    from paper_2006_00561_b200 import binding, dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    g = dist.init_from_env()
+    torch.cuda.set_device(g.local_rank)
+    peaks = measured_peaks()
+    wl = inputs.CONFIGS[args.config]
+    K, W = args.steps, max(args.warmup, 0)
+
+    pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed + 1000 * g.rank, beta0=wl.beta0,
+                                    flags=binding.PA_PROFILE)
+    if W > 0:
+        pa.run(schedule(wl, 1, W), wl.theta)
+    pa.profile_read()
+    betas = schedule(wl, W + 1, K)
+    sampler = ClockSampler(g.local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier(g)
+    torch.cuda.synchronize()
+    rs0, l0 = pa.replica_steps(), pa.launch_count()
+    ev0.record(pa.stream)
+    done = pa.run(betas, wl.theta)
+    ev1.record(pa.stream)
+    torch.cuda.synchronize()
+    dist.barrier(g)
+    seconds = ev0.elapsed_time(ev1) * 1e-3
+    clocks = sampler.stop()
+    assert done == K
+    replica_steps = pa.replica_steps() - rs0
+    launches = pa.launch_count() - l0
+    prof = pa.profile_read()
+    units = wl.theta * wl.N * replica_steps if wl.theta > 0 else replica_steps
+    value, total_units, tmax = dist.aggregate_throughput(g, units, seconds)
+    launches_total = int(dist.sum_over_ranks(g, launches))
+
+    # dominant kernel: the Metropolis sweep (ALU / issue bound)
+    sweep_ms, sweep_n = prof["sweep"]
+    step_kernel_ms = sum(v[0] for v in prof.values())
+    line = None
+    extra = {}
+    if wl.theta > 0 and sweep_n > 0:
+        attempts_per_launch = units / sweep_n
+        sweep_rate = attempts_per_launch / (sweep_ms / sweep_n * 1e-3)  # attempts/s inside the kernel
+        achieved = sweep_rate * I_MIN / 1e12
+        peak = SM_COUNT * SMSP * LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-instr/s (12 per flip attempt)",
+                "frac": achieved / peak, "traffic": None, "kernel": "k_sweep<%d>" % wl.L,
+                "kernel_attempts_per_s": sweep_rate, "kernel_ms_per_launch": sweep_ms / sweep_n,
+                "kernel_share_of_step": sweep_ms / step_kernel_ms,
+                "peak_src": "148 SM x 4 SMSP x 32 lanes x %d MHz (clocks.max.sm), 1 warp-instr/clk/SMSP" % peaks["sm_max_mhz"]}
+        if clocks.get("sm_mhz"):
+            roof["frac_at_measured_clock"] = achieved / (SM_COUNT * SMSP * LANES * clocks["sm_mhz"] * 1e6 / 1e12)
+    else:
+        roof = None
+    per_kernel = {k: {"ms_total": v[0], "launches": v[1]} for k, v in prof.items()}
+
+    e2e = cpu = resample = None
+    if g.is_main or g.world > 1:
+        if not args.no_e2e:
+            n_e2e = max(1, min(K, 6))
+            r = e2e_leg(pa, torch, wl, W + K + 1, n_e2e)
+            e2e_value, _, _ = dist.aggregate_throughput(g, r["attempts"], r["seconds"])
+            e2e = {"value": e2e_value, "unit": "attempts/s", "h2d_bytes_per_step": r["h2d_bytes_per_step"],
+                   "d2h_bytes_per_step": r["d2h_bytes_per_step"], "steps": n_e2e}
+    lnZ = pa.log_Z()["lnZ"]
+    beta_now = pa.beta_steps()[0]
+    R_final = pa.R
+    del pa
+    torch.cuda.empty_cache()
+    if g.is_main and g.world == 1:
+        if not args.no_resample:
+            resample = resample_leg(binding, torch, peaks)
+        if not args.no_cpu_baseline:
+            r = oracle_sample_run(wl, 2048, 24, 1)
+            cpu = {"value": r["attempts"] / r["seconds"], "unit": "attempts/s", "cores": r["cores"], "kind": "oracle",
+                   "sample": "%s at R=%d (same L, dbeta, theta, P), %d steps, %.1f s" % (wl.name, r["R_sample"], r["steps"], r["seconds"])}
+    if g.is_main:
+        line = {"metric": "spin_flip_attempts_per_s", "value": value, "unit": "attempts/s", "n_gpus": g.world, "steps": K,
+                "warmup": W, "ms_per_step": 1e3 * tmax / K, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "u32 bit-packed spins, i32 energies, f64 weights", "data": "synthetic",
+                "config": {"workload": wl.name, "L": wl.L, "R0": wl.R0, "dbeta": (wl.beta_K - wl.beta0) / wl.K,
+                           "theta": wl.theta, "P": wl.P, "beta_range": [betas[0], betas[-1]],
+                           "parallelism": "replicas only x%d" % g.world,
+                           "l2": "population %.0f MiB per buffer > 126 MB L2, no flush needed" % (wl.R0 * wl.bytes_per_replica / 2 ** 20)},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_total, "roofline": roof, "cpu_baseline": cpu,
+                "resample": resample, "kernels": per_kernel, "anneal": {"lnZ": lnZ, "beta": beta_now, "R": R_final,
+                                                                         "replica_steps": replica_steps}}
+        print(json.dumps(line))
+    dist.shutdown(g)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-resample", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3  # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -116,6 +116,9 @@ int pa_run(pa_ctx* ctx, const double* betas, int32_t K, int32_t theta, int32_t* 
 
 int pa_population(pa_ctx* ctx, int64_t* R);
 int pa_beta(pa_ctx* ctx, double* beta, int64_t* steps);
+/* work counter: sum over all committed steps of the resampled population size R' (replica-steps); the number of
+ * spin-flip attempts of a run with constant theta is theta * N * (difference of this counter) */
+int pa_totals(pa_ctx* ctx, int64_t* replica_steps);
 
 /* E_j (and M_j) of slots 0..n-1 of the current population, slot order.  n <= R.  M may be NULL. */
 int pa_energies(pa_ctx* ctx, int32_t* E, int32_t* M, int64_t n, int dst_on_device);

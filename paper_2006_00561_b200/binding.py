@@ -15,7 +15,7 @@ PA_OK, PA_EINVAL, PA_ENOMEM, PA_ECAPACITY, PA_EEXTINCT, PA_ECUDA = 0, -1, -2, -3
 PA_KEEP_TAU, PA_KEEP_COUNTS, PA_PROFILE = 1, 2, 4
 KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "copy", "sweep", "observe"]
 
-EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_population", "pa_beta", "pa_energies", "pa_log_Z",
+EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
            "pa_observables", "pa_spins", "pa_tau", "pa_counts", "pa_parents", "pa_partitions", "pa_thresholds",
            "pa_set_spins", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
 
@@ -59,6 +59,7 @@ def load_library():
         "pa_run": (C.c_int, [vp, f64p, C.c_int32, C.c_int32, i32p]),
         "pa_population": (C.c_int, [vp, i64p]),
         "pa_beta": (C.c_int, [vp, f64p, i64p]),
+        "pa_totals": (C.c_int, [vp, i64p]),
         "pa_energies": (C.c_int, [vp, vp, vp, C.c_int64, C.c_int]),
         "pa_log_Z": (C.c_int, [vp, f64p, f64p, f64p]),
         "pa_observables": (C.c_int, [vp, C.POINTER(PaObs)]),
@@ -157,6 +158,29 @@ class PopulationAnnealer:
         b, s = C.c_double(0), C.c_int64(0)
         self._check(self._lib.pa_beta(self._ctx, C.byref(b), C.byref(s)))
         return float(b.value), int(s.value)
+
+    def replica_steps(self):
+        r = C.c_int64(0)
+        self._check(self._lib.pa_totals(self._ctx, C.byref(r)))
+        return int(r.value)
+
+    # host-pointer variants for the end-to-end leg of bench.py (pinned torch CPU tensors)
+    def set_spins_host_tensor(self, t, R):
+        self._check(self._lib.pa_set_spins(self._ctx, C.c_void_p(t.data_ptr()), int(R), 0))
+
+    def spins_into_host_tensor(self, t, count):
+        self._check(self._lib.pa_spins(self._ctx, C.c_void_p(t.data_ptr()), 0, int(count), 0))
+
+    def energies_into_host_tensors(self, tE, tM, n):
+        self._check(self._lib.pa_energies(self._ctx, C.c_void_p(tE.data_ptr()), C.c_void_p(tM.data_ptr()), int(n), 0))
+
+    def counts_device(self):
+        """offsets off[0..parents] as a torch int32 tensor on the device (measurement helper)"""
+        torch = self._torch
+        npar = self.parents()
+        off = torch.empty(npar + 1, dtype=torch.int32, device=self.device)
+        self._check(self._lib.pa_counts(self._ctx, None, C.c_void_p(off.data_ptr()), npar, 1))
+        return off
 
     def energies(self, n=None):
         n = self.R if n is None else int(n)

@@ -451,6 +451,12 @@ int pa_population(pa_ctx* c, int64_t* R) {
   return PA_OK;
 }
 
+int pa_totals(pa_ctx* c, int64_t* replica_steps) {
+  if (!c || !replica_steps) return PA_EINVAL;
+  *replica_steps = (int64_t)c->h_state->replica_steps;
+  return PA_OK;
+}
+
 int pa_beta(pa_ctx* c, double* beta, int64_t* steps) {
   if (!c) return PA_EINVAL;
   if (beta) *beta = c->beta;

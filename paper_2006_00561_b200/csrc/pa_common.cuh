@@ -24,6 +24,7 @@ struct DevState {
   unsigned long long moved;      // children whose partition differs from the parent's (last step)
   unsigned long long obs[10];    // {lo,hi} x (sum E, sum E^2, sum |M|, sum M^2, sum M^4)
   unsigned long long obs_R;
+  unsigned long long replica_steps;  // sum over committed steps of R' (work counter for throughput metrics)
   unsigned int step;             // committed steps
   unsigned int cur;              // index of the buffer holding the current population
   unsigned int status;           // 0 = ok, else -pa_status of the failing step

@@ -107,6 +107,7 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
     if (mode == 0) {  // commit: the new population becomes the current one
       st->R_parents = st->R;
       st->R = st->Rnew;
+      st->replica_steps += st->Rnew;
       st->cur ^= 1u;
       st->step += 1u;
       st->sum_lnQ += st->lnQ;
