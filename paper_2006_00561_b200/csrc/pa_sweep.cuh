@@ -47,12 +47,20 @@ __device__ __forceinline__ uint32_t spread_bits(uint32_t x) {  // bits 0..15 -> 
   return x;
 }
 
-// all-ones iff w < T (unsigned): hi word of the 64-bit sum w + (2^64 - T); runs on the FMA pipe (IMAD.WIDE)
-// so that the compare does not compete with Philox's LOP3s for the ALU pipe.
-__device__ __forceinline__ uint32_t lt_mask(uint32_t w, unsigned long long negT) {
-  unsigned long long s;
-  asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(s) : "r"(w), "l"(negT));
-  return (uint32_t)(s >> 32);
+// acc |= BIT if w < T (unsigned).  Written as compare + predicated OR so that both instructions stay on the
+// ALU pipe: the FMA pipe is saturated by Philox's 32x32->64 multiplies (ptxas turns carry-based forms into IMAD.X).
+template <uint32_t BIT>
+__device__ __forceinline__ void or_if_lt(uint32_t& acc, uint32_t w, uint32_t T) {
+  asm("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %1, %2;\n\t@p or.b32 %0, %0, %3;\n\t}" : "+r"(acc) : "r"(w), "r"(T), "n"(BIT));
+}
+
+// the two random masks of one Philox block (4 consecutive active sites) at bit offset SH
+template <int SH>
+__device__ __forceinline__ void push_block(uint32_t& r4, uint32_t& r8, const uint4& w, uint32_t T4, uint32_t T8) {
+  or_if_lt<(1u << SH)>(r4, w.x, T4); or_if_lt<(2u << SH)>(r4, w.y, T4);
+  or_if_lt<(4u << SH)>(r4, w.z, T4); or_if_lt<(8u << SH)>(r4, w.w, T4);
+  or_if_lt<(1u << SH)>(r8, w.x, T8); or_if_lt<(2u << SH)>(r8, w.y, T8);
+  or_if_lt<(4u << SH)>(r8, w.z, T8); or_if_lt<(8u << SH)>(r8, w.w, T8);
 }
 
 template <int L>
@@ -84,7 +92,7 @@ __device__ __forceinline__ void rot_row(const uint32_t (&s)[Geo<L>::WPP], int di
 // One half-sweep of colour C on the lane's rows.  T = plane C (updated), S = plane 1-C (read only).
 template <int L, int C>
 __device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot, uint32_t t, uint32_t c3,
-                                           const PhiloxKey& key, unsigned long long negT4, unsigned long long negT8) {
+                                           const PhiloxKey& key, uint32_t T4, uint32_t T8) {
   using G_ = Geo<L>;
   constexpr unsigned FULL = 0xffffffffu;
   uint32_t(&T)[G_::RPL][G_::WPP] = lat.p[C];
@@ -117,16 +125,32 @@ __device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot
       // random masks: bit k set iff the site's keyed word < T4 (resp. T8)
       uint32_t r4 = 0u, r8 = 0u;
       const uint32_t call0 = (uint32_t)y * G_::CALLS_PER_ROW + (uint32_t)i * 8u;
-      // two independent Philox chains in flight per thread; the loop stays rolled to bound code size and registers
+      if constexpr (G_::RPL * G_::WPP <= 2) {
+        // small lattices per lane: fully unrolled, bit positions are immediates
+#pragma unroll
+        for (int cc = 0; cc < G_::CALLS_PER_WORD; ++cc) {
+          const uint4 w = philox4x32_10(call0 + cc, slot, c2, c3, key);
+          switch (cc) {
+            case 0: push_block<0>(r4, r8, w, T4, T8); break;
+            case 1: push_block<4>(r4, r8, w, T4, T8); break;
+            case 2: push_block<8>(r4, r8, w, T4, T8); break;
+            case 3: push_block<12>(r4, r8, w, T4, T8); break;
+            case 4: push_block<16>(r4, r8, w, T4, T8); break;
+            case 5: push_block<20>(r4, r8, w, T4, T8); break;
+            case 6: push_block<24>(r4, r8, w, T4, T8); break;
+            default: push_block<28>(r4, r8, w, T4, T8); break;
+          }
+        }
+      } else {
+        // L = 128: 8 plane words per lane; keep the block loop rolled (two chains in flight) to bound code size
 #pragma unroll 2
-      for (int cc = 0; cc < G_::CALLS_PER_WORD; ++cc) {
-        const uint4 w = philox4x32_10(call0 + cc, slot, c2, c3, key);
-        const uint32_t n4 = (lt_mask(w.x, negT4) & 1u) | (lt_mask(w.y, negT4) & 2u) | (lt_mask(w.z, negT4) & 4u) |
-                            (lt_mask(w.w, negT4) & 8u);
-        const uint32_t n8 = (lt_mask(w.x, negT8) & 1u) | (lt_mask(w.y, negT8) & 2u) | (lt_mask(w.z, negT8) & 4u) |
-                            (lt_mask(w.w, negT8) & 8u);
-        r4 |= n4 << (4 * cc);
-        r8 |= n8 << (4 * cc);
+        for (int cc = 0; cc < G_::CALLS_PER_WORD; ++cc) {
+          const uint4 w = philox4x32_10(call0 + cc, slot, c2, c3, key);
+          uint32_t n4 = 0u, n8 = 0u;
+          push_block<0>(n4, n8, w, T4, T8);
+          r4 |= n4 << (4 * cc);
+          r8 |= n8 << (4 * cc);
+        }
       }
       // flip iff a>=2, or a==1 and u<T4, or a==0 and u<T8
       const uint32_t flip = ge2 | (ge1 & r4) | (~ge1 & r8);
@@ -266,11 +290,10 @@ k_sweep(const DevState* __restrict__ st, const StepParams* __restrict__ sp, uint
   // ---- theta sweeps ----------------------------------------------------------------------------
   if (theta > 0) {
     const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
-    const unsigned long long negT4 = 0ull - (unsigned long long)sp->T4;
-    const unsigned long long negT8 = 0ull - (unsigned long long)sp->T8;
+    const uint32_t T4 = sp->T4, T8 = sp->T8;
     for (int t = 0; t < theta; ++t) {
-      half_sweep<L, 0>(lat, g, slot, (uint32_t)t, c3, key, negT4, negT8);
-      half_sweep<L, 1>(lat, g, slot, (uint32_t)t, c3, key, negT4, negT8);
+      half_sweep<L, 0>(lat, g, slot, (uint32_t)t, c3, key, T4, T8);
+      half_sweep<L, 1>(lat, g, slot, (uint32_t)t, c3, key, T4, T8);
     }
   }
 
