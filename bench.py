@@ -287,7 +287,7 @@ def run_ours(args):
     torch.cuda.empty_cache()
     if g.is_main and g.world == 1:
         if not args.no_resample:
-            resample = resample_leg(binding, torch, peaks)
+            resample = resample_leg(binding, torch, peaks, repeats=args.resample_repeats)
         if not args.no_cpu_baseline:
             r = oracle_sample_run(wl, 2048, 24, 1)
             cpu = {"value": r["attempts"] / r["seconds"], "unit": "attempts/s", "cores": r["cores"], "kind": "oracle",
@@ -318,11 +318,21 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-resample", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--leg", default="all", choices=["all", "resample"],
+                    help="'resample': only the config-5 resampling/redistribution leg (short; used for ncu captures)")
+    ap.add_argument("--resample-repeats", type=int, default=5)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3  # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         return run_reference(args)
+    if args.leg == "resample":
+        import torch
+        from paper_2006_00561_b200 import binding
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+        print(json.dumps({"resample": resample_leg(binding, torch, measured_peaks(), repeats=args.resample_repeats)}))
+        return 0
     return run_ours(args)
 
 

@@ -353,7 +353,7 @@ int64_t orc_partition_stats(int64_t R, const uint32_t* n, const uint32_t* off, i
  * Metropolis).  Thresholds T4/T8: floor(2^32 exp(-4 beta)), floor(2^32 exp(-8 beta)), clamped
  * to 2^32-1 (reading G10); accept iff dE <= 0 or u32 < T_dE (strict).
  * Random for an active site: ordinal q = y*(L/2) + k within the half-sweep, x = 2k + ((y+colour)&1),
- * word w[q&3] of counter (q>>2, slot, 2t+colour, tag2|step).
+ * word w[q&3] of counter (slot, q>>2, 2t+colour, tag2|step)   (C3, reading G19).
  * ---------------------------------------------------------------------------------------- */
 void orc_thresholds(double beta, uint32_t* T4, uint32_t* T8) {
   double a4 = floor(4294967296.0 * exp(-4.0 * beta));
@@ -373,7 +373,7 @@ static void sweeps_one_replica(int L, int8_t* s, uint64_t seed, uint32_t step, u
           int x = 2 * k + ((y + colour) & 1);
           uint32_t q = (uint32_t)(y * half + k);
           if ((q & 3u) == 0u) /* one Philox block serves four consecutive active sites */
-            philox_keyed(seed, q >> 2, slot, (uint32_t)(2 * t + colour), TAG_SWEEP, step, w);
+            philox_keyed(seed, slot, q >> 2, (uint32_t)(2 * t + colour), TAG_SWEEP, step, w);
           uint32_t u = w[q & 3u];
           int sig = s[y * L + x];
           int nb[4] = {s[y * L + (x + 1) % L], s[y * L + (x + L - 1) % L], s[((y + 1) % L) * L + x],

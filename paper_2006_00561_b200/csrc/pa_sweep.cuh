@@ -129,7 +129,7 @@ __device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot
         // small lattices per lane: fully unrolled, bit positions are immediates
 #pragma unroll
         for (int cc = 0; cc < G_::CALLS_PER_WORD; ++cc) {
-          const uint4 w = philox4x32_10(call0 + cc, slot, c2, c3, key);
+          const uint4 w = philox4x32_10(slot, call0 + cc, c2, c3, key);
           switch (cc) {
             case 0: push_block<0>(r4, r8, w, T4, T8); break;
             case 1: push_block<4>(r4, r8, w, T4, T8); break;
@@ -145,7 +145,7 @@ __device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot
         // L = 128: 8 plane words per lane; keep the block loop rolled (two chains in flight) to bound code size
 #pragma unroll 2
         for (int cc = 0; cc < G_::CALLS_PER_WORD; ++cc) {
-          const uint4 w = philox4x32_10(call0 + cc, slot, c2, c3, key);
+          const uint4 w = philox4x32_10(slot, call0 + cc, c2, c3, key);
           uint32_t n4 = 0u, n8 = 0u;
           push_block<0>(n4, n8, w, T4, T8);
           r4 |= n4 << (4 * cc);

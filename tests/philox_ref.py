@@ -25,7 +25,7 @@ def keyed(seed, c0, c1, c2, tag, step):
 
 def sweep_word(seed, step, slot, t, colour, q):
     """random word of the active site with ordinal q in half-sweep (t, colour) of population slot `slot`"""
-    return keyed(seed, q >> 2, slot, 2 * t + colour, 2, step)[q & 3]
+    return keyed(seed, slot, q >> 2, 2 * t + colour, 2, step)[q & 3]
 
 
 def init_word(seed, j, v):
