@@ -39,6 +39,12 @@ int copy_tile_for(int L) {
   }
 }
 
+int copy_shift_for(int L) {  // CopyGeo<L>::CT is a power of two
+  int sh = 0;
+  while ((1 << sh) < copy_tile_for(L)) ++sh;
+  return sh;
+}
+
 bool valid_L(int L) { return L == 8 || L == 16 || L == 32 || L == 64 || L == 128; }
 
 int64_t default_capacity(int64_t R0) {
@@ -236,7 +242,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, int theta) {
     k_poisson_scan<<<grid, SCAN_THREADS, 0, c->stream>>>(
         st, E0, E1, tb, N, c->dev<uint32_t>(c->lo.off), c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr,
         c->lo.tau ? c->dev<double>(c->lo.tau) : nullptr, c->dev<unsigned long long>(c->lo.tile_desc),
-        c->dev<uint32_t>(c->lo.tile_parent), copy_tile_for(c->cfg.L), (unsigned long long)c->cap, c->key);
+        c->dev<uint32_t>(c->lo.tile_parent), copy_shift_for(c->cfg.L), (unsigned long long)c->cap, c->key);
   }
   {
     Prof p(c, PA_K_BALANCE);

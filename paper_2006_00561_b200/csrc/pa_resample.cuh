@@ -10,7 +10,7 @@
 namespace pa {
 
 constexpr int PO_KMAX = 64;            // A4: cap of the CDF inversion loop
-constexpr int PO_ROW = PO_KMAX + 1;    // F_0 .. F_64 per level
+constexpr int PO_ROW = 72;             // F_0 .. F_64 per level, padded to 72 doubles (64-byte aligned rows)
 constexpr unsigned M_OVERFLOW = 0xffffffffu;
 
 struct LevelTables {
@@ -156,43 +156,62 @@ __global__ void k_levels_tau(const DevState* st, LevelTables tb, int N) {
 
 // ---------------------------------------------------------------------------------------------------
 // k_poisson_scan: a2-a4.  n_j ~ Poisson(lambda_j) by chunked CDF inversion with keyed uniforms, fused with a
-// single-pass exclusive scan (decoupled look-back).  Tile = 8 warps x 8 rounds x 32 lanes = 2048 parents;
-// parents with many chunks (lambda > 32) are drawn cooperatively by the whole warp.
+// single-pass exclusive scan (decoupled look-back).  Tile = 256 threads x 8 parents = 2048 parents.
+//   phase 1  every parent with m >= 1 draws its chunk 0 (one Philox block per parent, 8 parents per thread);
+//   phase 2  the remaining chunks (c = 1 .. m-1) of the tile's heavy parents (lambda > 8; 2 % of the parents but
+//            60 % of the children in config 5) form ONE flat work list that all 256 threads share, so that a parent
+//            with lambda = 10^4 (1250 chunks) costs the tile 5 passes instead of serialising one warp; counts are
+//            integer sums, so the result does not depend on who draws which chunk;
+//   phase 3  block scan of the counts, look-back across tiles, offsets / counts / copy-tile parents written.
 // ---------------------------------------------------------------------------------------------------
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ROUNDS = 8;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ROUNDS;
-constexpr unsigned HEAVY_M = 4;  // chunks drawn by one lane before the warp takes over
 
 constexpr unsigned long long DESC_AGG = 1ull << 62, DESC_PREFIX = 2ull << 62, DESC_VAL = (1ull << 62) - 1;
 
-// one chunk: u from Philox words, k = first index with u <= F_k (capped at KMAX)
+// one chunk: u from the keyed Philox words, k = #{i < 64 : u > F_i}.  F is non-decreasing (p_k >= 0), so this count
+// equals the A4 loop "while (u > F && k < 64) ++k"; rows are 64-byte aligned, four entries per step.
 __device__ __forceinline__ unsigned draw_chunk(const double* __restrict__ F, uint32_t j, unsigned long long c,
                                                uint32_t c3, const PhiloxKey& key) {
   const uint4 w = philox4x32_10((uint32_t)(c >> 1), j, 0u, c3, key);
   const uint32_t hi = (c & 1ull) ? w.z : w.x, lo = (c & 1ull) ? w.w : w.y;
   const unsigned long long x = ((unsigned long long)hi << 32) | lo;
-  const double u = ((double)(x >> 12) + 0.5) * 0x1p-52;  // exact
+  // u = ((x >> 12) + 0.5) * 2^-52, built without an int->double conversion: 1 + k 2^-52 has the bits
+  // 0x3FF0... | k, and subtracting 1 - 2^-53 gives (2k + 1) 2^-53 exactly (the result is representable)
+  const double u = __longlong_as_double((long long)(0x3FF0000000000000ull | (x >> 12))) - 0x1.fffffffffffffp-1;
+  const double2* __restrict__ F2 = reinterpret_cast<const double2*>(F);
   unsigned k = 0;
-  while (k < (unsigned)PO_KMAX && u > __ldg(F + k)) ++k;
+#pragma unroll 1
+  for (int g = 0; g < PO_KMAX / 4; ++g) {
+    const double2 a = __ldg(F2 + 2 * g), b = __ldg(F2 + 2 * g + 1);
+    const unsigned c4 = (unsigned)(u > a.x) + (unsigned)(u > a.y) + (unsigned)(u > b.x) + (unsigned)(u > b.y);
+    k += c4;
+    if (c4 < 4u) break;
+  }
   return k;
 }
 
 __global__ void __launch_bounds__(SCAN_THREADS)
 k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
                uint32_t* __restrict__ off, uint32_t* __restrict__ n_out, double* __restrict__ tau_out,
-               unsigned long long* tile_desc, uint32_t* __restrict__ tile_parent, int copy_tile,
+               unsigned long long* tile_desc, uint32_t* __restrict__ tile_parent, int copy_shift,
                unsigned long long capacity, const PhiloxKey key) {
   if (st->status != ST_OK) return;
   __shared__ unsigned s_tile;
+  __shared__ unsigned s_overflow;
+  __shared__ unsigned long long s_pack;  // (total extra chunks << 12) | number of heavy parents   (one atomic sequence)
   __shared__ unsigned long long s_warp_tot[SCAN_THREADS / 32];
   __shared__ unsigned long long s_prefix;
-  __shared__ unsigned s_overflow;
-  const unsigned long long R = st->R;
-  const unsigned ntiles = (unsigned)((R + SCAN_TILE - 1) / SCAN_TILE);
+  __shared__ unsigned s_cnt[SCAN_TILE];
+  __shared__ unsigned long long s_hstart[SCAN_TILE];  // first work-list position of heavy parent h
+  __shared__ unsigned short s_hitem[SCAN_TILE];       // its item index inside the tile
+  const uint32_t R = (uint32_t)st->R;  // R <= capacity < 2^32 - 4096: parent indices fit 32 bits
+  const unsigned ntiles = (R + SCAN_TILE - 1) / SCAN_TILE;
   if (threadIdx.x == 0) {
     s_tile = atomicAdd(&st->scan_tile, 1u);
     s_overflow = 0u;
+    s_pack = 0ull;
   }
   __syncthreads();
   const unsigned tile = s_tile;
@@ -200,53 +219,70 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
   const int32_t* __restrict__ E = st->cur ? E1 : E0;
   const uint32_t c3 = ctr3(TAG_RESAMPLE, st->step + 1u);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const unsigned long long warp_base = (unsigned long long)tile * SCAN_TILE + (unsigned long long)warp * (SCAN_ROUNDS * 32);
+  const uint32_t tile_base = tile * SCAN_TILE;
+  const unsigned witem0 = (unsigned)warp * (SCAN_ROUNDS * 32);  // the warp's 256 items are contiguous, lane-striped
 
-  // phase 1: sampling (divergent; kept rolled), counts parked in shared memory
-  __shared__ unsigned s_cnt[SCAN_TILE];
-  unsigned* my_cnt = s_cnt + warp * (SCAN_ROUNDS * 32);
-  bool overflow = false;
-#pragma unroll 1
-  for (int r = 0; r < SCAN_ROUNDS; ++r) {
-    const unsigned long long j = warp_base + r * 32 + lane;
-    unsigned n = 0, m = 0, lev = 0;
-    if (j < R) {
-      lev = (unsigned)((E[j] + 2 * N) >> 2);
-      m = tb.m[lev];
-      if (tau_out) tau_out[j] = tb.tau[lev];
-      if (m == M_OVERFLOW) { overflow = true; m = 0; }
-    }
-    if (m > 0 && m <= HEAVY_M) {
-      const double* F = tb.cdf + (size_t)lev * PO_ROW;
-      for (unsigned c = 0; c < m; ++c) n += draw_chunk(F, (uint32_t)j, c, c3, key);
-    }
-    // heavy parents: the whole warp draws the chunks of one parent at a time
-    unsigned heavy = __ballot_sync(0xffffffffu, m > HEAVY_M);
-    while (heavy) {
-      const int src = __ffs(heavy) - 1;
-      heavy &= heavy - 1;
-      const unsigned hm = __shfl_sync(0xffffffffu, m, src);
-      const unsigned hlev = __shfl_sync(0xffffffffu, lev, src);
-      const uint32_t hj = (uint32_t)(warp_base + r * 32 + src);
-      const double* F = tb.cdf + (size_t)hlev * PO_ROW;
-      unsigned part = 0;
-      for (unsigned c = lane; c < hm; c += 32) part += draw_chunk(F, hj, c, c3, key);
+  // phase 1: energies (all loads in flight), level tables, chunk 0
+  int e[SCAN_ROUNDS];
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-      if (lane == src) n = part;
-    }
-    my_cnt[r * 32 + lane] = n;
+  for (int r = 0; r < SCAN_ROUNDS; ++r) {
+    const uint32_t j = tile_base + witem0 + r * 32 + lane;
+    e[r] = (j < R) ? __ldg(E + j) : 0;
   }
-  if (overflow) s_overflow = 1u;
-  __syncwarp();
+#pragma unroll
+  for (int r = 0; r < SCAN_ROUNDS; ++r) {
+    const unsigned item = witem0 + r * 32 + lane;
+    const uint32_t j = tile_base + item;
+    unsigned n = 0;
+    if (j < R) {
+      const unsigned lev = (unsigned)((e[r] + 2 * N) >> 2);
+      unsigned m = __ldg(tb.m + lev);
+      if (tau_out) tau_out[j] = __ldg(tb.tau + lev);
+      if (m == M_OVERFLOW) {
+        s_overflow = 1u;
+        m = 0;
+      }
+      if (m > 0) {
+        n = draw_chunk(tb.cdf + (size_t)lev * PO_ROW, j, 0ull, c3, key);
+        if (m > 1) {
+          const unsigned long long old = atomicAdd(&s_pack, ((unsigned long long)(m - 1) << 12) + 1ull);
+          const unsigned h = (unsigned)(old & 0xfffull);
+          s_hstart[h] = old >> 12;
+          s_hitem[h] = (unsigned short)item;
+        }
+      }
+    }
+    s_cnt[item] = n;
+  }
+  __syncthreads();
 
-  // phase 2: warp-level scan in striped order (item = r*32 + lane)
+  // phase 2: flat work list over the extra chunks of the tile's heavy parents
+  {
+    const unsigned long long pack = s_pack;
+    const unsigned long long W = pack >> 12;
+    const unsigned nheavy = (unsigned)(pack & 0xfffull);  // <= SCAN_TILE = 2048 < 4096
+    for (unsigned long long wk = threadIdx.x; wk < W; wk += SCAN_THREADS) {
+      unsigned lo = 0, hi = nheavy;  // last h with s_hstart[h] <= wk
+      while (hi - lo > 1u) {
+        const unsigned mid = (lo + hi) >> 1;
+        if (s_hstart[mid] <= wk) lo = mid; else hi = mid;
+      }
+      const unsigned item = s_hitem[lo];
+      const uint32_t j = tile_base + item;
+      const unsigned lev = (unsigned)((__ldg(E + j) + 2 * N) >> 2);
+      const unsigned k = draw_chunk(tb.cdf + (size_t)lev * PO_ROW, j, 1ull + (wk - s_hstart[lo]), c3, key);
+      if (k) atomicAdd(&s_cnt[item], k);
+    }
+  }
+  __syncthreads();
+
+  // phase 3: warp-level scan in striped order (item = r*32 + lane)
   unsigned cnt[SCAN_ROUNDS];
-  unsigned excl[SCAN_ROUNDS];  // tile-local exclusive offsets within the warp's 256 items
+  unsigned excl[SCAN_ROUNDS];  // exclusive offsets within the warp's 256 items
   unsigned long long run = 0;
 #pragma unroll
   for (int r = 0; r < SCAN_ROUNDS; ++r) {
-    const unsigned v = my_cnt[r * 32 + lane];
+    const unsigned v = s_cnt[witem0 + r * 32 + lane];
     cnt[r] = v;
     unsigned inc = v;
 #pragma unroll
@@ -305,14 +341,16 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
   // offsets, counts, and for every copy tile the parent that covers its first child
 #pragma unroll
   for (int r = 0; r < SCAN_ROUNDS; ++r) {
-    const unsigned long long j = warp_base + r * 32 + lane;
+    const uint32_t j = tile_base + witem0 + r * 32 + lane;
     if (j < R) {
       const unsigned long long o = base + excl[r];  // exact whenever R' fits the capacity
       off[j] = (uint32_t)o;
       if (n_out) n_out[j] = cnt[r];
-      if (cnt[r] > 0 && o + cnt[r] <= capacity) {
-        const unsigned long long t_first = (o + copy_tile - 1) / copy_tile, t_last = (o + cnt[r] - 1) / copy_tile;
-        for (unsigned long long t = t_first; t <= t_last; ++t) tile_parent[t] = (uint32_t)j;
+      if (cnt[r] > 0 && o + cnt[r] <= capacity) {  // then o, o + cnt fit 32 bits
+        const uint32_t o32 = (uint32_t)o, ct1 = (1u << copy_shift) - 1u;
+        const uint32_t t_first = (o32 + ct1) >> copy_shift, t_last = (o32 + cnt[r] - 1u) >> copy_shift;
+#pragma unroll 1
+        for (uint32_t t = t_first; t <= t_last; ++t) tile_parent[t] = j;
       }
     }
   }
@@ -382,6 +420,7 @@ struct CopyGeo {
   static constexpr int VB = S < 16 ? S : 16;                 // bytes per vector access
   static constexpr int VT = S / VB;                          // threads per child
   static constexpr int CT = S <= 128 ? 1024 : (S <= 512 ? 512 : 256);  // children per tile (multiple of COPY_THREADS)
+  static_assert((CT & (CT - 1)) == 0, "k_poisson_scan divides child offsets by CT with a shift");
 };
 
 template <int VB> struct VecT;
