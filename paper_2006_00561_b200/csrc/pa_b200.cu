@@ -237,17 +237,25 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, int theta) {
     k_levels_tau<<<(N + 1 + 127) / 128, 128, 0, c->stream>>>(st, tb, N);
   }
   {
-    Prof p(c, PA_K_POISSON_SCAN);
-    const unsigned grid = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
-    k_poisson_scan<<<grid, SCAN_THREADS, 0, c->stream>>>(
-        st, E0, E1, tb, N, c->dev<uint32_t>(c->lo.off), c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr,
-        c->lo.tau ? c->dev<double>(c->lo.tau) : nullptr, c->dev<unsigned long long>(c->lo.tile_desc),
-        c->dev<uint32_t>(c->lo.tile_parent), copy_shift_for(c->cfg.L), (unsigned long long)c->cap, c->key);
-  }
-  {
-    Prof p(c, PA_K_BALANCE);
-    k_balance<<<1, 256, 0, c->stream>>>(st, c->dev<uint32_t>(c->lo.off), c->dev<uint32_t>(c->lo.part[0]),
-                                        c->dev<uint32_t>(c->lo.part[1]), c->dev<uint32_t>(c->lo.part_stats), c->cfg.P);
+    Prof p(c, PA_K_POISSON_SCAN);  // includes a5 (partition balance), run by the last tile to finish
+    // persistent blocks pull tiles from a ticket counter (5 blocks of 48 registers x 256 threads fit one SM)
+    const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
+    const unsigned grid = tiles_cap < 148u * 5u ? tiles_cap : 148u * 5u;
+    ScanOut out;
+    out.off = c->dev<uint32_t>(c->lo.off);
+    out.n = c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr;
+    out.tau = c->lo.tau ? c->dev<double>(c->lo.tau) : nullptr;
+    out.tile_desc = c->dev<unsigned long long>(c->lo.tile_desc);
+    out.tile_parent = c->dev<uint32_t>(c->lo.tile_parent);
+    out.part0 = c->dev<uint32_t>(c->lo.part[0]);
+    out.part1 = c->dev<uint32_t>(c->lo.part[1]);
+    out.part_stats = c->dev<uint32_t>(c->lo.part_stats);
+    if (out.n || out.tau)
+      k_poisson_scan<true><<<grid, SCAN_THREADS, 0, c->stream>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
+                                                                   (unsigned long long)c->cap, c->cfg.P, c->key);
+    else
+      k_poisson_scan<false><<<grid, SCAN_THREADS, 0, c->stream>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
+                                                                    (unsigned long long)c->cap, c->cfg.P, c->key);
   }
   launch_copy(c);
   if (theta > 0) launch_sweep(c, sp, 0);

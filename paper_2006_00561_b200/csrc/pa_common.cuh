@@ -31,9 +31,11 @@ struct DevState {
   unsigned int fail_step;        // ordinal of the step that failed
   unsigned int reduce_done;      // block counters (reset every step by k_levels_w)
   unsigned int scan_tile;
+  unsigned int scan_done;        // tiles of k_poisson_scan that have written their outputs
+  unsigned int scan_overflow;    // a parent sat on a level with lambda >= 2^31
   unsigned int obs_done;
   unsigned int T4, T8;           // thresholds of the last committed step with theta > 0
-  unsigned int pad_;
+  unsigned int pad_[3];
 };
 
 struct StepParams {

@@ -31,6 +31,8 @@ __global__ void k_levels_w(DevState* st, const StepParams* sp, LevelTables tb, i
   if (idx == 0) {
     st->reduce_done = 0u;
     st->scan_tile = 0u;
+    st->scan_done = 0u;
+    st->scan_overflow = 0u;
     st->obs_done = 0u;
   }
   for (int i = idx; i < n_desc; i += gridDim.x * blockDim.x) tile_desc[i] = 0ull;
@@ -170,214 +172,310 @@ constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ROUNDS;
 
 constexpr unsigned long long DESC_AGG = 1ull << 62, DESC_PREFIX = 2ull << 62, DESC_VAL = (1ull << 62) - 1;
 
-// one chunk: u from the keyed Philox words, k = #{i < 64 : u > F_i}.  F is non-decreasing (p_k >= 0), so this count
-// equals the A4 loop "while (u > F && k < 64) ++k"; rows are 64-byte aligned, four entries per step.
-__device__ __forceinline__ unsigned draw_chunk(const double* __restrict__ F, uint32_t j, unsigned long long c,
-                                               uint32_t c3, const PhiloxKey& key) {
-  const uint4 w = philox4x32_10((uint32_t)(c >> 1), j, 0u, c3, key);
-  const uint32_t hi = (c & 1ull) ? w.z : w.x, lo = (c & 1ull) ? w.w : w.y;
+// u = ((x >> 12) + 0.5) * 2^-52 from the two keyed words of chunk c, built without an int->double conversion:
+// 1 + k 2^-52 has the bits 0x3FF0... | k, and subtracting 1 - 2^-53 gives (2k + 1) 2^-53 exactly.
+__device__ __forceinline__ double chunk_uniform(const uint4& w, unsigned odd) {
+  const uint32_t hi = odd ? w.z : w.x, lo = odd ? w.w : w.y;
   const unsigned long long x = ((unsigned long long)hi << 32) | lo;
-  // u = ((x >> 12) + 0.5) * 2^-52, built without an int->double conversion: 1 + k 2^-52 has the bits
-  // 0x3FF0... | k, and subtracting 1 - 2^-53 gives (2k + 1) 2^-53 exactly (the result is representable)
-  const double u = __longlong_as_double((long long)(0x3FF0000000000000ull | (x >> 12))) - 0x1.fffffffffffffp-1;
-  const double2* __restrict__ F2 = reinterpret_cast<const double2*>(F);
+  return __longlong_as_double((long long)(0x3FF0000000000000ull | (x >> 12))) - 0x1.fffffffffffffp-1;
+}
+// k = #{i < 64 : u > F_i}.  F is non-decreasing (p_k >= 0), so this count equals the A4 loop
+// "while (u > F && k < 64) ++k"; rows are 64-byte aligned, four entries per step.
+__device__ __forceinline__ unsigned cdf_count4(const double2* __restrict__ F2, int g, double u) {
+  const double2 a = __ldg(F2 + 2 * g), b = __ldg(F2 + 2 * g + 1);
+  return (unsigned)(u > a.x) + (unsigned)(u > a.y) + (unsigned)(u > b.x) + (unsigned)(u > b.y);
+}
+__device__ __forceinline__ unsigned cdf_search_from(const double2* __restrict__ F2, int g0, double u) {
   unsigned k = 0;
 #pragma unroll 1
-  for (int g = 0; g < PO_KMAX / 4; ++g) {
-    const double2 a = __ldg(F2 + 2 * g), b = __ldg(F2 + 2 * g + 1);
-    const unsigned c4 = (unsigned)(u > a.x) + (unsigned)(u > a.y) + (unsigned)(u > b.x) + (unsigned)(u > b.y);
+  for (int g = g0; g < PO_KMAX / 4; ++g) {
+    const unsigned c4 = cdf_count4(F2, g, u);
     k += c4;
     if (c4 < 4u) break;
   }
   return k;
 }
+__device__ __forceinline__ unsigned draw_chunk(const double* __restrict__ F, uint32_t j, unsigned long long c,
+                                               uint32_t c3, const PhiloxKey& key) {
+  const uint4 w = philox4x32_10((uint32_t)(c >> 1), j, 0u, c3, key);
+  return cdf_search_from(reinterpret_cast<const double2*>(F), 0, chunk_uniform(w, (unsigned)(c & 1ull)));
+}
 
+// a5 (defined below); run by the last tile of k_poisson_scan to finish
+__device__ void balance_tile(DevState* st, const uint32_t* off, uint32_t* part0, uint32_t* part1, uint32_t* stats, int P);
+
+struct ScanOut {
+  uint32_t* off;            // [R + 1] exclusive offsets, off[R] = R'
+  uint32_t* n;              // [R] copy counts (PA_KEEP_COUNTS) or null
+  double* tau;              // [R] weights (PA_KEEP_TAU) or null
+  unsigned long long* tile_desc;
+  uint32_t* tile_parent;    // per copy tile: the parent covering its first child
+  uint32_t *part0, *part1, *part_stats;
+};
+
+constexpr int SCAN_BATCH = 4;  // independent Philox chains in flight per thread
+constexpr unsigned NO_TILE = 0xffffffffu;
+
+// The kernel is software-pipelined over tiles: a block draws the counts of tile B and publishes its aggregate BEFORE it
+// resolves the prefix of its previous tile A and writes A's offsets, so the look-back latency (descriptors of up to
+// A tiles, 32 per round trip) is hidden behind B's sampling.  Every ticket holder publishes its aggregate before it
+// waits on anything, so the look-back cannot deadlock.
+template <bool KEEP>
 __global__ void __launch_bounds__(SCAN_THREADS)
 k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
-               uint32_t* __restrict__ off, uint32_t* __restrict__ n_out, double* __restrict__ tau_out,
-               unsigned long long* tile_desc, uint32_t* __restrict__ tile_parent, int copy_shift,
-               unsigned long long capacity, const PhiloxKey key) {
+               ScanOut out, int copy_shift, unsigned long long capacity, int P, const PhiloxKey key) {
   if (st->status != ST_OK) return;
   __shared__ unsigned s_tile;
-  __shared__ unsigned s_overflow;
+  __shared__ unsigned s_flag;            // bit 0: a parent sits on an overflowing level; bit 1: this block finishes last
   __shared__ unsigned long long s_pack;  // (total extra chunks << 12) | number of heavy parents   (one atomic sequence)
   __shared__ unsigned long long s_warp_tot[SCAN_THREADS / 32];
   __shared__ unsigned long long s_prefix;
-  __shared__ unsigned s_cnt[SCAN_TILE];
+  __shared__ __align__(16) unsigned s_cnt[2][SCAN_TILE];
   __shared__ unsigned long long s_hstart[SCAN_TILE];  // first work-list position of heavy parent h
   __shared__ unsigned short s_hitem[SCAN_TILE];       // its item index inside the tile
   const uint32_t R = (uint32_t)st->R;  // R <= capacity < 2^32 - 4096: parent indices fit 32 bits
   const unsigned ntiles = (R + SCAN_TILE - 1) / SCAN_TILE;
-  if (threadIdx.x == 0) {
-    s_tile = atomicAdd(&st->scan_tile, 1u);
-    s_overflow = 0u;
-    s_pack = 0ull;
-  }
-  __syncthreads();
-  const unsigned tile = s_tile;
-  if (tile >= ntiles) return;
   const int32_t* __restrict__ E = st->cur ? E1 : E0;
   const uint32_t c3 = ctr3(TAG_RESAMPLE, st->step + 1u);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint32_t tile_base = tile * SCAN_TILE;
-  const unsigned witem0 = (unsigned)warp * (SCAN_ROUNDS * 32);  // the warp's 256 items are contiguous, lane-striped
+  if (threadIdx.x == 0) s_flag = 0u;
+  unsigned prev = NO_TILE;
+  int buf = 0;
 
-  // phase 1: energies (all loads in flight), level tables, chunk 0
-  int e[SCAN_ROUNDS];
-#pragma unroll
-  for (int r = 0; r < SCAN_ROUNDS; ++r) {
-    const uint32_t j = tile_base + witem0 + r * 32 + lane;
-    e[r] = (j < R) ? __ldg(E + j) : 0;
-  }
-#pragma unroll
-  for (int r = 0; r < SCAN_ROUNDS; ++r) {
-    const unsigned item = witem0 + r * 32 + lane;
-    const uint32_t j = tile_base + item;
-    unsigned n = 0;
-    if (j < R) {
-      const unsigned lev = (unsigned)((e[r] + 2 * N) >> 2);
-      unsigned m = __ldg(tb.m + lev);
-      if (tau_out) tau_out[j] = __ldg(tb.tau + lev);
-      if (m == M_OVERFLOW) {
-        s_overflow = 1u;
-        m = 0;
-      }
-      if (m > 0) {
-        n = draw_chunk(tb.cdf + (size_t)lev * PO_ROW, j, 0ull, c3, key);
-        if (m > 1) {
-          const unsigned long long old = atomicAdd(&s_pack, ((unsigned long long)(m - 1) << 12) + 1ull);
-          const unsigned h = (unsigned)(old & 0xfffull);
-          s_hstart[h] = old >> 12;
-          s_hitem[h] = (unsigned short)item;
-        }
-      }
+  for (;;) {
+    if (threadIdx.x == 0) {
+      s_tile = atomicAdd(&st->scan_tile, 1u);
+      s_pack = 0ull;
     }
-    s_cnt[item] = n;
-  }
-  __syncthreads();
+    __syncthreads();
+    const unsigned tile = s_tile < ntiles ? s_tile : NO_TILE;
+    if (tile == NO_TILE && prev == NO_TILE) break;
 
-  // phase 2: flat work list over the extra chunks of the tile's heavy parents
-  {
-    const unsigned long long pack = s_pack;
-    const unsigned long long W = pack >> 12;
-    const unsigned nheavy = (unsigned)(pack & 0xfffull);  // <= SCAN_TILE = 2048 < 4096
-    for (unsigned long long wk = threadIdx.x; wk < W; wk += SCAN_THREADS) {
-      unsigned lo = 0, hi = nheavy;  // last h with s_hstart[h] <= wk
-      while (hi - lo > 1u) {
-        const unsigned mid = (lo + hi) >> 1;
-        if (s_hstart[mid] <= wk) lo = mid; else hi = mid;
-      }
-      const unsigned item = s_hitem[lo];
-      const uint32_t j = tile_base + item;
-      const unsigned lev = (unsigned)((__ldg(E + j) + 2 * N) >> 2);
-      const unsigned k = draw_chunk(tb.cdf + (size_t)lev * PO_ROW, j, 1ull + (wk - s_hstart[lo]), c3, key);
-      if (k) atomicAdd(&s_cnt[item], k);
-    }
-  }
-  __syncthreads();
-
-  // phase 3: warp-level scan in striped order (item = r*32 + lane)
-  unsigned cnt[SCAN_ROUNDS];
-  unsigned excl[SCAN_ROUNDS];  // exclusive offsets within the warp's 256 items
-  unsigned long long run = 0;
-#pragma unroll
-  for (int r = 0; r < SCAN_ROUNDS; ++r) {
-    const unsigned v = s_cnt[witem0 + r * 32 + lane];
-    cnt[r] = v;
-    unsigned inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += t;
-    }
-    excl[r] = (unsigned)run + (inc - v);
-    run += __shfl_sync(0xffffffffu, inc, 31);
-  }
-  if (lane == 0) s_warp_tot[warp] = run;
-  __syncthreads();
-  unsigned long long warp_excl = 0, tile_total = 0;
-#pragma unroll
-  for (int w = 0; w < SCAN_THREADS / 32; ++w) {
-    const unsigned long long t = s_warp_tot[w];
-    if (w < warp) warp_excl += t;
-    tile_total += t;
-  }
-
-  // decoupled look-back (warp 0)
-  if (warp == 0) {
-    unsigned long long prefix = 0;
-    if (tile == 0) {
-      if (lane == 0) atomicExch(&tile_desc[0], DESC_PREFIX | tile_total);
-    } else {
-      if (lane == 0) atomicExch(&tile_desc[tile], DESC_AGG | tile_total);
-      int look = (int)tile - 1;
-      while (true) {
-        const int idx = look - lane;
-        unsigned long long d = DESC_PREFIX;  // lanes before tile 0 read as an empty prefix
-        if (idx >= 0) {
-          do {
-            d = *((volatile unsigned long long*)&tile_desc[idx]);
-          } while ((d >> 62) == 0ull);
-        }
-        const unsigned is_prefix = __ballot_sync(0xffffffffu, (d >> 62) == 2ull);
-        unsigned long long v = d & DESC_VAL;
-        if (is_prefix) {
-          const int first = __ffs(is_prefix) - 1;  // nearest tile that already knows its inclusive prefix
-          if (lane > first) v = 0ull;
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        prefix += v;
-        if (is_prefix) break;
-        look -= 32;
-      }
-      if (lane == 0) atomicExch(&tile_desc[tile], DESC_PREFIX | ((prefix + tile_total) & DESC_VAL));
-    }
-    if (lane == 0) s_prefix = prefix;
-  }
-  __syncthreads();
-  const unsigned long long base = s_prefix + warp_excl;
-
-  // offsets, counts, and for every copy tile the parent that covers its first child
-#pragma unroll
-  for (int r = 0; r < SCAN_ROUNDS; ++r) {
-    const uint32_t j = tile_base + witem0 + r * 32 + lane;
-    if (j < R) {
-      const unsigned long long o = base + excl[r];  // exact whenever R' fits the capacity
-      off[j] = (uint32_t)o;
-      if (n_out) n_out[j] = cnt[r];
-      if (cnt[r] > 0 && o + cnt[r] <= capacity) {  // then o, o + cnt fit 32 bits
-        const uint32_t o32 = (uint32_t)o, ct1 = (1u << copy_shift) - 1u;
-        const uint32_t t_first = (o32 + ct1) >> copy_shift, t_last = (o32 + cnt[r] - 1u) >> copy_shift;
+    if (tile != NO_TILE) {
+      const uint32_t tile_base = tile * SCAN_TILE;
+      unsigned* cntb = s_cnt[buf];
+      // phase 1: chunk 0 of every parent; item = r * 256 + tid (coalesced), SCAN_BATCH branch-free chains at a time
 #pragma unroll 1
-        for (uint32_t t = t_first; t <= t_last; ++t) tile_parent[t] = j;
+      for (int r0 = 0; r0 < SCAN_ROUNDS; r0 += SCAN_BATCH) {
+        uint32_t jj[SCAN_BATCH];
+        int e[SCAN_BATCH];
+        unsigned m[SCAN_BATCH], k[SCAN_BATCH], c4[SCAN_BATCH];
+        double u[SCAN_BATCH];
+        const double2* F2[SCAN_BATCH];
+#pragma unroll
+        for (int b = 0; b < SCAN_BATCH; ++b) {
+          jj[b] = tile_base + (r0 + b) * SCAN_THREADS + threadIdx.x;
+          e[b] = (jj[b] < R) ? __ldg(E + jj[b]) : -2 * N;
+        }
+#pragma unroll
+        for (int b = 0; b < SCAN_BATCH; ++b) {
+          const unsigned lev = (unsigned)((e[b] + 2 * N) >> 2);
+          m[b] = (jj[b] < R) ? __ldg(tb.m + lev) : 0u;
+          F2[b] = reinterpret_cast<const double2*>(tb.cdf + (size_t)lev * PO_ROW);
+          if (KEEP) {
+            if (out.tau && jj[b] < R) out.tau[jj[b]] = __ldg(tb.tau + lev);
+          }
+        }
+#pragma unroll
+        for (int b = 0; b < SCAN_BATCH; ++b) u[b] = chunk_uniform(philox4x32_10(0u, jj[b], 0u, c3, key), 0u);
+#pragma unroll
+        for (int b = 0; b < SCAN_BATCH; ++b) c4[b] = cdf_count4(F2[b], 0, u[b]);  // rows of unused levels are masked below
+#pragma unroll
+        for (int b = 0; b < SCAN_BATCH; ++b) {
+          k[b] = c4[b];
+          if (c4[b] == 4u) k[b] += cdf_search_from(F2[b], 1, u[b]);
+          if (m[b] == M_OVERFLOW) {
+            s_flag = 1u;
+            m[b] = 0u;
+          }
+          if (m[b] == 0u) k[b] = 0u;
+          if (m[b] > 1u) {
+            const unsigned long long old = atomicAdd(&s_pack, ((unsigned long long)(m[b] - 1u) << 12) + 1ull);
+            const unsigned h = (unsigned)(old & 0xfffull);
+            s_hstart[h] = old >> 12;
+            s_hitem[h] = (unsigned short)((r0 + b) * SCAN_THREADS + threadIdx.x);
+          }
+          cntb[(r0 + b) * SCAN_THREADS + threadIdx.x] = k[b];
+        }
+      }
+      __syncthreads();
+      // phase 2: flat work list over the extra chunks of the tile's heavy parents
+      {
+        const unsigned long long pack = s_pack;
+        const unsigned long long W = pack >> 12;
+        const unsigned nheavy = (unsigned)(pack & 0xfffull);  // <= SCAN_TILE = 2048 < 4096
+        for (unsigned long long wk = threadIdx.x; wk < W; wk += SCAN_THREADS) {
+          unsigned lo = 0, hi = nheavy;  // last h with s_hstart[h] <= wk
+          while (hi - lo > 1u) {
+            const unsigned mid = (lo + hi) >> 1;
+            if (s_hstart[mid] <= wk) lo = mid; else hi = mid;
+          }
+          const unsigned item = s_hitem[lo];
+          const uint32_t j = tile_base + item;
+          const unsigned lev = (unsigned)((__ldg(E + j) + 2 * N) >> 2);
+          const unsigned kk = draw_chunk(tb.cdf + (size_t)lev * PO_ROW, j, 1ull + (wk - s_hstart[lo]), c3, key);
+          if (kk) atomicAdd(&cntb[item], kk);
+        }
+      }
+      __syncthreads();
+      // aggregate of the tile, published at once
+      {
+        const uint4 a = *reinterpret_cast<const uint4*>(&cntb[SCAN_ROUNDS * threadIdx.x]);
+        const uint4 b = *reinterpret_cast<const uint4*>(&cntb[SCAN_ROUNDS * threadIdx.x + 4]);
+        unsigned long long t = (unsigned long long)a.x + a.y + a.z + a.w + b.x + b.y + b.z + b.w;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0) s_warp_tot[warp] = t;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+          unsigned long long tot = 0;
+#pragma unroll
+          for (int w = 0; w < SCAN_THREADS / 32; ++w) tot += s_warp_tot[w];
+          atomicExch(&out.tile_desc[tile], (tile == 0 ? DESC_PREFIX : DESC_AGG) | tot);
+        }
       }
     }
-  }
-  if (tile == ntiles - 1 && threadIdx.x == 0) {
-    const unsigned long long Rnew = s_prefix + tile_total;
-    off[R] = (uint32_t)Rnew;
-    st->Rnew = Rnew;
-    if (Rnew > capacity) st->status = ST_CAPACITY;
-    else if (Rnew == 0ull) st->status = ST_EXTINCT;
-    if (st->status != ST_OK) st->fail_step = st->step + 1u;
-  }
-  __syncthreads();
-  if (s_overflow && threadIdx.x == 0) {
-    atomicExch(&st->status, (unsigned)ST_CAPACITY);
-    st->fail_step = st->step + 1u;
+
+    if (prev != NO_TILE) {
+      // phase 3 of the PREVIOUS tile: block scan (thread t owns the 8 consecutive items 8t .. 8t+7), look-back, outputs
+      const unsigned* cntb = s_cnt[buf ^ 1];
+      const uint32_t tile_base = prev * SCAN_TILE;
+      unsigned cnt[SCAN_ROUNDS];
+      {
+        const uint4 a = *reinterpret_cast<const uint4*>(&cntb[SCAN_ROUNDS * threadIdx.x]);
+        const uint4 b = *reinterpret_cast<const uint4*>(&cntb[SCAN_ROUNDS * threadIdx.x + 4]);
+        cnt[0] = a.x; cnt[1] = a.y; cnt[2] = a.z; cnt[3] = a.w;
+        cnt[4] = b.x; cnt[5] = b.y; cnt[6] = b.z; cnt[7] = b.w;
+      }
+      unsigned long long tsum = 0;
+#pragma unroll
+      for (int i = 0; i < SCAN_ROUNDS; ++i) tsum += cnt[i];
+      unsigned long long inc = tsum;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+      }
+      __syncthreads();  // s_warp_tot of the aggregate step above has been consumed
+      if (lane == 31) s_warp_tot[warp] = inc;
+      // decoupled look-back (warp 0); the aggregate of `prev` was published one iteration ago
+      if (warp == 0) {
+        unsigned long long prefix = 0;
+        if (prev != 0u) {
+          int look = (int)prev - 1;
+          while (true) {
+            const int idx = look - lane;
+            unsigned long long d = DESC_PREFIX;  // lanes before tile 0 read as an empty prefix
+            if (idx >= 0) {
+              while (((d = *((volatile unsigned long long*)&out.tile_desc[idx])) >> 62) == 0ull) {}
+            }
+            const unsigned is_prefix = __ballot_sync(0xffffffffu, (d >> 62) == 2ull);
+            unsigned long long v = d & DESC_VAL;
+            if (is_prefix) {
+              const int first = __ffs(is_prefix) - 1;  // nearest tile that already knows its inclusive prefix
+              if (lane > first) v = 0ull;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            prefix += v;
+            if (is_prefix) break;
+            look -= 32;
+          }
+          if (lane == 0) {
+            const unsigned long long own = *((volatile unsigned long long*)&out.tile_desc[prev]) & DESC_VAL;
+            atomicExch(&out.tile_desc[prev], DESC_PREFIX | ((prefix + own) & DESC_VAL));
+          }
+        }
+        if (lane == 0) s_prefix = prefix;
+      }
+      __syncthreads();
+      unsigned long long warp_excl = 0, tile_total = 0;
+#pragma unroll
+      for (int w = 0; w < SCAN_THREADS / 32; ++w) {
+        const unsigned long long t = s_warp_tot[w];
+        if (w < warp) warp_excl += t;
+        tile_total += t;
+      }
+      unsigned long long o64 = s_prefix + warp_excl + (inc - tsum);  // offset of the thread's first item
+
+      // offsets, counts, and for every copy tile the parent that covers its first child
+      const uint32_t j0 = tile_base + SCAN_ROUNDS * threadIdx.x;
+      uint32_t offs[SCAN_ROUNDS];
+#pragma unroll
+      for (int i = 0; i < SCAN_ROUNDS; ++i) {
+        offs[i] = (uint32_t)o64;  // exact whenever R' fits the capacity
+        if (cnt[i] > 0u && j0 + i < R && o64 + cnt[i] <= capacity) {  // then o, o + cnt fit 32 bits
+          const uint32_t o32 = (uint32_t)o64, ct1 = (1u << copy_shift) - 1u;
+          const uint32_t t_first = (o32 + ct1) >> copy_shift, t_last = (o32 + cnt[i] - 1u) >> copy_shift;
+#pragma unroll 1
+          for (uint32_t t = t_first; t <= t_last; ++t) out.tile_parent[t] = j0 + i;
+        }
+        o64 += cnt[i];
+      }
+      if (j0 + SCAN_ROUNDS <= R) {
+        *reinterpret_cast<uint4*>(out.off + j0) = make_uint4(offs[0], offs[1], offs[2], offs[3]);
+        *reinterpret_cast<uint4*>(out.off + j0 + 4) = make_uint4(offs[4], offs[5], offs[6], offs[7]);
+        if (KEEP) {
+          if (out.n) {
+            *reinterpret_cast<uint4*>(out.n + j0) = make_uint4(cnt[0], cnt[1], cnt[2], cnt[3]);
+            *reinterpret_cast<uint4*>(out.n + j0 + 4) = make_uint4(cnt[4], cnt[5], cnt[6], cnt[7]);
+          }
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < SCAN_ROUNDS; ++i) {
+          if (j0 + i < R) {
+            out.off[j0 + i] = offs[i];
+            if (KEEP) {
+              if (out.n) out.n[j0 + i] = cnt[i];
+            }
+          }
+        }
+      }
+      if (prev == ntiles - 1 && threadIdx.x == 0) {
+        const unsigned long long Rnew = s_prefix + tile_total;
+        out.off[R] = (uint32_t)Rnew;
+        st->Rnew = Rnew;
+        if (Rnew > capacity) st->status = ST_CAPACITY;
+        else if (Rnew == 0ull) st->status = ST_EXTINCT;
+        if (st->status != ST_OK) st->fail_step = st->step + 1u;
+      }
+      __syncthreads();
+      // the block that writes the last outstanding tile sees every offset and R': it runs a5
+      if (threadIdx.x == 0) {
+        if (s_flag & 1u) atomicOr(&st->scan_overflow, 1u);
+        __threadfence();
+        const unsigned done = atomicAdd(&st->scan_done, 1u);
+        if (done == ntiles - 1) s_flag |= 2u;
+      }
+      __syncthreads();
+      if (s_flag & 2u) {
+        __threadfence();
+        if (threadIdx.x == 0 && *((volatile unsigned*)&st->scan_overflow) != 0u &&
+            *((volatile unsigned*)&st->status) == ST_OK) {
+          st->status = ST_CAPACITY;
+          st->fail_step = st->step + 1u;
+        }
+        __syncthreads();
+        balance_tile(st, out.off, out.part0, out.part1, out.part_stats, P);
+      }
+    }
+    if (tile == NO_TILE) break;
+    prev = tile;
+    buf ^= 1;
   }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// k_balance: a5.  One block.  New partition table, born/excess/shortage per partition, moved count.
+// balance_tile: a5.  One block (the last tile of k_poisson_scan to finish; every offset is then visible).  New
+// partition table, born/excess/shortage per partition, moved count.  PAPER.md:104-106; A6.
 // ---------------------------------------------------------------------------------------------------
-__global__ void k_balance(DevState* st, const uint32_t* __restrict__ off, uint32_t* part0, uint32_t* part1,
-                          uint32_t* __restrict__ stats, int P) {
-  if (st->status != ST_OK) return;
+__device__ void balance_tile(DevState* st, const uint32_t* off, uint32_t* part0, uint32_t* part1, uint32_t* stats,
+                             int P) {
+  if (*((volatile unsigned*)&st->status) != ST_OK) return;
   const uint32_t* old_start = st->cur ? part1 : part0;
   uint32_t* new_start = st->cur ? part0 : part1;
-  const unsigned long long Rnew = st->Rnew;
+  const unsigned long long Rnew = *((volatile unsigned long long*)&st->Rnew);
   const unsigned long long base = Rnew / P, rem = Rnew % P;
   __shared__ unsigned long long s_same;
   if (threadIdx.x == 0) s_same = 0ull;
@@ -389,7 +487,7 @@ __global__ void k_balance(DevState* st, const uint32_t* __restrict__ off, uint32
     if (p < P) {
       const unsigned long long e = (unsigned long long)(p + 1) * base + ((unsigned long long)(p + 1) < rem ? p + 1 : rem);
       const uint32_t cnt = (uint32_t)(e - s);
-      const uint32_t b0 = off[old_start[p]], b1 = off[old_start[p + 1]];
+      const uint32_t b0 = __ldcg(off + old_start[p]), b1 = __ldcg(off + old_start[p + 1]);
       const uint32_t born = b1 - b0;
       stats[4 * p + 0] = cnt;
       stats[4 * p + 1] = born;
