@@ -352,8 +352,11 @@ int64_t orc_partition_stats(int64_t R, const uint32_t* n, const uint32_t* off, i
  * C4.  MCMC equilibration ("any traditional MCMC"; reading G7: checkerboard
  * Metropolis).  Thresholds T4/T8: floor(2^32 exp(-4 beta)), floor(2^32 exp(-8 beta)), clamped
  * to 2^32-1 (reading G10); accept iff dE <= 0 or u32 < T_dE (strict).
- * Random for an active site: ordinal q = y*(L/2) + k within the half-sweep, x = 2k + ((y+colour)&1),
- * word w[q&3] of counter (slot, q>>2, 2t+colour, tag2|step)   (C3, reading G19).
+ * Random for an active site (C3, reading G20): ordinal q = y*(L/2) + k within the half-sweep,
+ * x = 2k + ((y+colour)&1).  32 consecutive ordinals form a group gamma = q>>5, position p = q&31.  The group
+ * owns 32 keyed words W_b, b = 0..31: W_b = word (b&3) of Philox counter (slot, 8*gamma + (b>>2), 2t+colour,
+ * tag2|step).  The site's 32-bit uniform is the bit column p of those words, word 0 giving the most
+ * significant bit:  u = sum_b bit_p(W_b) * 2^(31-b).
  * ---------------------------------------------------------------------------------------- */
 void orc_thresholds(double beta, uint32_t* T4, uint32_t* T8) {
   double a4 = floor(4294967296.0 * exp(-4.0 * beta));
@@ -367,14 +370,17 @@ static void sweeps_one_replica(int L, int8_t* s, uint64_t seed, uint32_t step, u
   int half = L / 2;
   for (int t = 0; t < theta; ++t) {
     for (int colour = 0; colour < 2; ++colour) {
-      uint32_t w[4] = {0, 0, 0, 0};
+      uint32_t W[32]; /* the keyed words of the current group of 32 active sites */
       for (int y = 0; y < L; ++y) {
         for (int k = 0; k < half; ++k) {
           int x = 2 * k + ((y + colour) & 1);
           uint32_t q = (uint32_t)(y * half + k);
-          if ((q & 3u) == 0u) /* one Philox block serves four consecutive active sites */
-            philox_keyed(seed, slot, q >> 2, (uint32_t)(2 * t + colour), TAG_SWEEP, step, w);
-          uint32_t u = w[q & 3u];
+          uint32_t gamma = q >> 5, p = q & 31u;
+          if (p == 0u) /* a new group starts: eight Philox blocks = 32 words */
+            for (uint32_t c = 0; c < 8u; ++c)
+              philox_keyed(seed, slot, 8u * gamma + c, (uint32_t)(2 * t + colour), TAG_SWEEP, step, W + 4 * c);
+          uint32_t u = 0u; /* bit column p, W[0] most significant */
+          for (int b = 0; b < 32; ++b) u |= ((W[b] >> p) & 1u) << (31 - b);
           int sig = s[y * L + x];
           int nb[4] = {s[y * L + (x + 1) % L], s[y * L + (x + L - 1) % L], s[((y + 1) % L) * L + x],
                        s[((y + L - 1) % L) * L + x]};

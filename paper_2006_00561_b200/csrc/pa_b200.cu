@@ -166,23 +166,43 @@ LevelTables tables(pa_ctx* c) {
   return t;
 }
 
-template <int L>
-void launch_sweep_L(pa_ctx* c, const StepParams* sp, int mode) {
-  const uint64_t threads = (uint64_t)c->cap * Geo<L>::G;
-  const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
-  k_sweep<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), sp, c->dev<uint32_t>(c->lo.spins[0]),
-                                                    c->dev<uint32_t>(c->lo.spins[1]), c->dev<int32_t>(c->lo.E[0]),
-                                                    c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]),
-                                                    c->dev<int32_t>(c->lo.M[1]), c->key, mode);
+SweepArgs sweep_args(int theta, uint32_t T4, uint32_t T8, int mode) {
+  SweepArgs sa;
+  for (int i = 0; i < 32; ++i) {  // threshold bits, most significant first, as LOP3 operands
+    sa.a[i] = ((T4 >> (31 - i)) & 1u) ? 0xffffffffu : 0u;
+    sa.b[i] = ((T8 >> (31 - i)) & 1u) ? 0xffffffffu : 0u;
+  }
+  sa.theta = theta;
+  sa.mode = mode;
+  return sa;
 }
-void launch_sweep(pa_ctx* c, const StepParams* sp, int mode) {
+
+template <int L>
+void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
+  uint32_t *s0 = c->dev<uint32_t>(c->lo.spins[0]), *s1 = c->dev<uint32_t>(c->lo.spins[1]);
+  int32_t *e0 = c->dev<int32_t>(c->lo.E[0]), *e1 = c->dev<int32_t>(c->lo.E[1]);
+  int32_t *m0 = c->dev<int32_t>(c->lo.M[0]), *m1 = c->dev<int32_t>(c->lo.M[1]);
+  const DevState* st = c->dev<DevState>(c->lo.state);
+  if constexpr (L >= 64) {
+    const uint64_t threads = (uint64_t)c->cap * Geo<L>::G;
+    const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
+    k_sweep<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa);
+  } else {
+    const uint64_t threads = (uint64_t)c->cap * SGeo<L>::G;
+    const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
+    k_sweep_small<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa);
+  }
+}
+// mode 0: theta sweeps of the resampled population with the thresholds of the step; mode 1: energies only
+void launch_sweep(pa_ctx* c, int theta, uint32_t T4, uint32_t T8, int mode) {
   Prof p(c, PA_K_SWEEP);
+  const SweepArgs sa = sweep_args(theta, T4, T8, mode);
   switch (c->cfg.L) {
-    case 8: launch_sweep_L<8>(c, sp, mode); break;
-    case 16: launch_sweep_L<16>(c, sp, mode); break;
-    case 32: launch_sweep_L<32>(c, sp, mode); break;
-    case 64: launch_sweep_L<64>(c, sp, mode); break;
-    default: launch_sweep_L<128>(c, sp, mode); break;
+    case 8: launch_sweep_L<8>(c, sa); break;
+    case 16: launch_sweep_L<16>(c, sa); break;
+    case 32: launch_sweep_L<32>(c, sa); break;
+    case 64: launch_sweep_L<64>(c, sa); break;
+    default: launch_sweep_L<128>(c, sa); break;
   }
 }
 
@@ -215,7 +235,8 @@ void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
 }
 
 // all kernels of one temperature step, parameters in device slot sp
-void enqueue_step(pa_ctx* c, const StepParams* sp, int theta) {
+void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
+  const int theta = hp.theta;
   DevState* st = c->dev<DevState>(c->lo.state);
   const LevelTables tb = tables(c);
   const int N = c->N;
@@ -258,7 +279,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, int theta) {
                                                                     (unsigned long long)c->cap, c->cfg.P, c->key);
   }
   launch_copy(c);
-  if (theta > 0) launch_sweep(c, sp, 0);
+  if (theta > 0) launch_sweep(c, theta, hp.T4, hp.T8, 0);
   launch_observe(c, sp, 0);
 }
 
@@ -413,7 +434,7 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
                                                                       c->dev<uint32_t>(c->lo.spins[1]), c->wrep, c->key);
     c->launches += 1;
   }
-  launch_sweep(c, nullptr, 1);   // E_j, M_j
+  launch_sweep(c, 0, 0u, 0u, 1);   // E_j, M_j
   launch_observe(c, nullptr, 1);  // population sums
   c->last_Q = 1.0;
   int rc = sync_state(c);
@@ -443,7 +464,7 @@ int pa_run(pa_ctx* c, const double* betas, int32_t K, int32_t theta, int32_t* st
       from = betas[base + k];
     }
     CK(cudaMemcpyAsync(d_params, c->h_params, sizeof(StepParams) * nk, cudaMemcpyHostToDevice, c->stream));
-    for (int k = 0; k < nk; ++k) enqueue_step(c, d_params + k, theta);
+    for (int k = 0; k < nk; ++k) enqueue_step(c, d_params + k, c->h_params[k]);
   }
   int rc = sync_state(c);
   if (rc != PA_OK) return rc;
@@ -570,7 +591,7 @@ int pa_set_spins(pa_ctx* c, const uint32_t* src, int64_t R, int src_on_device) {
   k_set_population<<<1, 256, 0, c->stream>>>(c->dev<DevState>(c->lo.state), (unsigned long long)R,
                                              c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]), c->cfg.P);
   c->launches += 1;
-  launch_sweep(c, nullptr, 1);
+  launch_sweep(c, 0, 0u, 0u, 1);
   launch_observe(c, nullptr, 1);
   return sync_state(c);
 }

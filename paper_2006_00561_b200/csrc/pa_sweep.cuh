@@ -1,33 +1,37 @@
 // pa_sweep.cuh -- a7/a8: theta checkerboard Metropolis sweeps of every replica + E, M from the final lattice.
 // PAPER.md:56 (MCMC equilibration at the new temperature), :126-128 (theta), :62 (observables);
-// rule and random keying: DESIGN.md "C3", "C4".
+// rule and random keying: DESIGN.md "C3" (reading G20), "C4".
 //
-// Layout in registers (multispin coding WITHIN a replica): G = min(L,32) lanes share one replica, lane g holds
-// rows g*RPL .. g*RPL+RPL-1.  Every row is split into its two colour planes so that one 32-bit word holds 32
-// sites that are updated simultaneously:
+// Multispin coding WITHIN a replica, lattice in registers.  Every row is split into its two colour planes,
 //   plane c of row y, bit k  <->  site x = 2k + ((y + c) & 1)          (colour (x+y)&1 == c)
-// The four neighbours of a colour-c site (k,y) are colour 1-c sites: rows y-1, y+1 at bit k, row y at bit k,
-// and row y at bit k-1 (if (y+c) even) or k+1 (if odd), all modulo L/2.  Up/down rows of neighbouring lanes
-// come by warp shuffle.  The lattice is read from HBM once and written once per step; nothing else touches
-// memory during the theta sweeps.
+// and 32 consecutive active sites of a half-sweep (ordinals q = y*(L/2) + k) share one 32-bit "plane word":
+//   L >= 64: a plane word is 32 consecutive k of one row; lane g of the replica's 32 lanes holds rows g*RPL ..
+//   L <  64: a plane word is 64/L consecutive rows of L/2 bits each; lane g of the replica's N/64 lanes holds word g.
+// The four neighbours of a colour-c site (k,y) are colour 1-c sites: rows y-1, y+1 at bit k, row y at bit k and
+// row y at bit k-1 (if (y+c) even) or k+1 (if odd), all modulo L/2.  Rows of neighbouring lanes come by warp shuffle.
+// The lattice is read from HBM once and written once per step; nothing else touches memory during the sweeps.
+//
+// Acceptance (C3/C4, G20): a plane word is exactly one keyed group: its 32 keyed Philox words W_0..W_31 hold,
+// in bit column p, the 32-bit uniform of the site at bit p (W_0 = most significant bit).  "u < T" is therefore
+// evaluated for the 32 sites of the word AT ONCE by a bit-sliced comparator that walks the words most significant
+// bit first: one LOP3 tracks the sites whose bits have all been equal to the threshold's so far, one LOP3 remembers
+// the last random bit seen while a site was still undecided.  A site is decided at the first bit that differs
+// (probability 1/2 per bit), so the loop stops -- warp-uniformly -- as soon as no site of the warp is undecided:
+// on average 3.3 of the 8 Philox blocks of a group are ever computed.  The result is independent of where the
+// loop stops (decided sites do not change), so it equals the plain definition bit for bit.
 #pragma once
 #include "pa_common.cuh"
 
 namespace pa {
 
-template <int L>
-struct Geo {
-  static constexpr int N = L * L;
-  static constexpr int G = L < 32 ? L : 32;       // lanes per replica
-  static constexpr int RPL = L / G;               // rows per lane
-  static constexpr int HB = L / 2;                // bits per row per colour plane
-  static constexpr int WPP = (HB + 31) / 32;      // words per row plane
-  static constexpr int WR = (L + 31) / 32;        // raw words per row
-  static constexpr int WREP = N / 32;             // words per replica
-  static constexpr int NB = HB < 32 ? HB : 32;    // used bits per plane word
-  static constexpr uint32_t HMASK = HB >= 32 ? 0xffffffffu : ((1u << (HB & 31)) - 1u);
-  static constexpr int CALLS_PER_WORD = NB / 4;   // Philox blocks per plane word
-  static constexpr int CALLS_PER_ROW = HB / 4;
+// threshold bits as all-ones / all-zeros masks, most significant bit first (host-filled kernel argument: the
+// LOP3s read them straight from the constant bank)
+struct SweepArgs {
+  uint32_t a[32];  // a[i] = ~0 iff bit (31 - i) of T4 is set
+  uint32_t b[32];  // same for T8
+  int theta;
+  int mode;  // 0: inside a step -> buffer cur^1, Rnew replicas, theta sweeps keyed with step ordinal st->step + 1
+             // 1: init / set_spins -> buffer cur, R replicas, no sweeps (energies only)
 };
 
 __device__ __forceinline__ uint32_t even_bits(uint32_t x) {  // bits 0,2,4,.. -> bits 0..15
@@ -47,21 +51,76 @@ __device__ __forceinline__ uint32_t spread_bits(uint32_t x) {  // bits 0..15 -> 
   return x;
 }
 
-// acc |= BIT if w < T (unsigned).  Written as compare + predicated OR so that both instructions stay on the
-// ALU pipe: the FMA pipe is saturated by Philox's 32x32->64 multiplies (ptxas turns carry-based forms into IMAD.X).
-template <uint32_t BIT>
-__device__ __forceinline__ void or_if_lt(uint32_t& acc, uint32_t w, uint32_t T) {
-  asm("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %1, %2;\n\t@p or.b32 %0, %0, %3;\n\t}" : "+r"(acc) : "r"(w), "r"(T), "n"(BIT));
+// one bit of the MSB-first comparator for 32 sites: u = random bits, A = threshold bit (all-ones / all-zeros)
+//   v   <- u where the site is still undecided (so that v ends as the random bit AT the deciding position)
+//   und <- und & ~(u ^ A)
+__device__ __forceinline__ void cmp_bit(uint32_t& und, uint32_t& v, uint32_t u, uint32_t A) {
+  v = (und & u) | (~und & v);
+  und = und & ~(u ^ A);
 }
 
-// the two random masks of one Philox block (4 consecutive active sites) at bit offset SH
-template <int SH>
-__device__ __forceinline__ void push_block(uint32_t& r4, uint32_t& r8, const uint4& w, uint32_t T4, uint32_t T8) {
-  or_if_lt<(1u << SH)>(r4, w.x, T4); or_if_lt<(2u << SH)>(r4, w.y, T4);
-  or_if_lt<(4u << SH)>(r4, w.z, T4); or_if_lt<(8u << SH)>(r4, w.w, T4);
-  or_if_lt<(1u << SH)>(r8, w.x, T8); or_if_lt<(2u << SH)>(r8, w.y, T8);
-  or_if_lt<(4u << SH)>(r8, w.z, T8); or_if_lt<(8u << SH)>(r8, w.w, T8);
+// flip masks of NW plane words.  ge1 / ge2: sites with a >= 1 / a >= 2 anti-aligned neighbours; call0 = 8 * group.
+// a >= 2: always flip;  a == 1: flip iff u < T4;  a == 0: flip iff u < T8   (u < T  <=>  at the first differing bit,
+// most significant first, u has 0).
+template <int NW>
+__device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uint32_t (&ge2)[NW], uint32_t slot,
+                                            const uint32_t (&call0)[NW], uint32_t c2, uint32_t c3, const PhiloxKey& key,
+                                            const SweepArgs& sa, uint32_t (&flip)[NW]) {
+  uint32_t und4[NW], und8[NW], v4[NW], v8[NW];
+#pragma unroll
+  for (int i = 0; i < NW; ++i) {
+    und4[i] = ge1[i] & ~ge2[i];
+    und8[i] = ~ge1[i];
+    v4[i] = 0xffffffffu;
+    v8[i] = 0xffffffffu;
+  }
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+#pragma unroll
+    for (int i = 0; i < NW; ++i) {
+      const uint4 w = philox4x32_10(slot, call0[i] + (uint32_t)c, c2, c3, key);
+      cmp_bit(und4[i], v4[i], w.x, sa.a[4 * c + 0]); cmp_bit(und8[i], v8[i], w.x, sa.b[4 * c + 0]);
+      cmp_bit(und4[i], v4[i], w.y, sa.a[4 * c + 1]); cmp_bit(und8[i], v8[i], w.y, sa.b[4 * c + 1]);
+      cmp_bit(und4[i], v4[i], w.z, sa.a[4 * c + 2]); cmp_bit(und8[i], v8[i], w.z, sa.b[4 * c + 2]);
+      cmp_bit(und4[i], v4[i], w.w, sa.a[4 * c + 3]); cmp_bit(und8[i], v8[i], w.w, sa.b[4 * c + 3]);
+    }
+    if (c >= 2 && c < 7) {  // nobody is done after 8 bits; after 12 bits 3 of 4 warps are
+      uint32_t any = 0u;
+#pragma unroll
+      for (int i = 0; i < NW; ++i) any |= und4[i] | und8[i];
+      if (__all_sync(0xffffffffu, any == 0u)) break;
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < NW; ++i) flip[i] = ge2[i] | (~v4[i] & ~und4[i]) | (~v8[i] & ~und8[i]);
 }
+
+// masks of the sites with a >= 1 and a >= 2 from the four difference words (1 = anti-aligned)
+__device__ __forceinline__ void neighbour_classes(uint32_t tt, uint32_t U, uint32_t D, uint32_t Sm, uint32_t B,
+                                                  uint32_t& ge1, uint32_t& ge2) {
+  const uint32_t d0 = tt ^ U, d1 = tt ^ D, d2 = tt ^ Sm, d3 = tt ^ B;
+  const uint32_t maj = (d0 & d1) | (d0 & d2) | (d1 & d2);
+  const uint32_t any3 = d0 | d1 | d2;
+  ge2 = maj | (any3 & d3);
+  ge1 = any3 | d3;
+}
+
+constexpr int SWEEP_THREADS = 256;
+
+// =====================================================================================================
+// L >= 64
+// =====================================================================================================
+template <int L>
+struct Geo {
+  static constexpr int N = L * L;
+  static constexpr int G = 32;                    // lanes per replica
+  static constexpr int RPL = L / G;               // rows per lane
+  static constexpr int HB = L / 2;                // bits per row per colour plane
+  static constexpr int WPP = HB / 32;             // words per row plane
+  static constexpr int WR = L / 32;               // raw words per row
+  static constexpr int WREP = N / 32;             // words per replica
+  static constexpr int NWB = 2;                   // plane words whose Philox chains run interleaved
+};
 
 template <int L>
 struct Lattice {
@@ -73,28 +132,22 @@ struct Lattice {
 template <int L>
 __device__ __forceinline__ void rot_row(const uint32_t (&s)[Geo<L>::WPP], int dir, uint32_t (&out)[Geo<L>::WPP]) {
   using G_ = Geo<L>;
-  if constexpr (G_::HB >= 32) {
 #pragma unroll
-    for (int i = 0; i < G_::WPP; ++i) {
-      const uint32_t prev = s[(i + G_::WPP - 1) % G_::WPP], next = s[(i + 1) % G_::WPP];
-      const uint32_t left = __funnelshift_l(prev, s[i], 1);   // (s[i] << 1) | (prev >> 31)
-      const uint32_t right = __funnelshift_r(s[i], next, 1);  // (s[i] >> 1) | (next << 31)
-      out[i] = dir ? right : left;
-    }
-  } else {
-    const uint32_t a = s[0];
-    const uint32_t left = ((a << 1) | (a >> (G_::HB - 1))) & G_::HMASK;
-    const uint32_t right = ((a >> 1) | (a << (G_::HB - 1))) & G_::HMASK;
-    out[0] = dir ? right : left;
+  for (int i = 0; i < G_::WPP; ++i) {
+    const uint32_t prev = s[(i + G_::WPP - 1) % G_::WPP], next = s[(i + 1) % G_::WPP];
+    const uint32_t left = __funnelshift_l(prev, s[i], 1);   // (s[i] << 1) | (prev >> 31)
+    const uint32_t right = __funnelshift_r(s[i], next, 1);  // (s[i] >> 1) | (next << 31)
+    out[i] = dir ? right : left;
   }
 }
 
 // One half-sweep of colour C on the lane's rows.  T = plane C (updated), S = plane 1-C (read only).
 template <int L, int C>
 __device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot, uint32_t t, uint32_t c3,
-                                           const PhiloxKey& key, uint32_t T4, uint32_t T8) {
+                                           const PhiloxKey& key, const SweepArgs& sa) {
   using G_ = Geo<L>;
   constexpr unsigned FULL = 0xffffffffu;
+  constexpr int NWL = G_::RPL * G_::WPP;  // plane words of this lane
   uint32_t(&T)[G_::RPL][G_::WPP] = lat.p[C];
   uint32_t(&S)[G_::RPL][G_::WPP] = lat.p[1 - C];
   // rows above the lane's first row and below its last row
@@ -106,56 +159,32 @@ __device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot
     dn[i] = __shfl_sync(FULL, S[0][i], gd, G_::G);
   }
   const uint32_t c2 = 2u * t + (uint32_t)C;
+  uint32_t ge1[NWL], ge2[NWL], call0[NWL];
 #pragma unroll
   for (int r = 0; r < G_::RPL; ++r) {
     const int y = g * G_::RPL + r;
-    const int dir = (y + C) & 1;
     uint32_t B[G_::WPP];
-    rot_row<L>(S[r], dir, B);
+    rot_row<L>(S[r], (y + C) & 1, B);
 #pragma unroll
     for (int i = 0; i < G_::WPP; ++i) {
       const uint32_t U = (r > 0) ? S[r > 0 ? r - 1 : 0][i] : up[i];
       const uint32_t D = (r < G_::RPL - 1) ? S[r < G_::RPL - 1 ? r + 1 : 0][i] : dn[i];
-      const uint32_t tt = T[r][i];
-      const uint32_t d0 = tt ^ U, d1 = tt ^ D, d2 = tt ^ S[r][i], d3 = tt ^ B[i];  // 1 = anti-aligned
-      const uint32_t maj = (d0 & d1) | (d0 & d2) | (d1 & d2);
-      const uint32_t any3 = d0 | d1 | d2;
-      const uint32_t ge2 = maj | (any3 & d3);  // a >= 2: dE <= 0, always flip
-      const uint32_t ge1 = any3 | d3;
-      // random masks: bit k set iff the site's keyed word < T4 (resp. T8)
-      uint32_t r4 = 0u, r8 = 0u;
-      const uint32_t call0 = (uint32_t)y * G_::CALLS_PER_ROW + (uint32_t)i * 8u;
-      if constexpr (G_::RPL * G_::WPP <= 2) {
-        // small lattices per lane: fully unrolled, bit positions are immediates
-#pragma unroll
-        for (int cc = 0; cc < G_::CALLS_PER_WORD; ++cc) {
-          const uint4 w = philox4x32_10(slot, call0 + cc, c2, c3, key);
-          switch (cc) {
-            case 0: push_block<0>(r4, r8, w, T4, T8); break;
-            case 1: push_block<4>(r4, r8, w, T4, T8); break;
-            case 2: push_block<8>(r4, r8, w, T4, T8); break;
-            case 3: push_block<12>(r4, r8, w, T4, T8); break;
-            case 4: push_block<16>(r4, r8, w, T4, T8); break;
-            case 5: push_block<20>(r4, r8, w, T4, T8); break;
-            case 6: push_block<24>(r4, r8, w, T4, T8); break;
-            default: push_block<28>(r4, r8, w, T4, T8); break;
-          }
-        }
-      } else {
-        // L = 128: 8 plane words per lane; keep the block loop rolled (two chains in flight) to bound code size
-#pragma unroll 2
-        for (int cc = 0; cc < G_::CALLS_PER_WORD; ++cc) {
-          const uint4 w = philox4x32_10(slot, call0 + cc, c2, c3, key);
-          uint32_t n4 = 0u, n8 = 0u;
-          push_block<0>(n4, n8, w, T4, T8);
-          r4 |= n4 << (4 * cc);
-          r8 |= n8 << (4 * cc);
-        }
-      }
-      // flip iff a>=2, or a==1 and u<T4, or a==0 and u<T8
-      const uint32_t flip = ge2 | (ge1 & r4) | (~ge1 & r8);
-      T[r][i] = tt ^ flip;
+      neighbour_classes(T[r][i], U, D, S[r][i], B[i], ge1[r * G_::WPP + i], ge2[r * G_::WPP + i]);
+      call0[r * G_::WPP + i] = 8u * ((uint32_t)y * G_::WPP + (uint32_t)i);  // group = y * WPP + i
     }
+  }
+#pragma unroll
+  for (int w0 = 0; w0 < NWL; w0 += G_::NWB) {
+    uint32_t a1[G_::NWB], a2[G_::NWB], cc[G_::NWB], flip[G_::NWB];
+#pragma unroll
+    for (int j = 0; j < G_::NWB; ++j) {
+      a1[j] = ge1[w0 + j];
+      a2[j] = ge2[w0 + j];
+      cc[j] = call0[w0 + j];
+    }
+    lazy_accept<G_::NWB>(a1, a2, slot, cc, c2, c3, key, sa, flip);
+#pragma unroll
+    for (int j = 0; j < G_::NWB; ++j) T[(w0 + j) / G_::WPP][(w0 + j) % G_::WPP] ^= flip[j];
   }
 }
 
@@ -197,21 +226,12 @@ template <int L>
 __device__ __forceinline__ void row_to_planes(const uint32_t (&raw)[Geo<L>::WR], int y_odd,
                                               uint32_t (&p0)[Geo<L>::WPP], uint32_t (&p1)[Geo<L>::WPP]) {
   using G_ = Geo<L>;
-  uint32_t ev[G_::WPP], od[G_::WPP];
-  if constexpr (L >= 64) {
-#pragma unroll
-    for (int i = 0; i < G_::WPP; ++i) {
-      ev[i] = even_bits(raw[2 * i]) | (even_bits(raw[2 * i + 1]) << 16);
-      od[i] = even_bits(raw[2 * i] >> 1) | (even_bits(raw[2 * i + 1] >> 1) << 16);
-    }
-  } else {
-    ev[0] = even_bits(raw[0]);
-    od[0] = even_bits(raw[0] >> 1);
-  }
 #pragma unroll
   for (int i = 0; i < G_::WPP; ++i) {  // even row: colour 0 sits at even x; odd row: at odd x
-    p0[i] = y_odd ? od[i] : ev[i];
-    p1[i] = y_odd ? ev[i] : od[i];
+    const uint32_t ev = even_bits(raw[2 * i]) | (even_bits(raw[2 * i + 1]) << 16);
+    const uint32_t od = even_bits(raw[2 * i] >> 1) | (even_bits(raw[2 * i + 1] >> 1) << 16);
+    p0[i] = y_odd ? od : ev;
+    p1[i] = y_odd ? ev : od;
   }
 }
 template <int L>
@@ -221,29 +241,137 @@ __device__ __forceinline__ void planes_to_row(const uint32_t (&p0)[Geo<L>::WPP],
 #pragma unroll
   for (int i = 0; i < G_::WPP; ++i) {
     const uint32_t ev = y_odd ? p1[i] : p0[i], od = y_odd ? p0[i] : p1[i];
-    if constexpr (L >= 64) {
-      raw[2 * i] = spread_bits(ev) | (spread_bits(od) << 1);
-      raw[2 * i + 1] = spread_bits(ev >> 16) | (spread_bits(od >> 16) << 1);
-    } else {
-      raw[0] = spread_bits(ev) | (spread_bits(od) << 1);
-    }
+    raw[2 * i] = spread_bits(ev) | (spread_bits(od) << 1);
+    raw[2 * i + 1] = spread_bits(ev >> 16) | (spread_bits(od >> 16) << 1);
   }
 }
 
-constexpr int SWEEP_THREADS = 256;
-
-// mode 0: inside a step -> buffer cur^1, Rnew replicas, theta sweeps keyed with step ordinal st->step+1
-// mode 1: init / set_spins -> buffer cur, R replicas, no sweeps (energies only)
 template <int L>
 __global__ void __launch_bounds__(SWEEP_THREADS, (L >= 128 ? 2 : 3))
-k_sweep(const DevState* __restrict__ st, const StepParams* __restrict__ sp, uint32_t* __restrict__ spins0,
-        uint32_t* __restrict__ spins1, int32_t* __restrict__ E0, int32_t* __restrict__ E1, int32_t* __restrict__ M0,
-        int32_t* __restrict__ M1, const PhiloxKey key, const int mode) {
+k_sweep(const DevState* __restrict__ st, uint32_t* __restrict__ spins0, uint32_t* __restrict__ spins1,
+        int32_t* __restrict__ E0, int32_t* __restrict__ E1, int32_t* __restrict__ M0, int32_t* __restrict__ M1,
+        const PhiloxKey key, const SweepArgs sa) {
   using G_ = Geo<L>;
+  static_assert(L >= 64, "k_sweep_small handles L < 64");
   if (st->status != ST_OK) return;
-  const unsigned buf = mode == 0 ? (st->cur ^ 1u) : st->cur;
-  const unsigned long long count = mode == 0 ? st->Rnew : st->R;
-  const int theta = mode == 0 ? sp->theta : 0;
+  const unsigned buf = sa.mode == 0 ? (st->cur ^ 1u) : st->cur;
+  const unsigned long long count = sa.mode == 0 ? st->Rnew : st->R;
+  const int theta = sa.mode == 0 ? sa.theta : 0;
+  uint32_t* __restrict__ spins = buf ? spins1 : spins0;
+  int32_t* __restrict__ Eo = buf ? E1 : E0;
+  int32_t* __restrict__ Mo = buf ? M1 : M0;
+
+  const unsigned long long tid = (unsigned long long)blockIdx.x * SWEEP_THREADS + threadIdx.x;
+  const unsigned long long slot64 = tid / G_::G;  // one warp per replica
+  const int g = (int)(tid % G_::G);
+  if (slot64 >= count) return;  // warp-uniform
+  const uint32_t slot = (uint32_t)slot64;
+  uint32_t* rep = spins + slot64 * G_::WREP;
+
+  // ---- load (once per step): the lane's rows are RPL*WR contiguous words = RPL*WR/4 16-byte vectors ----
+  Lattice<L> lat;
+  constexpr int NV = G_::RPL * G_::WR / 4;
+  {
+    uint32_t rawall[G_::RPL * G_::WR];
+    const uint4* src = reinterpret_cast<const uint4*>(rep) + g * NV;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const uint4 q = src[v];
+      rawall[4 * v] = q.x; rawall[4 * v + 1] = q.y; rawall[4 * v + 2] = q.z; rawall[4 * v + 3] = q.w;
+    }
+#pragma unroll
+    for (int r = 0; r < G_::RPL; ++r) {
+      uint32_t raw[G_::WR];
+#pragma unroll
+      for (int i = 0; i < G_::WR; ++i) raw[i] = rawall[r * G_::WR + i];
+      row_to_planes<L>(raw, (g * G_::RPL + r) & 1, lat.p[0][r], lat.p[1][r]);
+    }
+  }
+
+  // ---- theta sweeps ----------------------------------------------------------------------------
+  if (theta > 0) {
+    const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
+    for (int t = 0; t < theta; ++t) {
+      half_sweep<L, 0>(lat, g, slot, (uint32_t)t, c3, key, sa);
+      half_sweep<L, 1>(lat, g, slot, (uint32_t)t, c3, key, sa);
+    }
+  }
+
+  // ---- a8: E = 2u - 2N, M = 2*popc - N ----------------------------------------------------------
+  int unsat, ups;
+  count_bonds<L>(lat, g, unsat, ups);
+#pragma unroll
+  for (int o = G_::G / 2; o > 0; o >>= 1) {
+    unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
+    ups += __shfl_xor_sync(0xffffffffu, ups, o);
+  }
+  if (g == 0) {
+    Eo[slot64] = 2 * unsat - 2 * G_::N;
+    Mo[slot64] = 2 * ups - G_::N;
+  }
+
+  // ---- store (once per step) -------------------------------------------------------------------
+  if (theta > 0) {
+    uint32_t rawall[G_::RPL * G_::WR];
+#pragma unroll
+    for (int r = 0; r < G_::RPL; ++r) {
+      uint32_t raw[G_::WR];
+      planes_to_row<L>(lat.p[0][r], lat.p[1][r], (g * G_::RPL + r) & 1, raw);
+#pragma unroll
+      for (int i = 0; i < G_::WR; ++i) rawall[r * G_::WR + i] = raw[i];
+    }
+    uint4* dst = reinterpret_cast<uint4*>(rep) + g * NV;
+#pragma unroll
+    for (int v = 0; v < NV; ++v)
+      dst[v] = make_uint4(rawall[4 * v], rawall[4 * v + 1], rawall[4 * v + 2], rawall[4 * v + 3]);
+  }
+}
+
+// =====================================================================================================
+// L < 64: one plane word = RG = 64/L consecutive rows of HB = L/2 bits; a replica is G = N/64 lanes with one
+// word per colour each (L = 32: 16 lanes, L = 16: 4 lanes, L = 8: one thread holds the whole replica).
+// =====================================================================================================
+template <int L>
+struct SGeo {
+  static constexpr int N = L * L;
+  static constexpr int G = N / 64;      // lanes per replica
+  static constexpr int HB = L / 2;      // bits per row field
+  static constexpr int RG = 32 / HB;    // rows per word (even)
+  static constexpr int WREP = N / 32;
+  static constexpr uint32_t FIELD = (1u << HB) - 1u;
+  static constexpr uint32_t ER = L == 32 ? 0x0000ffffu : (L == 16 ? 0x00ff00ffu : 0x0f0f0f0fu);   // fields of even rows
+  static constexpr uint32_t LSBS = L == 32 ? 0x00010001u : (L == 16 ? 0x01010101u : 0x11111111u);  // bit 0 of every field
+  static constexpr uint32_t MSBS = LSBS << (HB - 1);
+};
+
+// neighbour words of the lane's word of plane C: S = the lane's word of plane 1-C
+template <int L, int C>
+__device__ __forceinline__ void small_neighbours(uint32_t S, int g, uint32_t& U, uint32_t& D, uint32_t& B) {
+  using G_ = SGeo<L>;
+  uint32_t Sp = S, Sn = S;
+  if constexpr (G_::G > 1) {
+    Sp = __shfl_sync(0xffffffffu, S, (g + G_::G - 1) % G_::G, G_::G);
+    Sn = __shfl_sync(0xffffffffu, S, (g + 1) % G_::G, G_::G);
+  }
+  U = __funnelshift_l(Sp, S, G_::HB);  // row y-1 at the position of row y: (S << HB) | (Sp >> (32 - HB))
+  D = __funnelshift_r(S, Sn, G_::HB);  // row y+1:                          (S >> HB) | (Sn << (32 - HB))
+  const uint32_t rotl = ((S << 1) & ~G_::LSBS) | ((S >> (G_::HB - 1)) & G_::LSBS);  // bit k <- bit k-1 inside every field
+  const uint32_t rotr = ((S >> 1) & ~G_::MSBS) | ((S << (G_::HB - 1)) & G_::MSBS);  // bit k <- bit k+1
+  // row y uses k-1 when (y + C) is even; the word's first row is even
+  B = C == 0 ? ((rotl & G_::ER) | (rotr & ~G_::ER)) : ((rotr & G_::ER) | (rotl & ~G_::ER));
+}
+
+template <int L>
+__global__ void __launch_bounds__(SWEEP_THREADS)
+k_sweep_small(const DevState* __restrict__ st, uint32_t* __restrict__ spins0, uint32_t* __restrict__ spins1,
+              int32_t* __restrict__ E0, int32_t* __restrict__ E1, int32_t* __restrict__ M0, int32_t* __restrict__ M1,
+              const PhiloxKey key, const SweepArgs sa) {
+  using G_ = SGeo<L>;
+  static_assert(L == 8 || L == 16 || L == 32, "");
+  if (st->status != ST_OK) return;
+  const unsigned buf = sa.mode == 0 ? (st->cur ^ 1u) : st->cur;
+  const unsigned long long count = sa.mode == 0 ? st->Rnew : st->R;
+  const int theta = sa.mode == 0 ? sa.theta : 0;
   uint32_t* __restrict__ spins = buf ? spins1 : spins0;
   int32_t* __restrict__ Eo = buf ? E1 : E0;
   int32_t* __restrict__ Mo = buf ? M1 : M0;
@@ -259,84 +387,65 @@ k_sweep(const DevState* __restrict__ st, const StepParams* __restrict__ sp, uint
   const uint32_t slot = (uint32_t)slot64;
   uint32_t* rep = spins + (valid ? slot64 : 0ull) * G_::WREP;
 
-  // ---- load (once per step) -------------------------------------------------------------------
-  Lattice<L> lat;
-  if constexpr (L >= 64) {
-    // lane's rows are RPL*WR contiguous words = RPL*WR/4 16-byte vectors
-    constexpr int NV = G_::RPL * G_::WR / 4;
-    uint32_t rawall[G_::RPL * G_::WR];
-    const uint4* src = reinterpret_cast<const uint4*>(rep) + g * NV;
-#pragma unroll
-    for (int v = 0; v < NV; ++v) {
-      const uint4 q = valid ? src[v] : make_uint4(0, 0, 0, 0);
-      rawall[4 * v] = q.x; rawall[4 * v + 1] = q.y; rawall[4 * v + 2] = q.z; rawall[4 * v + 3] = q.w;
-    }
-#pragma unroll
-    for (int r = 0; r < G_::RPL; ++r) {
-      uint32_t raw[G_::WR];
-#pragma unroll
-      for (int i = 0; i < G_::WR; ++i) raw[i] = rawall[r * G_::WR + i];
-      row_to_planes<L>(raw, (g * G_::RPL + r) & 1, lat.p[0][r], lat.p[1][r]);
-    }
-  } else {
-    // one row per lane; 32/L rows share a word
-    constexpr int RW = 32 / L;
-    const uint32_t word = valid ? rep[g / RW] : 0u;
-    uint32_t raw[1];
-    raw[0] = (L == 32) ? word : ((word >> ((g % RW) * L)) & ((1u << (L & 31)) - 1u));
-    row_to_planes<L>(raw, g & 1, lat.p[0][0], lat.p[1][0]);
+  // ---- load: 64 raw bits = RG rows ---------------------------------------------------------------
+  uint32_t p[2];
+  {
+    const uint2 q = valid ? reinterpret_cast<const uint2*>(rep)[g] : make_uint2(0u, 0u);
+    const uint32_t ev = even_bits(q.x) | (even_bits(q.y) << 16);
+    const uint32_t od = even_bits(q.x >> 1) | (even_bits(q.y >> 1) << 16);
+    p[0] = (ev & G_::ER) | (od & ~G_::ER);  // even row: colour 0 sits at even x; odd row: at odd x
+    p[1] = (od & G_::ER) | (ev & ~G_::ER);
   }
 
   // ---- theta sweeps ----------------------------------------------------------------------------
   if (theta > 0) {
     const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
-    const uint32_t T4 = sp->T4, T8 = sp->T8;
+    const uint32_t call0[1] = {8u * (uint32_t)g};  // group = g
     for (int t = 0; t < theta; ++t) {
-      half_sweep<L, 0>(lat, g, slot, (uint32_t)t, c3, key, T4, T8);
-      half_sweep<L, 1>(lat, g, slot, (uint32_t)t, c3, key, T4, T8);
+      {
+        uint32_t U, D, B, ge1[1], ge2[1], flip[1];
+        small_neighbours<L, 0>(p[1], g, U, D, B);
+        neighbour_classes(p[0], U, D, p[1], B, ge1[0], ge2[0]);
+        if (!valid) { ge1[0] = 0xffffffffu; ge2[0] = 0xffffffffu; }  // padding lanes never hold the warp back
+        lazy_accept<1>(ge1, ge2, slot, call0, 2u * (uint32_t)t, c3, key, sa, flip);
+        p[0] ^= flip[0];
+      }
+      {
+        uint32_t U, D, B, ge1[1], ge2[1], flip[1];
+        small_neighbours<L, 1>(p[0], g, U, D, B);
+        neighbour_classes(p[1], U, D, p[0], B, ge1[0], ge2[0]);
+        if (!valid) { ge1[0] = 0xffffffffu; ge2[0] = 0xffffffffu; }
+        lazy_accept<1>(ge1, ge2, slot, call0, 2u * (uint32_t)t + 1u, c3, key, sa, flip);
+        p[1] ^= flip[0];
+      }
     }
   }
 
-  // ---- a8: E = 2u - 2N, M = 2*popc - N ----------------------------------------------------------
-  int unsat, ups;
-  count_bonds<L>(lat, g, unsat, ups);
+  // ---- a8: every bond has exactly one colour-0 end ------------------------------------------------
+  {
+    uint32_t U, D, B;
+    small_neighbours<L, 0>(p[1], g, U, D, B);
+    int unsat = __popc(p[0] ^ U) + __popc(p[0] ^ D) + __popc(p[0] ^ p[1]) + __popc(p[0] ^ B);
+    int ups = __popc(p[0]) + __popc(p[1]);
 #pragma unroll
-  for (int o = G_::G / 2; o > 0; o >>= 1) {
-    unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
-    ups += __shfl_xor_sync(0xffffffffu, ups, o);
-  }
-  if (valid && g == 0) {
-    Eo[slot64] = 2 * unsat - 2 * G_::N;
-    Mo[slot64] = 2 * ups - G_::N;
+    for (int o = G_::G / 2; o > 0; o >>= 1) {
+      unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
+      ups += __shfl_xor_sync(0xffffffffu, ups, o);
+    }
+    if (valid && g == 0) {
+      Eo[slot64] = 2 * unsat - 2 * G_::N;
+      Mo[slot64] = 2 * ups - G_::N;
+    }
   }
 
-  // ---- store (once per step) -------------------------------------------------------------------
-  if (theta > 0) {
-    if constexpr (L >= 64) {
-      constexpr int NV = G_::RPL * G_::WR / 4;
-      uint32_t rawall[G_::RPL * G_::WR];
-#pragma unroll
-      for (int r = 0; r < G_::RPL; ++r) {
-        uint32_t raw[G_::WR];
-        planes_to_row<L>(lat.p[0][r], lat.p[1][r], (g * G_::RPL + r) & 1, raw);
-#pragma unroll
-        for (int i = 0; i < G_::WR; ++i) rawall[r * G_::WR + i] = raw[i];
-      }
-      uint4* dst = reinterpret_cast<uint4*>(rep) + g * NV;
-      if (valid) {
-#pragma unroll
-        for (int v = 0; v < NV; ++v)
-          dst[v] = make_uint4(rawall[4 * v], rawall[4 * v + 1], rawall[4 * v + 2], rawall[4 * v + 3]);
-      }
-    } else {
-      constexpr int RW = 32 / L;
-      uint32_t raw[1];
-      planes_to_row<L>(lat.p[0][0], lat.p[1][0], g & 1, raw);
-      uint32_t word = (L == 32) ? raw[0] : (raw[0] << ((g % RW) * L));
-#pragma unroll
-      for (int o = 1; o < RW; o <<= 1) word |= __shfl_xor_sync(0xffffffffu, word, o);
-      if (valid && (g % RW) == 0) rep[g / RW] = word;
-    }
+  // ---- store -------------------------------------------------------------------------------------
+  if (theta > 0 && valid) {
+    const uint32_t ev = (p[0] & G_::ER) | (p[1] & ~G_::ER);
+    const uint32_t od = (p[1] & G_::ER) | (p[0] & ~G_::ER);
+    uint2 q;
+    q.x = spread_bits(ev) | (spread_bits(od) << 1);
+    q.y = spread_bits(ev >> 16) | (spread_bits(od >> 16) << 1);
+    reinterpret_cast<uint2*>(rep)[g] = q;
   }
 }
 

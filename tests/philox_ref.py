@@ -24,8 +24,14 @@ def keyed(seed, c0, c1, c2, tag, step):
 
 
 def sweep_word(seed, step, slot, t, colour, q):
-    """random word of the active site with ordinal q in half-sweep (t, colour) of population slot `slot`"""
-    return keyed(seed, slot, q >> 2, 2 * t + colour, 2, step)[q & 3]
+    """32-bit uniform of the active site with ordinal q in half-sweep (t, colour) of population slot `slot`
+    (C3, reading G20): bit column p = q & 31 of the 32 keyed words of group q >> 5, word 0 = MSB"""
+    gamma, p = q >> 5, q & 31
+    u = 0
+    for b in range(32):
+        w = keyed(seed, slot, 8 * gamma + (b >> 2), 2 * t + colour, 2, step)[b & 3]
+        u |= ((w >> p) & 1) << (31 - b)
+    return u
 
 
 def init_word(seed, j, v):

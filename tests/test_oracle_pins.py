@@ -388,7 +388,7 @@ def test_sweep_random_keying_on_all_up_lattice():
     # all-up lattice at finite beta: every colour-0 site has a=0, so it flips iff its keyed word < T8;
     # colour-0 sites are not touched again in the same sweep.  Predict with the big-int Philox.
     L, seed, step, slot_count = 8, 0xABCDEF0123456789, 12, 3
-    T4, T8 = 2 ** 31, 2 ** 30  # synthetic thresholds: p=1/2, 1/4
+    T4, T8 = 0x9E3779B9, 0x3243F6A8  # synthetic thresholds with all 32 bits in play (p = 0.62, 0.20)
     pop = np.stack([orc.pack(L, np.ones(L * L, np.int8))] * slot_count)
     orc.sweeps(L, pop, seed, step, 1, T4, T8)
     for slot in range(slot_count):
