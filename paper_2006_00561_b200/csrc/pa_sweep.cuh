@@ -51,48 +51,76 @@ __device__ __forceinline__ uint32_t spread_bits(uint32_t x) {  // bits 0..15 -> 
   return x;
 }
 
-// one bit of the MSB-first comparator for 32 sites: u = random bits, A = threshold bit (all-ones / all-zeros)
+// one bit of the MSB-first comparator for 32 sites: u = random bits, A / B = the bit of T4 / T8 (all-ones / all-zeros),
+// ge1 = sites that compare against T4 (a == 1; the others against T8)
 //   v   <- u where the site is still undecided (so that v ends as the random bit AT the deciding position)
-//   und <- und & ~(u ^ A)
-__device__ __forceinline__ void cmp_bit(uint32_t& und, uint32_t& v, uint32_t u, uint32_t A) {
+//   und <- und & ~(u ^ X),  X = the site's own threshold bit
+__device__ __forceinline__ void cmp_bit(uint32_t& und, uint32_t& v, uint32_t u, uint32_t ge1, uint32_t A, uint32_t B) {
+  const uint32_t X = (ge1 & A) | (~ge1 & B);
   v = (und & u) | (~und & v);
-  und = und & ~(u ^ A);
+  und = und & ~(u ^ X);
+}
+__device__ __forceinline__ void cmp_block(uint32_t& und, uint32_t& v, const uint4& w, uint32_t ge1, const uint32_t* a,
+                                          const uint32_t* b) {
+  cmp_bit(und, v, w.x, ge1, a[0], b[0]);
+  cmp_bit(und, v, w.y, ge1, a[1], b[1]);
+  cmp_bit(und, v, w.z, ge1, a[2], b[2]);
+  cmp_bit(und, v, w.w, ge1, a[3], b[3]);
 }
 
-// flip masks of NW plane words.  ge1 / ge2: sites with a >= 1 / a >= 2 anti-aligned neighbours; call0 = 8 * group.
-// a >= 2: always flip;  a == 1: flip iff u < T4;  a == 0: flip iff u < T8   (u < T  <=>  at the first differing bit,
-// most significant first, u has 0).
+// flip masks of the NW plane words of a lane.  ge1 / ge2: sites with a >= 1 / a >= 2 anti-aligned neighbours;
+// call0 = 8 * group.   a >= 2: always flip;  a == 1: flip iff u < T4;  a == 0: flip iff u < T8
+// (u < T  <=>  at the first differing bit, most significant first, u has 0).
+//   stage 1: Philox blocks 0 and 1 of every word (8 bits decide 255 of 256 sites; 88 % of the (lane, word) pairs are
+//            completely decided afterwards);
+//   stage 2: while some lane of the warp still has an undecided word, every lane advances ONE of its undecided words
+//            by one block -- the stragglers of different words of a lane share the warp's instruction slots.
+// Blocks that are never computed cannot change a decided site, so the result is the plain definition's.
 template <int NW>
 __device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uint32_t (&ge2)[NW], uint32_t slot,
                                             const uint32_t (&call0)[NW], uint32_t c2, uint32_t c3, const PhiloxKey& key,
                                             const SweepArgs& sa, uint32_t (&flip)[NW]) {
-  uint32_t und4[NW], und8[NW], v4[NW], v8[NW];
+  uint32_t und[NW], v[NW], nxt[NW];
 #pragma unroll
   for (int i = 0; i < NW; ++i) {
-    und4[i] = ge1[i] & ~ge2[i];
-    und8[i] = ~ge1[i];
-    v4[i] = 0xffffffffu;
-    v8[i] = 0xffffffffu;
+    und[i] = ~ge2[i];
+    v[i] = 0xffffffffu;
+    nxt[i] = 2u;
   }
 #pragma unroll
-  for (int c = 0; c < 8; ++c) {
+  for (int c = 0; c < 2; ++c) {
 #pragma unroll
     for (int i = 0; i < NW; ++i) {
       const uint4 w = philox4x32_10(slot, call0[i] + (uint32_t)c, c2, c3, key);
-      cmp_bit(und4[i], v4[i], w.x, sa.a[4 * c + 0]); cmp_bit(und8[i], v8[i], w.x, sa.b[4 * c + 0]);
-      cmp_bit(und4[i], v4[i], w.y, sa.a[4 * c + 1]); cmp_bit(und8[i], v8[i], w.y, sa.b[4 * c + 1]);
-      cmp_bit(und4[i], v4[i], w.z, sa.a[4 * c + 2]); cmp_bit(und8[i], v8[i], w.z, sa.b[4 * c + 2]);
-      cmp_bit(und4[i], v4[i], w.w, sa.a[4 * c + 3]); cmp_bit(und8[i], v8[i], w.w, sa.b[4 * c + 3]);
-    }
-    if (c >= 2 && c < 7) {  // nobody is done after 8 bits; after 12 bits 3 of 4 warps are
-      uint32_t any = 0u;
-#pragma unroll
-      for (int i = 0; i < NW; ++i) any |= und4[i] | und8[i];
-      if (__all_sync(0xffffffffu, any == 0u)) break;
+      cmp_block(und[i], v[i], w, ge1[i], sa.a + 4 * c, sa.b + 4 * c);
     }
   }
+  for (;;) {
+    int sel = -1;
 #pragma unroll
-  for (int i = 0; i < NW; ++i) flip[i] = ge2[i] | (~v4[i] & ~und4[i]) | (~v8[i] & ~und8[i]);
+    for (int i = NW - 1; i >= 0; --i)
+      if (und[i] != 0u) sel = i;
+    if (!__any_sync(0xffffffffu, sel >= 0)) break;
+    uint32_t s_und = 0u, s_v = 0u, s_ge1 = 0u, s_call = 0u, s_c = 2u;
+#pragma unroll
+    for (int i = 0; i < NW; ++i)
+      if (sel == i) {
+        s_und = und[i]; s_v = v[i]; s_ge1 = ge1[i]; s_call = call0[i]; s_c = nxt[i];
+      }
+    const uint4 w = philox4x32_10(slot, s_call + s_c, c2, c3, key);
+    cmp_block(s_und, s_v, w, s_ge1, sa.a + 4u * s_c, sa.b + 4u * s_c);
+    if (s_c == 7u) {  // all 32 bits equal: u == T is not less
+      s_v |= s_und;
+      s_und = 0u;
+    }
+#pragma unroll
+    for (int i = 0; i < NW; ++i)
+      if (sel == i) {
+        und[i] = s_und; v[i] = s_v; nxt[i] = s_c + 1u;
+      }
+  }
+#pragma unroll
+  for (int i = 0; i < NW; ++i) flip[i] = ge2[i] | ~v[i];
 }
 
 // masks of the sites with a >= 1 and a >= 2 from the four difference words (1 = anti-aligned)
@@ -119,7 +147,6 @@ struct Geo {
   static constexpr int WPP = HB / 32;             // words per row plane
   static constexpr int WR = L / 32;               // raw words per row
   static constexpr int WREP = N / 32;             // words per replica
-  static constexpr int NWB = 2;                   // plane words whose Philox chains run interleaved
 };
 
 template <int L>
@@ -173,19 +200,10 @@ __device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot
       call0[r * G_::WPP + i] = 8u * ((uint32_t)y * G_::WPP + (uint32_t)i);  // group = y * WPP + i
     }
   }
+  uint32_t flip[NWL];
+  lazy_accept<NWL>(ge1, ge2, slot, call0, c2, c3, key, sa, flip);
 #pragma unroll
-  for (int w0 = 0; w0 < NWL; w0 += G_::NWB) {
-    uint32_t a1[G_::NWB], a2[G_::NWB], cc[G_::NWB], flip[G_::NWB];
-#pragma unroll
-    for (int j = 0; j < G_::NWB; ++j) {
-      a1[j] = ge1[w0 + j];
-      a2[j] = ge2[w0 + j];
-      cc[j] = call0[w0 + j];
-    }
-    lazy_accept<G_::NWB>(a1, a2, slot, cc, c2, c3, key, sa, flip);
-#pragma unroll
-    for (int j = 0; j < G_::NWB; ++j) T[(w0 + j) / G_::WPP][(w0 + j) % G_::WPP] ^= flip[j];
-  }
+  for (int w = 0; w < NWL; ++w) T[w / G_::WPP][w % G_::WPP] ^= flip[w];
 }
 
 // number of anti-aligned bonds u (each bond has exactly one colour-0 end) and number of up spins
