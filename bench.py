@@ -26,9 +26,16 @@ if ROOT not in sys.path:
 
 from paper_2006_00561_b200 import inputs  # noqa: E402
 
-I_MIN = 12.0          # algorithmic lane-instructions per flip attempt
-WIDE_PER_ATTEMPT = 4.5  # 32x32->64 multiplies per attempt that cannot be hoisted (18 per Philox block of 4 sites)
-SM_COUNT, SMSP, LANES = 148, 4, 32
+# Roofline of the sweep kernel: bound by the integer ALU pipe, 16 lanes/clk/SMSP
+# (B300_MICROARCH.md "alu-pipe ... rt_SMSP=2"; LOP3 measured at 2.03 cycles per warp instruction on B200).
+# Algorithmic ALU lane-operations per flip attempt of the bit-sliced lazy comparator (reading G20), per plane word of
+# 32 sites:  E_BLK Philox blocks x (19 LOP3 of Philox4x32-10 with the loop-invariant first round hoisted + 12 LOP3 of
+# the comparator) + 12 for the neighbour classes and the flip;  E_BLK = 2 + sum_{c>=2} [1 - (1 - 2^-4c)^32] = 2.126
+# blocks that a (lane, word) pair needs when every site of the word needs a uniform.
+E_BLK = 2.0 + sum(1.0 - (1.0 - 2.0 ** (-4 * c)) ** 32 for c in range(2, 8))
+ALU_OPS_PER_ATTEMPT = (E_BLK * (19 + 12) + 12) / 32.0
+I_MIN_SURVEY = 12.0   # one 32-bit Philox word per attempt at 1 warp-instr/clk/SMSP (kept for continuity)
+SM_COUNT, SMSP, LANES, ALU_LANES = 148, 4, 32, 16
 
 
 def measured_peaks():
@@ -123,7 +130,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     wl = inputs.CONFIGS[args.config]
-    R_sample = 2048
+    R_sample = 4096
     r = oracle_sample_run(wl, R_sample, args.steps, args.warmup)
     value = r["attempts"] / r["seconds"]
     sample = "oracle on %s at R=%d (same L, dbeta, theta, P), %d steps" % (wl.name, R_sample, args.steps)
@@ -259,15 +266,18 @@ def run_ours(args):
     if wl.theta > 0 and sweep_n > 0:
         attempts_per_launch = units / sweep_n
         sweep_rate = attempts_per_launch / (sweep_ms / sweep_n * 1e-3)  # attempts/s inside the kernel
-        achieved = sweep_rate * I_MIN / 1e12
-        peak = SM_COUNT * SMSP * LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
-        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-instr/s (12 per flip attempt)",
+        achieved = sweep_rate * ALU_OPS_PER_ATTEMPT / 1e12
+        peak = SM_COUNT * SMSP * ALU_LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak,
+                "unit": "T ALU-pipe lane-ops/s (%.3f algorithmic per flip attempt)" % ALU_OPS_PER_ATTEMPT,
                 "frac": achieved / peak, "traffic": None, "kernel": "k_sweep<%d>" % wl.L,
                 "kernel_attempts_per_s": sweep_rate, "kernel_ms_per_launch": sweep_ms / sweep_n,
                 "kernel_share_of_step": sweep_ms / step_kernel_ms,
-                "peak_src": "148 SM x 4 SMSP x 32 lanes x %d MHz (clocks.max.sm), 1 warp-instr/clk/SMSP" % peaks["sm_max_mhz"]}
+                "peak_src": "148 SM x 4 SMSP x 16 ALU lanes x %d MHz (clocks.max.sm)" % peaks["sm_max_mhz"],
+                "frac_survey_12_instr_per_attempt_at_issue_rate":
+                    sweep_rate * I_MIN_SURVEY / (SM_COUNT * SMSP * LANES * peaks["sm_max_mhz"] * 1e6)}
         if clocks.get("sm_mhz"):
-            roof["frac_at_measured_clock"] = achieved / (SM_COUNT * SMSP * LANES * clocks["sm_mhz"] * 1e6 / 1e12)
+            roof["frac_at_measured_clock"] = achieved / (SM_COUNT * SMSP * ALU_LANES * clocks["sm_mhz"] * 1e6 / 1e12)
     else:
         roof = None
     per_kernel = {k: {"ms_total": v[0], "launches": v[1]} for k, v in prof.items()}
@@ -289,7 +299,7 @@ def run_ours(args):
         if not args.no_resample:
             resample = resample_leg(binding, torch, peaks, repeats=args.resample_repeats)
         if not args.no_cpu_baseline:
-            r = oracle_sample_run(wl, 2048, 24, 1)
+            r = oracle_sample_run(wl, 4096, 24, 1)
             cpu = {"value": r["attempts"] / r["seconds"], "unit": "attempts/s", "cores": r["cores"], "kind": "oracle",
                    "sample": "%s at R=%d (same L, dbeta, theta, P), %d steps, %.1f s" % (wl.name, r["R_sample"], r["steps"], r["seconds"])}
     if g.is_main:

@@ -22,6 +22,20 @@
 #pragma once
 #include "pa_common.cuh"
 
+// tuning knobs (defaults are the measured best on B200)
+#ifndef PA_SWEEP_THREADS
+#define PA_SWEEP_THREADS 256
+#endif
+#ifndef PA_SWEEP_MINB64
+#define PA_SWEEP_MINB64 3
+#endif
+#ifndef PA_SWEEP_MINB128
+#define PA_SWEEP_MINB128 2
+#endif
+#ifndef PA_SWEEP_STAGE1
+#define PA_SWEEP_STAGE1 2
+#endif
+
 namespace pa {
 
 // threshold bits as all-ones / all-zeros masks, most significant bit first (host-filled kernel argument: the
@@ -85,10 +99,10 @@ __device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uin
   for (int i = 0; i < NW; ++i) {
     und[i] = ~ge2[i];
     v[i] = 0xffffffffu;
-    nxt[i] = 2u;
+    nxt[i] = (uint32_t)PA_SWEEP_STAGE1;
   }
 #pragma unroll
-  for (int c = 0; c < 2; ++c) {
+  for (int c = 0; c < PA_SWEEP_STAGE1; ++c) {
 #pragma unroll
     for (int i = 0; i < NW; ++i) {
       const uint4 w = philox4x32_10(slot, call0[i] + (uint32_t)c, c2, c3, key);
@@ -133,7 +147,7 @@ __device__ __forceinline__ void neighbour_classes(uint32_t tt, uint32_t U, uint3
   ge1 = any3 | d3;
 }
 
-constexpr int SWEEP_THREADS = 256;
+constexpr int SWEEP_THREADS = PA_SWEEP_THREADS;
 
 // =====================================================================================================
 // L >= 64
@@ -265,7 +279,7 @@ __device__ __forceinline__ void planes_to_row(const uint32_t (&p0)[Geo<L>::WPP],
 }
 
 template <int L>
-__global__ void __launch_bounds__(SWEEP_THREADS, (L >= 128 ? 2 : 3))
+__global__ void __launch_bounds__(SWEEP_THREADS, (L >= 128 ? PA_SWEEP_MINB128 : PA_SWEEP_MINB64))
 k_sweep(const DevState* __restrict__ st, uint32_t* __restrict__ spins0, uint32_t* __restrict__ spins1,
         int32_t* __restrict__ E0, int32_t* __restrict__ E1, int32_t* __restrict__ M0, int32_t* __restrict__ M1,
         const PhiloxKey key, const SweepArgs sa) {
