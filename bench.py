@@ -219,6 +219,42 @@ def e2e_leg(pa, torch, wl, first_step, steps):
     return {"attempts": attempts, "seconds": dt, "h2d_bytes_per_step": h2d // steps, "d2h_bytes_per_step": d2h // steps}
 
 
+# exact ln Z of the L x L torus at the final temperature of configs 1-4 (Kaufman closed form, 30 digits by mpmath:
+# tests/golden/ising_exact.json, written by tests/golden/make_ising_exact.py; SURVEY.md 8(c) "Reference values")
+EXACT_LNZ = {1: 128.715437337408418, 2: 2049.04978969008727, 3: 4202.34050797894262, 4: 19827.5021968979168}
+
+
+def anneal_leg(binding, torch, configs):
+    """BASELINE.json metric "anneal wall time": the whole schedule of a config queued with ONE pa_run call (no host
+    round trip between steps), timed with CUDA events on the stream and with the host clock around the call."""
+    out = []
+    for ci in configs:
+        wl = inputs.CONFIGS[ci]
+        pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0)
+        betas = [wl.beta(k) for k in range(1, wl.K + 1)]
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ev0.record(pa.stream)
+        done = pa.run(betas, wl.theta)
+        ev1.record(pa.stream)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        sec = ev0.elapsed_time(ev1) * 1e-3
+        rs = pa.replica_steps()
+        lz = pa.log_Z()["lnZ"]
+        ob = pa.observables()
+        out.append({"workload": wl.name, "steps_done": done, "K": wl.K, "theta": wl.theta, "seconds_device": sec,
+                    "seconds_wall": wall, "replica_steps": rs, "attempts_per_s": wl.theta * wl.N * rs / sec,
+                    "replica_steps_per_s": rs / sec, "R_final": pa.R, "lnZ": lz, "lnZ_exact": EXACT_LNZ.get(ci),
+                    "lnZ_minus_exact_per_spin": (lz - EXACT_LNZ[ci]) / wl.N if ci in EXACT_LNZ else None,
+                    "mean_E_per_spin": ob["mean_E"] / wl.N, "mean_absM_per_spin": ob["mean_absM"] / wl.N,
+                    "launches": pa.launch_count()})
+        del pa
+        torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(args):
     import torch
     from paper_2006_00561_b200 import binding, dist
@@ -328,14 +364,23 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-resample", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--leg", default="all", choices=["all", "resample"],
-                    help="'resample': only the config-5 resampling/redistribution leg (short; used for ncu captures)")
+    ap.add_argument("--leg", default="all", choices=["all", "resample", "anneal"],
+                    help="'resample': only the config-5 resampling/redistribution leg (short; used for ncu captures); "
+                         "'anneal': whole anneals of --anneal-configs (wall time, ln Z against the exact value)")
+    ap.add_argument("--anneal-configs", default="1,2,3,4")
     ap.add_argument("--resample-repeats", type=int, default=5)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3  # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         return run_reference(args)
+    if args.leg == "anneal":
+        import torch
+        from paper_2006_00561_b200 import binding
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+        print(json.dumps({"anneal": anneal_leg(binding, torch, [int(x) for x in args.anneal_configs.split(",")])}))
+        return 0
     if args.leg == "resample":
         import torch
         from paper_2006_00561_b200 import binding

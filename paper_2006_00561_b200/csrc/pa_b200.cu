@@ -20,7 +20,7 @@ namespace {
 
 constexpr int RUN_CHUNK = 1024;  // step-parameter slots uploaded per pa_run chunk
 constexpr int RED_GRID = 148 * 4;
-constexpr int OBS_GRID = 148 * 2;
+constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
   uint64_t state, params, spins[2], E[2], M[2], off, n, tau, tile_desc, tile_parent, red_partial, obs_partial,

@@ -58,19 +58,41 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   const unsigned long long count = mode == 0 ? st->Rnew : st->R;
   const int32_t* __restrict__ E = buf ? E1 : E0;
   const int32_t* __restrict__ M = buf ? M1 : M0;
-  U128 acc[OBS_Q];
-#pragma unroll
-  for (int q = 0; q < OBS_Q; ++q) acc[q] = {0ull, 0ull};
+  // per-thread partial sums: a thread sees at most cap / (grid * 256) < 2^17 replicas, |E| <= 2^15, |M| <= 2^14, so
+  // sum E, sum E^2 (< 2^47), sum |M|, sum M^2 fit 64 bits; only M^4 (< 2^56 each) needs the 128-bit accumulator.
+  long long sE = 0;
+  unsigned long long sE2 = 0, sA = 0, sM2 = 0;
+  U128 sM4 = {0ull, 0ull};
+  auto add = [&](int ei, int mi) {
+    const long long e = ei;
+    const unsigned long long am = (unsigned long long)(mi < 0 ? -mi : mi), m2 = am * am;
+    sE += e;
+    sE2 += (unsigned long long)(e * e);
+    sA += am;
+    sM2 += m2;
+    u128_add(sM4, m2 * m2, 0ull);
+  };
+  const unsigned long long nvec = count / 4, tid = (unsigned long long)blockIdx.x * OBS_THREADS + threadIdx.x;
   const unsigned long long stride = (unsigned long long)gridDim.x * OBS_THREADS;
-  for (unsigned long long j = (unsigned long long)blockIdx.x * OBS_THREADS + threadIdx.x; j < count; j += stride) {
-    const long long e = E[j], m = M[j];
-    const unsigned long long am = (unsigned long long)(m < 0 ? -m : m);
-    u128_add(acc[0], (unsigned long long)e, e < 0 ? ~0ull : 0ull);  // sign-extended
-    u128_add(acc[1], (unsigned long long)(e * e), 0ull);
-    u128_add(acc[2], am, 0ull);
-    u128_add(acc[3], am * am, 0ull);
-    u128_add(acc[4], am * am * am * am, 0ull);  // |M| <= 2^14 -> < 2^56
+  const int4* __restrict__ E4 = reinterpret_cast<const int4*>(E);  // buffers are 256-byte aligned
+  const int4* __restrict__ M4 = reinterpret_cast<const int4*>(M);
+  unsigned long long v = tid;
+  for (; v + stride < nvec; v += 2 * stride) {  // 64 bytes in flight per thread
+    const int4 e0 = __ldg(E4 + v), m0 = __ldg(M4 + v), e1 = __ldg(E4 + v + stride), m1 = __ldg(M4 + v + stride);
+    add(e0.x, m0.x); add(e0.y, m0.y); add(e0.z, m0.z); add(e0.w, m0.w);
+    add(e1.x, m1.x); add(e1.y, m1.y); add(e1.z, m1.z); add(e1.w, m1.w);
   }
+  for (; v < nvec; v += stride) {
+    const int4 e0 = __ldg(E4 + v), m0 = __ldg(M4 + v);
+    add(e0.x, m0.x); add(e0.y, m0.y); add(e0.z, m0.z); add(e0.w, m0.w);
+  }
+  for (unsigned long long j = 4 * nvec + tid; j < count; j += stride) add(E[j], M[j]);
+  U128 acc[OBS_Q];
+  acc[0] = {(unsigned long long)sE, sE < 0 ? ~0ull : 0ull};  // sign-extended
+  acc[1] = {sE2, 0ull};
+  acc[2] = {sA, 0ull};
+  acc[3] = {sM2, 0ull};
+  acc[4] = sM4;
   __shared__ U128 s_part[OBS_THREADS / 32][OBS_Q];
   __shared__ bool s_last;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;

@@ -63,16 +63,24 @@ k_q_reduce(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restri
   const int32_t* __restrict__ E = st->cur ? E1 : E0;
   const unsigned long long R = st->R;
   double acc = 0.0;
-  // four independent loads in flight per thread
+  // 128-bit loads of E (the buffers are 256-byte aligned), two in flight per thread; the 8 table look-ups hit L1
   const unsigned long long stride = (unsigned long long)gridDim.x * RED_THREADS;
-  unsigned long long j = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x;
-  for (; j + 3 * stride < R; j += 4 * stride) {
-    const int e0 = E[j], e1 = E[j + stride], e2 = E[j + 2 * stride], e3 = E[j + 3 * stride];
-    const double w0 = tb.w[(e0 + 2 * N) >> 2], w1 = tb.w[(e1 + 2 * N) >> 2];
-    const double w2 = tb.w[(e2 + 2 * N) >> 2], w3 = tb.w[(e3 + 2 * N) >> 2];
-    acc += (w0 + w1) + (w2 + w3);
+  const unsigned long long tid = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x, nvec = R / 4;
+  const int4* __restrict__ E4 = reinterpret_cast<const int4*>(E);
+  const int twoN = 2 * N;
+  unsigned long long v = tid;
+  for (; v + stride < nvec; v += 2 * stride) {
+    const int4 a = __ldg(E4 + v), b = __ldg(E4 + v + stride);
+    const double w0 = tb.w[(a.x + twoN) >> 2], w1 = tb.w[(a.y + twoN) >> 2], w2 = tb.w[(a.z + twoN) >> 2],
+                 w3 = tb.w[(a.w + twoN) >> 2], w4 = tb.w[(b.x + twoN) >> 2], w5 = tb.w[(b.y + twoN) >> 2],
+                 w6 = tb.w[(b.z + twoN) >> 2], w7 = tb.w[(b.w + twoN) >> 2];
+    acc += ((w0 + w1) + (w2 + w3)) + ((w4 + w5) + (w6 + w7));
   }
-  for (; j < R; j += stride) acc += tb.w[(E[j] + 2 * N) >> 2];
+  for (; v < nvec; v += stride) {
+    const int4 a = __ldg(E4 + v);
+    acc += (tb.w[(a.x + twoN) >> 2] + tb.w[(a.y + twoN) >> 2]) + (tb.w[(a.z + twoN) >> 2] + tb.w[(a.w + twoN) >> 2]);
+  }
+  for (unsigned long long j = 4 * nvec + tid; j < R; j += stride) acc += tb.w[(E[j] + twoN) >> 2];
 
   __shared__ double s_part[RED_THREADS / 32];
   __shared__ bool s_last;
