@@ -130,7 +130,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     wl = inputs.CONFIGS[args.config]
-    R_sample = 4096
+    R_sample = min(4096, wl.R0)
     r = oracle_sample_run(wl, R_sample, args.steps, args.warmup)
     value = r["attempts"] / r["seconds"]
     sample = "oracle on %s at R=%d (same L, dbeta, theta, P), %d steps" % (wl.name, R_sample, args.steps)

@@ -290,6 +290,32 @@ def test_capacity_error_leaves_population_unchanged():
     assert g.beta_steps()[1] == 59 - failures
 
 
+def test_extinction_matches_the_oracle_and_leaves_population_unchanged():
+    """degenerate case R' = 0 (PA_EEXTINCT): R0 = 2 replicas die out with probability e^-2 per step; the first seed on
+    which the ORACLE goes extinct must make the GPU fail at the same step, with nothing committed"""
+    b = _binding()
+    hit = None
+    for seed in range(40):
+        ora = orc.OraclePA(8, 2, seed=seed)
+        try:
+            for k in range(1, 6):
+                ora.step(0.01 * k, 1)
+        except orc.OracleError:
+            hit = (seed, k)
+            break
+    assert hit is not None
+    seed, kfail = hit
+    g = b.PopulationAnnealer(8, 2, seed=seed)
+    for k in range(1, kfail):
+        g.step(0.01 * k, 1)
+    before, R_before, lz, bs = g.spins(), g.R, g.log_Z(), g.beta_steps()
+    with pytest.raises(b.PaError) as ei:
+        g.step(0.01 * kfail, 1)
+    assert ei.value.code == b.PA_EEXTINCT
+    assert g.R == R_before and np.array_equal(g.spins(), before) and g.log_Z() == lz and g.beta_steps() == bs
+    assert np.array_equal(before, ora.spins) and R_before == ora.R  # oracle state is also the pre-step one
+
+
 def test_invalid_arguments():
     b = _binding()
     with pytest.raises(b.PaError):
