@@ -86,11 +86,11 @@ typedef struct {
 
 /* kernels of one pa_step, in launch order (indices of pa_profile_read arrays) */
 enum {
-  PA_K_LEVELS_W = 0, /* w_e = exp(-dbeta e) per energy level */
+  PA_K_LEVELS_W = 0, /* (w_e = exp(-dbeta e) per level is tabulated inside PA_K_Q_REDUCE: reports 0 launches) */
   PA_K_Q_REDUCE,     /* eq. 3: fp64 warp-shuffle reduction, Q, ln Q */
   PA_K_LEVELS_TAU,   /* eq. 4 per level + Poisson chunk tables */
   PA_K_POISSON_SCAN, /* Poisson copy counts + single-pass exclusive scan */
-  PA_K_BALANCE,      /* partition table + diagnostics: fused into PA_K_POISSON_SCAN (last tile), reports 0 launches */
+  PA_K_BALANCE,      /* partition table + diagnostics: run by block 0 of PA_K_COPY, reports 0 launches */
   PA_K_COPY,         /* replica redistribution (gather copy) */
   PA_K_SWEEP,        /* theta checkerboard Metropolis sweeps + E, M */
   PA_K_OBSERVE,      /* population sums + commit of the step */

@@ -24,7 +24,7 @@ constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
   uint64_t state, params, spins[2], E[2], M[2], off, n, tau, tile_desc, tile_parent, red_partial, obs_partial,
-      lev_w, lev_tau, lev_mu, lev_m, lev_cdf, part[2], part_stats, total;
+      lev_tau, lev_mu, lev_m, lev_cdf, part[2], part_stats, total;
 };
 
 inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
@@ -77,8 +77,7 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   lo->tile_desc = take(((ucap + SCAN_TILE - 1) / SCAN_TILE + 1) * 8);
   lo->tile_parent = take((ucap / copy_tile_for(c->L) + 2) * 4);
   lo->red_partial = take(RED_GRID * 8);
-  lo->obs_partial = take((uint64_t)OBS_GRID * 10 * 8);
-  lo->lev_w = take(nlev * 8);
+  lo->obs_partial = take((uint64_t)OBS_GRID * 12 * 8);
   lo->lev_tau = take(nlev * 8);
   lo->lev_mu = take(nlev * 8);
   lo->lev_m = take(nlev * 4);
@@ -111,6 +110,7 @@ struct pa_ctx {
   double beta, sum_lnQ, last_Q;
   int64_t launches;
   bool profile;
+  int scan_grid_max;  // co-resident blocks of k_poisson_scan on this device
   std::vector<EventPair> ev_used, ev_free;
   std::string err;
 
@@ -158,7 +158,6 @@ struct Prof {  // records an event pair around one launch when profiling is on
 
 LevelTables tables(pa_ctx* c) {
   LevelTables t;
-  t.w = c->dev<double>(c->lo.lev_w);
   t.tau = c->dev<double>(c->lo.lev_tau);
   t.mu = c->dev<double>(c->lo.lev_mu);
   t.m = c->dev<uint32_t>(c->lo.lev_m);
@@ -213,7 +212,9 @@ void launch_copy_L(pa_ctx* c) {
   int32_t *e0 = c->dev<int32_t>(c->lo.E[0]), *e1 = c->dev<int32_t>(c->lo.E[1]);
   int32_t *m0 = c->dev<int32_t>(c->lo.M[0]), *m1 = c->dev<int32_t>(c->lo.M[1]);
   k_copy<L><<<grid, COPY_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), c->dev<uint32_t>(c->lo.off),
-                                                  c->dev<uint32_t>(c->lo.tile_parent), s0, s1, e0, e1, m0, m1);
+                                                  c->dev<uint32_t>(c->lo.tile_parent), s0, s1, e0, e1, m0, m1,
+                                                  c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]),
+                                                  c->dev<uint32_t>(c->lo.part_stats), c->cfg.P);
 }
 void launch_copy(pa_ctx* c) {
   Prof p(c, PA_K_COPY);
@@ -231,7 +232,7 @@ void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
   k_observe<<<OBS_GRID, OBS_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.E[0]),
                                                      c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]),
                                                      c->dev<int32_t>(c->lo.M[1]),
-                                                     c->dev<unsigned long long>(c->lo.obs_partial), mode);
+                                                     c->dev<unsigned long long>(c->lo.obs_partial), mode, c->N);
 }
 
 // all kernels of one temperature step, parameters in device slot sp
@@ -243,25 +244,28 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   const int n_desc = (int)((c->cap + SCAN_TILE - 1) / SCAN_TILE + 1);
   const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
   {
-    Prof p(c, PA_K_LEVELS_W);
-    const int threads = 256, work = (N + 1 > n_desc ? N + 1 : n_desc);
-    k_levels_w<<<(work + threads - 1) / threads, threads, 0, c->stream>>>(
-        st, sp, tb, N, c->dev<unsigned long long>(c->lo.tile_desc), n_desc);
+    Prof p(c, PA_K_Q_REDUCE);  // also resets the step's counters and look-back descriptors
+    k_q_reduce<<<RED_GRID, RED_THREADS, 0, c->stream>>>(st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
+                                                        (double)c->cfg.R0,
+                                                        c->dev<unsigned long long>(c->lo.tile_desc), n_desc);
   }
   {
-    Prof p(c, PA_K_Q_REDUCE);
-    k_q_reduce<<<RED_GRID, RED_THREADS, 0, c->stream>>>(st, E0, E1, tb, N, c->dev<double>(c->lo.red_partial),
-                                                        (double)c->cfg.R0);
-  }
-  {
-    Prof p(c, PA_K_LEVELS_TAU);
-    k_levels_tau<<<(N + 1 + 127) / 128, 128, 0, c->stream>>>(st, tb, N);
+    Prof p(c, PA_K_LEVELS_TAU);  // the window of occupied levels is on the device: launch for all N + 1
+    k_levels_tau<<<(N + 1 + 127) / 128, 128, 0, c->stream>>>(st, sp, tb, N);
   }
   {
     Prof p(c, PA_K_POISSON_SCAN);  // includes a5 (partition balance), run by the last tile to finish
-    // persistent blocks pull tiles from a ticket counter (5 blocks of 48 registers x 256 threads fit one SM)
+    // persistent blocks pull tiles from a ticket counter
     const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
-    const unsigned grid = tiles_cap < 148u * 5u ? tiles_cap : 148u * 5u;
+    const bool keep = c->lo.n || c->lo.tau;
+    if (c->scan_grid_max == 0) {  // all blocks co-resident: blocks per SM (occupancy) x SMs
+      int per_sm = 0, sms = 0;
+      if (keep) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true>, SCAN_THREADS, 0);
+      else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<false>, SCAN_THREADS, 0);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+      c->scan_grid_max = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
+    }
+    const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? tiles_cap : (unsigned)c->scan_grid_max;
     ScanOut out;
     out.off = c->dev<uint32_t>(c->lo.off);
     out.n = c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr;
@@ -271,7 +275,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     out.part0 = c->dev<uint32_t>(c->lo.part[0]);
     out.part1 = c->dev<uint32_t>(c->lo.part[1]);
     out.part_stats = c->dev<uint32_t>(c->lo.part_stats);
-    if (out.n || out.tau)
+    if (keep)
       k_poisson_scan<true><<<grid, SCAN_THREADS, 0, c->stream>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
                                                                    (unsigned long long)c->cap, c->cfg.P, c->key);
     else
@@ -403,6 +407,7 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   c->stream = static_cast<cudaStream_t>(cfg->stream);
   c->profile = (cfg->flags & PA_PROFILE) != 0;
   c->launches = 0;
+  c->scan_grid_max = 0;
   uint32_t k0 = (uint32_t)(cfg->seed & 0xffffffffull), k1 = (uint32_t)(cfg->seed >> 32);
   for (int r = 0; r < 10; ++r) {
     c->key.k0[r] = k0;

@@ -29,13 +29,13 @@ struct DevState {
   unsigned int cur;              // index of the buffer holding the current population
   unsigned int status;           // 0 = ok, else -pa_status of the failing step
   unsigned int fail_step;        // ordinal of the step that failed
-  unsigned int reduce_done;      // block counters (reset every step by k_levels_w)
+  unsigned int reduce_done;      // block counters (reset every step by k_q_reduce)
   unsigned int scan_tile;
-  unsigned int scan_done;        // tiles of k_poisson_scan that have written their outputs
   unsigned int scan_overflow;    // a parent sat on a level with lambda >= 2^31
   unsigned int obs_done;
   unsigned int T4, T8;           // thresholds of the last committed step with theta > 0
-  unsigned int pad_[3];
+  int lev_lo, lev_hi;            // occupied energy levels (E + 2N)/4 of the CURRENT population, inclusive (by k_observe)
+  unsigned int pad_[1];
 };
 
 struct StepParams {

@@ -52,7 +52,7 @@ constexpr int OBS_Q = 5;  // sum E (two's complement), sum E^2, sum |M|, sum M^2
 __global__ void __launch_bounds__(OBS_THREADS)
 k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
           const int32_t* __restrict__ E1, const int32_t* __restrict__ M0, const int32_t* __restrict__ M1,
-          unsigned long long* __restrict__ partial /* [grid][10] */, const int mode) {
+          unsigned long long* __restrict__ partial /* [grid][12] */, const int mode, const int N) {
   if (st->status != ST_OK) return;
   const unsigned buf = mode == 0 ? (st->cur ^ 1u) : st->cur;
   const unsigned long long count = mode == 0 ? st->Rnew : st->R;
@@ -63,7 +63,10 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   long long sE = 0;
   unsigned long long sE2 = 0, sA = 0, sM2 = 0;
   U128 sM4 = {0ull, 0ull};
+  int emin = 0x7fffffff, emax = -0x7fffffff;  // occupied energy range: the level window of the next step's tables
   auto add = [&](int ei, int mi) {
+    emin = min(emin, ei);
+    emax = max(emax, ei);
     const long long e = ei;
     const unsigned long long am = (unsigned long long)(mi < 0 ? -mi : mi), m2 = am * am;
     sE += e;
@@ -94,6 +97,7 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   acc[3] = {sM2, 0ull};
   acc[4] = sM4;
   __shared__ U128 s_part[OBS_THREADS / 32][OBS_Q];
+  __shared__ int s_emin[OBS_THREADS / 32], s_emax[OBS_THREADS / 32];
   __shared__ bool s_last;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
@@ -101,12 +105,30 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
     const U128 v = warp_sum_u128(acc[q]);
     if (lane == 0) s_part[warp][q] = v;
   }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    emin = min(emin, __shfl_xor_sync(0xffffffffu, emin, o));
+    emax = max(emax, __shfl_xor_sync(0xffffffffu, emax, o));
+  }
+  if (lane == 0) {
+    s_emin[warp] = emin;
+    s_emax[warp] = emax;
+  }
   __syncthreads();
   if (threadIdx.x < OBS_Q) {
     U128 t = {0ull, 0ull};
     for (int w = 0; w < OBS_THREADS / 32; ++w) u128_add(t, s_part[w][threadIdx.x].lo, s_part[w][threadIdx.x].hi);
-    partial[(size_t)blockIdx.x * 10 + 2 * threadIdx.x] = t.lo;
-    partial[(size_t)blockIdx.x * 10 + 2 * threadIdx.x + 1] = t.hi;
+    partial[(size_t)blockIdx.x * 12 + 2 * threadIdx.x] = t.lo;
+    partial[(size_t)blockIdx.x * 12 + 2 * threadIdx.x + 1] = t.hi;
+  }
+  if (threadIdx.x == OBS_Q) {
+    int lo = s_emin[0], hi = s_emax[0];
+    for (int w = 1; w < OBS_THREADS / 32; ++w) {
+      lo = min(lo, s_emin[w]);
+      hi = max(hi, s_emax[w]);
+    }
+    partial[(size_t)blockIdx.x * 12 + 10] = (unsigned long long)(long long)lo;
+    partial[(size_t)blockIdx.x * 12 + 11] = (unsigned long long)(long long)hi;
   }
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -120,11 +142,20 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   if (threadIdx.x < OBS_Q) {
     U128 t = {0ull, 0ull};
     for (unsigned b = 0; b < gridDim.x; ++b)
-      u128_add(t, __ldcg(&partial[(size_t)b * 10 + 2 * threadIdx.x]), __ldcg(&partial[(size_t)b * 10 + 2 * threadIdx.x + 1]));
+      u128_add(t, __ldcg(&partial[(size_t)b * 12 + 2 * threadIdx.x]), __ldcg(&partial[(size_t)b * 12 + 2 * threadIdx.x + 1]));
     st->obs[2 * threadIdx.x] = t.lo;
     st->obs[2 * threadIdx.x + 1] = t.hi;
   }
   if (threadIdx.x == 0) {
+    long long lo = 0x7fffffff, hi = -0x7fffffff;
+    for (unsigned b = 0; b < gridDim.x; ++b) {
+      const long long l = (long long)__ldcg(&partial[(size_t)b * 12 + 10]), h = (long long)__ldcg(&partial[(size_t)b * 12 + 11]);
+      lo = l < lo ? l : lo;
+      hi = h > hi ? h : hi;
+    }
+    if (lo > hi) lo = hi = -2 * N;  // empty population: cannot happen (R >= 1), keep the window valid
+    st->lev_lo = (int)((lo + 2 * N) >> 2);
+    st->lev_hi = (int)((hi + 2 * N) >> 2);
     st->obs_R = count;
     if (mode == 0) {  // commit: the new population becomes the current one
       st->R_parents = st->R;

@@ -14,41 +14,29 @@ constexpr int PO_ROW = 72;             // F_0 .. F_64 per level, padded to 72 do
 constexpr unsigned M_OVERFLOW = 0xffffffffu;
 
 struct LevelTables {
-  double* w;        // [N+1]  exp(-dbeta * e)
   double* tau;      // [N+1]  w / Q
   double* mu;       // [N+1]  lambda / m
   uint32_t* m;      // [N+1]  number of chunks (0: lambda <= 0; M_OVERFLOW: lambda >= 2^31)
   double* cdf;      // [N+1][65]  F_k of Poisson(mu) built by the A4 recurrence
 };
 
-// ---------------------------------------------------------------------------------------------------
-// k_levels_w: w_e = exp(-dbeta * e) for every level; also resets the per-step counters and the scan's
-// tile descriptors (it is the first kernel of every step).
-// ---------------------------------------------------------------------------------------------------
-__global__ void k_levels_w(DevState* st, const StepParams* sp, LevelTables tb, int N, unsigned long long* tile_desc,
-                           int n_desc) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx == 0) {
-    st->reduce_done = 0u;
-    st->scan_tile = 0u;
-    st->scan_done = 0u;
-    st->scan_overflow = 0u;
-    st->obs_done = 0u;
-  }
-  for (int i = idx; i < n_desc; i += gridDim.x * blockDim.x) tile_desc[i] = 0ull;
-  if (st->status != ST_OK) return;
-  if (idx <= N) {
-    const double e = (double)(4 * idx - 2 * N);
-    tb.w[idx] = exp(-sp->dbeta * e);
-  }
+// w_e = exp(-dbeta * e) of energy level lev (e = 4 lev - 2N): the ONE expression that k_q_reduce (eq. 3) and
+// k_levels_tau (eq. 4) both evaluate, so that tau = w / Q uses the very bits that were summed into Q
+__device__ __forceinline__ double level_weight(double dbeta, int lev, int N) {
+  const double e = (double)(4 * lev - 2 * N);
+  return exp(-dbeta * e);
 }
 
 // ---------------------------------------------------------------------------------------------------
-// k_q_reduce: eq. 3.  Grid-stride gather of w[level(E_j)], per-thread serial sum, warp-shuffle tree, block
-// partials; the last block to finish adds the partials in index order (deterministic for a given grid) and
-// writes sumw, Q = sumw / R, ln Q, scale = R0 / R.
+// k_q_reduce: eq. 3, first kernel of every step (it also resets the per-step counters and the scan's tile
+// descriptors).  The population occupies the levels lev_lo..lev_hi (found by k_observe when the population was
+// written); every block tabulates w for that window in shared memory (a few hundred exp per block), then: grid-stride
+// 128-bit loads of E, look-up, per-thread serial sum, warp-shuffle tree, block partials; the last block to finish adds
+// the partials in index order (deterministic for a given grid) and writes sumw, Q = sumw / R, ln Q, scale = R0 / R.
+// A window wider than QW_MAX levels (crafted test populations) evaluates exp per replica instead: same bits.
 // ---------------------------------------------------------------------------------------------------
 constexpr int RED_THREADS = 256;
+constexpr int QW_MAX = 2048;
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -57,30 +45,51 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 __global__ void __launch_bounds__(RED_THREADS)
-k_q_reduce(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
-           double* __restrict__ partial, double R0) {
+k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
+           const int32_t* __restrict__ E1, int N, double* __restrict__ partial, double R0,
+           unsigned long long* __restrict__ tile_desc, int n_desc) {
+  const unsigned long long tid = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x;
+  const unsigned long long stride = (unsigned long long)gridDim.x * RED_THREADS;
+  if (tid == 0) {  // counters of the later kernels of this step (reduce_done is reset by the last block below)
+    st->scan_tile = 0u;
+    st->scan_overflow = 0u;
+    st->obs_done = 0u;
+  }
+  for (unsigned long long i = tid; i < (unsigned long long)n_desc; i += stride) tile_desc[i] = 0ull;
   if (st->status != ST_OK) return;
   const int32_t* __restrict__ E = st->cur ? E1 : E0;
   const unsigned long long R = st->R;
-  double acc = 0.0;
-  // 128-bit loads of E (the buffers are 256-byte aligned), two in flight per thread; the 8 table look-ups hit L1
-  const unsigned long long stride = (unsigned long long)gridDim.x * RED_THREADS;
-  const unsigned long long tid = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x, nvec = R / 4;
-  const int4* __restrict__ E4 = reinterpret_cast<const int4*>(E);
+  const double dbeta = sp->dbeta;
+  const int lev_lo = st->lev_lo, W = st->lev_hi - lev_lo + 1;
   const int twoN = 2 * N;
-  unsigned long long v = tid;
-  for (; v + stride < nvec; v += 2 * stride) {
-    const int4 a = __ldg(E4 + v), b = __ldg(E4 + v + stride);
-    const double w0 = tb.w[(a.x + twoN) >> 2], w1 = tb.w[(a.y + twoN) >> 2], w2 = tb.w[(a.z + twoN) >> 2],
-                 w3 = tb.w[(a.w + twoN) >> 2], w4 = tb.w[(b.x + twoN) >> 2], w5 = tb.w[(b.y + twoN) >> 2],
-                 w6 = tb.w[(b.z + twoN) >> 2], w7 = tb.w[(b.w + twoN) >> 2];
-    acc += ((w0 + w1) + (w2 + w3)) + ((w4 + w5) + (w6 + w7));
+  const unsigned long long nvec = R / 4;
+  const int4* __restrict__ E4 = reinterpret_cast<const int4*>(E);  // the buffers are 256-byte aligned
+  __shared__ double s_w[QW_MAX];
+  double acc = 0.0;
+  if (W <= QW_MAX) {
+    for (int i = threadIdx.x; i < W; i += RED_THREADS) s_w[i] = level_weight(dbeta, lev_lo + i, N);
+    __syncthreads();
+    const int shift = twoN - 4 * lev_lo;  // level(E) - lev_lo = (E + 2N - 4 lev_lo) / 4
+    auto wl = [&](int e) { return s_w[(e + shift) >> 2]; };
+    unsigned long long v = tid;
+    for (; v + stride < nvec; v += 2 * stride) {  // two 128-bit loads in flight per thread
+      const int4 a = __ldg(E4 + v), b = __ldg(E4 + v + stride);
+      acc += ((wl(a.x) + wl(a.y)) + (wl(a.z) + wl(a.w))) + ((wl(b.x) + wl(b.y)) + (wl(b.z) + wl(b.w)));
+    }
+    for (; v < nvec; v += stride) {
+      const int4 a = __ldg(E4 + v);
+      acc += (wl(a.x) + wl(a.y)) + (wl(a.z) + wl(a.w));
+    }
+    for (unsigned long long j = 4 * nvec + tid; j < R; j += stride) acc += wl(E[j]);
+  } else {
+    auto wl = [&](int e) { return level_weight(dbeta, (e + twoN) >> 2, N); };
+    unsigned long long v = tid;
+    for (; v < nvec; v += stride) {
+      const int4 a = __ldg(E4 + v);
+      acc += (wl(a.x) + wl(a.y)) + (wl(a.z) + wl(a.w));
+    }
+    for (unsigned long long j = 4 * nvec + tid; j < R; j += stride) acc += wl(E[j]);
   }
-  for (; v < nvec; v += stride) {
-    const int4 a = __ldg(E4 + v);
-    acc += (tb.w[(a.x + twoN) >> 2] + tb.w[(a.y + twoN) >> 2]) + (tb.w[(a.z + twoN) >> 2] + tb.w[(a.w + twoN) >> 2]);
-  }
-  for (unsigned long long j = 4 * nvec + tid; j < R; j += stride) acc += tb.w[(E[j] + twoN) >> 2];
 
   __shared__ double s_part[RED_THREADS / 32];
   __shared__ bool s_last;
@@ -108,6 +117,7 @@ k_q_reduce(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restri
       st->Q = Q;
       st->lnQ = log(Q);
       st->scale = R0 / (double)R;
+      st->reduce_done = 0u;  // every block has arrived: ready for the next step
     }
   }
 }
@@ -132,11 +142,11 @@ __device__ __forceinline__ double expneg_a4(double mu) {
   return p;
 }
 
-__global__ void k_levels_tau(const DevState* st, LevelTables tb, int N) {
+__global__ void k_levels_tau(const DevState* st, const StepParams* __restrict__ sp, LevelTables tb, int N) {
   if (st->status != ST_OK) return;
-  const int lev = blockIdx.x * blockDim.x + threadIdx.x;
-  if (lev > N) return;
-  const double tau = __ddiv_rn(tb.w[lev], st->Q);
+  const int lev = st->lev_lo + blockIdx.x * blockDim.x + threadIdx.x;  // only the occupied window is ever looked up
+  if (lev > st->lev_hi || lev > N) return;
+  const double tau = __ddiv_rn(level_weight(sp->dbeta, lev, N), st->Q);
   const double lambda = __dmul_rn(tau, st->scale);
   tb.tau[lev] = tau;
   double* F = tb.cdf + (size_t)lev * PO_ROW;
@@ -157,11 +167,17 @@ __global__ void k_levels_tau(const DevState* st, LevelTables tb, int N) {
   tb.mu[lev] = mu;
   double p = expneg_a4(mu), Fk = p;
   F[0] = Fk;
-  for (int k = 1; k <= PO_KMAX; ++k) {
+  int k = 1;
+  for (; k <= PO_KMAX; ++k) {
     p = __ddiv_rn(__dmul_rn(p, mu), (double)k);
-    Fk = __dadd_rn(Fk, p);
-    F[k] = Fk;
+    const double Fn = __dadd_rn(Fk, p);
+    F[k] = Fn;
+    // past the mode (k > mu) p only shrinks: once it no longer moves F, no later term does (identical bits, fewer
+    // dependent divisions)
+    if (Fn == Fk && (double)k > mu) break;
+    Fk = Fn;
   }
+  for (++k; k <= PO_KMAX; ++k) F[k] = Fk;
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -209,7 +225,7 @@ __device__ __forceinline__ unsigned draw_chunk(const double* __restrict__ F, uin
   return cdf_search_from(reinterpret_cast<const double2*>(F), 0, chunk_uniform(w, (unsigned)(c & 1ull)));
 }
 
-// a5 (defined below); run by the last tile of k_poisson_scan to finish
+// a5 (defined below); run by block 0 of k_copy
 __device__ void balance_tile(DevState* st, const uint32_t* off, uint32_t* part0, uint32_t* part1, uint32_t* stats, int P);
 
 struct ScanOut {
@@ -222,6 +238,7 @@ struct ScanOut {
 };
 
 constexpr int SCAN_BATCH = 4;  // independent Philox chains in flight per thread
+constexpr int SCAN_HW = 256;   // levels whose first CDF group is cached in shared memory
 constexpr unsigned NO_TILE = 0xffffffffu;
 
 // The kernel is software-pipelined over tiles: a block draws the counts of tile B and publishes its aggregate BEFORE it
@@ -229,18 +246,28 @@ constexpr unsigned NO_TILE = 0xffffffffu;
 // A tiles, 32 per round trip) is hidden behind B's sampling.  Every ticket holder publishes its aggregate before it
 // waits on anything, so the look-back cannot deadlock.
 template <bool KEEP>
-__global__ void __launch_bounds__(SCAN_THREADS)
+__global__ void __launch_bounds__(SCAN_THREADS, 5)
 k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
                ScanOut out, int copy_shift, unsigned long long capacity, int P, const PhiloxKey key) {
   if (st->status != ST_OK) return;
   __shared__ unsigned s_tile;
-  __shared__ unsigned s_flag;            // bit 0: a parent sits on an overflowing level; bit 1: this block finishes last
+  __shared__ unsigned s_flag;            // bit 0: a parent of this block sits on an overflowing level
   __shared__ unsigned long long s_pack;  // (total extra chunks << 12) | number of heavy parents   (one atomic sequence)
   __shared__ unsigned long long s_warp_tot[SCAN_THREADS / 32];
   __shared__ unsigned long long s_prefix;
   __shared__ __align__(16) unsigned s_cnt[2][SCAN_TILE];
-  __shared__ unsigned long long s_hstart[SCAN_TILE];  // first work-list position of heavy parent h
+  __shared__ uint32_t s_hstart[SCAN_TILE];  // first work-list position of heavy parent h (sum of lambda = R0 < 2^31: fits)
   __shared__ unsigned short s_hitem[SCAN_TILE];       // its item index inside the tile
+  // the first CDF group F_0..F_3 and the chunk count m of the first SCAN_HW occupied levels, in shared memory: almost every
+  // parent is decided by them (the population sits on a few hundred adjacent levels), the rest of a row stays in L1/L2
+  __shared__ __align__(16) double s_head[SCAN_HW][4];
+  __shared__ unsigned s_m[SCAN_HW];
+  const int lev_lo = st->lev_lo;
+  {
+    const int W = min(st->lev_hi - lev_lo + 1, SCAN_HW);
+    for (int i = threadIdx.x; i < 4 * W; i += SCAN_THREADS) s_head[i >> 2][i & 3] = tb.cdf[(size_t)(lev_lo + (i >> 2)) * PO_ROW + (i & 3)];
+    for (int i = threadIdx.x; i < W; i += SCAN_THREADS) s_m[i] = tb.m[lev_lo + i];
+  }
   const uint32_t R = (uint32_t)st->R;  // R <= capacity < 2^32 - 4096: parent indices fit 32 bits
   const unsigned ntiles = (R + SCAN_TILE - 1) / SCAN_TILE;
   const int32_t* __restrict__ E = st->cur ? E1 : E0;
@@ -275,10 +302,12 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
           jj[b] = tile_base + (r0 + b) * SCAN_THREADS + threadIdx.x;
           e[b] = (jj[b] < R) ? __ldg(E + jj[b]) : -2 * N;
         }
+        unsigned hl[SCAN_BATCH];  // level relative to the cached window (>= SCAN_HW: not cached)
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           const unsigned lev = (unsigned)((e[b] + 2 * N) >> 2);
-          m[b] = (jj[b] < R) ? __ldg(tb.m + lev) : 0u;
+          hl[b] = (jj[b] < R) ? lev - (unsigned)lev_lo : 0xffffffffu;
+          m[b] = (jj[b] < R) ? (hl[b] < (unsigned)SCAN_HW ? s_m[hl[b]] : __ldg(tb.m + lev)) : 0u;
           F2[b] = reinterpret_cast<const double2*>(tb.cdf + (size_t)lev * PO_ROW);
           if (KEEP) {
             if (out.tau && jj[b] < R) out.tau[jj[b]] = __ldg(tb.tau + lev);
@@ -287,7 +316,15 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) u[b] = chunk_uniform(philox4x32_10(0u, jj[b], 0u, c3, key), 0u);
 #pragma unroll
-        for (int b = 0; b < SCAN_BATCH; ++b) c4[b] = cdf_count4(F2[b], 0, u[b]);  // rows of unused levels are masked below
+        for (int b = 0; b < SCAN_BATCH; ++b) {  // rows of unused levels are masked below
+          if (hl[b] < (unsigned)SCAN_HW) {
+            const double2 f01 = *reinterpret_cast<const double2*>(&s_head[hl[b]][0]);
+            const double2 f23 = *reinterpret_cast<const double2*>(&s_head[hl[b]][2]);
+            c4[b] = (unsigned)(u[b] > f01.x) + (unsigned)(u[b] > f01.y) + (unsigned)(u[b] > f23.x) + (unsigned)(u[b] > f23.y);
+          } else {
+            c4[b] = cdf_count4(F2[b], 0, u[b]);
+          }
+        }
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           k[b] = c4[b];
@@ -300,7 +337,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
           if (m[b] > 1u) {
             const unsigned long long old = atomicAdd(&s_pack, ((unsigned long long)(m[b] - 1u) << 12) + 1ull);
             const unsigned h = (unsigned)(old & 0xfffull);
-            s_hstart[h] = old >> 12;
+            s_hstart[h] = (uint32_t)(old >> 12);
             s_hitem[h] = (unsigned short)((r0 + b) * SCAN_THREADS + threadIdx.x);
           }
           cntb[(r0 + b) * SCAN_THREADS + threadIdx.x] = k[b];
@@ -440,32 +477,21 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
           }
         }
       }
-      if (prev == ntiles - 1 && threadIdx.x == 0) {
-        const unsigned long long Rnew = s_prefix + tile_total;
-        out.off[R] = (uint32_t)Rnew;
-        st->Rnew = Rnew;
-        if (Rnew > capacity) st->status = ST_CAPACITY;
-        else if (Rnew == 0ull) st->status = ST_EXTINCT;
-        if (st->status != ST_OK) st->fail_step = st->step + 1u;
-      }
-      __syncthreads();
-      // the block that writes the last outstanding tile sees every offset and R': it runs a5
       if (threadIdx.x == 0) {
-        if (s_flag & 1u) atomicOr(&st->scan_overflow, 1u);
-        __threadfence();
-        const unsigned done = atomicAdd(&st->scan_done, 1u);
-        if (done == ntiles - 1) s_flag |= 2u;
-      }
-      __syncthreads();
-      if (s_flag & 2u) {
-        __threadfence();
-        if (threadIdx.x == 0 && *((volatile unsigned*)&st->scan_overflow) != 0u &&
-            *((volatile unsigned*)&st->status) == ST_OK) {
-          st->status = ST_CAPACITY;
+        if (prev == ntiles - 1) {
+          const unsigned long long Rnew = s_prefix + tile_total;
+          out.off[R] = (uint32_t)Rnew;
+          st->Rnew = Rnew;
+          const unsigned bad = Rnew > capacity ? (unsigned)ST_CAPACITY : (Rnew == 0ull ? (unsigned)ST_EXTINCT : (unsigned)ST_OK);
+          if (bad != ST_OK) {
+            atomicCAS(&st->status, (unsigned)ST_OK, bad);
+            st->fail_step = st->step + 1u;
+          }
+        }
+        if (s_flag & 1u) {  // a parent sits on a level with lambda >= 2^31: over any capacity (wins over "extinct")
+          atomicExch(&st->status, (unsigned)ST_CAPACITY);
           st->fail_step = st->step + 1u;
         }
-        __syncthreads();
-        balance_tile(st, out.off, out.part0, out.part1, out.part_stats, P);
       }
     }
     if (tile == NO_TILE) break;
@@ -475,7 +501,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
 }
 
 // ---------------------------------------------------------------------------------------------------
-// balance_tile: a5.  One block (the last tile of k_poisson_scan to finish; every offset is then visible).  New
+// balance_tile: a5.  One block (block 0 of k_copy: the scan kernel has finished, every offset is visible).  New
 // partition table, born/excess/shortage per partition, moved count.  PAPER.md:104-106; A6.
 // ---------------------------------------------------------------------------------------------------
 __device__ void balance_tile(DevState* st, const uint32_t* off, uint32_t* part0, uint32_t* part1, uint32_t* stats,
@@ -535,8 +561,9 @@ template <> struct VecT<8> { using type = uint2; };
 
 template <int L>
 __global__ void __launch_bounds__(COPY_THREADS)
-k_copy(const DevState* __restrict__ st, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tile_parent,
-       uint32_t* spins0, uint32_t* spins1, int32_t* E0, int32_t* E1, int32_t* M0, int32_t* M1) {
+k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tile_parent,
+       uint32_t* spins0, uint32_t* spins1, int32_t* E0, int32_t* E1, int32_t* M0, int32_t* M1, uint32_t* part0,
+       uint32_t* part1, uint32_t* part_stats, int P) {
   using CG = CopyGeo<L>;
   using V = typename VecT<CG::VB>::type;
   if (st->status != ST_OK) return;
@@ -620,6 +647,11 @@ k_copy(const DevState* __restrict__ st, const uint32_t* __restrict__ off, const 
       for (int u = 0; u < UNR; ++u) dst[(i0 + c + u * GROUPS) * CG::VT + sub] = tmp[u];
     }
     for (; c < nchild; c += GROUPS) dst[(i0 + c) * CG::VT + sub] = src[(unsigned long long)s_par[c] * CG::VT + sub];
+  }
+  // a5: every offset is in memory once this kernel runs; block 0 writes the partition table and the diagnostics
+  if (blockIdx.x == 0) {
+    __syncthreads();
+    balance_tile(st, off, part0, part1, part_stats, P);
   }
 }
 

@@ -354,9 +354,9 @@ def test_device_getters_and_launch_count():
     g.profile_read()  # drain the launches of pa_init
     l0 = g.launch_count()
     g.step(0.1, 2)
-    assert g.launch_count() - l0 == 7  # levels_w, q_reduce, levels_tau, poisson_scan(+balance), copy, sweep, observe
+    assert g.launch_count() - l0 == 6  # q_reduce, levels_tau, poisson_scan, copy (+ partition balance), sweep, observe
     Ed, Md = g.energies_device()
     E, M = g.energies()
     assert np.array_equal(Ed.cpu().numpy(), E) and np.array_equal(Md.cpu().numpy(), M)
     prof = g.profile_read()
-    assert all(cnt == (0 if k == "balance" else 1) for k, (_, cnt) in prof.items()) and prof["sweep"][0] > 0
+    assert all(cnt == (0 if k in ("balance", "levels_w") else 1) for k, (_, cnt) in prof.items()) and prof["sweep"][0] > 0
