@@ -72,9 +72,10 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
     const int shift = twoN - 4 * lev_lo;  // level(E) - lev_lo = (E + 2N - 4 lev_lo) / 4
     auto wl = [&](int e) { return s_w[(e + shift) >> 2]; };
     unsigned long long v = tid;
-    for (; v + stride < nvec; v += 2 * stride) {  // two 128-bit loads in flight per thread
-      const int4 a = __ldg(E4 + v), b = __ldg(E4 + v + stride);
-      acc += ((wl(a.x) + wl(a.y)) + (wl(a.z) + wl(a.w))) + ((wl(b.x) + wl(b.y)) + (wl(b.z) + wl(b.w)));
+    for (; v + 3 * stride < nvec; v += 4 * stride) {  // four 128-bit loads in flight per thread
+      const int4 a = __ldg(E4 + v), b = __ldg(E4 + v + stride), c = __ldg(E4 + v + 2 * stride), d = __ldg(E4 + v + 3 * stride);
+      acc += (((wl(a.x) + wl(a.y)) + (wl(a.z) + wl(a.w))) + ((wl(b.x) + wl(b.y)) + (wl(b.z) + wl(b.w)))) +
+             (((wl(c.x) + wl(c.y)) + (wl(c.z) + wl(c.w))) + ((wl(d.x) + wl(d.y)) + (wl(d.z) + wl(d.w))));
     }
     for (; v < nvec; v += stride) {
       const int4 a = __ldg(E4 + v);
