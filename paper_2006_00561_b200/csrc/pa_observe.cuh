@@ -139,20 +139,39 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  if (threadIdx.x < OBS_Q) {
+  // final reduction by the last block: warp q < 5 adds the partials of sum q (lanes stride over the blocks, then a
+  // warp tree; integer sums, so the order does not matter), warp 5 takes min / max of E
+  __shared__ long long s_lohi[2];
+  if (warp < OBS_Q) {
     U128 t = {0ull, 0ull};
-    for (unsigned b = 0; b < gridDim.x; ++b)
-      u128_add(t, __ldcg(&partial[(size_t)b * 12 + 2 * threadIdx.x]), __ldcg(&partial[(size_t)b * 12 + 2 * threadIdx.x + 1]));
-    st->obs[2 * threadIdx.x] = t.lo;
-    st->obs[2 * threadIdx.x + 1] = t.hi;
-  }
-  if (threadIdx.x == 0) {
+    for (unsigned b = lane; b < gridDim.x; b += 32)
+      u128_add(t, __ldcg(&partial[(size_t)b * 12 + 2 * warp]), __ldcg(&partial[(size_t)b * 12 + 2 * warp + 1]));
+    t = warp_sum_u128(t);
+    if (lane == 0) {
+      st->obs[2 * warp] = t.lo;
+      st->obs[2 * warp + 1] = t.hi;
+    }
+  } else if (warp == OBS_Q) {
     long long lo = 0x7fffffff, hi = -0x7fffffff;
-    for (unsigned b = 0; b < gridDim.x; ++b) {
+    for (unsigned b = lane; b < gridDim.x; b += 32) {
       const long long l = (long long)__ldcg(&partial[(size_t)b * 12 + 10]), h = (long long)__ldcg(&partial[(size_t)b * 12 + 11]);
       lo = l < lo ? l : lo;
       hi = h > hi ? h : hi;
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const long long l = __shfl_xor_sync(0xffffffffu, lo, o), h = __shfl_xor_sync(0xffffffffu, hi, o);
+      lo = l < lo ? l : lo;
+      hi = h > hi ? h : hi;
+    }
+    if (lane == 0) {
+      s_lohi[0] = lo;
+      s_lohi[1] = hi;
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    long long lo = s_lohi[0], hi = s_lohi[1];
     if (lo > hi) lo = hi = -2 * N;  // empty population: cannot happen (R >= 1), keep the window valid
     st->lev_lo = (int)((lo + 2 * N) >> 2);
     st->lev_hi = (int)((hi + 2 * N) >> 2);
