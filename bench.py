@@ -36,6 +36,10 @@ E_BLK = 2.0 + sum(1.0 - (1.0 - 2.0 ** (-4 * c)) ** 32 for c in range(2, 8))
 ALU_OPS_PER_ATTEMPT = (E_BLK * (19 + 12) + 12) / 32.0
 I_MIN_SURVEY = 12.0   # one 32-bit Philox word per attempt at 1 warp-instr/clk/SMSP (kept for continuity)
 SM_COUNT, SMSP, LANES, ALU_LANES = 148, 4, 32, 16
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the `ncu --set full` capture
+# (profiles/r1j_sweep64_ncu.md: config 3, one launch = theta sweeps of R' ~ 2^21 replicas; algorithmic 2*S*R' + 8R').
+# Reported only for the workload it was captured on.
+NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 1.076945e9 + 1.032770e9}
 
 
 def measured_peaks():
@@ -149,13 +153,14 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
-def resample_leg(binding, torch, peaks, repeats=5):
+def resample_leg(binding, torch, peaks, repeats=5, scan_chunks=0):
     """config 5: a1-a6 only (theta=0) on R=2^24 L=32 lattices; algorithmic bytes S*(U+R') + 28*R per step"""
     wl = inputs.CONFIGS[5]
     S = wl.bytes_per_replica
     times, res = [], None
     for rep in range(repeats + 2):  # a fresh context per repeat: same parents, same step (pa_init is deterministic)
-        pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0, flags=binding.PA_PROFILE)
+        pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0, flags=binding.PA_PROFILE,
+                                        scan_chunks=scan_chunks)
         pa.profile_read()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record(pa.stream)
@@ -167,7 +172,10 @@ def resample_leg(binding, torch, peaks, repeats=5):
         off = pa.counts_device()
         U = int(torch.count_nonzero(off[1:] != off[:-1]).item())
         k_ms = {k: v[0] for k, v in prof.items()}
-        chain_ms = sum(k_ms[k] for k in ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "copy"])
+        # a1-a6 as ONE span on the caller's stream (start of k_q_reduce .. end of the last k_copy): with scan_chunks > 1
+        # the scan launches overlap the copy launches, so the sum of the kernels is not the elapsed time
+        chain_ms = k_ms["resample_span"]
+        k_ms["sum_of_kernels"] = sum(k_ms[k] for k in ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "copy"])
         if rep >= 2:
             times.append((chain_ms, ev0.elapsed_time(ev1), k_ms))
         res = (R, Rn, U)
@@ -181,8 +189,9 @@ def resample_leg(binding, torch, peaks, repeats=5):
     red_ms = statistics.median(t[2]["q_reduce"] for t in times)
     alg_bytes = S * (U + Rn) + 28 * R
     copy_bytes = S * (U + Rn) + 4 * R + 8 * Rn + 8 * U  # lattices + offsets read + E,M written/read
+    ksum = statistics.median(t[2]["sum_of_kernels"] for t in times)
     return {"workload": wl.name, "R": R, "R_new": Rn, "U": U, "algorithmic_bytes": alg_bytes,
-            "ms_a1_a6_kernels": chain, "ms_step_wall": wall, "ms_copy": copy_ms, "ms_poisson_scan": scan_ms,
+            "ms_a1_a6_kernels": chain, "ms_sum_of_kernel_durations": ksum, "ms_step_wall": wall, "ms_copy": copy_ms, "ms_poisson_scan": scan_ms,
             "ms_q_reduce": red_ms, "replicas_per_s": Rn / (chain * 1e-3),
             "roofline": {"bound": "hbm", "achieved": alg_bytes / (chain * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                          "unit": "GB/s", "frac": alg_bytes / (chain * 1e-3) / 1e9 / peaks["hbm_gbs"],
@@ -296,7 +305,7 @@ def run_ours(args):
 
     # dominant kernel: the Metropolis sweep (ALU / issue bound)
     sweep_ms, sweep_n = prof["sweep"]
-    step_kernel_ms = sum(v[0] for v in prof.values())
+    step_kernel_ms = sum(v[0] for k, v in prof.items() if k != "resample_span")
     line = None
     extra = {}
     if wl.theta > 0 and sweep_n > 0:
@@ -306,7 +315,9 @@ def run_ours(args):
         peak = SM_COUNT * SMSP * ALU_LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
         roof = {"bound": "alu", "achieved": achieved, "peak": peak,
                 "unit": "T ALU-pipe lane-ops/s (%.3f algorithmic per flip attempt)" % ALU_OPS_PER_ATTEMPT,
-                "frac": achieved / peak, "traffic": None, "kernel": "k_sweep<%d>" % wl.L,
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(("k_sweep<%d>" % wl.L, args.config)),
+                "traffic_algorithmic": (2 * wl.bytes_per_replica + 8) * (replica_steps / sweep_n),
+                "kernel": "k_sweep<%d>" % wl.L,
                 "kernel_attempts_per_s": sweep_rate, "kernel_ms_per_launch": sweep_ms / sweep_n,
                 "kernel_share_of_step": sweep_ms / step_kernel_ms,
                 "peak_src": "148 SM x 4 SMSP x 16 ALU lanes x %d MHz (clocks.max.sm)" % peaks["sm_max_mhz"],
@@ -333,7 +344,7 @@ def run_ours(args):
     torch.cuda.empty_cache()
     if g.is_main and g.world == 1:
         if not args.no_resample:
-            resample = resample_leg(binding, torch, peaks, repeats=args.resample_repeats)
+            resample = resample_leg(binding, torch, peaks, repeats=args.resample_repeats, scan_chunks=args.scan_chunks)
         if not args.no_cpu_baseline:
             r = oracle_sample_run(wl, 4096, 24, 1)
             cpu = {"value": r["attempts"] / r["seconds"], "unit": "attempts/s", "cores": r["cores"], "kind": "oracle",
@@ -369,6 +380,7 @@ def main():
                          "'anneal': whole anneals of --anneal-configs (wall time, ln Z against the exact value)")
     ap.add_argument("--anneal-configs", default="1,2,3,4")
     ap.add_argument("--resample-repeats", type=int, default=5)
+    ap.add_argument("--scan-chunks", type=int, default=0, help="pa_config.scan_chunks of the resample leg (0 = automatic)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3  # timing rule: at least 3 warm-up steps
@@ -386,7 +398,7 @@ def main():
         from paper_2006_00561_b200 import binding
         if not torch.cuda.is_available():
             raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-        print(json.dumps({"resample": resample_leg(binding, torch, measured_peaks(), repeats=args.resample_repeats)}))
+        print(json.dumps({"resample": resample_leg(binding, torch, measured_peaks(), repeats=args.resample_repeats, scan_chunks=args.scan_chunks)}))
         return 0
     return run_ours(args)
 

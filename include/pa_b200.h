@@ -62,7 +62,9 @@ typedef struct {
   uint64_t workspace_bytes;
   void* stream;     /* cudaStream_t, caller owned (NULL = legacy default stream) */
   uint32_t flags;   /* PA_KEEP_TAU | PA_KEEP_COUNTS | PA_PROFILE */
-  uint32_t reserved;
+  uint32_t scan_chunks; /* 0 = automatic (currently 1: overlap measured slower on B200).  1..8: number of launches the Poisson/scan kernel is split into; with more than
+                           one, the copy of chunk i (cfg.stream) overlaps the scan of chunk i+1 (a stream of the library).
+                           Results do not depend on it. */
 } pa_config;
 
 /* population sums after the last committed step (or after pa_init / pa_set_spins); 128-bit integers as {lo, hi} */
@@ -94,6 +96,8 @@ enum {
   PA_K_COPY,         /* replica redistribution (gather copy) */
   PA_K_SWEEP,        /* theta checkerboard Metropolis sweeps + E, M */
   PA_K_OBSERVE,      /* population sums + commit of the step */
+  PA_K_RESAMPLE_SPAN, /* not a kernel: elapsed time on cfg.stream from the start of PA_K_Q_REDUCE to the end of the last
+                         PA_K_COPY (a1-a6 as one span; with scan_chunks > 1 the kernels inside it overlap) */
   PA_K_COUNT
 };
 

@@ -111,6 +111,11 @@ struct pa_ctx {
   int64_t launches;
   bool profile;
   int scan_grid_max;  // co-resident blocks of k_poisson_scan on this device
+  // large populations: the scan runs in SCAN_CHUNKS launches on a high-priority stream of the library, the copy of
+  // chunk i (caller's stream) overlaps the scan of chunk i+1
+  int nchunks;
+  cudaStream_t scan_stream;
+  cudaEvent_t ev_fork, ev_scan[8];
   std::vector<EventPair> ev_used, ev_free;
   std::string err;
 
@@ -136,8 +141,10 @@ struct Prof {  // records an event pair around one launch when profiling is on
   pa_ctx* c;
   EventPair ep;
   bool on;
-  Prof(pa_ctx* c_, int kernel) : c(c_), on(c_->profile) {
-    c->launches += 1;
+  cudaStream_t s;
+  Prof(pa_ctx* c_, int kernel, cudaStream_t stream = nullptr, bool is_launch = true)
+      : c(c_), on(c_->profile), s(stream ? stream : c_->stream) {
+    if (is_launch) c->launches += 1;
     if (!on) return;
     if (!c->ev_free.empty()) {
       ep = c->ev_free.back();
@@ -147,11 +154,11 @@ struct Prof {  // records an event pair around one launch when profiling is on
       cudaEventCreate(&ep.b);
     }
     ep.kernel = kernel;
-    cudaEventRecord(ep.a, c->stream);
+    cudaEventRecord(ep.a, s);
   }
   ~Prof() {
     if (!on) return;
-    cudaEventRecord(ep.b, c->stream);
+    cudaEventRecord(ep.b, s);
     c->ev_used.push_back(ep);
   }
 };
@@ -206,7 +213,7 @@ void launch_sweep(pa_ctx* c, int theta, uint32_t T4, uint32_t T8, int mode) {
 }
 
 template <int L>
-void launch_copy_L(pa_ctx* c) {
+void launch_copy_L(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end) {
   const unsigned grid = (unsigned)((c->cap + CopyGeo<L>::CT - 1) / CopyGeo<L>::CT);
   uint32_t *s0 = c->dev<uint32_t>(c->lo.spins[0]), *s1 = c->dev<uint32_t>(c->lo.spins[1]);
   int32_t *e0 = c->dev<int32_t>(c->lo.E[0]), *e1 = c->dev<int32_t>(c->lo.E[1]);
@@ -214,16 +221,18 @@ void launch_copy_L(pa_ctx* c) {
   k_copy<L><<<grid, COPY_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), c->dev<uint32_t>(c->lo.off),
                                                   c->dev<uint32_t>(c->lo.tile_parent), s0, s1, e0, e1, m0, m1,
                                                   c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]),
-                                                  c->dev<uint32_t>(c->lo.part_stats), c->cfg.P);
+                                                  c->dev<uint32_t>(c->lo.part_stats), c->cfg.P,
+                                                  c->dev<unsigned long long>(c->lo.tile_desc), chunk, c->nchunks,
+                                                  tile_begin, tile_end);
 }
-void launch_copy(pa_ctx* c) {
+void launch_copy(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end) {
   Prof p(c, PA_K_COPY);
   switch (c->cfg.L) {
-    case 8: launch_copy_L<8>(c); break;
-    case 16: launch_copy_L<16>(c); break;
-    case 32: launch_copy_L<32>(c); break;
-    case 64: launch_copy_L<64>(c); break;
-    default: launch_copy_L<128>(c); break;
+    case 8: launch_copy_L<8>(c, chunk, tile_begin, tile_end); break;
+    case 16: launch_copy_L<16>(c, chunk, tile_begin, tile_end); break;
+    case 32: launch_copy_L<32>(c, chunk, tile_begin, tile_end); break;
+    case 64: launch_copy_L<64>(c, chunk, tile_begin, tile_end); break;
+    default: launch_copy_L<128>(c, chunk, tile_begin, tile_end); break;
   }
 }
 
@@ -243,6 +252,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   const int N = c->N;
   const int n_desc = (int)((c->cap + SCAN_TILE - 1) / SCAN_TILE + 1);
   const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
+  Prof* span = new Prof(c, PA_K_RESAMPLE_SPAN, nullptr, false);  // a1-a6 as one span on the caller's stream
   {
     Prof p(c, PA_K_Q_REDUCE);  // also resets the step's counters and look-back descriptors
     k_q_reduce<<<RED_GRID, RED_THREADS, 0, c->stream>>>(st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
@@ -254,7 +264,6 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     k_levels_tau<<<(N + 1 + 127) / 128, 128, 0, c->stream>>>(st, sp, tb, N);
   }
   {
-    Prof p(c, PA_K_POISSON_SCAN);  // includes a5 (partition balance), run by the last tile to finish
     // persistent blocks pull tiles from a ticket counter
     const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
     const bool keep = c->lo.n || c->lo.tau;
@@ -265,7 +274,6 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
       c->scan_grid_max = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
     }
-    const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? tiles_cap : (unsigned)c->scan_grid_max;
     ScanOut out;
     out.off = c->dev<uint32_t>(c->lo.off);
     out.n = c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr;
@@ -275,14 +283,37 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     out.part0 = c->dev<uint32_t>(c->lo.part[0]);
     out.part1 = c->dev<uint32_t>(c->lo.part[1]);
     out.part_stats = c->dev<uint32_t>(c->lo.part_stats);
-    if (keep)
-      k_poisson_scan<true><<<grid, SCAN_THREADS, 0, c->stream>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
-                                                                   (unsigned long long)c->cap, c->cfg.P, c->key);
-    else
-      k_poisson_scan<false><<<grid, SCAN_THREADS, 0, c->stream>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
-                                                                    (unsigned long long)c->cap, c->cfg.P, c->key);
+    // a2-a6.  One chunk: scan then copy on the caller's stream.  Several chunks: the issue-bound scan of chunk i+1
+    // (library stream, high priority so that its persistent blocks are placed first) runs under the HBM-bound copy of
+    // chunk i (caller's stream); events order scan i -> copy i, and everything joins the caller's stream again.
+    const int C = c->nchunks;
+    const unsigned per = (tiles_cap + C - 1) / C;
+    cudaStream_t ss = C > 1 ? c->scan_stream : c->stream;
+    if (C > 1) {
+      cudaEventRecord(c->ev_fork, c->stream);
+      cudaStreamWaitEvent(ss, c->ev_fork, 0);
+    }
+    for (int i = 0; i < C; ++i) {
+      const unsigned t0 = per * i, t1 = (i == C - 1) ? tiles_cap : per * (i + 1);
+      const unsigned ntl = t1 - t0;
+      const unsigned grid = ntl < (unsigned)c->scan_grid_max ? (ntl ? ntl : 1u) : (unsigned)c->scan_grid_max;
+      {
+        Prof p(c, PA_K_POISSON_SCAN, ss);
+        if (keep)
+          k_poisson_scan<true><<<grid, SCAN_THREADS, 0, ss>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
+                                                              (unsigned long long)c->cap, c->key, i, t0, t1);
+        else
+          k_poisson_scan<false><<<grid, SCAN_THREADS, 0, ss>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
+                                                               (unsigned long long)c->cap, c->key, i, t0, t1);
+      }
+      if (C > 1) {
+        cudaEventRecord(c->ev_scan[i], ss);
+        cudaStreamWaitEvent(c->stream, c->ev_scan[i], 0);
+      }
+      launch_copy(c, i, t0, t1);
+    }
   }
-  launch_copy(c);
+  delete span;
   if (theta > 0) launch_sweep(c, theta, hp.T4, hp.T8, 0);
   launch_observe(c, sp, 0);
 }
@@ -408,6 +439,15 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   c->profile = (cfg->flags & PA_PROFILE) != 0;
   c->launches = 0;
   c->scan_grid_max = 0;
+  {
+    const uint64_t tiles_cap = ((uint64_t)c->cap + SCAN_TILE - 1) / SCAN_TILE;
+    int C = (int)cfg->scan_chunks;
+    if (C == 0) C = 1;  // measured on B200 (config 5): 2 / 4 / 8 chunks are 4 % / 12 % / 26 % SLOWER than one
+    if (C > 8) C = 8;
+    if ((uint64_t)C > tiles_cap) C = (int)tiles_cap;
+    c->nchunks = C < 1 ? 1 : C;
+    c->scan_stream = nullptr;
+  }
   uint32_t k0 = (uint32_t)(cfg->seed & 0xffffffffull), k1 = (uint32_t)(cfg->seed >> 32);
   for (int r = 0; r < 10; ++r) {
     c->key.k0[r] = k0;
@@ -427,6 +467,13 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
     return PA_ECUDA;
   }
   *out = c;  // from here on errors keep the ctx so that pa_last_error works; caller destroys it
+  if (c->nchunks > 1) {
+    int lo_prio = 0, hi_prio = 0;
+    CK(cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio));
+    CK(cudaStreamCreateWithPriority(&c->scan_stream, cudaStreamNonBlocking, hi_prio));
+    CK(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+    for (int i = 0; i < c->nchunks; ++i) CK(cudaEventCreateWithFlags(&c->ev_scan[i], cudaEventDisableTiming));
+  }
   DevState* st = c->dev<DevState>(c->lo.state);
   k_init_state<<<1, 256, 0, c->stream>>>(st, (unsigned long long)cfg->R0, cfg->beta0, c->dev<uint32_t>(c->lo.part[0]),
                                          cfg->P);
@@ -632,6 +679,12 @@ int pa_destroy(pa_ctx* c) {
   cudaStreamSynchronize(c->stream);
   for (EventPair& ep : c->ev_used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
   for (EventPair& ep : c->ev_free) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
+  if (c->scan_stream) {
+    cudaStreamSynchronize(c->scan_stream);
+    cudaStreamDestroy(c->scan_stream);
+    cudaEventDestroy(c->ev_fork);
+    for (int i = 0; i < c->nchunks; ++i) cudaEventDestroy(c->ev_scan[i]);
+  }
   if (c->h_state) cudaFreeHost(c->h_state);
   if (c->h_params) cudaFreeHost(c->h_params);
   delete c;

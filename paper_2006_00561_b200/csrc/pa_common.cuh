@@ -30,7 +30,7 @@ struct DevState {
   unsigned int status;           // 0 = ok, else -pa_status of the failing step
   unsigned int fail_step;        // ordinal of the step that failed
   unsigned int reduce_done;      // block counters (reset every step by k_q_reduce)
-  unsigned int scan_tile;
+  unsigned int scan_tile[8];     // ticket counters of k_poisson_scan, one per chunk launch
   unsigned int scan_overflow;    // a parent sat on a level with lambda >= 2^31
   unsigned int obs_done;
   unsigned int T4, T8;           // thresholds of the last committed step with theta > 0

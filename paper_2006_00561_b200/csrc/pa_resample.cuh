@@ -51,7 +51,7 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
   const unsigned long long tid = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x;
   const unsigned long long stride = (unsigned long long)gridDim.x * RED_THREADS;
   if (tid == 0) {  // counters of the later kernels of this step (reduce_done is reset by the last block below)
-    st->scan_tile = 0u;
+    for (int i = 0; i < 8; ++i) st->scan_tile[i] = 0u;
     st->scan_overflow = 0u;
     st->obs_done = 0u;
   }
@@ -249,7 +249,8 @@ constexpr unsigned NO_TILE = 0xffffffffu;
 template <bool KEEP>
 __global__ void __launch_bounds__(SCAN_THREADS, 5)
 k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
-               ScanOut out, int copy_shift, unsigned long long capacity, int P, const PhiloxKey key) {
+               ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key, int chunk,
+               unsigned tile_begin, unsigned tile_end_cap) {
   if (st->status != ST_OK) return;
   __shared__ unsigned s_tile;
   __shared__ unsigned s_flag;            // bit 0: a parent of this block sits on an overflowing level
@@ -271,6 +272,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
   }
   const uint32_t R = (uint32_t)st->R;  // R <= capacity < 2^32 - 4096: parent indices fit 32 bits
   const unsigned ntiles = (R + SCAN_TILE - 1) / SCAN_TILE;
+  const unsigned tile_end = tile_end_cap < ntiles ? tile_end_cap : ntiles;
   const int32_t* __restrict__ E = st->cur ? E1 : E0;
   const uint32_t c3 = ctr3(TAG_RESAMPLE, st->step + 1u);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -280,11 +282,11 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
 
   for (;;) {
     if (threadIdx.x == 0) {
-      s_tile = atomicAdd(&st->scan_tile, 1u);
+      s_tile = tile_begin + atomicAdd(&st->scan_tile[chunk], 1u);
       s_pack = 0ull;
     }
     __syncthreads();
-    const unsigned tile = s_tile < ntiles ? s_tile : NO_TILE;
+    const unsigned tile = s_tile < tile_end ? s_tile : NO_TILE;  // tiles of this launch: [tile_begin, tile_end)
     if (tile == NO_TILE && prev == NO_TILE) break;
 
     if (tile != NO_TILE) {
@@ -461,6 +463,9 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
       if (j0 + SCAN_ROUNDS <= R) {
         *reinterpret_cast<uint4*>(out.off + j0) = make_uint4(offs[0], offs[1], offs[2], offs[3]);
         *reinterpret_cast<uint4*>(out.off + j0 + 4) = make_uint4(offs[4], offs[5], offs[6], offs[7]);
+        // the tile's inclusive prefix = first offset of the next tile: a copy launch that runs while the next chunk of
+        // the scan is still in flight reads it (the next tile writes the same value again)
+        if (threadIdx.x == SCAN_THREADS - 1) out.off[j0 + SCAN_ROUNDS] = (uint32_t)o64;
         if (KEEP) {
           if (out.n) {
             *reinterpret_cast<uint4*>(out.n + j0) = make_uint4(cnt[0], cnt[1], cnt[2], cnt[3]);
@@ -564,13 +569,29 @@ template <int L>
 __global__ void __launch_bounds__(COPY_THREADS)
 k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tile_parent,
        uint32_t* spins0, uint32_t* spins1, int32_t* E0, int32_t* E1, int32_t* M0, int32_t* M1, uint32_t* part0,
-       uint32_t* part1, uint32_t* part_stats, int P) {
+       uint32_t* part1, uint32_t* part_stats, int P, const unsigned long long* __restrict__ tile_desc, int chunk,
+       int nchunks, unsigned tile_begin, unsigned tile_end_cap) {
   using CG = CopyGeo<L>;
   using V = typename VecT<CG::VB>::type;
   if (st->status != ST_OK) return;
-  const unsigned long long Rnew = st->Rnew, R = st->R;
+  // Launch `chunk` of `nchunks` runs when the scan tiles [0, tile_end) are done (tile_end = min(tile_end_cap, all)):
+  // `hi` children have all their parents' offsets in memory, `lo` of them were already complete for the previous
+  // launch.  A copy tile belongs to the launch in which its END becomes complete; the last launch (every scan tile
+  // done, R' final) also takes the ragged last tile.
+  const unsigned long long R = st->R;
+  const unsigned ntiles = (unsigned)((R + SCAN_TILE - 1) / SCAN_TILE);
+  const unsigned b0 = tile_begin < ntiles ? tile_begin : ntiles, b1 = tile_end_cap < ntiles ? tile_end_cap : ntiles;
+  const bool last = (chunk == nchunks - 1);
+  const unsigned long long lo = b0 ? (tile_desc[b0 - 1] & DESC_VAL) : 0ull;
+  const unsigned long long hi = b1 ? (tile_desc[b1 - 1] & DESC_VAL) : 0ull;
+  const unsigned long long Rnew = last ? st->Rnew : hi;
+  const unsigned long long lim = (unsigned long long)b1 * SCAN_TILE < R ? (unsigned long long)b1 * SCAN_TILE : R;  // parents done
   const unsigned long long i0 = (unsigned long long)blockIdx.x * CG::CT;
-  if (i0 >= Rnew) return;
+  const bool mine = (i0 + CG::CT > lo) && (last ? (i0 < Rnew) : (i0 + CG::CT <= hi));
+  if (!mine) {
+    if (last && blockIdx.x == 0) balance_tile(st, off, part0, part1, part_stats, P);  // a5 (see the end of the kernel)
+    return;
+  }
   const unsigned cur = st->cur;  // source = buffer cur, destination = buffer cur^1 (never the same memory)
   const V* __restrict__ src = reinterpret_cast<const V*>(cur ? spins1 : spins0);
   V* __restrict__ dst = reinterpret_cast<V*>(cur ? spins0 : spins1);
@@ -591,7 +612,7 @@ k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restric
   for (unsigned long long jb = (unsigned long long)j_first + 1;; jb += COPY_THREADS) {
     const unsigned long long j = jb + threadIdx.x;
     bool past = true;
-    if (j < R) {
+    if (j < lim) {  // off[lim] is in memory too: every scan tile also writes the first offset of the next tile
       const uint32_t o = off[j], o1 = off[j + 1];
       past = (o >= i1);
       if (!past && o1 > o) s_par[o - i0] = (uint32_t)j;  // o >= i0 because j > j_first
@@ -650,7 +671,7 @@ k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restric
     for (; c < nchild; c += GROUPS) dst[(i0 + c) * CG::VT + sub] = src[(unsigned long long)s_par[c] * CG::VT + sub];
   }
   // a5: every offset is in memory once this kernel runs; block 0 writes the partition table and the diagnostics
-  if (blockIdx.x == 0) {
+  if (last && blockIdx.x == 0) {
     __syncthreads();
     balance_tile(st, off, part0, part1, part_stats, P);
   }

@@ -31,10 +31,10 @@ def rel(a, b):
     return abs(a - b) / max(abs(b), 1e-300)
 
 
-def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None):
+def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None, scan_chunks=0):
     b = _binding()
     gpu = b.PopulationAnnealer(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity,
-                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS)
+                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS, scan_chunks=scan_chunks)
     if spins is not None:
         gpu.set_spins(spins)
     ora = orc.OraclePA(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity, spins=spins)
@@ -288,6 +288,19 @@ def test_capacity_error_leaves_population_unchanged():
             assert g.log_Z() == lz_before and g.beta_steps() == bs
     assert failures > 5  # R' ~ Poisson(1024) exceeds 1024 about half of the time
     assert g.beta_steps()[1] == 59 - failures
+
+
+@pytest.mark.parametrize("chunks", [2, 4, 8])
+def test_chunked_scan_with_overlapped_copy_lockstep(chunks):
+    """pa_config.scan_chunks > 1: the scan runs in several launches on the library's stream and the copy of chunk i
+    overlaps the scan of chunk i+1; every result must be what the single-launch path and the oracle give (ragged last
+    tile, copy tiles that straddle chunk boundaries, skewed counts)"""
+    L, R0, P = 32, 40000 + 137, 7
+    spins = inputs.structured_population(L, R0, seed=11)
+    gpu, ora = make_pair(L, R0, P, seed=21, spins=spins, scan_chunks=chunks)
+    lockstep(gpu, ora, [0.02, 0.05, 0.11], 1)
+    gpu2, ora2 = make_pair(16, 9000, 3, seed=5, scan_chunks=chunks)  # fewer tiles (5) than some chunk counts
+    lockstep(gpu2, ora2, [0.1, 0.2], 2)
 
 
 def test_extinction_matches_the_oracle_and_leaves_population_unchanged():
