@@ -134,6 +134,9 @@ def run_reference(args):
     if rank != 0:
         return 0
     wl = inputs.CONFIGS[args.config]
+    if args.theta > 0:
+        import dataclasses
+        wl = dataclasses.replace(wl, theta=args.theta, name=wl.name + "_theta%d" % args.theta)
     R_sample = min(4096, wl.R0)
     r = oracle_sample_run(wl, R_sample, args.steps, args.warmup)
     value = r["attempts"] / r["seconds"]
@@ -273,6 +276,9 @@ def run_ours(args):
     torch.cuda.set_device(g.local_rank)
     peaks = measured_peaks()
     wl = inputs.CONFIGS[args.config]
+    if args.theta > 0:
+        import dataclasses
+        wl = dataclasses.replace(wl, theta=args.theta, name=wl.name + "_theta%d" % args.theta)
     K, W = args.steps, max(args.warmup, 0)
 
     pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed + 1000 * g.rank, beta0=wl.beta0,
@@ -372,6 +378,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4])
+    ap.add_argument("--theta", type=int, default=0,
+                    help="override the sweeps per step of the workload (theta = 1 is the paper's scalability regime, "
+                         "PAPER.md:126: resampling and redistribution dominate); 0 = the config's own theta")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-resample", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -5,6 +5,8 @@
 // floating point is tabulated per energy LEVEL (N+1 levels) by two tiny kernels; the per-replica kernels only
 // look the tables up.  The arithmetic per level is exactly the sequence written in DESIGN.md.
 #pragma once
+#include <type_traits>
+
 #include "pa_common.cuh"
 
 namespace pa {
@@ -265,6 +267,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
   __shared__ __align__(16) double s_head[SCAN_HW][4];
   __shared__ unsigned s_m[SCAN_HW];
   const int lev_lo = st->lev_lo;
+  const bool all_cached = st->lev_hi - lev_lo < SCAN_HW;
   {
     const int W = min(st->lev_hi - lev_lo + 1, SCAN_HW);
     for (int i = threadIdx.x; i < 4 * W; i += SCAN_THREADS) s_head[i >> 2][i & 3] = tb.cdf[(size_t)(lev_lo + (i >> 2)) * PO_ROW + (i & 3)];
@@ -292,26 +295,26 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
     if (tile != NO_TILE) {
       const uint32_t tile_base = tile * SCAN_TILE;
       unsigned* cntb = s_cnt[buf];
-      // phase 1: chunk 0 of every parent; item = r * 256 + tid (coalesced), SCAN_BATCH branch-free chains at a time
-#pragma unroll 1
-      for (int r0 = 0; r0 < SCAN_ROUNDS; r0 += SCAN_BATCH) {
+      // phase 1: chunk 0 of every parent; item = r * 256 + tid (coalesced), SCAN_BATCH branch-free chains at a time.
+      // Two instances of the batch: ALL = the whole occupied window is cached in shared memory (the usual case: no
+      // global look-up and no address arithmetic for it on the common path), or the mixed path.
+      auto batch = [&](auto all_tag, int r0) {
+        constexpr bool ALL = decltype(all_tag)::value;
         uint32_t jj[SCAN_BATCH];
         int e[SCAN_BATCH];
-        unsigned m[SCAN_BATCH], k[SCAN_BATCH], c4[SCAN_BATCH];
+        unsigned m[SCAN_BATCH], k[SCAN_BATCH], c4[SCAN_BATCH], hl[SCAN_BATCH];
         double u[SCAN_BATCH];
-        const double2* F2[SCAN_BATCH];
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           jj[b] = tile_base + (r0 + b) * SCAN_THREADS + threadIdx.x;
-          e[b] = (jj[b] < R) ? __ldg(E + jj[b]) : -2 * N;
+          e[b] = (jj[b] < R) ? __ldg(E + jj[b]) : 4 * lev_lo - 2 * N;  // padding reads as the first occupied level
         }
-        unsigned hl[SCAN_BATCH];  // level relative to the cached window (>= SCAN_HW: not cached)
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           const unsigned lev = (unsigned)((e[b] + 2 * N) >> 2);
-          hl[b] = (jj[b] < R) ? lev - (unsigned)lev_lo : 0xffffffffu;
-          m[b] = (jj[b] < R) ? (hl[b] < (unsigned)SCAN_HW ? s_m[hl[b]] : __ldg(tb.m + lev)) : 0u;
-          F2[b] = reinterpret_cast<const double2*>(tb.cdf + (size_t)lev * PO_ROW);
+          hl[b] = lev - (unsigned)lev_lo;  // level relative to the cached window (>= SCAN_HW: not cached)
+          const unsigned mm = (ALL || hl[b] < (unsigned)SCAN_HW) ? s_m[hl[b]] : __ldg(tb.m + lev);
+          m[b] = (jj[b] < R) ? mm : 0u;
           if (KEEP) {
             if (out.tau && jj[b] < R) out.tau[jj[b]] = __ldg(tb.tau + lev);
           }
@@ -320,18 +323,19 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
         for (int b = 0; b < SCAN_BATCH; ++b) u[b] = chunk_uniform(philox4x32_10(0u, jj[b], 0u, c3, key), 0u);
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {  // rows of unused levels are masked below
-          if (hl[b] < (unsigned)SCAN_HW) {
+          if (ALL || hl[b] < (unsigned)SCAN_HW) {
             const double2 f01 = *reinterpret_cast<const double2*>(&s_head[hl[b]][0]);
             const double2 f23 = *reinterpret_cast<const double2*>(&s_head[hl[b]][2]);
             c4[b] = (unsigned)(u[b] > f01.x) + (unsigned)(u[b] > f01.y) + (unsigned)(u[b] > f23.x) + (unsigned)(u[b] > f23.y);
           } else {
-            c4[b] = cdf_count4(F2[b], 0, u[b]);
+            c4[b] = cdf_count4(reinterpret_cast<const double2*>(tb.cdf + (size_t)(hl[b] + (unsigned)lev_lo) * PO_ROW), 0, u[b]);
           }
         }
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           k[b] = c4[b];
-          if (c4[b] == 4u) k[b] += cdf_search_from(F2[b], 1, u[b]);
+          if (c4[b] == 4u)
+            k[b] += cdf_search_from(reinterpret_cast<const double2*>(tb.cdf + (size_t)(hl[b] + (unsigned)lev_lo) * PO_ROW), 1, u[b]);
           if (m[b] == M_OVERFLOW) {
             s_flag = 1u;
             m[b] = 0u;
@@ -345,6 +349,13 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
           }
           cntb[(r0 + b) * SCAN_THREADS + threadIdx.x] = k[b];
         }
+      };
+      if (all_cached) {
+#pragma unroll 1
+        for (int r0 = 0; r0 < SCAN_ROUNDS; r0 += SCAN_BATCH) batch(std::true_type{}, r0);
+      } else {
+#pragma unroll 1
+        for (int r0 = 0; r0 < SCAN_ROUNDS; r0 += SCAN_BATCH) batch(std::false_type{}, r0);
       }
       __syncthreads();
       // phase 2: flat work list over the extra chunks of the tile's heavy parents
