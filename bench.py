@@ -40,6 +40,9 @@ SM_COUNT, SMSP, LANES, ALU_LANES = 148, 4, 32, 16
 # (profiles/r1j_sweep64_ncu.md: config 3, one launch = theta sweeps of R' ~ 2^21 replicas; algorithmic 2*S*R' + 8R').
 # Reported only for the workload it was captured on.
 NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 1.076945e9 + 1.032770e9}
+# same for the a1-a6 chain of config 5 (profiles/r1k_resample_ncu.md; k_q_reduce from the r1f capture): q_reduce + levels_tau
+# + poisson_scan + copy, read + write
+NCU_RESAMPLE_TRAFFIC_BYTES = 67.12e6 + 0.014e6 + (67.28e6 + 21.58e6) + (671.23e6 + 2223.73e6)
 
 
 def measured_peaks():
@@ -198,7 +201,7 @@ def resample_leg(binding, torch, peaks, repeats=5, scan_chunks=0):
             "ms_q_reduce": red_ms, "replicas_per_s": Rn / (chain * 1e-3),
             "roofline": {"bound": "hbm", "achieved": alg_bytes / (chain * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                          "unit": "GB/s", "frac": alg_bytes / (chain * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                         "peak_src": peaks["src"], "traffic": None,
+                         "peak_src": peaks["src"], "traffic": NCU_RESAMPLE_TRAFFIC_BYTES,
                          "copy_kernel_GBps": copy_bytes / (copy_ms * 1e-3) / 1e9,
                          "frac_vs_8000": alg_bytes / (chain * 1e-3) / 1e9 / 8000.0}}
 
