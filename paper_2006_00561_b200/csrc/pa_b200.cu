@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <optional>
 #include <string>
 #include <vector>
 
@@ -252,7 +253,8 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   const int N = c->N;
   const int n_desc = (int)((c->cap + SCAN_TILE - 1) / SCAN_TILE + 1);
   const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
-  Prof* span = new Prof(c, PA_K_RESAMPLE_SPAN, nullptr, false);  // a1-a6 as one span on the caller's stream
+  std::optional<Prof> span;  // a1-a6 as one span on the caller's stream (not a launch)
+  span.emplace(c, PA_K_RESAMPLE_SPAN, nullptr, false);
   {
     Prof p(c, PA_K_Q_REDUCE);  // also resets the step's counters and look-back descriptors
     k_q_reduce<<<RED_GRID, RED_THREADS, 0, c->stream>>>(st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
@@ -313,7 +315,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
       launch_copy(c, i, t0, t1);
     }
   }
-  delete span;
+  span.reset();
   if (theta > 0) launch_sweep(c, theta, hp.T4, hp.T8, 0);
   launch_observe(c, sp, 0);
 }
