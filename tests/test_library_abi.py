@@ -79,3 +79,20 @@ def test_product_does_not_reference_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle|pa_oracle|libpa_oracle", text, flags=re.M), (dirpath, f)
+
+
+def test_bench_reference_arm_prints_the_contract_line():
+    """bench.py --impl reference (the oracle as it stands, on the host cores) needs no GPU: one JSON line with the
+    driver contract's keys, the same metric / unit as our arm, and the e2e / cpu_baseline objects of the tier framing"""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--config", "1",
+                          "--steps", "2", "--warmup", "1"], capture_output=True, text=True, timeout=300, check=True).stdout
+    line = json.loads(out.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["metric"] == "spin_flip_attempts_per_s" and line["unit"] == "attempts/s"
+    assert line["higher_is_better"] is True and line["steps"] == 2 and line["value"] > 0 and line["vs_baseline"] is None
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
+    assert line["e2e"] == {"value": line["value"], "unit": "attempts/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert line["gpu_launches"] == 0 and line["config"]["workload"].startswith("config1")
