@@ -93,7 +93,8 @@ enum {
   PA_K_LEVELS_TAU,   /* eq. 4 per level + Poisson chunk tables */
   PA_K_POISSON_SCAN, /* Poisson copy counts + single-pass exclusive scan */
   PA_K_BALANCE,      /* partition table + diagnostics: run by block 0 of PA_K_COPY, reports 0 launches */
-  PA_K_COPY,         /* replica redistribution (gather copy) */
+  PA_K_COPY,         /* replica redistribution: gather copy (theta = 0) or only the child -> parent map (theta > 0: the
+                        lattices are gathered by PA_K_SWEEP's load) */
   PA_K_SWEEP,        /* theta checkerboard Metropolis sweeps + E, M */
   PA_K_OBSERVE,      /* population sums + commit of the step */
   PA_K_RESAMPLE_SPAN, /* not a kernel: elapsed time on cfg.stream from the start of PA_K_Q_REDUCE to the end of the last

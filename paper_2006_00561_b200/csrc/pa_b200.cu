@@ -24,7 +24,7 @@ constexpr int RED_GRID = 148 * 4;
 constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
-  uint64_t state, params, spins[2], E[2], M[2], off, n, tau, tile_desc, tile_parent, red_partial, obs_partial,
+  uint64_t state, params, spins[2], E[2], M[2], off, n, tau, tile_desc, tile_parent, parent_of, red_partial, obs_partial,
       lev_tau, lev_mu, lev_m, lev_cdf, part[2], part_stats, total;
 };
 
@@ -77,6 +77,7 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   lo->tau = (c->flags & PA_KEEP_TAU) ? take(ucap * 8) : 0;
   lo->tile_desc = take(((ucap + SCAN_TILE - 1) / SCAN_TILE + 1) * 8);
   lo->tile_parent = take((ucap / copy_tile_for(c->L) + 2) * 4);
+  lo->parent_of = take(ucap * 4);  // child -> parent map of the gather-on-load sweep (theta > 0)
   lo->red_partial = take(RED_GRID * 8);
   lo->obs_partial = take((uint64_t)OBS_GRID * 12 * 8);
   lo->lev_tau = take(nlev * 8);
@@ -193,11 +194,13 @@ void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
   if constexpr (L >= 64) {
     const uint64_t threads = (uint64_t)c->cap * Geo<L>::G;
     const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
-    k_sweep<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa);
+    k_sweep<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa,
+                                                      c->dev<uint32_t>(c->lo.parent_of));
   } else {
     const uint64_t threads = (uint64_t)c->cap * SGeo<L>::G;
     const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
-    k_sweep_small<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa);
+    k_sweep_small<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa,
+                                                            c->dev<uint32_t>(c->lo.parent_of));
   }
 }
 // mode 0: theta sweeps of the resampled population with the thresholds of the step; mode 1: energies only
@@ -214,7 +217,7 @@ void launch_sweep(pa_ctx* c, int theta, uint32_t T4, uint32_t T8, int mode) {
 }
 
 template <int L>
-void launch_copy_L(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end) {
+void launch_copy_L(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end, bool map_only) {
   const unsigned grid = (unsigned)((c->cap + CopyGeo<L>::CT - 1) / CopyGeo<L>::CT);
   uint32_t *s0 = c->dev<uint32_t>(c->lo.spins[0]), *s1 = c->dev<uint32_t>(c->lo.spins[1]);
   int32_t *e0 = c->dev<int32_t>(c->lo.E[0]), *e1 = c->dev<int32_t>(c->lo.E[1]);
@@ -224,16 +227,17 @@ void launch_copy_L(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end)
                                                   c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]),
                                                   c->dev<uint32_t>(c->lo.part_stats), c->cfg.P,
                                                   c->dev<unsigned long long>(c->lo.tile_desc), chunk, c->nchunks,
-                                                  tile_begin, tile_end);
+                                                  tile_begin, tile_end,
+                                                  map_only ? c->dev<uint32_t>(c->lo.parent_of) : nullptr);
 }
-void launch_copy(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end) {
+void launch_copy(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end, bool map_only) {
   Prof p(c, PA_K_COPY);
   switch (c->cfg.L) {
-    case 8: launch_copy_L<8>(c, chunk, tile_begin, tile_end); break;
-    case 16: launch_copy_L<16>(c, chunk, tile_begin, tile_end); break;
-    case 32: launch_copy_L<32>(c, chunk, tile_begin, tile_end); break;
-    case 64: launch_copy_L<64>(c, chunk, tile_begin, tile_end); break;
-    default: launch_copy_L<128>(c, chunk, tile_begin, tile_end); break;
+    case 8: launch_copy_L<8>(c, chunk, tile_begin, tile_end, map_only); break;
+    case 16: launch_copy_L<16>(c, chunk, tile_begin, tile_end, map_only); break;
+    case 32: launch_copy_L<32>(c, chunk, tile_begin, tile_end, map_only); break;
+    case 64: launch_copy_L<64>(c, chunk, tile_begin, tile_end, map_only); break;
+    default: launch_copy_L<128>(c, chunk, tile_begin, tile_end, map_only); break;
   }
 }
 
@@ -312,11 +316,12 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
         cudaEventRecord(c->ev_scan[i], ss);
         cudaStreamWaitEvent(c->stream, c->ev_scan[i], 0);
       }
-      launch_copy(c, i, t0, t1);
+      launch_copy(c, i, t0, t1, theta > 0);
     }
   }
   span.reset();
-  if (theta > 0) launch_sweep(c, theta, hp.T4, hp.T8, 0);
+  // theta > 0: a6 is fused into the sweep's load (k_copy only wrote the child -> parent map)
+  if (theta > 0) launch_sweep(c, theta, hp.T4, hp.T8, 2);
   launch_observe(c, sp, 0);
 }
 

@@ -581,7 +581,7 @@ __global__ void __launch_bounds__(COPY_THREADS)
 k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tile_parent,
        uint32_t* spins0, uint32_t* spins1, int32_t* E0, int32_t* E1, int32_t* M0, int32_t* M1, uint32_t* part0,
        uint32_t* part1, uint32_t* part_stats, int P, const unsigned long long* __restrict__ tile_desc, int chunk,
-       int nchunks, unsigned tile_begin, unsigned tile_end_cap) {
+       int nchunks, unsigned tile_begin, unsigned tile_end_cap, uint32_t* __restrict__ parent_of) {
   using CG = CopyGeo<L>;
   using V = typename VecT<CG::VB>::type;
   if (st->status != ST_OK) return;
@@ -660,6 +660,11 @@ k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restric
   }
   __syncthreads();
 
+  if (parent_of != nullptr) {
+    // gather-on-load mode (theta > 0): the sweep kernel reads every child's lattice straight from its parent's slot and
+    // recomputes E, M, so a6 shrinks to the child -> parent map (4 B per child instead of 2 S + 16)
+    for (unsigned c = threadIdx.x; c < nchild; c += COPY_THREADS) parent_of[i0 + c] = s_par[c];
+  } else {
   // E, M of the children
   for (unsigned c = threadIdx.x; c < nchild; c += COPY_THREADS) {
     const uint32_t pj = s_par[c];
@@ -680,6 +685,7 @@ k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restric
       for (int u = 0; u < UNR; ++u) dst[(i0 + c + u * GROUPS) * CG::VT + sub] = tmp[u];
     }
     for (; c < nchild; c += GROUPS) dst[(i0 + c) * CG::VT + sub] = src[(unsigned long long)s_par[c] * CG::VT + sub];
+  }
   }
   // a5: every offset is in memory once this kernel runs; block 0 writes the partition table and the diagnostics
   if (last && blockIdx.x == 0) {

@@ -46,6 +46,8 @@ struct SweepArgs {
   int theta;
   int mode;  // 0: inside a step -> buffer cur^1, Rnew replicas, theta sweeps keyed with step ordinal st->step + 1
              // 1: init / set_spins -> buffer cur, R replicas, no sweeps (energies only)
+             // 2: as 0, but the lattice of slot i is LOADED from slot parent_of[i] of buffer cur (gather-on-load: the
+             //    redistribution copy a6 is fused into the sweep's load) and stored to slot i of buffer cur^1
 };
 
 __device__ __forceinline__ uint32_t even_bits(uint32_t x) {  // bits 0,2,4,.. -> bits 0..15
@@ -280,16 +282,16 @@ __device__ __forceinline__ void planes_to_row(const uint32_t (&p0)[Geo<L>::WPP],
 
 template <int L>
 __global__ void __launch_bounds__(SWEEP_THREADS, (L >= 128 ? PA_SWEEP_MINB128 : PA_SWEEP_MINB64))
-k_sweep(const DevState* __restrict__ st, uint32_t* __restrict__ spins0, uint32_t* __restrict__ spins1,
+k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
         int32_t* __restrict__ E0, int32_t* __restrict__ E1, int32_t* __restrict__ M0, int32_t* __restrict__ M1,
-        const PhiloxKey key, const SweepArgs sa) {
+        const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of) {
   using G_ = Geo<L>;
   static_assert(L >= 64, "k_sweep_small handles L < 64");
   if (st->status != ST_OK) return;
-  const unsigned buf = sa.mode == 0 ? (st->cur ^ 1u) : st->cur;
-  const unsigned long long count = sa.mode == 0 ? st->Rnew : st->R;
-  const int theta = sa.mode == 0 ? sa.theta : 0;
-  uint32_t* __restrict__ spins = buf ? spins1 : spins0;
+  const unsigned buf = sa.mode != 1 ? (st->cur ^ 1u) : st->cur;
+  const unsigned long long count = sa.mode != 1 ? st->Rnew : st->R;
+  const int theta = sa.mode != 1 ? sa.theta : 0;
+  uint32_t* spins = buf ? spins1 : spins0;
   int32_t* __restrict__ Eo = buf ? E1 : E0;
   int32_t* __restrict__ Mo = buf ? M1 : M0;
 
@@ -299,13 +301,15 @@ k_sweep(const DevState* __restrict__ st, uint32_t* __restrict__ spins0, uint32_t
   if (slot64 >= count) return;  // warp-uniform
   const uint32_t slot = (uint32_t)slot64;
   uint32_t* rep = spins + slot64 * G_::WREP;
+  const uint32_t* rep_src = rep;
+  if (sa.mode == 2) rep_src = (buf ? spins0 : spins1) + (unsigned long long)parent_of[slot64] * G_::WREP;  // parent, buffer cur
 
   // ---- load (once per step): the lane's rows are RPL*WR contiguous words = RPL*WR/4 16-byte vectors ----
   Lattice<L> lat;
   constexpr int NV = G_::RPL * G_::WR / 4;
   {
     uint32_t rawall[G_::RPL * G_::WR];
-    const uint4* src = reinterpret_cast<const uint4*>(rep) + g * NV;
+    const uint4* src = reinterpret_cast<const uint4*>(rep_src) + g * NV;
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const uint4 q = src[v];
@@ -395,16 +399,16 @@ __device__ __forceinline__ void small_neighbours(uint32_t S, int g, uint32_t& U,
 
 template <int L>
 __global__ void __launch_bounds__(SWEEP_THREADS)
-k_sweep_small(const DevState* __restrict__ st, uint32_t* __restrict__ spins0, uint32_t* __restrict__ spins1,
+k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
               int32_t* __restrict__ E0, int32_t* __restrict__ E1, int32_t* __restrict__ M0, int32_t* __restrict__ M1,
-              const PhiloxKey key, const SweepArgs sa) {
+              const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of) {
   using G_ = SGeo<L>;
   static_assert(L == 8 || L == 16 || L == 32, "");
   if (st->status != ST_OK) return;
-  const unsigned buf = sa.mode == 0 ? (st->cur ^ 1u) : st->cur;
-  const unsigned long long count = sa.mode == 0 ? st->Rnew : st->R;
-  const int theta = sa.mode == 0 ? sa.theta : 0;
-  uint32_t* __restrict__ spins = buf ? spins1 : spins0;
+  const unsigned buf = sa.mode != 1 ? (st->cur ^ 1u) : st->cur;
+  const unsigned long long count = sa.mode != 1 ? st->Rnew : st->R;
+  const int theta = sa.mode != 1 ? sa.theta : 0;
+  uint32_t* spins = buf ? spins1 : spins0;
   int32_t* __restrict__ Eo = buf ? E1 : E0;
   int32_t* __restrict__ Mo = buf ? M1 : M0;
 
@@ -418,11 +422,13 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* __restrict__ spins0, ui
   const bool valid = slot64 < count;
   const uint32_t slot = (uint32_t)slot64;
   uint32_t* rep = spins + (valid ? slot64 : 0ull) * G_::WREP;
+  const uint32_t* rep_src = rep;
+  if (sa.mode == 2 && valid) rep_src = (buf ? spins0 : spins1) + (unsigned long long)parent_of[slot64] * G_::WREP;
 
   // ---- load: 64 raw bits = RG rows ---------------------------------------------------------------
   uint32_t p[2];
   {
-    const uint2 q = valid ? reinterpret_cast<const uint2*>(rep)[g] : make_uint2(0u, 0u);
+    const uint2 q = valid ? reinterpret_cast<const uint2*>(rep_src)[g] : make_uint2(0u, 0u);
     const uint32_t ev = even_bits(q.x) | (even_bits(q.y) << 16);
     const uint32_t od = even_bits(q.x >> 1) | (even_bits(q.y >> 1) << 16);
     p[0] = (ev & G_::ER) | (od & ~G_::ER);  // even row: colour 0 sits at even x; odd row: at odd x
