@@ -112,17 +112,24 @@ __device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uin
     }
   }
   for (;;) {
-    int sel = -1;
+    // the lane's first undecided word; a lane with none idles on word 0 (und = 0 there: the comparator leaves a decided
+    // word untouched, so nothing has to be masked)
+    int sel = 0;
+    bool busy = und[0] != 0u;
 #pragma unroll
-    for (int i = NW - 1; i >= 0; --i)
-      if (und[i] != 0u) sel = i;
-    if (!__any_sync(0xffffffffu, sel >= 0)) break;
-    uint32_t s_und = 0u, s_v = 0u, s_ge1 = 0u, s_call = 0u, s_c = 2u;
+    for (int i = NW - 1; i >= 1; --i)  // descending: the lowest undecided index wins
+      if (und[i] != 0u) {
+        if (und[0] == 0u) sel = i;
+        busy = true;
+      }
+    if (!__any_sync(0xffffffffu, busy)) break;
+    uint32_t s_und = und[0], s_v = v[0], s_ge1 = ge1[0], s_call = call0[0], s_c = nxt[0];
 #pragma unroll
-    for (int i = 0; i < NW; ++i)
+    for (int i = 1; i < NW; ++i)
       if (sel == i) {
         s_und = und[i]; s_v = v[i]; s_ge1 = ge1[i]; s_call = call0[i]; s_c = nxt[i];
       }
+    s_c &= 7u;  // an idling lane may have counted past the last block
     const uint4 w = philox4x32_10(slot, s_call + s_c, c2, c3, key);
     cmp_block(s_und, s_v, w, s_ge1, sa.a + 4u * s_c, sa.b + 4u * s_c);
     if (s_c == 7u) {  // all 32 bits equal: u == T is not less
