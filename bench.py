@@ -37,9 +37,10 @@ ALU_OPS_PER_ATTEMPT = (E_BLK * (19 + 12) + 12) / 32.0
 I_MIN_SURVEY = 12.0   # one 32-bit Philox word per attempt at 1 warp-instr/clk/SMSP (kept for continuity)
 SM_COUNT, SMSP, LANES, ALU_LANES = 148, 4, 32, 16
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the `ncu --set full` capture
-# (profiles/r1j_sweep64_ncu.md: config 3, one launch = theta sweeps of R' ~ 2^21 replicas; algorithmic 2*S*R' + 8R').
+# (profiles/r1l_sweep64_ncu.md: config 3, one launch = gather + theta sweeps of R' ~ 2^21 replicas; algorithmic
+# S*(U + R') + 12R': each surviving parent read once, each child written once).
 # Reported only for the workload it was captured on.
-NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 1.076945e9 + 1.032770e9}
+NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 0.650892e9 + 1.039523e9}
 # same for the a1-a6 chain of config 5 (profiles/r1k_resample_ncu.md; k_q_reduce from the r1f capture): q_reduce + levels_tau
 # + poisson_scan + copy, read + write
 NCU_RESAMPLE_TRAFFIC_BYTES = 67.12e6 + 0.014e6 + (67.28e6 + 21.58e6) + (671.23e6 + 2223.73e6)
