@@ -197,7 +197,7 @@ void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
     k_sweep<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa,
                                                       c->dev<uint32_t>(c->lo.parent_of));
   } else {
-    const uint64_t threads = (uint64_t)c->cap * SGeo<L>::G;
+    const uint64_t threads = ((uint64_t)c->cap + 1) / 2 * SGeo<L>::G;  // a group of G lanes holds two replicas
     const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
     k_sweep_small<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa,
                                                             c->dev<uint32_t>(c->lo.parent_of));

@@ -93,7 +93,8 @@ __device__ __forceinline__ void cmp_block(uint32_t& und, uint32_t& v, const uint
 //            by one block -- the stragglers of different words of a lane share the warp's instruction slots.
 // Blocks that are never computed cannot change a decided site, so the result is the plain definition's.
 template <int NW>
-__device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uint32_t (&ge2)[NW], uint32_t slot,
+__device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uint32_t (&ge2)[NW],
+                                            const uint32_t (&slot)[NW],  // replica of each word (all equal for L >= 64)
                                             const uint32_t (&call0)[NW], uint32_t c2, uint32_t c3, const PhiloxKey& key,
                                             const SweepArgs& sa, uint32_t (&flip)[NW]) {
   uint32_t und[NW], v[NW], nxt[NW];
@@ -107,7 +108,7 @@ __device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uin
   for (int c = 0; c < PA_SWEEP_STAGE1; ++c) {
 #pragma unroll
     for (int i = 0; i < NW; ++i) {
-      const uint4 w = philox4x32_10(slot, call0[i] + (uint32_t)c, c2, c3, key);
+      const uint4 w = philox4x32_10(slot[i], call0[i] + (uint32_t)c, c2, c3, key);
       cmp_block(und[i], v[i], w, ge1[i], sa.a + 4 * c, sa.b + 4 * c);
     }
   }
@@ -123,14 +124,14 @@ __device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uin
         busy = true;
       }
     if (!__any_sync(0xffffffffu, busy)) break;
-    uint32_t s_und = und[0], s_v = v[0], s_ge1 = ge1[0], s_call = call0[0], s_c = nxt[0];
+    uint32_t s_und = und[0], s_v = v[0], s_ge1 = ge1[0], s_call = call0[0], s_c = nxt[0], s_slot = slot[0];
 #pragma unroll
     for (int i = 1; i < NW; ++i)
       if (sel == i) {
-        s_und = und[i]; s_v = v[i]; s_ge1 = ge1[i]; s_call = call0[i]; s_c = nxt[i];
+        s_und = und[i]; s_v = v[i]; s_ge1 = ge1[i]; s_call = call0[i]; s_c = nxt[i]; s_slot = slot[i];
       }
     s_c &= 7u;  // an idling lane may have counted past the last block
-    const uint4 w = philox4x32_10(slot, s_call + s_c, c2, c3, key);
+    const uint4 w = philox4x32_10(s_slot, s_call + s_c, c2, c3, key);
     cmp_block(s_und, s_v, w, s_ge1, sa.a + 4u * s_c, sa.b + 4u * s_c);
     if (s_c == 7u) {  // all 32 bits equal: u == T is not less
       s_v |= s_und;
@@ -223,8 +224,10 @@ __device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot
       call0[r * G_::WPP + i] = 8u * ((uint32_t)y * G_::WPP + (uint32_t)i);  // group = y * WPP + i
     }
   }
-  uint32_t flip[NWL];
-  lazy_accept<NWL>(ge1, ge2, slot, call0, c2, c3, key, sa, flip);
+  uint32_t flip[NWL], slots[NWL];
+#pragma unroll
+  for (int w = 0; w < NWL; ++w) slots[w] = slot;
+  lazy_accept<NWL>(ge1, ge2, slots, call0, c2, c3, key, sa, flip);
 #pragma unroll
   for (int w = 0; w < NWL; ++w) T[w / G_::WPP][w % G_::WPP] ^= flip[w];
 }
@@ -419,78 +422,98 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
   int32_t* __restrict__ Eo = buf ? E1 : E0;
   int32_t* __restrict__ Mo = buf ? M1 : M0;
 
+  // A group of G lanes holds TWO consecutive replicas (one plane word per colour and replica per lane): the two words
+  // of a lane share the straggler iterations of the lazy comparison, as the rows of a lane do for L >= 64.
+  constexpr int NR = 2;
   const unsigned long long tid = (unsigned long long)blockIdx.x * SWEEP_THREADS + threadIdx.x;
-  const unsigned long long slot64 = tid / G_::G;
+  const unsigned long long pair = tid / G_::G;
   const int g = (int)(tid % G_::G);
   {  // warp-uniform exit for warps entirely past the population
-    const unsigned long long first_slot_of_warp = (tid & ~31ull) / G_::G;
+    const unsigned long long first_slot_of_warp = ((tid & ~31ull) / G_::G) * NR;
     if (first_slot_of_warp >= count) return;
   }
-  const bool valid = slot64 < count;
-  const uint32_t slot = (uint32_t)slot64;
-  uint32_t* rep = spins + (valid ? slot64 : 0ull) * G_::WREP;
-  const uint32_t* rep_src = rep;
-  if (sa.mode == 2 && valid) rep_src = (buf ? spins0 : spins1) + (unsigned long long)parent_of[slot64] * G_::WREP;
-
-  // ---- load: 64 raw bits = RG rows ---------------------------------------------------------------
-  uint32_t p[2];
-  {
-    const uint2 q = valid ? reinterpret_cast<const uint2*>(rep_src)[g] : make_uint2(0u, 0u);
+  unsigned long long slot64[NR];
+  bool valid[NR];
+  uint32_t slots[NR];
+  uint32_t* rep[NR];
+  uint32_t p[NR][2];
+#pragma unroll
+  for (int r = 0; r < NR; ++r) {
+    slot64[r] = pair * NR + r;
+    valid[r] = slot64[r] < count;
+    slots[r] = (uint32_t)slot64[r];
+    rep[r] = spins + (valid[r] ? slot64[r] : 0ull) * G_::WREP;
+    const uint32_t* rep_src = rep[r];
+    if (sa.mode == 2 && valid[r]) rep_src = (buf ? spins0 : spins1) + (unsigned long long)parent_of[slot64[r]] * G_::WREP;
+    // ---- load: 64 raw bits = RG rows -------------------------------------------------------------
+    const uint2 q = valid[r] ? reinterpret_cast<const uint2*>(rep_src)[g] : make_uint2(0u, 0u);
     const uint32_t ev = even_bits(q.x) | (even_bits(q.y) << 16);
     const uint32_t od = even_bits(q.x >> 1) | (even_bits(q.y >> 1) << 16);
-    p[0] = (ev & G_::ER) | (od & ~G_::ER);  // even row: colour 0 sits at even x; odd row: at odd x
-    p[1] = (od & G_::ER) | (ev & ~G_::ER);
+    p[r][0] = (ev & G_::ER) | (od & ~G_::ER);  // even row: colour 0 sits at even x; odd row: at odd x
+    p[r][1] = (od & G_::ER) | (ev & ~G_::ER);
   }
 
   // ---- theta sweeps ----------------------------------------------------------------------------
   if (theta > 0) {
     const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
-    const uint32_t call0[1] = {8u * (uint32_t)g};  // group = g
+    uint32_t call0[NR];
+#pragma unroll
+    for (int r = 0; r < NR; ++r) call0[r] = 8u * (uint32_t)g;  // group = g
     for (int t = 0; t < theta; ++t) {
       {
-        uint32_t U, D, B, ge1[1], ge2[1], flip[1];
-        small_neighbours<L, 0>(p[1], g, U, D, B);
-        neighbour_classes(p[0], U, D, p[1], B, ge1[0], ge2[0]);
-        if (!valid) { ge1[0] = 0xffffffffu; ge2[0] = 0xffffffffu; }  // padding lanes never hold the warp back
-        lazy_accept<1>(ge1, ge2, slot, call0, 2u * (uint32_t)t, c3, key, sa, flip);
-        p[0] ^= flip[0];
+        uint32_t ge1[NR], ge2[NR], flip[NR];
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+          uint32_t U, D, B;
+          small_neighbours<L, 0>(p[r][1], g, U, D, B);
+          neighbour_classes(p[r][0], U, D, p[r][1], B, ge1[r], ge2[r]);
+          if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }  // padding never holds the warp back
+        }
+        lazy_accept<NR>(ge1, ge2, slots, call0, 2u * (uint32_t)t, c3, key, sa, flip);
+#pragma unroll
+        for (int r = 0; r < NR; ++r) p[r][0] ^= flip[r];
       }
       {
-        uint32_t U, D, B, ge1[1], ge2[1], flip[1];
-        small_neighbours<L, 1>(p[0], g, U, D, B);
-        neighbour_classes(p[1], U, D, p[0], B, ge1[0], ge2[0]);
-        if (!valid) { ge1[0] = 0xffffffffu; ge2[0] = 0xffffffffu; }
-        lazy_accept<1>(ge1, ge2, slot, call0, 2u * (uint32_t)t + 1u, c3, key, sa, flip);
-        p[1] ^= flip[0];
+        uint32_t ge1[NR], ge2[NR], flip[NR];
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+          uint32_t U, D, B;
+          small_neighbours<L, 1>(p[r][0], g, U, D, B);
+          neighbour_classes(p[r][1], U, D, p[r][0], B, ge1[r], ge2[r]);
+          if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }
+        }
+        lazy_accept<NR>(ge1, ge2, slots, call0, 2u * (uint32_t)t + 1u, c3, key, sa, flip);
+#pragma unroll
+        for (int r = 0; r < NR; ++r) p[r][1] ^= flip[r];
       }
     }
   }
 
-  // ---- a8: every bond has exactly one colour-0 end ------------------------------------------------
-  {
+#pragma unroll
+  for (int r = 0; r < NR; ++r) {
+    // ---- a8: every bond has exactly one colour-0 end ----------------------------------------------
     uint32_t U, D, B;
-    small_neighbours<L, 0>(p[1], g, U, D, B);
-    int unsat = __popc(p[0] ^ U) + __popc(p[0] ^ D) + __popc(p[0] ^ p[1]) + __popc(p[0] ^ B);
-    int ups = __popc(p[0]) + __popc(p[1]);
+    small_neighbours<L, 0>(p[r][1], g, U, D, B);
+    int unsat = __popc(p[r][0] ^ U) + __popc(p[r][0] ^ D) + __popc(p[r][0] ^ p[r][1]) + __popc(p[r][0] ^ B);
+    int ups = __popc(p[r][0]) + __popc(p[r][1]);
 #pragma unroll
     for (int o = G_::G / 2; o > 0; o >>= 1) {
       unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
       ups += __shfl_xor_sync(0xffffffffu, ups, o);
     }
-    if (valid && g == 0) {
-      Eo[slot64] = 2 * unsat - 2 * G_::N;
-      Mo[slot64] = 2 * ups - G_::N;
+    if (valid[r] && g == 0) {
+      Eo[slot64[r]] = 2 * unsat - 2 * G_::N;
+      Mo[slot64[r]] = 2 * ups - G_::N;
     }
-  }
-
-  // ---- store -------------------------------------------------------------------------------------
-  if (theta > 0 && valid) {
-    const uint32_t ev = (p[0] & G_::ER) | (p[1] & ~G_::ER);
-    const uint32_t od = (p[1] & G_::ER) | (p[0] & ~G_::ER);
-    uint2 q;
-    q.x = spread_bits(ev) | (spread_bits(od) << 1);
-    q.y = spread_bits(ev >> 16) | (spread_bits(od >> 16) << 1);
-    reinterpret_cast<uint2*>(rep)[g] = q;
+    // ---- store -----------------------------------------------------------------------------------
+    if (theta > 0 && valid[r]) {
+      const uint32_t ev = (p[r][0] & G_::ER) | (p[r][1] & ~G_::ER);
+      const uint32_t od = (p[r][1] & G_::ER) | (p[r][0] & ~G_::ER);
+      uint2 q;
+      q.x = spread_bits(ev) | (spread_bits(od) << 1);
+      q.y = spread_bits(ev >> 16) | (spread_bits(od >> 16) << 1);
+      reinterpret_cast<uint2*>(rep[r])[g] = q;
+    }
   }
 }
 
