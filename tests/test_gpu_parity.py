@@ -214,6 +214,17 @@ def test_skewed_resampling_heavy_parents():
     lockstep(gpu, ora, [0.32], 2)
 
 
+@pytest.mark.parametrize("L,R", [(64, 3000), (128, 1500), (16, 5000)])
+def test_wide_level_window_fallback_paths(L, R):
+    """crafted populations spanning -2N..+2N: the occupied level window is wider than the shared-memory tables
+    (k_q_reduce evaluates exp per replica beyond 2048 levels; k_poisson_scan mixes cached and uncached levels), then
+    narrows again after resampling -- every path must give the oracle's bits"""
+    spins = inputs.structured_population(L, R, seed=100 + L)
+    gpu, ora = make_pair(L, R, P=5, seed=9, beta0=0.2, spins=spins, capacity=4 * R)
+    dbeta = 0.25 * 700.0 / (2 * L * L) if L >= 64 else 0.01   # large enough to skew the counts, within |dbeta| 2N < 700
+    lockstep(gpu, ora, [0.2 + dbeta, 0.2 + 1.5 * dbeta, 0.2 + 1.6 * dbeta], 1)
+
+
 def test_config5_reduced_resample_only():
     wl = inputs.CONFIGS[5].scaled(1 << 17)
     gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed, beta0=wl.beta0)
