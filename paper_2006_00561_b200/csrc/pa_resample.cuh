@@ -241,15 +241,21 @@ struct ScanOut {
 };
 
 constexpr int SCAN_BATCH = 4;  // independent Philox chains in flight per thread
-constexpr int SCAN_HW = 256;   // levels whose first CDF group is cached in shared memory
+#ifndef PA_SCAN_HW
+#define PA_SCAN_HW 192
+#endif
+constexpr int SCAN_HW = PA_SCAN_HW;
 constexpr unsigned NO_TILE = 0xffffffffu;
 
 // The kernel is software-pipelined over tiles: a block draws the counts of tile B and publishes its aggregate BEFORE it
 // resolves the prefix of its previous tile A and writes A's offsets, so the look-back latency (descriptors of up to
 // A tiles, 32 per round trip) is hidden behind B's sampling.  Every ticket holder publishes its aggregate before it
 // waits on anything, so the look-back cannot deadlock.
+#ifndef PA_SCAN_MINB
+#define PA_SCAN_MINB 6
+#endif
 template <bool KEEP>
-__global__ void __launch_bounds__(SCAN_THREADS, 5)
+__global__ void __launch_bounds__(SCAN_THREADS, PA_SCAN_MINB)
 k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
                ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key, int chunk,
                unsigned tile_begin, unsigned tile_end_cap) {
