@@ -41,7 +41,7 @@ SM_COUNT, SMSP, LANES, ALU_LANES = 148, 4, 32, 16
 # S*(U + R') + 12R': each surviving parent read once, each child written once).
 # Reported only for the workload it was captured on.
 NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 0.650892e9 + 1.039523e9}
-# same for the a1-a6 chain of config 5 (profiles/r1k_resample_ncu.md; k_q_reduce from the r1f capture): q_reduce + levels_tau
+# same for the a1-a6 chain of config 5 (profiles/r1n_resample_ncu.md; k_q_reduce from the r1f capture): q_reduce + levels_tau
 # + poisson_scan + copy, read + write
 NCU_RESAMPLE_TRAFFIC_BYTES = 67.12e6 + 0.014e6 + (67.28e6 + 21.58e6) + (671.23e6 + 2223.73e6)
 
