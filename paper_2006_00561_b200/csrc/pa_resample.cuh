@@ -2,8 +2,10 @@
 // partition balance and the replica gather-copy.  PAPER.md:44-56, :84, :94, :104-106; C5, A4, A5, A6.
 //
 // lambda_j depends on j only through the integer energy E_j = 4*lev - 2N, lev = 0..N, so everything that is
-// floating point is tabulated per energy LEVEL (N+1 levels) by two tiny kernels; the per-replica kernels only
-// look the tables up.  The arithmetic per level is exactly the sequence written in DESIGN.md.
+// floating point is tabulated per energy LEVEL; the per-replica kernels only look the tables up.  A population
+// occupies a few hundred adjacent levels [lev_lo, lev_hi] (recorded by k_observe when the population is written), so
+// the tables are built for that window only (w inside k_q_reduce, the rest by k_levels_tau) and their hot part is held
+// in shared memory.  The arithmetic per level is exactly the sequence written in DESIGN.md.
 #pragma once
 #include <type_traits>
 
