@@ -384,3 +384,24 @@ def test_device_getters_and_launch_count():
     assert np.array_equal(Ed.cpu().numpy(), E) and np.array_equal(Md.cpu().numpy(), M)
     prof = g.profile_read()
     assert all(cnt == (0 if k in ("balance", "levels_w") else 1) for k, (_, cnt) in prof.items()) and prof["sweep"][0] > 0
+
+
+def test_bench_line_carries_the_contract_keys():
+    """bench.py (our arm, config 1 to keep it short): one JSON line with the driver contract's keys, the roofline /
+    e2e / cpu_baseline objects of the tier framing, and a non-zero count of OUR kernel launches"""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--config", "1", "--steps", "5", "--warmup", "3",
+                          "--no-resample"], capture_output=True, text=True, timeout=600, check=True).stdout
+    line = json.loads(out.strip().splitlines()[-1])
+    for key in ["metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"]:
+        assert key in line, key
+    assert line["metric"] == "spin_flip_attempts_per_s" and line["steps"] == 5 and line["n_gpus"] == 1
+    assert line["value"] > 0 and line["gpu_launches"] == 5 * 6 and line["data"] == "synthetic"
+    assert line["config"]["workload"].startswith("config1") and line["vs_baseline"] is None
+    assert set(["bound", "achieved", "peak", "unit", "frac", "traffic"]) <= set(line["roofline"])
+    assert line["e2e"]["h2d_bytes_per_step"] > 0 and line["e2e"]["d2h_bytes_per_step"] > 0 and line["e2e"]["value"] > 0
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
