@@ -284,6 +284,25 @@ def test_run_equals_repeated_step_and_is_deterministic():
     assert a.beta_steps() == c.beta_steps() == (betas[-1], len(betas))
 
 
+def test_run_longer_than_the_parameter_ring():
+    """pa_run uploads step parameters in chunks of 1024: a schedule of 2100 steps in one call equals the same schedule
+    in three calls (and the oracle at a few check points would be slow: determinism + ln Z continuity is the check)"""
+    b = _binding()
+    betas = [2e-4 * k for k in range(1, 2101)]
+    a = b.PopulationAnnealer(8, 300, P=3, seed=12)
+    assert a.run(betas, 1) == 2100
+    c = b.PopulationAnnealer(8, 300, P=3, seed=12)
+    assert c.run(betas[:7], 1) + c.run(betas[7:1500], 1) + c.run(betas[1500:], 1) == 2100
+    assert a.R == c.R and np.array_equal(a.spins(), c.spins())
+    assert a.log_Z() == c.log_Z() and a.observables() == c.observables() and a.beta_steps() == c.beta_steps()
+    ora = orc.OraclePA(8, 300, P=3, seed=12)
+    for beta in betas[:40]:
+        ora.step(beta, 1)
+    d = b.PopulationAnnealer(8, 300, P=3, seed=12)
+    d.run(betas[:40], 1)
+    compare_population(d, ora, "40 steps")  # counts come from each side's own tau here: equal unless a 1e-16 tie
+
+
 def test_capacity_error_leaves_population_unchanged():
     b = _binding()
     g = b.PopulationAnnealer(16, 1024, P=2, seed=3, capacity=1024)
