@@ -405,6 +405,67 @@ def test_sweep_random_keying_on_all_up_lattice():
     assert not np.array_equal(pop2[0], pop[0])
 
 
+@pytest.mark.parametrize("L", [16, 32])
+def test_sweep_keying_groups_beyond_the_first_on_all_up_lattice(L):
+    """DESIGN.md C3 (reading G20) for group index gamma > 0: L = 16 has 4 groups per half-sweep, L = 32 has 16, so the
+    counter word c1 = 8*gamma + (b >> 2) is exercised for gamma up to 15.  All-up lattice: every colour-0 site has
+    a = 0 and flips iff its keyed 32-bit uniform (big-integer writing, tests/philox_ref.py) is < T8."""
+    seed, step = 0x0F1E2D3C4B5A6978, 7
+    T4, T8 = 0x9E3779B9, 0x3243F6A8
+    slots = [0, 5]
+    pop = np.stack([orc.pack(L, np.ones(L * L, np.int8))] * 6)
+    orc.sweeps(L, pop, seed, step, 1, T4, T8)
+    half = L // 2
+    for slot in slots:
+        s = orc.unpack(L, pop[slot]).reshape(L, L)
+        flips = 0
+        for y in range(L):
+            for k in range(half):
+                x = 2 * k + (y & 1)  # colour 0
+                w = philox_ref.sweep_word(seed, step, slot, 0, 0, y * half + k)
+                assert s[y, x] == (-1 if w < T8 else 1), (slot, y, x)
+                flips += w < T8
+        assert 0.1 * L * half < flips < 0.3 * L * half  # p = T8 / 2^32 = 0.196: the pin is not vacuous
+
+
+def _reference_metropolis(L, spins, seed, step, slot, theta, T4, T8):
+    """C4 + C3 (reading G20) written a second time, from DESIGN.md's prose, on a +-1 numpy grid with the big-integer
+    Philox of tests/philox_ref.py: sweep t = colour 0 then colour 1; active site ordinal q = y*(L/2) + k,
+    x = 2k + ((y + colour) & 1); a = number of anti-aligned neighbours; flip iff a >= 2, or a == 1 and u < T4, or
+    a == 0 and u < T8; u = philox_ref.sweep_word(seed, step, slot, t, colour, q)."""
+    g = np.array(spins, np.int64).reshape(L, L).copy()
+    half = L // 2
+    for t in range(theta):
+        for colour in (0, 1):
+            for y in range(L):
+                for k in range(half):
+                    x = 2 * k + ((y + colour) & 1)
+                    nb = (g[y, (x + 1) % L], g[y, (x - 1) % L], g[(y + 1) % L, x], g[(y - 1) % L, x])
+                    a = sum(1 for v in nb if v != g[y, x])
+                    u = philox_ref.sweep_word(seed, step, slot, t, colour, y * half + k)
+                    if a >= 2 or (a == 1 and u < T4) or (a == 0 and u < T8):
+                        g[y, x] = -g[y, x]
+    return g.reshape(-1).astype(np.int8)
+
+
+@pytest.mark.parametrize("L,beta", [(16, 0.3), (32, 0.44)])
+def test_sweeps_whole_lattice_against_second_writing(L, beta):
+    """Whole lattice after theta = 2 sweeps of random lattices == the independent writing above: fixes the keying of
+    colour 1 (c2 = 2t + 1), of the second sweep (t = 1), of every group gamma, and the bit order of the uniform, for
+    all three neighbour classes (random lattices have a = 0..4 sites)."""
+    seed, step, theta = 0x1122334455667788 + L, 3, 2
+    T4, T8 = orc.thresholds(beta)
+    pop = orc.init_population(L, 3, seed)
+    want = {slot: _reference_metropolis(L, orc.unpack(L, pop[slot]), seed, step, slot, theta, T4, T8) for slot in (0, 2)}
+    orc.sweeps(L, pop, seed, step, theta, T4, T8)
+    for slot, w in want.items():
+        assert np.array_equal(orc.unpack(L, pop[slot]), w), slot
+    # the same through the slot-list entry point with a slot index that is not the position in the list
+    one = orc.init_population(L, 3, seed)[2:3].copy()
+    orc.sweeps_slots(L, np.array([2], np.uint32), one, seed, step, theta, T4, T8)
+    assert np.array_equal(orc.unpack(L, one[0]), want[2])
+
+
 def test_sweeps_slots_equals_sweeps_and_slot_keying():
     L, R, seed, step = 8, 64, 77, 5
     pop = orc.init_population(L, R, seed)
