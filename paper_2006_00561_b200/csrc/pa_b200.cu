@@ -192,8 +192,7 @@ void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
   int32_t *m0 = c->dev<int32_t>(c->lo.M[0]), *m1 = c->dev<int32_t>(c->lo.M[1]);
   const DevState* st = c->dev<DevState>(c->lo.state);
   if constexpr (L >= 64) {
-    const uint64_t threads = (uint64_t)c->cap * Geo<L>::G;
-    const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
+    const unsigned grid = (unsigned)(((uint64_t)c->cap + Geo<L>::RPB - 1) / Geo<L>::RPB);
     k_sweep<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa,
                                                       c->dev<uint32_t>(c->lo.parent_of));
   } else {

@@ -16,21 +16,32 @@
 // evaluated for the 32 sites of the word AT ONCE by a bit-sliced comparator that walks the words most significant
 // bit first: one LOP3 tracks the sites whose bits have all been equal to the threshold's so far, one LOP3 remembers
 // the last random bit seen while a site was still undecided.  A site is decided at the first bit that differs
-// (probability 1/2 per bit), so the loop stops -- warp-uniformly -- as soon as no site of the warp is undecided:
-// on average 3.3 of the 8 Philox blocks of a group are ever computed.  The result is independent of where the
-// loop stops (decided sites do not change), so it equals the plain definition bit for bit.
+// (probability 1/2 per bit).  Every word gets its first two Philox blocks (8 bits: 255 of 256 sites decided, 88 % of the
+// words complete) from the lane that owns it; the words that still have an undecided site -- the stragglers -- are
+// COMPACTED across the whole thread block into a shared-memory queue and finished densely, one word per thread, so
+// that a straggler costs one lane-block instead of a warp-wide iteration.  Blocks that are never computed cannot
+// change a decided site, and a word's result does not depend on which thread finishes it, so the result equals the
+// plain definition bit for bit.
 #pragma once
+#include <cstddef>
+
 #include "pa_common.cuh"
 
 // tuning knobs (defaults are the measured best on B200)
 #ifndef PA_SWEEP_THREADS
-#define PA_SWEEP_THREADS 256
+#define PA_SWEEP_THREADS 128
 #endif
 #ifndef PA_SWEEP_MINB64
-#define PA_SWEEP_MINB64 3
+#define PA_SWEEP_MINB64 4
 #endif
 #ifndef PA_SWEEP_MINB128
-#define PA_SWEEP_MINB128 2
+#define PA_SWEEP_MINB128 4
+#endif
+#ifndef PA_SWEEP_RW64
+#define PA_SWEEP_RW64 4
+#endif
+#ifndef PA_SWEEP_RW128
+#define PA_SWEEP_RW128 1
 #endif
 #ifndef PA_SWEEP_STAGE1
 #define PA_SWEEP_STAGE1 2
@@ -84,25 +95,82 @@ __device__ __forceinline__ void cmp_block(uint32_t& und, uint32_t& v, const uint
   cmp_bit(und, v, w.w, ge1, a[3], b[3]);
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Straggler queue of one thread block (shared memory).  An item is one plane word that still has undecided sites
+// after its two mandatory Philox blocks: the comparator state (und, v), the word's a >= 1 mask, and where its keyed
+// words come from (replica slot relative to the block's first slot, first Philox call of the group).
+// Protocol per half-sweep h (parity = h & 1), two block barriers:
+//   push (owners)  --A--  finish items densely, one per thread; thread 0 clears the OTHER parity's counter  --B--
+//   owners OR the late flips of their pushed words into their flip masks.
+// Items and results live in separate arrays, so a fast warp that already pushes for h + 1 never touches what a slow
+// warp still reads for h; only the counter is double buffered.  A push past CAP (cannot happen for L <= 64, where CAP
+// covers every word of the block; 50 sigma away for L = 128) is finished in place by its owner.
+// ---------------------------------------------------------------------------------------------------
+template <int CAP>
+struct SweepQueue {
+  uint4 item[CAP];    // und, v, ge1, (slot - slot_base) << 16 | call0
+  uint32_t res[CAP];  // late flips of the item
+  uint32_t count[2];
+  static constexpr uint32_t OFF_RES = 16u * CAP, OFF_COUNT = 20u * CAP;  // byte offsets (checked in k_sweep*)
+};
+// The queue is addressed through its 32-bit shared-window address (taken once per kernel) so that every access is a
+// plain LDS / STS / ATOMS with an immediate offset.
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr) : "memory");
+  return r;
+}
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t a) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(a) : "memory");
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+  uint32_t r;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(addr) : "memory");
+  return r;
+}
+__device__ __forceinline__ uint32_t atoms_add(uint32_t addr, uint32_t a) {
+  uint32_t r;
+  asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(r) : "r"(addr), "r"(a) : "memory");
+  return r;
+}
+
+// blocks 2..7 of one word: returns the sites of und0 that end with u < T
+__device__ __forceinline__ uint32_t finish_word(uint32_t und, uint32_t v, uint32_t ge1, uint32_t slot, uint32_t call0,
+                                                uint32_t c2, uint32_t c3, const PhiloxKey& key, const SweepArgs& sa) {
+  const uint32_t und0 = und;
+#pragma unroll 1
+  for (uint32_t c = (uint32_t)PA_SWEEP_STAGE1; und != 0u; ++c) {
+    const uint4 w = philox4x32_10(slot, call0 + c, c2, c3, key);
+    cmp_block(und, v, w, ge1, sa.a + 4u * c, sa.b + 4u * c);
+    if (c == 7u) {  // all 32 bits equal: u == T is not less
+      v |= und;
+      und = 0u;
+    }
+  }
+  return ~v & und0;
+}
+
 // flip masks of the NW plane words of a lane.  ge1 / ge2: sites with a >= 1 / a >= 2 anti-aligned neighbours;
 // call0 = 8 * group.   a >= 2: always flip;  a == 1: flip iff u < T4;  a == 0: flip iff u < T8
 // (u < T  <=>  at the first differing bit, most significant first, u has 0).
-//   stage 1: Philox blocks 0 and 1 of every word (8 bits decide 255 of 256 sites; 88 % of the (lane, word) pairs are
-//            completely decided afterwards);
-//   stage 2: while some lane of the warp still has an undecided word, every lane advances ONE of its undecided words
-//            by one block -- the stragglers of different words of a lane share the warp's instruction slots.
-// Blocks that are never computed cannot change a decided site, so the result is the plain definition's.
-template <int NW>
-__device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uint32_t (&ge2)[NW],
-                                            const uint32_t (&slot)[NW],  // replica of each word (all equal for L >= 64)
-                                            const uint32_t (&call0)[NW], uint32_t c2, uint32_t c3, const PhiloxKey& key,
-                                            const SweepArgs& sa, uint32_t (&flip)[NW]) {
-  uint32_t und[NW], v[NW], nxt[NW];
+// Must be called by EVERY thread of the block (it contains block barriers); lanes without work pass ge2 = ~0.
+template <int NW, int THREADS, int CAP>
+__device__ __forceinline__ void queued_accept(uint32_t q /* shared address of the SweepQueue<CAP> */, unsigned parity, const uint32_t (&ge1)[NW],
+                                              const uint32_t (&ge2)[NW],
+                                              const uint32_t (&slot)[NW],  // replica of each word
+                                              uint32_t slot_base,          // first slot of the thread block
+                                              const uint32_t (&call0)[NW], uint32_t c2, uint32_t c3, const PhiloxKey& key,
+                                              const SweepArgs& sa, uint32_t (&flip)[NW]) {
+  constexpr unsigned FULL = 0xffffffffu;
+  constexpr bool CAN_OVERFLOW = CAP < NW * THREADS;
+  uint32_t und[NW], v[NW];
 #pragma unroll
   for (int i = 0; i < NW; ++i) {
     und[i] = ~ge2[i];
     v[i] = 0xffffffffu;
-    nxt[i] = (uint32_t)PA_SWEEP_STAGE1;
   }
 #pragma unroll
   for (int c = 0; c < PA_SWEEP_STAGE1; ++c) {
@@ -112,39 +180,46 @@ __device__ __forceinline__ void lazy_accept(const uint32_t (&ge1)[NW], const uin
       cmp_block(und[i], v[i], w, ge1[i], sa.a + 4 * c, sa.b + 4 * c);
     }
   }
-  for (;;) {
-    // the lane's first undecided word; a lane with none idles on word 0 (und = 0 there: the comparator leaves a decided
-    // word untouched, so nothing has to be masked)
-    int sel = 0;
-    bool busy = und[0] != 0u;
+  // ---- push the stragglers: one shared-memory atomic per warp ----
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned lt = (1u << lane) - 1u;
+  unsigned idx[NW], tot = 0u;
 #pragma unroll
-    for (int i = NW - 1; i >= 1; --i)  // descending: the lowest undecided index wins
-      if (und[i] != 0u) {
-        if (und[0] == 0u) sel = i;
-        busy = true;
-      }
-    if (!__any_sync(0xffffffffu, busy)) break;
-    uint32_t s_und = und[0], s_v = v[0], s_ge1 = ge1[0], s_call = call0[0], s_c = nxt[0], s_slot = slot[0];
-#pragma unroll
-    for (int i = 1; i < NW; ++i)
-      if (sel == i) {
-        s_und = und[i]; s_v = v[i]; s_ge1 = ge1[i]; s_call = call0[i]; s_c = nxt[i]; s_slot = slot[i];
-      }
-    s_c &= 7u;  // an idling lane may have counted past the last block
-    const uint4 w = philox4x32_10(s_slot, s_call + s_c, c2, c3, key);
-    cmp_block(s_und, s_v, w, s_ge1, sa.a + 4u * s_c, sa.b + 4u * s_c);
-    if (s_c == 7u) {  // all 32 bits equal: u == T is not less
-      s_v |= s_und;
-      s_und = 0u;
-    }
-#pragma unroll
-    for (int i = 0; i < NW; ++i)
-      if (sel == i) {
-        und[i] = s_und; v[i] = s_v; nxt[i] = s_c + 1u;
-      }
+  for (int i = 0; i < NW; ++i) {
+    const unsigned bal = __ballot_sync(FULL, und[i] != 0u);
+    idx[i] = tot + (unsigned)__popc(bal & lt);
+    tot += (unsigned)__popc(bal);
+  }
+  unsigned base = 0u;
+  if (tot != 0u) {  // warp-uniform
+    if (lane == 0u) base = atoms_add(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity, tot);
+    base = __shfl_sync(FULL, base, 0);
   }
 #pragma unroll
-  for (int i = 0; i < NW; ++i) flip[i] = ge2[i] | ~v[i];
+  for (int i = 0; i < NW; ++i) {
+    idx[i] += base;
+    flip[i] = (ge2[i] | ~v[i]) & ~und[i];  // the sites decided so far; the rest comes back through q.res
+    if (CAN_OVERFLOW && und[i] != 0u && idx[i] >= (unsigned)CAP) {  // queue full: the owner finishes its word in place
+      flip[i] |= finish_word(und[i], v[i], ge1[i], slot[i], call0[i], c2, c3, key, sa);
+      und[i] = 0u;
+    }
+    if (und[i] != 0u) sts128(q + 16u * idx[i], und[i], v[i], ge1[i], ((slot[i] - slot_base) << 16) | call0[i]);
+  }
+  __syncthreads();  // A: every push of this half-sweep is visible
+  {
+    unsigned n = lds32(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity);
+    if (CAN_OVERFLOW && n > (unsigned)CAP) n = (unsigned)CAP;
+    if (threadIdx.x == 0) sts32(q + SweepQueue<CAP>::OFF_COUNT + 4u * (parity ^ 1u), 0u);  // last read before barrier B of the previous half-sweep
+    for (unsigned it = threadIdx.x; it < n; it += THREADS) {
+      const uint4 m = lds128(q + 16u * it);
+      sts32(q + SweepQueue<CAP>::OFF_RES + 4u * it,
+            finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
+    }
+  }
+  __syncthreads();  // B: every result is visible
+#pragma unroll
+  for (int i = 0; i < NW; ++i)
+    if (und[i] != 0u) flip[i] |= lds32(q + SweepQueue<CAP>::OFF_RES + 4u * idx[i]);
 }
 
 // masks of the sites with a >= 1 and a >= 2 from the four difference words (1 = anti-aligned)
@@ -160,7 +235,8 @@ __device__ __forceinline__ void neighbour_classes(uint32_t tt, uint32_t U, uint3
 constexpr int SWEEP_THREADS = PA_SWEEP_THREADS;
 
 // =====================================================================================================
-// L >= 64
+// L >= 64: a warp holds RW consecutive replicas (lane g holds rows g*RPL .. of each), so that a lane owns
+// NWL = RW * RPL * WPP plane words per half-sweep and the block's straggler queue is fed by 8 words per lane.
 // =====================================================================================================
 template <int L>
 struct Geo {
@@ -171,6 +247,17 @@ struct Geo {
   static constexpr int WPP = HB / 32;             // words per row plane
   static constexpr int WR = L / 32;               // raw words per row
   static constexpr int WREP = N / 32;             // words per replica
+  static constexpr int RW = L >= 128 ? PA_SWEEP_RW128 : PA_SWEEP_RW64;  // replicas per warp
+  static constexpr int NWR = RPL * WPP;           // plane words of one replica per lane and half-sweep
+  static constexpr int NWL = RW * NWR;            // plane words per lane and half-sweep
+  static constexpr int RPB = (SWEEP_THREADS / 32) * RW;  // replicas per block
+};
+
+// capacity of the block's straggler queue: every word of a half-sweep up to 1024 items, 1024 beyond
+template <int NW>
+struct SweepCap {
+  static constexpr int WORDS = NW * SWEEP_THREADS;  // plane words per block and half-sweep
+  static constexpr int CAP = WORDS <= 1024 ? WORDS : 1024;
 };
 
 template <int L>
@@ -192,44 +279,52 @@ __device__ __forceinline__ void rot_row(const uint32_t (&s)[Geo<L>::WPP], int di
   }
 }
 
-// One half-sweep of colour C on the lane's rows.  T = plane C (updated), S = plane 1-C (read only).
+// One half-sweep of colour C on the lane's rows of the warp's RW replicas.  T = plane C (updated), S = plane 1-C.
 template <int L, int C>
-__device__ __forceinline__ void half_sweep(Lattice<L>& lat, int g, uint32_t slot, uint32_t t, uint32_t c3,
-                                           const PhiloxKey& key, const SweepArgs& sa) {
+__device__ __forceinline__ void half_sweep(Lattice<L> (&lat)[Geo<L>::RW], uint32_t q, int g,
+                                           uint32_t slot0, uint32_t slot_base, const bool (&valid)[Geo<L>::RW],
+                                           uint32_t t, uint32_t c3, const PhiloxKey& key, const SweepArgs& sa) {
   using G_ = Geo<L>;
   constexpr unsigned FULL = 0xffffffffu;
-  constexpr int NWL = G_::RPL * G_::WPP;  // plane words of this lane
-  uint32_t(&T)[G_::RPL][G_::WPP] = lat.p[C];
-  uint32_t(&S)[G_::RPL][G_::WPP] = lat.p[1 - C];
-  // rows above the lane's first row and below its last row
-  uint32_t up[G_::WPP], dn[G_::WPP];
+  constexpr int NWL = G_::NWL;
   const int gu = (g + G_::G - 1) % G_::G, gd = (g + 1) % G_::G;
-#pragma unroll
-  for (int i = 0; i < G_::WPP; ++i) {
-    up[i] = __shfl_sync(FULL, S[G_::RPL - 1][i], gu, G_::G);
-    dn[i] = __shfl_sync(FULL, S[0][i], gd, G_::G);
-  }
   const uint32_t c2 = 2u * t + (uint32_t)C;
-  uint32_t ge1[NWL], ge2[NWL], call0[NWL];
+  uint32_t ge1[NWL], ge2[NWL], call0[NWL], slots[NWL];
 #pragma unroll
-  for (int r = 0; r < G_::RPL; ++r) {
-    const int y = g * G_::RPL + r;
-    uint32_t B[G_::WPP];
-    rot_row<L>(S[r], (y + C) & 1, B);
+  for (int rep = 0; rep < G_::RW; ++rep) {
+    uint32_t(&T)[G_::RPL][G_::WPP] = lat[rep].p[C];
+    uint32_t(&S)[G_::RPL][G_::WPP] = lat[rep].p[1 - C];
+    // rows above the lane's first row and below its last row
+    uint32_t up[G_::WPP], dn[G_::WPP];
 #pragma unroll
     for (int i = 0; i < G_::WPP; ++i) {
-      const uint32_t U = (r > 0) ? S[r > 0 ? r - 1 : 0][i] : up[i];
-      const uint32_t D = (r < G_::RPL - 1) ? S[r < G_::RPL - 1 ? r + 1 : 0][i] : dn[i];
-      neighbour_classes(T[r][i], U, D, S[r][i], B[i], ge1[r * G_::WPP + i], ge2[r * G_::WPP + i]);
-      call0[r * G_::WPP + i] = 8u * ((uint32_t)y * G_::WPP + (uint32_t)i);  // group = y * WPP + i
+      up[i] = __shfl_sync(FULL, S[G_::RPL - 1][i], gu, G_::G);
+      dn[i] = __shfl_sync(FULL, S[0][i], gd, G_::G);
+    }
+#pragma unroll
+    for (int r = 0; r < G_::RPL; ++r) {
+      const int y = g * G_::RPL + r;
+      uint32_t B[G_::WPP];
+      rot_row<L>(S[r], (y + C) & 1, B);
+#pragma unroll
+      for (int i = 0; i < G_::WPP; ++i) {
+        const int w = rep * G_::NWR + r * G_::WPP + i;
+        const uint32_t U = (r > 0) ? S[r > 0 ? r - 1 : 0][i] : up[i];
+        const uint32_t D = (r < G_::RPL - 1) ? S[r < G_::RPL - 1 ? r + 1 : 0][i] : dn[i];
+        neighbour_classes(T[r][i], U, D, S[r][i], B[i], ge1[w], ge2[w]);
+        if (!valid[rep]) ge2[w] = 0xffffffffu;  // a replica past the population has nothing to decide
+        call0[w] = 8u * ((uint32_t)y * G_::WPP + (uint32_t)i);  // group = y * WPP + i
+        slots[w] = slot0 + (uint32_t)rep;
+      }
     }
   }
-  uint32_t flip[NWL], slots[NWL];
+  uint32_t flip[NWL];
+  queued_accept<NWL, SWEEP_THREADS, SweepCap<NWL>::CAP>(q, (unsigned)C, ge1, ge2, slots, slot_base, call0, c2, c3, key, sa,
+                                                        flip);
 #pragma unroll
-  for (int w = 0; w < NWL; ++w) slots[w] = slot;
-  lazy_accept<NWL>(ge1, ge2, slots, call0, c2, c3, key, sa, flip);
+  for (int rep = 0; rep < G_::RW; ++rep)
 #pragma unroll
-  for (int w = 0; w < NWL; ++w) T[w / G_::WPP][w % G_::WPP] ^= flip[w];
+    for (int w = 0; w < G_::NWR; ++w) lat[rep].p[C][w / G_::WPP][w % G_::WPP] ^= flip[rep * G_::NWR + w];
 }
 
 // number of anti-aligned bonds u (each bond has exactly one colour-0 end) and number of up spins
@@ -302,74 +397,88 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
   const unsigned long long count = sa.mode != 1 ? st->Rnew : st->R;
   const int theta = sa.mode != 1 ? sa.theta : 0;
   uint32_t* spins = buf ? spins1 : spins0;
+  const uint32_t* spins_other = buf ? spins0 : spins1;  // buffer cur inside a step
   int32_t* __restrict__ Eo = buf ? E1 : E0;
   int32_t* __restrict__ Mo = buf ? M1 : M0;
 
-  const unsigned long long tid = (unsigned long long)blockIdx.x * SWEEP_THREADS + threadIdx.x;
-  const unsigned long long slot64 = tid / G_::G;  // one warp per replica
-  const int g = (int)(tid % G_::G);
-  if (slot64 >= count) return;  // warp-uniform
-  const uint32_t slot = (uint32_t)slot64;
-  uint32_t* rep = spins + slot64 * G_::WREP;
-  const uint32_t* rep_src = rep;
-  if (sa.mode == 2) rep_src = (buf ? spins0 : spins1) + (unsigned long long)parent_of[slot64] * G_::WREP;  // parent, buffer cur
+  const unsigned long long slot_base64 = (unsigned long long)blockIdx.x * G_::RPB;
+  if (slot_base64 >= count) return;  // block-uniform: the sweeps below contain block barriers
+  const int g = (int)(threadIdx.x % G_::G);
+  const unsigned long long slot0_64 = slot_base64 + (unsigned long long)(threadIdx.x / G_::G) * G_::RW;  // the warp's first replica
+  const uint32_t slot0 = (uint32_t)slot0_64, slot_base = (uint32_t)slot_base64;
+  bool valid[G_::RW];  // warp-uniform
 
   // ---- load (once per step): the lane's rows are RPL*WR contiguous words = RPL*WR/4 16-byte vectors ----
-  Lattice<L> lat;
+  Lattice<L> lat[G_::RW];
   constexpr int NV = G_::RPL * G_::WR / 4;
-  {
+#pragma unroll
+  for (int rep = 0; rep < G_::RW; ++rep) {
+    const unsigned long long slot64 = slot0_64 + rep;
+    valid[rep] = slot64 < count;
+    const uint32_t* rep_src = spins + (valid[rep] ? slot64 : slot_base64) * G_::WREP;
+    if (sa.mode == 2 && valid[rep]) rep_src = spins_other + (unsigned long long)parent_of[slot64] * G_::WREP;  // parent
     uint32_t rawall[G_::RPL * G_::WR];
     const uint4* src = reinterpret_cast<const uint4*>(rep_src) + g * NV;
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
-      const uint4 q = src[v];
-      rawall[4 * v] = q.x; rawall[4 * v + 1] = q.y; rawall[4 * v + 2] = q.z; rawall[4 * v + 3] = q.w;
+      const uint4 x = src[v];
+      rawall[4 * v] = x.x; rawall[4 * v + 1] = x.y; rawall[4 * v + 2] = x.z; rawall[4 * v + 3] = x.w;
     }
 #pragma unroll
     for (int r = 0; r < G_::RPL; ++r) {
       uint32_t raw[G_::WR];
 #pragma unroll
       for (int i = 0; i < G_::WR; ++i) raw[i] = rawall[r * G_::WR + i];
-      row_to_planes<L>(raw, (g * G_::RPL + r) & 1, lat.p[0][r], lat.p[1][r]);
+      row_to_planes<L>(raw, (g * G_::RPL + r) & 1, lat[rep].p[0][r], lat[rep].p[1][r]);
     }
   }
 
   // ---- theta sweeps ----------------------------------------------------------------------------
   if (theta > 0) {
+    using Q_ = SweepQueue<SweepCap<G_::NWL>::CAP>;
+    __shared__ Q_ q_mem;
+    static_assert(offsetof(Q_, res) == Q_::OFF_RES && offsetof(Q_, count) == Q_::OFF_COUNT, "queue layout");
+    const uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
+    if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
+    __syncthreads();
     const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
     for (int t = 0; t < theta; ++t) {
-      half_sweep<L, 0>(lat, g, slot, (uint32_t)t, c3, key, sa);
-      half_sweep<L, 1>(lat, g, slot, (uint32_t)t, c3, key, sa);
+      half_sweep<L, 0>(lat, q, g, slot0, slot_base, valid, (uint32_t)t, c3, key, sa);
+      half_sweep<L, 1>(lat, q, g, slot0, slot_base, valid, (uint32_t)t, c3, key, sa);
     }
   }
 
-  // ---- a8: E = 2u - 2N, M = 2*popc - N ----------------------------------------------------------
-  int unsat, ups;
-  count_bonds<L>(lat, g, unsat, ups);
 #pragma unroll
-  for (int o = G_::G / 2; o > 0; o >>= 1) {
-    unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
-    ups += __shfl_xor_sync(0xffffffffu, ups, o);
-  }
-  if (g == 0) {
-    Eo[slot64] = 2 * unsat - 2 * G_::N;
-    Mo[slot64] = 2 * ups - G_::N;
-  }
-
-  // ---- store (once per step) -------------------------------------------------------------------
-  if (theta > 0) {
-    uint32_t rawall[G_::RPL * G_::WR];
+  for (int rep = 0; rep < G_::RW; ++rep) {
+    if (!valid[rep]) continue;  // warp-uniform
+    const unsigned long long slot64 = slot0_64 + rep;
+    // ---- a8: E = 2u - 2N, M = 2*popc - N ----------------------------------------------------------
+    int unsat, ups;
+    count_bonds<L>(lat[rep], g, unsat, ups);
 #pragma unroll
-    for (int r = 0; r < G_::RPL; ++r) {
-      uint32_t raw[G_::WR];
-      planes_to_row<L>(lat.p[0][r], lat.p[1][r], (g * G_::RPL + r) & 1, raw);
-#pragma unroll
-      for (int i = 0; i < G_::WR; ++i) rawall[r * G_::WR + i] = raw[i];
+    for (int o = G_::G / 2; o > 0; o >>= 1) {
+      unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
+      ups += __shfl_xor_sync(0xffffffffu, ups, o);
     }
-    uint4* dst = reinterpret_cast<uint4*>(rep) + g * NV;
+    if (g == 0) {
+      Eo[slot64] = 2 * unsat - 2 * G_::N;
+      Mo[slot64] = 2 * ups - G_::N;
+    }
+    // ---- store (once per step) -------------------------------------------------------------------
+    if (theta > 0) {
+      uint32_t rawall[G_::RPL * G_::WR];
 #pragma unroll
-    for (int v = 0; v < NV; ++v)
-      dst[v] = make_uint4(rawall[4 * v], rawall[4 * v + 1], rawall[4 * v + 2], rawall[4 * v + 3]);
+      for (int r = 0; r < G_::RPL; ++r) {
+        uint32_t raw[G_::WR];
+        planes_to_row<L>(lat[rep].p[0][r], lat[rep].p[1][r], (g * G_::RPL + r) & 1, raw);
+#pragma unroll
+        for (int i = 0; i < G_::WR; ++i) rawall[r * G_::WR + i] = raw[i];
+      }
+      uint4* dst = reinterpret_cast<uint4*>(spins + slot64 * G_::WREP) + g * NV;
+#pragma unroll
+      for (int v = 0; v < NV; ++v)
+        dst[v] = make_uint4(rawall[4 * v], rawall[4 * v + 1], rawall[4 * v + 2], rawall[4 * v + 3]);
+    }
   }
 }
 
@@ -422,16 +531,14 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
   int32_t* __restrict__ Eo = buf ? E1 : E0;
   int32_t* __restrict__ Mo = buf ? M1 : M0;
 
-  // A group of G lanes holds TWO consecutive replicas (one plane word per colour and replica per lane): the two words
-  // of a lane share the straggler iterations of the lazy comparison, as the rows of a lane do for L >= 64.
+  // A group of G lanes holds TWO consecutive replicas (one plane word per colour and replica per lane).
   constexpr int NR = 2;
   const unsigned long long tid = (unsigned long long)blockIdx.x * SWEEP_THREADS + threadIdx.x;
   const unsigned long long pair = tid / G_::G;
   const int g = (int)(tid % G_::G);
-  {  // warp-uniform exit for warps entirely past the population
-    const unsigned long long first_slot_of_warp = ((tid & ~31ull) / G_::G) * NR;
-    if (first_slot_of_warp >= count) return;
-  }
+  const unsigned long long slot_base64 = ((unsigned long long)blockIdx.x * SWEEP_THREADS / G_::G) * NR;
+  if (slot_base64 >= count) return;  // block-uniform: the sweeps below contain block barriers
+  const uint32_t slot_base = (uint32_t)slot_base64;
   unsigned long long slot64[NR];
   bool valid[NR];
   uint32_t slots[NR];
@@ -455,6 +562,12 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
 
   // ---- theta sweeps ----------------------------------------------------------------------------
   if (theta > 0) {
+    using Q_ = SweepQueue<SweepCap<NR>::CAP>;
+    __shared__ Q_ q_mem;
+    static_assert(offsetof(Q_, res) == Q_::OFF_RES && offsetof(Q_, count) == Q_::OFF_COUNT, "queue layout");
+    const uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
+    if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
+    __syncthreads();
     const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
     uint32_t call0[NR];
 #pragma unroll
@@ -469,7 +582,8 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           neighbour_classes(p[r][0], U, D, p[r][1], B, ge1[r], ge2[r]);
           if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }  // padding never holds the warp back
         }
-        lazy_accept<NR>(ge1, ge2, slots, call0, 2u * (uint32_t)t, c3, key, sa, flip);
+        queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 0u, ge1, ge2, slots, slot_base, call0, 2u * (uint32_t)t, c3, key,
+                                                           sa, flip);
 #pragma unroll
         for (int r = 0; r < NR; ++r) p[r][0] ^= flip[r];
       }
@@ -482,7 +596,8 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           neighbour_classes(p[r][1], U, D, p[r][0], B, ge1[r], ge2[r]);
           if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }
         }
-        lazy_accept<NR>(ge1, ge2, slots, call0, 2u * (uint32_t)t + 1u, c3, key, sa, flip);
+        queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 1u, ge1, ge2, slots, slot_base, call0, 2u * (uint32_t)t + 1u, c3,
+                                                           key, sa, flip);
 #pragma unroll
         for (int r = 0; r < NR; ++r) p[r][1] ^= flip[r];
       }
