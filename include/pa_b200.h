@@ -111,7 +111,8 @@ int pa_init(const pa_config* cfg, pa_ctx** out);
 
 /* a1-a8. One temperature step beta -> beta_next with theta >= 0 sweeps.  Synchronous: returns after the step's
  * kernels finished and its status was read back.  On PA_ECAPACITY / PA_EEXTINCT the population, beta, step
- * counter and ln Z are unchanged. */
+ * counter and ln Z (and pa_log_Z's last_Q) are unchanged.  pa_step is pa_run with K = 1: one stream synchronisation
+ * and one 264-byte read-back of the device state per call; queue whole schedules with pa_run to avoid both. */
 int pa_step(pa_ctx* ctx, double beta_next, int32_t theta);
 
 /* K steps beta_k = betas[k] (HOST array of K doubles), all launched back to back with ONE synchronisation at the
@@ -136,7 +137,9 @@ int pa_observables(pa_ctx* ctx, pa_obs* out);
 /* ---- parity / debug getters --------------------------------------------------------------------------- */
 /* packed lattices of slots first..first+count-1 (count * N/32 uint32 words) */
 int pa_spins(pa_ctx* ctx, uint32_t* dst, int64_t first, int64_t count, int dst_on_device);
-/* tau_j of the LAST step's parents, j = 0..n-1, n <= number of parents (needs PA_KEEP_TAU) */
+/* tau_j of the LAST step's parents, j = 0..n-1, n <= number of parents (needs PA_KEEP_TAU).  PA_EINVAL after a step
+ * that was not committed (PA_ECAPACITY / PA_EEXTINCT) until the next committed step: the arrays then hold the failed
+ * attempt.  Same for pa_counts. */
 int pa_tau(pa_ctx* ctx, double* dst, int64_t n, int dst_on_device);
 /* copy counts n_j (needs PA_KEEP_COUNTS; may be NULL) and exclusive offsets off_j, j = 0..n_parents (off has
  * n_parents+1 entries, off[n_parents] = R') of the LAST step */
@@ -148,6 +151,10 @@ int pa_parents(pa_ctx* ctx, int64_t* n_parents);
 int pa_partitions(pa_ctx* ctx, uint32_t* part_start, pa_part_stats* stats, int64_t* moved);
 /* acceptance thresholds used by the last step with theta > 0 */
 int pa_thresholds(pa_ctx* ctx, uint32_t* T4, uint32_t* T8);
+/* test hook (parity only): while enabled, every later step uses T4, T8 as its acceptance thresholds instead of
+ * floor(2^32 exp(-4 beta')), floor(2^32 exp(-8 beta')) (C4) -- lets a test reach u == T and the extreme
+ * thresholds 0 and 2^32 - 1, which no temperature produces on demand.  pa_thresholds reports the values used. */
+int pa_debug_set_thresholds(pa_ctx* ctx, int enable, uint32_t T4, uint32_t T8);
 /* test hook: replace the population by R packed lattices (R <= capacity); recomputes E, M, sums, partitions;
  * beta, step counter and ln Z are kept */
 int pa_set_spins(pa_ctx* ctx, const uint32_t* src, int64_t R, int src_on_device);

@@ -17,7 +17,7 @@ KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "cop
 
 EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
            "pa_observables", "pa_spins", "pa_tau", "pa_counts", "pa_parents", "pa_partitions", "pa_thresholds",
-           "pa_set_spins", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
+           "pa_set_spins", "pa_debug_set_thresholds", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
 
 
 class PaConfig(C.Structure):
@@ -70,6 +70,7 @@ def load_library():
         "pa_partitions": (C.c_int, [vp, vp, vp, i64p]),
         "pa_thresholds": (C.c_int, [vp, u32p, u32p]),
         "pa_set_spins": (C.c_int, [vp, vp, C.c_int64, C.c_int]),
+        "pa_debug_set_thresholds": (C.c_int, [vp, C.c_int, C.c_uint32, C.c_uint32]),
         "pa_profile_read": (C.c_int, [vp, f64p, i64p]),
         "pa_launch_count": (C.c_int, [vp, i64p]),
         "pa_last_error": (C.c_char_p, [vp]),
@@ -252,6 +253,9 @@ class PopulationAnnealer:
         else:
             a = np.ascontiguousarray(packed, np.uint32)
             self._check(self._lib.pa_set_spins(self._ctx, _np_ptr(a), a.shape[0], 0))
+
+    def debug_set_thresholds(self, enable, T4=0, T8=0):
+        self._check(self._lib.pa_debug_set_thresholds(self._ctx, int(bool(enable)), int(T4), int(T8)))
 
     def profile_read(self):
         ms = (C.c_double * len(KERNELS))()

@@ -112,6 +112,9 @@ struct pa_ctx {
   double beta, sum_lnQ, last_Q;
   int64_t launches;
   bool profile;
+  bool attempt_failed;  // the last pa_step / pa_run ended with an uncommitted step: off / n / tau hold that attempt
+  bool dbg_thresholds;  // test hook: pa_debug_set_thresholds
+  uint32_t dbg_T4, dbg_T8;
   int scan_grid_max;  // co-resident blocks of k_poisson_scan on this device
   // large populations: the scan runs in SCAN_CHUNKS launches on a high-priority stream of the library, the copy of
   // chunk i (caller's stream) overlaps the scan of chunk i+1
@@ -331,6 +334,7 @@ __global__ void k_init_state(DevState* st, unsigned long long R, double beta0, u
     st->R_parents = R;
     st->beta = beta0;
     st->Q = 1.0;
+    st->Q_committed = 1.0;
   }
   const unsigned long long base = R / P, rem = R % P;
   for (int p = threadIdx.x; p <= P; p += blockDim.x)
@@ -363,7 +367,7 @@ int sync_state(pa_ctx* c) {
   c->steps = s.step;
   c->beta = s.beta;
   c->sum_lnQ = s.sum_lnQ;
-  if (s.step > 0) c->last_Q = s.Q;
+  if (s.step > 0) c->last_Q = s.Q_committed;
   return PA_OK;
 }
 
@@ -398,7 +402,7 @@ int check_step_args(pa_ctx* c, double beta_from, double beta_next, int theta) {
   return PA_OK;
 }
 
-StepParams make_params(double beta_from, double beta_next, int theta) {
+StepParams make_params(const pa_ctx* c, double beta_from, double beta_next, int theta) {
   StepParams p;
   p.dbeta = beta_next - beta_from;
   p.beta_next = beta_next;
@@ -406,6 +410,10 @@ StepParams make_params(double beta_from, double beta_next, int theta) {
   const double a8 = std::floor(4294967296.0 * std::exp(-8.0 * beta_next));
   p.T4 = a4 >= 4294967295.0 ? 0xffffffffu : (a4 > 0.0 ? (uint32_t)a4 : 0u);
   p.T8 = a8 >= 4294967295.0 ? 0xffffffffu : (a8 > 0.0 ? (uint32_t)a8 : 0u);
+  if (c->dbg_thresholds) {
+    p.T4 = c->dbg_T4;
+    p.T8 = c->dbg_T8;
+  }
   p.theta = theta;
   p.pad_ = 0;
   return p;
@@ -444,6 +452,9 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   c->stream = static_cast<cudaStream_t>(cfg->stream);
   c->profile = (cfg->flags & PA_PROFILE) != 0;
   c->launches = 0;
+  c->attempt_failed = false;
+  c->dbg_thresholds = false;
+  c->dbg_T4 = c->dbg_T8 = 0u;
   c->scan_grid_max = 0;
   {
     const uint64_t tiles_cap = ((uint64_t)c->cap + SCAN_TILE - 1) / SCAN_TILE;
@@ -467,8 +478,11 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
     return PA_ECUDA;  // no CPU fallback
   }
   cudaGetDevice(&c->device);
+  c->h_state = nullptr;
+  c->h_params = nullptr;
   if (cudaHostAlloc((void**)&c->h_state, sizeof(DevState), cudaHostAllocDefault) != cudaSuccess ||
       cudaHostAlloc((void**)&c->h_params, sizeof(StepParams) * RUN_CHUNK, cudaHostAllocDefault) != cudaSuccess) {
+    if (c->h_state) cudaFreeHost(c->h_state);
     delete c;
     return PA_ECUDA;
   }
@@ -518,7 +532,7 @@ int pa_run(pa_ctx* c, const double* betas, int32_t K, int32_t theta, int32_t* st
     const int nk = (K - base < RUN_CHUNK) ? (K - base) : RUN_CHUNK;
     if (base > 0) CK(cudaStreamSynchronize(c->stream));  // staging buffer is reused
     for (int k = 0; k < nk; ++k) {
-      c->h_params[k] = make_params(from, betas[base + k], theta);
+      c->h_params[k] = make_params(c, from, betas[base + k], theta);
       from = betas[base + k];
     }
     CK(cudaMemcpyAsync(d_params, c->h_params, sizeof(StepParams) * nk, cudaMemcpyHostToDevice, c->stream));
@@ -528,6 +542,7 @@ int pa_run(pa_ctx* c, const double* betas, int32_t K, int32_t theta, int32_t* st
   if (rc != PA_OK) return rc;
   if (steps_done) *steps_done = (int32_t)(c->steps - steps_before);
   rc = status_to_code(c);
+  c->attempt_failed = (rc != PA_OK);
   if (rc != PA_OK) {
     k_clear_status<<<1, 1, 0, c->stream>>>(c->dev<DevState>(c->lo.state));
     c->launches += 1;
@@ -606,6 +621,7 @@ int pa_tau(pa_ctx* c, double* dst, int64_t n, int dst_on_device) {
   if (!c || !dst || n < 0) return fail(c, PA_EINVAL, "pa_tau: bad arguments");
   if (!c->lo.tau) return fail(c, PA_EINVAL, "pa_tau needs PA_KEEP_TAU");
   if (c->steps == 0 || n > c->R_parents) return fail(c, PA_EINVAL, "pa_tau: no step yet or n > parents");
+  if (c->attempt_failed) return fail(c, PA_EINVAL, "pa_tau: the last step was not committed (its tau array is not that of the last committed step)");
   return copy_out(c, dst, c->dev<double>(c->lo.tau), (size_t)n * 8, dst_on_device);
 }
 
@@ -613,6 +629,7 @@ int pa_counts(pa_ctx* c, uint32_t* n, uint32_t* off, int64_t n_parents, int dst_
   if (!c || n_parents < 0 || (!n && !off)) return fail(c, PA_EINVAL, "pa_counts: bad arguments");
   if (c->steps == 0 || n_parents > c->R_parents) return fail(c, PA_EINVAL, "pa_counts: no step yet or n_parents > parents");
   if (n && !c->lo.n) return fail(c, PA_EINVAL, "pa_counts(n) needs PA_KEEP_COUNTS");
+  if (c->attempt_failed) return fail(c, PA_EINVAL, "pa_counts: the last step was not committed (off / n hold the failed attempt)");
   int rc = PA_OK;
   if (n) rc = copy_out(c, n, c->dev<uint32_t>(c->lo.n), (size_t)n_parents * 4, dst_on_device);
   if (rc == PA_OK && off) rc = copy_out(c, off, c->dev<uint32_t>(c->lo.off), (size_t)(n_parents + 1) * 4, dst_on_device);
@@ -638,6 +655,14 @@ int pa_thresholds(pa_ctx* c, uint32_t* T4, uint32_t* T8) {
   if (!c) return PA_EINVAL;
   if (T4) *T4 = c->h_state->T4;
   if (T8) *T8 = c->h_state->T8;
+  return PA_OK;
+}
+
+int pa_debug_set_thresholds(pa_ctx* c, int enable, uint32_t T4, uint32_t T8) {
+  if (!c) return PA_EINVAL;
+  c->dbg_thresholds = enable != 0;
+  c->dbg_T4 = T4;
+  c->dbg_T8 = T8;
   return PA_OK;
 }
 

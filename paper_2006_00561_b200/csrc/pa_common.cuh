@@ -36,6 +36,7 @@ struct DevState {
   unsigned int T4, T8;           // thresholds of the last committed step with theta > 0
   int lev_lo, lev_hi;            // occupied energy levels (E + 2N)/4 of the CURRENT population, inclusive (by k_observe)
   unsigned int pad_[1];
+  double Q_committed;            // Q of the last COMMITTED step (Q above is overwritten by every attempt)
 };
 
 struct StepParams {

@@ -183,6 +183,7 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
       st->cur ^= 1u;
       st->step += 1u;
       st->sum_lnQ += st->lnQ;
+      st->Q_committed = st->Q;
       st->beta = sp->beta_next;
       if (sp->theta > 0) {
         st->T4 = sp->T4;

@@ -269,6 +269,150 @@ def test_config5_full_size():
 
 
 # ---------------------------------------------------------------------------------------------------
+# parity reach (round 2): low temperatures at L = 128, zero temperature, theta = 1 at full size, u == T
+# ---------------------------------------------------------------------------------------------------
+def adopt(gpu, ora):
+    """put the oracle into the GPU's state after a stretch of pa_run (population, beta, step ordinal, ln Z accumulator);
+    E, M are recomputed by the oracle's own energy function and compared"""
+    got = gpu.spins()
+    E, M = gpu.energies()
+    Eo, Mo = orc.energy_mag(ora.L, got)
+    assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+    ora.spins, ora.E, ora.M, ora.R = got, Eo, Mo, got.shape[0]
+    ora.beta, ora.step_no = gpu.beta_steps()
+    ora.sum_lnQ = gpu.log_Z()["sum_lnQ"]
+    ora.part_start = orc.partition_table(ora.R, ora.P)
+
+
+def test_L128_lockstep_down_to_beta_0p6():
+    """config 4 shape at reduced R: 30 steps of dbeta = 0.02 (|dbeta| 2N = 655 < 700) reach beta = 0.6, the end of config
+    4's schedule -- L = 128 sweeps compared on the whole population in the ordered phase, where almost every site
+    needs a uniform and most of them are rejected"""
+    gpu, ora = make_pair(128, 600, 148, seed=404)
+    lockstep(gpu, ora, [0.02 * k for k in range(1, 31)], 2)
+    assert gpu.observables()["mean_E"] / 128 ** 2 < -1.2  # a fast quench: domains, but deep in the low-energy region
+
+
+def test_config4_full_size_sampled_late_in_the_schedule():
+    """config 4 at full size, brought to beta = 0.45 and then to beta = 0.5988 by pa_run (its own schedule), with a
+    lock-step step (a1-a6 on the whole population, theta = 20 sweeps on sampled slots) taken at each point"""
+    wl = inputs.CONFIGS[4]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
+    k1, k2 = 375, 499
+    assert gpu.run([wl.beta(k) for k in range(1, k1 + 1)], wl.theta) == k1
+    adopt(gpu, ora)
+    lockstep(gpu, ora, [wl.beta(k1 + 1)], wl.theta, sweep_slots=512)
+    assert gpu.run([wl.beta(k) for k in range(k1 + 2, k2 + 1)], wl.theta) == k2 - k1 - 1
+    adopt(gpu, ora)
+    lockstep(gpu, ora, [wl.beta(k2 + 1)], wl.theta, sweep_slots=512)
+    assert abs(gpu.beta_steps()[0] - 0.6) < 1e-12 and gpu.beta_steps()[1] == 500
+
+
+@pytest.mark.parametrize("L", [8, 16, 64])
+def test_zero_temperature_dynamics(L):
+    """beta large enough that T4 = T8 = 0: deterministic zero-temperature dynamics (flip iff a >= 2), the regime the
+    oracle's sweep is pinned in by hand (tests/test_oracle_pins.py::test_zero_temperature_dynamics_by_hand)"""
+    R = 400
+    pop = inputs.structured_population(L, R, seed=3 * L)
+    step = 600.0 / (2 * L * L)  # |dbeta| 2N < 700 (reading G11)
+    beta0 = 30.0
+    gpu, ora = make_pair(L, R, P=3, seed=17, beta0=beta0, spins=pop, capacity=8 * R)
+    lockstep(gpu, ora, [beta0 + step * k for k in range(1, 4)], 2)
+    assert gpu.thresholds() == (0, 0)
+
+
+def test_config3_full_size_theta1():
+    """theta = 1 is the paper's scalability regime; full size, sampled slots"""
+    wl = inputs.CONFIGS[3]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
+    lockstep(gpu, ora, [0.08, 0.16, 0.165], 1, sweep_slots=4096)
+
+
+@pytest.mark.parametrize("L", [8, 32, 64])
+def test_threshold_equal_to_the_uniform_is_not_accepted(L):
+    """u == T (probability 2^-32 per site, never met by a temperature-derived threshold in any other test): with the
+    test hook pa_debug_set_thresholds the thresholds are set to the very 32-bit uniform of one chosen site of an
+    all-up lattice (every colour-0 site has a = 0 and compares against T8).  u < T is strict (C4): the site
+    must stay; with T + 1 it must flip.  All 32 comparator bits are equal for that site, which takes the kernel to
+    its last Philox block (c = 7)."""
+    b = _binding()
+    seed, R = 0x5EED0000 + L, 40
+    half = L // 2
+    y, k = L // 2 + 1, half - 1       # a site in the last group of its row block, colour 0
+    q = y * half + k
+    x = 2 * k + (y & 1)
+    up = np.stack([orc.pack(L, np.ones(L * L, np.int8))] * R)
+    for slot in (0, 2):
+        for plus in (0, 1):
+            g = b.PopulationAnnealer(L, R, seed=seed, capacity=256)
+            g.set_spins(up)
+            u = philox_ref.sweep_word(seed, 1, slot, 0, 0, q)  # step ordinal 1, sweep t = 0, colour 0
+            T = min(u + plus, 0xFFFFFFFF)
+            g.debug_set_thresholds(True, T4=0x12345678, T8=T)
+            g.step(1e-9, 1)  # all energies are equal: tau = 1, R' ~ Poisson(40), every child is all-up again
+            assert g.thresholds() == (0x12345678, T) and g.R > slot
+            # oracle: the resampled population is all-up again (copies of identical parents); same thresholds
+            want = np.stack([orc.pack(L, np.ones(L * L, np.int8))] * g.R)
+            orc.sweeps(L, want, seed, 1, 1, 0x12345678, T)
+            got = g.spins()
+            assert np.array_equal(got, want)
+            s = orc.unpack(L, got[slot]).reshape(L, L)
+            # colour-0 site (x, y) was decided on the all-up lattice; colour 1 may have flipped neighbours afterwards but
+            # never the site itself
+            assert s[y, x] == (1 if plus == 0 else -1), (slot, plus)
+
+
+def test_extreme_thresholds_through_the_hook():
+    """T = 0 (never accept an uphill move) and T = 2^32 - 1 (accept unless u = 2^32 - 1) against the oracle"""
+    b = _binding()
+    L, R, seed = 32, 500, 99
+    pop = inputs.random_packed_population(L, R, seed=5)
+    for T4, T8 in [(0, 0), (0xFFFFFFFF, 0xFFFFFFFF), (0xFFFFFFFF, 0), (0x80000000, 0x7FFFFFFF)]:
+        g = b.PopulationAnnealer(L, R, seed=seed, capacity=4096, flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS)
+        g.set_spins(pop)
+        g.debug_set_thresholds(True, T4, T8)
+        g.step(0.05, 2)
+        o = orc.OraclePA(L, R, seed=seed, capacity=4096, spins=pop)
+        o.resample(0.05, tau_override=g.tau())
+        orc.sweeps(L, o.spins, seed, 1, 2, T4, T8)
+        assert g.R == o.R and np.array_equal(g.spins(), o.spins), (T4, T8)
+        g.debug_set_thresholds(False)
+        g.step(0.1, 1)
+        assert g.thresholds() == orc.thresholds(0.1)
+
+
+def test_failed_step_does_not_leak_into_the_getters():
+    """after PA_ECAPACITY the getters of the last step refuse (their arrays hold the failed attempt) and last_Q is still
+    the Q of the last committed step"""
+    b = _binding()
+    g = b.PopulationAnnealer(16, 1024, P=2, seed=3, capacity=1024, flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS)
+    k, failed = 0, False
+    while not failed and k < 60:
+        k += 1
+        lz = g.log_Z()
+        try:
+            g.step(0.002 * k, 1)
+        except b.PaError as e:
+            assert e.code == b.PA_ECAPACITY
+            failed = True
+    assert failed
+    assert g.log_Z() == lz
+    for call in (g.tau, g.counts):
+        with pytest.raises(b.PaError) as ei:
+            call()
+        assert ei.value.code == b.PA_EINVAL
+    while True:  # the next committed step makes them valid again
+        k += 1
+        try:
+            g.step(0.002 * k, 1)
+            break
+        except b.PaError:
+            pass
+    n, off = g.counts()
+    assert int(n.sum()) == g.R == int(off[-1])
+
+
+# ---------------------------------------------------------------------------------------------------
 # boundary behaviour
 # ---------------------------------------------------------------------------------------------------
 def test_run_equals_repeated_step_and_is_deterministic():
