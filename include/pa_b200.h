@@ -48,7 +48,9 @@ typedef enum {
 enum {
   PA_KEEP_TAU = 1u,    /* materialise tau_j of every step (8 B per parent) for pa_tau */
   PA_KEEP_COUNTS = 2u, /* materialise n_j of every step (4 B per parent) for pa_counts(n != NULL) */
-  PA_PROFILE = 4u      /* record CUDA events around every kernel (pa_profile_read) */
+  PA_PROFILE = 4u,     /* record CUDA events around every kernel (pa_profile_read); the events between the kernels
+                          keep a kernel's blocks from being placed while its predecessor drains */
+  PA_PROFILE_SPAN = 8u /* record only the PA_K_RESAMPLE_SPAN pair around a1-a6 of every step */
 };
 
 typedef struct {
@@ -61,10 +63,8 @@ typedef struct {
   void* workspace;  /* DEVICE memory, caller owned, 256-byte aligned, >= pa_workspace_bytes(cfg) */
   uint64_t workspace_bytes;
   void* stream;     /* cudaStream_t, caller owned (NULL = legacy default stream) */
-  uint32_t flags;   /* PA_KEEP_TAU | PA_KEEP_COUNTS | PA_PROFILE */
-  uint32_t scan_chunks; /* 0 = automatic (currently 1: overlap measured slower on B200).  1..8: number of launches the Poisson/scan kernel is split into; with more than
-                           one, the copy of chunk i (cfg.stream) overlaps the scan of chunk i+1 (a stream of the library).
-                           Results do not depend on it. */
+  uint32_t flags;   /* PA_KEEP_TAU | PA_KEEP_COUNTS | PA_PROFILE | PA_PROFILE_SPAN */
+  uint32_t reserved; /* must be 0 */
 } pa_config;
 
 /* population sums after the last committed step (or after pa_init / pa_set_spins); 128-bit integers as {lo, hi} */
@@ -89,16 +89,16 @@ typedef struct {
 /* kernels of one pa_step, in launch order (indices of pa_profile_read arrays) */
 enum {
   PA_K_LEVELS_W = 0, /* (w_e = exp(-dbeta e) per level is tabulated inside PA_K_Q_REDUCE: reports 0 launches) */
-  PA_K_Q_REDUCE,     /* eq. 3: fp64 warp-shuffle reduction, Q, ln Q */
-  PA_K_LEVELS_TAU,   /* eq. 4 per level + Poisson chunk tables */
-  PA_K_POISSON_SCAN, /* Poisson copy counts + single-pass exclusive scan */
-  PA_K_BALANCE,      /* partition table + diagnostics: run by block 0 of PA_K_COPY, reports 0 launches */
-  PA_K_COPY,         /* replica redistribution: gather copy (theta = 0) or only the child -> parent map (theta > 0: the
-                        lattices are gathered by PA_K_SWEEP's load) */
+  PA_K_Q_REDUCE,     /* eq. 3: fp64 warp-shuffle reduction, Q, ln Q; its last block: eq. 4 per level + Poisson tables */
+  PA_K_LEVELS_TAU,   /* (run by the last block of PA_K_Q_REDUCE: reports 0 launches) */
+  PA_K_POISSON_SCAN, /* Poisson copy counts + single-pass exclusive scan + child -> parent map */
+  PA_K_BALANCE,      /* partition table + diagnostics: run by the last block of PA_K_OBSERVE, reports 0 launches */
+  PA_K_COPY,         /* replica redistribution: gather copy (theta = 0 only; with theta > 0 the lattices are gathered
+                        by PA_K_SWEEP's load and this reports 0 launches) */
   PA_K_SWEEP,        /* theta checkerboard Metropolis sweeps + E, M */
   PA_K_OBSERVE,      /* population sums + commit of the step */
-  PA_K_RESAMPLE_SPAN, /* not a kernel: elapsed time on cfg.stream from the start of PA_K_Q_REDUCE to the end of the last
-                         PA_K_COPY (a1-a6 as one span; with scan_chunks > 1 the kernels inside it overlap) */
+  PA_K_RESAMPLE_SPAN, /* not a kernel: elapsed time on cfg.stream from the start of PA_K_Q_REDUCE to the end of PA_K_COPY
+                         (theta = 0) or of PA_K_POISSON_SCAN (theta > 0): a1-a6 as one span */
   PA_K_COUNT
 };
 

@@ -20,7 +20,10 @@ using namespace pa;
 namespace {
 
 constexpr int RUN_CHUNK = 1024;  // step-parameter slots uploaded per pa_run chunk
-constexpr int RED_GRID = 148 * 4;
+#ifndef PA_RED_GRID
+#define PA_RED_GRID (148 * 4)
+#endif
+constexpr int RED_GRID = PA_RED_GRID;
 constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
@@ -76,8 +79,8 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   lo->n = (c->flags & PA_KEEP_COUNTS) ? take(ucap * 4) : 0;
   lo->tau = (c->flags & PA_KEEP_TAU) ? take(ucap * 8) : 0;
   lo->tile_desc = take(((ucap + SCAN_TILE - 1) / SCAN_TILE + 1) * 8);
-  lo->tile_parent = take((ucap / copy_tile_for(c->L) + 2) * 4);
-  lo->parent_of = take(ucap * 4);  // child -> parent map of the gather-on-load sweep (theta > 0)
+  lo->tile_parent = take((ucap / copy_tile_for(c->L) + 2) * 4);  // theta = 0: first parent of every copy tile
+  lo->parent_of = take(ucap * 4);  // theta > 0: child -> parent map of the sweep's gather-on-load
   lo->red_partial = take(RED_GRID * 8);
   lo->obs_partial = take((uint64_t)OBS_GRID * 12 * 8);
   lo->lev_tau = take(nlev * 8);
@@ -111,18 +114,13 @@ struct pa_ctx {
   int64_t R, R_parents, steps;
   double beta, sum_lnQ, last_Q;
   int64_t launches;
-  bool profile;
+  bool profile, profile_span;
   bool attempt_failed;  // the last pa_step / pa_run ended with an uncommitted step: off / n / tau hold that attempt
   bool dbg_thresholds;  // test hook: pa_debug_set_thresholds
   uint32_t dbg_T4, dbg_T8;
   int scan_grid_max;  // co-resident blocks of k_poisson_scan on this device
-  // large populations: the scan runs in SCAN_CHUNKS launches on a high-priority stream of the library, the copy of
-  // chunk i (caller's stream) overlaps the scan of chunk i+1
-  int nchunks;
-  cudaStream_t scan_stream;
-  cudaEvent_t ev_fork, ev_scan[8];
   std::vector<EventPair> ev_used, ev_free;
-  std::string err;
+  std::string err, launch_err;
 
   template <class T> T* dev(uint64_t off) const { return reinterpret_cast<T*>(ws + off); }
 };
@@ -147,16 +145,19 @@ struct Prof {  // records an event pair around one launch when profiling is on
   EventPair ep;
   bool on;
   cudaStream_t s;
-  Prof(pa_ctx* c_, int kernel, cudaStream_t stream = nullptr, bool is_launch = true)
-      : c(c_), on(c_->profile), s(stream ? stream : c_->stream) {
+  // per-kernel pairs only with PA_PROFILE; the a1-a6 span pair (is_launch = false) also with PA_PROFILE_SPAN
+  Prof(pa_ctx* c_, int kernel, bool is_launch = true)
+      : c(c_), on(c_->profile || (!is_launch && c_->profile_span)), s(c_->stream) {
     if (is_launch) c->launches += 1;
     if (!on) return;
     if (!c->ev_free.empty()) {
       ep = c->ev_free.back();
       c->ev_free.pop_back();
     } else {
-      cudaEventCreate(&ep.a);
-      cudaEventCreate(&ep.b);
+      if (cudaEventCreate(&ep.a) != cudaSuccess || cudaEventCreate(&ep.b) != cudaSuccess) {
+        on = false;  // out of events: this launch goes unprofiled rather than recording into an invalid handle
+        return;
+      }
     }
     ep.kernel = kernel;
     cudaEventRecord(ep.a, s);
@@ -188,24 +189,42 @@ SweepArgs sweep_args(int theta, uint32_t T4, uint32_t T8, int mode) {
   return sa;
 }
 
+// Every kernel of the path is launched with programmatic stream serialisation (PDL): its blocks may be placed while
+// the predecessor drains and wait in griddepcontrol.wait (pa_common.cuh) until the predecessor's memory is visible.
+template <class... KArgs, class... Args>
+void launch(pa_ctx* c, const char* name, void (*kern)(KArgs...), unsigned grid, unsigned block, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(block);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = c->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = PA_PDL ? 1 : 0;
+  const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+  if (e != cudaSuccess && c->launch_err.empty())  // reported by the next sync_state
+    c->launch_err = std::string(name) + ": " + cudaGetErrorString(e);
+}
+
 template <int L>
 void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
   uint32_t *s0 = c->dev<uint32_t>(c->lo.spins[0]), *s1 = c->dev<uint32_t>(c->lo.spins[1]);
   int32_t *e0 = c->dev<int32_t>(c->lo.E[0]), *e1 = c->dev<int32_t>(c->lo.E[1]);
   int32_t *m0 = c->dev<int32_t>(c->lo.M[0]), *m1 = c->dev<int32_t>(c->lo.M[1]);
   const DevState* st = c->dev<DevState>(c->lo.state);
+  const uint32_t* parent_of = c->dev<uint32_t>(c->lo.parent_of);
   if constexpr (L >= 64) {
     const unsigned grid = (unsigned)(((uint64_t)c->cap + Geo<L>::RPB - 1) / Geo<L>::RPB);
-    k_sweep<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa,
-                                                      c->dev<uint32_t>(c->lo.parent_of));
+    launch(c, "k_sweep", k_sweep<L>, grid, SWEEP_THREADS, st, s0, s1, e0, e1, m0, m1, c->key, sa, parent_of);
   } else {
     const uint64_t threads = ((uint64_t)c->cap + 1) / 2 * SGeo<L>::G;  // a group of G lanes holds two replicas
     const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
-    k_sweep_small<L><<<grid, SWEEP_THREADS, 0, c->stream>>>(st, s0, s1, e0, e1, m0, m1, c->key, sa,
-                                                            c->dev<uint32_t>(c->lo.parent_of));
+    launch(c, "k_sweep_small", k_sweep_small<L>, grid, SWEEP_THREADS, st, s0, s1, e0, e1, m0, m1, c->key, sa, parent_of);
   }
 }
-// mode 0: theta sweeps of the resampled population with the thresholds of the step; mode 1: energies only
+// mode 2: theta sweeps of the resampled population (lattices gathered from the parents' slots); mode 1: energies only
 void launch_sweep(pa_ctx* c, int theta, uint32_t T4, uint32_t T8, int mode) {
   Prof p(c, PA_K_SWEEP);
   const SweepArgs sa = sweep_args(theta, T4, T8, mode);
@@ -219,39 +238,37 @@ void launch_sweep(pa_ctx* c, int theta, uint32_t T4, uint32_t T8, int mode) {
 }
 
 template <int L>
-void launch_copy_L(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end, bool map_only) {
+void launch_copy_L(pa_ctx* c) {
   const unsigned grid = (unsigned)((c->cap + CopyGeo<L>::CT - 1) / CopyGeo<L>::CT);
-  uint32_t *s0 = c->dev<uint32_t>(c->lo.spins[0]), *s1 = c->dev<uint32_t>(c->lo.spins[1]);
-  int32_t *e0 = c->dev<int32_t>(c->lo.E[0]), *e1 = c->dev<int32_t>(c->lo.E[1]);
-  int32_t *m0 = c->dev<int32_t>(c->lo.M[0]), *m1 = c->dev<int32_t>(c->lo.M[1]);
-  k_copy<L><<<grid, COPY_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), c->dev<uint32_t>(c->lo.off),
-                                                  c->dev<uint32_t>(c->lo.tile_parent), s0, s1, e0, e1, m0, m1,
-                                                  c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]),
-                                                  c->dev<uint32_t>(c->lo.part_stats), c->cfg.P,
-                                                  c->dev<unsigned long long>(c->lo.tile_desc), chunk, c->nchunks,
-                                                  tile_begin, tile_end,
-                                                  map_only ? c->dev<uint32_t>(c->lo.parent_of) : nullptr);
+  launch(c, "k_copy", k_copy<L>, grid, COPY_THREADS, c->dev<DevState>(c->lo.state), c->dev<uint32_t>(c->lo.off),
+         c->dev<uint32_t>(c->lo.tile_parent), c->dev<uint32_t>(c->lo.spins[0]), c->dev<uint32_t>(c->lo.spins[1]),
+         c->dev<int32_t>(c->lo.E[0]), c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]),
+         c->dev<int32_t>(c->lo.M[1]));
 }
-void launch_copy(pa_ctx* c, int chunk, unsigned tile_begin, unsigned tile_end, bool map_only) {
+void launch_copy(pa_ctx* c) {
   Prof p(c, PA_K_COPY);
   switch (c->cfg.L) {
-    case 8: launch_copy_L<8>(c, chunk, tile_begin, tile_end, map_only); break;
-    case 16: launch_copy_L<16>(c, chunk, tile_begin, tile_end, map_only); break;
-    case 32: launch_copy_L<32>(c, chunk, tile_begin, tile_end, map_only); break;
-    case 64: launch_copy_L<64>(c, chunk, tile_begin, tile_end, map_only); break;
-    default: launch_copy_L<128>(c, chunk, tile_begin, tile_end, map_only); break;
+    case 8: launch_copy_L<8>(c); break;
+    case 16: launch_copy_L<16>(c); break;
+    case 32: launch_copy_L<32>(c); break;
+    case 64: launch_copy_L<64>(c); break;
+    default: launch_copy_L<128>(c); break;
   }
 }
 
+// mode 0: sums of the new population, a5 (partition table + diagnostics) and the commit of the step; mode 1: sums only
 void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
   Prof p(c, PA_K_OBSERVE);
-  k_observe<<<OBS_GRID, OBS_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.E[0]),
-                                                     c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]),
-                                                     c->dev<int32_t>(c->lo.M[1]),
-                                                     c->dev<unsigned long long>(c->lo.obs_partial), mode, c->N);
+  launch(c, "k_observe", k_observe, OBS_GRID, OBS_THREADS, c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.E[0]),
+         c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]), c->dev<int32_t>(c->lo.M[1]),
+         c->dev<unsigned long long>(c->lo.obs_partial), mode, c->N, c->dev<uint32_t>(c->lo.off),
+         c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]), c->dev<uint32_t>(c->lo.part_stats), c->cfg.P);
 }
 
-// all kernels of one temperature step, parameters in device slot sp
+// all kernels of one temperature step, parameters in device slot sp:
+//   theta = 0:  k_q_reduce (+ level tables), k_poisson_scan, k_copy, k_observe (+ a5)
+//   theta > 0:  k_q_reduce (+ level tables), k_poisson_scan (+ child -> parent map), k_sweep (gathers the lattices
+//               itself), k_observe (+ a5)
 void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   const int theta = hp.theta;
   DevState* st = c->dev<DevState>(c->lo.state);
@@ -259,26 +276,20 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   const int N = c->N;
   const int n_desc = (int)((c->cap + SCAN_TILE - 1) / SCAN_TILE + 1);
   const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
-  std::optional<Prof> span;  // a1-a6 as one span on the caller's stream (not a launch)
-  span.emplace(c, PA_K_RESAMPLE_SPAN, nullptr, false);
+  std::optional<Prof> span;  // a1-a6 as one span on the stream (not a launch)
+  span.emplace(c, PA_K_RESAMPLE_SPAN, false);
   {
     Prof p(c, PA_K_Q_REDUCE);  // also resets the step's counters and look-back descriptors
-    k_q_reduce<<<RED_GRID, RED_THREADS, 0, c->stream>>>(st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
-                                                        (double)c->cfg.R0,
-                                                        c->dev<unsigned long long>(c->lo.tile_desc), n_desc);
-  }
-  {
-    Prof p(c, PA_K_LEVELS_TAU);  // the window of occupied levels is on the device: launch for all N + 1
-    k_levels_tau<<<(N + 1 + 127) / 128, 128, 0, c->stream>>>(st, sp, tb, N);
+    launch(c, "k_q_reduce", k_q_reduce, RED_GRID, RED_THREADS, st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
+           (double)c->cfg.R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tb);
   }
   {
     // persistent blocks pull tiles from a ticket counter
     const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
     const bool keep = c->lo.n || c->lo.tau;
-    if (c->scan_grid_max == 0) {  // all blocks co-resident: blocks per SM (occupancy) x SMs
+    if (c->scan_grid_max == 0) {  // blocks per SM (occupancy) x SMs
       int per_sm = 0, sms = 0;
-      if (keep) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true>, SCAN_THREADS, 0);
-      else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<false>, SCAN_THREADS, 0);
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true>, SCAN_THREADS, 0);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
       c->scan_grid_max = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
     }
@@ -287,42 +298,19 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     out.n = c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr;
     out.tau = c->lo.tau ? c->dev<double>(c->lo.tau) : nullptr;
     out.tile_desc = c->dev<unsigned long long>(c->lo.tile_desc);
+    out.parent_of = c->dev<uint32_t>(c->lo.parent_of);
     out.tile_parent = c->dev<uint32_t>(c->lo.tile_parent);
-    out.part0 = c->dev<uint32_t>(c->lo.part[0]);
-    out.part1 = c->dev<uint32_t>(c->lo.part[1]);
-    out.part_stats = c->dev<uint32_t>(c->lo.part_stats);
-    // a2-a6.  One chunk: scan then copy on the caller's stream.  Several chunks: the issue-bound scan of chunk i+1
-    // (library stream, high priority so that its persistent blocks are placed first) runs under the HBM-bound copy of
-    // chunk i (caller's stream); events order scan i -> copy i, and everything joins the caller's stream again.
-    const int C = c->nchunks;
-    const unsigned per = (tiles_cap + C - 1) / C;
-    cudaStream_t ss = C > 1 ? c->scan_stream : c->stream;
-    if (C > 1) {
-      cudaEventRecord(c->ev_fork, c->stream);
-      cudaStreamWaitEvent(ss, c->ev_fork, 0);
-    }
-    for (int i = 0; i < C; ++i) {
-      const unsigned t0 = per * i, t1 = (i == C - 1) ? tiles_cap : per * (i + 1);
-      const unsigned ntl = t1 - t0;
-      const unsigned grid = ntl < (unsigned)c->scan_grid_max ? (ntl ? ntl : 1u) : (unsigned)c->scan_grid_max;
-      {
-        Prof p(c, PA_K_POISSON_SCAN, ss);
-        if (keep)
-          k_poisson_scan<true><<<grid, SCAN_THREADS, 0, ss>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
-                                                              (unsigned long long)c->cap, c->key, i, t0, t1);
-        else
-          k_poisson_scan<false><<<grid, SCAN_THREADS, 0, ss>>>(st, E0, E1, tb, N, out, copy_shift_for(c->cfg.L),
-                                                               (unsigned long long)c->cap, c->key, i, t0, t1);
-      }
-      if (C > 1) {
-        cudaEventRecord(c->ev_scan[i], ss);
-        cudaStreamWaitEvent(c->stream, c->ev_scan[i], 0);
-      }
-      launch_copy(c, i, t0, t1, theta > 0);
-    }
+    const int shift = copy_shift_for(c->cfg.L);
+    const unsigned long long cap = (unsigned long long)c->cap;
+    const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? (tiles_cap ? tiles_cap : 1u) : (unsigned)c->scan_grid_max;
+    Prof p(c, PA_K_POISSON_SCAN);
+    if (keep && theta > 0) launch(c, "k_poisson_scan", k_poisson_scan<true, true>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key);
+    else if (keep) launch(c, "k_poisson_scan", k_poisson_scan<true, false>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key);
+    else if (theta > 0) launch(c, "k_poisson_scan", k_poisson_scan<false, true>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key);
+    else launch(c, "k_poisson_scan", k_poisson_scan<false, false>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key);
   }
+  if (theta == 0) launch_copy(c);  // a6; with sweeps to follow it is fused into the sweep's load
   span.reset();
-  // theta > 0: a6 is fused into the sweep's load (k_copy only wrote the child -> parent map)
   if (theta > 0) launch_sweep(c, theta, hp.T4, hp.T8, 2);
   launch_observe(c, sp, 0);
 }
@@ -356,11 +344,24 @@ __global__ void k_clear_status(DevState* st) {
   st->obs_done = 0u;
 }
 
+// a context is bound to the device that was current in pa_init
+int bind_device(pa_ctx* c) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) == cudaSuccess && dev == c->device) return PA_OK;
+  CK(cudaSetDevice(c->device));
+  return PA_OK;
+}
+
 // read the device state back (synchronises) and refresh the host mirrors
 int sync_state(pa_ctx* c) {
   CK(cudaMemcpyAsync(c->h_state, c->dev<DevState>(c->lo.state), sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   CK(cudaGetLastError());
+  if (!c->launch_err.empty()) {
+    const std::string msg = "kernel launch failed: " + c->launch_err;
+    c->launch_err.clear();
+    return fail(c, PA_ECUDA, msg);
+  }
   const DevState& s = *c->h_state;
   c->R = (int64_t)s.R;
   c->R_parents = (int64_t)s.R_parents;
@@ -388,6 +389,7 @@ int status_to_code(pa_ctx* c) {
 
 int copy_out(pa_ctx* c, void* dst, const void* src_dev, size_t bytes, int dst_on_device) {
   if (bytes == 0) return PA_OK;
+  if (int rc = bind_device(c)) return rc;
   CK(cudaMemcpyAsync(dst, src_dev, bytes, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   return PA_OK;
@@ -438,7 +440,7 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   if (!c) return PA_ENOMEM;
   c->cfg = *cfg;
   c->cap = cfg->capacity > 0 ? cfg->capacity : (cfg->R0 >= 1 ? default_capacity(cfg->R0) : 0);
-  if (!make_layout(cfg, c->cap, &c->lo) || !(cfg->beta0 == cfg->beta0)) {
+  if (!make_layout(cfg, c->cap, &c->lo) || !(cfg->beta0 == cfg->beta0) || cfg->reserved != 0u) {
     delete c;
     return PA_EINVAL;
   }
@@ -451,20 +453,12 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   c->ws = static_cast<char*>(cfg->workspace);
   c->stream = static_cast<cudaStream_t>(cfg->stream);
   c->profile = (cfg->flags & PA_PROFILE) != 0;
+  c->profile_span = (cfg->flags & PA_PROFILE_SPAN) != 0;
   c->launches = 0;
   c->attempt_failed = false;
   c->dbg_thresholds = false;
   c->dbg_T4 = c->dbg_T8 = 0u;
   c->scan_grid_max = 0;
-  {
-    const uint64_t tiles_cap = ((uint64_t)c->cap + SCAN_TILE - 1) / SCAN_TILE;
-    int C = (int)cfg->scan_chunks;
-    if (C == 0) C = 1;  // measured on B200 (config 5): 2 / 4 / 8 chunks are 4 % / 12 % / 26 % SLOWER than one
-    if (C > 8) C = 8;
-    if ((uint64_t)C > tiles_cap) C = (int)tiles_cap;
-    c->nchunks = C < 1 ? 1 : C;
-    c->scan_stream = nullptr;
-  }
   uint32_t k0 = (uint32_t)(cfg->seed & 0xffffffffull), k1 = (uint32_t)(cfg->seed >> 32);
   for (int r = 0; r < 10; ++r) {
     c->key.k0[r] = k0;
@@ -487,13 +481,6 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
     return PA_ECUDA;
   }
   *out = c;  // from here on errors keep the ctx so that pa_last_error works; caller destroys it
-  if (c->nchunks > 1) {
-    int lo_prio = 0, hi_prio = 0;
-    CK(cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio));
-    CK(cudaStreamCreateWithPriority(&c->scan_stream, cudaStreamNonBlocking, hi_prio));
-    CK(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
-    for (int i = 0; i < c->nchunks; ++i) CK(cudaEventCreateWithFlags(&c->ev_scan[i], cudaEventDisableTiming));
-  }
   DevState* st = c->dev<DevState>(c->lo.state);
   k_init_state<<<1, 256, 0, c->stream>>>(st, (unsigned long long)cfg->R0, cfg->beta0, c->dev<uint32_t>(c->lo.part[0]),
                                          cfg->P);
@@ -518,6 +505,7 @@ int pa_run(pa_ctx* c, const double* betas, int32_t K, int32_t theta, int32_t* st
   if (!c) return PA_EINVAL;
   if (steps_done) *steps_done = 0;
   if (K < 0 || (K > 0 && !betas)) return fail(c, PA_EINVAL, "bad betas/K");
+  if (int rc = bind_device(c)) return rc;
   double from = c->beta;
   for (int k = 0; k < K; ++k) {
     const int rc = check_step_args(c, from, betas[k], theta);
@@ -668,6 +656,7 @@ int pa_debug_set_thresholds(pa_ctx* c, int enable, uint32_t T4, uint32_t T8) {
 
 int pa_set_spins(pa_ctx* c, const uint32_t* src, int64_t R, int src_on_device) {
   if (!c || !src || R < 1 || R > c->cap) return fail(c, PA_EINVAL, "pa_set_spins: bad arguments");
+  if (int rc = bind_device(c)) return rc;
   const unsigned cur = c->h_state->cur;
   CK(cudaMemcpyAsync(c->dev<uint32_t>(c->lo.spins[cur]), src, (size_t)R * c->wrep * 4,
                      src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
@@ -710,12 +699,6 @@ int pa_destroy(pa_ctx* c) {
   cudaStreamSynchronize(c->stream);
   for (EventPair& ep : c->ev_used) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
   for (EventPair& ep : c->ev_free) { cudaEventDestroy(ep.a); cudaEventDestroy(ep.b); }
-  if (c->scan_stream) {
-    cudaStreamSynchronize(c->scan_stream);
-    cudaStreamDestroy(c->scan_stream);
-    cudaEventDestroy(c->ev_fork);
-    for (int i = 0; i < c->nchunks; ++i) cudaEventDestroy(c->ev_scan[i]);
-  }
   if (c->h_state) cudaFreeHost(c->h_state);
   if (c->h_params) cudaFreeHost(c->h_params);
   delete c;

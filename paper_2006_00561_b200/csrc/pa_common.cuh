@@ -30,7 +30,8 @@ struct DevState {
   unsigned int status;           // 0 = ok, else -pa_status of the failing step
   unsigned int fail_step;        // ordinal of the step that failed
   unsigned int reduce_done;      // block counters (reset every step by k_q_reduce)
-  unsigned int scan_tile[8];     // ticket counters of k_poisson_scan, one per chunk launch
+  unsigned int scan_tile;        // ticket counter of k_poisson_scan
+  unsigned int pad2_[7];
   unsigned int scan_overflow;    // a parent sat on a level with lambda >= 2^31
   unsigned int obs_done;
   unsigned int T4, T8;           // thresholds of the last committed step with theta > 0
@@ -80,5 +81,23 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 }
 
 __device__ __forceinline__ uint32_t ctr3(uint32_t tag, uint32_t step) { return (tag << 28) | step; }
+
+#ifndef PA_PDL_TRIGGER
+#define PA_PDL_TRIGGER 0
+#endif
+#ifndef PA_PDL
+#define PA_PDL 1
+#endif
+// Programmatic dependent launch: the kernels of a step are launched with programmatic stream serialisation, so a
+// kernel's launch is staged while its predecessor runs; nothing the predecessor wrote is touched before this returns
+// (a no-op when the kernel was launched without the attribute).  An early griddepcontrol.launch_dependents was
+// measured SLOWER on B200 (config 5: a1-a6 0.738 ms with it, 0.679 ms without, 0.683 ms without PDL at all): the
+// successor's blocks park on the SMs and take registers and warp slots from the kernel that still works.
+__device__ __forceinline__ void grid_dependency_wait() {
+#if PA_PDL_TRIGGER
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the successor's blocks may be placed once all of ours have started
+#endif
+  asm volatile("griddepcontrol.wait;" ::: "memory");               // ... but nobody reads before the predecessor is complete
+}
 
 }  // namespace pa

@@ -44,6 +44,43 @@ __device__ __forceinline__ U128 warp_sum_u128(U128 v) {
   return v;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// balance_tile: a5.  One block (the last block of k_observe: every offset of the step is in memory).
+// New partition table, born/excess/shortage per partition, moved count.  PAPER.md:104-106; A6.
+// ---------------------------------------------------------------------------------------------------
+__device__ void balance_tile(DevState* st, const uint32_t* off, uint32_t* part0, uint32_t* part1, uint32_t* stats,
+                             int P) {
+  if (*((volatile unsigned*)&st->status) != ST_OK) return;
+  const uint32_t* old_start = st->cur ? part1 : part0;
+  uint32_t* new_start = st->cur ? part0 : part1;
+  const unsigned long long Rnew = *((volatile unsigned long long*)&st->Rnew);
+  const unsigned long long base = Rnew / P, rem = Rnew % P;
+  __shared__ unsigned long long s_same;
+  if (threadIdx.x == 0) s_same = 0ull;
+  __syncthreads();
+  unsigned long long same = 0;
+  for (int p = threadIdx.x; p <= P; p += blockDim.x) {
+    const unsigned long long s = (unsigned long long)p * base + ((unsigned long long)p < rem ? p : rem);
+    new_start[p] = (uint32_t)s;
+    if (p < P) {
+      const unsigned long long e = (unsigned long long)(p + 1) * base + ((unsigned long long)(p + 1) < rem ? p + 1 : rem);
+      const uint32_t cnt = (uint32_t)(e - s);
+      const uint32_t b0 = __ldcg(off + old_start[p]), b1 = __ldcg(off + old_start[p + 1]);
+      const uint32_t born = b1 - b0;
+      stats[4 * p + 0] = cnt;
+      stats[4 * p + 1] = born;
+      stats[4 * p + 2] = born > cnt ? born - cnt : 0u;
+      stats[4 * p + 3] = cnt > born ? cnt - born : 0u;
+      // children of partition p's parents occupy [b0, b1); those inside [s, e) stay in partition p
+      const unsigned long long lo = b0 > s ? b0 : s, hi = b1 < e ? b1 : e;
+      if (hi > lo) same += hi - lo;
+    }
+  }
+  atomicAdd(&s_same, same);
+  __syncthreads();
+  if (threadIdx.x == 0) st->moved = Rnew - s_same;
+}
+
 constexpr int OBS_THREADS = 256;
 constexpr int OBS_Q = 5;  // sum E (two's complement), sum E^2, sum |M|, sum M^2, sum M^4
 
@@ -52,7 +89,9 @@ constexpr int OBS_Q = 5;  // sum E (two's complement), sum E^2, sum |M|, sum M^2
 __global__ void __launch_bounds__(OBS_THREADS)
 k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
           const int32_t* __restrict__ E1, const int32_t* __restrict__ M0, const int32_t* __restrict__ M1,
-          unsigned long long* __restrict__ partial /* [grid][12] */, const int mode, const int N) {
+          unsigned long long* __restrict__ partial /* [grid][12] */, const int mode, const int N,
+          const uint32_t* __restrict__ off, uint32_t* part0, uint32_t* part1, uint32_t* part_stats, const int P) {
+  grid_dependency_wait();
   if (st->status != ST_OK) return;
   const unsigned buf = mode == 0 ? (st->cur ^ 1u) : st->cur;
   const unsigned long long count = mode == 0 ? st->Rnew : st->R;
@@ -170,6 +209,10 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
     }
   }
   __syncthreads();
+  if (mode == 0) {  // a5: partition table of the new population + the paper's diagnostics, before the commit flips `cur`
+    balance_tile(st, off, part0, part1, part_stats, P);
+    __syncthreads();
+  }
   if (threadIdx.x == 0) {
     long long lo = s_lohi[0], hi = s_lohi[1];
     if (lo > hi) lo = hi = -2 * N;  // empty population: cannot happen (R >= 1), keep the window valid

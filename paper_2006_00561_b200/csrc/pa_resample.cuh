@@ -32,14 +32,74 @@ __device__ __forceinline__ double level_weight(double dbeta, int lev, int N) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// level_tables: per level tau = w / Q (eq. 4), lambda = tau * scale, and the A4 chunk tables
+// (m, mu, F_0..F_64).  Only individually rounded IEEE operations (no FMA contraction).  Run by the last block of
+// k_q_reduce, one thread per occupied level (a few hundred levels, up to 64 dependent divisions each).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double expneg_a4(double mu) {
+  // c_i = nearest double to (-1)^i / i!, i = 0..14
+  constexpr double c[15] = {0x1.0000000000000p+0,   -0x1.0000000000000p+0,  0x1.0000000000000p-1,
+                            -0x1.5555555555555p-3,  0x1.5555555555555p-5,   -0x1.1111111111111p-7,
+                            0x1.6c16c16c16c17p-10,  -0x1.a01a01a01a01ap-13, 0x1.a01a01a01a01ap-16,
+                            -0x1.71de3a556c734p-19, 0x1.27e4fb7789f5cp-22,  -0x1.ae64567f544e4p-26,
+                            0x1.1eed8eff8d898p-29,  -0x1.6124613a86d09p-33, 0x1.93974a8c07c9dp-37};
+  const double t = __dmul_rn(mu, 0.0625);
+  double p = c[14];
+#pragma unroll
+  for (int i = 13; i >= 0; --i) p = __dadd_rn(__dmul_rn(p, t), c[i]);
+#pragma unroll
+  for (int s = 0; s < 4; ++s) p = __dmul_rn(p, p);
+  return p;
+}
+
+__device__ __forceinline__ void level_tables(double dbeta, int lev, int N, double Q, double scale, const LevelTables& tb) {
+  const double tau = __ddiv_rn(level_weight(dbeta, lev, N), Q);
+  const double lambda = __dmul_rn(tau, scale);
+  tb.tau[lev] = tau;
+  double* F = tb.cdf + (size_t)lev * PO_ROW;
+  if (!(lambda > 0.0)) {
+    tb.m[lev] = 0u;
+    tb.mu[lev] = 0.0;
+    return;
+  }
+  if (!(lambda < 2147483648.0)) {  // would exceed any capacity: reported as PA_ECAPACITY if a replica sits here
+    tb.m[lev] = M_OVERFLOW;
+    tb.mu[lev] = 0.0;
+    return;
+  }
+  long long m = (long long)ceil(__ddiv_rn(lambda, 8.0));
+  if (m < 1) m = 1;
+  const double mu = __ddiv_rn(lambda, (double)m);
+  tb.m[lev] = (unsigned)m;
+  tb.mu[lev] = mu;
+  double p = expneg_a4(mu), Fk = p;
+  F[0] = Fk;
+  int k = 1;
+  for (; k <= PO_KMAX; ++k) {
+    p = __ddiv_rn(__dmul_rn(p, mu), (double)k);
+    const double Fn = __dadd_rn(Fk, p);
+    F[k] = Fn;
+    // past the mode (k > mu) p only shrinks: once it no longer moves F, no later term does (identical bits, fewer
+    // dependent divisions)
+    if (Fn == Fk && (double)k > mu) break;
+    Fk = Fn;
+  }
+  for (++k; k <= PO_KMAX; ++k) F[k] = Fk;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // k_q_reduce: eq. 3, first kernel of every step (it also resets the per-step counters and the scan's tile
 // descriptors).  The population occupies the levels lev_lo..lev_hi (found by k_observe when the population was
 // written); every block tabulates w for that window in shared memory (a few hundred exp per block), then: grid-stride
 // 128-bit loads of E, look-up, per-thread serial sum, warp-shuffle tree, block partials; the last block to finish adds
-// the partials in index order (deterministic for a given grid) and writes sumw, Q = sumw / R, ln Q, scale = R0 / R.
+// the partials in index order (deterministic for a given grid) and writes sumw, Q = sumw / R, ln Q, scale = R0 / R,
+// and then the per-level tables of eq. 4 and of the Poisson sampler (level_tables above).
 // A window wider than QW_MAX levels (crafted test populations) evaluates exp per replica instead: same bits.
 // ---------------------------------------------------------------------------------------------------
 constexpr int RED_THREADS = 256;
+#ifndef PA_RED_UNR8
+#define PA_RED_UNR8 0
+#endif
 constexpr int QW_MAX = 2048;
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -51,11 +111,12 @@ __device__ __forceinline__ double warp_sum(double v) {
 __global__ void __launch_bounds__(RED_THREADS)
 k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
            const int32_t* __restrict__ E1, int N, double* __restrict__ partial, double R0,
-           unsigned long long* __restrict__ tile_desc, int n_desc) {
+           unsigned long long* __restrict__ tile_desc, int n_desc, LevelTables tb) {
+  grid_dependency_wait();
   const unsigned long long tid = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x;
   const unsigned long long stride = (unsigned long long)gridDim.x * RED_THREADS;
   if (tid == 0) {  // counters of the later kernels of this step (reduce_done is reset by the last block below)
-    for (int i = 0; i < 8; ++i) st->scan_tile[i] = 0u;
+    st->scan_tile = 0u;
     st->scan_overflow = 0u;
     st->obs_done = 0u;
   }
@@ -76,6 +137,17 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
     const int shift = twoN - 4 * lev_lo;  // level(E) - lev_lo = (E + 2N - 4 lev_lo) / 4
     auto wl = [&](int e) { return s_w[(e + shift) >> 2]; };
     unsigned long long v = tid;
+#if PA_RED_UNR8
+    for (; v + 7 * stride < nvec; v += 8 * stride) {  // eight 128-bit loads in flight per thread
+      int4 x[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) x[u] = __ldg(E4 + v + u * stride);
+      double t[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) t[u] = (wl(x[u].x) + wl(x[u].y)) + (wl(x[u].z) + wl(x[u].w));
+      acc += ((t[0] + t[1]) + (t[2] + t[3])) + ((t[4] + t[5]) + (t[6] + t[7]));
+    }
+#endif
     for (; v + 3 * stride < nvec; v += 4 * stride) {  // four 128-bit loads in flight per thread
       const int4 a = __ldg(E4 + v), b = __ldg(E4 + v + stride), c = __ldg(E4 + v + 2 * stride), d = __ldg(E4 + v + 3 * stride);
       acc += (((wl(a.x) + wl(a.y)) + (wl(a.z) + wl(a.w))) + ((wl(b.x) + wl(b.y)) + (wl(b.z) + wl(b.w)))) +
@@ -111,7 +183,9 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
     s_last = (done == gridDim.x - 1);
   }
   __syncthreads();
-  if (s_last && threadIdx.x < 32) {
+  if (!s_last) return;
+  __shared__ double s_Q;
+  if (threadIdx.x < 32) {
     __threadfence();
     double t = 0.0;
     for (unsigned b = threadIdx.x; b < gridDim.x; b += 32) t += __ldcg(&partial[b]);
@@ -123,66 +197,16 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
       st->lnQ = log(Q);
       st->scale = R0 / (double)R;
       st->reduce_done = 0u;  // every block has arrived: ready for the next step
+      s_Q = Q;
     }
   }
-}
-
-// ---------------------------------------------------------------------------------------------------
-// k_levels_tau: per level tau = w / Q (eq. 4), lambda = tau * scale, and the A4 chunk tables
-// (m, mu, F_0..F_64).  Only individually rounded IEEE operations (no FMA contraction).
-// ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double expneg_a4(double mu) {
-  // c_i = nearest double to (-1)^i / i!, i = 0..14
-  constexpr double c[15] = {0x1.0000000000000p+0,   -0x1.0000000000000p+0,  0x1.0000000000000p-1,
-                            -0x1.5555555555555p-3,  0x1.5555555555555p-5,   -0x1.1111111111111p-7,
-                            0x1.6c16c16c16c17p-10,  -0x1.a01a01a01a01ap-13, 0x1.a01a01a01a01ap-16,
-                            -0x1.71de3a556c734p-19, 0x1.27e4fb7789f5cp-22,  -0x1.ae64567f544e4p-26,
-                            0x1.1eed8eff8d898p-29,  -0x1.6124613a86d09p-33, 0x1.93974a8c07c9dp-37};
-  const double t = __dmul_rn(mu, 0.0625);
-  double p = c[14];
-#pragma unroll
-  for (int i = 13; i >= 0; --i) p = __dadd_rn(__dmul_rn(p, t), c[i]);
-#pragma unroll
-  for (int s = 0; s < 4; ++s) p = __dmul_rn(p, p);
-  return p;
-}
-
-__global__ void k_levels_tau(const DevState* st, const StepParams* __restrict__ sp, LevelTables tb, int N) {
-  if (st->status != ST_OK) return;
-  const int lev = st->lev_lo + blockIdx.x * blockDim.x + threadIdx.x;  // only the occupied window is ever looked up
-  if (lev > st->lev_hi || lev > N) return;
-  const double tau = __ddiv_rn(level_weight(sp->dbeta, lev, N), st->Q);
-  const double lambda = __dmul_rn(tau, st->scale);
-  tb.tau[lev] = tau;
-  double* F = tb.cdf + (size_t)lev * PO_ROW;
-  if (!(lambda > 0.0)) {
-    tb.m[lev] = 0u;
-    tb.mu[lev] = 0.0;
-    return;
+  __syncthreads();
+  // a2 per level: the tables of the occupied window (only that window is ever looked up)
+  {
+    const double Q = s_Q, scale = R0 / (double)R;
+    const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
+    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(dbeta, lev, N, Q, scale, tb);
   }
-  if (!(lambda < 2147483648.0)) {  // would exceed any capacity: reported as PA_ECAPACITY if a replica sits here
-    tb.m[lev] = M_OVERFLOW;
-    tb.mu[lev] = 0.0;
-    return;
-  }
-  long long m = (long long)ceil(__ddiv_rn(lambda, 8.0));
-  if (m < 1) m = 1;
-  const double mu = __ddiv_rn(lambda, (double)m);
-  tb.m[lev] = (unsigned)m;
-  tb.mu[lev] = mu;
-  double p = expneg_a4(mu), Fk = p;
-  F[0] = Fk;
-  int k = 1;
-  for (; k <= PO_KMAX; ++k) {
-    p = __ddiv_rn(__dmul_rn(p, mu), (double)k);
-    const double Fn = __dadd_rn(Fk, p);
-    F[k] = Fn;
-    // past the mode (k > mu) p only shrinks: once it no longer moves F, no later term does (identical bits, fewer
-    // dependent divisions)
-    if (Fn == Fk && (double)k > mu) break;
-    Fk = Fn;
-  }
-  for (++k; k <= PO_KMAX; ++k) F[k] = Fk;
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -193,7 +217,15 @@ __global__ void k_levels_tau(const DevState* st, const StepParams* __restrict__ 
 //            60 % of the children in config 5) form ONE flat work list that all 256 threads share, so that a parent
 //            with lambda = 10^4 (1250 chunks) costs the tile 5 passes instead of serialising one warp; counts are
 //            integer sums, so the result does not depend on who draws which chunk;
-//   phase 3  block scan of the counts, look-back across tiles, offsets / counts / copy-tile parents written.
+//   phase 3  block scan of the counts, look-back across tiles, offsets / counts written.  Then what the consumer of
+//            the step needs to find the parents:
+//            MAP (theta > 0)   the child -> parent map parent_of[i] (A5: the unique j with off_j <= i < off_j + n_j),
+//                              expanded warp by warp: the 256 parents of a warp own one contiguous range of children,
+//                              which the warp marks and max-scans 256 children at a time in its slice of shared memory
+//                              (no block barrier, coalesced stores); the sweep's gather-on-load reads it;
+//            !MAP (theta = 0)  only the parent that covers the first child of every copy tile; k_copy walks the
+//                              offsets from there (measured on config 5: the full map costs the scan 0.05 ms and does
+//                              not make the copy faster).
 // ---------------------------------------------------------------------------------------------------
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ROUNDS = 8;
@@ -230,16 +262,13 @@ __device__ __forceinline__ unsigned draw_chunk(const double* __restrict__ F, uin
   return cdf_search_from(reinterpret_cast<const double2*>(F), 0, chunk_uniform(w, (unsigned)(c & 1ull)));
 }
 
-// a5 (defined below); run by block 0 of k_copy
-__device__ void balance_tile(DevState* st, const uint32_t* off, uint32_t* part0, uint32_t* part1, uint32_t* stats, int P);
-
 struct ScanOut {
   uint32_t* off;            // [R + 1] exclusive offsets, off[R] = R'
   uint32_t* n;              // [R] copy counts (PA_KEEP_COUNTS) or null
   double* tau;              // [R] weights (PA_KEEP_TAU) or null
   unsigned long long* tile_desc;
-  uint32_t* tile_parent;    // per copy tile: the parent covering its first child
-  uint32_t *part0, *part1, *part_stats;
+  uint32_t* parent_of;      // MAP:  [R'] child -> parent map (theta > 0: read by the sweep's gather-on-load)
+  uint32_t* tile_parent;    // !MAP: per copy tile the parent covering its first child (theta = 0: read by k_copy)
 };
 
 constexpr int SCAN_BATCH = 4;  // independent Philox chains in flight per thread
@@ -254,13 +283,13 @@ constexpr unsigned NO_TILE = 0xffffffffu;
 // A tiles, 32 per round trip) is hidden behind B's sampling.  Every ticket holder publishes its aggregate before it
 // waits on anything, so the look-back cannot deadlock.
 #ifndef PA_SCAN_MINB
-#define PA_SCAN_MINB 6
+#define PA_SCAN_MINB 7
 #endif
-template <bool KEEP>
-__global__ void __launch_bounds__(SCAN_THREADS, PA_SCAN_MINB)
+template <bool KEEP, bool MAP>
+__global__ void __launch_bounds__(SCAN_THREADS, (MAP ? PA_SCAN_MINB - 1 : PA_SCAN_MINB))
 k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
-               ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key, int chunk,
-               unsigned tile_begin, unsigned tile_end_cap) {
+               ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key) {
+  grid_dependency_wait();
   if (st->status != ST_OK) return;
   __shared__ unsigned s_tile;
   __shared__ unsigned s_flag;            // bit 0: a parent of this block sits on an overflowing level
@@ -283,7 +312,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
   }
   const uint32_t R = (uint32_t)st->R;  // R <= capacity < 2^32 - 4096: parent indices fit 32 bits
   const unsigned ntiles = (R + SCAN_TILE - 1) / SCAN_TILE;
-  const unsigned tile_end = tile_end_cap < ntiles ? tile_end_cap : ntiles;
+  const unsigned tile_end = ntiles;
   const int32_t* __restrict__ E = st->cur ? E1 : E0;
   const uint32_t c3 = ctr3(TAG_RESAMPLE, st->step + 1u);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -293,11 +322,11 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
 
   for (;;) {
     if (threadIdx.x == 0) {
-      s_tile = tile_begin + atomicAdd(&st->scan_tile[chunk], 1u);
+      s_tile = atomicAdd(&st->scan_tile, 1u);
       s_pack = 0ull;
     }
     __syncthreads();
-    const unsigned tile = s_tile < tile_end ? s_tile : NO_TILE;  // tiles of this launch: [tile_begin, tile_end)
+    const unsigned tile = s_tile < tile_end ? s_tile : NO_TILE;
     if (tile == NO_TILE && prev == NO_TILE) break;
 
     if (tile != NO_TILE) {
@@ -465,26 +494,26 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
       }
       unsigned long long o64 = s_prefix + warp_excl + (inc - tsum);  // offset of the thread's first item
 
-      // offsets, counts, and for every copy tile the parent that covers its first child
+      // offsets and counts
       const uint32_t j0 = tile_base + SCAN_ROUNDS * threadIdx.x;
+      const unsigned long long o_first = o64;
       uint32_t offs[SCAN_ROUNDS];
 #pragma unroll
       for (int i = 0; i < SCAN_ROUNDS; ++i) {
         offs[i] = (uint32_t)o64;  // exact whenever R' fits the capacity
-        if (cnt[i] > 0u && j0 + i < R && o64 + cnt[i] <= capacity) {  // then o, o + cnt fit 32 bits
-          const uint32_t o32 = (uint32_t)o64, ct1 = (1u << copy_shift) - 1u;
-          const uint32_t t_first = (o32 + ct1) >> copy_shift, t_last = (o32 + cnt[i] - 1u) >> copy_shift;
+        if constexpr (!MAP) {  // for every copy tile the parent that covers its first child
+          if (cnt[i] > 0u && j0 + i < R && o64 + cnt[i] <= capacity) {  // then o, o + cnt fit 32 bits
+            const uint32_t o32 = (uint32_t)o64, ct1 = (1u << copy_shift) - 1u;
+            const uint32_t t_first = (o32 + ct1) >> copy_shift, t_last = (o32 + cnt[i] - 1u) >> copy_shift;
 #pragma unroll 1
-          for (uint32_t t = t_first; t <= t_last; ++t) out.tile_parent[t] = j0 + i;
+            for (uint32_t t = t_first; t <= t_last; ++t) out.tile_parent[t] = j0 + i;
+          }
         }
         o64 += cnt[i];
       }
       if (j0 + SCAN_ROUNDS <= R) {
         *reinterpret_cast<uint4*>(out.off + j0) = make_uint4(offs[0], offs[1], offs[2], offs[3]);
         *reinterpret_cast<uint4*>(out.off + j0 + 4) = make_uint4(offs[4], offs[5], offs[6], offs[7]);
-        // the tile's inclusive prefix = first offset of the next tile: a copy launch that runs while the next chunk of
-        // the scan is still in flight reads it (the next tile writes the same value again)
-        if (threadIdx.x == SCAN_THREADS - 1) out.off[j0 + SCAN_ROUNDS] = (uint32_t)o64;
         if (KEEP) {
           if (out.n) {
             *reinterpret_cast<uint4*>(out.n + j0) = make_uint4(cnt[0], cnt[1], cnt[2], cnt[3]);
@@ -500,6 +529,81 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
               if (out.n) out.n[j0 + i] = cnt[i];
             }
           }
+        }
+      }
+      // child -> parent map of the warp's 256 parents: their children are the contiguous range [w_lo, w_lo + w_n).  Chunks
+      // of 256 children: every parent marks the position of its first child with its index inside the warp (+1), the
+      // parent that reaches into the chunk from before it is the carry, an inclusive max-scan fills the rest.  A chunk
+      // that lies inside one heavy parent's range is a plain fill.
+      if constexpr (MAP) {
+        unsigned* mk = const_cast<unsigned*>(cntb) + 256 * warp;  // the warp's slice: its counts are in registers by now
+        const unsigned long long w_lo = __shfl_sync(0xffffffffu, o_first, 0);
+        unsigned long long w_n64 = __shfl_sync(0xffffffffu, inc, 31);
+        if (w_lo >= capacity) w_n64 = 0ull;  // a step that will not be committed: stay inside the buffers
+        else if (w_lo + w_n64 > capacity) w_n64 = capacity - w_lo;
+        const uint32_t w_n = (uint32_t)w_n64;  // <= capacity < 2^32
+        const uint32_t wp_base = tile_base + 256u * (unsigned)warp;
+        uint32_t* __restrict__ pw = out.parent_of + w_lo;
+        // first child of each of the lane's parents relative to w_lo, saturated (counts of an uncommitted step may overflow)
+        uint32_t fr[SCAN_ROUNDS + 1];
+        {
+          unsigned long long f = o_first - w_lo;
+#pragma unroll
+          for (int i = 0; i <= SCAN_ROUNDS; ++i) {
+            fr[i] = f < 0xffffffffull ? (uint32_t)f : 0xffffffffu;
+            if (i < SCAN_ROUNDS) f += cnt[i];
+          }
+        }
+        __syncwarp();
+        for (uint32_t c_lo = 0u; c_lo < w_n; c_lo += 256u) {
+          // carry: the parent whose range starts before the chunk and reaches into it (at most one in the warp)
+          unsigned carry = 0u, cover = 0u;
+#pragma unroll
+          for (int i = 0; i < SCAN_ROUNDS; ++i)
+            if (fr[i] < c_lo && fr[i + 1] > c_lo) {
+              carry = (unsigned)(SCAN_ROUNDS * lane + i + 1);
+              cover = fr[i + 1] - c_lo;  // children of the chunk it covers (may exceed 256)
+            }
+          carry = __reduce_max_sync(0xffffffffu, carry);
+          cover = __reduce_max_sync(0xffffffffu, cover);
+          const unsigned n_here = w_n - c_lo < 256u ? w_n - c_lo : 256u;
+          if (cover >= n_here) {  // warp-uniform: the whole chunk belongs to the carry parent
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+              const unsigned c = (unsigned)lane + 32u * k;
+              if (c < n_here) pw[c_lo + c] = wp_base + carry - 1u;
+            }
+            continue;
+          }
+#pragma unroll
+          for (int k = 0; k < 8; ++k) mk[lane + 32 * k] = 0u;
+          __syncwarp();
+#pragma unroll
+          for (int i = 0; i < SCAN_ROUNDS; ++i)
+            if (fr[i + 1] > fr[i] && fr[i] >= c_lo && fr[i] < c_lo + 256u) mk[fr[i] - c_lo] = (unsigned)(SCAN_ROUNDS * lane + i + 1);
+          __syncwarp();
+          uint4 a = *reinterpret_cast<const uint4*>(&mk[8 * lane]), b = *reinterpret_cast<const uint4*>(&mk[8 * lane + 4]);
+          a.y = max(a.y, a.x); a.z = max(a.z, a.y); a.w = max(a.w, a.z);
+          b.x = max(b.x, a.w); b.y = max(b.y, b.x); b.z = max(b.z, b.y); b.w = max(b.w, b.z);
+          unsigned run = b.w;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const unsigned t = __shfl_up_sync(0xffffffffu, run, o);
+            if (lane >= o) run = max(run, t);
+          }
+          unsigned before = __shfl_up_sync(0xffffffffu, run, 1);
+          before = lane > 0 ? max(before, carry) : carry;
+          a.x = max(a.x, before); a.y = max(a.y, before); a.z = max(a.z, before); a.w = max(a.w, before);
+          b.x = max(b.x, before); b.y = max(b.y, before); b.z = max(b.z, before); b.w = max(b.w, before);
+          *reinterpret_cast<uint4*>(&mk[8 * lane]) = a;
+          *reinterpret_cast<uint4*>(&mk[8 * lane + 4]) = b;
+          __syncwarp();
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const unsigned c = (unsigned)lane + 32u * k;
+            if (c < n_here) pw[c_lo + c] = wp_base + mk[c] - 1u;
+          }
+          __syncwarp();
         }
       }
       if (threadIdx.x == 0) {
@@ -526,45 +630,9 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
 }
 
 // ---------------------------------------------------------------------------------------------------
-// balance_tile: a5.  One block (block 0 of k_copy: the scan kernel has finished, every offset is visible).  New
-// partition table, born/excess/shortage per partition, moved count.  PAPER.md:104-106; A6.
-// ---------------------------------------------------------------------------------------------------
-__device__ void balance_tile(DevState* st, const uint32_t* off, uint32_t* part0, uint32_t* part1, uint32_t* stats,
-                             int P) {
-  if (*((volatile unsigned*)&st->status) != ST_OK) return;
-  const uint32_t* old_start = st->cur ? part1 : part0;
-  uint32_t* new_start = st->cur ? part0 : part1;
-  const unsigned long long Rnew = *((volatile unsigned long long*)&st->Rnew);
-  const unsigned long long base = Rnew / P, rem = Rnew % P;
-  __shared__ unsigned long long s_same;
-  if (threadIdx.x == 0) s_same = 0ull;
-  __syncthreads();
-  unsigned long long same = 0;
-  for (int p = threadIdx.x; p <= P; p += blockDim.x) {
-    const unsigned long long s = (unsigned long long)p * base + ((unsigned long long)p < rem ? p : rem);
-    new_start[p] = (uint32_t)s;
-    if (p < P) {
-      const unsigned long long e = (unsigned long long)(p + 1) * base + ((unsigned long long)(p + 1) < rem ? p + 1 : rem);
-      const uint32_t cnt = (uint32_t)(e - s);
-      const uint32_t b0 = __ldcg(off + old_start[p]), b1 = __ldcg(off + old_start[p + 1]);
-      const uint32_t born = b1 - b0;
-      stats[4 * p + 0] = cnt;
-      stats[4 * p + 1] = born;
-      stats[4 * p + 2] = born > cnt ? born - cnt : 0u;
-      stats[4 * p + 3] = cnt > born ? cnt - born : 0u;
-      // children of partition p's parents occupy [b0, b1); those inside [s, e) stay in partition p
-      const unsigned long long lo = b0 > s ? b0 : s, hi = b1 < e ? b1 : e;
-      if (hi > lo) same += hi - lo;
-    }
-  }
-  atomicAdd(&s_same, same);
-  __syncthreads();
-  if (threadIdx.x == 0) st->moved = Rnew - s_same;
-}
-
-// ---------------------------------------------------------------------------------------------------
-// k_copy: a6.  Child-centric gather.  Block t owns children [t*CT, (t+1)*CT): it starts from the parent that
-// covers its first child (tile_parent, written by the scan), walks the offsets forward (coalesced), marks every
+// k_copy: a6 for theta = 0 (with sweeps to follow, the sweep kernel gathers each child's lattice from its parent's slot
+// through the child -> parent map that the scan then writes).  Child-centric gather.  Block t owns children
+// [t*CT, (t+1)*CT): it starts from the parent that covers its first child (tile_parent, written by the scan), walks the offsets forward (coalesced), marks every
 // parent at the position of its first child in shared memory and max-scans the marks into a child->parent map;
 // then VT = S/16 lanes copy one lattice with 128-bit loads/stores.  Children are in parent order, so parent
 // reads are monotone and repeated parents hit L1/L2.
@@ -586,31 +654,16 @@ template <> struct VecT<8> { using type = uint2; };
 
 template <int L>
 __global__ void __launch_bounds__(COPY_THREADS)
-k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tile_parent,
-       uint32_t* spins0, uint32_t* spins1, int32_t* E0, int32_t* E1, int32_t* M0, int32_t* M1, uint32_t* part0,
-       uint32_t* part1, uint32_t* part_stats, int P, const unsigned long long* __restrict__ tile_desc, int chunk,
-       int nchunks, unsigned tile_begin, unsigned tile_end_cap, uint32_t* __restrict__ parent_of) {
+k_copy(const DevState* __restrict__ st, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tile_parent,
+       uint32_t* spins0, uint32_t* spins1, int32_t* E0, int32_t* E1, int32_t* M0, int32_t* M1) {
   using CG = CopyGeo<L>;
   using V = typename VecT<CG::VB>::type;
+  grid_dependency_wait();
   if (st->status != ST_OK) return;
-  // Launch `chunk` of `nchunks` runs when the scan tiles [0, tile_end) are done (tile_end = min(tile_end_cap, all)):
-  // `hi` children have all their parents' offsets in memory, `lo` of them were already complete for the previous
-  // launch.  A copy tile belongs to the launch in which its END becomes complete; the last launch (every scan tile
-  // done, R' final) also takes the ragged last tile.
-  const unsigned long long R = st->R;
-  const unsigned ntiles = (unsigned)((R + SCAN_TILE - 1) / SCAN_TILE);
-  const unsigned b0 = tile_begin < ntiles ? tile_begin : ntiles, b1 = tile_end_cap < ntiles ? tile_end_cap : ntiles;
-  const bool last = (chunk == nchunks - 1);
-  const unsigned long long lo = b0 ? (tile_desc[b0 - 1] & DESC_VAL) : 0ull;
-  const unsigned long long hi = b1 ? (tile_desc[b1 - 1] & DESC_VAL) : 0ull;
-  const unsigned long long Rnew = last ? st->Rnew : hi;
-  const unsigned long long lim = (unsigned long long)b1 * SCAN_TILE < R ? (unsigned long long)b1 * SCAN_TILE : R;  // parents done
+  const unsigned long long R = st->R, Rnew = st->Rnew;
+  const unsigned long long lim = R;  // off[0 .. R] are all in memory
   const unsigned long long i0 = (unsigned long long)blockIdx.x * CG::CT;
-  const bool mine = (i0 + CG::CT > lo) && (last ? (i0 < Rnew) : (i0 + CG::CT <= hi));
-  if (!mine) {
-    if (last && blockIdx.x == 0) balance_tile(st, off, part0, part1, part_stats, P);  // a5 (see the end of the kernel)
-    return;
-  }
+  if (i0 >= Rnew) return;
   const unsigned cur = st->cur;  // source = buffer cur, destination = buffer cur^1 (never the same memory)
   const V* __restrict__ src = reinterpret_cast<const V*>(cur ? spins1 : spins0);
   V* __restrict__ dst = reinterpret_cast<V*>(cur ? spins0 : spins1);
@@ -631,7 +684,7 @@ k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restric
   for (unsigned long long jb = (unsigned long long)j_first + 1;; jb += COPY_THREADS) {
     const unsigned long long j = jb + threadIdx.x;
     bool past = true;
-    if (j < lim) {  // off[lim] is in memory too: every scan tile also writes the first offset of the next tile
+    if (j < lim) {  // off[0 .. R] are all in memory: the scan kernel has finished
       const uint32_t o = off[j], o1 = off[j + 1];
       past = (o >= i1);
       if (!past && o1 > o) s_par[o - i0] = (uint32_t)j;  // o >= i0 because j > j_first
@@ -668,11 +721,6 @@ k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restric
   }
   __syncthreads();
 
-  if (parent_of != nullptr) {
-    // gather-on-load mode (theta > 0): the sweep kernel reads every child's lattice straight from its parent's slot and
-    // recomputes E, M, so a6 shrinks to the child -> parent map (4 B per child instead of 2 S + 16)
-    for (unsigned c = threadIdx.x; c < nchild; c += COPY_THREADS) parent_of[i0 + c] = s_par[c];
-  } else {
   // E, M of the children
   for (unsigned c = threadIdx.x; c < nchild; c += COPY_THREADS) {
     const uint32_t pj = s_par[c];
@@ -681,7 +729,7 @@ k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restric
   }
   // lattices: VT threads per child, 4 children in flight per thread group
   constexpr int GROUPS = COPY_THREADS / (CG::VT < COPY_THREADS ? CG::VT : COPY_THREADS);
-  if constexpr (CG::VT <= COPY_THREADS) {
+  {
     const int sub = threadIdx.x % CG::VT, grp = threadIdx.x / CG::VT;
     constexpr int UNR = 4;
     unsigned c = grp;
@@ -693,12 +741,6 @@ k_copy(DevState* st, const uint32_t* __restrict__ off, const uint32_t* __restric
       for (int u = 0; u < UNR; ++u) dst[(i0 + c + u * GROUPS) * CG::VT + sub] = tmp[u];
     }
     for (; c < nchild; c += GROUPS) dst[(i0 + c) * CG::VT + sub] = src[(unsigned long long)s_par[c] * CG::VT + sub];
-  }
-  }
-  // a5: every offset is in memory once this kernel runs; block 0 writes the partition table and the diagnostics
-  if (last && blockIdx.x == 0) {
-    __syncthreads();
-    balance_tile(st, off, part0, part1, part_stats, P);
   }
 }
 

@@ -392,6 +392,7 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
         const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of) {
   using G_ = Geo<L>;
   static_assert(L >= 64, "k_sweep_small handles L < 64");
+  grid_dependency_wait();
   if (st->status != ST_OK) return;
   const unsigned buf = sa.mode != 1 ? (st->cur ^ 1u) : st->cur;
   const unsigned long long count = sa.mode != 1 ? st->Rnew : st->R;
@@ -523,6 +524,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
               const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of) {
   using G_ = SGeo<L>;
   static_assert(L == 8 || L == 16 || L == 32, "");
+  grid_dependency_wait();
   if (st->status != ST_OK) return;
   const unsigned buf = sa.mode != 1 ? (st->cur ^ 1u) : st->cur;
   const unsigned long long count = sa.mode != 1 ? st->Rnew : st->R;

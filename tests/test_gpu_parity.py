@@ -31,10 +31,10 @@ def rel(a, b):
     return abs(a - b) / max(abs(b), 1e-300)
 
 
-def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None, scan_chunks=0):
+def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None):
     b = _binding()
     gpu = b.PopulationAnnealer(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity,
-                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS, scan_chunks=scan_chunks)
+                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS)
     if spins is not None:
         gpu.set_spins(spins)
     ora = orc.OraclePA(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity, spins=spins)
@@ -464,19 +464,6 @@ def test_capacity_error_leaves_population_unchanged():
     assert g.beta_steps()[1] == 59 - failures
 
 
-@pytest.mark.parametrize("chunks", [2, 4, 8])
-def test_chunked_scan_with_overlapped_copy_lockstep(chunks):
-    """pa_config.scan_chunks > 1: the scan runs in several launches on the library's stream and the copy of chunk i
-    overlaps the scan of chunk i+1; every result must be what the single-launch path and the oracle give (ragged last
-    tile, copy tiles that straddle chunk boundaries, skewed counts)"""
-    L, R0, P = 32, 40000 + 137, 7
-    spins = inputs.structured_population(L, R0, seed=11)
-    gpu, ora = make_pair(L, R0, P, seed=21, spins=spins, scan_chunks=chunks)
-    lockstep(gpu, ora, [0.02, 0.05, 0.11], 1)
-    gpu2, ora2 = make_pair(16, 9000, 3, seed=5, scan_chunks=chunks)  # fewer tiles (5) than some chunk counts
-    lockstep(gpu2, ora2, [0.1, 0.2], 2)
-
-
 def test_extinction_matches_the_oracle_and_leaves_population_unchanged():
     """degenerate case R' = 0 (PA_EEXTINCT): R0 = 2 replicas die out with probability e^-2 per step; the first seed on
     which the ORACLE goes extinct must make the GPU fail at the same step, with nothing committed"""
@@ -541,12 +528,16 @@ def test_device_getters_and_launch_count():
     g.profile_read()  # drain the launches of pa_init
     l0 = g.launch_count()
     g.step(0.1, 2)
-    assert g.launch_count() - l0 == 6  # q_reduce, levels_tau, poisson_scan, copy (+ partition balance), sweep, observe
+    assert g.launch_count() - l0 == 4  # q_reduce (+ level tables), poisson_scan (+ child -> parent map), sweep (gathers), observe (+ a5)
     Ed, Md = g.energies_device()
     E, M = g.energies()
     assert np.array_equal(Ed.cpu().numpy(), E) and np.array_equal(Md.cpu().numpy(), M)
     prof = g.profile_read()
-    assert all(cnt == (0 if k in ("balance", "levels_w") else 1) for k, (_, cnt) in prof.items()) and prof["sweep"][0] > 0
+    assert all(cnt == (0 if k in ("balance", "levels_w", "levels_tau", "copy") else 1) for k, (_, cnt) in prof.items()) and prof["sweep"][0] > 0
+    g.profile_read()
+    g.step(0.2, 0)  # theta = 0: the gather copy runs instead of the sweep
+    prof = g.profile_read()
+    assert prof["copy"][1] == 1 and prof["sweep"][1] == 0 and g.launch_count() - l0 == 8
 
 
 def test_bench_line_carries_the_contract_keys():
@@ -563,7 +554,7 @@ def test_bench_line_carries_the_contract_keys():
                 "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"]:
         assert key in line, key
     assert line["metric"] == "spin_flip_attempts_per_s" and line["steps"] == 5 and line["n_gpus"] == 1
-    assert line["value"] > 0 and line["gpu_launches"] == 5 * 6 and line["data"] == "synthetic"
+    assert line["value"] > 0 and line["gpu_launches"] == 5 * 4 and line["data"] == "synthetic"
     assert line["config"]["workload"].startswith("config1") and line["vs_baseline"] is None
     assert set(["bound", "achieved", "peak", "unit", "frac", "traffic"]) <= set(line["roofline"])
     assert line["e2e"]["h2d_bytes_per_step"] > 0 and line["e2e"]["d2h_bytes_per_step"] > 0 and line["e2e"]["value"] > 0

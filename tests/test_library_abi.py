@@ -44,7 +44,7 @@ def test_workspace_query_and_invalid_configs_without_gpu():
     from paper_2006_00561_b200 import binding
     lib = binding.load_library()
     cfg = binding.PaConfig(L=64, P=148, R0=1 << 21, capacity=0, seed=3, beta0=0.0, workspace=None, workspace_bytes=0,
-                           stream=None, flags=0, scan_chunks=0)
+                           stream=None, flags=0, reserved=0)
     nbytes = lib.pa_workspace_bytes(C.byref(cfg))
     cap = (1 << 21) + 16 * 1449  # 16*ceil(sqrt(2^21))
     cap = (cap + 1023) // 1024 * 1024
@@ -53,7 +53,7 @@ def test_workspace_query_and_invalid_configs_without_gpu():
         kw = dict(L=64, P=1, R0=1024)
         kw.update(bad)
         c2 = binding.PaConfig(capacity=0, seed=0, beta0=0.0, workspace=None, workspace_bytes=0, stream=None, flags=0,
-                              scan_chunks=0, **kw)
+                              reserved=0, **kw)
         assert lib.pa_workspace_bytes(C.byref(c2)) == 0
 
 
@@ -67,7 +67,7 @@ def test_product_path_fails_loudly_without_cuda():
     # the C entry point itself refuses as well (no device -> PA_ECUDA, never a CPU computation)
     lib = binding.load_library()
     cfg = binding.PaConfig(L=8, P=1, R0=64, capacity=0, seed=0, beta0=0.0, workspace=256, workspace_bytes=1 << 30,
-                           stream=None, flags=0, scan_chunks=0)
+                           stream=None, flags=0, reserved=0)
     ctx = C.c_void_p()
     assert lib.pa_init(C.byref(cfg), C.byref(ctx)) == binding.PA_ECUDA
 
