@@ -349,6 +349,73 @@ int64_t orc_partition_stats(int64_t R, const uint32_t* n, const uint32_t* off, i
 }
 
 /* ------------------------------------------------------------------------------------------
+ * A6b.  Redistribution policies (readings G21-G23).  The children are in parent order;
+ * partition p's parents produced born_p of them (a contiguous range); a policy chooses how many, cnt_p, each
+ * partition holds afterwards (contiguous ranges again, sum cnt_p = R').
+ *   policy 0  "balanced": r_p = floor(R'/P) + (p < R' mod P)  -- orc_partition_table above (counts differ <= 1 replica).
+ *   policy 1  "main": replicas move in blocks of B; desired r_p as in policy 0; window W = maxexc * B.
+ *             Start from cnt_p = born_p.  While some partition lies outside the window (cnt_p - r_p > W or
+ *             r_p - cnt_p > W): move one block of B replicas from the partition with the largest excess cnt_p - r_p
+ *             to the one with the largest shortage r_p - cnt_p (ties: lowest index).
+ *   policy 2  "naive": every partition hands floor(born_p / 2) replicas -- a number proportional to its
+ *             offspring -- to a common pool, and the pool is dealt back evenly: partition p receives
+ *             floor(pool / P) + (p < pool mod P).
+ *   policy 3  "none": cnt_p = born_p, nothing moves.
+ * Returns the number of block moves made (policy 1), else 0.
+ * ---------------------------------------------------------------------------------------- */
+int64_t orc_policy_counts(int P, const uint32_t* born, int policy, uint32_t B, uint32_t maxexc, uint32_t* cnt) {
+  int64_t Rnew = 0;
+  for (int p = 0; p < P; ++p) Rnew += born[p];
+  int64_t base = Rnew / P, rem = Rnew % P;
+  if (policy == 0) {
+    for (int p = 0; p < P; ++p) cnt[p] = (uint32_t)(base + (p < rem ? 1 : 0));
+    return 0;
+  }
+  if (policy == 3) {
+    for (int p = 0; p < P; ++p) cnt[p] = born[p];
+    return 0;
+  }
+  if (policy == 2) {
+    int64_t pool = 0;
+    for (int p = 0; p < P; ++p) pool += born[p] / 2u;
+    int64_t share = pool / P, extra = pool % P;
+    for (int p = 0; p < P; ++p) cnt[p] = (uint32_t)((int64_t)born[p] - (int64_t)(born[p] / 2u) + share + (p < extra ? 1 : 0));
+    return 0;
+  }
+  /* policy 1 */
+  int64_t W = (int64_t)maxexc * (int64_t)B, moves = 0;
+  int64_t* c = (int64_t*)malloc((size_t)P * sizeof(int64_t));
+  for (int p = 0; p < P; ++p) c[p] = born[p];
+  for (;;) {
+    int hi = 0, lo = 0;
+    int64_t e_hi = 0, e_lo = 0;
+    for (int p = 0; p < P; ++p) {
+      int64_t r = base + (p < rem ? 1 : 0);
+      int64_t e = c[p] - r; /* excess (positive) or shortage (negative) */
+      if (p == 0 || e > e_hi) { e_hi = e; hi = p; }
+      if (p == 0 || e < e_lo) { e_lo = e; lo = p; }
+    }
+    if (e_hi <= W && -e_lo <= W) break; /* every partition inside the window */
+    c[hi] -= (int64_t)B;
+    c[lo] += (int64_t)B;
+    moves += 1;
+  }
+  for (int p = 0; p < P; ++p) cnt[p] = (uint32_t)c[p];
+  free(c);
+  return moves;
+}
+
+/* partition table from counts: start[0] = 0, start[p+1] = start[p] + cnt[p] */
+void orc_starts_from_counts(int P, const uint32_t* cnt, uint32_t* start /* P+1 */) {
+  uint64_t run = 0;
+  for (int p = 0; p < P; ++p) {
+    start[p] = (uint32_t)run;
+    run += cnt[p];
+  }
+  start[P] = (uint32_t)run;
+}
+
+/* ------------------------------------------------------------------------------------------
  * C4.  MCMC equilibration ("any traditional MCMC"; reading G7: checkerboard
  * Metropolis).  Thresholds T4/T8: floor(2^32 exp(-4 beta)), floor(2^32 exp(-8 beta)), clamped
  * to 2^32-1 (reading G10); accept iff dE <= 0 or u32 < T_dE (strict).

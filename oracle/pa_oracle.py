@@ -43,6 +43,8 @@ def lib():
             "orc_parent_of": (None, [C.c_int64, u32p, u32p, C.c_int64, u32p]),
             "orc_partition_table": (None, [C.c_int64, C.c_int, u32p]),
             "orc_partition_stats": (C.c_int64, [C.c_int64, u32p, u32p, C.c_int, u32p, u32p, u32p]),
+            "orc_policy_counts": (C.c_int64, [C.c_int, u32p, C.c_int, C.c_uint32, C.c_uint32, u32p]),
+            "orc_starts_from_counts": (None, [C.c_int, u32p, u32p]),
             "orc_thresholds": (None, [C.c_double, u32p, u32p]),
             "orc_sweeps": (None, [C.c_int, C.c_int64, C.c_int64, u32p, C.c_uint64, C.c_uint32, C.c_int,
                                   C.c_uint32, C.c_uint32]),
@@ -193,6 +195,25 @@ def partition_stats(n, off, P, old_start, new_start):
     return stats, moved
 
 
+POLICY_BALANCED, POLICY_MAIN, POLICY_NAIVE, POLICY_NONE = 0, 1, 2, 3
+
+
+def policy_counts(born, policy, block=1024, maxexc=1):
+    """cnt_p of every partition after redistribution under `policy` (A6b); also the number of block moves"""
+    born = _c(born, np.uint32)
+    cnt = np.zeros(born.shape[0], np.uint32)
+    moves = int(lib().orc_policy_counts(born.shape[0], _p(born, C.c_uint32), int(policy), int(block), int(maxexc),
+                                        _p(cnt, C.c_uint32)))
+    return cnt, moves
+
+
+def starts_from_counts(cnt):
+    cnt = _c(cnt, np.uint32)
+    start = np.zeros(cnt.shape[0] + 1, np.uint32)
+    lib().orc_starts_from_counts(cnt.shape[0], _p(cnt, C.c_uint32), _p(start, C.c_uint32))
+    return start
+
+
 def thresholds(beta):
     t4 = C.c_uint32(0)
     t8 = C.c_uint32(0)
@@ -263,9 +284,11 @@ class OraclePA:
     """State + step sequencing.  Notation follows the paper: R (current population R_beta_i), R0
     (R_beta_0), Q (eq. 3), tau (eq. 4), theta (MCMC sweeps per temperature)."""
 
-    def __init__(self, L, R0, P=1, seed=0, beta0=0.0, capacity=0, spins=None):
+    def __init__(self, L, R0, P=1, seed=0, beta0=0.0, capacity=0, spins=None, policy=POLICY_BALANCED, block=1024,
+                 maxexc=1):
         self.L, self.N, self.R0, self.P, self.seed = int(L), int(L) * int(L), int(R0), int(P), int(seed)
         self.capacity = int(capacity) if capacity else default_capacity(self.R0)
+        self.policy, self.block, self.maxexc = int(policy), int(block), int(maxexc)
         self.beta = float(beta0)
         self.step_no = 0
         # A1: initial population (PAPER.md:42); or a caller-supplied population (test hook)
@@ -302,7 +325,12 @@ class OraclePA:
             raise OracleError("capacity")
         if Rnew == 0:
             raise OracleError("extinct")
-        new_start = partition_table(Rnew, self.P)                    # A6
+        if self.policy == POLICY_BALANCED:
+            new_start = partition_table(Rnew, self.P)                # A6
+        else:                                                        # A6b: main / naive / none
+            born = np.diff(off[self.part_start].astype(np.int64)).astype(np.uint32)
+            cnt, _ = policy_counts(born, self.policy, self.block, self.maxexc)
+            new_start = starts_from_counts(cnt)
         stats, moved = partition_stats(n, off, self.P, self.part_start, new_start)
         spins, E, M = copy_population(self.L, n, off, self.spins, self.E, self.M, Rnew)
         self.last = {"Q": Q, "tau": tau, "n": n, "off": off, "Rnew": Rnew, "part_start": new_start,

@@ -332,6 +332,90 @@ def test_partition_table_and_stats_invariants(P):
 
 
 # ---------------------------------------------------------------------------------------------------
+# A6b redistribution policies (readings G21-G23)
+# ---------------------------------------------------------------------------------------------------
+def test_policy_none_and_balanced_and_naive_closed_forms():
+    rng = np.random.default_rng(5)
+    for P in [1, 2, 8, 148]:
+        born = rng.integers(0, 50000, P).astype(np.uint32)
+        Rn = int(born.sum())
+        cnt, _ = orc.policy_counts(born, orc.POLICY_NONE)
+        assert np.array_equal(cnt, born)                      # nothing moves
+        cnt, _ = orc.policy_counts(born, orc.POLICY_BALANCED)
+        assert np.array_equal(cnt, np.diff(orc.partition_table(Rn, P).astype(np.int64)))
+        cnt, _ = orc.policy_counts(born, orc.POLICY_NAIVE)
+        assert int(cnt.sum()) == Rn
+        pool = int((born // 2).sum())
+        want = born.astype(np.int64) - born // 2 + pool // P + (np.arange(P) < pool % P)
+        assert np.array_equal(cnt, want)
+        # the excess over the mean halves (up to rounding): "relaxes fast to the flat behaviour"
+        e0, e1 = born.astype(np.float64) - Rn / P, cnt.astype(np.float64) - Rn / P
+        assert np.all(np.abs(e1 - e0 / 2) <= 1.0)
+
+
+def test_policy_main_by_hand():
+    # P = 3, B = 10, maxexc = 1 (window 10), R' = 90, r = (30, 30, 30)
+    cnt, moves = orc.policy_counts([30, 35, 25], orc.POLICY_MAIN, 10, 1)
+    assert cnt.tolist() == [30, 35, 25] and moves == 0          # everyone inside the window: nothing moves
+    cnt, moves = orc.policy_counts([60, 20, 10], orc.POLICY_MAIN, 10, 1)
+    # excess (30,-10,-20): 0->2 (50,20,20) e=(20,-10,-10); 0->1 [tie: lowest index] (40,30,20) e=(10,0,-10): stop
+    assert cnt.tolist() == [40, 30, 20] and moves == 2
+    cnt, moves = orc.policy_counts([60, 20, 10], orc.POLICY_MAIN, 10, 2)
+    # window 20: (30,-10,-20): 0->2 gives (50,20,20) e=(20,-10,-10): stop after one move
+    assert cnt.tolist() == [50, 20, 20] and moves == 1
+    cnt, moves = orc.policy_counts([0, 0, 91], orc.POLICY_MAIN, 10, 1)
+    # r = (31,30,30): e=(-31,-30,61): 2->0 (10,0,81) e=(-21,-30,51); 2->1 (10,10,71) e=(-21,-20,41); 2->0 (20,10,61)
+    # e=(-11,-20,31); 2->1 (20,20,51) e=(-11,-10,21); 2->0 (30,20,41) e=(-1,-10,11); 2->1 (30,30,31) e=(-1,0,1): stop
+    assert cnt.tolist() == [30, 30, 31] and moves == 6
+    # block size 1, window 1: stops as soon as every |cnt - r| <= 1
+    cnt, moves = orc.policy_counts([5, 1, 0], orc.POLICY_MAIN, 1, 1)
+    assert cnt.tolist() == [3, 2, 1] and moves == 2  # r=(2,2,2), e=(3,-1,-2): 0->2, (4,1,1) e=(2,-1,-1): 0->1, (3,2,1) e=(1,0,-1): stop
+
+
+@pytest.mark.parametrize("P,B,maxexc", [(8, 1024, 1), (8, 1024, 2), (148, 1024, 1), (5, 1, 1), (16, 256, 3)])
+def test_policy_main_invariants(P, B, maxexc):
+    rng = np.random.default_rng(P * 7 + maxexc)
+    for trial in range(30):
+        scale = rng.choice([2000, 20480, 90000])
+        born = (rng.gamma(2.0, scale / 2.0, P)).astype(np.uint32)
+        Rn = int(born.sum())
+        cnt, moves = orc.policy_counts(born, orc.POLICY_MAIN, B, maxexc)
+        r = np.diff(orc.partition_table(Rn, P).astype(np.int64))
+        c = cnt.astype(np.int64)
+        assert int(c.sum()) == Rn and np.all(c >= 0)
+        assert np.all(np.abs(c - r) <= maxexc * B)                     # everyone inside the window
+        assert np.all((c - born.astype(np.int64)) % B == 0)            # replicas move in whole blocks
+        inside = np.all(np.abs(born.astype(np.int64) - r) <= maxexc * B)
+        assert (moves == 0) == bool(inside)                            # untouched iff already inside the window
+        maxg, minl = np.maximum(c - r, 0), np.maximum(r - c, 0)
+        assert maxg.sum() == minl.sum()
+        assert np.array_equal(orc.starts_from_counts(cnt), np.concatenate([[0], np.cumsum(c)]).astype(np.uint32))
+
+
+def test_policies_inside_the_pa_loop():
+    # the policy only re-draws partition boundaries: populations, Q, counts are those of the default policy; the paper's
+    # diagnostics follow their definitions
+    ref = orc.OraclePA(8, 4096, P=8, seed=21)
+    runs = {pol: orc.OraclePA(8, 4096, P=8, seed=21, policy=pol, block=64, maxexc=1)
+            for pol in (orc.POLICY_MAIN, orc.POLICY_NAIVE, orc.POLICY_NONE)}
+    for k in range(1, 13):
+        ir = ref.step(0.04 * k, 1)
+        for pol, pa in runs.items():
+            info = pa.step(0.04 * k, 1)
+            assert np.array_equal(pa.spins, ref.spins) and info["Q"] == ir["Q"] and np.array_equal(info["n"], ir["n"])
+            st = info["part_stats"].astype(np.int64)
+            cnt, born, maxg, minl = st[:, 0], st[:, 1], st[:, 2], st[:, 3]
+            assert cnt.sum() == born.sum() == pa.R and maxg.sum() == minl.sum()
+            assert np.array_equal(np.maximum(born - cnt, 0), maxg) and np.array_equal(np.maximum(cnt - born, 0), minl)
+            assert np.array_equal(np.diff(info["part_start"].astype(np.int64)), cnt)
+            if pol == orc.POLICY_NONE:
+                assert np.array_equal(cnt, born) and info["moved"] == 0
+            if pol == orc.POLICY_MAIN:
+                r = np.diff(orc.partition_table(pa.R, 8).astype(np.int64))
+                assert np.all(np.abs(cnt - r) <= 64)
+
+
+# ---------------------------------------------------------------------------------------------------
 # C4 Metropolis
 # ---------------------------------------------------------------------------------------------------
 def test_thresholds():
