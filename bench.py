@@ -275,6 +275,45 @@ def anneal_leg(binding, torch, configs):
     return out
 
 
+def policies_leg(binding, torch, out_csv=None):
+    """SURVEY.md 8(f)-2 / PAPER.md:94-118 (Fig. 1-2): the paper's 8-GPU task with the 8 GPUs as 8 logical partitions of
+    one device, under the redistribution policies none / naive / main (blocks of 1024, maxexc 1 and 2) / balanced.
+    The population, Q and copy counts are the same under every policy (the policy only draws the partition
+    boundaries), so one seed gives directly comparable traces.  Per step: replicas per partition after
+    redistribution.  'relative_makespan' = sum over steps of the largest partition / sum of the mean partition: the
+    time a synchronous multi-GPU run would take relative to perfect balance (the paper: naive runs 1.45x longer than
+    main)."""
+    wl = inputs.PAPER_TASK
+    runs = [("none", binding.PA_POLICY_NONE, 1024, 1), ("naive", binding.PA_POLICY_NAIVE, 1024, 1),
+            ("main_maxexc1", binding.PA_POLICY_MAIN, 1024, 1), ("main_maxexc2", binding.PA_POLICY_MAIN, 1024, 2),
+            ("balanced", binding.PA_POLICY_BALANCED, 1024, 1)]
+    rows, summary = [], {}
+    for name, pol, block, maxexc in runs:
+        pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0, policy=pol, block=block,
+                                        maxexc=maxexc)
+        mx, mean, moved_total = [], [], 0
+        for k in range(1, wl.K + 1):
+            pa.step(wl.beta(k), wl.theta)
+            _, st, moved = pa.partitions()
+            cnt = [int(x) for x in st[:, 0]]
+            rows.append([name, k, "%.3f" % wl.beta(k), pa.R, moved] + cnt)
+            mx.append(max(cnt))
+            mean.append(pa.R / wl.P)
+            moved_total += moved
+        peak = max(range(wl.K), key=lambda i: mx[i])
+        summary[name] = {"max_partition": mx[peak], "at_step": peak + 1, "max_over_desired": mx[peak] / mean[peak],
+                         "relative_makespan": sum(mx) / sum(mean), "replicas_moved_per_step": moved_total / wl.K,
+                         "lnZ": pa.log_Z()["lnZ"], "block": block, "maxexc": maxexc}
+        del pa
+    if out_csv:
+        with open(out_csv, "w") as f:
+            f.write("policy,step,beta,R,moved," + ",".join("cnt%d" % p for p in range(wl.P)) + "\n")
+            for r in rows:
+                f.write(",".join(str(x) for x in r) + "\n")
+    summary["naive_over_main_makespan"] = summary["naive"]["relative_makespan"] / summary["main_maxexc1"]["relative_makespan"]
+    return {"workload": wl.name, "L": wl.L, "R0": wl.R0, "K": wl.K, "theta": wl.theta, "P": wl.P, "policies": summary}
+
+
 def run_ours(args):
     import torch
     from paper_2006_00561_b200 import binding, dist
@@ -394,11 +433,13 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-resample", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--leg", default="all", choices=["all", "resample", "anneal"],
+    ap.add_argument("--leg", default="all", choices=["all", "resample", "anneal", "policies"],
                     help="'resample': only the config-5 resampling/redistribution leg (short; used for ncu captures); "
-                         "'anneal': whole anneals of --anneal-configs (wall time, ln Z against the exact value)")
+                         "'anneal': whole anneals of --anneal-configs (wall time, ln Z against the exact value); "
+                         "'policies': the paper's 8-GPU task under the redistribution policies none / naive / main")
     ap.add_argument("--anneal-configs", default="1,2,3,4")
     ap.add_argument("--resample-repeats", type=int, default=5)
+    ap.add_argument("--trace-csv", default=None, help="--leg policies: write the per-step partition counts to this file")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3  # timing rule: at least 3 warm-up steps
@@ -410,6 +451,13 @@ def main():
         if not torch.cuda.is_available():
             raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
         print(json.dumps({"anneal": anneal_leg(binding, torch, [int(x) for x in args.anneal_configs.split(",")])}))
+        return 0
+    if args.leg == "policies":
+        import torch
+        from paper_2006_00561_b200 import binding
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+        print(json.dumps({"policies": policies_leg(binding, torch, args.trace_csv)}))
         return 0
     if args.leg == "resample":
         import torch

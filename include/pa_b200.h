@@ -53,9 +53,21 @@ enum {
   PA_PROFILE_SPAN = 8u /* record only the PA_K_RESAMPLE_SPAN pair around a1-a6 of every step */
 };
 
+/* Redistribution policies (A6b, readings G21-G23).  The children are in parent order and a
+ * partition is a contiguous range of them; a policy decides the counts cnt_p.  It changes the partition table and the
+ * diagnostics only -- population, weights and copy counts do not depend on it. */
+enum {
+  PA_POLICY_BALANCED = 0, /* cnt_p = floor(R'/P) + (p < R' mod P): counts differ by <= 1 replica */
+  PA_POLICY_MAIN = 1,     /* the paper's main algorithm: blocks of `block` replicas move from the largest excess to the
+                             largest shortage until every partition is within `maxexc` blocks of its balanced count */
+  PA_POLICY_NAIVE = 2,    /* the paper's naive algorithm: every partition pools floor(born_p / 2) replicas -- a number
+                             proportional to its offspring -- and the pool is dealt back evenly */
+  PA_POLICY_NONE = 3      /* no redistribution: cnt_p = born_p */
+};
+
 typedef struct {
   int32_t L;        /* lattice side: 8, 16, 32, 64 or 128 */
-  int32_t P;        /* logical partitions, >= 1 (148 = one per B200 SM) */
+  int32_t P;        /* logical partitions, >= 1 (148 = one per B200 SM); <= 1024 unless policy = PA_POLICY_BALANCED */
   int64_t R0;       /* initial = target population R_beta0, 1 <= R0 < 2^31 */
   int64_t capacity; /* slots per population buffer; 0 => R0 + max(1024, 16*ceil(sqrt(R0))) rounded up to 1024 */
   uint64_t seed;    /* Philox key */
@@ -64,7 +76,9 @@ typedef struct {
   uint64_t workspace_bytes;
   void* stream;     /* cudaStream_t, caller owned (NULL = legacy default stream) */
   uint32_t flags;   /* PA_KEEP_TAU | PA_KEEP_COUNTS | PA_PROFILE | PA_PROFILE_SPAN */
-  uint32_t reserved; /* must be 0 */
+  uint32_t policy;  /* PA_POLICY_*: how the new population is divided over the P partitions (default 0 = balanced) */
+  uint32_t block;   /* PA_POLICY_MAIN: replicas per block (0 => 1024) */
+  uint32_t maxexc;  /* PA_POLICY_MAIN: window in blocks (0 => 1) */
 } pa_config;
 
 /* population sums after the last committed step (or after pa_init / pa_set_spins); 128-bit integers as {lo, hi} */
@@ -80,7 +94,7 @@ typedef struct {
 
 /* per-partition diagnostics of the last step, in the paper's vocabulary */
 typedef struct {
-  uint32_t cnt;  /* replicas the partition holds after redistribution ("desired" r_n; counts differ by <= 1) */
+  uint32_t cnt;  /* replicas the partition holds after redistribution */
   uint32_t born; /* offspring of the parents that lived in this partition (what it would hold without redistribution) */
   uint32_t maxg; /* excess   max(0, born - cnt) */
   uint32_t minl; /* shortage max(0, cnt - born) */

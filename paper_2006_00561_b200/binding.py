@@ -13,6 +13,7 @@ LIB_PATH = os.path.join(HERE, "libpa_b200.so")
 
 PA_OK, PA_EINVAL, PA_ENOMEM, PA_ECAPACITY, PA_EEXTINCT, PA_ECUDA = 0, -1, -2, -3, -4, -5
 PA_KEEP_TAU, PA_KEEP_COUNTS, PA_PROFILE, PA_PROFILE_SPAN = 1, 2, 4, 8
+PA_POLICY_BALANCED, PA_POLICY_MAIN, PA_POLICY_NAIVE, PA_POLICY_NONE = 0, 1, 2, 3
 KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "copy", "sweep", "observe", "resample_span"]
 
 EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
@@ -23,7 +24,8 @@ EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_population"
 class PaConfig(C.Structure):
     _fields_ = [("L", C.c_int32), ("P", C.c_int32), ("R0", C.c_int64), ("capacity", C.c_int64), ("seed", C.c_uint64),
                 ("beta0", C.c_double), ("workspace", C.c_void_p), ("workspace_bytes", C.c_uint64),
-                ("stream", C.c_void_p), ("flags", C.c_uint32), ("reserved", C.c_uint32)]
+                ("stream", C.c_void_p), ("flags", C.c_uint32), ("policy", C.c_uint32), ("block", C.c_uint32),
+                ("maxexc", C.c_uint32)]
 
 
 class PaObs(C.Structure):
@@ -91,7 +93,8 @@ def _np_ptr(a):
 class PopulationAnnealer:
     """One PA context on the current CUDA device.  Method names mirror the C ABI (pa_*)."""
 
-    def __init__(self, L, R0, P=1, seed=0, beta0=0.0, capacity=0, flags=0, device=None, stream=None):
+    def __init__(self, L, R0, P=1, seed=0, beta0=0.0, capacity=0, flags=0, device=None, stream=None,
+                 policy=PA_POLICY_BALANCED, block=0, maxexc=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2006_00561_b200 needs a CUDA device (no CPU fallback)")
@@ -103,7 +106,7 @@ class PopulationAnnealer:
         self.L, self.N, self.P, self.R0, self.seed = int(L), int(L) * int(L), int(P), int(R0), int(seed)
         self.wpr = self.N // 32
         cfg = PaConfig(L=L, P=P, R0=R0, capacity=capacity, seed=seed, beta0=beta0, workspace=None, workspace_bytes=0,
-                       stream=self.stream.cuda_stream, flags=flags, reserved=0)
+                       stream=self.stream.cuda_stream, flags=flags, policy=policy, block=block, maxexc=maxexc)
         nbytes = self._lib.pa_workspace_bytes(C.byref(cfg))
         if nbytes == 0:
             raise PaError(PA_EINVAL, "invalid configuration")

@@ -63,6 +63,7 @@ int64_t default_capacity(int64_t R0) {
 bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   if (!c || !valid_L(c->L) || c->P < 1 || c->R0 < 1 || c->R0 >= (1ll << 31) || cap < c->R0 || cap >= (1ll << 32) - 4096)
     return false;
+  if (c->policy > PA_POLICY_NONE || (c->policy != PA_POLICY_BALANCED && c->P > BAL_PMAX)) return false;
   const uint64_t N = (uint64_t)c->L * c->L, S = N / 8, nlev = N + 1, ucap = (uint64_t)cap;
   uint64_t o = 0;
   auto take = [&](uint64_t bytes) {
@@ -262,7 +263,8 @@ void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
   launch(c, "k_observe", k_observe, OBS_GRID, OBS_THREADS, c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.E[0]),
          c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]), c->dev<int32_t>(c->lo.M[1]),
          c->dev<unsigned long long>(c->lo.obs_partial), mode, c->N, c->dev<uint32_t>(c->lo.off),
-         c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]), c->dev<uint32_t>(c->lo.part_stats), c->cfg.P);
+         c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]), c->dev<uint32_t>(c->lo.part_stats),
+         BalanceArgs{c->cfg.P, (int)c->cfg.policy, c->cfg.block ? c->cfg.block : 1024u, c->cfg.maxexc ? c->cfg.maxexc : 1u});
 }
 
 // all kernels of one temperature step, parameters in device slot sp:
@@ -440,7 +442,7 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   if (!c) return PA_ENOMEM;
   c->cfg = *cfg;
   c->cap = cfg->capacity > 0 ? cfg->capacity : (cfg->R0 >= 1 ? default_capacity(cfg->R0) : 0);
-  if (!make_layout(cfg, c->cap, &c->lo) || !(cfg->beta0 == cfg->beta0) || cfg->reserved != 0u) {
+  if (!make_layout(cfg, c->cap, &c->lo) || !(cfg->beta0 == cfg->beta0)) {
     delete c;
     return PA_EINVAL;
   }

@@ -45,25 +45,89 @@ __device__ __forceinline__ U128 warp_sum_u128(U128 v) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// balance_tile: a5.  One block (the last block of k_observe: every offset of the step is in memory).
-// New partition table, born/excess/shortage per partition, moved count.  PAPER.md:104-106; A6.
+// balance_tile: a5.  One block (the last block of k_observe: every offset of the step is in memory).  New partition
+// table, born/excess/shortage per partition, moved count.  PAPER.md:84-118; A6, A6b (readings G21-G23).
+//   policy 0  balanced: cnt_p = floor(R'/P) + (p < R' mod P)           (any P)
+//   policy 1  main:     blocks of B replicas move from the largest excess to the largest shortage until every partition
+//                       is within maxexc blocks of its balanced count
+//   policy 2  naive:    every partition pools floor(born_p / 2), the pool is dealt back evenly
+//   policy 3  none:     cnt_p = born_p
+// Policies 1-3 keep the partition counts in shared memory (P <= BAL_PMAX).
 // ---------------------------------------------------------------------------------------------------
+constexpr int BAL_PMAX = 1024;
+
+struct BalanceArgs {
+  int P, policy;
+  unsigned B, maxexc;
+};
+
 __device__ void balance_tile(DevState* st, const uint32_t* off, uint32_t* part0, uint32_t* part1, uint32_t* stats,
-                             int P) {
+                             const BalanceArgs ba) {
   if (*((volatile unsigned*)&st->status) != ST_OK) return;
+  const int P = ba.P;
   const uint32_t* old_start = st->cur ? part1 : part0;
   uint32_t* new_start = st->cur ? part0 : part1;
   const unsigned long long Rnew = *((volatile unsigned long long*)&st->Rnew);
   const unsigned long long base = Rnew / P, rem = Rnew % P;
   __shared__ unsigned long long s_same;
+  __shared__ long long s_c[BAL_PMAX];        // counts of policies 1-3
+  __shared__ uint32_t s_start[BAL_PMAX + 1];
   if (threadIdx.x == 0) s_same = 0ull;
+  if (ba.policy != 0) {
+    for (int p = threadIdx.x; p < P; p += blockDim.x)
+      s_c[p] = (long long)__ldcg(off + old_start[p + 1]) - (long long)__ldcg(off + old_start[p]);  // born_p
+    __syncthreads();
+    if (ba.policy == 2 && threadIdx.x == 0) {
+      long long pool = 0;
+      for (int p = 0; p < P; ++p) pool += s_c[p] / 2;
+      const long long share = pool / P, extra = pool % P;
+      for (int p = 0; p < P; ++p) s_c[p] = s_c[p] - s_c[p] / 2 + share + (p < extra ? 1 : 0);
+    }
+    if (ba.policy == 1 && threadIdx.x < 32) {  // warp 0: one block move per iteration
+      const long long W = (long long)ba.maxexc * (long long)ba.B;
+      const int lane = threadIdx.x;
+      for (;;) {
+        long long e_hi = 0, e_lo = 0;
+        int hi = -1, lo = -1;
+        for (int p = lane; p < P; p += 32) {  // ascending p: strict comparisons keep the lowest index on ties
+          const long long e = s_c[p] - (long long)(base + ((unsigned long long)p < rem ? 1ull : 0ull));
+          if (hi < 0 || e > e_hi) { e_hi = e; hi = p; }
+          if (lo < 0 || e < e_lo) { e_lo = e; lo = p; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          const long long oe_hi = __shfl_xor_sync(0xffffffffu, e_hi, o), oe_lo = __shfl_xor_sync(0xffffffffu, e_lo, o);
+          const int ohi = __shfl_xor_sync(0xffffffffu, hi, o), olo = __shfl_xor_sync(0xffffffffu, lo, o);
+          if (ohi >= 0 && (hi < 0 || oe_hi > e_hi || (oe_hi == e_hi && ohi < hi))) { e_hi = oe_hi; hi = ohi; }
+          if (olo >= 0 && (lo < 0 || oe_lo < e_lo || (oe_lo == e_lo && olo < lo))) { e_lo = oe_lo; lo = olo; }
+        }
+        if (e_hi <= W && -e_lo <= W) break;  // every partition inside the window
+        if (lane == 0) {
+          s_c[hi] -= (long long)ba.B;
+          s_c[lo] += (long long)ba.B;
+        }
+        __syncwarp();
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      unsigned long long run = 0;
+      for (int p = 0; p < P; ++p) {
+        s_start[p] = (uint32_t)run;
+        run += (unsigned long long)s_c[p];
+      }
+      s_start[P] = (uint32_t)run;
+    }
+  }
   __syncthreads();
   unsigned long long same = 0;
   for (int p = threadIdx.x; p <= P; p += blockDim.x) {
-    const unsigned long long s = (unsigned long long)p * base + ((unsigned long long)p < rem ? p : rem);
+    const unsigned long long s =
+        ba.policy != 0 ? s_start[p] : (unsigned long long)p * base + ((unsigned long long)p < rem ? p : rem);
     new_start[p] = (uint32_t)s;
     if (p < P) {
-      const unsigned long long e = (unsigned long long)(p + 1) * base + ((unsigned long long)(p + 1) < rem ? p + 1 : rem);
+      const unsigned long long e = ba.policy != 0 ? s_start[p + 1]
+                                                  : (unsigned long long)(p + 1) * base + ((unsigned long long)(p + 1) < rem ? p + 1 : rem);
       const uint32_t cnt = (uint32_t)(e - s);
       const uint32_t b0 = __ldcg(off + old_start[p]), b1 = __ldcg(off + old_start[p + 1]);
       const uint32_t born = b1 - b0;
@@ -90,7 +154,7 @@ __global__ void __launch_bounds__(OBS_THREADS)
 k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
           const int32_t* __restrict__ E1, const int32_t* __restrict__ M0, const int32_t* __restrict__ M1,
           unsigned long long* __restrict__ partial /* [grid][12] */, const int mode, const int N,
-          const uint32_t* __restrict__ off, uint32_t* part0, uint32_t* part1, uint32_t* part_stats, const int P) {
+          const uint32_t* __restrict__ off, uint32_t* part0, uint32_t* part1, uint32_t* part_stats, const BalanceArgs ba) {
   grid_dependency_wait();
   if (st->status != ST_OK) return;
   const unsigned buf = mode == 0 ? (st->cur ^ 1u) : st->cur;
@@ -210,7 +274,7 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   }
   __syncthreads();
   if (mode == 0) {  // a5: partition table of the new population + the paper's diagnostics, before the commit flips `cur`
-    balance_tile(st, off, part0, part1, part_stats, P);
+    balance_tile(st, off, part0, part1, part_stats, ba);
     __syncthreads();
   }
   if (threadIdx.x == 0) {

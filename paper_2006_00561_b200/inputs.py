@@ -54,6 +54,10 @@ CONFIGS = {
     5: Workload("config5_resample_L32_R16M", 32, 1 << 24, 1, 0.40, 0.45, 0, 148, 5),
 }
 
+# the paper's own scalability task on 8 GPUs: L = 64, beta 0 -> 1 in K = 200 steps, 20 480 replicas
+# per GPU, theta = 1; here the 8 GPUs are 8 logical partitions of one device (Fig. 1-2 shapes)
+PAPER_TASK = Workload("paper_task_L64_8x20480", 64, 8 * 20480, 200, 0.0, 1.0, 1, 8, 6)
+
 
 def random_packed_population(L, R, seed, p_up=0.5):
     """generic random bit lattices (R, N/32) uint32 for tests of set_spins / energy kernels; NOT the method's

@@ -31,13 +31,14 @@ def rel(a, b):
     return abs(a - b) / max(abs(b), 1e-300)
 
 
-def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None):
+def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None, policy=0, block=1024, maxexc=1):
     b = _binding()
     gpu = b.PopulationAnnealer(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity,
-                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS)
+                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS, policy=policy, block=block, maxexc=maxexc)
     if spins is not None:
         gpu.set_spins(spins)
-    ora = orc.OraclePA(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity, spins=spins)
+    ora = orc.OraclePA(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity, spins=spins, policy=policy, block=block,
+                       maxexc=maxexc)
     return gpu, ora
 
 
@@ -410,6 +411,34 @@ def test_failed_step_does_not_leak_into_the_getters():
             pass
     n, off = g.counts()
     assert int(n.sum()) == g.R == int(off[-1])
+
+
+# ---------------------------------------------------------------------------------------------------
+# redistribution policies: partition tables, born / excess / shortage, moved
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("policy,P,block,maxexc", [(1, 8, 1024, 1), (1, 8, 1024, 2), (1, 148, 64, 1), (1, 5, 1, 1),
+                                                   (2, 8, 1024, 1), (2, 148, 1024, 1), (3, 8, 1024, 1), (3, 37, 1024, 1)])
+def test_policies_lockstep(policy, P, block, maxexc):
+    """lockstep() compares part_start, cnt/born/maxg/minl and `moved` with the oracle every step; the populations of the
+    partitions drift apart under `none` and `naive`, which is what the paper's Fig. 1 shows"""
+    gpu, ora = make_pair(64, 8 * 2048 + 77, P, seed=31 + policy, policy=policy, block=block, maxexc=maxexc)
+    lockstep(gpu, ora, [0.06 * k for k in range(1, 9)], 1)   # up to beta = 0.48, across beta_c
+    ps, st, moved = gpu.partitions()
+    if policy == 3:
+        assert moved == 0 and np.array_equal(st[:, 0], st[:, 1])
+        assert st[:, 0].max() > 1.2 * st[:, 0].mean()  # partitions have drifted apart
+    if policy == 1:
+        r = np.diff(orc.partition_table(gpu.R, P).astype(np.int64))
+        assert np.all(np.abs(st[:, 0].astype(np.int64) - r) <= maxexc * block)
+
+
+def test_policy_arguments_are_validated():
+    b = _binding()
+    with pytest.raises(b.PaError):
+        b.PopulationAnnealer(8, 64, P=4, policy=7)
+    with pytest.raises(b.PaError):
+        b.PopulationAnnealer(8, 5000, P=2000, policy=b.PA_POLICY_MAIN)  # P <= 1024 for the paper's policies
+    b.PopulationAnnealer(8, 5000, P=2000)  # the balanced table has no such limit
 
 
 # ---------------------------------------------------------------------------------------------------

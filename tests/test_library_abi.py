@@ -35,16 +35,16 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
 
 def test_struct_layouts_match_the_header():
     from paper_2006_00561_b200 import binding
-    assert C.sizeof(binding.PaConfig) == 4 + 4 + 8 + 8 + 8 + 8 + 8 + 8 + 8 + 4 + 4
+    assert C.sizeof(binding.PaConfig) == 4 + 4 + 8 + 8 + 8 + 8 + 8 + 8 + 8 + 4 + 4 + 4 + 4
     assert C.sizeof(binding.PaObs) == 8 + 8 + 4 * 16 + 5 * 8
-    assert binding.PaConfig.workspace.offset == 40 and binding.PaConfig.flags.offset == 64
+    assert binding.PaConfig.workspace.offset == 40 and binding.PaConfig.flags.offset == 64 and binding.PaConfig.maxexc.offset == 76
 
 
 def test_workspace_query_and_invalid_configs_without_gpu():
     from paper_2006_00561_b200 import binding
     lib = binding.load_library()
     cfg = binding.PaConfig(L=64, P=148, R0=1 << 21, capacity=0, seed=3, beta0=0.0, workspace=None, workspace_bytes=0,
-                           stream=None, flags=0, reserved=0)
+                           stream=None, flags=0, policy=0, block=0, maxexc=0)
     nbytes = lib.pa_workspace_bytes(C.byref(cfg))
     cap = (1 << 21) + 16 * 1449  # 16*ceil(sqrt(2^21))
     cap = (cap + 1023) // 1024 * 1024
@@ -53,7 +53,7 @@ def test_workspace_query_and_invalid_configs_without_gpu():
         kw = dict(L=64, P=1, R0=1024)
         kw.update(bad)
         c2 = binding.PaConfig(capacity=0, seed=0, beta0=0.0, workspace=None, workspace_bytes=0, stream=None, flags=0,
-                              reserved=0, **kw)
+                              policy=0, block=0, maxexc=0, **kw)
         assert lib.pa_workspace_bytes(C.byref(c2)) == 0
 
 
@@ -67,7 +67,7 @@ def test_product_path_fails_loudly_without_cuda():
     # the C entry point itself refuses as well (no device -> PA_ECUDA, never a CPU computation)
     lib = binding.load_library()
     cfg = binding.PaConfig(L=8, P=1, R0=64, capacity=0, seed=0, beta0=0.0, workspace=256, workspace_bytes=1 << 30,
-                           stream=None, flags=0, reserved=0)
+                           stream=None, flags=0, policy=0, block=0, maxexc=0)
     ctx = C.c_void_p()
     assert lib.pa_init(C.byref(cfg), C.byref(ctx)) == binding.PA_ECUDA
 
