@@ -173,6 +173,53 @@ int pa_debug_set_thresholds(pa_ctx* ctx, int enable, uint32_t T4, uint32_t T8);
  * beta, step counter and ln Z are kept */
 int pa_set_spins(pa_ctx* ctx, const uint32_t* src, int64_t R, int src_on_device);
 
+/* ---- multi-GPU: partitioned redistribution, one rank = one partition -------- */
+/* The population is sharded over `world` ranks in global slot order: rank r owns the contiguous global slots
+ * [start_r, start_{r+1}).  Every random number is keyed by the GLOBAL replica index, so the ranks together compute
+ * exactly what one context with the whole population computes (up to the rounding of Q: the ranks' weight sums are
+ * added in rank order).  A step is four calls with three small exchanges in between, which the CALLER performs (NCCL
+ * through torch.distributed in paper_2006_00561_b200/dist.py; plain copies when the ranks are emulated on one device):
+ *
+ *   pa_dist_begin     local sum of weights                                  -> all-gather of pa_dist_partial
+ *   pa_dist_resample  Q over all ranks, local Poisson counts + scan, the local offspring expanded in child order
+ *                                                                           -> all-gather of the offspring totals T_r
+ *   pa_dist_exchange_plan  (pure host function) global child offsets, new partition table under cfg.policy with
+ *                     born_p = T_p (the paper's per-node offspring count), and the slice every rank sends to every other
+ *                                                                           -> all-to-all-v of lattices (contiguous slices)
+ *   pa_dist_finish    theta sweeps of the new local population in place, E, M, local sums, commit
+ *
+ * Because global child order is source-rank order, the slices a rank receives are contiguous in its new buffer in source
+ * order: the all-to-all-v writes straight into the population buffer (pa_dist_buffers), nothing is unpacked. */
+typedef struct {
+  double sumw; /* sum over the rank's replicas of exp[-(beta'-beta) E_j] */
+  int64_t R;   /* the rank's current population */
+} pa_dist_partial;
+
+/* cfg.R0 = GLOBAL target population; cfg.capacity = slots per buffer of THIS rank (0 => twice the balanced share + 4096,
+ * rounded up to 1024); cfg.P is ignored (partition = rank; <= 1024 ranks unless policy = balanced); cfg.policy / block /
+ * maxexc govern the rank-level plan.  Creates the rank's share of the initial population (global balanced table). */
+int pa_dist_init(const pa_config* cfg, int32_t rank, int32_t world, pa_ctx** out);
+/* bytes of device workspace a rank needs for cfg (as given to pa_dist_init) */
+uint64_t pa_dist_workspace_bytes(const pa_config* cfg, int32_t world);
+int pa_dist_begin(pa_ctx* ctx, double beta_next, int32_t theta, pa_dist_partial* mine);
+/* all: `world` entries in rank order (HOST).  *offspring = T_rank, or -1 if the rank's offspring exceed its capacity. */
+int pa_dist_resample(pa_ctx* ctx, const pa_dist_partial* all, int64_t* offspring);
+/* Pure host function, no CUDA: T = offspring totals in rank order; new_start[world+1] = global child index where each
+ * rank's new range starts; base[world+1] = global child index where each rank's offspring start;
+ * counts[src * world + dst] = children rank src sends to rank dst (its own share included).  PA_EEXTINCT if sum T = 0. */
+int pa_dist_exchange_plan(int32_t world, const int64_t* T, int32_t policy, uint32_t block, uint32_t maxexc,
+                          int64_t* new_start, int64_t* base, int64_t* counts);
+/* DEVICE pointers of the step in flight: children = the rank's offspring in child order (send side), population = where
+ * the rank's new population must be written (receive side); valid between pa_dist_resample and pa_dist_finish. */
+int pa_dist_buffers(pa_ctx* ctx, void** children, void** population);
+/* T_all as given to the plan.  PA_ECAPACITY if the rank's new share exceeds its capacity (check BEFORE exchanging with
+ * pa_dist_new_count).  local (may be NULL) receives the rank's population sums. */
+int pa_dist_finish(pa_ctx* ctx, const int64_t* T_all, pa_obs* local);
+/* the rank's share of the new population under the plan (and its first global slot); PA_ECAPACITY if it does not fit */
+int pa_dist_new_count(pa_ctx* ctx, const int64_t* T_all, int64_t* count, int64_t* first_global_slot);
+/* drop the step in flight on this rank (another rank failed): nothing was committed */
+int pa_dist_abort(pa_ctx* ctx);
+
 /* ---- profiling (PA_PROFILE) --------------------------------------------------------------------------- */
 /* Sum of CUDA-event durations (ms) and number of launches per kernel since the last call; synchronises.
  * Both arrays have PA_K_COUNT entries (HOST). */

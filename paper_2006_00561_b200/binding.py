@@ -18,7 +18,9 @@ KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "cop
 
 EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
            "pa_observables", "pa_spins", "pa_tau", "pa_counts", "pa_parents", "pa_partitions", "pa_thresholds",
-           "pa_set_spins", "pa_debug_set_thresholds", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
+           "pa_set_spins", "pa_debug_set_thresholds", "pa_dist_init", "pa_dist_workspace_bytes", "pa_dist_begin",
+           "pa_dist_resample", "pa_dist_exchange_plan", "pa_dist_buffers", "pa_dist_finish", "pa_dist_new_count",
+           "pa_dist_abort", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
 
 
 class PaConfig(C.Structure):
@@ -32,6 +34,10 @@ class PaObs(C.Structure):
     _fields_ = [("R", C.c_int64), ("sum_E", C.c_int64), ("sum_E2", C.c_uint64 * 2), ("sum_absM", C.c_uint64 * 2),
                 ("sum_M2", C.c_uint64 * 2), ("sum_M4", C.c_uint64 * 2), ("mean_E", C.c_double), ("mean_E2", C.c_double),
                 ("mean_absM", C.c_double), ("mean_M2", C.c_double), ("mean_M4", C.c_double)]
+
+
+class PaDistPartial(C.Structure):
+    _fields_ = [("sumw", C.c_double), ("R", C.c_int64)]
 
 
 class PaError(RuntimeError):
@@ -73,6 +79,15 @@ def load_library():
         "pa_thresholds": (C.c_int, [vp, u32p, u32p]),
         "pa_set_spins": (C.c_int, [vp, vp, C.c_int64, C.c_int]),
         "pa_debug_set_thresholds": (C.c_int, [vp, C.c_int, C.c_uint32, C.c_uint32]),
+        "pa_dist_init": (C.c_int, [C.POINTER(PaConfig), C.c_int32, C.c_int32, C.POINTER(vp)]),
+        "pa_dist_workspace_bytes": (C.c_uint64, [C.POINTER(PaConfig), C.c_int32]),
+        "pa_dist_begin": (C.c_int, [vp, C.c_double, C.c_int32, C.POINTER(PaDistPartial)]),
+        "pa_dist_resample": (C.c_int, [vp, C.POINTER(PaDistPartial), i64p]),
+        "pa_dist_exchange_plan": (C.c_int, [C.c_int32, i64p, C.c_int32, C.c_uint32, C.c_uint32, i64p, i64p, i64p]),
+        "pa_dist_buffers": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp)]),
+        "pa_dist_finish": (C.c_int, [vp, i64p, C.POINTER(PaObs)]),
+        "pa_dist_new_count": (C.c_int, [vp, i64p, i64p, i64p]),
+        "pa_dist_abort": (C.c_int, [vp]),
         "pa_profile_read": (C.c_int, [vp, f64p, i64p]),
         "pa_launch_count": (C.c_int, [vp, i64p]),
         "pa_last_error": (C.c_char_p, [vp]),
@@ -90,11 +105,28 @@ def _np_ptr(a):
     return C.c_void_p(a.ctypes.data)
 
 
+def exchange_plan(T, policy=PA_POLICY_BALANCED, block=0, maxexc=0):
+    """pa_dist_exchange_plan (pure host function; works without a GPU): T = offspring totals in rank order.
+    Returns (new_start[world+1], base[world+1], counts[world, world]) with counts[src, dst] = children src sends to dst;
+    raises PaError(PA_EEXTINCT) for an extinct population, PaError(PA_ECAPACITY) if a rank reported -1."""
+    lib = load_library()
+    t = np.ascontiguousarray(T, np.int64)
+    W = t.shape[0]
+    ns, base, counts = np.zeros(W + 1, np.int64), np.zeros(W + 1, np.int64), np.zeros((W, W), np.int64)
+    p64 = lambda a: a.ctypes.data_as(C.POINTER(C.c_int64))
+    rc = lib.pa_dist_exchange_plan(W, p64(t), int(policy), int(block), int(maxexc), p64(ns), p64(base), p64(counts))
+    if rc != PA_OK:
+        raise PaError(rc, {PA_EEXTINCT: "population extinct", PA_ECAPACITY: "a rank's offspring exceed its capacity"}.get(rc, "bad plan arguments"))
+    return ns, base, counts
+
+
 class PopulationAnnealer:
     """One PA context on the current CUDA device.  Method names mirror the C ABI (pa_*)."""
 
     def __init__(self, L, R0, P=1, seed=0, beta0=0.0, capacity=0, flags=0, device=None, stream=None,
-                 policy=PA_POLICY_BALANCED, block=0, maxexc=0):
+                 policy=PA_POLICY_BALANCED, block=0, maxexc=0, rank=None, world=None):
+        """rank / world given: this context is one rank's shard of a multi-GPU run (pa_dist_init; R0 is the GLOBAL
+        target population) and is stepped with dist_begin / dist_resample / dist_finish (see dist.ShardedAnnealer)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2006_00561_b200 needs a CUDA device (no CPU fallback)")
@@ -107,7 +139,11 @@ class PopulationAnnealer:
         self.wpr = self.N // 32
         cfg = PaConfig(L=L, P=P, R0=R0, capacity=capacity, seed=seed, beta0=beta0, workspace=None, workspace_bytes=0,
                        stream=self.stream.cuda_stream, flags=flags, policy=policy, block=block, maxexc=maxexc)
-        nbytes = self._lib.pa_workspace_bytes(C.byref(cfg))
+        self.rank, self.world = rank, world
+        if world is None:
+            nbytes = self._lib.pa_workspace_bytes(C.byref(cfg))
+        else:
+            nbytes = self._lib.pa_dist_workspace_bytes(C.byref(cfg), int(world))
         if nbytes == 0:
             raise PaError(PA_EINVAL, "invalid configuration")
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
@@ -117,7 +153,10 @@ class PopulationAnnealer:
         cfg.workspace_bytes = nbytes
         self.workspace_bytes = nbytes
         self._ctx = C.c_void_p()
-        rc = self._lib.pa_init(C.byref(cfg), C.byref(self._ctx))
+        if world is None:
+            rc = self._lib.pa_init(C.byref(cfg), C.byref(self._ctx))
+        else:
+            rc = self._lib.pa_dist_init(C.byref(cfg), int(rank), int(world), C.byref(self._ctx))
         if rc != PA_OK:
             msg = self._lib.pa_last_error(self._ctx).decode() if self._ctx else "pa_init failed"
             if self._ctx:
@@ -259,6 +298,42 @@ class PopulationAnnealer:
 
     def debug_set_thresholds(self, enable, T4=0, T8=0):
         self._check(self._lib.pa_debug_set_thresholds(self._ctx, int(bool(enable)), int(T4), int(T8)))
+
+    # ---- multi-GPU shard (include/pa_b200.h "multi-GPU") --------------------------------------------
+    def dist_begin(self, beta_next, theta):
+        p = PaDistPartial()
+        self._check(self._lib.pa_dist_begin(self._ctx, float(beta_next), int(theta), C.byref(p)))
+        return float(p.sumw), int(p.R)
+
+    def dist_resample(self, partials):
+        arr = (PaDistPartial * len(partials))(*[PaDistPartial(float(a), int(b)) for a, b in partials])
+        T = C.c_int64(0)
+        self._check(self._lib.pa_dist_resample(self._ctx, arr, C.byref(T)))
+        return int(T.value)
+
+    def dist_buffers(self):
+        """(children, population) as uint8 views of the workspace tensor: send side / receive side of the exchange"""
+        a, b = C.c_void_p(), C.c_void_p()
+        self._check(self._lib.pa_dist_buffers(self._ctx, C.byref(a), C.byref(b)))
+        base = self.workspace.data_ptr()
+        return self.workspace[a.value - base:], self.workspace[b.value - base:]
+
+    def dist_new_count(self, T_all):
+        t = np.ascontiguousarray(T_all, np.int64)
+        n, first = C.c_int64(0), C.c_int64(0)
+        self._check(self._lib.pa_dist_new_count(self._ctx, t.ctypes.data_as(C.POINTER(C.c_int64)), C.byref(n), C.byref(first)))
+        return int(n.value), int(first.value)
+
+    def dist_finish(self, T_all):
+        t = np.ascontiguousarray(T_all, np.int64)
+        o = PaObs()
+        self._check(self._lib.pa_dist_finish(self._ctx, t.ctypes.data_as(C.POINTER(C.c_int64)), C.byref(o)))
+        big = lambda p: int(p[0]) | (int(p[1]) << 64)
+        return {"R": int(o.R), "sum_E": int(o.sum_E), "sum_E2": big(o.sum_E2), "sum_absM": big(o.sum_absM),
+                "sum_M2": big(o.sum_M2), "sum_M4": big(o.sum_M4)}
+
+    def dist_abort(self):
+        self._check(self._lib.pa_dist_abort(self._ctx))
 
     def profile_read(self):
         ms = (C.c_double * len(KERNELS))()

@@ -117,6 +117,12 @@ struct pa_ctx {
   int64_t launches;
   bool profile, profile_span;
   bool attempt_failed;  // the last pa_step / pa_run ended with an uncommitted step: off / n / tau hold that attempt
+  // multi-GPU shard (pa_dist_*): rank = partition
+  int rank, world;          // world = 0: not a shard
+  int64_t g_R0;             // target population of the WHOLE run (= cfg.R0 unless this is a shard)
+  int dist_phase;           // 0 idle, 1 after pa_dist_begin, 2 after pa_dist_resample
+  int dist_theta;
+  double dist_beta_next;
   bool dbg_thresholds;  // test hook: pa_debug_set_thresholds
   uint32_t dbg_T4, dbg_T8;
   int scan_grid_max;  // co-resident blocks of k_poisson_scan on this device
@@ -283,7 +289,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   {
     Prof p(c, PA_K_Q_REDUCE);  // also resets the step's counters and look-back descriptors
     launch(c, "k_q_reduce", k_q_reduce, RED_GRID, RED_THREADS, st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
-           (double)c->cfg.R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tb);
+           (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tb);
   }
   {
     // persistent blocks pull tiles from a ticket counter
@@ -340,6 +346,17 @@ __global__ void k_set_population(DevState* st, unsigned long long R, uint32_t* p
   const unsigned long long base = R / P, rem = R % P;
   for (int p = threadIdx.x; p <= P; p += blockDim.x)
     part[p] = (uint32_t)((unsigned long long)p * base + ((unsigned long long)p < rem ? p : rem));
+}
+// multi-GPU shard: mark the context, set the global index of local slot 0
+__global__ void k_dist_mark(DevState* st, unsigned slot0) {
+  st->dist = 1u;
+  st->slot0 = slot0;
+  st->slot0_new = slot0;
+}
+// ... and the size / first global slot of the population the exchange has just delivered
+__global__ void k_dist_set_new(DevState* st, unsigned long long count, unsigned slot0_new) {
+  st->Rnew = count;
+  st->slot0_new = slot0_new;
 }
 __global__ void k_clear_status(DevState* st) {
   st->status = 0u;
@@ -435,7 +452,9 @@ uint64_t pa_workspace_bytes(const pa_config* cfg) {
   return lo.total;
 }
 
-int pa_init(const pa_config* cfg, pa_ctx** out) {
+namespace {
+// shared by pa_init (world = 0) and pa_dist_init (world >= 1: cfg holds the rank's local R0, global values in g_*)
+int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t g_R0, int64_t g_first) {
   if (!cfg || !out) return PA_EINVAL;
   *out = nullptr;
   pa_ctx* c = new (std::nothrow) pa_ctx();
@@ -458,6 +477,9 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   c->profile_span = (cfg->flags & PA_PROFILE_SPAN) != 0;
   c->launches = 0;
   c->attempt_failed = false;
+  c->rank = 0;
+  c->world = 0;
+  c->dist_phase = 0;
   c->dbg_thresholds = false;
   c->dbg_T4 = c->dbg_T8 = 0u;
   c->scan_grid_max = 0;
@@ -487,6 +509,13 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   k_init_state<<<1, 256, 0, c->stream>>>(st, (unsigned long long)cfg->R0, cfg->beta0, c->dev<uint32_t>(c->lo.part[0]),
                                          cfg->P);
   c->launches += 1;
+  c->rank = rank;
+  c->world = world;
+  c->g_R0 = world > 0 ? g_R0 : cfg->R0;
+  if (world > 0) {
+    k_dist_mark<<<1, 1, 0, c->stream>>>(st, (unsigned)g_first);
+    c->launches += 1;
+  }
   CK(cudaMemsetAsync(c->dev<char>(c->lo.part_stats), 0, (size_t)cfg->P * 16, c->stream));
   {
     const int bpr = (c->wrep + 3) / 4;
@@ -502,11 +531,15 @@ int pa_init(const pa_config* cfg, pa_ctx** out) {
   if (rc != PA_OK) return rc;
   return PA_OK;
 }
+}  // namespace
+
+int pa_init(const pa_config* cfg, pa_ctx** out) { return init_common(cfg, out, 0, 0, 0, 0); }
 
 int pa_run(pa_ctx* c, const double* betas, int32_t K, int32_t theta, int32_t* steps_done) {
   if (!c) return PA_EINVAL;
   if (steps_done) *steps_done = 0;
   if (K < 0 || (K > 0 && !betas)) return fail(c, PA_EINVAL, "bad betas/K");
+  if (c->world > 0) return fail(c, PA_EINVAL, "this context is a multi-GPU shard: step it with pa_dist_begin / _resample / _finish");
   if (int rc = bind_device(c)) return rc;
   double from = c->beta;
   for (int k = 0; k < K; ++k) {
@@ -668,6 +701,236 @@ int pa_set_spins(pa_ctx* c, const uint32_t* src, int64_t R, int src_on_device) {
   launch_sweep(c, 0, 0u, 0u, 1);
   launch_observe(c, nullptr, 1);
   return sync_state(c);
+}
+
+// ---- multi-GPU: partitioned redistribution ------------------------------------------------------------
+namespace {
+// balanced table value: start of partition p of `total` items over P partitions
+inline int64_t balanced_start(int64_t total, int P, int p) {
+  const int64_t base = total / P, rem = total % P;
+  return (int64_t)p * base + (p < rem ? p : rem);
+}
+// counts under a policy from the per-rank offspring totals (host mirror of balance_tile; A6b)
+void policy_counts_host(int P, const int64_t* born, int policy, uint32_t B, uint32_t maxexc, std::vector<int64_t>& cnt) {
+  int64_t total = 0;
+  for (int p = 0; p < P; ++p) total += born[p];
+  const int64_t base = total / P, rem = total % P;
+  cnt.assign(P, 0);
+  if (policy == PA_POLICY_NONE) {
+    for (int p = 0; p < P; ++p) cnt[p] = born[p];
+  } else if (policy == PA_POLICY_NAIVE) {
+    int64_t pool = 0;
+    for (int p = 0; p < P; ++p) pool += born[p] / 2;
+    const int64_t share = pool / P, extra = pool % P;
+    for (int p = 0; p < P; ++p) cnt[p] = born[p] - born[p] / 2 + share + (p < extra ? 1 : 0);
+  } else if (policy == PA_POLICY_MAIN) {
+    const int64_t W = (int64_t)maxexc * (int64_t)B;
+    for (int p = 0; p < P; ++p) cnt[p] = born[p];
+    for (;;) {
+      int hi = 0, lo = 0;
+      int64_t e_hi = 0, e_lo = 0;
+      for (int p = 0; p < P; ++p) {
+        const int64_t e = cnt[p] - (base + (p < rem ? 1 : 0));
+        if (p == 0 || e > e_hi) { e_hi = e; hi = p; }
+        if (p == 0 || e < e_lo) { e_lo = e; lo = p; }
+      }
+      if (e_hi <= W && -e_lo <= W) break;
+      cnt[hi] -= (int64_t)B;
+      cnt[lo] += (int64_t)B;
+    }
+  } else {
+    for (int p = 0; p < P; ++p) cnt[p] = base + (p < rem ? 1 : 0);
+  }
+}
+}  // namespace
+
+int pa_dist_exchange_plan(int32_t world, const int64_t* T, int32_t policy, uint32_t block, uint32_t maxexc,
+                          int64_t* new_start, int64_t* base, int64_t* counts) {
+  if (world < 1 || !T || !new_start || !base || !counts || policy < 0 || policy > PA_POLICY_NONE) return PA_EINVAL;
+  for (int r = 0; r < world; ++r)
+    if (T[r] < 0) return PA_ECAPACITY;
+  std::vector<int64_t> cnt;
+  policy_counts_host(world, T, policy, block ? block : 1024u, maxexc ? maxexc : 1u, cnt);
+  base[0] = 0;
+  new_start[0] = 0;
+  for (int r = 0; r < world; ++r) {
+    base[r + 1] = base[r] + T[r];
+    new_start[r + 1] = new_start[r] + cnt[r];
+  }
+  if (base[world] == 0) return PA_EEXTINCT;
+  // rank src's offspring are the global children [base[src], base[src+1]); rank dst's new range is
+  // [new_start[dst], new_start[dst+1]): the slice is the intersection (contiguous on both sides)
+  for (int src = 0; src < world; ++src)
+    for (int dst = 0; dst < world; ++dst) {
+      const int64_t lo = base[src] > new_start[dst] ? base[src] : new_start[dst];
+      const int64_t hi = base[src + 1] < new_start[dst + 1] ? base[src + 1] : new_start[dst + 1];
+      counts[(size_t)src * world + dst] = hi > lo ? hi - lo : 0;
+    }
+  return PA_OK;
+}
+
+int pa_dist_init(const pa_config* cfg, int32_t rank, int32_t world, pa_ctx** out) {
+  if (!cfg || !out || world < 1 || rank < 0 || rank >= world || cfg->R0 < world) return PA_EINVAL;
+  if (cfg->policy != PA_POLICY_BALANCED && world > BAL_PMAX) return PA_EINVAL;
+  pa_config local = *cfg;
+  const int64_t first = balanced_start(cfg->R0, world, rank), last = balanced_start(cfg->R0, world, rank + 1);
+  local.R0 = last - first;
+  local.P = 1;
+  local.policy = PA_POLICY_BALANCED;  // the device keeps one local partition; the policy acts between the ranks
+  if (local.capacity == 0) local.capacity = (2 * ((cfg->R0 + world - 1) / world) + 4096 + 1023) / 1024 * 1024;
+  int rc = init_common(&local, out, rank, world, cfg->R0, first);
+  if (*out) {
+    (*out)->cfg.policy = cfg->policy;  // for the rank-level plan
+    (*out)->cfg.block = cfg->block;
+    (*out)->cfg.maxexc = cfg->maxexc;
+  }
+  return rc;
+}
+
+uint64_t pa_dist_workspace_bytes(const pa_config* cfg, int32_t world) {
+  if (!cfg || world < 1 || cfg->R0 < world) return 0;
+  pa_config local = *cfg;
+  local.R0 = (cfg->R0 + world - 1) / world;
+  local.P = 1;
+  local.policy = PA_POLICY_BALANCED;
+  if (local.capacity == 0) local.capacity = (2 * ((cfg->R0 + world - 1) / world) + 4096 + 1023) / 1024 * 1024;
+  return pa_workspace_bytes(&local);
+}
+
+int pa_dist_begin(pa_ctx* c, double beta_next, int32_t theta, pa_dist_partial* mine) {
+  if (!c || !mine) return PA_EINVAL;
+  if (c->world < 1) return fail(c, PA_EINVAL, "pa_dist_begin: not a shard (use pa_dist_init)");
+  if (c->dist_phase != 0) return fail(c, PA_EINVAL, "pa_dist_begin: a step is in flight");
+  if (int rc = bind_device(c)) return rc;
+  if (int rc = check_step_args(c, c->beta, beta_next, theta)) return rc;
+  if ((uint64_t)c->steps + 1u >= (1ull << 28)) return fail(c, PA_EINVAL, "step counter would exceed 2^28");
+  c->h_params[0] = make_params(c, c->beta, beta_next, theta);
+  StepParams* d_params = c->dev<StepParams>(c->lo.params);
+  CK(cudaMemcpyAsync(d_params, c->h_params, sizeof(StepParams), cudaMemcpyHostToDevice, c->stream));
+  DevState* st = c->dev<DevState>(c->lo.state);
+  const int n_desc = (int)((c->cap + SCAN_TILE - 1) / SCAN_TILE + 1);
+  {
+    Prof p(c, PA_K_Q_REDUCE);  // a shard: stops at the rank's own sum of weights
+    launch(c, "k_q_reduce", k_q_reduce, RED_GRID, RED_THREADS, st, (const StepParams*)d_params,
+           (const int32_t*)c->dev<int32_t>(c->lo.E[0]), (const int32_t*)c->dev<int32_t>(c->lo.E[1]), c->N,
+           c->dev<double>(c->lo.red_partial), (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tables(c));
+  }
+  if (int rc = sync_state(c)) return rc;
+  mine->sumw = c->h_state->sumw;
+  mine->R = c->R;
+  c->dist_phase = 1;
+  c->dist_theta = theta;
+  c->dist_beta_next = beta_next;
+  return PA_OK;
+}
+
+int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) {
+  if (!c || !all || !offspring) return PA_EINVAL;
+  if (c->world < 1 || c->dist_phase != 1) return fail(c, PA_EINVAL, "pa_dist_resample: call pa_dist_begin first");
+  if (int rc = bind_device(c)) return rc;
+  double sumw = 0.0;  // the ranks' sums are added in rank order on every rank: all ranks get the same bits
+  int64_t R = 0;
+  for (int r = 0; r < c->world; ++r) {
+    sumw += all[r].sumw;
+    R += all[r].R;
+  }
+  if (all[c->rank].R != c->R) return fail(c, PA_EINVAL, "pa_dist_resample: all[rank] is not this rank's partial");
+  DevState* st = c->dev<DevState>(c->lo.state);
+  const StepParams* d_params = c->dev<StepParams>(c->lo.params);
+  const LevelTables tb = tables(c);
+  const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
+  {
+    Prof p(c, PA_K_LEVELS_TAU);
+    launch(c, "k_dist_tables", k_dist_tables, 1u, RED_THREADS, st, d_params, c->N, sumw, (double)R, (double)c->g_R0, tb);
+  }
+  {
+    const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
+    const bool keep = c->lo.n || c->lo.tau;
+    if (c->scan_grid_max == 0) {
+      int per_sm = 0, sms = 0;
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true>, SCAN_THREADS, 0);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+      c->scan_grid_max = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
+    }
+    ScanOut out;
+    out.off = c->dev<uint32_t>(c->lo.off);
+    out.n = c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr;
+    out.tau = c->lo.tau ? c->dev<double>(c->lo.tau) : nullptr;
+    out.tile_desc = c->dev<unsigned long long>(c->lo.tile_desc);
+    out.parent_of = c->dev<uint32_t>(c->lo.parent_of);
+    out.tile_parent = c->dev<uint32_t>(c->lo.tile_parent);
+    const int shift = copy_shift_for(c->cfg.L);
+    const unsigned long long cap = (unsigned long long)c->cap;
+    const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? (tiles_cap ? tiles_cap : 1u) : (unsigned)c->scan_grid_max;
+    Prof p(c, PA_K_POISSON_SCAN);
+    if (keep) launch(c, "k_poisson_scan", k_poisson_scan<true, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
+    else launch(c, "k_poisson_scan", k_poisson_scan<false, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
+  }
+  launch_copy(c);  // the rank's offspring, expanded in child order, into the spare buffer: the send side of the exchange
+  CK(cudaMemcpyAsync(c->h_state, st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  CK(cudaGetLastError());
+  const DevState& hs = *c->h_state;
+  // a rank without offspring is fine here (extinction is a property of the whole population: the plan reports it)
+  if (hs.status == ST_CAPACITY) *offspring = -1;
+  else *offspring = (int64_t)hs.Rnew;
+  c->dist_phase = 2;
+  return PA_OK;
+}
+
+int pa_dist_buffers(pa_ctx* c, void** children, void** population) {
+  if (!c) return PA_EINVAL;
+  if (c->world < 1 || c->dist_phase != 2) return fail(c, PA_EINVAL, "pa_dist_buffers: no step in flight");
+  const unsigned cur = c->h_state->cur;
+  if (children) *children = c->dev<char>(c->lo.spins[cur ^ 1u]);
+  if (population) *population = c->dev<char>(c->lo.spins[cur]);
+  return PA_OK;
+}
+
+int pa_dist_new_count(pa_ctx* c, const int64_t* T_all, int64_t* count, int64_t* first_global_slot) {
+  if (!c || !T_all) return PA_EINVAL;
+  if (c->world < 1) return fail(c, PA_EINVAL, "pa_dist_new_count: not a shard");
+  const int W = c->world;
+  std::vector<int64_t> ns(W + 1), base(W + 1), counts((size_t)W * W);
+  const int rc = pa_dist_exchange_plan(W, T_all, (int)c->cfg.policy, c->cfg.block, c->cfg.maxexc, ns.data(), base.data(), counts.data());
+  if (rc != PA_OK) return fail(c, rc, rc == PA_EEXTINCT ? "population extinct (sum of offspring = 0)" : "a rank's offspring exceed its capacity");
+  const int64_t n = ns[c->rank + 1] - ns[c->rank];
+  if (count) *count = n;
+  if (first_global_slot) *first_global_slot = ns[c->rank];
+  if (n > c->cap) return fail(c, PA_ECAPACITY, "the rank's share of the new population exceeds its capacity");
+  if (ns[W] >= (1ll << 32) - 4096) return fail(c, PA_ECAPACITY, "global population does not fit 32-bit slot indices");
+  return PA_OK;
+}
+
+int pa_dist_abort(pa_ctx* c) {
+  if (!c) return PA_EINVAL;
+  if (c->world < 1) return fail(c, PA_EINVAL, "pa_dist_abort: not a shard");
+  if (int rc = bind_device(c)) return rc;
+  k_clear_status<<<1, 1, 0, c->stream>>>(c->dev<DevState>(c->lo.state));
+  c->launches += 1;
+  c->dist_phase = 0;
+  return sync_state(c);
+}
+
+int pa_dist_finish(pa_ctx* c, const int64_t* T_all, pa_obs* local) {
+  if (!c || !T_all) return PA_EINVAL;
+  if (c->world < 1 || c->dist_phase != 2) return fail(c, PA_EINVAL, "pa_dist_finish: call pa_dist_resample first");
+  if (int rc = bind_device(c)) return rc;
+  int64_t n = 0, first = 0;
+  if (int rc = pa_dist_new_count(c, T_all, &n, &first)) return rc;
+  if (n < 1) return fail(c, PA_EEXTINCT, "this rank's share of the new population is empty");
+  DevState* st = c->dev<DevState>(c->lo.state);
+  k_clear_status<<<1, 1, 0, c->stream>>>(st);  // a capacity flag of the local expansion cannot be pending here (plan refused it)
+  k_dist_set_new<<<1, 1, 0, c->stream>>>(st, (unsigned long long)n, (unsigned)first);
+  c->launches += 2;
+  const StepParams& hp = c->h_params[0];
+  launch_sweep(c, c->dist_theta, hp.T4, hp.T8, 3);  // theta sweeps in place (theta = 0: E, M only)
+  launch_observe(c, c->dev<StepParams>(c->lo.params), 2);
+  c->dist_phase = 0;
+  if (int rc = sync_state(c)) return rc;
+  c->attempt_failed = false;
+  if (local) return pa_observables(c, local);
+  return PA_OK;
 }
 
 int pa_profile_read(pa_ctx* c, double* ms, int64_t* launches) {

@@ -31,7 +31,10 @@ struct DevState {
   unsigned int fail_step;        // ordinal of the step that failed
   unsigned int reduce_done;      // block counters (reset every step by k_q_reduce)
   unsigned int scan_tile;        // ticket counter of k_poisson_scan
-  unsigned int pad2_[7];
+  unsigned int slot0;            // shard of a multi-GPU run: global index of local slot 0 of the CURRENT population (else 0)
+  unsigned int slot0_new;        // ... of the population the running step builds
+  unsigned int dist;             // 1: this context is one rank's shard (Q comes from all ranks; the step is committed in place)
+  unsigned int pad2_[4];
   unsigned int scan_overflow;    // a parent sat on a level with lambda >= 2^31
   unsigned int obs_done;
   unsigned int T4, T8;           // thresholds of the last committed step with theta > 0

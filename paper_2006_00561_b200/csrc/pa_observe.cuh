@@ -15,7 +15,7 @@ __global__ void k_init(const DevState* __restrict__ st, uint32_t* __restrict__ s
   const unsigned long long j = idx / blocks_per_rep;
   const unsigned b = (unsigned)(idx % blocks_per_rep);
   if (j >= R) return;
-  const uint4 w = philox4x32_10(b, (uint32_t)j, 0u, ctr3(TAG_INIT, 0u), key);
+  const uint4 w = philox4x32_10(b, (uint32_t)j + st->slot0, 0u, ctr3(TAG_INIT, 0u), key);  // keyed by the GLOBAL replica index
   uint32_t* dst = spins + j * wrep + 4 * b;
   if (wrep - 4 * (int)b >= 4) {
     *reinterpret_cast<uint4*>(dst) = w;
@@ -150,6 +150,8 @@ constexpr int OBS_Q = 5;  // sum E (two's complement), sum E^2, sum |M|, sum M^2
 
 // mode 0: end of a step -> sums over buffer cur^1 (Rnew replicas), then COMMIT the step.
 // mode 1: after init / set_spins -> sums over buffer cur (R replicas), no commit.
+// mode 2: end of a step of a multi-GPU shard -> the exchange has put the new local population (Rnew replicas) into
+//         buffer cur itself; sums over it, then COMMIT without flipping the buffers.
 __global__ void __launch_bounds__(OBS_THREADS)
 k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
           const int32_t* __restrict__ E1, const int32_t* __restrict__ M0, const int32_t* __restrict__ M1,
@@ -158,7 +160,7 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   grid_dependency_wait();
   if (st->status != ST_OK) return;
   const unsigned buf = mode == 0 ? (st->cur ^ 1u) : st->cur;
-  const unsigned long long count = mode == 0 ? st->Rnew : st->R;
+  const unsigned long long count = mode != 1 ? st->Rnew : st->R;
   const int32_t* __restrict__ E = buf ? E1 : E0;
   const int32_t* __restrict__ M = buf ? M1 : M0;
   // per-thread partial sums: a thread sees at most cap / (grid * 256) < 2^17 replicas, |E| <= 2^15, |M| <= 2^14, so
@@ -283,11 +285,12 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
     st->lev_lo = (int)((lo + 2 * N) >> 2);
     st->lev_hi = (int)((hi + 2 * N) >> 2);
     st->obs_R = count;
-    if (mode == 0) {  // commit: the new population becomes the current one
+    if (mode != 1) {  // commit: the new population becomes the current one
       st->R_parents = st->R;
       st->R = st->Rnew;
       st->replica_steps += st->Rnew;
-      st->cur ^= 1u;
+      if (mode == 0) st->cur ^= 1u;
+      st->slot0 = st->slot0_new;
       st->step += 1u;
       st->sum_lnQ += st->lnQ;
       st->Q_committed = st->Q;

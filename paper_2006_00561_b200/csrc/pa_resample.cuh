@@ -190,7 +190,11 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
     double t = 0.0;
     for (unsigned b = threadIdx.x; b < gridDim.x; b += 32) t += __ldcg(&partial[b]);
     t = warp_sum(t);
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0 && st->dist) {  // a shard: Q needs every rank's sum (k_dist_tables finishes the job)
+      st->sumw = t;
+      st->reduce_done = 0u;
+    }
+    if (threadIdx.x == 0 && !st->dist) {
       const double Q = t / (double)R;
       st->sumw = t;
       st->Q = Q;
@@ -201,12 +205,34 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
     }
   }
   __syncthreads();
+  if (st->dist) return;
   // a2 per level: the tables of the occupied window (only that window is ever looked up)
   {
     const double Q = s_Q, scale = R0 / (double)R;
     const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
     for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(dbeta, lev, N, Q, scale, tb);
   }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// k_dist_tables: multi-GPU shard.  Every rank has summed its own weights (k_q_reduce); the host has added the ranks'
+// sums in rank order (sumw_global, R_global).  One block: Q = sumw / R over the WHOLE population (the
+// central node "sends this number to the nodes as the normalization factor"), ln Q, scale = R0 / R, and the level
+// tables of this rank's occupied window.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(RED_THREADS)
+k_dist_tables(DevState* st, const StepParams* __restrict__ sp, int N, double sumw_global, double R_global, double R0,
+              LevelTables tb) {
+  grid_dependency_wait();
+  if (st->status != ST_OK) return;
+  const double Q = sumw_global / R_global, scale = R0 / R_global;
+  if (threadIdx.x == 0) {
+    st->Q = Q;
+    st->lnQ = log(Q);
+    st->scale = scale;
+  }
+  const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
+  for (int lev = st->lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(sp->dbeta, lev, N, Q, scale, tb);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -315,6 +341,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
   const unsigned tile_end = ntiles;
   const int32_t* __restrict__ E = st->cur ? E1 : E0;
   const uint32_t c3 = ctr3(TAG_RESAMPLE, st->step + 1u);
+  const uint32_t slot0 = st->slot0;  // the copy counts are keyed by the GLOBAL parent index (a multi-GPU shard: slot0 > 0)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x == 0) s_flag = 0u;
   unsigned prev = NO_TILE;
@@ -357,7 +384,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
           }
         }
 #pragma unroll
-        for (int b = 0; b < SCAN_BATCH; ++b) u[b] = chunk_uniform(philox4x32_10(0u, jj[b], 0u, c3, key), 0u);
+        for (int b = 0; b < SCAN_BATCH; ++b) u[b] = chunk_uniform(philox4x32_10(0u, jj[b] + slot0, 0u, c3, key), 0u);
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {  // rows of unused levels are masked below
           if (ALL || hl[b] < (unsigned)SCAN_HW) {
@@ -409,7 +436,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
           const unsigned item = s_hitem[lo];
           const uint32_t j = tile_base + item;
           const unsigned lev = (unsigned)((__ldg(E + j) + 2 * N) >> 2);
-          const unsigned kk = draw_chunk(tb.cdf + (size_t)lev * PO_ROW, j, 1ull + (wk - s_hstart[lo]), c3, key);
+          const unsigned kk = draw_chunk(tb.cdf + (size_t)lev * PO_ROW, j + slot0, 1ull + (wk - s_hstart[lo]), c3, key);
           if (kk) atomicAdd(&cntb[item], kk);
         }
       }

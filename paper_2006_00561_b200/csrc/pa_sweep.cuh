@@ -59,6 +59,8 @@ struct SweepArgs {
              // 1: init / set_spins -> buffer cur, R replicas, no sweeps (energies only)
              // 2: as 0, but the lattice of slot i is LOADED from slot parent_of[i] of buffer cur (gather-on-load: the
              //    redistribution copy a6 is fused into the sweep's load) and stored to slot i of buffer cur^1
+             // 3: multi-GPU shard -> the exchange has put the new local population (Rnew replicas) into buffer cur; theta
+             //    sweeps in place.  The sweeps of every mode are keyed by the GLOBAL slot index (slot0_new + i).
 };
 
 __device__ __forceinline__ uint32_t even_bits(uint32_t x) {  // bits 0,2,4,.. -> bits 0..15
@@ -394,7 +396,7 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
   static_assert(L >= 64, "k_sweep_small handles L < 64");
   grid_dependency_wait();
   if (st->status != ST_OK) return;
-  const unsigned buf = sa.mode != 1 ? (st->cur ^ 1u) : st->cur;
+  const unsigned buf = (sa.mode == 1 || sa.mode == 3) ? st->cur : (st->cur ^ 1u);
   const unsigned long long count = sa.mode != 1 ? st->Rnew : st->R;
   const int theta = sa.mode != 1 ? sa.theta : 0;
   uint32_t* spins = buf ? spins1 : spins0;
@@ -443,9 +445,10 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
     if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
     __syncthreads();
     const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
+    const uint32_t gs = st->slot0_new;  // global index of local slot 0 (0 unless this is a multi-GPU shard)
     for (int t = 0; t < theta; ++t) {
-      half_sweep<L, 0>(lat, q, g, slot0, slot_base, valid, (uint32_t)t, c3, key, sa);
-      half_sweep<L, 1>(lat, q, g, slot0, slot_base, valid, (uint32_t)t, c3, key, sa);
+      half_sweep<L, 0>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa);
+      half_sweep<L, 1>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa);
     }
   }
 
@@ -526,12 +529,13 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
   static_assert(L == 8 || L == 16 || L == 32, "");
   grid_dependency_wait();
   if (st->status != ST_OK) return;
-  const unsigned buf = sa.mode != 1 ? (st->cur ^ 1u) : st->cur;
+  const unsigned buf = (sa.mode == 1 || sa.mode == 3) ? st->cur : (st->cur ^ 1u);
   const unsigned long long count = sa.mode != 1 ? st->Rnew : st->R;
   const int theta = sa.mode != 1 ? sa.theta : 0;
   uint32_t* spins = buf ? spins1 : spins0;
   int32_t* __restrict__ Eo = buf ? E1 : E0;
   int32_t* __restrict__ Mo = buf ? M1 : M0;
+  const uint32_t gs = sa.mode != 1 ? st->slot0_new : 0u;  // global index of local slot 0 (multi-GPU shard)
 
   // A group of G lanes holds TWO consecutive replicas (one plane word per colour and replica per lane).
   constexpr int NR = 2;
@@ -550,7 +554,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
   for (int r = 0; r < NR; ++r) {
     slot64[r] = pair * NR + r;
     valid[r] = slot64[r] < count;
-    slots[r] = (uint32_t)slot64[r];
+    slots[r] = (uint32_t)slot64[r] + gs;
     rep[r] = spins + (valid[r] ? slot64[r] : 0ull) * G_::WREP;
     const uint32_t* rep_src = rep[r];
     if (sa.mode == 2 && valid[r]) rep_src = (buf ? spins0 : spins1) + (unsigned long long)parent_of[slot64[r]] * G_::WREP;
@@ -584,7 +588,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           neighbour_classes(p[r][0], U, D, p[r][1], B, ge1[r], ge2[r]);
           if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }  // padding never holds the warp back
         }
-        queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 0u, ge1, ge2, slots, slot_base, call0, 2u * (uint32_t)t, c3, key,
+        queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 0u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t, c3, key,
                                                            sa, flip);
 #pragma unroll
         for (int r = 0; r < NR; ++r) p[r][0] ^= flip[r];
@@ -598,7 +602,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           neighbour_classes(p[r][1], U, D, p[r][0], B, ge1[r], ge2[r]);
           if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }
         }
-        queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 1u, ge1, ge2, slots, slot_base, call0, 2u * (uint32_t)t + 1u, c3,
+        queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 1u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t + 1u, c3,
                                                            key, sa, flip);
 #pragma unroll
         for (int r = 0; r < NR; ++r) p[r][1] ^= flip[r];

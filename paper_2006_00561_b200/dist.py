@@ -1,7 +1,7 @@
-"""Multi-process plumbing for bench.py: one process per GPU, torch.distributed for barrier / max / sum only.
-
-The path does not shard across GPUs in this build ("replicas only"): every rank runs an
-independent replica of the whole simulation, there is no data-path collective.  The helpers work with the
+"""Multi-process plumbing: one process per GPU; torch.distributed for the barrier / max / sum of bench.py's timing and
+for the three exchanges of the partitioned redistribution (include/pa_b200.h "multi-GPU"):
+all-gather of the ranks' weight sums, all-gather of their offspring totals, all-to-all-v of contiguous lattice
+slices.  Every kernel runs in the library; this module only moves bytes between ranks.  The helpers work with the
 `nccl` backend on CUDA tensors and with `gloo` on CPU tensors (the latter is what the CPU tests exercise)."""
 import os
 
@@ -83,3 +83,120 @@ def shutdown(g):
         import torch.distributed as dist
         if dist.is_initialized():
             dist.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------------------------------
+# partitioned redistribution: rank = partition
+# ---------------------------------------------------------------------------------------------------
+def all_gather_doubles(g, values):
+    """every rank contributes len(values) doubles; returns a (world, len(values)) nested list in rank order"""
+    if g.world == 1:
+        return [list(map(float, values))]
+    import torch
+    import torch.distributed as dist
+    mine = _tensor(g, [float(v) for v in values], torch.float64)
+    out = [torch.empty_like(mine) for _ in range(g.world)]
+    dist.all_gather(out, mine)
+    return [[float(x) for x in t.tolist()] for t in out]
+
+
+def exchange_slices(g, send, recv, counts, unit):
+    """all-to-all-v of contiguous slices.  send / recv: 1-D tensors (uint8 bytes or int32 words) on this rank; counts[src][dst]
+    = items src sends to dst; one item = `unit` tensor elements.  Rank r's slices leave `send` in destination order and
+    arrive in `recv` in source order (global child order is source-rank order, so `recv` ends up in global order).
+    Point-to-point operations in one batch: the same code runs on NCCL (one group call) and on gloo."""
+    me, W = g.rank, g.world
+    s_off = [0] * (W + 1)
+    r_off = [0] * (W + 1)
+    for p in range(W):
+        s_off[p + 1] = s_off[p] + int(counts[me][p]) * unit
+        r_off[p + 1] = r_off[p] + int(counts[p][me]) * unit
+    if counts[me][me]:
+        recv[r_off[me]:r_off[me + 1]].copy_(send[s_off[me]:s_off[me + 1]])
+    if W == 1:
+        return
+    import torch.distributed as dist
+    ops = []
+    for p in range(W):
+        if p == me:
+            continue
+        if counts[me][p]:
+            ops.append(dist.P2POp(dist.isend, send[s_off[p]:s_off[p + 1]], p))
+        if counts[p][me]:
+            ops.append(dist.P2POp(dist.irecv, recv[r_off[p]:r_off[p + 1]], p))
+    if ops:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+
+
+class ShardedAnnealer:
+    """One rank's shard of a multi-GPU population annealing run, or -- with `emulate` ranks -- all ranks of such a run on
+    ONE device, stepped phase by phase in lock-step by the host (no kernel ever waits on another rank's kernel, so this
+    is safe on one GPU; it is how the device path is parity-tested where only one GPU is available)."""
+
+    def __init__(self, L, R0, seed=0, beta0=0.0, capacity=0, policy=0, block=0, maxexc=0, group=None, emulate=None, flags=0):
+        from . import binding
+        self._b = binding
+        self.policy, self.block, self.maxexc = policy, block, maxexc
+        self.L, self.S = L, L * L // 8
+        if emulate:
+            self.g, self.world = Group(), int(emulate)
+            ranks = range(self.world)
+        else:
+            self.g = group if group is not None else Group()
+            self.world = self.g.world
+            ranks = [self.g.rank]
+        self.shards = [binding.PopulationAnnealer(L, R0, seed=seed, beta0=beta0, capacity=capacity, policy=policy, block=block,
+                                                  maxexc=maxexc, rank=r, world=self.world, flags=flags) for r in ranks]
+        self.emulated = bool(emulate)
+        self.last_T = None
+
+    @property
+    def R_local(self):
+        return [s.R for s in self.shards]
+
+    def step(self, beta_next, theta):
+        b = self._b
+        partials = [s.dist_begin(beta_next, theta) for s in self.shards]
+        if self.emulated:
+            all_partials = partials
+        else:
+            rows = all_gather_doubles(self.g, [partials[0][0], float(partials[0][1])])
+            all_partials = [(r[0], int(r[1])) for r in rows]
+        T_local = [s.dist_resample(all_partials) for s in self.shards]
+        if self.emulated:
+            T_all = T_local
+        else:
+            T_all = [int(r[0]) for r in all_gather_doubles(self.g, [float(T_local[0])])]
+        try:  # every rank evaluates the same plan and the same capacity checks: all ranks fail or none does
+            ns, base, counts = b.exchange_plan(T_all, self.policy, self.block, self.maxexc)
+            for s in self.shards:
+                s.dist_new_count(T_all)
+        except b.PaError:
+            for s in self.shards:
+                s.dist_abort()
+            raise
+        S = self.S
+        if self.emulated:
+            bufs = [s.dist_buffers() for s in self.shards]
+            for src in range(self.world):
+                s_off = 0
+                for dst in range(self.world):
+                    n = int(counts[src][dst])
+                    if n:
+                        r_off = int(sum(counts[q][dst] for q in range(src)))
+                        bufs[dst][1][r_off * S:(r_off + n) * S].copy_(bufs[src][0][s_off * S:(s_off + n) * S])
+                    s_off += n
+        else:
+            children, population = self.shards[0].dist_buffers()
+            exchange_slices(self.g, children, population, counts, S)
+        self.last_T, self.last_counts, self.last_new_start = T_all, counts, ns
+        return [s.dist_finish(T_all) for s in self.shards]
+
+    def log_Z(self):
+        return self.shards[0].log_Z()
+
+    def gather_spins(self):
+        """emulation only: the whole population in global slot order"""
+        import numpy as np
+        return np.concatenate([s.spins() for s in self.shards], axis=0)

@@ -58,3 +58,117 @@ def test_single_process_is_identity():
     g = dist.Group()
     assert dist.aggregate_throughput(g, 10.0, 2.0) == (5.0, 10.0, 2.0)
     dist.barrier(g)
+
+
+# ---------------------------------------------------------------------------------------------------
+# partitioned redistribution, rank = partition
+# ---------------------------------------------------------------------------------------------------
+def test_exchange_plan_against_the_oracle_policies_and_its_invariants():
+    """pa_dist_exchange_plan is a pure host function of the product library (no GPU needed): its partition counts must be
+    the oracle's policy counts with born_p = T_p, and its slices must tile both sides exactly"""
+    import numpy as np
+    from oracle import pa_oracle as orc
+    from paper_2006_00561_b200 import binding
+    rng = np.random.default_rng(8)
+    for world in [1, 2, 3, 8, 64]:
+        for policy, block, maxexc in [(0, 1024, 1), (1, 1024, 1), (1, 64, 2), (2, 1024, 1), (3, 1024, 1)]:
+            T = rng.integers(0, 60000, world).astype(np.int64)
+            T[rng.integers(0, world)] = 0  # a rank without offspring
+            if T.sum() == 0:
+                T[0] = 5
+            ns, base, counts = binding.exchange_plan(T, policy, block, maxexc)
+            cnt, _ = orc.policy_counts(T.astype(np.uint32), policy, block, maxexc)
+            assert np.array_equal(np.diff(ns), cnt.astype(np.int64)), (world, policy)
+            assert np.array_equal(np.diff(base), T) and ns[-1] == base[-1] == T.sum()
+            assert np.array_equal(counts.sum(axis=1), T)            # every child is sent exactly once
+            assert np.array_equal(counts.sum(axis=0), np.diff(ns))  # every new slot is filled exactly once
+            # order preserving: the destinations of a source's slices are non-decreasing, and so are the sources of a destination's
+            for src in range(world):
+                nz = np.nonzero(counts[src])[0]
+                assert np.all(np.diff(nz) == 1) or len(nz) <= 1     # contiguous block of destinations
+            if policy == 3:
+                assert np.array_equal(counts, np.diag(T))           # nothing crosses a rank boundary (PAPER.md:88)
+    with pytest.raises(binding.PaError) as ei:
+        binding.exchange_plan([0, 0, 0])
+    assert ei.value.code == binding.PA_EEXTINCT
+    with pytest.raises(binding.PaError) as ei:
+        binding.exchange_plan([5, -1, 3])
+    assert ei.value.code == binding.PA_ECAPACITY
+
+
+def _sharded_oracle_worker(rank, world, port, q, L, R0, seed, betas, theta, policy):
+    """one rank of the partitioned run on the CPU: the oracle does the rank's arithmetic with GLOBAL replica indices as
+    keys, the product's host plan (pa_dist_exchange_plan) and exchange (dist.exchange_slices over gloo) move the replicas"""
+    os.environ.update({"RANK": str(rank), "WORLD_SIZE": str(world), "LOCAL_RANK": str(rank),
+                       "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    import numpy as np
+    import torch
+    from paper_2006_00561_b200 import binding, dist
+    from oracle import pa_oracle as orc
+    g = dist.init_from_env(backend="gloo", device_kind="cpu")
+    orc.set_threads(1)
+    wpr = orc.words_per_replica(L)
+    start = [r * (R0 // world) + min(r, R0 % world) for r in range(world + 1)]
+    spins = orc.init_population(L, R0, seed)[start[rank]:start[rank + 1]].copy()  # keyed by the global replica index
+    first, beta, sum_lnQ = start[rank], 0.0, 0.0
+    for step, beta_next in enumerate(betas, 1):
+        E, M = orc.energy_mag(L, spins)
+        R_loc, dbeta = spins.shape[0], beta_next - beta
+        w_sum = float(np.sum(np.exp(-dbeta * E.astype(np.float64))))  # the rank's sum of weights
+        rows = dist.all_gather_doubles(g, [w_sum, float(R_loc)])
+        sumw, R = 0.0, 0
+        for r in rows:  # rank order
+            sumw += r[0]
+            R += int(r[1])
+        Q = sumw / R
+        tau = orc.tau_weights(E, dbeta, Q)
+        tau_global = np.zeros(first + R_loc, np.float64)  # the sampler keys parent j by its GLOBAL index
+        tau_global[first:] = tau
+        n = orc.poisson_counts(tau_global, float(R0) / float(R), seed, step)[first:]
+        off, T_loc = orc.exclusive_scan(n)
+        children, _, _ = orc.copy_population(L, n, off, spins, E, M, T_loc)
+        T_all = [int(r[0]) for r in dist.all_gather_doubles(g, [float(T_loc)])]
+        ns, base, counts = binding.exchange_plan(T_all, policy, 16, 1)
+        new_n = int(ns[rank + 1] - ns[rank])
+        send = torch.from_numpy(children.reshape(-1).view(np.uint8).copy())
+        recv = torch.zeros(new_n * wpr * 4, dtype=torch.uint8)
+        dist.exchange_slices(g, send, recv, counts, wpr * 4)
+        spins = recv.numpy().view(np.uint32).reshape(new_n, wpr).copy()
+        first = int(ns[rank])
+        if theta > 0:
+            T4, T8 = orc.thresholds(beta_next)
+            orc.sweeps_slots(L, np.arange(first, first + new_n, dtype=np.uint32), spins, seed, step, theta, T4, T8)
+        beta = beta_next
+        sum_lnQ += float(np.log(Q))
+    q.put((rank, first, spins, sum_lnQ))
+    dist.barrier(g)
+    dist.shutdown(g)
+
+
+@pytest.mark.parametrize("world,policy", [(2, 0), (4, 0), (3, 1), (2, 2), (2, 3)])
+def test_sharded_run_equals_the_single_population_run_gloo(world, policy):
+    """world-size 2/3/4 over gloo: the concatenation of the ranks' populations equals the one-population oracle run bit
+    for bit (random numbers are keyed by global replica index and global step; the policy only moves rank boundaries)"""
+    import numpy as np
+    from oracle import pa_oracle as orc
+    L, R0, seed, theta = 8, 600, 77, 2
+    betas = [0.05 * k for k in range(1, 9)]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_sharded_oracle_worker, args=(r, world, port, q, L, R0, seed, betas, theta, policy))
+             for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((q.get(timeout=300) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    ref = orc.OraclePA(L, R0, seed=seed)
+    for b in betas:
+        ref.step(b, theta)
+    got = np.concatenate([r[2] for r in res], axis=0)
+    assert got.shape == ref.spins.shape and np.array_equal(got, ref.spins)
+    assert [r[1] for r in res] == sorted(r[1] for r in res) and res[0][1] == 0   # ranks own increasing global ranges
+    for r in res:
+        assert abs(r[3] - ref.sum_lnQ) <= 1e-12 * abs(ref.sum_lnQ)               # same ln Z on every rank (rounding of Q only)

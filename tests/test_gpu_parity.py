@@ -442,6 +442,56 @@ def test_policy_arguments_are_validated():
 
 
 # ---------------------------------------------------------------------------------------------------
+# multi-GPU partitioned redistribution: the ranks of a sharded run, emulated on ONE device and stepped
+# phase by phase by the host, must reproduce the single-context run bit for bit
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("world,L,R0,theta,policy", [(2, 32, 5000, 2, 0), (4, 64, 3001, 1, 0), (3, 16, 4099, 0, 0),
+                                                     (2, 64, 2500, 3, 1), (3, 32, 3000, 1, 2), (2, 8, 4000, 2, 3),
+                                                     (5, 128, 700, 1, 0)])
+def test_sharded_ranks_equal_the_single_context(world, L, R0, theta, policy):
+    b = _binding()
+    from paper_2006_00561_b200 import dist
+    seed = 1000 + 7 * world + L
+    single = b.PopulationAnnealer(L, R0, P=1, seed=seed)
+    sh = dist.ShardedAnnealer(L, R0, seed=seed, policy=policy, block=64, maxexc=1, emulate=world)
+    assert np.array_equal(sh.gather_spins(), single.spins())  # the initial population is keyed by global replica index
+    dbeta = min(0.05, 600.0 / (2 * L * L))
+    for k in range(1, 7):
+        single.step(dbeta * k, theta)
+        obs = sh.step(dbeta * k, theta)
+        assert sum(sh.R_local) == single.R == sum(o["R"] for o in obs)
+        assert np.array_equal(sh.gather_spins(), single.spins()), (k, "spins")
+        so = single.observables()
+        for key in ["sum_E", "sum_E2", "sum_absM", "sum_M2", "sum_M4"]:
+            assert sum(o[key] for o in obs) == so[key], (k, key)
+        for s_ in sh.shards:  # every rank carries the same ln Z (the ranks' weight sums are added in rank order)
+            assert rel(s_.log_Z()["lnZ"], single.log_Z()["lnZ"]) <= RTOL
+        E = np.concatenate([s_.energies()[0] for s_ in sh.shards])
+        assert np.array_equal(E, single.energies()[0])
+        # what the plan moved is what the ranks hold
+        ns = sh.last_new_start
+        assert [int(ns[r + 1] - ns[r]) for r in range(world)] == sh.R_local
+        if policy == 3:
+            assert np.array_equal(np.asarray(sh.last_counts), np.diag(sh.last_T))
+
+
+def test_sharded_capacity_failure_is_consistent_and_leaves_the_population_unchanged():
+    b = _binding()
+    from paper_2006_00561_b200 import dist
+    sh = dist.ShardedAnnealer(16, 2048, seed=5, capacity=1100, emulate=2)  # 1024 per rank, almost no slack
+    failures = 0
+    for k in range(1, 40):
+        before, Rb, lz = sh.gather_spins(), sh.R_local, sh.log_Z()
+        try:
+            sh.step(0.003 * k, 1)
+        except b.PaError as e:
+            assert e.code == b.PA_ECAPACITY
+            failures += 1
+            assert sh.R_local == Rb and np.array_equal(sh.gather_spins(), before) and sh.log_Z() == lz
+    assert failures > 0
+
+
+# ---------------------------------------------------------------------------------------------------
 # boundary behaviour
 # ---------------------------------------------------------------------------------------------------
 def test_run_equals_repeated_step_and_is_deterministic():
