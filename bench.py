@@ -8,8 +8,8 @@ A "step" is one pa_step: Q/tau reduction, Poisson resampling, scan, partition ba
 Metropolis sweeps, observables.  Workload: BASELINE.json configs[2] ("config 3": L=64, R0=2^21, dbeta=0.005,
 theta=10, P=148) -- the paper's own workload shape on one GPU; its population (1 GiB)
 is larger than L2.  metric = spin-flip attempts/s over the whole step.  The resampling/redistribution path
-(config 5, theta=0) is measured in the same run and reported under "resample".  N > 1: independent replicas of
-the whole simulation, one per GPU ("replicas only"), no data-path collective.
+(config 5, theta=0) is measured in the same run and reported under "resample".  N > 1: ONE population of N x R0 replicas sharded over the N GPUs, rank =
+partition (the paper's partitioned redistribution): weak scaling.
 """
 import argparse
 import json
@@ -211,13 +211,13 @@ def resample_leg(binding, torch, peaks, repeats=5):
                          "frac_vs_8000": alg_bytes / (chain * 1e-3) / 1e9 / 8000.0}}
 
 
-def e2e_leg(pa, torch, wl, first_step, steps):
+def e2e_leg(pa, torch, wl, first_step, steps, step_fn=None):
     """same metric through the C ABI with HOST buffers: every step uploads the population from pinned host memory
     (pa_set_spins), runs pa_step, and reads the new population + E, M back to pinned host memory."""
-    cap_words = (pa.R + 65536) * pa.wpr
-    host_pop = torch.empty(cap_words, dtype=torch.int32).pin_memory()
-    host_E = torch.empty(pa.R + 65536, dtype=torch.int32).pin_memory()
-    host_M = torch.empty(pa.R + 65536, dtype=torch.int32).pin_memory()
+    room = pa.R + max(65536, pa.R // 2)  # a shard's population may grow past its initial share
+    host_pop = torch.empty(room * pa.wpr, dtype=torch.int32).pin_memory()
+    host_E = torch.empty(room, dtype=torch.int32).pin_memory()
+    host_M = torch.empty(room, dtype=torch.int32).pin_memory()
     R = pa.R
     pa.spins_into_host_tensor(host_pop, R)
     betas = schedule(wl, first_step, steps)
@@ -228,7 +228,7 @@ def e2e_leg(pa, torch, wl, first_step, steps):
     for b in betas:
         pa.set_spins_host_tensor(host_pop, R)            # H2D: R*S bytes
         h2d += R * pa.wpr * 4
-        pa.step(b, wl.theta)
+        (step_fn or pa.step)(b, wl.theta)
         R = pa.R
         pa.spins_into_host_tensor(host_pop, R)           # D2H: R'*S bytes
         pa.energies_into_host_tensors(host_E, host_M, R)  # D2H: 8 R' bytes
@@ -314,12 +314,35 @@ def policies_leg(binding, torch, out_csv=None):
     return {"workload": wl.name, "L": wl.L, "R0": wl.R0, "K": wl.K, "theta": wl.theta, "P": wl.P, "policies": summary}
 
 
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without a torchrun environment: start the N ranks ourselves (one process per GPU) --
+    or fail loudly; never report a single-GPU number as an N-GPU one."""
+    import socket
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < args.gpus:
+        sys.stderr.write("bench.py: --gpus %d requested but %d CUDA device(s) visible; refusing to run fewer ranks than asked\n"
+                         % (args.gpus, have))
+        return 2
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def run_ours(args):
     import torch
     from paper_2006_00561_b200 import binding, dist
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     g = dist.init_from_env()
+    if g.world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but the launcher started %d rank(s)" % (args.gpus, g.world))
     torch.cuda.set_device(g.local_rank)
     peaks = measured_peaks()
     wl = inputs.CONFIGS[args.config]
@@ -328,10 +351,24 @@ def run_ours(args):
         wl = dataclasses.replace(wl, theta=args.theta, name=wl.name + "_theta%d" % args.theta)
     K, W = args.steps, max(args.warmup, 0)
 
-    pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed + 1000 * g.rank, beta0=wl.beta0,
-                                    flags=binding.PA_PROFILE)
+    # N = 1: one context, the whole schedule queued with one pa_run call.  N > 1: ONE population of N x R0 replicas
+    # sharded over the ranks (rank = partition): per-GPU work is fixed as N grows (weak scaling), and
+    # every step exchanges the ranks' weight sums, their offspring totals and the lattice slices that cross rank
+    # boundaries (dist.ShardedAnnealer).
+    use_shards = g.world > 1 or args.sharded
+    if not use_shards:
+        pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0, flags=binding.PA_PROFILE)
+        run_steps = lambda betas: pa.run(betas, wl.theta)
+    else:
+        sharded = dist.ShardedAnnealer(wl.L, wl.R0 * g.world, seed=wl.seed, beta0=wl.beta0, group=g, flags=binding.PA_PROFILE)
+        pa = sharded.shards[0]
+
+        def run_steps(betas):
+            for b in betas:
+                sharded.step(b, wl.theta)
+            return len(betas)
     if W > 0:
-        pa.run(schedule(wl, 1, W), wl.theta)
+        run_steps(schedule(wl, 1, W))
     pa.profile_read()
     betas = schedule(wl, W + 1, K)
     sampler = ClockSampler(g.local_rank)
@@ -342,7 +379,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     rs0, l0 = pa.replica_steps(), pa.launch_count()
     ev0.record(pa.stream)
-    done = pa.run(betas, wl.theta)
+    done = run_steps(betas)
     ev1.record(pa.stream)
     torch.cuda.synchronize()
     dist.barrier(g)
@@ -386,7 +423,7 @@ def run_ours(args):
     if g.is_main or g.world > 1:
         if not args.no_e2e:
             n_e2e = max(1, min(K, 6))
-            r = e2e_leg(pa, torch, wl, W + K + 1, n_e2e)
+            r = e2e_leg(pa, torch, wl, W + K + 1, n_e2e, sharded.step if use_shards else None)
             e2e_value, _, _ = dist.aggregate_throughput(g, r["attempts"], r["seconds"])
             e2e = {"value": e2e_value, "unit": "attempts/s", "h2d_bytes_per_step": r["h2d_bytes_per_step"],
                    "d2h_bytes_per_step": r["d2h_bytes_per_step"], "steps": n_e2e}
@@ -394,6 +431,8 @@ def run_ours(args):
     beta_now = pa.beta_steps()[0]
     R_final = pa.R
     del pa
+    if use_shards:
+        del sharded
     torch.cuda.empty_cache()
     if g.is_main and g.world == 1:
         if not args.no_resample:
@@ -408,11 +447,16 @@ def run_ours(args):
                 "vs_baseline": None, "dtype": "u32 bit-packed spins, i32 energies, f64 weights", "data": "synthetic",
                 "config": {"workload": wl.name, "L": wl.L, "R0": wl.R0, "dbeta": (wl.beta_K - wl.beta0) / wl.K,
                            "theta": wl.theta, "P": wl.P, "beta_range": [betas[0], betas[-1]],
-                           "parallelism": "replicas only x%d" % g.world,
+                           "parallelism": ("one context, whole schedule queued by pa_run" if not use_shards else
+                                           "ONE population of %d x R0 replicas sharded over %d ranks (rank = partition): per step "
+                                           "all-gather of weight sums and offspring totals + all-to-all-v of the lattice slices "
+                                           "that cross rank boundaries (NCCL point-to-point)" % (g.world, g.world)),
                            "l2": "population %.0f MiB per buffer > 126 MB L2, no flush needed" % (wl.R0 * wl.bytes_per_replica / 2 ** 20)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_total, "roofline": roof, "cpu_baseline": cpu,
                 "resample": resample, "kernels": per_kernel, "anneal": {"lnZ": lnZ, "beta": beta_now, "R": R_final,
                                                                          "replica_steps": replica_steps}}
+        if g.world > 1:
+            line["config"]["R0"] = wl.R0 * g.world
         print(json.dumps(line))
     dist.shutdown(g)
     return 0
@@ -430,6 +474,9 @@ def main():
     ap.add_argument("--theta", type=int, default=0,
                     help="override the sweeps per step of the workload (theta = 1 is the paper's scalability regime, "
                          "PAPER.md:126: resampling and redistribution dominate); 0 = the config's own theta")
+    ap.add_argument("--sharded", action="store_true",
+                    help="drive the step through the multi-GPU path (dist.ShardedAnnealer) even with one rank: exercises the "
+                         "rank = partition protocol on a single GPU")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-resample", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -475,6 +475,18 @@ def test_sharded_ranks_equal_the_single_context(world, L, R0, theta, policy):
             assert np.array_equal(np.asarray(sh.last_counts), np.diag(sh.last_T))
 
 
+def test_sharded_driver_with_one_rank_equals_the_single_context():
+    """the non-emulated driver path (the one torchrun ranks take), world size 1"""
+    b = _binding()
+    from paper_2006_00561_b200 import dist
+    single = b.PopulationAnnealer(32, 3000, seed=4)
+    sh = dist.ShardedAnnealer(32, 3000, seed=4, group=dist.Group())
+    for k in range(1, 5):
+        single.step(0.1 * k, 2)
+        sh.step(0.1 * k, 2)
+        assert np.array_equal(sh.gather_spins(), single.spins()) and sh.log_Z() == single.log_Z()
+
+
 def test_sharded_capacity_failure_is_consistent_and_leaves_the_population_unchanged():
     b = _binding()
     from paper_2006_00561_b200 import dist
