@@ -114,10 +114,13 @@ def schedule(wl, first_step, count):
 # ---------------------------------------------------------------------------------------------------
 # CPU oracle legs (cpu_baseline of our arm; the whole reference arm)
 # ---------------------------------------------------------------------------------------------------
-def oracle_sample_run(wl, R_sample, steps, warmup):
+def oracle_sample_run(wl, R_sample, steps, warmup, threads=None):
     """the oracle, as it stands, on a bounded sample of the workload: same L, dbeta, theta, P; R = R_sample"""
     from oracle import pa_oracle as orc
-    cores = orc.max_threads()
+    all_cores = orc.max_threads()
+    if threads:
+        orc.set_threads(threads)
+    cores = threads or all_cores
     small = wl.scaled(R_sample)
     pa = orc.OraclePA(small.L, small.R0, P=small.P, seed=small.seed, beta0=small.beta0)
     betas = schedule(wl, 1, warmup + steps)
@@ -129,8 +132,22 @@ def oracle_sample_run(wl, R_sample, steps, warmup):
         pa.step(b, wl.theta)
         attempts += wl.theta * wl.N * pa.R
     dt = time.perf_counter() - t0
+    if threads:
+        orc.set_threads(all_cores)
     return {"attempts": attempts, "seconds": dt, "cores": cores, "R_sample": R_sample, "steps": steps,
             "lnZ": pa.lnZ}
+
+
+def oracle_resample_run(R_sample):
+    """the oracle's a1-a6 (Q, tau, Poisson counts, scan, partition table, gather copy) on a bounded sample of config 5;
+    the population is built (untimed) by the oracle itself"""
+    from oracle import pa_oracle as orc
+    wl = inputs.CONFIGS[5].scaled(R_sample)
+    pa = orc.OraclePA(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0)
+    t0 = time.perf_counter()
+    info = pa.resample(wl.beta_K)
+    dt = time.perf_counter() - t0
+    return {"replicas": info["Rnew"], "seconds": dt, "cores": orc.max_threads(), "R_sample": R_sample}
 
 
 def run_reference(args):
@@ -441,6 +458,15 @@ def run_ours(args):
             r = oracle_sample_run(wl, 4096, 24, 1)
             cpu = {"value": r["attempts"] / r["seconds"], "unit": "attempts/s", "cores": r["cores"], "kind": "oracle",
                    "sample": "%s at R=%d (same L, dbeta, theta, P), %d steps, %.1f s" % (wl.name, r["R_sample"], r["steps"], r["seconds"])}
+            r1 = oracle_sample_run(wl, 1024, 4, 1, threads=1)  # the single-thread figure beside the all-core one
+            cpu["single_thread"] = {"value": r1["attempts"] / r1["seconds"], "unit": "attempts/s", "cores": 1,
+                                    "sample": "%s at R=%d, %d steps, %.1f s" % (wl.name, r1["R_sample"], r1["steps"], r1["seconds"])}
+            if resample is not None:
+                rr = oracle_resample_run(1 << 22)
+                resample["cpu_baseline"] = {"value": rr["replicas"] / rr["seconds"], "unit": "resampled replicas/s",
+                                            "cores": rr["cores"], "kind": "oracle",
+                                            "sample": "oracle a1-a6 on config 5 at R=2^22 (same L, beta, dbeta, P), one step, %.2f s"
+                                                      % rr["seconds"]}
     if g.is_main:
         line = {"metric": "spin_flip_attempts_per_s", "value": value, "unit": "attempts/s", "n_gpus": g.world, "steps": K,
                 "warmup": W, "ms_per_step": 1e3 * tmax / K, "higher_is_better": True, "scaling": "weak",

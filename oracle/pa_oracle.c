@@ -277,6 +277,59 @@ void orc_poisson_counts(int64_t R, const double* tau, double scale, uint64_t see
 }
 
 /* ------------------------------------------------------------------------------------------
+ * A4b.  Nearest-integer resampling, one of the "possible modifications of this step" the paper points to
+ * (PAPER.md:54 -> ref. [3]; reading G24):  n_j = floor(lambda_j) + [u_j > 1 - frac(lambda_j)],
+ * frac(lambda) = lambda - floor(lambda), u_j the keyed uniform of chunk 0 of parent j (the same number the Poisson
+ * sampler would use).  E[n_j] = lambda_j like the Poisson rule, but n_j is one of the two integers next to lambda_j,
+ * so the population size fluctuates much less.  floor, the subtractions and the comparison are exact / individually
+ * rounded binary64 operations.
+ * ---------------------------------------------------------------------------------------- */
+uint32_t orc_nearest(double lambda, uint64_t seed, uint32_t step, uint32_t j) {
+  if (!(lambda > 0.0)) return 0u;
+  double fl = floor(lambda);
+  double thr = 1.0 - (lambda - fl);
+  double u = orc_uniform_resample(seed, step, j, 0u);
+  return (uint32_t)fl + (u > thr ? 1u : 0u);
+}
+void orc_nearest_counts(int64_t R, const double* tau, double scale, uint64_t seed, uint32_t step, uint32_t* n) {
+#pragma omp parallel for schedule(static)
+  for (int64_t j = 0; j < R; ++j) n[j] = orc_nearest(tau[j] * scale, seed, step, (uint32_t)j);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * A9.  Adaptive temperature step ("Fluctuations can be made smaller and less frequent using the adaptive
+ * temperature step, as discussed in the papers [4]"; reading G25).  The overlap of the energy histograms at
+ * beta and beta + dbeta, estimated from the population as in ref. [4]:
+ *     alpha(dbeta) = (1/R) sum_j min(1, tau_j(dbeta)),   tau_j by eq. 3-4,
+ * is 1 at dbeta = 0 and decreases with dbeta.  The step is the largest dbeta in (0, dbeta_max] with
+ * alpha(dbeta) >= target, located by `iters` bisection steps on [0, dbeta_max] (dbeta_max itself if it already
+ * satisfies the target).
+ * ---------------------------------------------------------------------------------------- */
+double orc_overlap(int64_t R, const int32_t* E, double dbeta) {
+  double Q = orc_q(R, E, dbeta);
+  double sum = 0.0, comp = 0.0;
+  for (int64_t j = 0; j < R; ++j) {
+    double tau = exp(-dbeta * (double)E[j]) / Q;
+    double w = tau < 1.0 ? tau : 1.0;
+    double t = sum + w;
+    if (fabs(sum) >= fabs(w)) comp += (sum - t) + w;
+    else comp += (w - t) + sum;
+    sum = t;
+  }
+  return (sum + comp) / (double)R;
+}
+double orc_adaptive_dbeta(int64_t R, const int32_t* E, double target, double dbeta_max, int iters) {
+  if (orc_overlap(R, E, dbeta_max) >= target) return dbeta_max;
+  double lo = 0.0, hi = dbeta_max; /* alpha(lo) >= target > alpha(hi) */
+  for (int it = 0; it < iters; ++it) {
+    double mid = 0.5 * (lo + hi);
+    if (orc_overlap(R, E, mid) >= target) lo = mid;
+    else hi = mid;
+  }
+  return lo;
+}
+
+/* ------------------------------------------------------------------------------------------
  * A5.  Offspring placement ("off-springs, as exact copies"; reading G5):
  * off_j = sum_{i<j} n_i, R' = off_R; child slots off_j .. off_j + n_j - 1 are copies of parent j.
  * ---------------------------------------------------------------------------------------- */

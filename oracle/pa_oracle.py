@@ -38,6 +38,10 @@ def lib():
             "orc_uniform_resample": (C.c_double, [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint64]),
             "orc_poisson": (C.c_uint32, [C.c_double, C.c_uint64, C.c_uint32, C.c_uint32]),
             "orc_poisson_counts": (None, [C.c_int64, f64p, C.c_double, C.c_uint64, C.c_uint32, u32p]),
+            "orc_nearest": (C.c_uint32, [C.c_double, C.c_uint64, C.c_uint32, C.c_uint32]),
+            "orc_nearest_counts": (None, [C.c_int64, f64p, C.c_double, C.c_uint64, C.c_uint32, u32p]),
+            "orc_overlap": (C.c_double, [C.c_int64, i32p, C.c_double]),
+            "orc_adaptive_dbeta": (C.c_double, [C.c_int64, i32p, C.c_double, C.c_double, C.c_int]),
             "orc_exclusive_scan": (C.c_int64, [C.c_int64, u32p, u32p]),
             "orc_copy": (None, [C.c_int, C.c_int64, u32p, u32p, u32p, i32p, i32p, u32p, i32p, i32p]),
             "orc_parent_of": (None, [C.c_int64, u32p, u32p, C.c_int64, u32p]),
@@ -145,6 +149,31 @@ def poisson_counts(tau, scale, seed, step):
     lib().orc_poisson_counts(tau.shape[0], _p(tau, C.c_double), float(scale), C.c_uint64(seed), int(step),
                              _p(n, C.c_uint32))
     return n
+
+
+RULE_POISSON, RULE_NEAREST = 0, 1
+ADAPTIVE_ITERS = 40  # bisection steps of the adaptive temperature step (reading G25)
+
+
+def nearest(lam, seed, step, j):
+    return int(lib().orc_nearest(float(lam), C.c_uint64(seed), int(step), int(j)))
+
+
+def nearest_counts(tau, scale, seed, step):
+    tau = _c(tau, np.float64)
+    n = np.zeros(tau.shape[0], np.uint32)
+    lib().orc_nearest_counts(tau.shape[0], _p(tau, C.c_double), float(scale), C.c_uint64(seed), int(step), _p(n, C.c_uint32))
+    return n
+
+
+def overlap(E, dbeta):
+    E = _c(E, np.int32)
+    return float(lib().orc_overlap(E.shape[0], _p(E, C.c_int32), float(dbeta)))
+
+
+def adaptive_dbeta(E, target, dbeta_max, iters=ADAPTIVE_ITERS):
+    E = _c(E, np.int32)
+    return float(lib().orc_adaptive_dbeta(E.shape[0], _p(E, C.c_int32), float(target), float(dbeta_max), int(iters)))
 
 
 def exclusive_scan(n):
@@ -285,7 +314,8 @@ class OraclePA:
     (R_beta_0), Q (eq. 3), tau (eq. 4), theta (MCMC sweeps per temperature)."""
 
     def __init__(self, L, R0, P=1, seed=0, beta0=0.0, capacity=0, spins=None, policy=POLICY_BALANCED, block=1024,
-                 maxexc=1):
+                 maxexc=1, rule=RULE_POISSON):
+        self.rule = int(rule)
         self.L, self.N, self.R0, self.P, self.seed = int(L), int(L) * int(L), int(R0), int(P), int(seed)
         self.capacity = int(capacity) if capacity else default_capacity(self.R0)
         self.policy, self.block, self.maxexc = int(policy), int(block), int(maxexc)
@@ -319,7 +349,10 @@ class OraclePA:
         tau = tau_weights(self.E, dbeta, Q)                          # eq. 4
         scale = float(self.R0) / float(self.R)                       # reading G2
         tau_used = tau if tau_override is None else _c(tau_override, np.float64)
-        n = poisson_counts(tau_used, scale, self.seed, step)        # A4
+        if self.rule == RULE_NEAREST:
+            n = nearest_counts(tau_used, scale, self.seed, step)     # A4b
+        else:
+            n = poisson_counts(tau_used, scale, self.seed, step)    # A4
         off, Rnew = exclusive_scan(n)                                # A5
         if Rnew > self.capacity:
             raise OracleError("capacity")
@@ -354,6 +387,10 @@ class OraclePA:
         info = self.resample(beta_next, tau_override)
         self.equilibrate(theta)
         return info
+
+    def adaptive_beta(self, target, dbeta_max):
+        """A9: the next inverse temperature for a histogram overlap `target`"""
+        return self.beta + adaptive_dbeta(self.E, target, dbeta_max)
 
     def observables(self):
         s = moment_sums(self.E, self.M)

@@ -126,6 +126,7 @@ struct pa_ctx {
   bool dbg_thresholds;  // test hook: pa_debug_set_thresholds
   uint32_t dbg_T4, dbg_T8;
   int scan_grid_max;  // co-resident blocks of k_poisson_scan on this device
+  unsigned red_grid, obs_grid;  // blocks of the two reductions: 4 per SM for large populations, fewer for small ones
   std::vector<EventPair> ev_used, ev_free;
   std::string err, launch_err;
 
@@ -266,7 +267,7 @@ void launch_copy(pa_ctx* c) {
 // mode 0: sums of the new population, a5 (partition table + diagnostics) and the commit of the step; mode 1: sums only
 void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
   Prof p(c, PA_K_OBSERVE);
-  launch(c, "k_observe", k_observe, OBS_GRID, OBS_THREADS, c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.E[0]),
+  launch(c, "k_observe", k_observe, c->obs_grid, OBS_THREADS, c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.E[0]),
          c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]), c->dev<int32_t>(c->lo.M[1]),
          c->dev<unsigned long long>(c->lo.obs_partial), mode, c->N, c->dev<uint32_t>(c->lo.off),
          c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]), c->dev<uint32_t>(c->lo.part_stats),
@@ -288,7 +289,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   span.emplace(c, PA_K_RESAMPLE_SPAN, false);
   {
     Prof p(c, PA_K_Q_REDUCE);  // also resets the step's counters and look-back descriptors
-    launch(c, "k_q_reduce", k_q_reduce, RED_GRID, RED_THREADS, st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
+    launch(c, "k_q_reduce", k_q_reduce, c->red_grid, RED_THREADS, st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
            (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tb);
   }
   {
@@ -476,6 +477,11 @@ int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t
   c->profile = (cfg->flags & PA_PROFILE) != 0;
   c->profile_span = (cfg->flags & PA_PROFILE_SPAN) != 0;
   c->launches = 0;
+  {  // a small population (config 1: 1024 replicas) is latency-bound: one block per 4096 replicas, at most 4 per SM
+    const int64_t want = (c->cap + 4095) / 4096;
+    c->red_grid = (unsigned)(want < 1 ? 1 : (want > RED_GRID ? RED_GRID : want));
+    c->obs_grid = (unsigned)(want < 1 ? 1 : (want > OBS_GRID ? OBS_GRID : want));
+  }
   c->attempt_failed = false;
   c->rank = 0;
   c->world = 0;
@@ -811,7 +817,7 @@ int pa_dist_begin(pa_ctx* c, double beta_next, int32_t theta, pa_dist_partial* m
   const int n_desc = (int)((c->cap + SCAN_TILE - 1) / SCAN_TILE + 1);
   {
     Prof p(c, PA_K_Q_REDUCE);  // a shard: stops at the rank's own sum of weights
-    launch(c, "k_q_reduce", k_q_reduce, RED_GRID, RED_THREADS, st, (const StepParams*)d_params,
+    launch(c, "k_q_reduce", k_q_reduce, c->red_grid, RED_THREADS, st, (const StepParams*)d_params,
            (const int32_t*)c->dev<int32_t>(c->lo.E[0]), (const int32_t*)c->dev<int32_t>(c->lo.E[1]), c->N,
            c->dev<double>(c->lo.red_partial), (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tables(c));
   }

@@ -280,6 +280,71 @@ def test_poisson_degenerate_inputs():
 
 
 # ---------------------------------------------------------------------------------------------------
+# A4b nearest-integer resampling, A9 adaptive temperature step (readings G24, G25)
+# ---------------------------------------------------------------------------------------------------
+def test_nearest_integer_resampling():
+    seed, step = 4242, 6
+    for lam in [0.0, 0.3, 1.0, 2.75, 17.5, 1234.001]:
+        n = np.array([orc.nearest(lam, seed, step, j) for j in range(20000)])
+        assert set(np.unique(n)) <= {math.floor(lam), math.floor(lam) + 1}   # one of the two neighbouring integers
+        f = lam - math.floor(lam)
+        assert abs(n.mean() - lam) <= 5 * math.sqrt(max(f * (1 - f), 1e-12) / n.size) + 1e-12   # E[n] = lambda
+        if f == 0.0:
+            assert np.all(n == int(lam))                                     # integer lambda: no randomness at all
+    # the decision uses the keyed uniform of chunk 0 of parent j: n = floor + [u > 1 - frac]
+    lam = 3.37
+    for j in [0, 5, 999]:
+        u = orc.uniform_resample(seed, step, j, 0)
+        assert orc.nearest(lam, seed, step, j) == 3 + (1 if u > 1.0 - (lam - 3.0) else 0)
+    assert orc.nearest(-1.0, 1, 1, 0) == 0 and orc.nearest(float("nan"), 1, 1, 0) == 0
+    # population size: sum_j n_j stays within a few sqrt(R/4) of R0 (Poisson: sqrt(R0))
+    rng = np.random.default_rng(1)
+    tau = rng.gamma(2.0, 0.5, 50000)
+    tau *= tau.size / tau.sum()
+    tot = int(orc.nearest_counts(tau, 1.0, seed, step).sum())
+    assert abs(tot - tau.size) < 5 * math.sqrt(tau.size / 4)
+    pa = orc.OraclePA(8, 2000, seed=3, rule=orc.RULE_NEAREST)
+    sizes = [pa.step(0.05 * k, 2)["Rnew"] for k in range(1, 11)]
+    assert max(abs(s - 2000) for s in sizes) < 5 * math.sqrt(2000 / 4)
+    assert abs(pa.lnZ - float(exact_ising.kaufman_lnZ(8, 0.5))) < 0.5         # still a valid PA estimate of ln Z
+
+
+def test_overlap_closed_forms_and_adaptive_step():
+    # all energies equal: every tau = 1 -> overlap 1 for any dbeta
+    E = np.full(500, -24, np.int32)
+    assert orc.overlap(E, 0.3) == 1.0
+    # two levels: a replicas at E1, b at E2 (E1 < E2, dbeta > 0): tau1 > 1 > tau2 -> alpha = (a + b tau2) / (a + b)
+    a, b, E1, E2, db = 300, 700, -64, 16, 0.02
+    E = np.array([E1] * a + [E2] * b, np.int32)
+    w1, w2 = mp.exp(-mpf(db) * E1), mp.exp(-mpf(db) * E2)
+    Q = (a * w1 + b * w2) / (a + b)
+    want = float((a + b * w2 / Q) / (a + b))
+    assert abs(orc.overlap(E, db) - want) <= 1e-14
+    rng = np.random.default_rng(12)
+    E = (4 * rng.integers(-300, 300, 20000)).astype(np.int32)
+    assert orc.overlap(E, 0.0) == 1.0
+    al = [orc.overlap(E, d) for d in [0.0005, 0.001, 0.002, 0.004, 0.008]]
+    assert all(x > y for x, y in zip(al, al[1:])) and 0 < al[-1] < al[0] < 1   # decreasing in dbeta
+    # independent writing with numpy: alpha = mean(min(1, tau))
+    tau = np.exp(-0.002 * E.astype(np.float64))
+    tau /= tau.mean()
+    assert abs(orc.overlap(E, 0.002) - np.minimum(1.0, tau).mean()) <= 1e-13
+    # the adaptive step brackets the target
+    for target in [0.95, 0.85, 0.6]:
+        d = orc.adaptive_dbeta(E, target, 0.05)
+        assert 0 < d < 0.05 and orc.overlap(E, d) >= target > orc.overlap(E, d * (1 + 1e-9) + 1e-12)
+    assert orc.adaptive_dbeta(E, 0.01, 0.001) == 0.001          # dbeta_max already satisfies the target
+    # inside the loop: steps shrink where the energy distribution is wide (critical region) -- PAPER.md:108
+    pa = orc.OraclePA(16, 3000, seed=8)
+    steps = []
+    while pa.beta < 0.6 and len(steps) < 200:
+        nb = pa.adaptive_beta(0.85, 0.05)
+        steps.append(nb - pa.beta)
+        pa.step(nb, 2)
+    assert pa.beta >= 0.6 and min(steps) < 0.5 * max(steps)
+
+
+# ---------------------------------------------------------------------------------------------------
 # A5 scan / copy, A6 partitions
 # ---------------------------------------------------------------------------------------------------
 def test_scan_copy_parent_plain_definitions():
