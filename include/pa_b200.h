@@ -50,7 +50,9 @@ enum {
   PA_KEEP_COUNTS = 2u, /* materialise n_j of every step (4 B per parent) for pa_counts(n != NULL) */
   PA_PROFILE = 4u,     /* record CUDA events around every kernel (pa_profile_read); the events between the kernels
                           keep a kernel's blocks from being placed while its predecessor drains */
-  PA_PROFILE_SPAN = 8u /* record only the PA_K_RESAMPLE_SPAN pair around a1-a6 of every step */
+  PA_PROFILE_SPAN = 8u, /* record only the PA_K_RESAMPLE_SPAN pair around a1-a6 of every step */
+  PA_RESAMPLE_NEAREST = 16u /* copy counts n_j = floor(lambda_j) + [u_j > 1 - frac(lambda_j)] (nearest integers) instead of
+                               Poisson(lambda_j): one of the modifications PAPER.md:54 points to; A4b */
 };
 
 /* Redistribution policies (A6b, readings G21-G23).  The children are in parent order and a
@@ -133,6 +135,11 @@ int pa_step(pa_ctx* ctx, double beta_next, int32_t theta);
  * end; stops committing at the first failing step (later steps are no-ops) and reports it.  *steps_done (may be
  * NULL) receives the number of committed steps. */
 int pa_run(pa_ctx* ctx, const double* betas, int32_t K, int32_t theta, int32_t* steps_done);
+
+/* Adaptive temperature step (A9): *beta_next = beta + the largest dbeta in (0, dbeta_max] whose
+ * histogram overlap alpha(dbeta) = (1/R) sum_j min(1, tau_j(dbeta)) is >= target_overlap (40 bisection steps on
+ * [0, dbeta_max]).  Only proposes the temperature: follow with pa_step(*beta_next, theta).  Synchronises. */
+int pa_adaptive_beta(pa_ctx* ctx, double target_overlap, double dbeta_max, double* beta_next);
 
 int pa_population(pa_ctx* ctx, int64_t* R);
 int pa_beta(pa_ctx* ctx, double* beta, int64_t* steps);

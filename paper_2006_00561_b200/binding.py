@@ -12,11 +12,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libpa_b200.so")
 
 PA_OK, PA_EINVAL, PA_ENOMEM, PA_ECAPACITY, PA_EEXTINCT, PA_ECUDA = 0, -1, -2, -3, -4, -5
-PA_KEEP_TAU, PA_KEEP_COUNTS, PA_PROFILE, PA_PROFILE_SPAN = 1, 2, 4, 8
+PA_KEEP_TAU, PA_KEEP_COUNTS, PA_PROFILE, PA_PROFILE_SPAN, PA_RESAMPLE_NEAREST = 1, 2, 4, 8, 16
 PA_POLICY_BALANCED, PA_POLICY_MAIN, PA_POLICY_NAIVE, PA_POLICY_NONE = 0, 1, 2, 3
 KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "copy", "sweep", "observe", "resample_span"]
 
-EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
+EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_adaptive_beta", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
            "pa_observables", "pa_spins", "pa_tau", "pa_counts", "pa_parents", "pa_partitions", "pa_thresholds",
            "pa_set_spins", "pa_debug_set_thresholds", "pa_dist_init", "pa_dist_workspace_bytes", "pa_dist_begin",
            "pa_dist_resample", "pa_dist_exchange_plan", "pa_dist_buffers", "pa_dist_finish", "pa_dist_new_count",
@@ -65,6 +65,7 @@ def load_library():
         "pa_init": (C.c_int, [C.POINTER(PaConfig), C.POINTER(vp)]),
         "pa_step": (C.c_int, [vp, C.c_double, C.c_int32]),
         "pa_run": (C.c_int, [vp, f64p, C.c_int32, C.c_int32, i32p]),
+        "pa_adaptive_beta": (C.c_int, [vp, C.c_double, C.c_double, f64p]),
         "pa_population": (C.c_int, [vp, i64p]),
         "pa_beta": (C.c_int, [vp, f64p, i64p]),
         "pa_totals": (C.c_int, [vp, i64p]),
@@ -183,6 +184,11 @@ class PopulationAnnealer:
     # ---- the path --------------------------------------------------------------------------------
     def step(self, beta_next, theta):
         self._check(self._lib.pa_step(self._ctx, float(beta_next), int(theta)))
+
+    def adaptive_beta(self, target_overlap, dbeta_max):
+        b = C.c_double(0)
+        self._check(self._lib.pa_adaptive_beta(self._ctx, float(target_overlap), float(dbeta_max), C.byref(b)))
+        return float(b.value)
 
     def run(self, betas, theta):
         b = np.ascontiguousarray(betas, np.float64)

@@ -28,7 +28,7 @@ constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
   uint64_t state, params, spins[2], E[2], M[2], off, n, tau, tile_desc, tile_parent, parent_of, red_partial, obs_partial,
-      lev_tau, lev_mu, lev_m, lev_cdf, part[2], part_stats, total;
+      lev_tau, lev_mu, lev_m, lev_cdf, lev_hist, part[2], part_stats, total;
 };
 
 inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
@@ -88,6 +88,7 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   lo->lev_mu = take(nlev * 8);
   lo->lev_m = take(nlev * 4);
   lo->lev_cdf = take(nlev * PO_ROW * 8);
+  lo->lev_hist = take(nlev * 4);  // level histogram of the adaptive temperature step (all zero between calls)
   for (int b = 0; b < 2; ++b) lo->part[b] = take(((uint64_t)c->P + 1) * 4);
   lo->part_stats = take((uint64_t)c->P * 16);
   lo->total = o;
@@ -116,6 +117,7 @@ struct pa_ctx {
   double beta, sum_lnQ, last_Q;
   int64_t launches;
   bool profile, profile_span;
+  int nearest;  // PA_RESAMPLE_NEAREST: nearest-integer copy counts instead of Poisson
   bool attempt_failed;  // the last pa_step / pa_run ended with an uncommitted step: off / n / tau hold that attempt
   // multi-GPU shard (pa_dist_*): rank = partition
   int rank, world;          // world = 0: not a shard
@@ -290,7 +292,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   {
     Prof p(c, PA_K_Q_REDUCE);  // also resets the step's counters and look-back descriptors
     launch(c, "k_q_reduce", k_q_reduce, c->red_grid, RED_THREADS, st, sp, E0, E1, N, c->dev<double>(c->lo.red_partial),
-           (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tb);
+           (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tb, c->nearest);
   }
   {
     // persistent blocks pull tiles from a ticket counter
@@ -313,10 +315,10 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     const unsigned long long cap = (unsigned long long)c->cap;
     const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? (tiles_cap ? tiles_cap : 1u) : (unsigned)c->scan_grid_max;
     Prof p(c, PA_K_POISSON_SCAN);
-    if (keep && theta > 0) launch(c, "k_poisson_scan", k_poisson_scan<true, true>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key);
-    else if (keep) launch(c, "k_poisson_scan", k_poisson_scan<true, false>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key);
-    else if (theta > 0) launch(c, "k_poisson_scan", k_poisson_scan<false, true>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key);
-    else launch(c, "k_poisson_scan", k_poisson_scan<false, false>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key);
+    if (keep && theta > 0) launch(c, "k_poisson_scan", k_poisson_scan<true, true>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key, c->nearest);
+    else if (keep) launch(c, "k_poisson_scan", k_poisson_scan<true, false>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key, c->nearest);
+    else if (theta > 0) launch(c, "k_poisson_scan", k_poisson_scan<false, true>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key, c->nearest);
+    else launch(c, "k_poisson_scan", k_poisson_scan<false, false>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key, c->nearest);
   }
   if (theta == 0) launch_copy(c);  // a6; with sweeps to follow it is fused into the sweep's load
   span.reset();
@@ -476,6 +478,7 @@ int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t
   c->stream = static_cast<cudaStream_t>(cfg->stream);
   c->profile = (cfg->flags & PA_PROFILE) != 0;
   c->profile_span = (cfg->flags & PA_PROFILE_SPAN) != 0;
+  c->nearest = (cfg->flags & PA_RESAMPLE_NEAREST) ? 1 : 0;
   c->launches = 0;
   {  // a small population (config 1: 1024 replicas) is latency-bound: one block per 4096 replicas, at most 4 per SM
     const int64_t want = (c->cap + 4095) / 4096;
@@ -523,6 +526,7 @@ int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t
     c->launches += 1;
   }
   CK(cudaMemsetAsync(c->dev<char>(c->lo.part_stats), 0, (size_t)cfg->P * 16, c->stream));
+  CK(cudaMemsetAsync(c->dev<char>(c->lo.lev_hist), 0, ((size_t)c->N + 1) * 4, c->stream));
   {
     const int bpr = (c->wrep + 3) / 4;
     const uint64_t threads = (uint64_t)cfg->R0 * bpr;
@@ -687,6 +691,22 @@ int pa_thresholds(pa_ctx* c, uint32_t* T4, uint32_t* T8) {
   return PA_OK;
 }
 
+int pa_adaptive_beta(pa_ctx* c, double target_overlap, double dbeta_max, double* beta_next) {
+  if (!c || !beta_next) return PA_EINVAL;
+  if (!(target_overlap > 0.0 && target_overlap < 1.0) || !(dbeta_max > 0.0) || !(dbeta_max * 2.0 * c->N < 700.0))
+    return fail(c, PA_EINVAL, "pa_adaptive_beta: need 0 < target < 1 and 0 < dbeta_max with dbeta_max*2N < 700");
+  if (c->world > 0) return fail(c, PA_EINVAL, "pa_adaptive_beta: not available on a multi-GPU shard");
+  if (int rc = bind_device(c)) return rc;
+  DevState* st = c->dev<DevState>(c->lo.state);
+  unsigned* hist = c->dev<unsigned>(c->lo.lev_hist);
+  k_level_hist<<<c->obs_grid, OBS_THREADS, 0, c->stream>>>(st, c->dev<int32_t>(c->lo.E[0]), c->dev<int32_t>(c->lo.E[1]), hist, c->N);
+  k_adaptive_step<<<1, OBS_THREADS, 0, c->stream>>>(st, hist, c->N, target_overlap, dbeta_max, 40);
+  c->launches += 2;
+  if (int rc = sync_state(c)) return rc;
+  *beta_next = c->beta + c->h_state->adaptive_dbeta;
+  return PA_OK;
+}
+
 int pa_debug_set_thresholds(pa_ctx* c, int enable, uint32_t T4, uint32_t T8) {
   if (!c) return PA_EINVAL;
   c->dbg_thresholds = enable != 0;
@@ -819,7 +839,7 @@ int pa_dist_begin(pa_ctx* c, double beta_next, int32_t theta, pa_dist_partial* m
     Prof p(c, PA_K_Q_REDUCE);  // a shard: stops at the rank's own sum of weights
     launch(c, "k_q_reduce", k_q_reduce, c->red_grid, RED_THREADS, st, (const StepParams*)d_params,
            (const int32_t*)c->dev<int32_t>(c->lo.E[0]), (const int32_t*)c->dev<int32_t>(c->lo.E[1]), c->N,
-           c->dev<double>(c->lo.red_partial), (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tables(c));
+           c->dev<double>(c->lo.red_partial), (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tables(c), c->nearest);
   }
   if (int rc = sync_state(c)) return rc;
   mine->sumw = c->h_state->sumw;
@@ -847,7 +867,7 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
   const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
   {
     Prof p(c, PA_K_LEVELS_TAU);
-    launch(c, "k_dist_tables", k_dist_tables, 1u, RED_THREADS, st, d_params, c->N, sumw, (double)R, (double)c->g_R0, tb);
+    launch(c, "k_dist_tables", k_dist_tables, 1u, RED_THREADS, st, d_params, c->N, sumw, (double)R, (double)c->g_R0, tb, c->nearest);
   }
   {
     const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
@@ -869,8 +889,8 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
     const unsigned long long cap = (unsigned long long)c->cap;
     const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? (tiles_cap ? tiles_cap : 1u) : (unsigned)c->scan_grid_max;
     Prof p(c, PA_K_POISSON_SCAN);
-    if (keep) launch(c, "k_poisson_scan", k_poisson_scan<true, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
-    else launch(c, "k_poisson_scan", k_poisson_scan<false, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
+    if (keep) launch(c, "k_poisson_scan", k_poisson_scan<true, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key, c->nearest);
+    else launch(c, "k_poisson_scan", k_poisson_scan<false, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key, c->nearest);
   }
   launch_copy(c);  // the rank's offspring, expanded in child order, into the spare buffer: the send side of the exchange
   CK(cudaMemcpyAsync(c->h_state, st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));

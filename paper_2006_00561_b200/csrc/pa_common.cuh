@@ -41,6 +41,7 @@ struct DevState {
   int lev_lo, lev_hi;            // occupied energy levels (E + 2N)/4 of the CURRENT population, inclusive (by k_observe)
   unsigned int pad_[1];
   double Q_committed;            // Q of the last COMMITTED step (Q above is overwritten by every attempt)
+  double adaptive_dbeta;         // result of the last k_adaptive_step
 };
 
 struct StepParams {

@@ -303,4 +303,65 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Adaptive temperature step (PAPER.md:108 -> ref. [4]; A9, reading G25): the largest dbeta in (0, dbeta_max]
+// whose histogram overlap alpha(dbeta) = (1/R) sum_j min(1, tau_j(dbeta)) is >= target.  tau_j depends on j only through
+// the energy level, so one pass builds the level histogram of the population (k_level_hist) and one block bisects on it
+// (k_adaptive_step): 40 halvings, each two block reductions over the occupied levels.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(OBS_THREADS)
+k_level_hist(const DevState* __restrict__ st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1,
+             unsigned* __restrict__ hist, const int N) {
+  const int32_t* __restrict__ E = st->cur ? E1 : E0;
+  const unsigned long long R = st->R;
+  const unsigned long long stride = (unsigned long long)gridDim.x * OBS_THREADS;
+  for (unsigned long long j = (unsigned long long)blockIdx.x * OBS_THREADS + threadIdx.x; j < R; j += stride)
+    atomicAdd(&hist[(E[j] + 2 * N) >> 2], 1u);
+}
+
+__device__ __forceinline__ double block_sum_256(double v, double* s_red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();  // s_red of the previous call has been consumed
+  if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double t = 0.0;
+#pragma unroll
+  for (int w = 0; w < OBS_THREADS / 32; ++w) t += s_red[w];
+  return t;
+}
+
+__global__ void __launch_bounds__(OBS_THREADS)
+k_adaptive_step(DevState* st, unsigned* __restrict__ hist, const int N, const double target, const double dbeta_max,
+                const int iters) {
+  __shared__ double s_red[OBS_THREADS / 32];
+  const int lev_lo = st->lev_lo, lev_hi = st->lev_hi;
+  const double R = (double)st->R;
+  auto overlap = [&](double dbeta) {
+    double sw = 0.0;
+    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += OBS_THREADS)
+      sw += (double)hist[lev] * exp(-dbeta * (double)(4 * lev - 2 * N));
+    const double Q = block_sum_256(sw, s_red) / R;
+    double sa = 0.0;
+    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += OBS_THREADS) {
+      const double tau = exp(-dbeta * (double)(4 * lev - 2 * N)) / Q;
+      sa += (double)hist[lev] * (tau < 1.0 ? tau : 1.0);
+    }
+    return block_sum_256(sa, s_red) / R;
+  };
+  double result = dbeta_max;
+  if (!(overlap(dbeta_max) >= target)) {
+    double lo = 0.0, hi = dbeta_max;  // alpha(lo) >= target > alpha(hi)
+    for (int it = 0; it < iters; ++it) {
+      const double mid = 0.5 * (lo + hi);
+      if (overlap(mid) >= target) lo = mid;  // block-uniform: every thread holds the same sums
+      else hi = mid;
+    }
+    result = lo;
+  }
+  __syncthreads();
+  for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += OBS_THREADS) hist[lev] = 0u;  // ready for the next call
+  if (threadIdx.x == 0) st->adaptive_dbeta = result;
+}
+
 }  // namespace pa

@@ -52,7 +52,8 @@ __device__ __forceinline__ double expneg_a4(double mu) {
   return p;
 }
 
-__device__ __forceinline__ void level_tables(double dbeta, int lev, int N, double Q, double scale, const LevelTables& tb) {
+__device__ __forceinline__ void level_tables(double dbeta, int lev, int N, double Q, double scale, const LevelTables& tb,
+                                             const bool nearest) {
   const double tau = __ddiv_rn(level_weight(dbeta, lev, N), Q);
   const double lambda = __dmul_rn(tau, scale);
   tb.tau[lev] = tau;
@@ -65,6 +66,16 @@ __device__ __forceinline__ void level_tables(double dbeta, int lev, int N, doubl
   if (!(lambda < 2147483648.0)) {  // would exceed any capacity: reported as PA_ECAPACITY if a replica sits here
     tb.m[lev] = M_OVERFLOW;
     tb.mu[lev] = 0.0;
+    return;
+  }
+  if (nearest) {  // A4b: n = floor(lambda) + [u > 1 - frac(lambda)]: one uniform per parent, never a heavy parent
+    const double fl = floor(lambda);
+    tb.m[lev] = 1u;
+    tb.mu[lev] = lambda;
+    F[0] = __dsub_rn(1.0, __dsub_rn(lambda, fl));              // threshold
+    F[1] = __longlong_as_double((long long)fl);                // floor(lambda) as an integer bit pattern
+    F[2] = 2.0;
+    F[3] = 2.0;
     return;
   }
   long long m = (long long)ceil(__ddiv_rn(lambda, 8.0));
@@ -111,7 +122,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 __global__ void __launch_bounds__(RED_THREADS)
 k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
            const int32_t* __restrict__ E1, int N, double* __restrict__ partial, double R0,
-           unsigned long long* __restrict__ tile_desc, int n_desc, LevelTables tb) {
+           unsigned long long* __restrict__ tile_desc, int n_desc, LevelTables tb, int nearest) {
   grid_dependency_wait();
   const unsigned long long tid = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x;
   const unsigned long long stride = (unsigned long long)gridDim.x * RED_THREADS;
@@ -210,7 +221,7 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
   {
     const double Q = s_Q, scale = R0 / (double)R;
     const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
-    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(dbeta, lev, N, Q, scale, tb);
+    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(dbeta, lev, N, Q, scale, tb, nearest != 0);
   }
 }
 
@@ -222,7 +233,7 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(RED_THREADS)
 k_dist_tables(DevState* st, const StepParams* __restrict__ sp, int N, double sumw_global, double R_global, double R0,
-              LevelTables tb) {
+              LevelTables tb, int nearest) {
   grid_dependency_wait();
   if (st->status != ST_OK) return;
   const double Q = sumw_global / R_global, scale = R0 / R_global;
@@ -232,7 +243,7 @@ k_dist_tables(DevState* st, const StepParams* __restrict__ sp, int N, double sum
     st->scale = scale;
   }
   const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
-  for (int lev = st->lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(sp->dbeta, lev, N, Q, scale, tb);
+  for (int lev = st->lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(sp->dbeta, lev, N, Q, scale, tb, nearest != 0);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -314,7 +325,7 @@ constexpr unsigned NO_TILE = 0xffffffffu;
 template <bool KEEP, bool MAP>
 __global__ void __launch_bounds__(SCAN_THREADS, (MAP ? PA_SCAN_MINB - 1 : PA_SCAN_MINB))
 k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
-               ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key) {
+               ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key, int nearest) {
   grid_dependency_wait();
   if (st->status != ST_OK) return;
   __shared__ unsigned s_tile;
@@ -398,7 +409,10 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           k[b] = c4[b];
-          if (c4[b] == 4u)
+          if (nearest) {  // A4b (block-uniform): n = floor(lambda) + [u > 1 - frac(lambda)], both from the head of the row
+            const double* F = (ALL || hl[b] < (unsigned)SCAN_HW) ? &s_head[hl[b]][0] : tb.cdf + (size_t)(hl[b] + (unsigned)lev_lo) * PO_ROW;
+            k[b] = (unsigned)__double_as_longlong(F[1]) + (u[b] > F[0] ? 1u : 0u);
+          } else if (c4[b] == 4u)
             k[b] += cdf_search_from(reinterpret_cast<const double2*>(tb.cdf + (size_t)(hl[b] + (unsigned)lev_lo) * PO_ROW), 1, u[b]);
           if (m[b] == M_OVERFLOW) {
             s_flag = 1u;

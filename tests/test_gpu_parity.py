@@ -31,14 +31,15 @@ def rel(a, b):
     return abs(a - b) / max(abs(b), 1e-300)
 
 
-def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None, policy=0, block=1024, maxexc=1):
+def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None, policy=0, block=1024, maxexc=1, rule=0):
     b = _binding()
     gpu = b.PopulationAnnealer(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity,
-                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS, policy=policy, block=block, maxexc=maxexc)
+                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS | (b.PA_RESAMPLE_NEAREST if rule else 0), policy=policy,
+                               block=block, maxexc=maxexc)
     if spins is not None:
         gpu.set_spins(spins)
     ora = orc.OraclePA(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity, spins=spins, policy=policy, block=block,
-                       maxexc=maxexc)
+                       maxexc=maxexc, rule=rule)
     return gpu, ora
 
 
@@ -411,6 +412,44 @@ def test_failed_step_does_not_leak_into_the_getters():
             pass
     n, off = g.counts()
     assert int(n.sum()) == g.R == int(off[-1])
+
+
+# ---------------------------------------------------------------------------------------------------
+# variants of the step: nearest-integer resampling, adaptive temperature step
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,R0,P,theta", [(8, 3000, 1, 2), (32, 4099, 7, 1), (64, 2048, 148, 2)])
+def test_nearest_integer_resampling_lockstep(L, R0, P, theta):
+    gpu, ora = make_pair(L, R0, P, seed=61 + L, rule=1)
+    lockstep(gpu, ora, [0.07 * k for k in range(1, 8)], theta)
+    assert abs(gpu.R - R0) < 5 * math.sqrt(R0 / 4)  # the population size barely moves under this rule
+
+
+def test_nearest_integer_resampling_heavy_parents():
+    # skewed weights: lambda up to hundreds -- the rule has no chunk loop, one uniform per parent whatever lambda is
+    L, R = 32, 20000
+    pop = inputs.random_packed_population(L, R, seed=5)
+    pop[np.random.default_rng(7).choice(R, 64, replace=False)] = inputs.structured_population(L, 64, seed=6)
+    gpu, ora = make_pair(L, R, P=3, seed=55, beta0=0.3, spins=pop, capacity=40960, rule=1)
+    lockstep(gpu, ora, [0.304, 0.31], 1)
+    assert gpu.counts()[0].max() > 8
+
+
+@pytest.mark.parametrize("L,R0", [(16, 4000), (64, 3000)])
+def test_adaptive_temperature_step(L, R0):
+    """pa_adaptive_beta against the oracle's bisection on the same population, then a lock-step step to that temperature;
+    the steps must shrink in the critical region"""
+    gpu, ora = make_pair(L, R0, 5, seed=23)
+    dbeta_max = min(0.05, 600.0 / (2 * L * L))
+    steps = []
+    while gpu.beta_steps()[0] < 0.46 and len(steps) < 250:  # past beta_c = 0.4407
+        b_gpu = gpu.adaptive_beta(0.85, dbeta_max)
+        b_ora = ora.adaptive_beta(0.85, dbeta_max)
+        assert rel(b_gpu - ora.beta, b_ora - ora.beta) <= 1e-9, (b_gpu, b_ora)  # the bisection grids coincide unless a tie
+        steps.append(b_gpu - ora.beta)
+        lockstep(gpu, ora, [b_gpu], 1)
+    assert gpu.beta_steps()[0] >= 0.46 and min(steps) < 0.7 * max(steps)
+    with pytest.raises(_binding().PaError):
+        gpu.adaptive_beta(1.5, 0.01)
 
 
 # ---------------------------------------------------------------------------------------------------
