@@ -27,7 +27,7 @@ constexpr int RED_GRID = PA_RED_GRID;
 constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
-  uint64_t state, params, spins[2], E[2], M[2], off, n, tau, tile_desc, tile_parent, parent_of, red_partial, obs_partial,
+  uint64_t state, params, spins[2], EM[2], off, n, tau, tile_desc, tile_parent, parent_of, red_partial, obs_partial,
       lev_tau, lev_mu, lev_m, lev_cdf, lev_hist, part[2], part_stats, total;
 };
 
@@ -73,9 +73,8 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   };
   lo->state = take(sizeof(DevState));
   lo->params = take(sizeof(StepParams) * RUN_CHUNK);
-  for (int b = 0; b < 2; ++b) lo->spins[b] = take(ucap * S);
-  for (int b = 0; b < 2; ++b) lo->E[b] = take(ucap * 4);
-  for (int b = 0; b < 2; ++b) lo->M[b] = take(ucap * 4);
+  for (int b = 0; b < 2; ++b) lo->spins[b] = take(ucap * S + 64);  // + 64: the spare buffer doubles as the E / M staging area of pa_energies (8 n + 12 bytes at L = 8)
+  for (int b = 0; b < 2; ++b) lo->EM[b] = take(ucap * 4);  // packed E/4 : M/2, one word per replica
   lo->off = take((ucap + 1) * 4);
   lo->n = (c->flags & PA_KEEP_COUNTS) ? take(ucap * 4) : 0;
   lo->tau = (c->flags & PA_KEEP_TAU) ? take(ucap * 8) : 0;
@@ -221,17 +220,16 @@ void launch(pa_ctx* c, const char* name, void (*kern)(KArgs...), unsigned grid, 
 template <int L>
 void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
   uint32_t *s0 = c->dev<uint32_t>(c->lo.spins[0]), *s1 = c->dev<uint32_t>(c->lo.spins[1]);
-  int32_t *e0 = c->dev<int32_t>(c->lo.E[0]), *e1 = c->dev<int32_t>(c->lo.E[1]);
-  int32_t *m0 = c->dev<int32_t>(c->lo.M[0]), *m1 = c->dev<int32_t>(c->lo.M[1]);
+  int32_t *em0 = c->dev<int32_t>(c->lo.EM[0]), *em1 = c->dev<int32_t>(c->lo.EM[1]);
   const DevState* st = c->dev<DevState>(c->lo.state);
   const uint32_t* parent_of = c->dev<uint32_t>(c->lo.parent_of);
   if constexpr (L >= 64) {
     const unsigned grid = (unsigned)(((uint64_t)c->cap + Geo<L>::RPB - 1) / Geo<L>::RPB);
-    launch(c, "k_sweep", k_sweep<L>, grid, SWEEP_THREADS, st, s0, s1, e0, e1, m0, m1, c->key, sa, parent_of);
+    launch(c, "k_sweep", k_sweep<L>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of);
   } else {
     const uint64_t threads = ((uint64_t)c->cap + 1) / 2 * SGeo<L>::G;  // a group of G lanes holds two replicas
     const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
-    launch(c, "k_sweep_small", k_sweep_small<L>, grid, SWEEP_THREADS, st, s0, s1, e0, e1, m0, m1, c->key, sa, parent_of);
+    launch(c, "k_sweep_small", k_sweep_small<L>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of);
   }
 }
 // mode 2: theta sweeps of the resampled population (lattices gathered from the parents' slots); mode 1: energies only
@@ -252,8 +250,7 @@ void launch_copy_L(pa_ctx* c) {
   const unsigned grid = (unsigned)((c->cap + CopyGeo<L>::CT - 1) / CopyGeo<L>::CT);
   launch(c, "k_copy", k_copy<L>, grid, COPY_THREADS, c->dev<DevState>(c->lo.state), c->dev<uint32_t>(c->lo.off),
          c->dev<uint32_t>(c->lo.tile_parent), c->dev<uint32_t>(c->lo.spins[0]), c->dev<uint32_t>(c->lo.spins[1]),
-         c->dev<int32_t>(c->lo.E[0]), c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]),
-         c->dev<int32_t>(c->lo.M[1]));
+         c->dev<int32_t>(c->lo.EM[0]), c->dev<int32_t>(c->lo.EM[1]));
 }
 void launch_copy(pa_ctx* c) {
   Prof p(c, PA_K_COPY);
@@ -269,11 +266,27 @@ void launch_copy(pa_ctx* c) {
 // mode 0: sums of the new population, a5 (partition table + diagnostics) and the commit of the step; mode 1: sums only
 void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
   Prof p(c, PA_K_OBSERVE);
-  launch(c, "k_observe", k_observe, c->obs_grid, OBS_THREADS, c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.E[0]),
-         c->dev<int32_t>(c->lo.E[1]), c->dev<int32_t>(c->lo.M[0]), c->dev<int32_t>(c->lo.M[1]),
+  launch(c, "k_observe", k_observe, c->obs_grid, OBS_THREADS, c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.EM[0]),
+         c->dev<int32_t>(c->lo.EM[1]),
          c->dev<unsigned long long>(c->lo.obs_partial), mode, c->N, c->dev<uint32_t>(c->lo.off),
          c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]), c->dev<uint32_t>(c->lo.part_stats),
          BalanceArgs{c->cfg.P, (int)c->cfg.policy, c->cfg.block ? c->cfg.block : 1024u, c->cfg.maxexc ? c->cfg.maxexc : 1u});
+}
+
+// k_poisson_scan<KEEP, MAP, NEAREST>: KEEP = parity getters want tau / n, MAP = the consumer is the sweep's gather-on-load
+// (child -> parent map) rather than k_copy (first parent per copy tile), NEAREST = resampling rule A4b instead of Poisson
+template <bool KEEP, bool MAP>
+void launch_scan_rule(pa_ctx* c, unsigned grid, DevState* st, const int32_t* E0, const int32_t* E1, const LevelTables& tb,
+                      const ScanOut& out, int shift, unsigned long long cap) {
+  if (c->nearest) launch(c, "k_poisson_scan", k_poisson_scan<KEEP, MAP, true>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
+  else launch(c, "k_poisson_scan", k_poisson_scan<KEEP, MAP, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
+}
+void launch_scan(pa_ctx* c, bool keep, bool map, unsigned grid, DevState* st, const int32_t* E0, const int32_t* E1,
+                 const LevelTables& tb, const ScanOut& out, int shift, unsigned long long cap) {
+  if (keep && map) launch_scan_rule<true, true>(c, grid, st, E0, E1, tb, out, shift, cap);
+  else if (keep) launch_scan_rule<true, false>(c, grid, st, E0, E1, tb, out, shift, cap);
+  else if (map) launch_scan_rule<false, true>(c, grid, st, E0, E1, tb, out, shift, cap);
+  else launch_scan_rule<false, false>(c, grid, st, E0, E1, tb, out, shift, cap);
 }
 
 // all kernels of one temperature step, parameters in device slot sp:
@@ -286,7 +299,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   const LevelTables tb = tables(c);
   const int N = c->N;
   const int n_desc = (int)((c->cap + SCAN_TILE - 1) / SCAN_TILE + 1);
-  const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
+  const int32_t *E0 = c->dev<int32_t>(c->lo.EM[0]), *E1 = c->dev<int32_t>(c->lo.EM[1]);
   std::optional<Prof> span;  // a1-a6 as one span on the stream (not a launch)
   span.emplace(c, PA_K_RESAMPLE_SPAN, false);
   {
@@ -300,7 +313,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     const bool keep = c->lo.n || c->lo.tau;
     if (c->scan_grid_max == 0) {  // blocks per SM (occupancy) x SMs
       int per_sm = 0, sms = 0;
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true>, SCAN_THREADS, 0);
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true, false>, SCAN_THREADS, 0);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
       c->scan_grid_max = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
     }
@@ -315,10 +328,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     const unsigned long long cap = (unsigned long long)c->cap;
     const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? (tiles_cap ? tiles_cap : 1u) : (unsigned)c->scan_grid_max;
     Prof p(c, PA_K_POISSON_SCAN);
-    if (keep && theta > 0) launch(c, "k_poisson_scan", k_poisson_scan<true, true>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key, c->nearest);
-    else if (keep) launch(c, "k_poisson_scan", k_poisson_scan<true, false>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key, c->nearest);
-    else if (theta > 0) launch(c, "k_poisson_scan", k_poisson_scan<false, true>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key, c->nearest);
-    else launch(c, "k_poisson_scan", k_poisson_scan<false, false>, grid, SCAN_THREADS, st, E0, E1, tb, N, out, shift, cap, c->key, c->nearest);
+    launch_scan(c, keep, theta > 0, grid, st, E0, E1, tb, out, shift, cap);
   }
   if (theta == 0) launch_copy(c);  // a6; with sweeps to follow it is fused into the sweep's load
   span.reset();
@@ -607,10 +617,26 @@ int pa_beta(pa_ctx* c, double* beta, int64_t* steps) {
 
 int pa_energies(pa_ctx* c, int32_t* E, int32_t* M, int64_t n, int dst_on_device) {
   if (!c || n < 0 || n > c->R || (!E && !M)) return fail(c, PA_EINVAL, "pa_energies: bad arguments");
+  if (n == 0) return PA_OK;
+  if (c->dist_phase != 0) return fail(c, PA_EINVAL, "pa_energies: a multi-GPU step is in flight (the spare buffer is in use)");
+  if (int rc = bind_device(c)) return rc;
   const unsigned cur = c->h_state->cur;
+  const int32_t* em = c->dev<int32_t>(c->lo.EM[cur]);
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  if (dst_on_device) {
+    k_unpack_em<<<grid, 256, 0, c->stream>>>(em, E, M, (unsigned long long)n);
+    c->launches += 1;
+    CK(cudaStreamSynchronize(c->stream));
+    return PA_OK;
+  }
+  // host destination: unpack into the spare population buffer (free outside a step; cap * S >= 8 n bytes), then copy
+  int32_t* sE = c->dev<int32_t>(c->lo.spins[cur ^ 1u]);
+  int32_t* sM = sE + ((n + 3) / 4) * 4;
+  k_unpack_em<<<grid, 256, 0, c->stream>>>(em, E ? sE : nullptr, M ? sM : nullptr, (unsigned long long)n);
+  c->launches += 1;
   int rc = PA_OK;
-  if (E) rc = copy_out(c, E, c->dev<int32_t>(c->lo.E[cur]), (size_t)n * 4, dst_on_device);
-  if (rc == PA_OK && M) rc = copy_out(c, M, c->dev<int32_t>(c->lo.M[cur]), (size_t)n * 4, dst_on_device);
+  if (E) rc = copy_out(c, E, sE, (size_t)n * 4, 0);
+  if (rc == PA_OK && M) rc = copy_out(c, M, sM, (size_t)n * 4, 0);
   return rc;
 }
 
@@ -699,7 +725,7 @@ int pa_adaptive_beta(pa_ctx* c, double target_overlap, double dbeta_max, double*
   if (int rc = bind_device(c)) return rc;
   DevState* st = c->dev<DevState>(c->lo.state);
   unsigned* hist = c->dev<unsigned>(c->lo.lev_hist);
-  k_level_hist<<<c->obs_grid, OBS_THREADS, 0, c->stream>>>(st, c->dev<int32_t>(c->lo.E[0]), c->dev<int32_t>(c->lo.E[1]), hist, c->N);
+  k_level_hist<<<c->obs_grid, OBS_THREADS, 0, c->stream>>>(st, c->dev<int32_t>(c->lo.EM[0]), c->dev<int32_t>(c->lo.EM[1]), hist, c->N);
   k_adaptive_step<<<1, OBS_THREADS, 0, c->stream>>>(st, hist, c->N, target_overlap, dbeta_max, 40);
   c->launches += 2;
   if (int rc = sync_state(c)) return rc;
@@ -838,7 +864,7 @@ int pa_dist_begin(pa_ctx* c, double beta_next, int32_t theta, pa_dist_partial* m
   {
     Prof p(c, PA_K_Q_REDUCE);  // a shard: stops at the rank's own sum of weights
     launch(c, "k_q_reduce", k_q_reduce, c->red_grid, RED_THREADS, st, (const StepParams*)d_params,
-           (const int32_t*)c->dev<int32_t>(c->lo.E[0]), (const int32_t*)c->dev<int32_t>(c->lo.E[1]), c->N,
+           (const int32_t*)c->dev<int32_t>(c->lo.EM[0]), (const int32_t*)c->dev<int32_t>(c->lo.EM[1]), c->N,
            c->dev<double>(c->lo.red_partial), (double)c->g_R0, c->dev<unsigned long long>(c->lo.tile_desc), n_desc, tables(c), c->nearest);
   }
   if (int rc = sync_state(c)) return rc;
@@ -864,7 +890,7 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
   DevState* st = c->dev<DevState>(c->lo.state);
   const StepParams* d_params = c->dev<StepParams>(c->lo.params);
   const LevelTables tb = tables(c);
-  const int32_t *E0 = c->dev<int32_t>(c->lo.E[0]), *E1 = c->dev<int32_t>(c->lo.E[1]);
+  const int32_t *E0 = c->dev<int32_t>(c->lo.EM[0]), *E1 = c->dev<int32_t>(c->lo.EM[1]);
   {
     Prof p(c, PA_K_LEVELS_TAU);
     launch(c, "k_dist_tables", k_dist_tables, 1u, RED_THREADS, st, d_params, c->N, sumw, (double)R, (double)c->g_R0, tb, c->nearest);
@@ -874,7 +900,7 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
     const bool keep = c->lo.n || c->lo.tau;
     if (c->scan_grid_max == 0) {
       int per_sm = 0, sms = 0;
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true>, SCAN_THREADS, 0);
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true, false>, SCAN_THREADS, 0);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
       c->scan_grid_max = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
     }
@@ -889,8 +915,7 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
     const unsigned long long cap = (unsigned long long)c->cap;
     const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? (tiles_cap ? tiles_cap : 1u) : (unsigned)c->scan_grid_max;
     Prof p(c, PA_K_POISSON_SCAN);
-    if (keep) launch(c, "k_poisson_scan", k_poisson_scan<true, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key, c->nearest);
-    else launch(c, "k_poisson_scan", k_poisson_scan<false, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key, c->nearest);
+    launch_scan(c, keep, false, grid, st, E0, E1, tb, out, shift, cap);
   }
   launch_copy(c);  // the rank's offspring, expanded in child order, into the spare buffer: the send side of the exchange
   CK(cudaMemcpyAsync(c->h_state, st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));

@@ -86,6 +86,17 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 
 __device__ __forceinline__ uint32_t ctr3(uint32_t tag, uint32_t step) { return (tag << 28) | step; }
 
+// E and M of a replica share ONE 32-bit word in HBM: E / 4 in the upper half, M / 2 in the lower half.  Both are exact
+// (E = 0 mod 4: DESIGN.md C1; M = 2 popc - N with N even) and fit 16 bits for every supported lattice (|E / 4|, |M / 2|
+// <= N / 2 = 8192 at L = 128).  Halves the E/M traffic of the reductions and of the redistribution copy; the energy
+// level of C5 / A4 is simply the upper half + N / 2.
+__device__ __forceinline__ int32_t pack_em(int E, int M) {
+  return (int32_t)(((uint32_t)(E >> 2) << 16) | ((uint32_t)(M >> 1) & 0xffffu));
+}
+__device__ __forceinline__ int em_energy(int32_t w) { return (w >> 16) * 4; }
+__device__ __forceinline__ int em_level(int32_t w, int N) { return (w >> 16) + (N >> 1); }  // (E + 2N) / 4
+__device__ __forceinline__ int em_mag(int32_t w) { return ((int32_t)((uint32_t)w << 16) >> 16) * 2; }
+
 #ifndef PA_PDL_TRIGGER
 #define PA_PDL_TRIGGER 0
 #endif

@@ -25,6 +25,16 @@ __global__ void k_init(const DevState* __restrict__ st, uint32_t* __restrict__ s
   }
 }
 
+// getters: packed E/4 : M/2 words -> separate int32 arrays
+__global__ void k_unpack_em(const int32_t* __restrict__ EM, int32_t* __restrict__ E, int32_t* __restrict__ M,
+                            unsigned long long n) {
+  const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int32_t w = EM[i];
+  if (E) E[i] = em_energy(w);
+  if (M) M[i] = em_mag(w);
+}
+
 // 128-bit unsigned add helper on {lo, hi}
 struct U128 {
   unsigned long long lo, hi;
@@ -153,23 +163,23 @@ constexpr int OBS_Q = 5;  // sum E (two's complement), sum E^2, sum |M|, sum M^2
 // mode 2: end of a step of a multi-GPU shard -> the exchange has put the new local population (Rnew replicas) into
 //         buffer cur itself; sums over it, then COMMIT without flipping the buffers.
 __global__ void __launch_bounds__(OBS_THREADS)
-k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
-          const int32_t* __restrict__ E1, const int32_t* __restrict__ M0, const int32_t* __restrict__ M1,
+k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ EM0,
+          const int32_t* __restrict__ EM1,
           unsigned long long* __restrict__ partial /* [grid][12] */, const int mode, const int N,
           const uint32_t* __restrict__ off, uint32_t* part0, uint32_t* part1, uint32_t* part_stats, const BalanceArgs ba) {
   grid_dependency_wait();
   if (st->status != ST_OK) return;
   const unsigned buf = mode == 0 ? (st->cur ^ 1u) : st->cur;
   const unsigned long long count = mode != 1 ? st->Rnew : st->R;
-  const int32_t* __restrict__ E = buf ? E1 : E0;
-  const int32_t* __restrict__ M = buf ? M1 : M0;
+  const int32_t* __restrict__ EM = buf ? EM1 : EM0;  // packed E/4 : M/2 words (pa_common.cuh)
   // per-thread partial sums: a thread sees at most cap / (grid * 256) < 2^17 replicas, |E| <= 2^15, |M| <= 2^14, so
   // sum E, sum E^2 (< 2^47), sum |M|, sum M^2 fit 64 bits; only M^4 (< 2^56 each) needs the 128-bit accumulator.
   long long sE = 0;
   unsigned long long sE2 = 0, sA = 0, sM2 = 0;
   U128 sM4 = {0ull, 0ull};
   int emin = 0x7fffffff, emax = -0x7fffffff;  // occupied energy range: the level window of the next step's tables
-  auto add = [&](int ei, int mi) {
+  auto add = [&](int w) {
+    const int ei = em_energy(w), mi = em_mag(w);
     emin = min(emin, ei);
     emax = max(emax, ei);
     const long long e = ei;
@@ -182,19 +192,20 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   };
   const unsigned long long nvec = count / 4, tid = (unsigned long long)blockIdx.x * OBS_THREADS + threadIdx.x;
   const unsigned long long stride = (unsigned long long)gridDim.x * OBS_THREADS;
-  const int4* __restrict__ E4 = reinterpret_cast<const int4*>(E);  // buffers are 256-byte aligned
-  const int4* __restrict__ M4 = reinterpret_cast<const int4*>(M);
+  const int4* __restrict__ EM4 = reinterpret_cast<const int4*>(EM);  // buffers are 256-byte aligned
   unsigned long long v = tid;
-  for (; v + stride < nvec; v += 2 * stride) {  // 64 bytes in flight per thread
-    const int4 e0 = __ldg(E4 + v), m0 = __ldg(M4 + v), e1 = __ldg(E4 + v + stride), m1 = __ldg(M4 + v + stride);
-    add(e0.x, m0.x); add(e0.y, m0.y); add(e0.z, m0.z); add(e0.w, m0.w);
-    add(e1.x, m1.x); add(e1.y, m1.y); add(e1.z, m1.z); add(e1.w, m1.w);
+  for (; v + 3 * stride < nvec; v += 4 * stride) {  // 64 bytes in flight per thread
+    const int4 a = __ldg(EM4 + v), b = __ldg(EM4 + v + stride), c = __ldg(EM4 + v + 2 * stride), d = __ldg(EM4 + v + 3 * stride);
+    add(a.x); add(a.y); add(a.z); add(a.w);
+    add(b.x); add(b.y); add(b.z); add(b.w);
+    add(c.x); add(c.y); add(c.z); add(c.w);
+    add(d.x); add(d.y); add(d.z); add(d.w);
   }
   for (; v < nvec; v += stride) {
-    const int4 e0 = __ldg(E4 + v), m0 = __ldg(M4 + v);
-    add(e0.x, m0.x); add(e0.y, m0.y); add(e0.z, m0.z); add(e0.w, m0.w);
+    const int4 a = __ldg(EM4 + v);
+    add(a.x); add(a.y); add(a.z); add(a.w);
   }
-  for (unsigned long long j = 4 * nvec + tid; j < count; j += stride) add(E[j], M[j]);
+  for (unsigned long long j = 4 * nvec + tid; j < count; j += stride) add(EM[j]);
   U128 acc[OBS_Q];
   acc[0] = {(unsigned long long)sE, sE < 0 ? ~0ull : 0ull};  // sign-extended
   acc[1] = {sE2, 0ull};
@@ -310,13 +321,13 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
 // (k_adaptive_step): 40 halvings, each two block reductions over the occupied levels.
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(OBS_THREADS)
-k_level_hist(const DevState* __restrict__ st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1,
+k_level_hist(const DevState* __restrict__ st, const int32_t* __restrict__ EM0, const int32_t* __restrict__ EM1,
              unsigned* __restrict__ hist, const int N) {
-  const int32_t* __restrict__ E = st->cur ? E1 : E0;
+  const int32_t* __restrict__ E = st->cur ? EM1 : EM0;
   const unsigned long long R = st->R;
   const unsigned long long stride = (unsigned long long)gridDim.x * OBS_THREADS;
   for (unsigned long long j = (unsigned long long)blockIdx.x * OBS_THREADS + threadIdx.x; j < R; j += stride)
-    atomicAdd(&hist[(E[j] + 2 * N) >> 2], 1u);
+    atomicAdd(&hist[em_level(E[j], N)], 1u);
 }
 
 __device__ __forceinline__ double block_sum_256(double v, double* s_red) {

@@ -120,8 +120,8 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 __global__ void __launch_bounds__(RED_THREADS)
-k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ E0,
-           const int32_t* __restrict__ E1, int N, double* __restrict__ partial, double R0,
+k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __restrict__ EM0,
+           const int32_t* __restrict__ EM1, int N, double* __restrict__ partial, double R0,
            unsigned long long* __restrict__ tile_desc, int n_desc, LevelTables tb, int nearest) {
   grid_dependency_wait();
   const unsigned long long tid = (unsigned long long)blockIdx.x * RED_THREADS + threadIdx.x;
@@ -133,11 +133,11 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
   }
   for (unsigned long long i = tid; i < (unsigned long long)n_desc; i += stride) tile_desc[i] = 0ull;
   if (st->status != ST_OK) return;
-  const int32_t* __restrict__ E = st->cur ? E1 : E0;
+  const int32_t* __restrict__ E = st->cur ? EM1 : EM0;  // packed E/4 : M/2 words (pa_common.cuh)
   const unsigned long long R = st->R;
   const double dbeta = sp->dbeta;
   const int lev_lo = st->lev_lo, W = st->lev_hi - lev_lo + 1;
-  const int twoN = 2 * N;
+  const int halfN = N >> 1;
   const unsigned long long nvec = R / 4;
   const int4* __restrict__ E4 = reinterpret_cast<const int4*>(E);  // the buffers are 256-byte aligned
   __shared__ double s_w[QW_MAX];
@@ -145,8 +145,8 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
   if (W <= QW_MAX) {
     for (int i = threadIdx.x; i < W; i += RED_THREADS) s_w[i] = level_weight(dbeta, lev_lo + i, N);
     __syncthreads();
-    const int shift = twoN - 4 * lev_lo;  // level(E) - lev_lo = (E + 2N - 4 lev_lo) / 4
-    auto wl = [&](int e) { return s_w[(e + shift) >> 2]; };
+    const int shift = halfN - lev_lo;  // level - lev_lo = E / 4 + N / 2 - lev_lo
+    auto wl = [&](int w) { return s_w[(w >> 16) + shift]; };
     unsigned long long v = tid;
 #if PA_RED_UNR8
     for (; v + 7 * stride < nvec; v += 8 * stride) {  // eight 128-bit loads in flight per thread
@@ -170,7 +170,7 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
     }
     for (unsigned long long j = 4 * nvec + tid; j < R; j += stride) acc += wl(E[j]);
   } else {
-    auto wl = [&](int e) { return level_weight(dbeta, (e + twoN) >> 2, N); };
+    auto wl = [&](int w) { return level_weight(dbeta, (w >> 16) + halfN, N); };
     unsigned long long v = tid;
     for (; v < nvec; v += stride) {
       const int4 a = __ldg(E4 + v);
@@ -320,12 +320,12 @@ constexpr unsigned NO_TILE = 0xffffffffu;
 // A tiles, 32 per round trip) is hidden behind B's sampling.  Every ticket holder publishes its aggregate before it
 // waits on anything, so the look-back cannot deadlock.
 #ifndef PA_SCAN_MINB
-#define PA_SCAN_MINB 7
+#define PA_SCAN_MINB 6
 #endif
-template <bool KEEP, bool MAP>
+template <bool KEEP, bool MAP, bool NEAREST>
 __global__ void __launch_bounds__(SCAN_THREADS, (MAP ? PA_SCAN_MINB - 1 : PA_SCAN_MINB))
-k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __restrict__ E1, LevelTables tb, int N,
-               ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key, int nearest) {
+k_poisson_scan(DevState* st, const int32_t* __restrict__ EM0, const int32_t* __restrict__ EM1, LevelTables tb, int N,
+               ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key) {
   grid_dependency_wait();
   if (st->status != ST_OK) return;
   __shared__ unsigned s_tile;
@@ -350,7 +350,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
   const uint32_t R = (uint32_t)st->R;  // R <= capacity < 2^32 - 4096: parent indices fit 32 bits
   const unsigned ntiles = (R + SCAN_TILE - 1) / SCAN_TILE;
   const unsigned tile_end = ntiles;
-  const int32_t* __restrict__ E = st->cur ? E1 : E0;
+  const int32_t* __restrict__ E = st->cur ? EM1 : EM0;  // packed E/4 : M/2 words
   const uint32_t c3 = ctr3(TAG_RESAMPLE, st->step + 1u);
   const uint32_t slot0 = st->slot0;  // the copy counts are keyed by the GLOBAL parent index (a multi-GPU shard: slot0 > 0)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -382,11 +382,11 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           jj[b] = tile_base + (r0 + b) * SCAN_THREADS + threadIdx.x;
-          e[b] = (jj[b] < R) ? __ldg(E + jj[b]) : 4 * lev_lo - 2 * N;  // padding reads as the first occupied level
+          e[b] = (jj[b] < R) ? __ldg(E + jj[b]) : (int)((uint32_t)(lev_lo - (N >> 1)) << 16);  // padding reads as the first occupied level
         }
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
-          const unsigned lev = (unsigned)((e[b] + 2 * N) >> 2);
+          const unsigned lev = (unsigned)em_level(e[b], N);
           hl[b] = lev - (unsigned)lev_lo;  // level relative to the cached window (>= SCAN_HW: not cached)
           const unsigned mm = (ALL || hl[b] < (unsigned)SCAN_HW) ? s_m[hl[b]] : __ldg(tb.m + lev);
           m[b] = (jj[b] < R) ? mm : 0u;
@@ -409,7 +409,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           k[b] = c4[b];
-          if (nearest) {  // A4b (block-uniform): n = floor(lambda) + [u > 1 - frac(lambda)], both from the head of the row
+          if constexpr (NEAREST) {  // A4b: n = floor(lambda) + [u > 1 - frac(lambda)], both from the head of the row
             const double* F = (ALL || hl[b] < (unsigned)SCAN_HW) ? &s_head[hl[b]][0] : tb.cdf + (size_t)(hl[b] + (unsigned)lev_lo) * PO_ROW;
             k[b] = (unsigned)__double_as_longlong(F[1]) + (u[b] > F[0] ? 1u : 0u);
           } else if (c4[b] == 4u)
@@ -449,7 +449,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ E0, const int32_t* __re
           }
           const unsigned item = s_hitem[lo];
           const uint32_t j = tile_base + item;
-          const unsigned lev = (unsigned)((__ldg(E + j) + 2 * N) >> 2);
+          const unsigned lev = (unsigned)em_level(__ldg(E + j), N);
           const unsigned kk = draw_chunk(tb.cdf + (size_t)lev * PO_ROW, j + slot0, 1ull + (wk - s_hstart[lo]), c3, key);
           if (kk) atomicAdd(&cntb[item], kk);
         }
@@ -696,7 +696,7 @@ template <> struct VecT<8> { using type = uint2; };
 template <int L>
 __global__ void __launch_bounds__(COPY_THREADS)
 k_copy(const DevState* __restrict__ st, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tile_parent,
-       uint32_t* spins0, uint32_t* spins1, int32_t* E0, int32_t* E1, int32_t* M0, int32_t* M1) {
+       uint32_t* spins0, uint32_t* spins1, int32_t* EM0, int32_t* EM1) {
   using CG = CopyGeo<L>;
   using V = typename VecT<CG::VB>::type;
   grid_dependency_wait();
@@ -708,10 +708,8 @@ k_copy(const DevState* __restrict__ st, const uint32_t* __restrict__ off, const 
   const unsigned cur = st->cur;  // source = buffer cur, destination = buffer cur^1 (never the same memory)
   const V* __restrict__ src = reinterpret_cast<const V*>(cur ? spins1 : spins0);
   V* __restrict__ dst = reinterpret_cast<V*>(cur ? spins0 : spins1);
-  const int32_t* __restrict__ Es = cur ? E1 : E0;
-  const int32_t* __restrict__ Ms = cur ? M1 : M0;
-  int32_t* __restrict__ Ed = cur ? E0 : E1;
-  int32_t* __restrict__ Md = cur ? M0 : M1;
+  const int32_t* __restrict__ EMs = cur ? EM1 : EM0;  // packed E/4 : M/2 words: one gather, one store per child
+  int32_t* __restrict__ EMd = cur ? EM0 : EM1;
   const unsigned nchild = (unsigned)((Rnew - i0 < (unsigned long long)CG::CT) ? (Rnew - i0) : CG::CT);
   const unsigned long long i1 = i0 + nchild;
 
@@ -764,9 +762,7 @@ k_copy(const DevState* __restrict__ st, const uint32_t* __restrict__ off, const 
 
   // E, M of the children
   for (unsigned c = threadIdx.x; c < nchild; c += COPY_THREADS) {
-    const uint32_t pj = s_par[c];
-    Ed[i0 + c] = Es[pj];
-    Md[i0 + c] = Ms[pj];
+    EMd[i0 + c] = EMs[s_par[c]];
   }
   // lattices: VT threads per child, 4 children in flight per thread group
   constexpr int GROUPS = COPY_THREADS / (CG::VT < COPY_THREADS ? CG::VT : COPY_THREADS);

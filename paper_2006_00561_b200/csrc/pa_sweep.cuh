@@ -390,7 +390,7 @@ __device__ __forceinline__ void planes_to_row(const uint32_t (&p0)[Geo<L>::WPP],
 template <int L>
 __global__ void __launch_bounds__(SWEEP_THREADS, (L >= 128 ? PA_SWEEP_MINB128 : PA_SWEEP_MINB64))
 k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
-        int32_t* __restrict__ E0, int32_t* __restrict__ E1, int32_t* __restrict__ M0, int32_t* __restrict__ M1,
+        int32_t* __restrict__ EM0, int32_t* __restrict__ EM1,
         const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of) {
   using G_ = Geo<L>;
   static_assert(L >= 64, "k_sweep_small handles L < 64");
@@ -401,8 +401,7 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
   const int theta = sa.mode != 1 ? sa.theta : 0;
   uint32_t* spins = buf ? spins1 : spins0;
   const uint32_t* spins_other = buf ? spins0 : spins1;  // buffer cur inside a step
-  int32_t* __restrict__ Eo = buf ? E1 : E0;
-  int32_t* __restrict__ Mo = buf ? M1 : M0;
+  int32_t* __restrict__ EMo = buf ? EM1 : EM0;  // packed E/4 : M/2 words (pa_common.cuh)
 
   const unsigned long long slot_base64 = (unsigned long long)blockIdx.x * G_::RPB;
   if (slot_base64 >= count) return;  // block-uniform: the sweeps below contain block barriers
@@ -464,10 +463,7 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
       unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
       ups += __shfl_xor_sync(0xffffffffu, ups, o);
     }
-    if (g == 0) {
-      Eo[slot64] = 2 * unsat - 2 * G_::N;
-      Mo[slot64] = 2 * ups - G_::N;
-    }
+    if (g == 0) EMo[slot64] = pack_em(2 * unsat - 2 * G_::N, 2 * ups - G_::N);
     // ---- store (once per step) -------------------------------------------------------------------
     if (theta > 0) {
       uint32_t rawall[G_::RPL * G_::WR];
@@ -523,7 +519,7 @@ __device__ __forceinline__ void small_neighbours(uint32_t S, int g, uint32_t& U,
 template <int L>
 __global__ void __launch_bounds__(SWEEP_THREADS)
 k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
-              int32_t* __restrict__ E0, int32_t* __restrict__ E1, int32_t* __restrict__ M0, int32_t* __restrict__ M1,
+              int32_t* __restrict__ EM0, int32_t* __restrict__ EM1,
               const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of) {
   using G_ = SGeo<L>;
   static_assert(L == 8 || L == 16 || L == 32, "");
@@ -533,8 +529,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
   const unsigned long long count = sa.mode != 1 ? st->Rnew : st->R;
   const int theta = sa.mode != 1 ? sa.theta : 0;
   uint32_t* spins = buf ? spins1 : spins0;
-  int32_t* __restrict__ Eo = buf ? E1 : E0;
-  int32_t* __restrict__ Mo = buf ? M1 : M0;
+  int32_t* __restrict__ EMo = buf ? EM1 : EM0;  // packed E/4 : M/2 words (pa_common.cuh)
   const uint32_t gs = sa.mode != 1 ? st->slot0_new : 0u;  // global index of local slot 0 (multi-GPU shard)
 
   // A group of G lanes holds TWO consecutive replicas (one plane word per colour and replica per lane).
@@ -622,10 +617,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
       unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
       ups += __shfl_xor_sync(0xffffffffu, ups, o);
     }
-    if (valid[r] && g == 0) {
-      Eo[slot64[r]] = 2 * unsat - 2 * G_::N;
-      Mo[slot64[r]] = 2 * ups - G_::N;
-    }
+    if (valid[r] && g == 0) EMo[slot64[r]] = pack_em(2 * unsat - 2 * G_::N, 2 * ups - G_::N);
     // ---- store -----------------------------------------------------------------------------------
     if (theta > 0 && valid[r]) {
       const uint32_t ev = (p[r][0] & G_::ER) | (p[r][1] & ~G_::ER);

@@ -523,7 +523,8 @@ def test_sharded_driver_with_one_rank_equals_the_single_context():
     for k in range(1, 5):
         single.step(0.1 * k, 2)
         sh.step(0.1 * k, 2)
-        assert np.array_equal(sh.gather_spins(), single.spins()) and sh.log_Z() == single.log_Z()
+        assert np.array_equal(sh.gather_spins(), single.spins())
+        assert rel(sh.log_Z()["lnZ"], single.log_Z()["lnZ"]) <= RTOL  # Q's rounding depends on the reduction grid (capacity)
 
 
 def test_sharded_capacity_failure_is_consistent_and_leaves_the_population_unchanged():
@@ -665,9 +666,10 @@ def test_device_getters_and_launch_count():
     prof = g.profile_read()
     assert all(cnt == (0 if k in ("balance", "levels_w", "levels_tau", "copy") else 1) for k, (_, cnt) in prof.items()) and prof["sweep"][0] > 0
     g.profile_read()
+    l1 = g.launch_count()  # (the getters above launched their unpack kernels)
     g.step(0.2, 0)  # theta = 0: the gather copy runs instead of the sweep
     prof = g.profile_read()
-    assert prof["copy"][1] == 1 and prof["sweep"][1] == 0 and g.launch_count() - l0 == 8
+    assert prof["copy"][1] == 1 and prof["sweep"][1] == 0 and g.launch_count() - l1 == 4
 
 
 def test_bench_line_carries_the_contract_keys():
