@@ -113,6 +113,7 @@ struct SweepQueue {
   uint4 item[CAP];    // und, v, ge1, (slot - slot_base) << 16 | call0
   uint32_t res[CAP];  // late flips of the item
   uint32_t count[2];
+  uint32_t pad_[2];   // sizeof is a multiple of 16: queues can be laid side by side
   static constexpr uint32_t OFF_RES = 16u * CAP, OFF_COUNT = 20u * CAP;  // byte offsets (checked in k_sweep*)
 };
 // The queue is addressed through its 32-bit shared-window address (taken once per kernel) so that every access is a
@@ -158,17 +159,21 @@ __device__ __forceinline__ uint32_t finish_word(uint32_t und, uint32_t v, uint32
 // flip masks of the NW plane words of a lane.  ge1 / ge2: sites with a >= 1 / a >= 2 anti-aligned neighbours;
 // call0 = 8 * group.   a >= 2: always flip;  a == 1: flip iff u < T4;  a == 0: flip iff u < T8
 // (u < T  <=>  at the first differing bit, most significant first, u has 0).
-// Must be called by EVERY thread of the block (it contains block barriers); lanes without work pass ge2 = ~0.
+// Three phases around the two synchronisation points A and B of the queue protocol:
+//   accept_phase1    two mandatory Philox blocks per word; stragglers pushed; flip = the sites decided so far   --A--
+//   accept_process   the block finishes the queued items densely, one per thread                                 --B--
+//   accept_readback  owners OR the late flips of their pushed words into their flip masks
 template <int NW, int THREADS, int CAP>
-__device__ __forceinline__ void queued_accept(uint32_t q /* shared address of the SweepQueue<CAP> */, unsigned parity, const uint32_t (&ge1)[NW],
-                                              const uint32_t (&ge2)[NW],
+__device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of the SweepQueue<CAP> */, unsigned parity,
+                                              const uint32_t (&ge1)[NW], const uint32_t (&ge2)[NW],
                                               const uint32_t (&slot)[NW],  // replica of each word
                                               uint32_t slot_base,          // first slot of the thread block
                                               const uint32_t (&call0)[NW], uint32_t c2, uint32_t c3, const PhiloxKey& key,
-                                              const SweepArgs& sa, uint32_t (&flip)[NW]) {
+                                              const SweepArgs& sa, uint32_t (&flip)[NW], uint32_t (&und)[NW],
+                                              unsigned (&idx)[NW]) {
   constexpr unsigned FULL = 0xffffffffu;
   constexpr bool CAN_OVERFLOW = CAP < NW * THREADS;
-  uint32_t und[NW], v[NW];
+  uint32_t v[NW];
 #pragma unroll
   for (int i = 0; i < NW; ++i) {
     und[i] = ~ge2[i];
@@ -185,7 +190,7 @@ __device__ __forceinline__ void queued_accept(uint32_t q /* shared address of th
   // ---- push the stragglers: one shared-memory atomic per warp ----
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt = (1u << lane) - 1u;
-  unsigned idx[NW], tot = 0u;
+  unsigned tot = 0u;
 #pragma unroll
   for (int i = 0; i < NW; ++i) {
     const unsigned bal = __ballot_sync(FULL, und[i] != 0u);
@@ -207,21 +212,46 @@ __device__ __forceinline__ void queued_accept(uint32_t q /* shared address of th
     }
     if (und[i] != 0u) sts128(q + 16u * idx[i], und[i], v[i], ge1[i], ((slot[i] - slot_base) << 16) | call0[i]);
   }
-  __syncthreads();  // A: every push of this half-sweep is visible
-  {
-    unsigned n = lds32(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity);
-    if (CAN_OVERFLOW && n > (unsigned)CAP) n = (unsigned)CAP;
-    if (threadIdx.x == 0) sts32(q + SweepQueue<CAP>::OFF_COUNT + 4u * (parity ^ 1u), 0u);  // last read before barrier B of the previous half-sweep
-    for (unsigned it = threadIdx.x; it < n; it += THREADS) {
-      const uint4 m = lds128(q + 16u * it);
-      sts32(q + SweepQueue<CAP>::OFF_RES + 4u * it,
-            finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
-    }
+}
+
+// REVERSE: item `it` goes to thread THREADS - 1 - it (the second queue of a block is drained by the other warps)
+template <int NW, int THREADS, int CAP, bool REVERSE>
+__device__ __forceinline__ void accept_process(uint32_t q, unsigned parity, uint32_t slot_base, uint32_t c2, uint32_t c3,
+                                               const PhiloxKey& key, const SweepArgs& sa) {
+  constexpr bool CAN_OVERFLOW = CAP < NW * THREADS;
+  unsigned n = lds32(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity);
+  if (CAN_OVERFLOW && n > (unsigned)CAP) n = (unsigned)CAP;
+  if (threadIdx.x == 0) sts32(q + SweepQueue<CAP>::OFF_COUNT + 4u * (parity ^ 1u), 0u);  // last read before B of the previous half-sweep
+  const unsigned me = REVERSE ? (unsigned)THREADS - 1u - threadIdx.x : threadIdx.x;
+  for (unsigned it = me; it < n; it += THREADS) {
+    const uint4 m = lds128(q + 16u * it);
+    sts32(q + SweepQueue<CAP>::OFF_RES + 4u * it,
+          finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
   }
-  __syncthreads();  // B: every result is visible
+}
+
+template <int NW, int CAP>
+__device__ __forceinline__ void accept_readback(uint32_t q, const uint32_t (&und)[NW], const unsigned (&idx)[NW],
+                                                uint32_t (&flip)[NW]) {
 #pragma unroll
   for (int i = 0; i < NW; ++i)
     if (und[i] != 0u) flip[i] |= lds32(q + SweepQueue<CAP>::OFF_RES + 4u * idx[i]);
+}
+
+// the three phases with block barriers at A and B.  Must be called by EVERY thread of the block; lanes without work
+// pass ge2 = ~0.
+template <int NW, int THREADS, int CAP>
+__device__ __forceinline__ void queued_accept(uint32_t q, unsigned parity, const uint32_t (&ge1)[NW],
+                                              const uint32_t (&ge2)[NW], const uint32_t (&slot)[NW], uint32_t slot_base,
+                                              const uint32_t (&call0)[NW], uint32_t c2, uint32_t c3, const PhiloxKey& key,
+                                              const SweepArgs& sa, uint32_t (&flip)[NW]) {
+  uint32_t und[NW];
+  unsigned idx[NW];
+  accept_phase1<NW, THREADS, CAP>(q, parity, ge1, ge2, slot, slot_base, call0, c2, c3, key, sa, flip, und, idx);
+  __syncthreads();  // A: every push of this half-sweep is visible
+  accept_process<NW, THREADS, CAP, false>(q, parity, slot_base, c2, c3, key, sa);
+  __syncthreads();  // B: every result is visible
+  accept_readback<NW, CAP>(q, und, idx, flip);
 }
 
 // masks of the sites with a >= 1 and a >= 2 from the four difference words (1 = anti-aligned)
@@ -437,14 +467,14 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
 
   // ---- theta sweeps ----------------------------------------------------------------------------
   if (theta > 0) {
+    const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
+    const uint32_t gs = st->slot0_new;  // global index of local slot 0 (0 unless this is a multi-GPU shard)
     using Q_ = SweepQueue<SweepCap<G_::NWL>::CAP>;
     __shared__ Q_ q_mem;
     static_assert(offsetof(Q_, res) == Q_::OFF_RES && offsetof(Q_, count) == Q_::OFF_COUNT, "queue layout");
     const uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
     if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
     __syncthreads();
-    const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
-    const uint32_t gs = st->slot0_new;  // global index of local slot 0 (0 unless this is a multi-GPU shard)
     for (int t = 0; t < theta; ++t) {
       half_sweep<L, 0>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa);
       half_sweep<L, 1>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa);
