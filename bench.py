@@ -36,14 +36,17 @@ E_BLK = 2.0 + sum(1.0 - (1.0 - 2.0 ** (-4 * c)) ** 32 for c in range(2, 8))
 ALU_OPS_PER_ATTEMPT = (E_BLK * (19 + 12) + 12) / 32.0
 I_MIN_SURVEY = 12.0   # one 32-bit Philox word per attempt at 1 warp-instr/clk/SMSP (kept for continuity)
 SM_COUNT, SMSP, LANES, ALU_LANES = 148, 4, 32, 16
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the `ncu --set full` capture
-# (profiles/r1l_sweep64_ncu.md: config 3, one launch = gather + theta sweeps of R' ~ 2^21 replicas; algorithmic
-# S*(U + R') + 12R': each surviving parent read once, each child written once).
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures.  These are CAPTURED
+# constants, not something this run measures: each carries the profiles/ file it was read from and the commit the
+# captured library was built from, and the bench line prints both (`traffic_src`) so that a stale figure is visible.
 # Reported only for the workload it was captured on.
-NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 0.650892e9 + 1.039523e9}
-# same for the a1-a6 chain of config 5 (profiles/r1n_resample_ncu.md; k_q_reduce from the r1f capture): q_reduce + levels_tau
-# + poisson_scan + copy, read + write
-NCU_RESAMPLE_TRAFFIC_BYTES = 67.12e6 + 0.014e6 + (67.28e6 + 21.58e6) + (671.23e6 + 2223.73e6)
+NCU_CAPTURE_COMMIT = "3a5ddd8"
+# config 3, one launch of k_sweep<64> = gather + theta sweeps of R' ~ 2^21 replicas (algorithmic S*(U + R') + 8R')
+NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 0.652241e9 + 1.035193e9}
+NCU_TRAFFIC_SRC = {"file": "profiles/r2_sweep64_ncu.md", "commit": NCU_CAPTURE_COMMIT}
+# a1-a6 chain of config 5: q_reduce (+ level tables) + poisson_scan + copy, read + write
+NCU_RESAMPLE_TRAFFIC_BYTES = 67.15e6 + (67.32e6 + 22.38e6) + (605.01e6 + 2157.43e6)
+NCU_RESAMPLE_TRAFFIC_SRC = {"file": "profiles/r2_resample_ncu.md", "commit": NCU_CAPTURE_COMMIT}
 
 
 def measured_peaks():
@@ -224,6 +227,7 @@ def resample_leg(binding, torch, peaks, repeats=5):
             "roofline": {"bound": "hbm", "achieved": alg_bytes / (chain * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                          "unit": "GB/s", "frac": alg_bytes / (chain * 1e-3) / 1e9 / peaks["hbm_gbs"],
                          "peak_src": peaks["src"], "traffic": NCU_RESAMPLE_TRAFFIC_BYTES,
+                         "traffic_src": NCU_RESAMPLE_TRAFFIC_SRC,
                          "copy_kernel_GBps": copy_bytes / (copy_ms * 1e-3) / 1e9,
                          "frac_vs_8000": alg_bytes / (chain * 1e-3) / 1e9 / 8000.0}}
 
@@ -289,6 +293,31 @@ def anneal_leg(binding, torch, configs):
                     "launches": pa.launch_count()})
         del pa
         torch.cuda.empty_cache()
+    return out
+
+
+def theta1_leg(binding, torch, wl, steps=20, warmup=3):
+    """theta = 1, the paper's scalability regime ("the most time of simulations is spending for the population
+    re-weighting and redistribution"): the same workload with one sweep per temperature step"""
+    pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0, flags=binding.PA_PROFILE)
+    pa.run(schedule(wl, 1, warmup), 1)
+    pa.profile_read()
+    rs0 = pa.replica_steps()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record(pa.stream)
+    pa.run(schedule(wl, warmup + 1, steps), 1)
+    ev1.record(pa.stream)
+    torch.cuda.synchronize()
+    sec = ev0.elapsed_time(ev1) * 1e-3
+    prof = pa.profile_read()
+    rs = pa.replica_steps() - rs0
+    total = sum(v[0] for k, v in prof.items() if k != "resample_span")
+    out = {"theta": 1, "steps": steps, "attempts_per_s": wl.N * rs / sec, "ms_per_step": 1e3 * sec / steps,
+           "replicas_per_s": rs / sec, "share_a1_a5_and_map": prof["resample_span"][0] / total,
+           "share_sweep_incl_gather": prof["sweep"][0] / total}
+    del pa
+    torch.cuda.empty_cache()
     return out
 
 
@@ -423,7 +452,8 @@ def run_ours(args):
         roof = {"bound": "alu", "achieved": achieved, "peak": peak,
                 "unit": "T ALU-pipe lane-ops/s (%.3f algorithmic per flip attempt)" % ALU_OPS_PER_ATTEMPT,
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(("k_sweep<%d>" % wl.L, args.config)),
-                "traffic_algorithmic": (2 * wl.bytes_per_replica + 8) * (replica_steps / sweep_n),
+                "traffic_src": NCU_TRAFFIC_SRC if ("k_sweep<%d>" % wl.L, args.config) in NCU_TRAFFIC_BYTES else None,
+                "traffic_algorithmic": (2 * wl.bytes_per_replica + 8) * (replica_steps / sweep_n),  # upper bound: U = R'
                 "kernel": "k_sweep<%d>" % wl.L,
                 "kernel_attempts_per_s": sweep_rate, "kernel_ms_per_launch": sweep_ms / sweep_n,
                 "kernel_share_of_step": sweep_ms / step_kernel_ms,
@@ -451,7 +481,10 @@ def run_ours(args):
     if use_shards:
         del sharded
     torch.cuda.empty_cache()
+    theta1 = None
     if g.is_main and g.world == 1:
+        if wl.theta > 1 and not args.no_resample:
+            theta1 = theta1_leg(binding, torch, wl)
         if not args.no_resample:
             resample = resample_leg(binding, torch, peaks, repeats=args.resample_repeats)
         if not args.no_cpu_baseline:
@@ -479,7 +512,7 @@ def run_ours(args):
                                            "that cross rank boundaries (NCCL point-to-point)" % (g.world, g.world)),
                            "l2": "population %.0f MiB per buffer > 126 MB L2, no flush needed" % (wl.R0 * wl.bytes_per_replica / 2 ** 20)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_total, "roofline": roof, "cpu_baseline": cpu,
-                "resample": resample, "kernels": per_kernel, "anneal": {"lnZ": lnZ, "beta": beta_now, "R": R_final,
+                "resample": resample, "theta1": theta1, "kernels": per_kernel, "anneal": {"lnZ": lnZ, "beta": beta_now, "R": R_final,
                                                                          "replica_steps": replica_steps}}
         if g.world > 1:
             line["config"]["R0"] = wl.R0 * g.world

@@ -126,7 +126,7 @@ struct pa_ctx {
   double dist_beta_next;
   bool dbg_thresholds;  // test hook: pa_debug_set_thresholds
   uint32_t dbg_T4, dbg_T8;
-  int scan_grid_max;  // co-resident blocks of k_poisson_scan on this device
+  int scan_grid_max[2];  // co-resident blocks of k_poisson_scan on this device: [0] theta = 0 variant, [1] map-writing variant
   unsigned red_grid, obs_grid;  // blocks of the two reductions: 4 per SM for large populations, fewer for small ones
   std::vector<EventPair> ev_used, ev_free;
   std::string err, launch_err;
@@ -273,6 +273,20 @@ void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
          BalanceArgs{c->cfg.P, (int)c->cfg.policy, c->cfg.block ? c->cfg.block : 1024u, c->cfg.maxexc ? c->cfg.maxexc : 1u});
 }
 
+// persistent grid of k_poisson_scan: blocks per SM (occupancy of the variant) x SMs
+unsigned scan_grid(pa_ctx* c, bool map) {
+  int& g = c->scan_grid_max[map ? 1 : 0];
+  if (g == 0) {
+    int per_sm = 0, sms = 0;
+    if (map) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true, false>, SCAN_THREADS, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, false, false>, SCAN_THREADS, 0);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    g = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
+  }
+  const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
+  return tiles_cap < (unsigned)g ? (tiles_cap ? tiles_cap : 1u) : (unsigned)g;
+}
+
 // k_poisson_scan<KEEP, MAP, NEAREST>: KEEP = parity getters want tau / n, MAP = the consumer is the sweep's gather-on-load
 // (child -> parent map) rather than k_copy (first parent per copy tile), NEAREST = resampling rule A4b instead of Poisson
 template <bool KEEP, bool MAP>
@@ -309,14 +323,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
   }
   {
     // persistent blocks pull tiles from a ticket counter
-    const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
     const bool keep = c->lo.n || c->lo.tau;
-    if (c->scan_grid_max == 0) {  // blocks per SM (occupancy) x SMs
-      int per_sm = 0, sms = 0;
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true, false>, SCAN_THREADS, 0);
-      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
-      c->scan_grid_max = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
-    }
     ScanOut out;
     out.off = c->dev<uint32_t>(c->lo.off);
     out.n = c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr;
@@ -326,7 +333,7 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     out.tile_parent = c->dev<uint32_t>(c->lo.tile_parent);
     const int shift = copy_shift_for(c->cfg.L);
     const unsigned long long cap = (unsigned long long)c->cap;
-    const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? (tiles_cap ? tiles_cap : 1u) : (unsigned)c->scan_grid_max;
+    const unsigned grid = scan_grid(c, theta > 0);
     Prof p(c, PA_K_POISSON_SCAN);
     launch_scan(c, keep, theta > 0, grid, st, E0, E1, tb, out, shift, cap);
   }
@@ -501,7 +508,7 @@ int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t
   c->dist_phase = 0;
   c->dbg_thresholds = false;
   c->dbg_T4 = c->dbg_T8 = 0u;
-  c->scan_grid_max = 0;
+  c->scan_grid_max[0] = c->scan_grid_max[1] = 0;
   uint32_t k0 = (uint32_t)(cfg->seed & 0xffffffffull), k1 = (uint32_t)(cfg->seed >> 32);
   for (int r = 0; r < 10; ++r) {
     c->key.k0[r] = k0;
@@ -896,14 +903,7 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
     launch(c, "k_dist_tables", k_dist_tables, 1u, RED_THREADS, st, d_params, c->N, sumw, (double)R, (double)c->g_R0, tb, c->nearest);
   }
   {
-    const unsigned tiles_cap = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
     const bool keep = c->lo.n || c->lo.tau;
-    if (c->scan_grid_max == 0) {
-      int per_sm = 0, sms = 0;
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true, false>, SCAN_THREADS, 0);
-      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
-      c->scan_grid_max = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
-    }
     ScanOut out;
     out.off = c->dev<uint32_t>(c->lo.off);
     out.n = c->lo.n ? c->dev<uint32_t>(c->lo.n) : nullptr;
@@ -913,7 +913,7 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
     out.tile_parent = c->dev<uint32_t>(c->lo.tile_parent);
     const int shift = copy_shift_for(c->cfg.L);
     const unsigned long long cap = (unsigned long long)c->cap;
-    const unsigned grid = tiles_cap < (unsigned)c->scan_grid_max ? (tiles_cap ? tiles_cap : 1u) : (unsigned)c->scan_grid_max;
+    const unsigned grid = scan_grid(c, false);
     Prof p(c, PA_K_POISSON_SCAN);
     launch_scan(c, keep, false, grid, st, E0, E1, tb, out, shift, cap);
   }
