@@ -23,7 +23,10 @@
  * closed form, density of states, PA ln Z against the exact finite-L value, closed forms
  * for Q/tau, Poisson moments/chi-square, expneg against exp, Philox against an independent
  * big-integer writing, zero-temperature and detailed-balance checks of the Metropolis
- * rule, global-flip covariance.  No function here is "parity unpinned".
+ * rule, global-flip covariance.  Section D1 (+-J spin glass, overlap histogram): tests/test_oracle_spin_glass.py --
+ * numpy second writing on all 2^16 states of L = 4, parity law of E, gauge covariance onto the pinned ferromagnet,
+ * hand-worked zero-temperature moves, Boltzmann chi-square and PA ln Z of a frustrated sample against enumeration.
+ * No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -141,6 +144,62 @@ void orc_energy_mag(int L, int64_t R, const uint32_t* packed, int32_t* E, int32_
     }
     free(s);
   }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * D1. Second Hamiltonian behind the same step (PAPER.md:213 names the spin glass
+ * as the complex system the method is meant for; reading G27): the 2D +-J Edwards-Anderson
+ * model  H = - sum_<ij> J_ij sigma_i sigma_j  on the same periodic L x L lattice, one sample of
+ * couplings J_ij = +-1 shared by all replicas.  Jx[y*L+x] couples (x,y)-(x+1,y), Jy[y*L+x] couples
+ * (x,y)-(x,y+1), indices modulo L.  Every J = +1 is eq. (6).  E = 2u - 2N with u the number of
+ * unsatisfied bonds; u keeps the parity of the number of negative bonds, so E = 2 (#negative) mod 4.
+ * ---------------------------------------------------------------------------------------- */
+static int32_t energy_of_J(int L, const int8_t* s, const int8_t* Jx, const int8_t* Jy) {
+  int32_t e = 0; /* sum over the 2N bonds, each once: the bond to the right and the bond below every site */
+  for (int y = 0; y < L; ++y)
+    for (int x = 0; x < L; ++x) {
+      int sig = s[y * L + x];
+      e -= Jx[y * L + x] * sig * s[y * L + (x + 1) % L];
+      e -= Jy[y * L + x] * sig * s[((y + 1) % L) * L + x];
+    }
+  return e;
+}
+void orc_energy_mag_J(int L, int64_t R, const uint32_t* packed, const int8_t* Jx, const int8_t* Jy, int32_t* E,
+                      int32_t* M) {
+  int64_t wpr = orc_words_per_replica(L);
+#pragma omp parallel
+  {
+    int8_t* s = (int8_t*)malloc((size_t)L * L);
+#pragma omp for schedule(static)
+    for (int64_t j = 0; j < R; ++j) {
+      unpack_replica(L, packed + j * wpr, s);
+      E[j] = energy_of_J(L, s, Jx, Jy);
+      M[j] = magnetisation_of(L, s);
+    }
+    free(s);
+  }
+}
+int32_t orc_energy_int8_J(int L, const int8_t* s, const int8_t* Jx, const int8_t* Jy) { return energy_of_J(L, s, Jx, Jy); }
+
+/* Order parameter of the spin glass ("the distribution of the order parameter for the spin-glass
+ * model at each annealing step, averaging over the population"): overlap q_ab = sum_i sigma_i^a sigma_i^b of
+ * replica a = j and replica b = j + floor(R/2), j = 0 .. floor(R/2)-1 (reading G28: partners half a population
+ * apart, so that they are not siblings of one recent parent); hist[(q + N) / 2] counts the pairs (q = N mod 2). */
+void orc_overlap_hist(int L, int64_t R, const uint32_t* packed, uint64_t* hist /* N+1 */) {
+  int N = L * L;
+  int64_t wpr = orc_words_per_replica(L), half = R / 2;
+  int8_t* sa = (int8_t*)malloc((size_t)N);
+  int8_t* sb = (int8_t*)malloc((size_t)N);
+  for (int i = 0; i <= N; ++i) hist[i] = 0;
+  for (int64_t j = 0; j < half; ++j) {
+    unpack_replica(L, packed + j * wpr, sa);
+    unpack_replica(L, packed + (j + half) * wpr, sb);
+    int q = 0;
+    for (int i = 0; i < N; ++i) q += sa[i] * sb[i];
+    hist[(q + N) / 2] += 1;
+  }
+  free(sa);
+  free(sb);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -485,8 +544,9 @@ void orc_thresholds(double beta, uint32_t* T4, uint32_t* T8) {
   *T8 = a8 >= 4294967295.0 ? 0xffffffffu : (uint32_t)a8;
 }
 
+/* Jx, Jy: couplings of the +-J model (section D1 below), NULL = the ferromagnet of eq. (6) (every J = +1) */
 static void sweeps_one_replica(int L, int8_t* s, uint64_t seed, uint32_t step, uint32_t slot, int theta,
-                               uint32_t T4, uint32_t T8) {
+                               uint32_t T4, uint32_t T8, const int8_t* Jx, const int8_t* Jy) {
   int half = L / 2;
   for (int t = 0; t < theta; ++t) {
     for (int colour = 0; colour < 2; ++colour) {
@@ -502,11 +562,19 @@ static void sweeps_one_replica(int L, int8_t* s, uint64_t seed, uint32_t step, u
           uint32_t u = 0u; /* bit column p, W[0] most significant */
           for (int b = 0; b < 32; ++b) u |= ((W[b] >> p) & 1u) << (31 - b);
           int sig = s[y * L + x];
-          int nb[4] = {s[y * L + (x + 1) % L], s[y * L + (x + L - 1) % L], s[((y + 1) % L) * L + x],
-                       s[((y + L - 1) % L) * L + x]};
-          int a = 0; /* number of anti-aligned neighbours */
+          int xr = (x + 1) % L, xl = (x + L - 1) % L, yd = (y + 1) % L, yu = (y + L - 1) % L;
+          /* J_b * sigma_b of the four neighbours: right, left, down, up (the bond to the left neighbour is the
+           * left neighbour's Jx, the bond to the upper neighbour is the upper neighbour's Jy) */
+          int nb[4] = {s[y * L + xr], s[y * L + xl], s[yd * L + x], s[yu * L + x]};
+          if (Jx) {
+            nb[0] *= Jx[y * L + x];
+            nb[1] *= Jx[y * L + xl];
+            nb[2] *= Jy[y * L + x];
+            nb[3] *= Jy[yu * L + x];
+          }
+          int a = 0; /* number of unsatisfied bonds of the site (anti-aligned neighbours when J = +1) */
           for (int d = 0; d < 4; ++d) a += (nb[d] != sig);
-          int dE = 8 - 4 * a; /* = 2 sigma sum(neighbours) */
+          int dE = 8 - 4 * a; /* = 2 sigma sum_b J_b sigma_b */
           int flip;
           if (dE <= 0) flip = 1;
           else if (dE == 4) flip = (u < T4);
@@ -519,8 +587,8 @@ static void sweeps_one_replica(int L, int8_t* s, uint64_t seed, uint32_t step, u
 }
 
 /* theta sweeps of replicas first..first+count-1 (slot index = position in the population) */
-void orc_sweeps(int L, int64_t first, int64_t count, uint32_t* packed_base, uint64_t seed, uint32_t step,
-                int theta, uint32_t T4, uint32_t T8) {
+void orc_sweeps_J(int L, int64_t first, int64_t count, uint32_t* packed_base, uint64_t seed, uint32_t step,
+                  int theta, uint32_t T4, uint32_t T8, const int8_t* Jx, const int8_t* Jy) {
   int64_t wpr = orc_words_per_replica(L);
 #pragma omp parallel
   {
@@ -528,17 +596,21 @@ void orc_sweeps(int L, int64_t first, int64_t count, uint32_t* packed_base, uint
 #pragma omp for schedule(static)
     for (int64_t i = first; i < first + count; ++i) {
       unpack_replica(L, packed_base + i * wpr, s);
-      sweeps_one_replica(L, s, seed, step, (uint32_t)i, theta, T4, T8);
+      sweeps_one_replica(L, s, seed, step, (uint32_t)i, theta, T4, T8, Jx, Jy);
       pack_replica(L, s, packed_base + i * wpr);
     }
     free(s);
   }
 }
+void orc_sweeps(int L, int64_t first, int64_t count, uint32_t* packed_base, uint64_t seed, uint32_t step,
+                int theta, uint32_t T4, uint32_t T8) {
+  orc_sweeps_J(L, first, count, packed_base, seed, step, theta, T4, T8, NULL, NULL);
+}
 
 /* sweeps of an arbitrary list of slots, each given as its own packed lattice (used for the
  * sampled parity checks at full size: a replica's sweeps depend only on its lattice and slot) */
-void orc_sweeps_slots(int L, int64_t count, const uint32_t* slots, uint32_t* packed_list, uint64_t seed,
-                      uint32_t step, int theta, uint32_t T4, uint32_t T8) {
+void orc_sweeps_slots_J(int L, int64_t count, const uint32_t* slots, uint32_t* packed_list, uint64_t seed,
+                        uint32_t step, int theta, uint32_t T4, uint32_t T8, const int8_t* Jx, const int8_t* Jy) {
   int64_t wpr = orc_words_per_replica(L);
 #pragma omp parallel
   {
@@ -546,11 +618,15 @@ void orc_sweeps_slots(int L, int64_t count, const uint32_t* slots, uint32_t* pac
 #pragma omp for schedule(static)
     for (int64_t i = 0; i < count; ++i) {
       unpack_replica(L, packed_list + i * wpr, s);
-      sweeps_one_replica(L, s, seed, step, slots[i], theta, T4, T8);
+      sweeps_one_replica(L, s, seed, step, slots[i], theta, T4, T8, Jx, Jy);
       pack_replica(L, s, packed_list + i * wpr);
     }
     free(s);
   }
+}
+void orc_sweeps_slots(int L, int64_t count, const uint32_t* slots, uint32_t* packed_list, uint64_t seed,
+                      uint32_t step, int theta, uint32_t T4, uint32_t T8) {
+  orc_sweeps_slots_J(L, count, slots, packed_list, seed, step, theta, T4, T8, NULL, NULL);
 }
 
 /* ------------------------------------------------------------------------------------------

@@ -56,6 +56,13 @@ def lib():
                                         C.c_uint32, C.c_uint32]),
             "orc_moment_sums": (None, [C.c_int64, i32p, i32p, u64p]),
             "orc_energy_int8": (C.c_int32, [C.c_int, i8p]),
+            "orc_energy_mag_J": (None, [C.c_int, C.c_int64, u32p, i8p, i8p, i32p, i32p]),
+            "orc_energy_int8_J": (C.c_int32, [C.c_int, i8p, i8p, i8p]),
+            "orc_sweeps_J": (None, [C.c_int, C.c_int64, C.c_int64, u32p, C.c_uint64, C.c_uint32, C.c_int,
+                                    C.c_uint32, C.c_uint32, i8p, i8p]),
+            "orc_sweeps_slots_J": (None, [C.c_int, C.c_int64, u32p, u32p, C.c_uint64, C.c_uint32, C.c_int,
+                                          C.c_uint32, C.c_uint32, i8p, i8p]),
+            "orc_overlap_hist": (None, [C.c_int, C.c_int64, u32p, u64p]),
             "orc_pack": (None, [C.c_int, i8p, u32p]),
             "orc_unpack": (None, [C.c_int, u32p, i8p]),
         }
@@ -105,13 +112,33 @@ def init_population(L, R, seed):
     return packed
 
 
-def energy_mag(L, packed):
+def _bonds(L, bonds):
+    """(Jx, Jy): int8 arrays of N couplings +-1, site order b = y*L + x (oracle/pa_oracle.c section D1)"""
+    Jx, Jy = (_c(np.asarray(b).reshape(-1), np.int8) for b in bonds)
+    assert Jx.shape[0] == L * L and Jy.shape[0] == L * L and set(np.unique(np.concatenate([Jx, Jy]))) <= {-1, 1}
+    return Jx, Jy
+
+
+def energy_mag(L, packed, bonds=None):
     packed = _c(packed, np.uint32)
     R = packed.shape[0]
     E = np.zeros(R, np.int32)
     M = np.zeros(R, np.int32)
-    lib().orc_energy_mag(L, R, _p(packed, C.c_uint32), _p(E, C.c_int32), _p(M, C.c_int32))
+    if bonds is None:
+        lib().orc_energy_mag(L, R, _p(packed, C.c_uint32), _p(E, C.c_int32), _p(M, C.c_int32))
+    else:
+        Jx, Jy = _bonds(L, bonds)
+        lib().orc_energy_mag_J(L, R, _p(packed, C.c_uint32), _p(Jx, C.c_int8), _p(Jy, C.c_int8), _p(E, C.c_int32),
+                               _p(M, C.c_int32))
     return E, M
+
+
+def overlap_hist(L, packed):
+    """hist[(q + N) / 2] over the pairs (j, j + R // 2) (oracle/pa_oracle.c section D1, reading G28)"""
+    packed = _c(packed, np.uint32)
+    hist = np.zeros(L * L + 1, np.uint64)
+    lib().orc_overlap_hist(L, packed.shape[0], _p(packed, C.c_uint32), _p(hist, C.c_uint64))
+    return hist
 
 
 def q_ratio(E, dbeta):
@@ -250,21 +277,32 @@ def thresholds(beta):
     return int(t4.value), int(t8.value)
 
 
-def sweeps(L, packed, seed, step, theta, T4, T8, first=0, count=None):
+def sweeps(L, packed, seed, step, theta, T4, T8, first=0, count=None, bonds=None):
     """In place on `packed` (R, wpr) uint32, slots first..first+count-1."""
     assert packed.dtype == np.uint32 and packed.flags.c_contiguous
     if count is None:
         count = packed.shape[0] - first
-    lib().orc_sweeps(L, int(first), int(count), _p(packed, C.c_uint32), C.c_uint64(seed), int(step), int(theta),
-                     int(T4), int(T8))
+    if bonds is None:
+        lib().orc_sweeps(L, int(first), int(count), _p(packed, C.c_uint32), C.c_uint64(seed), int(step), int(theta),
+                         int(T4), int(T8))
+    else:
+        Jx, Jy = _bonds(L, bonds)
+        lib().orc_sweeps_J(L, int(first), int(count), _p(packed, C.c_uint32), C.c_uint64(seed), int(step), int(theta),
+                           int(T4), int(T8), _p(Jx, C.c_int8), _p(Jy, C.c_int8))
 
 
-def sweeps_slots(L, slots, packed_list, seed, step, theta, T4, T8):
+def sweeps_slots(L, slots, packed_list, seed, step, theta, T4, T8, bonds=None):
     """In place on packed_list[i] (the lattice living in population slot slots[i])."""
     assert packed_list.dtype == np.uint32 and packed_list.flags.c_contiguous
     slots = _c(slots, np.uint32)
-    lib().orc_sweeps_slots(L, slots.shape[0], _p(slots, C.c_uint32), _p(packed_list, C.c_uint32), C.c_uint64(seed),
-                           int(step), int(theta), int(T4), int(T8))
+    if bonds is None:
+        lib().orc_sweeps_slots(L, slots.shape[0], _p(slots, C.c_uint32), _p(packed_list, C.c_uint32), C.c_uint64(seed),
+                               int(step), int(theta), int(T4), int(T8))
+    else:
+        Jx, Jy = _bonds(L, bonds)
+        lib().orc_sweeps_slots_J(L, slots.shape[0], _p(slots, C.c_uint32), _p(packed_list, C.c_uint32),
+                                 C.c_uint64(seed), int(step), int(theta), int(T4), int(T8), _p(Jx, C.c_int8),
+                                 _p(Jy, C.c_int8))
 
 
 def moment_sums(E, M):
@@ -278,9 +316,12 @@ def moment_sums(E, M):
     return {"sum_E": vals[0], "sum_E2": vals[1], "sum_absM": vals[2], "sum_M2": vals[3], "sum_M4": vals[4]}
 
 
-def energy_int8(L, s):
+def energy_int8(L, s, bonds=None):
     s = _c(s, np.int8)
-    return int(lib().orc_energy_int8(L, _p(s, C.c_int8)))
+    if bonds is None:
+        return int(lib().orc_energy_int8(L, _p(s, C.c_int8)))
+    Jx, Jy = _bonds(L, bonds)
+    return int(lib().orc_energy_int8_J(L, _p(s, C.c_int8), _p(Jx, C.c_int8), _p(Jy, C.c_int8)))
 
 
 def pack(L, s):
@@ -314,8 +355,9 @@ class OraclePA:
     (R_beta_0), Q (eq. 3), tau (eq. 4), theta (MCMC sweeps per temperature)."""
 
     def __init__(self, L, R0, P=1, seed=0, beta0=0.0, capacity=0, spins=None, policy=POLICY_BALANCED, block=1024,
-                 maxexc=1, rule=RULE_POISSON):
+                 maxexc=1, rule=RULE_POISSON, bonds=None):
         self.rule = int(rule)
+        self.bonds = bonds  # None: the Ising ferromagnet of eq. (6); (Jx, Jy): the +-J model (section D1)
         self.L, self.N, self.R0, self.P, self.seed = int(L), int(L) * int(L), int(R0), int(P), int(seed)
         self.capacity = int(capacity) if capacity else default_capacity(self.R0)
         self.policy, self.block, self.maxexc = int(policy), int(block), int(maxexc)
@@ -324,7 +366,7 @@ class OraclePA:
         # A1: initial population; or a caller-supplied population (test hook)
         self.spins = init_population(self.L, self.R0, self.seed) if spins is None else _c(spins, np.uint32).copy()
         self.R = self.spins.shape[0]
-        self.E, self.M = energy_mag(self.L, self.spins)
+        self.E, self.M = energy_mag(self.L, self.spins, self.bonds)
         # eq. 5 (reading G1): ln Z(beta_i) = ln Omega + sum_l ln Q(beta_{l-1}, beta_l), ln Omega = N ln 2
         self.ln_omega = self.N * math.log(2.0)
         self.sum_lnQ = 0.0
@@ -380,8 +422,8 @@ class OraclePA:
     def equilibrate(self, theta):
         if theta > 0:
             T4, T8 = thresholds(self.beta)
-            sweeps(self.L, self.spins, self.seed, self.step_no, theta, T4, T8)
-            self.E, self.M = energy_mag(self.L, self.spins)
+            sweeps(self.L, self.spins, self.seed, self.step_no, theta, T4, T8, bonds=self.bonds)
+            self.E, self.M = energy_mag(self.L, self.spins, self.bonds)
 
     def step(self, beta_next, theta, tau_override=None):
         info = self.resample(beta_next, tau_override)

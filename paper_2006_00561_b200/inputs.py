@@ -96,3 +96,32 @@ def structured_population(L, R, seed):
     if pad:
         by = np.concatenate([by, np.zeros((R, pad), np.uint8)], axis=1)
     return np.ascontiguousarray(by).view(np.uint32).reshape(R, -1).copy()
+
+
+# ---- second workload: the 2D +-J spin glass ----------------------------------
+def bond_sample(L, seed, p_neg=0.5):
+    """one disorder sample: (Jx, Jy), int8 arrays of N couplings +-1 in site order b = y*L + x; Jx[b] couples
+    (x,y)-(x+1,y), Jy[b] couples (x,y)-(x,y+1), periodic.  P(J = -1) = p_neg (0.5: the symmetric +-J model)."""
+    rng = np.random.default_rng(seed)
+    N = L * L
+    Jx = np.where(rng.random(N) < p_neg, -1, 1).astype(np.int8)
+    Jy = np.where(rng.random(N) < p_neg, -1, 1).astype(np.int8)
+    return Jx, Jy
+
+
+def mattis_bonds(L, seed):
+    """gauge transform of the ferromagnet: J_ij = eps_i eps_j for random eps = +-1 (no frustration); returns
+    (Jx, Jy, eps).  Every quantity of the ferromagnet maps onto this sample by sigma -> eps * sigma."""
+    rng = np.random.default_rng(seed)
+    eps = np.where(rng.random((L, L)) < 0.5, -1, 1).astype(np.int8)
+    Jx = (eps * np.roll(eps, -1, axis=1)).astype(np.int8).reshape(-1)
+    Jy = (eps * np.roll(eps, -1, axis=0)).astype(np.int8).reshape(-1)
+    return Jx, Jy, eps.reshape(-1)
+
+
+def pack_pm1(a):
+    """+-1 values (..., n) with n a multiple of 32 -> little-endian bit string as uint32 words, bit 1 <-> +1 (layout C2)"""
+    a = np.asarray(a)
+    bits = (a > 0).astype(np.uint8)
+    by = np.packbits(bits, axis=-1, bitorder="little")
+    return np.ascontiguousarray(by).view(np.uint32).copy()
