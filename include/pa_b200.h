@@ -9,6 +9,7 @@
  *   equilibrate   theta MCMC (checkerboard Metropolis) sweeps at beta'
  *   observe    population sums of E, E^2, |M|, M^2, M^4; ln Z recursion     PAPER.md:62, :66 eq. (5)
  *   model      H = -(J/2) sum' sigma sigma', J = 1, periodic L x L          PAPER.md:76-80 eq. (6)
+ *              (or, after pa_set_bonds, the +-J spin glass on the same lattice  PAPER.md:213)
  *
  * Conventions
  *   - plain C, no exceptions; every function returns PA_OK (0) or a negative pa_status;
@@ -179,6 +180,19 @@ int pa_debug_set_thresholds(pa_ctx* ctx, int enable, uint32_t T4, uint32_t T8);
 /* test hook: replace the population by R packed lattices (R <= capacity); recomputes E, M, sums, partitions;
  * beta, step counter and ln Z are kept */
 int pa_set_spins(pa_ctx* ctx, const uint32_t* src, int64_t R, int src_on_device);
+
+/* ---- second Hamiltonian: the 2D +-J spin glass (D1) ---------- */
+/* Replace eq. (6) by H = - sum_<ij> J_ij sigma_i sigma_j with one sample of couplings J_ij = +-1 shared by all
+ * replicas.  Jx, Jy: HOST arrays of N/32 uint32 words each, bit layout C2 (bit b = y*L + x, bit 1 <-> J = +1):
+ * Jx couples (x,y)-(x+1,y), Jy couples (x,y)-(x,y+1), indices modulo L.  Both NULL: back to the ferromagnet.  Only
+ * before the first temperature step (PA_EINVAL afterwards); recomputes E_j and the population sums, synchronises.
+ * Everything else (weights, resampling, redistribution, acceptance thresholds, keying) is unchanged: E = 2u - 2N with
+ * u = number of unsatisfied bonds, E = 2 * (#negative bonds) mod 4.  On a multi-GPU shard every rank sets the same sample. */
+int pa_set_bonds(pa_ctx* ctx, const uint32_t* Jx, const uint32_t* Jy);
+/* Order parameter of the spin glass: overlap q = sum_i sigma_i^a sigma_i^b of replica j and replica
+ * j + floor(R/2), j < floor(R/2) (reading G28); hist (HOST, N+1 entries): hist[(q + N) / 2] = number of pairs.
+ * Works for either Hamiltonian; synchronises. */
+int pa_overlap_hist(pa_ctx* ctx, uint64_t* hist);
 
 /* ---- multi-GPU: partitioned redistribution, one rank = one partition -------- */
 /* The population is sharded over `world` ranks in global slot order: rank r owns the contiguous global slots

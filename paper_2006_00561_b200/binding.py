@@ -18,7 +18,7 @@ KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "cop
 
 EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_adaptive_beta", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
            "pa_observables", "pa_spins", "pa_tau", "pa_counts", "pa_parents", "pa_partitions", "pa_thresholds",
-           "pa_set_spins", "pa_debug_set_thresholds", "pa_dist_init", "pa_dist_workspace_bytes", "pa_dist_begin",
+           "pa_set_spins", "pa_debug_set_thresholds", "pa_set_bonds", "pa_overlap_hist", "pa_dist_init", "pa_dist_workspace_bytes", "pa_dist_begin",
            "pa_dist_resample", "pa_dist_exchange_plan", "pa_dist_buffers", "pa_dist_finish", "pa_dist_new_count",
            "pa_dist_abort", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
 
@@ -80,6 +80,8 @@ def load_library():
         "pa_thresholds": (C.c_int, [vp, u32p, u32p]),
         "pa_set_spins": (C.c_int, [vp, vp, C.c_int64, C.c_int]),
         "pa_debug_set_thresholds": (C.c_int, [vp, C.c_int, C.c_uint32, C.c_uint32]),
+        "pa_set_bonds": (C.c_int, [vp, vp, vp]),
+        "pa_overlap_hist": (C.c_int, [vp, vp]),
         "pa_dist_init": (C.c_int, [C.POINTER(PaConfig), C.c_int32, C.c_int32, C.POINTER(vp)]),
         "pa_dist_workspace_bytes": (C.c_uint64, [C.POINTER(PaConfig), C.c_int32]),
         "pa_dist_begin": (C.c_int, [vp, C.c_double, C.c_int32, C.POINTER(PaDistPartial)]),
@@ -304,6 +306,25 @@ class PopulationAnnealer:
 
     def debug_set_thresholds(self, enable, T4=0, T8=0):
         self._check(self._lib.pa_debug_set_thresholds(self._ctx, int(bool(enable)), int(T4), int(T8)))
+
+    # ---- second Hamiltonian: the 2D +-J spin glass (include/pa_b200.h) --------------------------------
+    def set_bonds(self, Jx, Jy):
+        """Jx, Jy: the two coupling planes as uint32 words in layout C2 (bit 1 <-> J = +1), N/32 words each; or
+        both None for the ferromagnet.  Only before the first step."""
+        if Jx is None and Jy is None:
+            self._check(self._lib.pa_set_bonds(self._ctx, None, None))
+            return
+        a = np.ascontiguousarray(Jx, np.uint32).reshape(-1)
+        b = np.ascontiguousarray(Jy, np.uint32).reshape(-1)
+        if a.shape[0] != self.wpr or b.shape[0] != self.wpr:
+            raise PaError(PA_EINVAL, "set_bonds: each coupling plane has N/32 words")
+        self._check(self._lib.pa_set_bonds(self._ctx, _np_ptr(a), _np_ptr(b)))
+
+    def overlap_hist(self):
+        """hist[(q + N) / 2] over the replica pairs (j, j + R // 2)"""
+        h = np.zeros(self.N + 1, np.uint64)
+        self._check(self._lib.pa_overlap_hist(self._ctx, _np_ptr(h)))
+        return h
 
     # ---- multi-GPU shard (include/pa_b200.h "multi-GPU") --------------------------------------------
     def dist_begin(self, beta_next, theta):

@@ -28,7 +28,7 @@ constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
   uint64_t state, params, spins[2], EM[2], off, n, tau, tile_desc, tile_parent, parent_of, red_partial, obs_partial,
-      lev_tau, lev_mu, lev_m, lev_cdf, lev_hist, part[2], part_stats, total;
+      lev_tau, lev_mu, lev_m, lev_cdf, lev_hist, part[2], part_stats, bond_mask, ovl_hist, total;
 };
 
 inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
@@ -90,6 +90,8 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   lo->lev_hist = take(nlev * 4);  // level histogram of the adaptive temperature step (all zero between calls)
   for (int b = 0; b < 2; ++b) lo->part[b] = take(((uint64_t)c->P + 1) * 4);
   lo->part_stats = take((uint64_t)c->P * 16);
+  lo->bond_mask = take(N / 2);        // +-J model: negative-bond masks, 2 colours x N/64 plane words x 4 bonds (pa_sweep.cuh)
+  lo->ovl_hist = take(nlev * 8);      // overlap histogram (pa_overlap_hist)
   lo->total = o;
   return true;
 }
@@ -117,6 +119,8 @@ struct pa_ctx {
   int64_t launches;
   bool profile, profile_span;
   int nearest;  // PA_RESAMPLE_NEAREST: nearest-integer copy counts instead of Poisson
+  bool glass;   // pa_set_bonds: the +-J Hamiltonian (sweep kernels compiled with the coupling masks)
+  int e_off;    // E mod 4 of every configuration (0 unless the sample has an odd number of negative bonds: 2)
   bool attempt_failed;  // the last pa_step / pa_run ended with an uncommitted step: off / n / tau hold that attempt
   // multi-GPU shard (pa_dist_*): rank = partition
   int rank, world;          // world = 0: not a shard
@@ -223,13 +227,16 @@ void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
   int32_t *em0 = c->dev<int32_t>(c->lo.EM[0]), *em1 = c->dev<int32_t>(c->lo.EM[1]);
   const DevState* st = c->dev<DevState>(c->lo.state);
   const uint32_t* parent_of = c->dev<uint32_t>(c->lo.parent_of);
+  const uint4* bm = c->dev<uint4>(c->lo.bond_mask);
   if constexpr (L >= 64) {
     const unsigned grid = (unsigned)(((uint64_t)c->cap + Geo<L>::RPB - 1) / Geo<L>::RPB);
-    launch(c, "k_sweep", k_sweep<L>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of);
+    if (c->glass) launch(c, "k_sweep", k_sweep<L, true>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+    else launch(c, "k_sweep", k_sweep<L, false>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
   } else {
     const uint64_t threads = ((uint64_t)c->cap + 1) / 2 * SGeo<L>::G;  // a group of G lanes holds two replicas
     const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
-    launch(c, "k_sweep_small", k_sweep_small<L>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of);
+    if (c->glass) launch(c, "k_sweep_small", k_sweep_small<L, true>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+    else launch(c, "k_sweep_small", k_sweep_small<L, false>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
   }
 }
 // mode 2: theta sweeps of the resampled population (lattices gathered from the parents' slots); mode 1: energies only
@@ -378,6 +385,10 @@ __global__ void k_dist_set_new(DevState* st, unsigned long long count, unsigned 
   st->Rnew = count;
   st->slot0_new = slot0_new;
 }
+__global__ void k_set_e_off(DevState* st, int e_off) {
+  st->e_off = e_off;
+  st->obs_done = 0u;  // the population sums are taken again (k_observe's last-block counter)
+}
 __global__ void k_clear_status(DevState* st) {
   st->status = 0u;
   st->obs_done = 0u;
@@ -496,6 +507,8 @@ int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t
   c->profile = (cfg->flags & PA_PROFILE) != 0;
   c->profile_span = (cfg->flags & PA_PROFILE_SPAN) != 0;
   c->nearest = (cfg->flags & PA_RESAMPLE_NEAREST) ? 1 : 0;
+  c->glass = false;
+  c->e_off = 0;
   c->launches = 0;
   {  // a small population (config 1: 1024 replicas) is latency-bound: one block per 4096 replicas, at most 4 per SM
     const int64_t want = (c->cap + 4095) / 4096;
@@ -631,7 +644,7 @@ int pa_energies(pa_ctx* c, int32_t* E, int32_t* M, int64_t n, int dst_on_device)
   const int32_t* em = c->dev<int32_t>(c->lo.EM[cur]);
   const unsigned grid = (unsigned)((n + 255) / 256);
   if (dst_on_device) {
-    k_unpack_em<<<grid, 256, 0, c->stream>>>(em, E, M, (unsigned long long)n);
+    k_unpack_em<<<grid, 256, 0, c->stream>>>(em, E, M, (unsigned long long)n, c->e_off);
     c->launches += 1;
     CK(cudaStreamSynchronize(c->stream));
     return PA_OK;
@@ -639,7 +652,7 @@ int pa_energies(pa_ctx* c, int32_t* E, int32_t* M, int64_t n, int dst_on_device)
   // host destination: unpack into the spare population buffer (free outside a step; cap * S >= 8 n bytes), then copy
   int32_t* sE = c->dev<int32_t>(c->lo.spins[cur ^ 1u]);
   int32_t* sM = sE + ((n + 3) / 4) * 4;
-  k_unpack_em<<<grid, 256, 0, c->stream>>>(em, E ? sE : nullptr, M ? sM : nullptr, (unsigned long long)n);
+  k_unpack_em<<<grid, 256, 0, c->stream>>>(em, E ? sE : nullptr, M ? sM : nullptr, (unsigned long long)n, c->e_off);
   c->launches += 1;
   int rc = PA_OK;
   if (E) rc = copy_out(c, E, sE, (size_t)n * 4, 0);
@@ -760,6 +773,63 @@ int pa_set_spins(pa_ctx* c, const uint32_t* src, int64_t R, int src_on_device) {
   launch_sweep(c, 0, 0u, 0u, 1);
   launch_observe(c, nullptr, 1);
   return sync_state(c);
+}
+
+// ---- second Hamiltonian: the 2D +-J spin glass (D1) -----------------------------
+int pa_set_bonds(pa_ctx* c, const uint32_t* Jx, const uint32_t* Jy) {
+  if (!c || ((Jx == nullptr) != (Jy == nullptr))) return fail(c, PA_EINVAL, "pa_set_bonds: give both coupling planes or neither");
+  if (c->steps != 0 || c->dist_phase != 0) return fail(c, PA_EINVAL, "pa_set_bonds: only before the first temperature step");
+  if (int rc = bind_device(c)) return rc;
+  const int L = c->cfg.L, N = c->N, HB = L / 2, groups = N / 64;
+  int e_off = 0;
+  if (Jx) {
+    // coupling of the bond that leaves site (x, y) to the right (Jx) / downwards (Jy): bit 1 <-> J = +1
+    auto neg = [&](const uint32_t* J, int x, int y) {
+      const int b = ((y + L) % L) * L + ((x + L) % L);
+      return ((J[b >> 5] >> (b & 31)) & 1u) == 0u;
+    };
+    std::vector<uint32_t> mask((size_t)2 * groups * 4, 0u);
+    int nneg = 0;
+    for (int b = 0; b < N; ++b) nneg += (int)neg(Jx, b % L, b / L) + (int)neg(Jy, b % L, b / L);
+    e_off = 2 * (nneg & 1);
+    for (int C = 0; C < 2; ++C)
+      for (int y = 0; y < L; ++y)
+        for (int k = 0; k < HB; ++k) {
+          const int odd = (y + C) & 1, x = 2 * k + odd;     // the active site (pa_sweep.cuh: plane C of row y, bit k)
+          const int q = y * HB + k;                         // its ordinal in the half-sweep: group q >> 5, bit q & 31
+          uint32_t* m = &mask[((size_t)C * groups + (q >> 5)) * 4];
+          const uint32_t bit = 1u << (q & 31);
+          if (neg(Jy, x, y - 1)) m[0] |= bit;               // up: the bond below (x, y-1)
+          if (neg(Jy, x, y)) m[1] |= bit;                   // down
+          // same plane bit k of the other colour is x+1 on an even (y+C), x-1 on an odd one; the shifted bit is the other side
+          if (neg(Jx, odd ? x - 1 : x, y)) m[2] |= bit;
+          if (neg(Jx, odd ? x : x - 1, y)) m[3] |= bit;
+        }
+    CK(cudaMemcpyAsync(c->dev<char>(c->lo.bond_mask), mask.data(), mask.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));  // `mask` is pageable host memory that dies with this scope
+  }
+  c->glass = Jx != nullptr;
+  c->e_off = e_off;
+  k_set_e_off<<<1, 1, 0, c->stream>>>(c->dev<DevState>(c->lo.state), e_off);
+  c->launches += 1;
+  launch_sweep(c, 0, 0u, 0u, 1);   // E_j, M_j of the current population under the new Hamiltonian
+  launch_observe(c, nullptr, 1);
+  return sync_state(c);
+}
+
+int pa_overlap_hist(pa_ctx* c, uint64_t* hist) {
+  if (!c || !hist) return fail(c, PA_EINVAL, "pa_overlap_hist: bad arguments");
+  if (c->world > 0) return fail(c, PA_EINVAL, "pa_overlap_hist: not available on a multi-GPU shard (partners live on other ranks)");
+  if (int rc = bind_device(c)) return rc;
+  unsigned long long* d_hist = c->dev<unsigned long long>(c->lo.ovl_hist);
+  CK(cudaMemsetAsync(d_hist, 0, ((size_t)c->N + 1) * 8, c->stream));
+  const int64_t pairs = c->R / 2;
+  int64_t want = (pairs + 63) / 64;  // 8 pairs per block pass
+  const unsigned grid = (unsigned)(want < 1 ? 1 : (want > 148 * 8 ? 148 * 8 : want));
+  k_overlap_hist<<<grid, OVL_THREADS, 0, c->stream>>>(c->dev<DevState>(c->lo.state), c->dev<uint32_t>(c->lo.spins[0]),
+                                                     c->dev<uint32_t>(c->lo.spins[1]), d_hist, c->N);
+  c->launches += 1;
+  return copy_out(c, hist, d_hist, ((size_t)c->N + 1) * 8, 0);
 }
 
 // ---- multi-GPU: partitioned redistribution ------------------------------------------------------------

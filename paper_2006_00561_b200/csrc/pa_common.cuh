@@ -39,7 +39,7 @@ struct DevState {
   unsigned int obs_done;
   unsigned int T4, T8;           // thresholds of the last committed step with theta > 0
   int lev_lo, lev_hi;            // occupied energy levels (E + 2N)/4 of the CURRENT population, inclusive (by k_observe)
-  unsigned int pad_[1];
+  int e_off;                     // E mod 4 of every configuration: 0 for the ferromagnet, 2 * (#negative bonds & 1) for a +-J sample
   double Q_committed;            // Q of the last COMMITTED step (Q above is overwritten by every attempt)
   double adaptive_dbeta;         // result of the last k_adaptive_step
 };
@@ -86,14 +86,15 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 
 __device__ __forceinline__ uint32_t ctr3(uint32_t tag, uint32_t step) { return (tag << 28) | step; }
 
-// E and M of a replica share ONE 32-bit word in HBM: E / 4 in the upper half, M / 2 in the lower half.  Both are exact
-// (E = 0 mod 4: DESIGN.md C1; M = 2 popc - N with N even) and fit 16 bits for every supported lattice (|E / 4|, |M / 2|
-// <= N / 2 = 8192 at L = 128).  Halves the E/M traffic of the reductions and of the redistribution copy; the energy
-// level of C5 / A4 is simply the upper half + N / 2.
+// E and M of a replica share ONE 32-bit word in HBM: floor(E / 4) in the upper half, M / 2 in the lower half.  Both are
+// exact (E = e_off mod 4 with e_off = 0 for the ferromagnet, C1, and 0 or 2 for a +-J sample, D1; M = 2 popc - N
+// with N even) and fit 16 bits for every supported lattice (|E / 4|, |M / 2| <= N / 2 = 8192 at L = 128).  Halves the E/M
+// traffic of the reductions and of the redistribution copy; the energy level of C5 / A4 is simply the upper half + N / 2,
+// and the energy of level lev is 4 lev - 2N + e_off.
 __device__ __forceinline__ int32_t pack_em(int E, int M) {
   return (int32_t)(((uint32_t)(E >> 2) << 16) | ((uint32_t)(M >> 1) & 0xffffu));
 }
-__device__ __forceinline__ int em_energy(int32_t w) { return (w >> 16) * 4; }
+__device__ __forceinline__ int em_energy(int32_t w, int e_off) { return (w >> 16) * 4 + e_off; }
 __device__ __forceinline__ int em_level(int32_t w, int N) { return (w >> 16) + (N >> 1); }  // (E + 2N) / 4
 __device__ __forceinline__ int em_mag(int32_t w) { return ((int32_t)((uint32_t)w << 16) >> 16) * 2; }
 

@@ -27,11 +27,11 @@ __global__ void k_init(const DevState* __restrict__ st, uint32_t* __restrict__ s
 
 // getters: packed E/4 : M/2 words -> separate int32 arrays
 __global__ void k_unpack_em(const int32_t* __restrict__ EM, int32_t* __restrict__ E, int32_t* __restrict__ M,
-                            unsigned long long n) {
+                            unsigned long long n, int e_off) {
   const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int32_t w = EM[i];
-  if (E) E[i] = em_energy(w);
+  if (E) E[i] = em_energy(w, e_off);
   if (M) M[i] = em_mag(w);
 }
 
@@ -178,8 +178,9 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
   unsigned long long sE2 = 0, sA = 0, sM2 = 0;
   U128 sM4 = {0ull, 0ull};
   int emin = 0x7fffffff, emax = -0x7fffffff;  // occupied energy range: the level window of the next step's tables
+  const int e_off = st->e_off;
   auto add = [&](int w) {
-    const int ei = em_energy(w), mi = em_mag(w);
+    const int ei = em_energy(w, e_off), mi = em_mag(w);
     emin = min(emin, ei);
     emax = max(emax, ei);
     const long long e = ei;
@@ -315,6 +316,45 @@ k_observe(DevState* st, const StepParams* __restrict__ sp, const int32_t* __rest
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Order parameter of the spin glass (D1, reading G28): overlap q = sum_i sigma_i^a sigma_i^b =
+// N - 2 popc(a xor b) of replica j and replica j + floor(R/2), histogram hist[(q + N) / 2] over j < floor(R/2).
+// One warp per pair, lanes stride over the words of the two lattices (coalesced 128-byte rows); block-level histogram in
+// shared memory when it fits (N + 1 <= 4097 bins), global atomics otherwise.  HBM: the population is read once.
+// ---------------------------------------------------------------------------------------------------
+constexpr int OVL_THREADS = 256;
+constexpr int OVL_SMEM_BINS = 4097;
+__global__ void __launch_bounds__(OVL_THREADS)
+k_overlap_hist(const DevState* __restrict__ st, const uint32_t* __restrict__ spins0, const uint32_t* __restrict__ spins1,
+               unsigned long long* __restrict__ hist, const int N) {
+  __shared__ unsigned s_hist[OVL_SMEM_BINS];
+  const bool use_smem = N + 1 <= OVL_SMEM_BINS;
+  if (use_smem)
+    for (int i = threadIdx.x; i <= N; i += OVL_THREADS) s_hist[i] = 0u;
+  __syncthreads();
+  const uint32_t* __restrict__ spins = st->cur ? spins1 : spins0;
+  const unsigned long long half = st->R / 2ull;
+  const int wrep = N / 32, lane = threadIdx.x & 31;
+  const unsigned long long warps = (unsigned long long)gridDim.x * (OVL_THREADS / 32);
+  for (unsigned long long j = (unsigned long long)blockIdx.x * (OVL_THREADS / 32) + (threadIdx.x >> 5); j < half; j += warps) {
+    const uint32_t* a = spins + j * wrep;
+    const uint32_t* b = spins + (j + half) * wrep;
+    int diff = 0;
+    for (int w = lane; w < wrep; w += 32) diff += __popc(__ldg(a + w) ^ __ldg(b + w));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) diff += __shfl_xor_sync(0xffffffffu, diff, o);
+    if (lane == 0) {
+      const int bin = N - diff;  // (q + N) / 2 with q = N - 2 diff
+      if (use_smem) atomicAdd(&s_hist[bin], 1u);
+      else atomicAdd(&hist[bin], 1ull);
+    }
+  }
+  __syncthreads();
+  if (use_smem)
+    for (int i = threadIdx.x; i <= N; i += OVL_THREADS)
+      if (s_hist[i]) atomicAdd(&hist[i], (unsigned long long)s_hist[i]);
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Adaptive temperature step (PAPER.md:108 -> ref. [4]; A9, reading G25): the largest dbeta in (0, dbeta_max]
 // whose histogram overlap alpha(dbeta) = (1/R) sum_j min(1, tau_j(dbeta)) is >= target.  tau_j depends on j only through
 // the energy level, so one pass builds the level histogram of the population (k_level_hist) and one block bisects on it
@@ -348,14 +388,15 @@ k_adaptive_step(DevState* st, unsigned* __restrict__ hist, const int N, const do
   __shared__ double s_red[OBS_THREADS / 32];
   const int lev_lo = st->lev_lo, lev_hi = st->lev_hi;
   const double R = (double)st->R;
+  const int e_off = st->e_off;
   auto overlap = [&](double dbeta) {
     double sw = 0.0;
     for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += OBS_THREADS)
-      sw += (double)hist[lev] * exp(-dbeta * (double)(4 * lev - 2 * N));
+      sw += (double)hist[lev] * exp(-dbeta * (double)(4 * lev - 2 * N + e_off));
     const double Q = block_sum_256(sw, s_red) / R;
     double sa = 0.0;
     for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += OBS_THREADS) {
-      const double tau = exp(-dbeta * (double)(4 * lev - 2 * N)) / Q;
+      const double tau = exp(-dbeta * (double)(4 * lev - 2 * N + e_off)) / Q;
       sa += (double)hist[lev] * (tau < 1.0 ? tau : 1.0);
     }
     return block_sum_256(sa, s_red) / R;

@@ -24,10 +24,11 @@ struct LevelTables {
   double* cdf;      // [N+1][65]  F_k of Poisson(mu) built by the A4 recurrence
 };
 
-// w_e = exp(-dbeta * e) of energy level lev (e = 4 lev - 2N): the ONE expression that k_q_reduce (eq. 3) and
+// w_e = exp(-dbeta * e) of energy level lev (e = 4 lev - 2N + e_off; e_off = 0 unless a +-J sample has an odd number of
+// negative bonds, pa_common.cuh): the ONE expression that k_q_reduce (eq. 3) and
 // k_levels_tau (eq. 4) both evaluate, so that tau = w / Q uses the very bits that were summed into Q
-__device__ __forceinline__ double level_weight(double dbeta, int lev, int N) {
-  const double e = (double)(4 * lev - 2 * N);
+__device__ __forceinline__ double level_weight(double dbeta, int lev, int N, int e_off) {
+  const double e = (double)(4 * lev - 2 * N + e_off);
   return exp(-dbeta * e);
 }
 
@@ -52,9 +53,9 @@ __device__ __forceinline__ double expneg_a4(double mu) {
   return p;
 }
 
-__device__ __forceinline__ void level_tables(double dbeta, int lev, int N, double Q, double scale, const LevelTables& tb,
+__device__ __forceinline__ void level_tables(double dbeta, int lev, int N, int e_off, double Q, double scale, const LevelTables& tb,
                                              const bool nearest) {
-  const double tau = __ddiv_rn(level_weight(dbeta, lev, N), Q);
+  const double tau = __ddiv_rn(level_weight(dbeta, lev, N, e_off), Q);
   const double lambda = __dmul_rn(tau, scale);
   tb.tau[lev] = tau;
   double* F = tb.cdf + (size_t)lev * PO_ROW;
@@ -137,13 +138,13 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
   const unsigned long long R = st->R;
   const double dbeta = sp->dbeta;
   const int lev_lo = st->lev_lo, W = st->lev_hi - lev_lo + 1;
-  const int halfN = N >> 1;
+  const int halfN = N >> 1, e_off = st->e_off;
   const unsigned long long nvec = R / 4;
   const int4* __restrict__ E4 = reinterpret_cast<const int4*>(E);  // the buffers are 256-byte aligned
   __shared__ double s_w[QW_MAX];
   double acc = 0.0;
   if (W <= QW_MAX) {
-    for (int i = threadIdx.x; i < W; i += RED_THREADS) s_w[i] = level_weight(dbeta, lev_lo + i, N);
+    for (int i = threadIdx.x; i < W; i += RED_THREADS) s_w[i] = level_weight(dbeta, lev_lo + i, N, e_off);
     __syncthreads();
     const int shift = halfN - lev_lo;  // level - lev_lo = E / 4 + N / 2 - lev_lo
     auto wl = [&](int w) { return s_w[(w >> 16) + shift]; };
@@ -170,7 +171,7 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
     }
     for (unsigned long long j = 4 * nvec + tid; j < R; j += stride) acc += wl(E[j]);
   } else {
-    auto wl = [&](int w) { return level_weight(dbeta, (w >> 16) + halfN, N); };
+    auto wl = [&](int w) { return level_weight(dbeta, (w >> 16) + halfN, N, e_off); };
     unsigned long long v = tid;
     for (; v < nvec; v += stride) {
       const int4 a = __ldg(E4 + v);
@@ -221,7 +222,7 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
   {
     const double Q = s_Q, scale = R0 / (double)R;
     const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
-    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(dbeta, lev, N, Q, scale, tb, nearest != 0);
+    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(dbeta, lev, N, e_off, Q, scale, tb, nearest != 0);
   }
 }
 
@@ -243,7 +244,7 @@ k_dist_tables(DevState* st, const StepParams* __restrict__ sp, int N, double sum
     st->scale = scale;
   }
   const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
-  for (int lev = st->lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(sp->dbeta, lev, N, Q, scale, tb, nearest != 0);
+  for (int lev = st->lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(sp->dbeta, lev, N, st->e_off, Q, scale, tb, nearest != 0);
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -264,6 +264,26 @@ __device__ __forceinline__ void neighbour_classes(uint32_t tt, uint32_t U, uint3
   ge1 = any3 | d3;
 }
 
+// Second Hamiltonian (D1: 2D +-J spin glass, H = -sum J_ij sigma_i sigma_j): a bond is unsatisfied iff the spins
+// differ XOR the coupling is negative.  The host tabulates, for every colour C and every plane word (= keyed group) of a
+// half-sweep, which of the four bonds of each active site are negative: bond_mask[C * N/64 + group] = {up, down, same-bit
+// neighbour of the row, shifted neighbour of the row}, bit p = site ordinal p of the group.  With the masks XORed into the
+// four difference words "a" counts unsatisfied bonds and everything downstream (classes, thresholds, E = 2u - 2N) is
+// unchanged.  SG = false compiles the masks away (ferromagnet, eq. 6).
+template <bool SG>
+__device__ __forceinline__ void neighbour_classes_j(uint32_t tt, uint32_t U, uint32_t D, uint32_t Sm, uint32_t B,
+                                                    const uint4& mk, uint32_t& ge1, uint32_t& ge2) {
+  if constexpr (SG) {
+    const uint32_t d0 = tt ^ U ^ mk.x, d1 = tt ^ D ^ mk.y, d2 = tt ^ Sm ^ mk.z, d3 = tt ^ B ^ mk.w;
+    const uint32_t maj = (d0 & d1) | (d0 & d2) | (d1 & d2);
+    const uint32_t any3 = d0 | d1 | d2;
+    ge2 = maj | (any3 & d3);
+    ge1 = any3 | d3;
+  } else {
+    neighbour_classes(tt, U, D, Sm, B, ge1, ge2);
+  }
+}
+
 constexpr int SWEEP_THREADS = PA_SWEEP_THREADS;
 
 // =====================================================================================================
@@ -312,10 +332,11 @@ __device__ __forceinline__ void rot_row(const uint32_t (&s)[Geo<L>::WPP], int di
 }
 
 // One half-sweep of colour C on the lane's rows of the warp's RW replicas.  T = plane C (updated), S = plane 1-C.
-template <int L, int C>
+template <int L, int C, bool SG>
 __device__ __forceinline__ void half_sweep(Lattice<L> (&lat)[Geo<L>::RW], uint32_t q, int g,
                                            uint32_t slot0, uint32_t slot_base, const bool (&valid)[Geo<L>::RW],
-                                           uint32_t t, uint32_t c3, const PhiloxKey& key, const SweepArgs& sa) {
+                                           uint32_t t, uint32_t c3, const PhiloxKey& key, const SweepArgs& sa,
+                                           const uint4* __restrict__ bond_mask) {
   using G_ = Geo<L>;
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int NWL = G_::NWL;
@@ -343,7 +364,9 @@ __device__ __forceinline__ void half_sweep(Lattice<L> (&lat)[Geo<L>::RW], uint32
         const int w = rep * G_::NWR + r * G_::WPP + i;
         const uint32_t U = (r > 0) ? S[r > 0 ? r - 1 : 0][i] : up[i];
         const uint32_t D = (r < G_::RPL - 1) ? S[r < G_::RPL - 1 ? r + 1 : 0][i] : dn[i];
-        neighbour_classes(T[r][i], U, D, S[r][i], B[i], ge1[w], ge2[w]);
+        uint4 mk = make_uint4(0u, 0u, 0u, 0u);
+        if constexpr (SG) mk = __ldg(bond_mask + C * (G_::N / 64) + y * G_::WPP + i);  // shared by all replicas: L1 resident
+        neighbour_classes_j<SG>(T[r][i], U, D, S[r][i], B[i], mk, ge1[w], ge2[w]);
         if (!valid[rep]) ge2[w] = 0xffffffffu;  // a replica past the population has nothing to decide
         call0[w] = 8u * ((uint32_t)y * G_::WPP + (uint32_t)i);  // group = y * WPP + i
         slots[w] = slot0 + (uint32_t)rep;
@@ -360,8 +383,9 @@ __device__ __forceinline__ void half_sweep(Lattice<L> (&lat)[Geo<L>::RW], uint32
 }
 
 // number of anti-aligned bonds u (each bond has exactly one colour-0 end) and number of up spins
-template <int L>
-__device__ __forceinline__ void count_bonds(const Lattice<L>& lat, int g, int& unsat, int& ups) {
+template <int L, bool SG>
+__device__ __forceinline__ void count_bonds(const Lattice<L>& lat, int g, const uint4* __restrict__ bond_mask, int& unsat,
+                                            int& ups) {
   using G_ = Geo<L>;
   constexpr unsigned FULL = 0xffffffffu;
   const uint32_t(&T)[G_::RPL][G_::WPP] = lat.p[0];
@@ -384,7 +408,9 @@ __device__ __forceinline__ void count_bonds(const Lattice<L>& lat, int g, int& u
       const uint32_t U = (r > 0) ? S[r > 0 ? r - 1 : 0][i] : up[i];
       const uint32_t D = (r < G_::RPL - 1) ? S[r < G_::RPL - 1 ? r + 1 : 0][i] : dn[i];
       const uint32_t tt = T[r][i];
-      u += __popc(tt ^ U) + __popc(tt ^ D) + __popc(tt ^ S[r][i]) + __popc(tt ^ B[i]);
+      uint4 mk = make_uint4(0u, 0u, 0u, 0u);
+      if constexpr (SG) mk = __ldg(bond_mask + y * G_::WPP + i);  // colour 0
+      u += __popc(tt ^ U ^ mk.x) + __popc(tt ^ D ^ mk.y) + __popc(tt ^ S[r][i] ^ mk.z) + __popc(tt ^ B[i] ^ mk.w);
       pc += __popc(tt) + __popc(S[r][i]);
     }
   }
@@ -417,11 +443,12 @@ __device__ __forceinline__ void planes_to_row(const uint32_t (&p0)[Geo<L>::WPP],
   }
 }
 
-template <int L>
+template <int L, bool SG>
 __global__ void __launch_bounds__(SWEEP_THREADS, (L >= 128 ? PA_SWEEP_MINB128 : PA_SWEEP_MINB64))
 k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
         int32_t* __restrict__ EM0, int32_t* __restrict__ EM1,
-        const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of) {
+        const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of,
+        const uint4* __restrict__ bond_mask) {
   using G_ = Geo<L>;
   static_assert(L >= 64, "k_sweep_small handles L < 64");
   grid_dependency_wait();
@@ -476,8 +503,8 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
     if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
     __syncthreads();
     for (int t = 0; t < theta; ++t) {
-      half_sweep<L, 0>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa);
-      half_sweep<L, 1>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa);
+      half_sweep<L, 0, SG>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa, bond_mask);
+      half_sweep<L, 1, SG>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa, bond_mask);
     }
   }
 
@@ -487,7 +514,7 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
     const unsigned long long slot64 = slot0_64 + rep;
     // ---- a8: E = 2u - 2N, M = 2*popc - N ----------------------------------------------------------
     int unsat, ups;
-    count_bonds<L>(lat[rep], g, unsat, ups);
+    count_bonds<L, SG>(lat[rep], g, bond_mask, unsat, ups);
 #pragma unroll
     for (int o = G_::G / 2; o > 0; o >>= 1) {
       unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
@@ -546,11 +573,12 @@ __device__ __forceinline__ void small_neighbours(uint32_t S, int g, uint32_t& U,
   B = C == 0 ? ((rotl & G_::ER) | (rotr & ~G_::ER)) : ((rotr & G_::ER) | (rotl & ~G_::ER));
 }
 
-template <int L>
+template <int L, bool SG>
 __global__ void __launch_bounds__(SWEEP_THREADS)
 k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
               int32_t* __restrict__ EM0, int32_t* __restrict__ EM1,
-              const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of) {
+              const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of,
+              const uint4* __restrict__ bond_mask) {
   using G_ = SGeo<L>;
   static_assert(L == 8 || L == 16 || L == 32, "");
   grid_dependency_wait();
@@ -569,6 +597,11 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
   const int g = (int)(tid % G_::G);
   const unsigned long long slot_base64 = ((unsigned long long)blockIdx.x * SWEEP_THREADS / G_::G) * NR;
   if (slot_base64 >= count) return;  // block-uniform: the sweeps below contain block barriers
+  uint4 mk[2] = {make_uint4(0u, 0u, 0u, 0u), make_uint4(0u, 0u, 0u, 0u)};  // negative bonds of the lane's word, per colour
+  if constexpr (SG) {
+    mk[0] = __ldg(bond_mask + g);
+    mk[1] = __ldg(bond_mask + G_::G + g);
+  }
   const uint32_t slot_base = (uint32_t)slot_base64;
   unsigned long long slot64[NR];
   bool valid[NR];
@@ -610,7 +643,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
         for (int r = 0; r < NR; ++r) {
           uint32_t U, D, B;
           small_neighbours<L, 0>(p[r][1], g, U, D, B);
-          neighbour_classes(p[r][0], U, D, p[r][1], B, ge1[r], ge2[r]);
+          neighbour_classes_j<SG>(p[r][0], U, D, p[r][1], B, mk[0], ge1[r], ge2[r]);
           if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }  // padding never holds the warp back
         }
         queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 0u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t, c3, key,
@@ -624,7 +657,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
         for (int r = 0; r < NR; ++r) {
           uint32_t U, D, B;
           small_neighbours<L, 1>(p[r][0], g, U, D, B);
-          neighbour_classes(p[r][1], U, D, p[r][0], B, ge1[r], ge2[r]);
+          neighbour_classes_j<SG>(p[r][1], U, D, p[r][0], B, mk[1], ge1[r], ge2[r]);
           if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }
         }
         queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 1u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t + 1u, c3,
@@ -640,7 +673,8 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
     // ---- a8: every bond has exactly one colour-0 end ----------------------------------------------
     uint32_t U, D, B;
     small_neighbours<L, 0>(p[r][1], g, U, D, B);
-    int unsat = __popc(p[r][0] ^ U) + __popc(p[r][0] ^ D) + __popc(p[r][0] ^ p[r][1]) + __popc(p[r][0] ^ B);
+    int unsat = __popc(p[r][0] ^ U ^ mk[0].x) + __popc(p[r][0] ^ D ^ mk[0].y) + __popc(p[r][0] ^ p[r][1] ^ mk[0].z) +
+                __popc(p[r][0] ^ B ^ mk[0].w);
     int ups = __popc(p[r][0]) + __popc(p[r][1]);
 #pragma unroll
     for (int o = G_::G / 2; o > 0; o >>= 1) {

@@ -31,15 +31,17 @@ def rel(a, b):
     return abs(a - b) / max(abs(b), 1e-300)
 
 
-def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None, policy=0, block=1024, maxexc=1, rule=0):
+def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None, policy=0, block=1024, maxexc=1, rule=0, bonds=None):
     b = _binding()
     gpu = b.PopulationAnnealer(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity,
                                flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS | (b.PA_RESAMPLE_NEAREST if rule else 0), policy=policy,
                                block=block, maxexc=maxexc)
     if spins is not None:
         gpu.set_spins(spins)
+    if bonds is not None:  # second Hamiltonian: +-J couplings (Jx, Jy) as int8 arrays in site order
+        gpu.set_bonds(inputs.pack_pm1(bonds[0]), inputs.pack_pm1(bonds[1]))
     ora = orc.OraclePA(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity, spins=spins, policy=policy, block=block,
-                       maxexc=maxexc, rule=rule)
+                       maxexc=maxexc, rule=rule, bonds=bonds)
     return gpu, ora
 
 
@@ -94,7 +96,7 @@ def lockstep(gpu, ora, betas, theta, sweep_slots=None):
             assert np.array_equal(before, spins_before[parent[slots]])
             if theta > 0:
                 T4, T8 = orc.thresholds(beta)
-                orc.sweeps_slots(L, slots, before, ora.seed, ora.step_no, theta, T4, T8)
+                orc.sweeps_slots(L, slots, before, ora.seed, ora.step_no, theta, T4, T8, bonds=ora.bonds)
             got = gpu.spins()
             assert np.array_equal(got[slots], before), "step %d: sampled sweeps" % k
             if theta == 0:  # no sweeps: the whole redistributed population is comparable
@@ -102,7 +104,7 @@ def lockstep(gpu, ora, betas, theta, sweep_slots=None):
             # adopt the GPU population for the next step, after checking E/M of ALL replicas against the oracle's
             # energy function (plain definition) -- keeps the oracle in lock-step without sweeping everything
             E, M = gpu.energies()
-            Eo, Mo = orc.energy_mag(L, got)
+            Eo, Mo = orc.energy_mag(L, got, ora.bonds)
             assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
             ora.spins, ora.E, ora.M = got, Eo, Mo
             og, oo = gpu.observables(), ora.observables()
