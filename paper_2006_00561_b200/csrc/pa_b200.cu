@@ -197,6 +197,7 @@ SweepArgs sweep_args(int theta, uint32_t T4, uint32_t T8, int mode) {
     sa.a[i] = ((T4 >> (31 - i)) & 1u) ? 0xffffffffu : 0u;
     sa.b[i] = ((T8 >> (31 - i)) & 1u) ? 0xffffffffu : 0u;
   }
+  for (int i = 0; i < 8; ++i) sa.kase[i] = 2u * ((T4 >> (31 - i)) & 1u) + ((T8 >> (31 - i)) & 1u);
   sa.theta = theta;
   sa.mode = mode;
   return sa;
@@ -234,9 +235,9 @@ void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
     else launch(c, "k_sweep", k_sweep<L, false>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
   } else {
     const uint64_t threads = ((uint64_t)c->cap + 1) / 2 * SGeo<L>::G;  // a group of G lanes holds two replicas
-    const unsigned grid = (unsigned)((threads + SWEEP_THREADS - 1) / SWEEP_THREADS);
-    if (c->glass) launch(c, "k_sweep_small", k_sweep_small<L, true>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
-    else launch(c, "k_sweep_small", k_sweep_small<L, false>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+    const unsigned grid = (unsigned)((threads + SWEEP_SMALL_THREADS - 1) / SWEEP_SMALL_THREADS);
+    if (c->glass) launch(c, "k_sweep_small", k_sweep_small<L, true>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+    else launch(c, "k_sweep_small", k_sweep_small<L, false>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
   }
 }
 // mode 2: theta sweeps of the resampled population (lattices gathered from the parents' slots); mode 1: energies only

@@ -31,6 +31,9 @@
 #ifndef PA_SWEEP_THREADS
 #define PA_SWEEP_THREADS 128
 #endif
+#ifndef PA_SWEEP_SMALL_THREADS
+#define PA_SWEEP_SMALL_THREADS 128
+#endif
 #ifndef PA_SWEEP_MINB64
 #define PA_SWEEP_MINB64 4
 #endif
@@ -43,6 +46,9 @@
 #ifndef PA_SWEEP_RW128
 #define PA_SWEEP_RW128 1
 #endif
+#ifndef PA_SWEEP_CMPG
+#define PA_SWEEP_CMPG 8
+#endif
 #ifndef PA_SWEEP_STAGE1
 #define PA_SWEEP_STAGE1 2
 #endif
@@ -54,6 +60,7 @@ namespace pa {
 struct SweepArgs {
   uint32_t a[32];  // a[i] = ~0 iff bit (31 - i) of T4 is set
   uint32_t b[32];  // same for T8
+  uint32_t kase[8];  // 2 * (bit of T4) + (bit of T8) for the 8 bits of the mandatory blocks (comparator specialisation)
   int theta;
   int mode;  // 0: inside a step -> buffer cur^1, Rnew replicas, theta sweeps keyed with step ordinal st->step + 1
              // 1: init / set_spins -> buffer cur, R replicas, no sweeps (energies only)
@@ -95,6 +102,34 @@ __device__ __forceinline__ void cmp_block(uint32_t& und, uint32_t& v, const uint
   cmp_bit(und, v, w.y, ge1, a[1], b[1]);
   cmp_bit(und, v, w.z, ge1, a[2], b[2]);
   cmp_bit(und, v, w.w, ge1, a[3], b[3]);
+}
+
+// The same bit for G words at once, specialised on the pair of threshold bits (warp-uniform: a kernel argument).  X is
+// 0, ~0, ge1 or ~ge1, so und <- und & ~(u ^ X) is ONE LOP3 in each of the four cases and the comparator costs 2 instead
+// of 3 LOP3 per word and bit; the price is one uniform branch per bit and group.
+template <int G>
+__device__ __forceinline__ void cmp_bit_group(uint32_t kase, uint32_t (&und)[G], uint32_t (&v)[G], const uint32_t (&u)[G],
+                                              const uint32_t (&ge1)[G]) {
+#pragma unroll
+  for (int i = 0; i < G; ++i) v[i] = (und[i] & u[i]) | (~und[i] & v[i]);
+  switch (kase) {
+    case 0u:  // T4 bit 0, T8 bit 0: X = 0
+#pragma unroll
+      for (int i = 0; i < G; ++i) und[i] &= ~u[i];
+      break;
+    case 3u:  // 1, 1: X = ~0
+#pragma unroll
+      for (int i = 0; i < G; ++i) und[i] &= u[i];
+      break;
+    case 2u:  // 1, 0: X = ge1
+#pragma unroll
+      for (int i = 0; i < G; ++i) und[i] &= ~(u[i] ^ ge1[i]);
+      break;
+    default:  // 0, 1: X = ~ge1
+#pragma unroll
+      for (int i = 0; i < G; ++i) und[i] &= (u[i] ^ ge1[i]);
+      break;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -140,12 +175,27 @@ __device__ __forceinline__ uint32_t atoms_add(uint32_t addr, uint32_t a) {
   return r;
 }
 
-// blocks 2..7 of one word: returns the sites of und0 that end with u < T
+// blocks 2..7 of one word: returns the sites of und0 that end with u < T.  The first PA_SWEEP_STAGE2 blocks are computed
+// unconditionally and side by side (two independent Philox chains; the thresholds are compile-time offsets): one item
+// in 14 needs the second of them, but a warp of 30 items almost always has such an item, and a warp-wide loop iteration
+// per extra block costs every lane of the warp a full, latency-bound Philox chain.  A block that is not needed cannot
+// change a decided site.  What is still undecided after 16 bits (one item in 4000) goes through the loop.
+#ifndef PA_SWEEP_STAGE2
+#define PA_SWEEP_STAGE2 1
+#endif
 __device__ __forceinline__ uint32_t finish_word(uint32_t und, uint32_t v, uint32_t ge1, uint32_t slot, uint32_t call0,
                                                 uint32_t c2, uint32_t c3, const PhiloxKey& key, const SweepArgs& sa) {
   const uint32_t und0 = und;
+  {
+    uint4 w[PA_SWEEP_STAGE2 > 0 ? PA_SWEEP_STAGE2 : 1];
+#pragma unroll
+    for (int k = 0; k < PA_SWEEP_STAGE2; ++k) w[k] = philox4x32_10(slot, call0 + (uint32_t)(PA_SWEEP_STAGE1 + k), c2, c3, key);
+#pragma unroll
+    for (int k = 0; k < PA_SWEEP_STAGE2; ++k)
+      cmp_block(und, v, w[k], ge1, sa.a + 4 * (PA_SWEEP_STAGE1 + k), sa.b + 4 * (PA_SWEEP_STAGE1 + k));
+  }
 #pragma unroll 1
-  for (uint32_t c = (uint32_t)PA_SWEEP_STAGE1; und != 0u; ++c) {
+  for (uint32_t c = (uint32_t)(PA_SWEEP_STAGE1 + PA_SWEEP_STAGE2); und != 0u; ++c) {
     const uint4 w = philox4x32_10(slot, call0 + c, c2, c3, key);
     cmp_block(und, v, w, ge1, sa.a + 4u * c, sa.b + 4u * c);
     if (c == 7u) {  // all 32 bits equal: u == T is not less
@@ -179,12 +229,44 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
     und[i] = ~ge2[i];
     v[i] = 0xffffffffu;
   }
+  if constexpr (PA_SWEEP_CMPG > 0 && NW >= PA_SWEEP_CMPG && NW % (PA_SWEEP_CMPG > 0 ? PA_SWEEP_CMPG : 1) == 0) {
+    // comparator specialised on the threshold bits, G words per uniform branch (cmp_bit_group)
+    constexpr int G = PA_SWEEP_CMPG > 0 ? PA_SWEEP_CMPG : 1;
 #pragma unroll
-  for (int c = 0; c < PA_SWEEP_STAGE1; ++c) {
+    for (int g0 = 0; g0 < NW; g0 += G) {
+      uint32_t gu[G], gv[G], gg[G];
 #pragma unroll
-    for (int i = 0; i < NW; ++i) {
-      const uint4 w = philox4x32_10(slot[i], call0[i] + (uint32_t)c, c2, c3, key);
-      cmp_block(und[i], v[i], w, ge1[i], sa.a + 4 * c, sa.b + 4 * c);
+      for (int i = 0; i < G; ++i) { gu[i] = und[g0 + i]; gv[i] = v[g0 + i]; gg[i] = ge1[g0 + i]; }
+#pragma unroll
+      for (int c = 0; c < PA_SWEEP_STAGE1; ++c) {
+        uint4 w[G];
+#pragma unroll
+        for (int i = 0; i < G; ++i) w[i] = philox4x32_10(slot[g0 + i], call0[g0 + i] + (uint32_t)c, c2, c3, key);
+        uint32_t u[G];
+#pragma unroll
+        for (int i = 0; i < G; ++i) u[i] = w[i].x;
+        cmp_bit_group<G>(sa.kase[4 * c], gu, gv, u, gg);
+#pragma unroll
+        for (int i = 0; i < G; ++i) u[i] = w[i].y;
+        cmp_bit_group<G>(sa.kase[4 * c + 1], gu, gv, u, gg);
+#pragma unroll
+        for (int i = 0; i < G; ++i) u[i] = w[i].z;
+        cmp_bit_group<G>(sa.kase[4 * c + 2], gu, gv, u, gg);
+#pragma unroll
+        for (int i = 0; i < G; ++i) u[i] = w[i].w;
+        cmp_bit_group<G>(sa.kase[4 * c + 3], gu, gv, u, gg);
+      }
+#pragma unroll
+      for (int i = 0; i < G; ++i) { und[g0 + i] = gu[i]; v[g0 + i] = gv[i]; }
+    }
+  } else {  // few words per lane (L < 64): the branch per bit would cost more than the LOP3 it saves
+#pragma unroll
+    for (int c = 0; c < PA_SWEEP_STAGE1; ++c) {
+#pragma unroll
+      for (int i = 0; i < NW; ++i) {
+        const uint4 w = philox4x32_10(slot[i], call0[i] + (uint32_t)c, c2, c3, key);
+        cmp_block(und[i], v[i], w, ge1[i], sa.a + 4 * c, sa.b + 4 * c);
+      }
     }
   }
   // ---- push the stragglers: one shared-memory atomic per warp ----
@@ -284,7 +366,8 @@ __device__ __forceinline__ void neighbour_classes_j(uint32_t tt, uint32_t U, uin
   }
 }
 
-constexpr int SWEEP_THREADS = PA_SWEEP_THREADS;
+constexpr int SWEEP_THREADS = PA_SWEEP_THREADS;              // k_sweep (L >= 64)
+constexpr int SWEEP_SMALL_THREADS = PA_SWEEP_SMALL_THREADS;  // k_sweep_small (L < 64): 2 words per lane need the block-wide queue
 
 // =====================================================================================================
 // L >= 64: a warp holds RW consecutive replicas (lane g holds rows g*RPL .. of each), so that a lane owns
@@ -306,9 +389,9 @@ struct Geo {
 };
 
 // capacity of the block's straggler queue: every word of a half-sweep up to 1024 items, 1024 beyond
-template <int NW>
+template <int NW, int THREADS = SWEEP_THREADS>
 struct SweepCap {
-  static constexpr int WORDS = NW * SWEEP_THREADS;  // plane words per block and half-sweep
+  static constexpr int WORDS = NW * THREADS;  // plane words per block and half-sweep
   static constexpr int CAP = WORDS <= 1024 ? WORDS : 1024;
 };
 
@@ -331,23 +414,29 @@ __device__ __forceinline__ void rot_row(const uint32_t (&s)[Geo<L>::WPP], int di
   }
 }
 
-// One half-sweep of colour C on the lane's rows of the warp's RW replicas.  T = plane C (updated), S = plane 1-C.
-template <int L, int C, bool SG>
-__device__ __forceinline__ void half_sweep(Lattice<L> (&lat)[Geo<L>::RW], uint32_t q, int g,
-                                           uint32_t slot0, uint32_t slot_base, const bool (&valid)[Geo<L>::RW],
-                                           uint32_t t, uint32_t c3, const PhiloxKey& key, const SweepArgs& sa,
-                                           const uint4* __restrict__ bond_mask) {
+// One half-sweep of the lane's rows of the warp's RW replicas, with the colour as a RUN-TIME value and ONE body for both
+// colours: the plane that is updated is always p[0] and the other one p[1]; after the update the two planes trade places (p[1] <- p[0] ^ flip, p[0] <- old
+// p[1]), so an even number of half-sweeps leaves them where they were.  Unrolling the two colours instead doubles the
+// loop body to 36 KB, which no longer fits the 32 KB instruction cache level an SM's warps share (the guide's I-cache
+// table: +5 % steady past 32 KB; ncu: 0.25 no-instruction stalls per issue); one body is 18 KB.  Cost: 16 register moves
+// per half-sweep and a run-time rotate amount.  Needs an even number of rows per lane (row parity = r parity).
+template <int L, bool SG>
+__device__ __forceinline__ void half_sweep_rt(Lattice<L> (&lat)[Geo<L>::RW], uint32_t q, int g, uint32_t C,
+                                              uint32_t slot0, uint32_t slot_base, uint32_t c2, uint32_t c3,
+                                              const PhiloxKey& key, const SweepArgs& sa,
+                                              const uint4* __restrict__ bond_mask) {
   using G_ = Geo<L>;
+  static_assert(G_::RPL % 2 == 0, "row parity must not depend on the lane");
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int NWL = G_::NWL;
   const int gu = (g + G_::G - 1) % G_::G, gd = (g + 1) % G_::G;
-  const uint32_t c2 = 2u * t + (uint32_t)C;
+  const uint32_t sh_even = C ? 31u : 1u, sh_odd = C ? 1u : 31u;  // rotate-left amounts: bit k <- bit k-1 (1) or k+1 (31)
+  const uint4* __restrict__ bm = bond_mask + C * (G_::N / 64) + g * G_::RPL * G_::WPP;
   uint32_t ge1[NWL], ge2[NWL], call0[NWL], slots[NWL];
 #pragma unroll
   for (int rep = 0; rep < G_::RW; ++rep) {
-    uint32_t(&T)[G_::RPL][G_::WPP] = lat[rep].p[C];
-    uint32_t(&S)[G_::RPL][G_::WPP] = lat[rep].p[1 - C];
-    // rows above the lane's first row and below its last row
+    uint32_t(&T)[G_::RPL][G_::WPP] = lat[rep].p[0];
+    uint32_t(&S)[G_::RPL][G_::WPP] = lat[rep].p[1];
     uint32_t up[G_::WPP], dn[G_::WPP];
 #pragma unroll
     for (int i = 0; i < G_::WPP; ++i) {
@@ -356,30 +445,43 @@ __device__ __forceinline__ void half_sweep(Lattice<L> (&lat)[Geo<L>::RW], uint32
     }
 #pragma unroll
     for (int r = 0; r < G_::RPL; ++r) {
-      const int y = g * G_::RPL + r;
+      const uint32_t sh = (r & 1) ? sh_odd : sh_even;  // row y = g * RPL + r uses bit k-1 when (y + C) is even
       uint32_t B[G_::WPP];
-      rot_row<L>(S[r], (y + C) & 1, B);
+      if constexpr (G_::WPP == 1) {
+        B[0] = __funnelshift_l(S[r][0], S[r][0], sh);
+      } else {
+#pragma unroll
+        for (int i = 0; i < G_::WPP; ++i) {
+          const uint32_t prev = S[r][(i + G_::WPP - 1) % G_::WPP], next = S[r][(i + 1) % G_::WPP];
+          const uint32_t left = __funnelshift_l(prev, S[r][i], 1), right = __funnelshift_r(S[r][i], next, 1);
+          B[i] = sh == 1u ? left : right;
+        }
+      }
 #pragma unroll
       for (int i = 0; i < G_::WPP; ++i) {
         const int w = rep * G_::NWR + r * G_::WPP + i;
         const uint32_t U = (r > 0) ? S[r > 0 ? r - 1 : 0][i] : up[i];
         const uint32_t D = (r < G_::RPL - 1) ? S[r < G_::RPL - 1 ? r + 1 : 0][i] : dn[i];
         uint4 mk = make_uint4(0u, 0u, 0u, 0u);
-        if constexpr (SG) mk = __ldg(bond_mask + C * (G_::N / 64) + y * G_::WPP + i);  // shared by all replicas: L1 resident
+        if constexpr (SG) mk = __ldg(bm + r * G_::WPP + i);
         neighbour_classes_j<SG>(T[r][i], U, D, S[r][i], B[i], mk, ge1[w], ge2[w]);
-        if (!valid[rep]) ge2[w] = 0xffffffffu;  // a replica past the population has nothing to decide
-        call0[w] = 8u * ((uint32_t)y * G_::WPP + (uint32_t)i);  // group = y * WPP + i
+        call0[w] = 8u * ((uint32_t)(g * G_::RPL + r) * G_::WPP + (uint32_t)i);  // group = y * WPP + i
         slots[w] = slot0 + (uint32_t)rep;
       }
     }
   }
   uint32_t flip[NWL];
-  queued_accept<NWL, SWEEP_THREADS, SweepCap<NWL>::CAP>(q, (unsigned)C, ge1, ge2, slots, slot_base, call0, c2, c3, key, sa,
-                                                        flip);
+  queued_accept<NWL, SWEEP_THREADS, SweepCap<NWL>::CAP>(q, C, ge1, ge2, slots, slot_base, call0, c2, c3, key, sa, flip);
 #pragma unroll
   for (int rep = 0; rep < G_::RW; ++rep)
 #pragma unroll
-    for (int w = 0; w < G_::NWR; ++w) lat[rep].p[C][w / G_::WPP][w % G_::WPP] ^= flip[rep * G_::NWR + w];
+    for (int w = 0; w < G_::NWR; ++w) {
+      uint32_t& a = lat[rep].p[0][w / G_::WPP][w % G_::WPP];
+      uint32_t& b = lat[rep].p[1][w / G_::WPP][w % G_::WPP];
+      const uint32_t updated = a ^ flip[rep * G_::NWR + w];
+      a = b;
+      b = updated;
+    }
 }
 
 // number of anti-aligned bonds u (each bond has exactly one colour-0 end) and number of up spins
@@ -499,13 +601,13 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
     using Q_ = SweepQueue<SweepCap<G_::NWL>::CAP>;
     __shared__ Q_ q_mem;
     static_assert(offsetof(Q_, res) == Q_::OFF_RES && offsetof(Q_, count) == Q_::OFF_COUNT, "queue layout");
-    const uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
+    uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
+    asm volatile("mov.u32 %0, %0;" : "+r"(q));  // keep it in a register: ptxas otherwise rebuilds it (S2R + LEA) at every use
     if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
     __syncthreads();
-    for (int t = 0; t < theta; ++t) {
-      half_sweep<L, 0, SG>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa, bond_mask);
-      half_sweep<L, 1, SG>(lat, q, g, slot0 + gs, slot_base + gs, valid, (uint32_t)t, c3, key, sa, bond_mask);
-    }
+#pragma unroll 1
+    for (uint32_t h = 0; h < 2u * (uint32_t)theta; ++h)  // half-sweep h = 2t + colour
+      half_sweep_rt<L, SG>(lat, q, g, h & 1u, slot0 + gs, slot_base + gs, h, c3, key, sa, bond_mask);
   }
 
 #pragma unroll
@@ -574,7 +676,7 @@ __device__ __forceinline__ void small_neighbours(uint32_t S, int g, uint32_t& U,
 }
 
 template <int L, bool SG>
-__global__ void __launch_bounds__(SWEEP_THREADS)
+__global__ void __launch_bounds__(SWEEP_SMALL_THREADS)
 k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
               int32_t* __restrict__ EM0, int32_t* __restrict__ EM1,
               const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of,
@@ -592,10 +694,10 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
 
   // A group of G lanes holds TWO consecutive replicas (one plane word per colour and replica per lane).
   constexpr int NR = 2;
-  const unsigned long long tid = (unsigned long long)blockIdx.x * SWEEP_THREADS + threadIdx.x;
+  const unsigned long long tid = (unsigned long long)blockIdx.x * SWEEP_SMALL_THREADS + threadIdx.x;
   const unsigned long long pair = tid / G_::G;
   const int g = (int)(tid % G_::G);
-  const unsigned long long slot_base64 = ((unsigned long long)blockIdx.x * SWEEP_THREADS / G_::G) * NR;
+  const unsigned long long slot_base64 = ((unsigned long long)blockIdx.x * SWEEP_SMALL_THREADS / G_::G) * NR;
   if (slot_base64 >= count) return;  // block-uniform: the sweeps below contain block barriers
   uint4 mk[2] = {make_uint4(0u, 0u, 0u, 0u), make_uint4(0u, 0u, 0u, 0u)};  // negative bonds of the lane's word, per colour
   if constexpr (SG) {
@@ -626,10 +728,11 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
 
   // ---- theta sweeps ----------------------------------------------------------------------------
   if (theta > 0) {
-    using Q_ = SweepQueue<SweepCap<NR>::CAP>;
+    using Q_ = SweepQueue<SweepCap<NR, SWEEP_SMALL_THREADS>::CAP>;
     __shared__ Q_ q_mem;
     static_assert(offsetof(Q_, res) == Q_::OFF_RES && offsetof(Q_, count) == Q_::OFF_COUNT, "queue layout");
-    const uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
+    uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
+    asm volatile("mov.u32 %0, %0;" : "+r"(q));  // keep it in a register: ptxas otherwise rebuilds it (S2R + LEA) at every use
     if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
     __syncthreads();
     const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
@@ -646,7 +749,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           neighbour_classes_j<SG>(p[r][0], U, D, p[r][1], B, mk[0], ge1[r], ge2[r]);
           if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }  // padding never holds the warp back
         }
-        queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 0u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t, c3, key,
+        queued_accept<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP>(q, 0u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t, c3, key,
                                                            sa, flip);
 #pragma unroll
         for (int r = 0; r < NR; ++r) p[r][0] ^= flip[r];
@@ -660,7 +763,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           neighbour_classes_j<SG>(p[r][1], U, D, p[r][0], B, mk[1], ge1[r], ge2[r]);
           if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }
         }
-        queued_accept<NR, SWEEP_THREADS, SweepCap<NR>::CAP>(q, 1u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t + 1u, c3,
+        queued_accept<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP>(q, 1u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t + 1u, c3,
                                                            key, sa, flip);
 #pragma unroll
         for (int r = 0; r < NR; ++r) p[r][1] ^= flip[r];
