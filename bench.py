@@ -321,6 +321,51 @@ def theta1_leg(binding, torch, wl, steps=20, warmup=3):
     return out
 
 
+def glass_leg(binding, torch, wl, peaks, steps=20, warmup=3):
+    """SURVEY.md 8(f)-4 / PAPER.md:213: the same workload shape with the second Hamiltonian, one seeded 2D +-J spin-glass
+    sample (inputs.bond_sample, P(J = -1) = 1/2) set through pa_set_bonds: flip attempts/s of the sweep kernel's +-J
+    variant against the same ALU roofline, and the order-parameter histogram pa_overlap_hist (one pass over the
+    population: HBM-bound)."""
+    Jx, Jy = inputs.bond_sample(wl.L, wl.seed)
+    pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0, flags=binding.PA_PROFILE)
+    pa.set_bonds(inputs.pack_pm1(Jx), inputs.pack_pm1(Jy))
+    pa.run(schedule(wl, 1, warmup), wl.theta)
+    pa.profile_read()
+    rs0 = pa.replica_steps()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record(pa.stream)
+    pa.run(schedule(wl, warmup + 1, steps), wl.theta)
+    ev1.record(pa.stream)
+    torch.cuda.synchronize()
+    sec = ev0.elapsed_time(ev1) * 1e-3
+    prof = pa.profile_read()
+    rs = pa.replica_steps() - rs0
+    attempts = wl.theta * wl.N * rs
+    sweep_rate = attempts / (prof["sweep"][0] * 1e-3)
+    peak = SM_COUNT * SMSP * ALU_LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
+    pa.overlap_hist()  # warm-up
+    t = []
+    for _ in range(5):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h = pa.overlap_hist()
+        t.append(time.perf_counter() - t0)
+    ovl_s = statistics.median(t)  # host clock around the synchronous call: memset + kernel + (N+1)*8-byte read-back
+    pairs = int(h.sum())
+    q = (2.0 * torch.arange(wl.N + 1, dtype=torch.float64) - wl.N) / wl.N
+    hq = torch.from_numpy(h.astype("float64"))
+    out = {"workload": wl.name + " with a +-J sample (seed %d, %d of %d bonds negative)" % (wl.seed, int((Jx < 0).sum() + (Jy < 0).sum()), 2 * wl.N),
+           "steps": steps, "attempts_per_s": attempts / sec, "kernel_attempts_per_s": sweep_rate,
+           "roofline_frac": sweep_rate * ALU_OPS_PER_ATTEMPT / 1e12 / peak, "ms_per_step": 1e3 * sec / steps,
+           "overlap_hist": {"pairs": pairs, "seconds_call": ovl_s, "GBps": pa.R * wl.bytes_per_replica / ovl_s / 1e9,
+                            "mean_abs_q": float((hq * q.abs()).sum() / max(pairs, 1)), "mean_q2": float((hq * q * q).sum() / max(pairs, 1))},
+           "lnZ": pa.log_Z()["lnZ"], "beta": pa.beta_steps()[0], "mean_E_per_spin": pa.observables()["mean_E"] / wl.N}
+    del pa
+    torch.cuda.empty_cache()
+    return out
+
+
 def policies_leg(binding, torch, out_csv=None):
     """SURVEY.md 8(f)-2 / PAPER.md:94-118 (Fig. 1-2): the paper's 8-GPU task with the 8 GPUs as 8 logical partitions of
     one device, under the redistribution policies none / naive / main (blocks of 1024, maxexc 1 and 2) / balanced.
@@ -481,10 +526,12 @@ def run_ours(args):
     if use_shards:
         del sharded
     torch.cuda.empty_cache()
-    theta1 = None
+    theta1 = glass = None
     if g.is_main and g.world == 1:
         if wl.theta > 1 and not args.no_resample:
             theta1 = theta1_leg(binding, torch, wl)
+        if wl.theta > 0 and not args.no_resample:
+            glass = glass_leg(binding, torch, wl, peaks)
         if not args.no_resample:
             resample = resample_leg(binding, torch, peaks, repeats=args.resample_repeats)
         if not args.no_cpu_baseline:
@@ -512,7 +559,7 @@ def run_ours(args):
                                            "that cross rank boundaries (NCCL point-to-point)" % (g.world, g.world)),
                            "l2": "population %.0f MiB per buffer > 126 MB L2, no flush needed" % (wl.R0 * wl.bytes_per_replica / 2 ** 20)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_total, "roofline": roof, "cpu_baseline": cpu,
-                "resample": resample, "theta1": theta1, "kernels": per_kernel, "anneal": {"lnZ": lnZ, "beta": beta_now, "R": R_final,
+                "resample": resample, "theta1": theta1, "spin_glass": glass, "kernels": per_kernel, "anneal": {"lnZ": lnZ, "beta": beta_now, "R": R_final,
                                                                          "replica_steps": replica_steps}}
         if g.world > 1:
             line["config"]["R0"] = wl.R0 * g.world

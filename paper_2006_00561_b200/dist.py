@@ -134,7 +134,10 @@ class ShardedAnnealer:
     ONE device, stepped phase by phase in lock-step by the host (no kernel ever waits on another rank's kernel, so this
     is safe on one GPU; it is how the device path is parity-tested where only one GPU is available)."""
 
-    def __init__(self, L, R0, seed=0, beta0=0.0, capacity=0, policy=0, block=0, maxexc=0, group=None, emulate=None, flags=0):
+    def __init__(self, L, R0, seed=0, beta0=0.0, capacity=0, policy=0, block=0, maxexc=0, group=None, emulate=None, flags=0,
+                 bonds=None):
+        """bonds: (Jx, Jy) packed coupling planes of a +-J sample (binding.PopulationAnnealer.set_bonds); every rank
+        sets the same sample"""
         from . import binding
         self._b = binding
         self.policy, self.block, self.maxexc = policy, block, maxexc
@@ -148,6 +151,9 @@ class ShardedAnnealer:
             ranks = [self.g.rank]
         self.shards = [binding.PopulationAnnealer(L, R0, seed=seed, beta0=beta0, capacity=capacity, policy=policy, block=block,
                                                   maxexc=maxexc, rank=r, world=self.world, flags=flags) for r in ranks]
+        if bonds is not None:
+            for s in self.shards:
+                s.set_bonds(bonds[0], bonds[1])
         self.emulated = bool(emulate)
         self.last_T = None
 

@@ -96,7 +96,7 @@ def test_exchange_plan_against_the_oracle_policies_and_its_invariants():
     assert ei.value.code == binding.PA_ECAPACITY
 
 
-def _sharded_oracle_worker(rank, world, port, q, L, R0, seed, betas, theta, policy):
+def _sharded_oracle_worker(rank, world, port, q, L, R0, seed, betas, theta, policy, glass_seed=None):
     """one rank of the partitioned run on the CPU: the oracle does the rank's arithmetic with GLOBAL replica indices as
     keys, the product's host plan (pa_dist_exchange_plan) and exchange (dist.exchange_slices over gloo) move the replicas"""
     os.environ.update({"RANK": str(rank), "WORLD_SIZE": str(world), "LOCAL_RANK": str(rank),
@@ -108,11 +108,13 @@ def _sharded_oracle_worker(rank, world, port, q, L, R0, seed, betas, theta, poli
     g = dist.init_from_env(backend="gloo", device_kind="cpu")
     orc.set_threads(1)
     wpr = orc.words_per_replica(L)
+    from paper_2006_00561_b200 import inputs
+    bonds = None if glass_seed is None else inputs.bond_sample(L, glass_seed)  # second Hamiltonian: every rank, same sample
     start = [r * (R0 // world) + min(r, R0 % world) for r in range(world + 1)]
     spins = orc.init_population(L, R0, seed)[start[rank]:start[rank + 1]].copy()  # keyed by the global replica index
     first, beta, sum_lnQ = start[rank], 0.0, 0.0
     for step, beta_next in enumerate(betas, 1):
-        E, M = orc.energy_mag(L, spins)
+        E, M = orc.energy_mag(L, spins, bonds)
         R_loc, dbeta = spins.shape[0], beta_next - beta
         w_sum = float(np.sum(np.exp(-dbeta * E.astype(np.float64))))  # the rank's sum of weights
         rows = dist.all_gather_doubles(g, [w_sum, float(R_loc)])
@@ -137,7 +139,8 @@ def _sharded_oracle_worker(rank, world, port, q, L, R0, seed, betas, theta, poli
         first = int(ns[rank])
         if theta > 0:
             T4, T8 = orc.thresholds(beta_next)
-            orc.sweeps_slots(L, np.arange(first, first + new_n, dtype=np.uint32), spins, seed, step, theta, T4, T8)
+            orc.sweeps_slots(L, np.arange(first, first + new_n, dtype=np.uint32), spins, seed, step, theta, T4, T8,
+                             bonds=bonds)
         beta = beta_next
         sum_lnQ += float(np.log(Q))
     q.put((rank, first, spins, sum_lnQ))
@@ -145,8 +148,9 @@ def _sharded_oracle_worker(rank, world, port, q, L, R0, seed, betas, theta, poli
     dist.shutdown(g)
 
 
-@pytest.mark.parametrize("world,policy", [(2, 0), (4, 0), (3, 1), (2, 2), (2, 3)])
-def test_sharded_run_equals_the_single_population_run_gloo(world, policy):
+@pytest.mark.parametrize("world,policy,glass_seed", [(2, 0, None), (4, 0, None), (3, 1, None), (2, 2, None), (2, 3, None),
+                                                     (2, 0, 5), (3, 1, 6)])
+def test_sharded_run_equals_the_single_population_run_gloo(world, policy, glass_seed):
     """world-size 2/3/4 over gloo: the concatenation of the ranks' populations equals the one-population oracle run bit
     for bit (random numbers are keyed by global replica index and global step; the policy only moves rank boundaries)"""
     import numpy as np
@@ -156,7 +160,7 @@ def test_sharded_run_equals_the_single_population_run_gloo(world, policy):
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_sharded_oracle_worker, args=(r, world, port, q, L, R0, seed, betas, theta, policy))
+    procs = [ctx.Process(target=_sharded_oracle_worker, args=(r, world, port, q, L, R0, seed, betas, theta, policy, glass_seed))
              for r in range(world)]
     for p in procs:
         p.start()
@@ -164,7 +168,8 @@ def test_sharded_run_equals_the_single_population_run_gloo(world, policy):
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    ref = orc.OraclePA(L, R0, seed=seed)
+    from paper_2006_00561_b200 import inputs
+    ref = orc.OraclePA(L, R0, seed=seed, bonds=None if glass_seed is None else inputs.bond_sample(L, glass_seed))
     for b in betas:
         ref.step(b, theta)
     got = np.concatenate([r[2] for r in res], axis=0)

@@ -123,3 +123,27 @@ def test_overlap_histogram_large_population_ising():
     gpu = b.PopulationAnnealer(32, 1 << 17, seed=2)
     gpu.run([0.2, 0.4], 2)
     assert np.array_equal(gpu.overlap_hist(), orc.overlap_hist(32, gpu.spins()))
+
+
+@pytest.mark.parametrize("world,L,theta", [(2, 32, 2), (3, 64, 1), (4, 16, 0)])
+def test_sharded_ranks_with_bonds_equal_the_single_context(world, L, theta):
+    """multi-GPU protocol (ranks emulated on one device) with the second Hamiltonian: every rank sets the same sample"""
+    b = _binding()
+    from paper_2006_00561_b200 import dist
+    R0, seed = 1500, 60 + L
+    Jx, Jy = sample_with_parity(L, 7 * L, 1)
+    px, py = inputs.pack_pm1(Jx), inputs.pack_pm1(Jy)
+    single = b.PopulationAnnealer(L, R0, P=1, seed=seed)
+    single.set_bonds(px, py)
+    sh = dist.ShardedAnnealer(L, R0, seed=seed, emulate=world, bonds=(px, py))
+    E0 = np.concatenate([s_.energies()[0] for s_ in sh.shards])
+    assert np.array_equal(E0, single.energies()[0]) and np.all(E0 % 4 == 2)
+    dbeta = min(0.06, 600.0 / (2 * L * L))
+    for k in range(1, 6):
+        single.step(dbeta * k, theta)
+        obs = sh.step(dbeta * k, theta)
+        assert np.array_equal(sh.gather_spins(), single.spins()), k
+        assert sum(o["sum_E"] for o in obs) == single.observables()["sum_E"]
+        assert np.array_equal(np.concatenate([s_.energies()[0] for s_ in sh.shards]), single.energies()[0])
+        for s_ in sh.shards:
+            assert rel(s_.log_Z()["lnZ"], single.log_Z()["lnZ"]) <= RTOL
