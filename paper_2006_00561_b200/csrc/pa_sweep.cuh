@@ -87,14 +87,23 @@ __device__ __forceinline__ uint32_t spread_bits(uint32_t x) {  // bits 0..15 -> 
   return x;
 }
 
+// one three-input logic operation, spelled out: NVVM otherwise splits und & ~(u ^ g) into an XOR (or a NOT) and an AND
+// that ptxas does not always fuse again.  LUT = f(0xF0, 0xCC, 0xAA) for f(a, b, c).
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t r;
+  asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(r) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+  return r;
+}
+
 // one bit of the MSB-first comparator for 32 sites: u = random bits, A / B = the bit of T4 / T8 (all-ones / all-zeros),
 // ge1 = sites that compare against T4 (a == 1; the others against T8)
 //   v   <- u where the site is still undecided (so that v ends as the random bit AT the deciding position)
 //   und <- und & ~(u ^ X),  X = the site's own threshold bit
 __device__ __forceinline__ void cmp_bit(uint32_t& und, uint32_t& v, uint32_t u, uint32_t ge1, uint32_t A, uint32_t B) {
-  const uint32_t X = (ge1 & A) | (~ge1 & B);
-  v = (und & u) | (~und & v);
-  und = und & ~(u ^ X);
+  const uint32_t X = lop3<0xCA>(ge1, A, B);  // ge1 ? A : B
+  v = lop3<0xCA>(und, u, v);                 // und ? u : v
+  und = lop3<0x90>(und, u, X);               // und & ~(u ^ X)
 }
 __device__ __forceinline__ void cmp_block(uint32_t& und, uint32_t& v, const uint4& w, uint32_t ge1, const uint32_t* a,
                                           const uint32_t* b) {
@@ -111,23 +120,23 @@ template <int G>
 __device__ __forceinline__ void cmp_bit_group(uint32_t kase, uint32_t (&und)[G], uint32_t (&v)[G], const uint32_t (&u)[G],
                                               const uint32_t (&ge1)[G]) {
 #pragma unroll
-  for (int i = 0; i < G; ++i) v[i] = (und[i] & u[i]) | (~und[i] & v[i]);
+  for (int i = 0; i < G; ++i) v[i] = lop3<0xCA>(und[i], u[i], v[i]);  // und ? u : v
   switch (kase) {
-    case 0u:  // T4 bit 0, T8 bit 0: X = 0
+    case 0u:  // T4 bit 0, T8 bit 0: X = 0      und & ~u
 #pragma unroll
-      for (int i = 0; i < G; ++i) und[i] &= ~u[i];
+      for (int i = 0; i < G; ++i) und[i] = lop3<0x30>(und[i], u[i], 0u);
       break;
-    case 3u:  // 1, 1: X = ~0
+    case 3u:  // 1, 1: X = ~0                   und & u
 #pragma unroll
-      for (int i = 0; i < G; ++i) und[i] &= u[i];
+      for (int i = 0; i < G; ++i) und[i] = lop3<0xC0>(und[i], u[i], 0u);
       break;
-    case 2u:  // 1, 0: X = ge1
+    case 2u:  // 1, 0: X = ge1                  und & ~(u ^ ge1)
 #pragma unroll
-      for (int i = 0; i < G; ++i) und[i] &= ~(u[i] ^ ge1[i]);
+      for (int i = 0; i < G; ++i) und[i] = lop3<0x90>(und[i], u[i], ge1[i]);
       break;
-    default:  // 0, 1: X = ~ge1
+    default:  // 0, 1: X = ~ge1                 und & (u ^ ge1)
 #pragma unroll
-      for (int i = 0; i < G; ++i) und[i] &= (u[i] ^ ge1[i]);
+      for (int i = 0; i < G; ++i) und[i] = lop3<0x60>(und[i], u[i], ge1[i]);
       break;
   }
 }
@@ -287,7 +296,7 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
 #pragma unroll
   for (int i = 0; i < NW; ++i) {
     idx[i] += base;
-    flip[i] = (ge2[i] | ~v[i]) & ~und[i];  // the sites decided so far; the rest comes back through q.res
+    flip[i] = lop3<0x51>(ge2[i], v[i], und[i]);  // (ge2 | ~v) & ~und: the sites decided so far; the rest comes back through q.res
     if (CAN_OVERFLOW && und[i] != 0u && idx[i] >= (unsigned)CAP) {  // queue full: the owner finishes its word in place
       flip[i] |= finish_word(und[i], v[i], ge1[i], slot[i], call0[i], c2, c3, key, sa);
       und[i] = 0u;
@@ -336,14 +345,14 @@ __device__ __forceinline__ void queued_accept(uint32_t q, unsigned parity, const
   accept_readback<NW, CAP>(q, und, idx, flip);
 }
 
-// masks of the sites with a >= 1 and a >= 2 from the four difference words (1 = anti-aligned)
+// masks of the sites with a >= 1 and a >= 2 anti-aligned neighbours, straight from the five words (7 LOP3): the four
+// neighbours in two pairs, "one of the pair differs from tt" and "both differ"
 __device__ __forceinline__ void neighbour_classes(uint32_t tt, uint32_t U, uint32_t D, uint32_t Sm, uint32_t B,
                                                   uint32_t& ge1, uint32_t& ge2) {
-  const uint32_t d0 = tt ^ U, d1 = tt ^ D, d2 = tt ^ Sm, d3 = tt ^ B;
-  const uint32_t maj = (d0 & d1) | (d0 & d2) | (d1 & d2);
-  const uint32_t any3 = d0 | d1 | d2;
-  ge2 = maj | (any3 & d3);
-  ge1 = any3 | d3;
+  const uint32_t any_ud = lop3<0x7E>(tt, U, D), both_ud = lop3<0x18>(tt, U, D);    // (tt^U)|(tt^D), (tt^U)&(tt^D)
+  const uint32_t any_sb = lop3<0x7E>(tt, Sm, B), both_sb = lop3<0x18>(tt, Sm, B);
+  ge1 = any_ud | any_sb;
+  ge2 = lop3<0xFE>(both_ud, both_sb, any_ud & any_sb);
 }
 
 // Second Hamiltonian (D1: 2D +-J spin glass, H = -sum J_ij sigma_i sigma_j): a bond is unsatisfied iff the spins
@@ -356,10 +365,10 @@ template <bool SG>
 __device__ __forceinline__ void neighbour_classes_j(uint32_t tt, uint32_t U, uint32_t D, uint32_t Sm, uint32_t B,
                                                     const uint4& mk, uint32_t& ge1, uint32_t& ge2) {
   if constexpr (SG) {
-    const uint32_t d0 = tt ^ U ^ mk.x, d1 = tt ^ D ^ mk.y, d2 = tt ^ Sm ^ mk.z, d3 = tt ^ B ^ mk.w;
-    const uint32_t maj = (d0 & d1) | (d0 & d2) | (d1 & d2);
-    const uint32_t any3 = d0 | d1 | d2;
-    ge2 = maj | (any3 & d3);
+    const uint32_t d0 = lop3<0x96>(tt, U, mk.x), d1 = lop3<0x96>(tt, D, mk.y), d2 = lop3<0x96>(tt, Sm, mk.z),
+                   d3 = lop3<0x96>(tt, B, mk.w);                      // unsatisfied bonds: spins differ XOR negative coupling
+    const uint32_t maj = lop3<0xE8>(d0, d1, d2), any3 = lop3<0xFE>(d0, d1, d2);
+    ge2 = lop3<0xF8>(maj, any3, d3);                                  // maj | (any3 & d3)
     ge1 = any3 | d3;
   } else {
     neighbour_classes(tt, U, D, Sm, B, ge1, ge2);
