@@ -116,27 +116,31 @@ __device__ __forceinline__ void cmp_block(uint32_t& und, uint32_t& v, const uint
 // The same bit for G words at once, specialised on the pair of threshold bits (warp-uniform: a kernel argument).  X is
 // 0, ~0, ge1 or ~ge1, so und <- und & ~(u ^ X) is ONE LOP3 in each of the four cases and the comparator costs 2 instead
 // of 3 LOP3 per word and bit; the price is one uniform branch per bit and group.
-template <int G>
+constexpr int lut_swap_a(int l, int sw) { return sw ? (((l & 0x0F) << 4) | (l >> 4)) : l; }  // LUT of f(~a, b, c)
+// FIRST: the very first bit of a half-sweep.  und comes in as ge2 (the sites that are NOT compared: und = ~ge2 is folded
+// into the LUTs by swapping their nibbles) and v as "all ones", which makes v' = und ? u : 1 = u | ge2.
+template <int G, bool FIRST>
 __device__ __forceinline__ void cmp_bit_group(uint32_t kase, uint32_t (&und)[G], uint32_t (&v)[G], const uint32_t (&u)[G],
                                               const uint32_t (&ge1)[G]) {
+  constexpr int SW = FIRST ? 1 : 0;
 #pragma unroll
-  for (int i = 0; i < G; ++i) v[i] = lop3<0xCA>(und[i], u[i], v[i]);  // und ? u : v
+  for (int i = 0; i < G; ++i) v[i] = FIRST ? (u[i] | und[i]) : lop3<0xCA>(und[i], u[i], v[i]);  // und ? u : v
   switch (kase) {
     case 0u:  // T4 bit 0, T8 bit 0: X = 0      und & ~u
 #pragma unroll
-      for (int i = 0; i < G; ++i) und[i] = lop3<0x30>(und[i], u[i], 0u);
+      for (int i = 0; i < G; ++i) und[i] = lop3<lut_swap_a(0x30, SW)>(und[i], u[i], 0u);
       break;
     case 3u:  // 1, 1: X = ~0                   und & u
 #pragma unroll
-      for (int i = 0; i < G; ++i) und[i] = lop3<0xC0>(und[i], u[i], 0u);
+      for (int i = 0; i < G; ++i) und[i] = lop3<lut_swap_a(0xC0, SW)>(und[i], u[i], 0u);
       break;
     case 2u:  // 1, 0: X = ge1                  und & ~(u ^ ge1)
 #pragma unroll
-      for (int i = 0; i < G; ++i) und[i] = lop3<0x90>(und[i], u[i], ge1[i]);
+      for (int i = 0; i < G; ++i) und[i] = lop3<lut_swap_a(0x90, SW)>(und[i], u[i], ge1[i]);
       break;
     default:  // 0, 1: X = ~ge1                 und & (u ^ ge1)
 #pragma unroll
-      for (int i = 0; i < G; ++i) und[i] = lop3<0x60>(und[i], u[i], ge1[i]);
+      for (int i = 0; i < G; ++i) und[i] = lop3<lut_swap_a(0x60, SW)>(und[i], u[i], ge1[i]);
       break;
   }
 }
@@ -158,7 +162,9 @@ struct SweepQueue {
   uint32_t res[CAP];  // late flips of the item
   uint32_t count[2];
   uint32_t pad_[2];   // sizeof is a multiple of 16: queues can be laid side by side
+  uint32_t wcount[2][4];  // region form (4 warps, CAP = every word of the block): items of warp w per half-sweep parity
   static constexpr uint32_t OFF_RES = 16u * CAP, OFF_COUNT = 20u * CAP;  // byte offsets (checked in k_sweep*)
+  static constexpr uint32_t OFF_WCOUNT = OFF_COUNT + 16u;
 };
 // The queue is addressed through its 32-bit shared-window address (taken once per kernel) so that every access is a
 // plain LDS / STS / ATOMS with an immediate offset.
@@ -245,7 +251,7 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
     for (int g0 = 0; g0 < NW; g0 += G) {
       uint32_t gu[G], gv[G], gg[G];
 #pragma unroll
-      for (int i = 0; i < G; ++i) { gu[i] = und[g0 + i]; gv[i] = v[g0 + i]; gg[i] = ge1[g0 + i]; }
+      for (int i = 0; i < G; ++i) { gu[i] = ge2[g0 + i]; gv[i] = 0u; gg[i] = ge1[g0 + i]; }  // first bit: FIRST form
 #pragma unroll
       for (int c = 0; c < PA_SWEEP_STAGE1; ++c) {
         uint4 w[G];
@@ -254,16 +260,17 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
         uint32_t u[G];
 #pragma unroll
         for (int i = 0; i < G; ++i) u[i] = w[i].x;
-        cmp_bit_group<G>(sa.kase[4 * c], gu, gv, u, gg);
+        if (c == 0) cmp_bit_group<G, true>(sa.kase[0], gu, gv, u, gg);
+        else cmp_bit_group<G, false>(sa.kase[4 * c], gu, gv, u, gg);
 #pragma unroll
         for (int i = 0; i < G; ++i) u[i] = w[i].y;
-        cmp_bit_group<G>(sa.kase[4 * c + 1], gu, gv, u, gg);
+        cmp_bit_group<G, false>(sa.kase[4 * c + 1], gu, gv, u, gg);
 #pragma unroll
         for (int i = 0; i < G; ++i) u[i] = w[i].z;
-        cmp_bit_group<G>(sa.kase[4 * c + 2], gu, gv, u, gg);
+        cmp_bit_group<G, false>(sa.kase[4 * c + 2], gu, gv, u, gg);
 #pragma unroll
         for (int i = 0; i < G; ++i) u[i] = w[i].w;
-        cmp_bit_group<G>(sa.kase[4 * c + 3], gu, gv, u, gg);
+        cmp_bit_group<G, false>(sa.kase[4 * c + 3], gu, gv, u, gg);
       }
 #pragma unroll
       for (int i = 0; i < G; ++i) { und[g0 + i] = gu[i]; v[g0 + i] = gv[i]; }
@@ -278,30 +285,56 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
       }
     }
   }
-  // ---- push the stragglers: one shared-memory atomic per warp ----
   const unsigned lane = threadIdx.x & 31u;
-  const unsigned lt = (1u << lane) - 1u;
-  unsigned tot = 0u;
+  if constexpr (THREADS == 128 && CAP == NW * THREADS) {
+    // ---- push, region form: warp w owns slots [w * 32 NW, (w + 1) * 32 NW); a lane numbers its own stragglers, one
+    // warp-wide exclusive scan of the lanes' counts places them; no ballots, no atomic, no counter to reset ----
+    unsigned k = 0u;
 #pragma unroll
-  for (int i = 0; i < NW; ++i) {
-    const unsigned bal = __ballot_sync(FULL, und[i] != 0u);
-    idx[i] = tot + (unsigned)__popc(bal & lt);
-    tot += (unsigned)__popc(bal);
-  }
-  unsigned base = 0u;
-  if (tot != 0u) {  // warp-uniform
-    if (lane == 0u) base = atoms_add(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity, tot);
-    base = __shfl_sync(FULL, base, 0);
-  }
-#pragma unroll
-  for (int i = 0; i < NW; ++i) {
-    idx[i] += base;
-    flip[i] = lop3<0x51>(ge2[i], v[i], und[i]);  // (ge2 | ~v) & ~und: the sites decided so far; the rest comes back through q.res
-    if (CAN_OVERFLOW && und[i] != 0u && idx[i] >= (unsigned)CAP) {  // queue full: the owner finishes its word in place
-      flip[i] |= finish_word(und[i], v[i], ge1[i], slot[i], call0[i], c2, c3, key, sa);
-      und[i] = 0u;
+    for (int i = 0; i < NW; ++i) {
+      idx[i] = k;
+      k += und[i] != 0u ? 1u : 0u;
     }
-    if (und[i] != 0u) sts128(q + 16u * idx[i], und[i], v[i], ge1[i], ((slot[i] - slot_base) << 16) | call0[i]);
+    unsigned incl = k;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned t = __shfl_up_sync(FULL, incl, o);
+      if (lane >= (unsigned)o) incl += t;
+    }
+    const unsigned warp = threadIdx.x >> 5;
+    if (lane == 31u) sts32(q + SweepQueue<CAP>::OFF_WCOUNT + 16u * parity + 4u * warp, incl);
+    const unsigned first = warp * (unsigned)(32 * NW) + incl - k;
+#pragma unroll
+    for (int i = 0; i < NW; ++i) {
+      idx[i] += first;
+      flip[i] = lop3<0x51>(ge2[i], v[i], und[i]);  // (ge2 | ~v) & ~und: the sites decided so far; the rest comes back through q.res
+      if (und[i] != 0u) sts128(q + 16u * idx[i], und[i], v[i], ge1[i], ((slot[i] - slot_base) << 16) | call0[i]);
+    }
+  } else {
+    // ---- push the stragglers: one shared-memory atomic per warp ----
+    const unsigned lt = (1u << lane) - 1u;
+    unsigned tot = 0u;
+#pragma unroll
+    for (int i = 0; i < NW; ++i) {
+      const unsigned bal = __ballot_sync(FULL, und[i] != 0u);
+      idx[i] = tot + (unsigned)__popc(bal & lt);
+      tot += (unsigned)__popc(bal);
+    }
+    unsigned base = 0u;
+    if (tot != 0u) {  // warp-uniform
+      if (lane == 0u) base = atoms_add(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity, tot);
+      base = __shfl_sync(FULL, base, 0);
+    }
+#pragma unroll
+    for (int i = 0; i < NW; ++i) {
+      idx[i] += base;
+      flip[i] = lop3<0x51>(ge2[i], v[i], und[i]);  // (ge2 | ~v) & ~und: the sites decided so far; the rest comes back through q.res
+      if (CAN_OVERFLOW && und[i] != 0u && idx[i] >= (unsigned)CAP) {  // queue full: the owner finishes its word in place
+        flip[i] |= finish_word(und[i], v[i], ge1[i], slot[i], call0[i], c2, c3, key, sa);
+        und[i] = 0u;
+      }
+      if (und[i] != 0u) sts128(q + 16u * idx[i], und[i], v[i], ge1[i], ((slot[i] - slot_base) << 16) | call0[i]);
+    }
   }
 }
 
@@ -309,15 +342,34 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
 template <int NW, int THREADS, int CAP, bool REVERSE>
 __device__ __forceinline__ void accept_process(uint32_t q, unsigned parity, uint32_t slot_base, uint32_t c2, uint32_t c3,
                                                const PhiloxKey& key, const SweepArgs& sa) {
-  constexpr bool CAN_OVERFLOW = CAP < NW * THREADS;
-  unsigned n = lds32(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity);
-  if (CAN_OVERFLOW && n > (unsigned)CAP) n = (unsigned)CAP;
-  if (threadIdx.x == 0) sts32(q + SweepQueue<CAP>::OFF_COUNT + 4u * (parity ^ 1u), 0u);  // last read before B of the previous half-sweep
-  const unsigned me = REVERSE ? (unsigned)THREADS - 1u - threadIdx.x : threadIdx.x;
-  for (unsigned it = me; it < n; it += THREADS) {
-    const uint4 m = lds128(q + 16u * it);
-    sts32(q + SweepQueue<CAP>::OFF_RES + 4u * it,
-          finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
+  if constexpr (THREADS == 128 && CAP == NW * THREADS) {  // region form: the 4 warps' items, densely numbered
+    const uint4 cn = lds128(q + SweepQueue<CAP>::OFF_WCOUNT + 16u * parity);
+    const unsigned n = cn.x + cn.y + cn.z + cn.w;
+    for (unsigned it = threadIdx.x; it < n; it += THREADS) {
+      unsigned loc = it, reg = 0u;
+      if (loc >= cn.x) {
+        loc -= cn.x; reg = 1u;
+        if (loc >= cn.y) {
+          loc -= cn.y; reg = 2u;
+          if (loc >= cn.z) { loc -= cn.z; reg = 3u; }
+        }
+      }
+      const unsigned pos = reg * (unsigned)(32 * NW) + loc;
+      const uint4 m = lds128(q + 16u * pos);
+      sts32(q + SweepQueue<CAP>::OFF_RES + 4u * pos,
+            finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
+    }
+  } else {
+    constexpr bool CAN_OVERFLOW = CAP < NW * THREADS;
+    unsigned n = lds32(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity);
+    if (CAN_OVERFLOW && n > (unsigned)CAP) n = (unsigned)CAP;
+    if (threadIdx.x == 0) sts32(q + SweepQueue<CAP>::OFF_COUNT + 4u * (parity ^ 1u), 0u);  // last read before B of the previous half-sweep
+    const unsigned me = REVERSE ? (unsigned)THREADS - 1u - threadIdx.x : threadIdx.x;
+    for (unsigned it = me; it < n; it += THREADS) {
+      const uint4 m = lds128(q + 16u * it);
+      sts32(q + SweepQueue<CAP>::OFF_RES + 4u * it,
+            finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
+    }
   }
 }
 
