@@ -22,6 +22,13 @@
 // that a straggler costs one lane-block instead of a warp-wide iteration.  Blocks that are never computed cannot
 // change a decided site, and a word's result does not depend on which thread finishes it, so the result equals the
 // plain definition bit for bit.
+//
+// What the instruction stream looks like matters more than anything else here: on sm_100a LOP3 (ALU pipe) and
+// IMAD.WIDE (FMA-heavy pipe) of one SMSP retire together at one warp instruction per 2 cycles (pipe_probe.cu), so the
+// kernel's time is its instruction count.  Hence: three-input logic spelled out as lop3.b32 (NVVM splits it otherwise),
+// the comparator specialised on the threshold bits by a uniform branch (2 instead of 3 LOP3 per word and bit), one
+// half-sweep body for both colours (the loop must fit the 32 KB instruction-cache level), and a straggler push that
+// needs no ballots and no atomics (DESIGN.md 8.2 lists the measured steps and the rejected variants).
 #pragma once
 #include <cstddef>
 
