@@ -385,6 +385,35 @@ def test_extreme_thresholds_through_the_hook():
         assert g.thresholds() == orc.thresholds(0.1)
 
 
+@pytest.mark.parametrize("L", [8, 16, 32, 64, 128])
+def test_every_threshold_bit_pair_in_every_position(L):
+    """The sweep kernels of L >= 64 specialise the comparator on the pair (bit of T4, bit of T8) of each of the first 8
+    bit positions -- four code paths per position, the first position with its own LUTs -- and the generic comparator
+    takes over from bit 8 on.  Temperature-derived thresholds never produce T8 > T4 and reach few of the 4^8 patterns;
+    the test hook sets crafted pairs that put every one of the four cases into every position (also T8 > T4: each class
+    is compared with its own threshold, whatever their order), on a population with all neighbour classes."""
+    b = _binding()
+    R, seed, theta = (300 if L <= 32 else 64), 4242 + L, 2
+    pop = inputs.random_packed_population(L, R, seed=L, p_up=0.75)  # plenty of sites with a = 0 and a = 1
+    pairs = [(0x33333333, 0x55555555), (0x66666666, 0xAAAAAAAA), (0xCCCCCCCC, 0x55555555), (0x99999999, 0xAAAAAAAA),
+             (0x0F0F3C3C, 0x3355CCAA), (0xF0F0C3C3, 0xCCAA3355)]  # the first four: case (p + i) mod 4 at position i
+    seen = [set() for _ in range(8)]
+    for T4, T8 in pairs:
+        for i in range(8):
+            seen[i].add((((T4 >> (31 - i)) & 1), ((T8 >> (31 - i)) & 1)))
+        g = b.PopulationAnnealer(L, R, seed=seed, capacity=2048, flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS)
+        g.set_spins(pop)
+        g.debug_set_thresholds(True, T4, T8)
+        dbeta = min(0.02, 300.0 / (2 * L * L))
+        g.step(dbeta, theta)
+        assert g.thresholds() == (T4, T8)
+        o = orc.OraclePA(L, R, seed=seed, capacity=2048, spins=pop)
+        o.resample(dbeta, tau_override=g.tau())
+        orc.sweeps(L, o.spins, seed, 1, theta, T4, T8)
+        assert g.R == o.R and np.array_equal(g.spins(), o.spins), (hex(T4), hex(T8))
+    assert all(len(sx) == 4 for sx in seen)
+
+
 def test_failed_step_does_not_leak_into_the_getters():
     """after PA_ECAPACITY the getters of the last step refuse (their arrays hold the failed attempt) and last_Q is still
     the Q of the last committed step"""
