@@ -234,10 +234,18 @@ void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
     if (c->glass) launch(c, "k_sweep", k_sweep<L, true>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
     else launch(c, "k_sweep", k_sweep<L, false>, grid, SWEEP_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
   } else {
-    const uint64_t threads = ((uint64_t)c->cap + 1) / 2 * SGeo<L>::G;  // a group of G lanes holds two replicas
-    const unsigned grid = (unsigned)((threads + SWEEP_SMALL_THREADS - 1) / SWEEP_SMALL_THREADS);
-    if (c->glass) launch(c, "k_sweep_small", k_sweep_small<L, true>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
-    else launch(c, "k_sweep_small", k_sweep_small<L, false>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+    // a group of G lanes holds NR replicas: 8 when that still gives every SM its four blocks (one full wave), else 2
+    constexpr int RPB8 = SWEEP_SMALL_THREADS / SGeo<L>::G * 8;  // replicas per block with NR = 8
+    if (PA_SWEEP_SMALL_WIDE && (uint64_t)c->cfg.R0 >= (uint64_t)RPB8 * 148 * 4) {
+      const unsigned grid = (unsigned)(((uint64_t)c->cap + RPB8 - 1) / RPB8);
+      if (c->glass) launch(c, "k_sweep_small", k_sweep_small<L, true, 8>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+      else launch(c, "k_sweep_small", k_sweep_small<L, false, 8>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+    } else {
+      const uint64_t threads = ((uint64_t)c->cap + 1) / 2 * SGeo<L>::G;
+      const unsigned grid = (unsigned)((threads + SWEEP_SMALL_THREADS - 1) / SWEEP_SMALL_THREADS);
+      if (c->glass) launch(c, "k_sweep_small", k_sweep_small<L, true, 2>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+      else launch(c, "k_sweep_small", k_sweep_small<L, false, 2>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
+    }
   }
 }
 // mode 2: theta sweeps of the resampled population (lattices gathered from the parents' slots); mode 1: energies only

@@ -38,6 +38,9 @@
 #ifndef PA_SWEEP_THREADS
 #define PA_SWEEP_THREADS 128
 #endif
+#ifndef PA_SWEEP_SMALL_WIDE
+#define PA_SWEEP_SMALL_WIDE 1
+#endif
 #ifndef PA_SWEEP_SMALL_THREADS
 #define PA_SWEEP_SMALL_THREADS 128
 #endif
@@ -743,8 +746,11 @@ __device__ __forceinline__ void small_neighbours(uint32_t S, int g, uint32_t& U,
   B = C == 0 ? ((rotl & G_::ER) | (rotr & ~G_::ER)) : ((rotr & G_::ER) | (rotl & ~G_::ER));
 }
 
-template <int L, bool SG>
-__global__ void __launch_bounds__(SWEEP_SMALL_THREADS)
+// NR = replicas per lane group: 2 for small populations (more blocks: config 1 is latency-bound), 8 for large ones (8
+// plane words per lane and half-sweep, as in k_sweep: specialised comparator, region-form queue, per-word overheads
+// amortised)
+template <int L, bool SG, int NR>
+__global__ void __launch_bounds__(SWEEP_SMALL_THREADS, NR >= 8 ? 4 : 5)
 k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
               int32_t* __restrict__ EM0, int32_t* __restrict__ EM1,
               const PhiloxKey key, const SweepArgs sa, const uint32_t* __restrict__ parent_of,
@@ -760,8 +766,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
   int32_t* __restrict__ EMo = buf ? EM1 : EM0;  // packed E/4 : M/2 words (pa_common.cuh)
   const uint32_t gs = sa.mode != 1 ? st->slot0_new : 0u;  // global index of local slot 0 (multi-GPU shard)
 
-  // A group of G lanes holds TWO consecutive replicas (one plane word per colour and replica per lane).
-  constexpr int NR = 2;
+  // A group of G lanes holds NR consecutive replicas (one plane word per colour and replica per lane).
   const unsigned long long tid = (unsigned long long)blockIdx.x * SWEEP_SMALL_THREADS + threadIdx.x;
   const unsigned long long pair = tid / G_::G;
   const int g = (int)(tid % G_::G);
@@ -773,21 +778,18 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
     mk[1] = __ldg(bond_mask + G_::G + g);
   }
   const uint32_t slot_base = (uint32_t)slot_base64;
-  unsigned long long slot64[NR];
-  bool valid[NR];
+  const unsigned long long slot0_64 = pair * NR;  // the group's first replica; slot r of the group is slot0_64 + r
   uint32_t slots[NR];
-  uint32_t* rep[NR];
   uint32_t p[NR][2];
 #pragma unroll
   for (int r = 0; r < NR; ++r) {
-    slot64[r] = pair * NR + r;
-    valid[r] = slot64[r] < count;
-    slots[r] = (uint32_t)slot64[r] + gs;
-    rep[r] = spins + (valid[r] ? slot64[r] : 0ull) * G_::WREP;
-    const uint32_t* rep_src = rep[r];
-    if (sa.mode == 2 && valid[r]) rep_src = (buf ? spins0 : spins1) + (unsigned long long)parent_of[slot64[r]] * G_::WREP;
+    const unsigned long long slot64 = slot0_64 + r;
+    const bool valid = slot64 < count;
+    slots[r] = (uint32_t)slot64 + gs;
+    const uint32_t* rep_src = spins + (valid ? slot64 : 0ull) * G_::WREP;
+    if (sa.mode == 2 && valid) rep_src = (buf ? spins0 : spins1) + (unsigned long long)parent_of[slot64] * G_::WREP;
     // ---- load: 64 raw bits = RG rows -------------------------------------------------------------
-    const uint2 q = valid[r] ? reinterpret_cast<const uint2*>(rep_src)[g] : make_uint2(0u, 0u);
+    const uint2 q = valid ? reinterpret_cast<const uint2*>(rep_src)[g] : make_uint2(0u, 0u);
     const uint32_t ev = even_bits(q.x) | (even_bits(q.y) << 16);
     const uint32_t od = even_bits(q.x >> 1) | (even_bits(q.y >> 1) << 16);
     p[r][0] = (ev & G_::ER) | (od & ~G_::ER);  // even row: colour 0 sits at even x; odd row: at odd x
@@ -815,7 +817,6 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           uint32_t U, D, B;
           small_neighbours<L, 0>(p[r][1], g, U, D, B);
           neighbour_classes_j<SG>(p[r][0], U, D, p[r][1], B, mk[0], ge1[r], ge2[r]);
-          if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }  // padding never holds the warp back
         }
         queued_accept<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP>(q, 0u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t, c3, key,
                                                            sa, flip);
@@ -829,7 +830,6 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           uint32_t U, D, B;
           small_neighbours<L, 1>(p[r][0], g, U, D, B);
           neighbour_classes_j<SG>(p[r][1], U, D, p[r][0], B, mk[1], ge1[r], ge2[r]);
-          if (!valid[r]) { ge1[r] = 0xffffffffu; ge2[r] = 0xffffffffu; }
         }
         queued_accept<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP>(q, 1u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t + 1u, c3,
                                                            key, sa, flip);
@@ -852,15 +852,17 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
       unsat += __shfl_xor_sync(0xffffffffu, unsat, o);
       ups += __shfl_xor_sync(0xffffffffu, ups, o);
     }
-    if (valid[r] && g == 0) EMo[slot64[r]] = pack_em(2 * unsat - 2 * G_::N, 2 * ups - G_::N);
+    const unsigned long long slot64 = slot0_64 + r;
+    const bool valid = slot64 < count;
+    if (valid && g == 0) EMo[slot64] = pack_em(2 * unsat - 2 * G_::N, 2 * ups - G_::N);
     // ---- store -----------------------------------------------------------------------------------
-    if (theta > 0 && valid[r]) {
+    if (theta > 0 && valid) {
       const uint32_t ev = (p[r][0] & G_::ER) | (p[r][1] & ~G_::ER);
       const uint32_t od = (p[r][1] & G_::ER) | (p[r][0] & ~G_::ER);
       uint2 q;
       q.x = spread_bits(ev) | (spread_bits(od) << 1);
       q.y = spread_bits(ev >> 16) | (spread_bits(od >> 16) << 1);
-      reinterpret_cast<uint2*>(rep[r])[g] = q;
+      reinterpret_cast<uint2*>(spins + slot64 * G_::WREP)[g] = q;
     }
   }
 }

@@ -414,6 +414,15 @@ def test_every_threshold_bit_pair_in_every_position(L):
     assert all(len(sx) == 4 for sx in seen)
 
 
+@pytest.mark.parametrize("L,R0", [(8, 620000), (16, 160000), (32, 40000)])
+def test_wide_small_lattice_kernel_on_large_populations(L, R0):
+    """k_sweep_small switches to 8 replicas per lane group once a population fills the GPU (L = 32: R0 >= 37 888, L = 16:
+    151 552, L = 8: 606 208): full-population lock-step at those sizes, ferromagnet and a +-J sample"""
+    for bonds in (None, inputs.bond_sample(L, 3 * L)):
+        gpu, ora = make_pair(L, R0, 5, seed=77 + L, bonds=bonds)
+        lockstep(gpu, ora, [0.1, 0.3, 0.45], theta=2)
+
+
 def test_failed_step_does_not_leak_into_the_getters():
     """after PA_ECAPACITY the getters of the last step refuse (their arrays hold the failed attempt) and last_Q is still
     the Q of the last committed step"""
