@@ -236,7 +236,7 @@ void launch_sweep_L(pa_ctx* c, const SweepArgs& sa) {
   } else {
     // a group of G lanes holds NR replicas: 8 when that still gives every SM its four blocks (one full wave), else 2
     constexpr int RPB8 = SWEEP_SMALL_THREADS / SGeo<L>::G * 8;  // replicas per block with NR = 8
-    if (PA_SWEEP_SMALL_WIDE && (uint64_t)c->cfg.R0 >= (uint64_t)RPB8 * 148 * 4) {
+    if ((uint64_t)c->cfg.R0 >= (uint64_t)RPB8 * 148 * 4) {
       const unsigned grid = (unsigned)(((uint64_t)c->cap + RPB8 - 1) / RPB8);
       if (c->glass) launch(c, "k_sweep_small", k_sweep_small<L, true, 8>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);
       else launch(c, "k_sweep_small", k_sweep_small<L, false, 8>, grid, SWEEP_SMALL_THREADS, st, s0, s1, em0, em1, c->key, sa, parent_of, bm);

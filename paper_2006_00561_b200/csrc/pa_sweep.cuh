@@ -38,9 +38,6 @@
 #ifndef PA_SWEEP_THREADS
 #define PA_SWEEP_THREADS 128
 #endif
-#ifndef PA_SWEEP_SMALL_WIDE
-#define PA_SWEEP_SMALL_WIDE 1
-#endif
 #ifndef PA_SWEEP_SMALL_THREADS
 #define PA_SWEEP_SMALL_THREADS 128
 #endif
@@ -348,8 +345,7 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
   }
 }
 
-// REVERSE: item `it` goes to thread THREADS - 1 - it (the second queue of a block is drained by the other warps)
-template <int NW, int THREADS, int CAP, bool REVERSE>
+template <int NW, int THREADS, int CAP>
 __device__ __forceinline__ void accept_process(uint32_t q, unsigned parity, uint32_t slot_base, uint32_t c2, uint32_t c3,
                                                const PhiloxKey& key, const SweepArgs& sa) {
   if constexpr (THREADS == 128 && CAP == NW * THREADS) {  // region form: the 4 warps' items, densely numbered
@@ -374,8 +370,7 @@ __device__ __forceinline__ void accept_process(uint32_t q, unsigned parity, uint
     unsigned n = lds32(q + SweepQueue<CAP>::OFF_COUNT + 4u * parity);
     if (CAN_OVERFLOW && n > (unsigned)CAP) n = (unsigned)CAP;
     if (threadIdx.x == 0) sts32(q + SweepQueue<CAP>::OFF_COUNT + 4u * (parity ^ 1u), 0u);  // last read before B of the previous half-sweep
-    const unsigned me = REVERSE ? (unsigned)THREADS - 1u - threadIdx.x : threadIdx.x;
-    for (unsigned it = me; it < n; it += THREADS) {
+    for (unsigned it = threadIdx.x; it < n; it += THREADS) {
       const uint4 m = lds128(q + 16u * it);
       sts32(q + SweepQueue<CAP>::OFF_RES + 4u * it,
             finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
@@ -402,7 +397,7 @@ __device__ __forceinline__ void queued_accept(uint32_t q, unsigned parity, const
   unsigned idx[NW];
   accept_phase1<NW, THREADS, CAP>(q, parity, ge1, ge2, slot, slot_base, call0, c2, c3, key, sa, flip, und, idx);
   __syncthreads();  // A: every push of this half-sweep is visible
-  accept_process<NW, THREADS, CAP, false>(q, parity, slot_base, c2, c3, key, sa);
+  accept_process<NW, THREADS, CAP>(q, parity, slot_base, c2, c3, key, sa);
   __syncthreads();  // B: every result is visible
   accept_readback<NW, CAP>(q, und, idx, flip);
 }
@@ -438,7 +433,7 @@ __device__ __forceinline__ void neighbour_classes_j(uint32_t tt, uint32_t U, uin
 }
 
 constexpr int SWEEP_THREADS = PA_SWEEP_THREADS;              // k_sweep (L >= 64)
-constexpr int SWEEP_SMALL_THREADS = PA_SWEEP_SMALL_THREADS;  // k_sweep_small (L < 64): 2 words per lane need the block-wide queue
+constexpr int SWEEP_SMALL_THREADS = PA_SWEEP_SMALL_THREADS;  // k_sweep_small (L < 64)
 
 // =====================================================================================================
 // L >= 64: a warp holds RW consecutive replicas (lane g holds rows g*RPL .. of each), so that a lane owns
