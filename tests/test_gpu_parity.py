@@ -423,6 +423,22 @@ def test_wide_small_lattice_kernel_on_large_populations(L, R0):
         lockstep(gpu, ora, [0.1, 0.3, 0.45], theta=2)
 
 
+@pytest.mark.parametrize("L,R0", [(8, 900), (32, 500), (64, 120)])
+def test_heating_protocol_lockstep(L, R0):
+    """PAPER.md:68 "the heating of the population": a population of ground states declared at a low temperature is
+    annealed towards beta = 0 (negative dbeta, reading G29): lock-step with the oracle, every step"""
+    N = L * L
+    up = orc.pack(L, np.ones(N, np.int8))
+    down = orc.pack(L, -np.ones(N, np.int8))
+    spins = np.stack([up if j % 2 == 0 else down for j in range(R0)])
+    beta0 = 1.0
+    gpu, ora = make_pair(L, R0, 4, seed=31 + L, beta0=beta0, spins=spins)
+    dbeta = min(0.08, 300.0 / (2 * N))
+    betas = [beta0 - dbeta * k for k in range(1, 11)]
+    lockstep(gpu, ora, betas, theta=2)
+    assert gpu.log_Z()["sum_lnQ"] < 0.0 and rel(gpu.log_Z()["sum_lnQ"], ora.sum_lnQ) <= RTOL
+
+
 def test_failed_step_does_not_leak_into_the_getters():
     """after PA_ECAPACITY the getters of the last step refuse (their arrays hold the failed attempt) and last_Q is still
     the Q of the last committed step"""

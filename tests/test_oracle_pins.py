@@ -754,3 +754,31 @@ def test_moment_sums_exact_integers():
     assert s["sum_M4"] == sum(m ** 4 for m in Mi)
     big = orc.moment_sums(np.zeros(300000, np.int32), np.full(300000, 16384, np.int32))
     assert big["sum_M4"] == 300000 * 16384 ** 4 > 2 ** 64  # needs the 128-bit accumulator
+
+
+# ---------------------------------------------------------------------------------------------------
+# heating protocol ("the cooling of the population and the heating of the population ... the initial
+# temperature of heating is chosen close to zero temperature.  The initial value of the corresponding free energy was
+# determined accordingly"): eq. 3 and eq. 5 with NEGATIVE dbeta (reading G29)
+# ---------------------------------------------------------------------------------------------------
+def test_heating_from_the_ground_states_reaches_the_exact_lnZ_L4():
+    L, N, R0, beta0 = 4, 16, 30000, 2.0
+    dos, _ = exact_ising.brute_force_dos(L)
+    lnZ0 = float(exact_ising.lnZ_from_dos(dos, beta0))          # ln Omega of the heating run, "determined accordingly"
+    assert abs(lnZ0 - (math.log(2.0) + 2 * N * beta0)) < 1e-5    # two ground states of energy -2N; excitations ~ 16 e^-16
+    up = orc.pack(L, np.ones(N, np.int8))
+    down = orc.pack(L, -np.ones(N, np.int8))
+    spins = np.stack([up if j % 2 == 0 else down for j in range(R0)])
+    pa = orc.OraclePA(L, R0, seed=21, beta0=beta0, spins=spins)
+    betas = [beta0 - 0.05 * k for k in range(1, 37)]             # 2.0 -> 0.2
+    for b in betas:
+        info = pa.step(b, 5)
+        assert info["dbeta"] < 0 and info["Q"] < 1.0   # E < 0 throughout: weights exp(-dbeta E) < 1
+    lnZ = lnZ0 + pa.sum_lnQ
+    exact = float(exact_ising.lnZ_from_dos(dos, betas[-1]))
+    assert abs(lnZ - exact) < 0.03, (lnZ, exact)
+    # and the population has left the ground states: <E> at beta = 0.2 from the density of states
+    Es = np.array([int(k) for k in dos.keys()], float)
+    g = np.array([float(v) for v in dos.values()])
+    w = g * np.exp(-betas[-1] * Es)
+    assert abs(pa.E.mean() - (w * Es).sum() / w.sum()) < 0.25
