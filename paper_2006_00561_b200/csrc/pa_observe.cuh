@@ -339,7 +339,16 @@ k_overlap_hist(const DevState* __restrict__ st, const uint32_t* __restrict__ spi
     const uint32_t* a = spins + j * wrep;
     const uint32_t* b = spins + (j + half) * wrep;
     int diff = 0;
-    for (int w = lane; w < wrep; w += 32) diff += __popc(__ldg(a + w) ^ __ldg(b + w));
+    if ((wrep & 127) == 0) {  // L >= 64: 128-bit loads, a warp covers 512 bytes of each lattice per step
+      const uint4* a4 = reinterpret_cast<const uint4*>(a);
+      const uint4* b4 = reinterpret_cast<const uint4*>(b);
+      for (int w = lane; w < wrep / 4; w += 32) {
+        const uint4 x = __ldg(a4 + w), y = __ldg(b4 + w);
+        diff += __popc(x.x ^ y.x) + __popc(x.y ^ y.y) + __popc(x.z ^ y.z) + __popc(x.w ^ y.w);
+      }
+    } else {
+      for (int w = lane; w < wrep; w += 32) diff += __popc(__ldg(a + w) ^ __ldg(b + w));
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) diff += __shfl_xor_sync(0xffffffffu, diff, o);
     if (lane == 0) {
