@@ -173,6 +173,14 @@ struct SweepQueue {
   static constexpr uint32_t OFF_RES = 16u * CAP, OFF_COUNT = 20u * CAP;  // byte offsets (checked in k_sweep*)
   static constexpr uint32_t OFF_WCOUNT = OFF_COUNT + 16u;
 };
+// REGION form of the queue (4 warps, CAP = every word of the block): per-warp regions, no atomics.  OWNER form on top of
+// it (a multiple of 4 words per thread): items name their owner and the late flips come back through per-thread slots.
+template <int NW, int THREADS, int CAP>
+struct QueueForm {
+  static constexpr bool REGION = THREADS == 128 && CAP == NW * THREADS;
+  static constexpr bool OWNER = REGION && NW % 4 == 0;
+};
+
 // The queue is addressed through its 32-bit shared-window address (taken once per kernel) so that every access is a
 // plain LDS / STS / ATOMS with an immediate offset.
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
@@ -293,7 +301,7 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
     }
   }
   const unsigned lane = threadIdx.x & 31u;
-  if constexpr (THREADS == 128 && CAP == NW * THREADS) {
+  if constexpr (QueueForm<NW, THREADS, CAP>::REGION) {
     // ---- push, region form: warp w owns slots [w * 32 NW, (w + 1) * 32 NW); a lane numbers its own stragglers, one
     // warp-wide exclusive scan of the lanes' counts places them; no ballots, no atomic, no counter to reset ----
     unsigned k = 0u;
@@ -315,7 +323,10 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
     for (int i = 0; i < NW; ++i) {
       idx[i] += first;
       flip[i] = lop3<0x51>(ge2[i], v[i], und[i]);  // (ge2 | ~v) & ~und: the sites decided so far; the rest comes back through q.res
-      if (und[i] != 0u) sts128(q + 16u * idx[i], und[i], v[i], ge1[i], ((slot[i] - slot_base) << 16) | call0[i]);
+      // the item names its OWNER (thread, word): the dense pass derives the replica from it and writes the late flips
+      // into the owner's own result slot
+      const uint32_t who = NW % 4 == 0 ? threadIdx.x * (unsigned)NW + (unsigned)i : slot[i] - slot_base;
+      if (und[i] != 0u) sts128(q + 16u * idx[i], und[i], v[i], ge1[i], (who << 16) | call0[i]);
     }
   } else {
     // ---- push the stragglers: one shared-memory atomic per warp ----
@@ -345,10 +356,10 @@ __device__ __forceinline__ void accept_phase1(uint32_t q /* shared address of th
   }
 }
 
-template <int NW, int THREADS, int CAP>
+template <int NW, int THREADS, int CAP, class SlotOf>
 __device__ __forceinline__ void accept_process(uint32_t q, unsigned parity, uint32_t slot_base, uint32_t c2, uint32_t c3,
                                                const PhiloxKey& key, const SweepArgs& sa) {
-  if constexpr (THREADS == 128 && CAP == NW * THREADS) {  // region form: the 4 warps' items, densely numbered
+  if constexpr (QueueForm<NW, THREADS, CAP>::REGION) {  // region form: the 4 warps' items, densely numbered
     const uint4 cn = lds128(q + SweepQueue<CAP>::OFF_WCOUNT + 16u * parity);
     const unsigned n = cn.x + cn.y + cn.z + cn.w;
     for (unsigned it = threadIdx.x; it < n; it += THREADS) {
@@ -362,8 +373,16 @@ __device__ __forceinline__ void accept_process(uint32_t q, unsigned parity, uint
       }
       const unsigned pos = reg * (unsigned)(32 * NW) + loc;
       const uint4 m = lds128(q + 16u * pos);
-      sts32(q + SweepQueue<CAP>::OFF_RES + 4u * pos,
-            finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
+      if constexpr (QueueForm<NW, THREADS, CAP>::OWNER) {
+        const unsigned owner = m.w >> 16, ot = owner / (unsigned)NW, oi = owner % (unsigned)NW;  // thread and word of the owner
+        // result slots: word oi of thread ot lives in 16-byte vector (oi / 4) * THREADS + ot, so that an owner reads its
+        // NW results with NW / 4 conflict-free 128-bit loads
+        sts32(q + SweepQueue<CAP>::OFF_RES + 16u * ((oi >> 2) * (unsigned)THREADS + ot) + 4u * (oi & 3u),
+              finish_word(m.x, m.y, m.z, slot_base + SlotOf::rel(ot, oi), m.w & 0xffffu, c2, c3, key, sa));
+      } else {
+        sts32(q + SweepQueue<CAP>::OFF_RES + 4u * pos,
+              finish_word(m.x, m.y, m.z, slot_base + (m.w >> 16), m.w & 0xffffu, c2, c3, key, sa));
+      }
     }
   } else {
     constexpr bool CAN_OVERFLOW = CAP < NW * THREADS;
@@ -378,17 +397,39 @@ __device__ __forceinline__ void accept_process(uint32_t q, unsigned parity, uint
   }
 }
 
-template <int NW, int CAP>
+// owner form: every thread's result slots start out empty
+template <int NW, int THREADS, int CAP>
+__device__ __forceinline__ void queue_clear_results(uint32_t q) {
+  if constexpr (QueueForm<NW, THREADS, CAP>::OWNER) {
+#pragma unroll
+    for (int h = 0; h < NW / 4; ++h) sts128(q + SweepQueue<CAP>::OFF_RES + 16u * ((unsigned)h * (unsigned)THREADS + threadIdx.x), 0u, 0u, 0u, 0u);
+  }
+}
+
+template <int NW, int THREADS, int CAP>
 __device__ __forceinline__ void accept_readback(uint32_t q, const uint32_t (&und)[NW], const unsigned (&idx)[NW],
                                                 uint32_t (&flip)[NW]) {
+  if constexpr (QueueForm<NW, THREADS, CAP>::OWNER) {
+    // owner form: the thread's own NW result words (zero unless a pushed word came back), NW / 4 vector loads, and the
+    // slots are cleared for the next half-sweep (whose dense pass writes them only after the next barrier A)
+    static_assert(NW % 4 == 0, "result slots are 128-bit vectors");
 #pragma unroll
-  for (int i = 0; i < NW; ++i)
-    if (und[i] != 0u) flip[i] |= lds32(q + SweepQueue<CAP>::OFF_RES + 4u * idx[i]);
+    for (int h = 0; h < NW / 4; ++h) {
+      const uint32_t a = q + SweepQueue<CAP>::OFF_RES + 16u * ((unsigned)h * (unsigned)THREADS + threadIdx.x);
+      const uint4 r = lds128(a);
+      flip[4 * h] |= r.x; flip[4 * h + 1] |= r.y; flip[4 * h + 2] |= r.z; flip[4 * h + 3] |= r.w;
+      sts128(a, 0u, 0u, 0u, 0u);
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < NW; ++i)
+      if (und[i] != 0u) flip[i] |= lds32(q + SweepQueue<CAP>::OFF_RES + 4u * idx[i]);
+  }
 }
 
 // the three phases with block barriers at A and B.  Must be called by EVERY thread of the block; lanes without work
 // pass ge2 = ~0.
-template <int NW, int THREADS, int CAP>
+template <int NW, int THREADS, int CAP, class SlotOf>
 __device__ __forceinline__ void queued_accept(uint32_t q, unsigned parity, const uint32_t (&ge1)[NW],
                                               const uint32_t (&ge2)[NW], const uint32_t (&slot)[NW], uint32_t slot_base,
                                               const uint32_t (&call0)[NW], uint32_t c2, uint32_t c3, const PhiloxKey& key,
@@ -397,9 +438,9 @@ __device__ __forceinline__ void queued_accept(uint32_t q, unsigned parity, const
   unsigned idx[NW];
   accept_phase1<NW, THREADS, CAP>(q, parity, ge1, ge2, slot, slot_base, call0, c2, c3, key, sa, flip, und, idx);
   __syncthreads();  // A: every push of this half-sweep is visible
-  accept_process<NW, THREADS, CAP>(q, parity, slot_base, c2, c3, key, sa);
+  accept_process<NW, THREADS, CAP, SlotOf>(q, parity, slot_base, c2, c3, key, sa);
   __syncthreads();  // B: every result is visible
-  accept_readback<NW, CAP>(q, und, idx, flip);
+  accept_readback<NW, THREADS, CAP>(q, und, idx, flip);
 }
 
 // masks of the sites with a >= 1 and a >= 2 anti-aligned neighbours, straight from the five words (7 LOP3): the four
@@ -452,6 +493,12 @@ struct Geo {
   static constexpr int NWR = RPL * WPP;           // plane words of one replica per lane and half-sweep
   static constexpr int NWL = RW * NWR;            // plane words per lane and half-sweep
   static constexpr int RPB = (SWEEP_THREADS / 32) * RW;  // replicas per block
+};
+
+// replica (relative to the block's first) that word w of thread t belongs to: what the dense pass needs to key an item
+template <int L>
+struct BigSlotOf {
+  static __device__ __forceinline__ uint32_t rel(unsigned t, unsigned w) { return (t >> 5) * (unsigned)Geo<L>::RW + w / (unsigned)Geo<L>::NWR; }
 };
 
 // capacity of the block's straggler queue: every word of a half-sweep up to 1024 items, 1024 beyond
@@ -537,7 +584,7 @@ __device__ __forceinline__ void half_sweep_rt(Lattice<L> (&lat)[Geo<L>::RW], uin
     }
   }
   uint32_t flip[NWL];
-  queued_accept<NWL, SWEEP_THREADS, SweepCap<NWL>::CAP>(q, C, ge1, ge2, slots, slot_base, call0, c2, c3, key, sa, flip);
+  queued_accept<NWL, SWEEP_THREADS, SweepCap<NWL>::CAP, BigSlotOf<L>>(q, C, ge1, ge2, slots, slot_base, call0, c2, c3, key, sa, flip);
 #pragma unroll
   for (int rep = 0; rep < G_::RW; ++rep)
 #pragma unroll
@@ -670,6 +717,7 @@ k_sweep(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1,
     uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
     asm volatile("mov.u32 %0, %0;" : "+r"(q));  // keep it in a register: ptxas otherwise rebuilds it (S2R + LEA) at every use
     if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
+    queue_clear_results<G_::NWL, SWEEP_THREADS, SweepCap<G_::NWL>::CAP>(q);
     __syncthreads();
 #pragma unroll 1
     for (uint32_t h = 0; h < 2u * (uint32_t)theta; ++h)  // half-sweep h = 2t + colour
@@ -722,6 +770,11 @@ struct SGeo {
   static constexpr uint32_t ER = L == 32 ? 0x0000ffffu : (L == 16 ? 0x00ff00ffu : 0x0f0f0f0fu);   // fields of even rows
   static constexpr uint32_t LSBS = L == 32 ? 0x00010001u : (L == 16 ? 0x01010101u : 0x11111111u);  // bit 0 of every field
   static constexpr uint32_t MSBS = LSBS << (HB - 1);
+};
+
+template <int L, int NR>
+struct SmallSlotOf {
+  static __device__ __forceinline__ uint32_t rel(unsigned t, unsigned w) { return (t / (unsigned)SGeo<L>::G) * (unsigned)NR + w; }
 };
 
 // neighbour words of the lane's word of plane C: S = the lane's word of plane 1-C
@@ -799,6 +852,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
     uint32_t q = (uint32_t)__cvta_generic_to_shared(&q_mem);
     asm volatile("mov.u32 %0, %0;" : "+r"(q));  // keep it in a register: ptxas otherwise rebuilds it (S2R + LEA) at every use
     if (threadIdx.x < 2) q_mem.count[threadIdx.x] = 0u;
+    queue_clear_results<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP>(q);
     __syncthreads();
     const uint32_t c3 = ctr3(TAG_SWEEP, st->step + 1u);
     uint32_t call0[NR];
@@ -813,7 +867,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           small_neighbours<L, 0>(p[r][1], g, U, D, B);
           neighbour_classes_j<SG>(p[r][0], U, D, p[r][1], B, mk[0], ge1[r], ge2[r]);
         }
-        queued_accept<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP>(q, 0u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t, c3, key,
+        queued_accept<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP, SmallSlotOf<L, NR>>(q, 0u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t, c3, key,
                                                            sa, flip);
 #pragma unroll
         for (int r = 0; r < NR; ++r) p[r][0] ^= flip[r];
@@ -826,7 +880,7 @@ k_sweep_small(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins
           small_neighbours<L, 1>(p[r][0], g, U, D, B);
           neighbour_classes_j<SG>(p[r][1], U, D, p[r][0], B, mk[1], ge1[r], ge2[r]);
         }
-        queued_accept<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP>(q, 1u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t + 1u, c3,
+        queued_accept<NR, SWEEP_SMALL_THREADS, SweepCap<NR, SWEEP_SMALL_THREADS>::CAP, SmallSlotOf<L, NR>>(q, 1u, ge1, ge2, slots, slot_base + gs, call0, 2u * (uint32_t)t + 1u, c3,
                                                            key, sa, flip);
 #pragma unroll
         for (int r = 0; r < NR; ++r) p[r][1] ^= flip[r];
