@@ -50,10 +50,11 @@ SM_COUNT, SMSP, LANES, ALU_LANES = 148, 4, 32, 16
 # constants, not something this run measures: each carries the profiles/ file it was read from and the commit the
 # captured library was built from, and the bench line prints both (`traffic_src`) so that a stale figure is visible.
 # Reported only for the workload it was captured on.
+NCU_SWEEP_CAPTURE_COMMIT = "8ae95eb"
 NCU_CAPTURE_COMMIT = "b3dc885"
 # config 3, one launch of k_sweep<64> = gather + theta sweeps of R' ~ 2^21 replicas (algorithmic S*(U + R') + 8R')
-NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 0.651307e9 + 1.031115e9}
-NCU_TRAFFIC_SRC = {"file": "profiles/r2_sweep64_ncu.md", "commit": NCU_CAPTURE_COMMIT}
+NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 0.652404e9 + 1.032230e9}
+NCU_TRAFFIC_SRC = {"file": "profiles/r2_sweep64_ncu.md", "commit": NCU_SWEEP_CAPTURE_COMMIT}
 # a1-a6 chain of config 5: q_reduce (+ level tables) + poisson_scan + copy, read + write
 NCU_RESAMPLE_TRAFFIC_BYTES = 67.15e6 + (67.25e6 + 20.55e6) + (604.61e6 + 2156.73e6)
 NCU_RESAMPLE_TRAFFIC_SRC = {"file": "profiles/r2_resample_ncu.md", "commit": NCU_CAPTURE_COMMIT}
