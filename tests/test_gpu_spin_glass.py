@@ -147,3 +147,21 @@ def test_sharded_ranks_with_bonds_equal_the_single_context(world, L, theta):
         assert np.array_equal(np.concatenate([s_.energies()[0] for s_ in sh.shards]), single.energies()[0])
         for s_ in sh.shards:
             assert rel(s_.log_Z()["lnZ"], single.log_Z()["lnZ"]) <= RTOL
+
+
+def test_set_spins_after_set_bonds_and_device_getters():
+    """the test hook pa_set_spins recomputes E under the Hamiltonian in force; pa_energies with a device destination
+    carries the energy offset of an odd sample too"""
+    b = _binding()
+    L, R = 32, 777
+    Jx, Jy = sample_with_parity(L, 1234, 1)
+    gpu = b.PopulationAnnealer(L, R, seed=8, capacity=4096)
+    gpu.set_bonds(inputs.pack_pm1(Jx), inputs.pack_pm1(Jy))
+    pop = inputs.structured_population(L, 1500, 3)
+    gpu.set_spins(pop)
+    Eo, Mo = orc.energy_mag(L, pop, (Jx, Jy))
+    E, M = gpu.energies()
+    assert gpu.R == 1500 and np.array_equal(E, Eo) and np.array_equal(M, Mo) and np.all(E % 4 == 2)
+    Ed, Md = gpu.energies_device()
+    assert np.array_equal(Ed.cpu().numpy(), Eo) and np.array_equal(Md.cpu().numpy(), Mo)
+    assert gpu.observables()["sum_E"] == int(Eo.astype(np.int64).sum())
