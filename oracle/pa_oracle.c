@@ -356,6 +356,34 @@ void orc_nearest_counts(int64_t R, const double* tau, double scale, uint64_t see
 }
 
 /* ------------------------------------------------------------------------------------------
+ * A4c.  Systematic resampling, another of the "possible modifications of this step" (PAPER.md:54 -> ref. [3]; DESIGN.md
+ * reading G30): ONE keyed 32-bit uniform U per temperature step for the whole population, copy numbers from the
+ * cumulative sum of the weights on a comb of spacing 1:
+ *     Lam_j = floor(lambda_j * 2^32)  (exact: a power-of-two scaling and a floor of a binary64 number, 64-bit integer)
+ *     C_j   = sum_{i<j} Lam_i         (exact 64-bit integer arithmetic: independent of the order of summation)
+ *     off_j = (C_j + U) >> 32,   n_j = off_{j+1} - off_j,   R' = off_R
+ * E[n_j] = Lam_j / 2^32 (= lambda_j up to 2^-32), n_j is one of the two integers next to it, and the population size
+ * is floor(sum_j lambda_j) or that + 1: it stays at R0 instead of fluctuating like sqrt(R0).  U = word 0 of the Philox
+ * counter (0, 0, 1, tag1|step): c2 = 1 keeps it apart from the per-parent chunk counters (c2 = 0).
+ * ---------------------------------------------------------------------------------------- */
+uint32_t orc_systematic_uniform(uint64_t seed, uint32_t step) {
+  uint32_t w[4];
+  philox_keyed(seed, 0u, 0u, 1u, TAG_RESAMPLE, step, w);
+  return w[0];
+}
+void orc_systematic_counts(int64_t R, const double* tau, double scale, uint64_t seed, uint32_t step, uint32_t* n) {
+  uint64_t U = orc_systematic_uniform(seed, step);
+  uint64_t C = 0; /* running sum of Lam, sequential on purpose */
+  for (int64_t j = 0; j < R; ++j) {
+    double lambda = tau[j] * scale;
+    uint64_t Lam = lambda > 0.0 ? (uint64_t)floor(lambda * 4294967296.0) : 0u;
+    uint64_t before = (C + U) >> 32;
+    C += Lam;
+    n[j] = (uint32_t)(((C + U) >> 32) - before);
+  }
+}
+
+/* ------------------------------------------------------------------------------------------
  * A9.  Adaptive temperature step ("Fluctuations can be made smaller and less frequent using the adaptive
  * temperature step, as discussed in the papers [4]"; reading G25).  The overlap of the energy histograms at
  * beta and beta + dbeta, estimated from the population as in ref. [4]:

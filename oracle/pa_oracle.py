@@ -40,6 +40,8 @@ def lib():
             "orc_poisson_counts": (None, [C.c_int64, f64p, C.c_double, C.c_uint64, C.c_uint32, u32p]),
             "orc_nearest": (C.c_uint32, [C.c_double, C.c_uint64, C.c_uint32, C.c_uint32]),
             "orc_nearest_counts": (None, [C.c_int64, f64p, C.c_double, C.c_uint64, C.c_uint32, u32p]),
+            "orc_systematic_uniform": (C.c_uint32, [C.c_uint64, C.c_uint32]),
+            "orc_systematic_counts": (None, [C.c_int64, f64p, C.c_double, C.c_uint64, C.c_uint32, u32p]),
             "orc_overlap": (C.c_double, [C.c_int64, i32p, C.c_double]),
             "orc_adaptive_dbeta": (C.c_double, [C.c_int64, i32p, C.c_double, C.c_double, C.c_int]),
             "orc_exclusive_scan": (C.c_int64, [C.c_int64, u32p, u32p]),
@@ -178,7 +180,7 @@ def poisson_counts(tau, scale, seed, step):
     return n
 
 
-RULE_POISSON, RULE_NEAREST = 0, 1
+RULE_POISSON, RULE_NEAREST, RULE_SYSTEMATIC = 0, 1, 2
 ADAPTIVE_ITERS = 40  # bisection steps of the adaptive temperature step (reading G25)
 
 
@@ -190,6 +192,17 @@ def nearest_counts(tau, scale, seed, step):
     tau = _c(tau, np.float64)
     n = np.zeros(tau.shape[0], np.uint32)
     lib().orc_nearest_counts(tau.shape[0], _p(tau, C.c_double), float(scale), C.c_uint64(seed), int(step), _p(n, C.c_uint32))
+    return n
+
+
+def systematic_uniform(seed, step):
+    return int(lib().orc_systematic_uniform(C.c_uint64(seed), int(step)))
+
+
+def systematic_counts(tau, scale, seed, step):
+    tau = _c(tau, np.float64)
+    n = np.zeros(tau.shape[0], np.uint32)
+    lib().orc_systematic_counts(tau.shape[0], _p(tau, C.c_double), float(scale), C.c_uint64(seed), int(step), _p(n, C.c_uint32))
     return n
 
 
@@ -391,7 +404,9 @@ class OraclePA:
         tau = tau_weights(self.E, dbeta, Q)                          # eq. 4
         scale = float(self.R0) / float(self.R)                       # reading G2
         tau_used = tau if tau_override is None else _c(tau_override, np.float64)
-        if self.rule == RULE_NEAREST:
+        if self.rule == RULE_SYSTEMATIC:
+            n = systematic_counts(tau_used, scale, self.seed, step)  # A4c
+        elif self.rule == RULE_NEAREST:
             n = nearest_counts(tau_used, scale, self.seed, step)     # A4b
         else:
             n = poisson_counts(tau_used, scale, self.seed, step)    # A4

@@ -782,3 +782,52 @@ def test_heating_from_the_ground_states_reaches_the_exact_lnZ_L4():
     g = np.array([float(v) for v in dos.values()])
     w = g * np.exp(-betas[-1] * Es)
     assert abs(pa.E.mean() - (w * Es).sum() / w.sum()) < 0.25
+
+
+# ---------------------------------------------------------------------------------------------------
+# A4c systematic resampling (PAPER.md:54 -> ref. [3]; reading G30)
+# ---------------------------------------------------------------------------------------------------
+def test_systematic_resampling_against_a_big_integer_writing_and_its_laws():
+    rng = np.random.default_rng(11)
+    seed = 0xABCDEF0123
+    for step, R in [(1, 1), (2, 7), (3, 1000), (9, 4097)]:
+        tau = np.exp(rng.normal(0.0, 1.2, R))
+        tau *= R / tau.sum()
+        scale = 0.97
+        n = orc.systematic_counts(tau, scale, seed, step)
+        # second writing: Python integers, U from the big-integer Philox (counter (0, 0, 1, tag 1 | step), word 0)
+        U = philox_ref.keyed(seed, 0, 0, 1, 1, step)[0]
+        assert orc.systematic_uniform(seed, step) == U
+        lam = [float(t) * scale for t in tau]
+        Lam = [int(math.floor(x * 4294967296.0)) for x in lam]
+        C, ref = 0, []
+        for L_ in Lam:
+            ref.append(((C + L_ + U) >> 32) - ((C + U) >> 32))
+            C += L_
+        assert [int(x) for x in n] == ref
+        # laws: n_j is floor or ceil of Lam_j / 2^32; the population is floor(sum Lam / 2^32) or that + 1
+        for nj, L_ in zip(ref, Lam):
+            assert nj in (L_ >> 32, (L_ >> 32) + 1)
+        assert sum(ref) in (C >> 32, (C >> 32) + 1)
+        assert abs(sum(ref) - sum(lam)) < 1.0 + R * 2.0 ** -32
+    # equal unit weights: every parent has exactly one child whatever U is
+    assert np.all(orc.systematic_counts(np.ones(500), 1.0, 5, 1) == 1)
+    assert np.all(orc.systematic_counts(np.zeros(10), 1.0, 5, 1) == 0)
+    # E[n_j] = lambda_j: U runs over the steps; a parent with lambda = 0.3 gets a child in 30 % of the steps
+    tau = np.array([0.3, 1.7, 2.0, 0.25, 3.75])
+    acc = np.zeros(5)
+    K = 4000
+    for step in range(1, K + 1):
+        acc += orc.systematic_counts(tau, 1.0, 77, step)
+    assert np.all(np.abs(acc / K - tau) < 4 * np.sqrt(0.25 / K))
+    assert acc[2] == 2 * K  # integer lambda: deterministic
+
+
+def test_pa_with_systematic_resampling_keeps_the_population_and_gets_lnZ_right():
+    L = 8
+    pa = orc.OraclePA(L, 4096, seed=5, rule=orc.RULE_SYSTEMATIC)
+    for k in range(1, 41):
+        pa.step(0.025 * k, 3)
+        assert abs(pa.R - 4096) <= 1  # sum lambda = R0 up to rounding: the population stays at R0
+    exact = float(exact_ising.kaufman_lnZ(L, 1.0))
+    assert abs(pa.lnZ - exact) < 0.3, (pa.lnZ, exact)
