@@ -52,8 +52,11 @@ enum {
   PA_PROFILE = 4u,     /* record CUDA events around every kernel (pa_profile_read); the events between the kernels
                           keep a kernel's blocks from being placed while its predecessor drains */
   PA_PROFILE_SPAN = 8u, /* record only the PA_K_RESAMPLE_SPAN pair around a1-a6 of every step */
-  PA_RESAMPLE_NEAREST = 16u /* copy counts n_j = floor(lambda_j) + [u_j > 1 - frac(lambda_j)] (nearest integers) instead of
-                               Poisson(lambda_j): one of the modifications PAPER.md:54 points to; A4b */
+  PA_RESAMPLE_NEAREST = 16u, /* copy counts n_j = floor(lambda_j) + [u_j > 1 - frac(lambda_j)] (nearest integers) instead of
+                                Poisson(lambda_j): one of the modifications PAPER.md:54 points to; A4b */
+  PA_RESAMPLE_SYSTEMATIC = 32u /* systematic resampling (A4c): one keyed uniform per step, copy counts from the exact
+                                  64-bit cumulative sum of floor(lambda_j 2^32): the population stays at R0.  Excludes
+                                  PA_RESAMPLE_NEAREST; not available for pa_dist_init (PA_EINVAL) */
 };
 
 /* Redistribution policies (A6b, readings G21-G23).  The children are in parent order and a
@@ -78,7 +81,7 @@ typedef struct {
   void* workspace;  /* DEVICE memory, caller owned, 256-byte aligned, >= pa_workspace_bytes(cfg) */
   uint64_t workspace_bytes;
   void* stream;     /* cudaStream_t, caller owned (NULL = legacy default stream) */
-  uint32_t flags;   /* PA_KEEP_TAU | PA_KEEP_COUNTS | PA_PROFILE | PA_PROFILE_SPAN */
+  uint32_t flags;   /* PA_KEEP_TAU | PA_KEEP_COUNTS | PA_PROFILE | PA_PROFILE_SPAN | PA_RESAMPLE_NEAREST or _SYSTEMATIC */
   uint32_t policy;  /* PA_POLICY_*: how the new population is divided over the P partitions (default 0 = balanced) */
   uint32_t block;   /* PA_POLICY_MAIN: replicas per block (0 => 1024) */
   uint32_t maxexc;  /* PA_POLICY_MAIN: window in blocks (0 => 1) */

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libpa_b200.so")
 
 PA_OK, PA_EINVAL, PA_ENOMEM, PA_ECAPACITY, PA_EEXTINCT, PA_ECUDA = 0, -1, -2, -3, -4, -5
-PA_KEEP_TAU, PA_KEEP_COUNTS, PA_PROFILE, PA_PROFILE_SPAN, PA_RESAMPLE_NEAREST = 1, 2, 4, 8, 16
+PA_KEEP_TAU, PA_KEEP_COUNTS, PA_PROFILE, PA_PROFILE_SPAN, PA_RESAMPLE_NEAREST, PA_RESAMPLE_SYSTEMATIC = 1, 2, 4, 8, 16, 32
 PA_POLICY_BALANCED, PA_POLICY_MAIN, PA_POLICY_NAIVE, PA_POLICY_NONE = 0, 1, 2, 3
 KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "copy", "sweep", "observe", "resample_span"]
 

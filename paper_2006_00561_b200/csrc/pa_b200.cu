@@ -28,7 +28,7 @@ constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
   uint64_t state, params, spins[2], EM[2], off, n, tau, tile_desc, tile_parent, parent_of, red_partial, obs_partial,
-      lev_tau, lev_mu, lev_m, lev_cdf, lev_hist, part[2], part_stats, bond_mask, ovl_hist, total;
+      lev_tau, lev_mu, lev_m, lev_cdf, lev_hist, part[2], part_stats, bond_mask, ovl_hist, sys_tiles, total;
 };
 
 inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
@@ -64,6 +64,7 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   if (!c || !valid_L(c->L) || c->P < 1 || c->R0 < 1 || c->R0 >= (1ll << 31) || cap < c->R0 || cap >= (1ll << 32) - 4096)
     return false;
   if (c->policy > PA_POLICY_NONE || (c->policy != PA_POLICY_BALANCED && c->P > BAL_PMAX)) return false;
+  if ((c->flags & PA_RESAMPLE_NEAREST) && (c->flags & PA_RESAMPLE_SYSTEMATIC)) return false;  // one resampling rule
   const uint64_t N = (uint64_t)c->L * c->L, S = N / 8, nlev = N + 1, ucap = (uint64_t)cap;
   uint64_t o = 0;
   auto take = [&](uint64_t bytes) {
@@ -76,7 +77,7 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   for (int b = 0; b < 2; ++b) lo->spins[b] = take(ucap * S + 64);  // + 64: the spare buffer doubles as the E / M staging area of pa_energies (8 n + 12 bytes at L = 8)
   for (int b = 0; b < 2; ++b) lo->EM[b] = take(ucap * 4);  // packed E/4 : M/2, one word per replica
   lo->off = take((ucap + 1) * 4);
-  lo->n = (c->flags & PA_KEEP_COUNTS) ? take(ucap * 4) : 0;
+  lo->n = (c->flags & (PA_KEEP_COUNTS | PA_RESAMPLE_SYSTEMATIC)) ? take(ucap * 4) : 0;  // A4c hands its counts to the scan through n
   lo->tau = (c->flags & PA_KEEP_TAU) ? take(ucap * 8) : 0;
   lo->tile_desc = take(((ucap + SCAN_TILE - 1) / SCAN_TILE + 1) * 8);
   lo->tile_parent = take((ucap / copy_tile_for(c->L) + 2) * 4);  // theta = 0: first parent of every copy tile
@@ -92,6 +93,7 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   lo->part_stats = take((uint64_t)c->P * 16);
   lo->bond_mask = take(N / 2);        // +-J model: negative-bond masks, 2 colours x N/64 plane words x 4 bonds (pa_sweep.cuh)
   lo->ovl_hist = take(nlev * 8);      // overlap histogram (pa_overlap_hist)
+  lo->sys_tiles = take(((ucap + SCAN_TILE - 1) / SCAN_TILE + 1) * 8);  // systematic resampling: tile sums / prefixes of Lam
   lo->total = o;
   return true;
 }
@@ -118,7 +120,7 @@ struct pa_ctx {
   double beta, sum_lnQ, last_Q;
   int64_t launches;
   bool profile, profile_span;
-  int nearest;  // PA_RESAMPLE_NEAREST: nearest-integer copy counts instead of Poisson
+  int nearest;  // resampling rule: 0 Poisson (A4), 1 PA_RESAMPLE_NEAREST (A4b), 2 PA_RESAMPLE_SYSTEMATIC (A4c)
   bool glass;   // pa_set_bonds: the +-J Hamiltonian (sweep kernels compiled with the coupling masks)
   int e_off;    // E mod 4 of every configuration (0 unless the sample has an odd number of negative bonds: 2)
   bool attempt_failed;  // the last pa_step / pa_run ended with an uncommitted step: off / n / tau hold that attempt
@@ -294,8 +296,8 @@ unsigned scan_grid(pa_ctx* c, bool map) {
   int& g = c->scan_grid_max[map ? 1 : 0];
   if (g == 0) {
     int per_sm = 0, sms = 0;
-    if (map) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true, false>, SCAN_THREADS, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, false, false>, SCAN_THREADS, 0);
+    if (map) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, true, 0>, SCAN_THREADS, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_poisson_scan<true, false, 0>, SCAN_THREADS, 0);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
     g = (per_sm > 0 && sms > 0) ? per_sm * sms : 148 * 4;
   }
@@ -303,13 +305,15 @@ unsigned scan_grid(pa_ctx* c, bool map) {
   return tiles_cap < (unsigned)g ? (tiles_cap ? tiles_cap : 1u) : (unsigned)g;
 }
 
-// k_poisson_scan<KEEP, MAP, NEAREST>: KEEP = parity getters want tau / n, MAP = the consumer is the sweep's gather-on-load
-// (child -> parent map) rather than k_copy (first parent per copy tile), NEAREST = resampling rule A4b instead of Poisson
+// k_poisson_scan<KEEP, MAP, RULE>: KEEP = parity getters want tau / n, MAP = the consumer is the sweep's gather-on-load
+// (child -> parent map) rather than k_copy (first parent per copy tile), RULE = 0 Poisson, 1 nearest integers (A4b),
+// 2 counts given by the systematic-resampling kernels (A4c)
 template <bool KEEP, bool MAP>
 void launch_scan_rule(pa_ctx* c, unsigned grid, DevState* st, const int32_t* E0, const int32_t* E1, const LevelTables& tb,
                       const ScanOut& out, int shift, unsigned long long cap) {
-  if (c->nearest) launch(c, "k_poisson_scan", k_poisson_scan<KEEP, MAP, true>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
-  else launch(c, "k_poisson_scan", k_poisson_scan<KEEP, MAP, false>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
+  if (c->nearest == 2) launch(c, "k_poisson_scan", k_poisson_scan<KEEP, MAP, 2>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
+  else if (c->nearest == 1) launch(c, "k_poisson_scan", k_poisson_scan<KEEP, MAP, 1>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
+  else launch(c, "k_poisson_scan", k_poisson_scan<KEEP, MAP, 0>, grid, SCAN_THREADS, st, E0, E1, tb, c->N, out, shift, cap, c->key);
 }
 void launch_scan(pa_ctx* c, bool keep, bool map, unsigned grid, DevState* st, const int32_t* E0, const int32_t* E1,
                  const LevelTables& tb, const ScanOut& out, int shift, unsigned long long cap) {
@@ -350,6 +354,16 @@ void enqueue_step(pa_ctx* c, const StepParams* sp, const StepParams& hp) {
     const int shift = copy_shift_for(c->cfg.L);
     const unsigned long long cap = (unsigned long long)c->cap;
     const unsigned grid = scan_grid(c, theta > 0);
+    if (c->nearest == 2) {  // A4c: 64-bit prefix of Lam -> copy counts in out.n, which the scan then only places
+      const unsigned ntiles = (unsigned)((c->cap + SCAN_TILE - 1) / SCAN_TILE);
+      unsigned long long* tiles = c->dev<unsigned long long>(c->lo.sys_tiles);
+      Prof p(c, PA_K_POISSON_SCAN);
+      launch(c, "k_sys_tile_sums", k_sys_tile_sums, ntiles, SYS_THREADS, (const DevState*)st, E0, E1, tb, N, tiles);
+      c->launches += 2;
+      launch(c, "k_sys_scan_tiles", k_sys_scan_tiles, 1u, 1024u, (const DevState*)st, tiles, ntiles);
+      launch(c, "k_sys_counts", k_sys_counts, ntiles, SYS_THREADS, (const DevState*)st, E0, E1, tb, N, (const unsigned long long*)tiles,
+             out.n, c->key);
+    }
     Prof p(c, PA_K_POISSON_SCAN);
     launch_scan(c, keep, theta > 0, grid, st, E0, E1, tb, out, shift, cap);
   }
@@ -515,7 +529,7 @@ int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t
   c->stream = static_cast<cudaStream_t>(cfg->stream);
   c->profile = (cfg->flags & PA_PROFILE) != 0;
   c->profile_span = (cfg->flags & PA_PROFILE_SPAN) != 0;
-  c->nearest = (cfg->flags & PA_RESAMPLE_NEAREST) ? 1 : 0;
+  c->nearest = (cfg->flags & PA_RESAMPLE_SYSTEMATIC) ? 2 : ((cfg->flags & PA_RESAMPLE_NEAREST) ? 1 : 0);
   c->glass = false;
   c->e_off = 0;
   c->launches = 0;
@@ -910,6 +924,7 @@ int pa_dist_exchange_plan(int32_t world, const int64_t* T, int32_t policy, uint3
 int pa_dist_init(const pa_config* cfg, int32_t rank, int32_t world, pa_ctx** out) {
   if (!cfg || !out || world < 1 || rank < 0 || rank >= world || cfg->R0 < world) return PA_EINVAL;
   if (cfg->policy != PA_POLICY_BALANCED && world > BAL_PMAX) return PA_EINVAL;
+  if (cfg->flags & PA_RESAMPLE_SYSTEMATIC) return PA_EINVAL;  // A4c's prefix sum would span the ranks (reading G30)
   pa_config local = *cfg;
   const int64_t first = balanced_start(cfg->R0, world, rank), last = balanced_start(cfg->R0, world, rank + 1);
   local.R0 = last - first;

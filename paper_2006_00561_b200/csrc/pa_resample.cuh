@@ -54,7 +54,7 @@ __device__ __forceinline__ double expneg_a4(double mu) {
 }
 
 __device__ __forceinline__ void level_tables(double dbeta, int lev, int N, int e_off, double Q, double scale, const LevelTables& tb,
-                                             const bool nearest) {
+                                             const int rule /* 0 Poisson, 1 nearest (A4b), 2 systematic (A4c) */) {
   const double tau = __ddiv_rn(level_weight(dbeta, lev, N, e_off), Q);
   const double lambda = __dmul_rn(tau, scale);
   tb.tau[lev] = tau;
@@ -69,7 +69,13 @@ __device__ __forceinline__ void level_tables(double dbeta, int lev, int N, int e
     tb.mu[lev] = 0.0;
     return;
   }
-  if (nearest) {  // A4b: n = floor(lambda) + [u > 1 - frac(lambda)]: one uniform per parent, never a heavy parent
+  if (rule == 2) {  // A4c: Lam = floor(lambda * 2^32) as a 64-bit integer (exact), kept in the mu slot
+    tb.m[lev] = 1u;
+    tb.mu[lev] = __longlong_as_double((long long)floor(__dmul_rn(lambda, 4294967296.0)));
+    F[0] = 2.0; F[1] = 2.0; F[2] = 2.0; F[3] = 2.0;
+    return;
+  }
+  if (rule == 1) {  // A4b: n = floor(lambda) + [u > 1 - frac(lambda)]: one uniform per parent, never a heavy parent
     const double fl = floor(lambda);
     tb.m[lev] = 1u;
     tb.mu[lev] = lambda;
@@ -222,7 +228,7 @@ k_q_reduce(DevState* st, const StepParams* __restrict__ sp, const int32_t* __res
   {
     const double Q = s_Q, scale = R0 / (double)R;
     const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
-    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(dbeta, lev, N, e_off, Q, scale, tb, nearest != 0);
+    for (int lev = lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(dbeta, lev, N, e_off, Q, scale, tb, nearest);
   }
 }
 
@@ -244,7 +250,7 @@ k_dist_tables(DevState* st, const StepParams* __restrict__ sp, int N, double sum
     st->scale = scale;
   }
   const int lev_hi = st->lev_hi < N ? st->lev_hi : N;
-  for (int lev = st->lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(sp->dbeta, lev, N, st->e_off, Q, scale, tb, nearest != 0);
+  for (int lev = st->lev_lo + threadIdx.x; lev <= lev_hi; lev += RED_THREADS) level_tables(sp->dbeta, lev, N, st->e_off, Q, scale, tb, nearest);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -323,7 +329,9 @@ constexpr unsigned NO_TILE = 0xffffffffu;
 #ifndef PA_SCAN_MINB
 #define PA_SCAN_MINB 6
 #endif
-template <bool KEEP, bool MAP, bool NEAREST>
+// RULE: 0 Poisson (A4), 1 nearest integers (A4b), 2 the copy counts are GIVEN in out.n (systematic resampling, A4c: written
+// by k_sys_counts) and only scanned and placed here
+template <bool KEEP, bool MAP, int RULE>
 __global__ void __launch_bounds__(SCAN_THREADS, (MAP ? PA_SCAN_MINB - 1 : PA_SCAN_MINB))
 k_poisson_scan(DevState* st, const int32_t* __restrict__ EM0, const int32_t* __restrict__ EM1, LevelTables tb, int N,
                ScanOut out, int copy_shift, unsigned long long capacity, const PhiloxKey key) {
@@ -379,7 +387,7 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ EM0, const int32_t* __r
         uint32_t jj[SCAN_BATCH];
         int e[SCAN_BATCH];
         unsigned m[SCAN_BATCH], k[SCAN_BATCH], c4[SCAN_BATCH], hl[SCAN_BATCH];
-        double u[SCAN_BATCH];
+        [[maybe_unused]] double u[SCAN_BATCH];
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           jj[b] = tile_base + (r0 + b) * SCAN_THREADS + threadIdx.x;
@@ -395,11 +403,15 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ EM0, const int32_t* __r
             if (out.tau && jj[b] < R) out.tau[jj[b]] = __ldg(tb.tau + lev);
           }
         }
+        if constexpr (RULE != 2) {
 #pragma unroll
-        for (int b = 0; b < SCAN_BATCH; ++b) u[b] = chunk_uniform(philox4x32_10(0u, jj[b] + slot0, 0u, c3, key), 0u);
+          for (int b = 0; b < SCAN_BATCH; ++b) u[b] = chunk_uniform(philox4x32_10(0u, jj[b] + slot0, 0u, c3, key), 0u);
+        }
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {  // rows of unused levels are masked below
-          if (ALL || hl[b] < (unsigned)SCAN_HW) {
+          if constexpr (RULE == 2) {
+            c4[b] = (jj[b] < R) ? __ldg(out.n + jj[b]) : 0u;
+          } else if (ALL || hl[b] < (unsigned)SCAN_HW) {
             const double2 f01 = *reinterpret_cast<const double2*>(&s_head[hl[b]][0]);
             const double2 f23 = *reinterpret_cast<const double2*>(&s_head[hl[b]][2]);
             c4[b] = (unsigned)(u[b] > f01.x) + (unsigned)(u[b] > f01.y) + (unsigned)(u[b] > f23.x) + (unsigned)(u[b] > f23.y);
@@ -410,7 +422,9 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ EM0, const int32_t* __r
 #pragma unroll
         for (int b = 0; b < SCAN_BATCH; ++b) {
           k[b] = c4[b];
-          if constexpr (NEAREST) {  // A4b: n = floor(lambda) + [u > 1 - frac(lambda)], both from the head of the row
+          if constexpr (RULE == 2) {
+            // given
+          } else if constexpr (RULE == 1) {  // A4b: n = floor(lambda) + [u > 1 - frac(lambda)], both from the head of the row
             const double* F = (ALL || hl[b] < (unsigned)SCAN_HW) ? &s_head[hl[b]][0] : tb.cdf + (size_t)(hl[b] + (unsigned)lev_lo) * PO_ROW;
             k[b] = (unsigned)__double_as_longlong(F[1]) + (u[b] > F[0] ? 1u : 0u);
           } else if (c4[b] == 4u)
@@ -668,6 +682,117 @@ k_poisson_scan(DevState* st, const int32_t* __restrict__ EM0, const int32_t* __r
     if (tile == NO_TILE) break;
     prev = tile;
     buf ^= 1;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Systematic resampling (A4c): the copy counts come from the 64-bit prefix sum of Lam_j = floor(lambda_j 2^32),
+// off_j = (C_j + U) >> 32.  Three small kernels in front of the scan, which then takes the counts as given:
+//   k_sys_tile_sums   sum of Lam over every tile of 2048 parents
+//   k_sys_scan_tiles  exclusive prefix over the tile sums (one block; the tiles are few: cap / 2048)
+//   k_sys_counts      prefix inside the tile, n_j = ((C_j + Lam_j + U) >> 32) - ((C_j + U) >> 32)
+// Integer arithmetic throughout: any order of the additions gives the oracle's bits.
+// ---------------------------------------------------------------------------------------------------
+constexpr int SYS_THREADS = 256, SYS_ITEMS = 8, SYS_TILE = SYS_THREADS * SYS_ITEMS;
+static_assert(SYS_TILE == SCAN_TILE, "one tile geometry");
+
+__device__ __forceinline__ unsigned long long sys_lam(const int32_t* __restrict__ E, uint32_t j, uint32_t R, const LevelTables& tb, int N) {
+  if (j >= R) return 0ull;
+  const int lev = em_level(__ldg(E + j), N);
+  return __ldg(tb.m + lev) == 1u ? (unsigned long long)__double_as_longlong(__ldg(tb.mu + lev)) : 0ull;  // 0 / overflow levels: the scan reports them
+}
+
+__device__ __forceinline__ unsigned long long block_sum_u64(unsigned long long v, unsigned long long* s_w /* SYS_THREADS / 32 */) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = v;
+  __syncthreads();
+  unsigned long long t = 0ull;
+#pragma unroll
+  for (int w = 0; w < SYS_THREADS / 32; ++w) t += s_w[w];
+  return t;
+}
+
+__global__ void __launch_bounds__(SYS_THREADS)
+k_sys_tile_sums(const DevState* __restrict__ st, const int32_t* __restrict__ EM0, const int32_t* __restrict__ EM1, LevelTables tb,
+                int N, unsigned long long* __restrict__ tile_sum) {
+  grid_dependency_wait();
+  if (st->status != ST_OK) return;
+  __shared__ unsigned long long s_w[SYS_THREADS / 32];
+  const int32_t* __restrict__ E = st->cur ? EM1 : EM0;
+  const uint32_t R = (uint32_t)st->R, base = blockIdx.x * SYS_TILE;
+  unsigned long long v = 0ull;
+  if (base < R) {
+#pragma unroll
+    for (int i = 0; i < SYS_ITEMS; ++i) v += sys_lam(E, base + i * SYS_THREADS + threadIdx.x, R, tb, N);
+  }
+  const unsigned long long t = block_sum_u64(v, s_w);
+  if (threadIdx.x == 0) tile_sum[blockIdx.x] = t;
+}
+
+// in place: tile_sum[t] <- sum of the tiles before t
+__global__ void __launch_bounds__(1024)
+k_sys_scan_tiles(const DevState* __restrict__ st, unsigned long long* __restrict__ tile_sum, unsigned ntiles) {
+  grid_dependency_wait();
+  if (st->status != ST_OK) return;
+  __shared__ unsigned long long s_w[32];
+  __shared__ unsigned long long s_carry;
+  if (threadIdx.x == 0) s_carry = 0ull;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (unsigned b = 0; b < ntiles; b += 1024u) {
+    const unsigned t = b + threadIdx.x;
+    const unsigned long long x = t < ntiles ? tile_sum[t] : 0ull;
+    unsigned long long inc = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned long long y = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += y;
+    }
+    if (lane == 31) s_w[warp] = inc;
+    __syncthreads();
+    unsigned long long before = s_carry;
+    for (int w = 0; w < warp; ++w) before += s_w[w];
+    if (t < ntiles) tile_sum[t] = before + inc - x;
+    __syncthreads();
+    if (threadIdx.x == 1023) s_carry = before + inc;
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(SYS_THREADS)
+k_sys_counts(const DevState* __restrict__ st, const int32_t* __restrict__ EM0, const int32_t* __restrict__ EM1, LevelTables tb, int N,
+             const unsigned long long* __restrict__ tile_prefix, uint32_t* __restrict__ n_out, const PhiloxKey key) {
+  grid_dependency_wait();
+  if (st->status != ST_OK) return;
+  __shared__ unsigned long long s_w[SYS_THREADS / 32];
+  const int32_t* __restrict__ E = st->cur ? EM1 : EM0;
+  const uint32_t R = (uint32_t)st->R, base = blockIdx.x * SYS_TILE;
+  if (base >= R) return;
+  const unsigned long long U = philox4x32_10(0u, 0u, 1u, ctr3(TAG_RESAMPLE, st->step + 1u), key).x;  // one uniform per step
+  const uint32_t j0 = base + SYS_ITEMS * threadIdx.x;  // the thread's SYS_ITEMS consecutive parents
+  unsigned long long lam[SYS_ITEMS], tsum = 0ull;
+#pragma unroll
+  for (int i = 0; i < SYS_ITEMS; ++i) {
+    lam[i] = sys_lam(E, j0 + i, R, tb, N);
+    tsum += lam[i];
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  unsigned long long inc = tsum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned long long y = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += y;
+  }
+  if (lane == 31) s_w[warp] = inc;
+  __syncthreads();
+  unsigned long long C = tile_prefix[blockIdx.x] + (inc - tsum);
+  for (int w = 0; w < warp; ++w) C += s_w[w];
+#pragma unroll
+  for (int i = 0; i < SYS_ITEMS; ++i) {
+    const unsigned long long before = (C + U) >> 32;
+    C += lam[i];
+    if (j0 + i < R) n_out[j0 + i] = (uint32_t)(((C + U) >> 32) - before);
   }
 }
 

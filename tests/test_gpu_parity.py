@@ -34,7 +34,7 @@ def rel(a, b):
 def make_pair(L, R0, P, seed, beta0=0.0, capacity=0, spins=None, policy=0, block=1024, maxexc=1, rule=0, bonds=None):
     b = _binding()
     gpu = b.PopulationAnnealer(L, R0, P=P, seed=seed, beta0=beta0, capacity=capacity,
-                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS | (b.PA_RESAMPLE_NEAREST if rule else 0), policy=policy,
+                               flags=b.PA_KEEP_TAU | b.PA_KEEP_COUNTS | {0: 0, 1: b.PA_RESAMPLE_NEAREST, 2: b.PA_RESAMPLE_SYSTEMATIC}[rule], policy=policy,
                                block=block, maxexc=maxexc)
     if spins is not None:
         gpu.set_spins(spins)
@@ -437,6 +437,39 @@ def test_heating_protocol_lockstep(L, R0):
     betas = [beta0 - dbeta * k for k in range(1, 11)]
     lockstep(gpu, ora, betas, theta=2)
     assert gpu.log_Z()["sum_lnQ"] < 0.0 and rel(gpu.log_Z()["sum_lnQ"], ora.sum_lnQ) <= RTOL
+
+
+@pytest.mark.parametrize("L,R0,theta", [(8, 1, 1), (8, 2049, 2), (16, 5000, 1), (32, 4097, 0), (64, 700, 2), (128, 90, 1),
+                                        (8, 3000001, 0)])  # the last: 1465 tiles, more than one pass of the tile-prefix block
+def test_systematic_resampling_lockstep(L, R0, theta):
+    """A4c (PA_RESAMPLE_SYSTEMATIC): counts from the exact 64-bit cumulative weights on the device == the oracle's
+    sequential loop, the population stays at R0 (+-1), lock-step over tile boundaries (2048 parents) and ragged sizes"""
+    gpu, ora = make_pair(L, R0, 3, seed=900 + L, rule=2)
+    dbeta = min(0.06, 300.0 / (2 * L * L))
+    lockstep(gpu, ora, [dbeta * k for k in range(1, 7 if R0 < 100000 else 3)], theta=theta)
+    assert abs(gpu.R - R0) <= 1
+
+
+def test_systematic_resampling_on_a_skewed_population_and_without_the_keep_flags():
+    b = _binding()
+    L, R0 = 32, 20000
+    spins = inputs.structured_population(L, R0, 5)
+    gpu, ora = make_pair(L, R0, 148, seed=4, spins=spins, rule=2)   # copy counts of thousands per parent
+    lockstep(gpu, ora, [0.03, 0.06], theta=0)
+    lockstep(gpu, ora, [0.09], theta=1)
+    assert abs(gpu.R - R0) <= 1
+    # the timed configuration: no KEEP flags (the counts still travel through the n array), whole schedule in one call
+    plain = b.PopulationAnnealer(L, R0, P=148, seed=4, flags=b.PA_RESAMPLE_SYSTEMATIC)
+    plain.set_spins(spins)
+    plain.run([0.03, 0.06], 0)
+    plain.run([0.09], 1)
+    assert plain.R == gpu.R and np.array_equal(plain.spins(), gpu.spins())
+    with pytest.raises(b.PaError) as e:
+        b.PopulationAnnealer(L, 100, flags=b.PA_RESAMPLE_SYSTEMATIC | b.PA_RESAMPLE_NEAREST)
+    assert e.value.code == b.PA_EINVAL
+    with pytest.raises(b.PaError) as e:
+        b.PopulationAnnealer(L, 100, flags=b.PA_RESAMPLE_SYSTEMATIC, rank=0, world=2)
+    assert e.value.code == b.PA_EINVAL
 
 
 def test_failed_step_does_not_leak_into_the_getters():
