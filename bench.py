@@ -222,6 +222,19 @@ def resample_leg(binding, torch, peaks, repeats=5):
         del pa, off
     torch.cuda.empty_cache()
     R, Rn, U = res
+    # the other resampling rules on the same population (A4b, A4c): a1-a6 span only
+    rules = {}
+    for name, flag in (("nearest", binding.PA_RESAMPLE_NEAREST), ("systematic", binding.PA_RESAMPLE_SYSTEMATIC)):
+        tt, Rr = [], None
+        for rep in range(3):
+            pa = binding.PopulationAnnealer(wl.L, wl.R0, P=wl.P, seed=wl.seed, beta0=wl.beta0, flags=binding.PA_PROFILE_SPAN | flag)
+            pa.profile_read()
+            pa.step(wl.beta_K, 0)
+            tt.append(pa.profile_read()["resample_span"][0])
+            Rr = pa.R
+            del pa
+        rules[name] = {"ms_a1_a6_kernels": statistics.median(tt), "R_new": Rr}
+    torch.cuda.empty_cache()
     chain = statistics.median(t[0] for t in spans)
     chain_profiled = statistics.median(t[0] for t in times)
     wall = statistics.median(t[1] for t in spans)
@@ -234,7 +247,7 @@ def resample_leg(binding, torch, peaks, repeats=5):
     return {"workload": wl.name, "R": R, "R_new": Rn, "U": U, "algorithmic_bytes": alg_bytes,
             "ms_a1_a6_kernels": chain, "ms_a1_a6_with_events_between_kernels": chain_profiled,
             "ms_sum_of_kernel_durations": ksum, "ms_step_wall": wall, "ms_copy": copy_ms, "ms_poisson_scan": scan_ms,
-            "ms_q_reduce": red_ms, "replicas_per_s": Rn / (chain * 1e-3),
+            "ms_q_reduce": red_ms, "replicas_per_s": Rn / (chain * 1e-3), "other_rules": rules,
             "roofline": {"bound": "hbm", "achieved": alg_bytes / (chain * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                          "unit": "GB/s", "frac": alg_bytes / (chain * 1e-3) / 1e9 / peaks["hbm_gbs"],
                          "peak_src": peaks["src"], "traffic": NCU_RESAMPLE_TRAFFIC_BYTES,
