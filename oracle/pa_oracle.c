@@ -26,6 +26,8 @@
  * rule, global-flip covariance.  Section D1 (+-J spin glass, overlap histogram): tests/test_oracle_spin_glass.py --
  * numpy second writing on all 2^16 states of L = 4, parity law of E, gauge covariance onto the pinned ferromagnet,
  * hand-worked zero-temperature moves, Boltzmann chi-square and PA ln Z of a frustrated sample against enumeration.
+ * Section A4c (systematic resampling): a Python-integer second writing with the big-integer Philox, floor / ceil and
+ * population laws, E[n] = lambda.  Heating protocol (negative dbeta): ln Z of the 4x4 torus from its ground states.
  * No function here is "parity unpinned".
  */
 #include <math.h>
