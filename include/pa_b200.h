@@ -197,6 +197,36 @@ int pa_set_bonds(pa_ctx* ctx, const uint32_t* Jx, const uint32_t* Jy);
  * Works for either Hamiltonian; synchronises. */
 int pa_overlap_hist(pa_ctx* ctx, uint64_t* hist);
 
+/* ---- for callers that must not allocate: one call that creates nothing ---------------------------------- */
+/* Every other entry point needs a pa_ctx (pa_init pins host memory) and a workspace the caller has allocated.  This one
+ * needs neither, for users who cannot allocate when they want the order-parameter histogram: a hook running while
+ * something else (a framework's caching allocator, another simulation) holds all of the GPU's memory; a monitoring loop
+ * that must not stall the device (cudaFree synchronises it, cudaMalloc can); code that is handed a device pointer and a
+ * stream and nothing else.  It calls no cudaMalloc / cudaFree / cudaHostAlloc and no routine that does.
+ *
+ * Computes what pa_overlap_hist computes (D1, reading G28), on lattices the CALLER holds:
+ *   spins  DEVICE, R packed lattices of L x L spins in layout C2 (R * L*L/32 uint32 words), on the current GPU, read only
+ *   hist   L*L + 1 uint64 entries, HOST (hist_on_device = 0) or DEVICE (1), overwritten:
+ *          hist[(q + N) / 2] = number of pairs (j, j + floor(R/2)), j < floor(R/2), with overlap q
+ *   stream cudaStream_t of the current GPU (NULL = legacy default stream); all device work is issued on it
+ * HOST hist: returns after the result has arrived (synchronises the stream).  DEVICE hist: returns after enqueueing.
+ *
+ * The 64-bit accumulation bins -- scratch the context path keeps in its workspace -- are a fixed array inside the
+ * library image: 131 328 bytes (128*128 + 1 counters, padded) on every GPU that loads the library, held until the process
+ * exits.  Limit: L <= PA_STATIC_MAX_L; a larger L returns PA_EINVAL ("lattice too large for the static scratch").
+ * Also PA_EINVAL: L not in {8,16,32,64,128}, R outside [0, 2^31), NULL pointers, spins not device memory of the
+ * current GPU.  PA_ECUDA: a CUDA call failed.  pa_static_last_error() has the message (per host thread).
+ *
+ * The array is shared by all calls on a GPU and keeps the previous call's counts; each call clears the bins it uses
+ * first.  Calls whose GPU work may overlap (different streams without an ordering between them, concurrent host
+ * threads) race on it and return garbage; calls on one stream or separated by a synchronisation are safe.
+ * The first call on each GPU looks up the array's device address (cudaGetSymbolAddress, with that GPU current), which
+ * can make the CUDA runtime load the library's device code: make that first call early, before any stream capture
+ * begins.  Later calls on that GPU reuse the address. */
+#define PA_STATIC_MAX_L 128
+int pa_overlap_hist_static(const uint32_t* spins, int32_t L, int64_t R, uint64_t* hist, int hist_on_device, void* stream);
+const char* pa_static_last_error(void);
+
 /* ---- multi-GPU: partitioned redistribution, one rank = one partition -------- */
 /* The population is sharded over `world` ranks in global slot order: rank r owns the contiguous global slots
  * [start_r, start_{r+1}).  Every random number is keyed by the GLOBAL replica index, so the ranks together compute

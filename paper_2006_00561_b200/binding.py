@@ -18,7 +18,7 @@ KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "cop
 
 EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_adaptive_beta", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
            "pa_observables", "pa_spins", "pa_tau", "pa_counts", "pa_parents", "pa_partitions", "pa_thresholds",
-           "pa_set_spins", "pa_debug_set_thresholds", "pa_set_bonds", "pa_overlap_hist", "pa_dist_init", "pa_dist_workspace_bytes", "pa_dist_begin",
+           "pa_set_spins", "pa_debug_set_thresholds", "pa_set_bonds", "pa_overlap_hist", "pa_overlap_hist_static", "pa_static_last_error", "pa_dist_init", "pa_dist_workspace_bytes", "pa_dist_begin",
            "pa_dist_resample", "pa_dist_exchange_plan", "pa_dist_buffers", "pa_dist_finish", "pa_dist_new_count",
            "pa_dist_abort", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
 
@@ -82,6 +82,8 @@ def load_library():
         "pa_debug_set_thresholds": (C.c_int, [vp, C.c_int, C.c_uint32, C.c_uint32]),
         "pa_set_bonds": (C.c_int, [vp, vp, vp]),
         "pa_overlap_hist": (C.c_int, [vp, vp]),
+        "pa_overlap_hist_static": (C.c_int, [vp, C.c_int32, C.c_int64, vp, C.c_int, vp]),
+        "pa_static_last_error": (C.c_char_p, []),
         "pa_dist_init": (C.c_int, [C.POINTER(PaConfig), C.c_int32, C.c_int32, C.POINTER(vp)]),
         "pa_dist_workspace_bytes": (C.c_uint64, [C.POINTER(PaConfig), C.c_int32]),
         "pa_dist_begin": (C.c_int, [vp, C.c_double, C.c_int32, C.POINTER(PaDistPartial)]),
@@ -121,6 +123,36 @@ def exchange_plan(T, policy=PA_POLICY_BALANCED, block=0, maxexc=0):
     if rc != PA_OK:
         raise PaError(rc, {PA_EEXTINCT: "population extinct", PA_ECAPACITY: "a rank's offspring exceed its capacity"}.get(rc, "bad plan arguments"))
     return ns, base, counts
+
+
+def overlap_hist_static(spins, L, R=None, out=None, stream=None):
+    """pa_overlap_hist_static: the overlap histogram of lattices the caller holds, for callers that cannot allocate
+    (no context, no workspace; the library's built-in scratch array holds the bins, L <= 128).
+
+    spins: torch uint8/int32 tensor on the current CUDA device holding R packed lattices (layout C2), R defaults to
+    what the tensor holds.  out: None -> a new numpy uint64 array of L*L + 1 entries is returned (the call has then
+    synchronised the stream); a torch int64 CUDA tensor of L*L + 1 entries -> filled asynchronously on `stream` and
+    returned.  stream: torch stream (default: the current one).  Calls that can overlap on the GPU race on the scratch."""
+    import torch
+    lib = load_library()
+    L = int(L)
+    N = L * L
+    nbytes = spins.numel() * spins.element_size()
+    R = nbytes // max(N // 8, 1) if R is None else int(R)
+    if R * (N // 8) > nbytes:
+        raise PaError(PA_EINVAL, "overlap_hist_static: the tensor holds fewer than R lattices")
+    st = torch.cuda.current_stream(spins.device) if stream is None else stream
+    if out is None:
+        h = np.zeros(N + 1, np.uint64)
+        dst, on_dev = _np_ptr(h), 0
+    else:
+        if out.numel() * out.element_size() < (N + 1) * 8 or not out.is_cuda:
+            raise PaError(PA_EINVAL, "overlap_hist_static: out must be a CUDA tensor of L*L + 1 64-bit entries")
+        h, dst, on_dev = out, C.c_void_p(out.data_ptr()), 1
+    rc = lib.pa_overlap_hist_static(C.c_void_p(spins.data_ptr()), L, R, dst, on_dev, C.c_void_p(st.cuda_stream))
+    if rc != PA_OK:
+        raise PaError(rc, lib.pa_static_last_error().decode())
+    return h
 
 
 class PopulationAnnealer:

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpa_b200.so")
-SOURCES = [os.path.join(CSRC, "pa_b200.cu")]
+SOURCES = [os.path.join(CSRC, "pa_b200.cu"), os.path.join(CSRC, "pa_static.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("pa_common.cuh", "pa_sweep.cuh", "pa_resample.cuh", "pa_observe.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "pa_b200.h")]
 
