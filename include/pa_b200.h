@@ -263,15 +263,28 @@ int pa_dist_resample(pa_ctx* ctx, const pa_dist_partial* all, int64_t* offspring
  * counts[src * world + dst] = children rank src sends to rank dst (its own share included).  PA_EEXTINCT if sum T = 0. */
 int pa_dist_exchange_plan(int32_t world, const int64_t* T, int32_t policy, uint32_t block, uint32_t maxexc,
                           int64_t* new_start, int64_t* base, int64_t* counts);
+/* Pure host function, no CUDA: may the plan be carried out?  new_start as written by pa_dist_exchange_plan; cap[r] = slots
+ * per buffer of rank r in rank order (pa_dist_capacity, gathered together with the offspring totals; NULL = do not check).
+ * PA_ECAPACITY if some rank's new share exceeds that rank's capacity (policy main can leave a rank up to block - 1
+ * replicas above its balanced count) or the population outgrows 32-bit slot indices; PA_EEXTINCT if some rank's new share
+ * is empty (policy none with a rank without offspring, or fewer children than ranks): a shard cannot be empty.  Every
+ * rank evaluates this on the same gathered numbers BEFORE the exchange, so all ranks refuse the step or none does;
+ * after a refusal every rank calls pa_dist_abort. */
+int pa_dist_plan_check(int32_t world, const int64_t* new_start, const int64_t* cap);
+/* slots per buffer of this rank (cfg.capacity as resolved by pa_dist_init) */
+int pa_dist_capacity(pa_ctx* ctx, int64_t* cap);
 /* DEVICE pointers of the step in flight: children = the rank's offspring in child order (send side), population = where
  * the rank's new population must be written (receive side); valid between pa_dist_resample and pa_dist_finish. */
 int pa_dist_buffers(pa_ctx* ctx, void** children, void** population);
-/* T_all as given to the plan.  PA_ECAPACITY if the rank's new share exceeds its capacity (check BEFORE exchanging with
- * pa_dist_new_count).  local (may be NULL) receives the rank's population sums. */
+/* T_all as given to the plan.  PA_ECAPACITY / PA_EEXTINCT if the rank's new share exceeds its capacity / is empty: check
+ * BEFORE exchanging, on every rank for every rank, with pa_dist_plan_check -- a refusal here comes after the other ranks
+ * have exchanged and would leave them committed while this one is not (the step stays in flight: pa_dist_abort).
+ * local (may be NULL) receives the rank's population sums. */
 int pa_dist_finish(pa_ctx* ctx, const int64_t* T_all, pa_obs* local);
 /* the rank's share of the new population under the plan (and its first global slot); PA_ECAPACITY if it does not fit */
 int pa_dist_new_count(pa_ctx* ctx, const int64_t* T_all, int64_t* count, int64_t* first_global_slot);
-/* drop the step in flight on this rank (another rank failed): nothing was committed */
+/* drop the step in flight on this rank (the plan was refused, or another rank failed): nothing was committed; pa_tau and
+ * pa_counts return PA_EINVAL until the next committed step */
 int pa_dist_abort(pa_ctx* ctx);
 
 /* ---- profiling (PA_PROFILE) --------------------------------------------------------------------------- */

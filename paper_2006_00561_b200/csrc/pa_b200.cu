@@ -921,6 +921,26 @@ int pa_dist_exchange_plan(int32_t world, const int64_t* T, int32_t policy, uint3
   return PA_OK;
 }
 
+int pa_dist_plan_check(int32_t world, const int64_t* new_start, const int64_t* cap) {
+  if (world < 1 || !new_start) return PA_EINVAL;
+  if (new_start[world] >= (1ll << 32) - 4096) return PA_ECAPACITY;  // global slot indices are 32-bit
+  int rc = PA_OK;
+  for (int r = 0; r < world; ++r) {
+    const int64_t n = new_start[r + 1] - new_start[r];
+    if (n < 0) return PA_EINVAL;
+    if (cap && n > cap[r]) return PA_ECAPACITY;  // capacity first: the same answer on every rank whatever the order of the defects
+    if (n == 0) rc = PA_EEXTINCT;
+  }
+  return rc;
+}
+
+int pa_dist_capacity(pa_ctx* c, int64_t* cap) {
+  if (!c || !cap) return PA_EINVAL;
+  if (c->world < 1) return fail(c, PA_EINVAL, "pa_dist_capacity: not a shard");
+  *cap = c->cap;
+  return PA_OK;
+}
+
 int pa_dist_init(const pa_config* cfg, int32_t rank, int32_t world, pa_ctx** out) {
   if (!cfg || !out || world < 1 || rank < 0 || rank >= world || cfg->R0 < world) return PA_EINVAL;
   if (cfg->policy != PA_POLICY_BALANCED && world > BAL_PMAX) return PA_EINVAL;
@@ -1015,6 +1035,11 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
   CK(cudaMemcpyAsync(c->h_state, st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   CK(cudaGetLastError());
+  if (!c->launch_err.empty()) {  // a launch of this phase failed: report it now, not at some later synchronisation
+    const std::string msg = "kernel launch failed: " + c->launch_err;
+    c->launch_err.clear();
+    return fail(c, PA_ECUDA, msg);
+  }
   const DevState& hs = *c->h_state;
   // a rank without offspring is fine here (extinction is a property of the whole population: the plan reports it)
   if (hs.status == ST_CAPACITY) *offspring = -1;
@@ -1054,6 +1079,7 @@ int pa_dist_abort(pa_ctx* c) {
   k_clear_status<<<1, 1, 0, c->stream>>>(c->dev<DevState>(c->lo.state));
   c->launches += 1;
   c->dist_phase = 0;
+  c->attempt_failed = true;  // off / n / tau hold the dropped attempt: pa_tau / pa_counts refuse until the next commit
   return sync_state(c);
 }
 
@@ -1062,8 +1088,16 @@ int pa_dist_finish(pa_ctx* c, const int64_t* T_all, pa_obs* local) {
   if (c->world < 1 || c->dist_phase != 2) return fail(c, PA_EINVAL, "pa_dist_finish: call pa_dist_resample first");
   if (int rc = bind_device(c)) return rc;
   int64_t n = 0, first = 0;
-  if (int rc = pa_dist_new_count(c, T_all, &n, &first)) return rc;
-  if (n < 1) return fail(c, PA_EEXTINCT, "this rank's share of the new population is empty");
+  // Both refusals below are reached only by a caller that skipped pa_dist_plan_check (which refuses them on EVERY rank
+  // before the exchange).  Nothing has been committed: the step stays in flight and pa_dist_abort drops it.
+  if (int rc = pa_dist_new_count(c, T_all, &n, &first)) {
+    c->attempt_failed = true;
+    return rc;
+  }
+  if (n < 1) {
+    c->attempt_failed = true;
+    return fail(c, PA_EEXTINCT, "this rank's share of the new population is empty (pa_dist_plan_check refuses such a plan on all ranks)");
+  }
   DevState* st = c->dev<DevState>(c->lo.state);
   k_clear_status<<<1, 1, 0, c->stream>>>(st);  // a capacity flag of the local expansion cannot be pending here (plan refused it)
   k_dist_set_new<<<1, 1, 0, c->stream>>>(st, (unsigned long long)n, (unsigned)first);
@@ -1072,7 +1106,10 @@ int pa_dist_finish(pa_ctx* c, const int64_t* T_all, pa_obs* local) {
   launch_sweep(c, c->dist_theta, hp.T4, hp.T8, 3);  // theta sweeps in place (theta = 0: E, M only)
   launch_observe(c, c->dev<StepParams>(c->lo.params), 2);
   c->dist_phase = 0;
-  if (int rc = sync_state(c)) return rc;
+  if (int rc = sync_state(c)) {
+    c->attempt_failed = true;
+    return rc;
+  }
   c->attempt_failed = false;
   if (local) return pa_observables(c, local);
   return PA_OK;

@@ -123,7 +123,7 @@ extern "C" {
 int pa_overlap_hist_static(const uint32_t* spins, int32_t L, int64_t R, uint64_t* hist, int hist_on_device, void* stream) {
   t_err[0] = 0;
   if (L > PA_STATIC_MAX_L) {
-    char d[96];
+    char d[128];
     std::snprintf(d, sizeof d, "L = %d needs %lld bins, the built-in scratch array holds %d (L <= %d)", (int)L,
                   (long long)L * L + 1, SOVL_BINS, PA_STATIC_MAX_L);
     return sfail(PA_EINVAL, "lattice too large for the static scratch", d);

@@ -170,14 +170,17 @@ class ShardedAnnealer:
             rows = all_gather_doubles(self.g, [partials[0][0], float(partials[0][1])])
             all_partials = [(r[0], int(r[1])) for r in rows]
         T_local = [s.dist_resample(all_partials) for s in self.shards]
+        caps_local = [s.dist_capacity() for s in self.shards]
         if self.emulated:
-            T_all = T_local
-        else:
-            T_all = [int(r[0]) for r in all_gather_doubles(self.g, [float(T_local[0])])]
-        try:  # every rank evaluates the same plan and the same capacity checks: all ranks fail or none does
+            T_all, caps = T_local, caps_local
+        else:  # the offspring total travels with the rank's capacity: every rank can judge every rank's share
+            rows = all_gather_doubles(self.g, [float(T_local[0]), float(caps_local[0])])
+            T_all, caps = [int(r[0]) for r in rows], [int(r[1]) for r in rows]
+        try:
+            # Every rank evaluates the same plan and the same check of EVERY rank's share (capacity of that rank, empty
+            # share) on the same gathered numbers, before anything is exchanged: all ranks refuse the step or none does.
             ns, base, counts = b.exchange_plan(T_all, self.policy, self.block, self.maxexc)
-            for s in self.shards:
-                s.dist_new_count(T_all)
+            b.plan_check(ns, caps)
         except b.PaError:
             for s in self.shards:
                 s.dist_abort()
@@ -195,7 +198,18 @@ class ShardedAnnealer:
                     s_off += n
         else:
             children, population = self.shards[0].dist_buffers()
+            # The exchange is issued on torch's current stream (the local copy directly, NCCL through req.wait()); the
+            # library works on the shard's own stream.  When the two differ, order them explicitly in both directions:
+            # dist_resample has already synchronised the library stream, dist_finish must not start before the receives.
+            lib_stream, cur = self.shards[0].stream, None
+            if population.is_cuda:
+                import torch
+                cur = torch.cuda.current_stream(population.device)
+                if cur != lib_stream:
+                    cur.wait_stream(lib_stream)
             exchange_slices(self.g, children, population, counts, S)
+            if cur is not None and cur != lib_stream:
+                lib_stream.wait_stream(cur)
         self.last_T, self.last_counts, self.last_new_start = T_all, counts, ns
         return [s.dist_finish(T_all) for s in self.shards]
 

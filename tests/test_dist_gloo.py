@@ -7,6 +7,8 @@ import socket
 import pytest
 import torch.multiprocessing as mp
 
+from main_by_hand import MAIN_BY_HAND
+
 
 def _free_port():
     s = socket.socket()
@@ -96,6 +98,75 @@ def test_exchange_plan_against_the_oracle_policies_and_its_invariants():
     assert ei.value.code == binding.PA_ECAPACITY
 
 
+def test_main_policy_ties_on_the_excess_side_by_hand():
+    """the same hand-worked cases through the oracle's policy function and through the product's host plan: two writings
+    of reading G21, each pinned to the moves written out above rather than to one another"""
+    import numpy as np
+    from oracle import pa_oracle as orc
+    from paper_2006_00561_b200 import binding
+    for born, B, maxexc, want, moves in MAIN_BY_HAND:
+        cnt, mv = orc.policy_counts(np.asarray(born, np.uint32), orc.POLICY_MAIN, B, maxexc)
+        assert cnt.tolist() == want and mv == moves, ("oracle", born)
+        ns, base, counts = binding.exchange_plan(born, binding.PA_POLICY_MAIN, B, maxexc)
+        assert np.diff(ns).tolist() == want, ("plan", born)
+        assert np.diff(base).tolist() == born
+        # children keep their global order: rank dst receives the global range [ns[dst], ns[dst+1]) cut at the sources' ends
+        for src in range(len(born)):
+            for dst in range(len(born)):
+                lo, hi = max(base[src], ns[dst]), min(base[src + 1], ns[dst + 1])
+                assert counts[src, dst] == max(0, hi - lo)
+
+
+def test_exchange_plan_invariants_of_the_main_policy():
+    """what PAPER.md:104-106 fixes without any tie rule: whole blocks move, everyone ends inside the window, nothing is lost"""
+    import numpy as np
+    from paper_2006_00561_b200 import binding
+    rng = np.random.default_rng(21)
+    for world, B, maxexc in [(2, 1024, 1), (8, 1024, 1), (8, 1024, 2), (5, 1, 1), (16, 256, 3), (148, 1024, 1)]:
+        for trial in range(20):
+            T = rng.gamma(2.0, rng.choice([2000, 20480, 90000]) / 2.0, world).astype(np.int64)
+            T[0] += 1
+            ns, base, counts = binding.exchange_plan(T, binding.PA_POLICY_MAIN, B, maxexc)
+            cnt, tot = np.diff(ns), int(T.sum())
+            r = tot // world + (np.arange(world) < tot % world)
+            assert cnt.sum() == tot and np.all(cnt >= 0)
+            assert np.all((cnt - T) % B == 0)                         # blocks of B replicas
+            assert np.all(np.abs(cnt - r) <= maxexc * B)              # the window `maxexc`
+            inside = np.all(np.abs(T - r) <= maxexc * B)
+            assert (not inside) or np.array_equal(cnt, T)             # nobody outside the window: nothing moves
+
+
+def test_plan_check_gives_every_rank_the_same_verdict():
+    """pa_dist_plan_check judges EVERY rank's share against THAT rank's capacity, so the rank that would overflow and the
+    ranks that would not all refuse the step before anything is exchanged (a refusal on one rank only would leave the
+    others waiting in the point-to-point exchange)"""
+    import numpy as np
+    from paper_2006_00561_b200 import binding
+    # policy main moves whole blocks: r = 1000 each, born = (2100, 0, 900), B = 1024: e = (1100,-1000,-100) -> 0->1: (76,24,-100)
+    ns, _, _ = binding.exchange_plan([2100, 0, 900], binding.PA_POLICY_MAIN, 1024, 1)
+    assert np.diff(ns).tolist() == [1076, 1024, 900]
+    binding.plan_check(ns, [1100, 1100, 1100])
+    binding.plan_check(ns, None)
+    with pytest.raises(binding.PaError) as e:
+        binding.plan_check(ns, [1100, 1023, 1100])    # rank 1 alone cannot hold its share: every rank learns that
+    assert e.value.code == binding.PA_ECAPACITY
+    # an empty share (policy none, a rank without offspring; or fewer children than ranks)
+    ns, _, _ = binding.exchange_plan([3000, 0, 500], binding.PA_POLICY_NONE)
+    with pytest.raises(binding.PaError) as e:
+        binding.plan_check(ns, [4096] * 3)
+    assert e.value.code == binding.PA_EEXTINCT
+    ns, _, _ = binding.exchange_plan([1, 0, 1, 0], binding.PA_POLICY_BALANCED)
+    with pytest.raises(binding.PaError) as e:
+        binding.plan_check(ns, None)
+    assert e.value.code == binding.PA_EEXTINCT
+    with pytest.raises(binding.PaError) as e:        # both defects: capacity wins, on every rank alike
+        binding.plan_check(binding.exchange_plan([3000, 0, 500], binding.PA_POLICY_NONE)[0], [100, 100, 100])
+    assert e.value.code == binding.PA_ECAPACITY
+    with pytest.raises(binding.PaError) as e:
+        binding.plan_check([0, 1 << 31, (1 << 32) - 4096], None)   # global slot indices are 32-bit
+    assert e.value.code == binding.PA_ECAPACITY
+
+
 def _sharded_oracle_worker(rank, world, port, q, L, R0, seed, betas, theta, policy, glass_seed=None):
     """one rank of the partitioned run on the CPU: the oracle does the rank's arithmetic with GLOBAL replica indices as
     keys, the product's host plan (pa_dist_exchange_plan) and exchange (dist.exchange_slices over gloo) move the replicas"""
@@ -131,6 +202,7 @@ def _sharded_oracle_worker(rank, world, port, q, L, R0, seed, betas, theta, poli
         children, _, _ = orc.copy_population(L, n, off, spins, E, M, T_loc)
         T_all = [int(r[0]) for r in dist.all_gather_doubles(g, [float(T_loc)])]
         ns, base, counts = binding.exchange_plan(T_all, policy, 16, 1)
+        binding.plan_check(ns, [4 * R0] * world)
         new_n = int(ns[rank + 1] - ns[rank])
         send = torch.from_numpy(children.reshape(-1).view(np.uint8).copy())
         recv = torch.zeros(new_n * wpr * 4, dtype=torch.uint8)

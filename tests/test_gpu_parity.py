@@ -632,6 +632,33 @@ def test_sharded_capacity_failure_is_consistent_and_leaves_the_population_unchan
     assert failures > 0
 
 
+def test_sharded_empty_share_is_refused_by_all_ranks_before_the_exchange():
+    """policy none and one replica or two per rank: sooner or later a rank has no offspring.  A shard cannot be empty, and
+    the refusal must come from the plan check on EVERY rank (same gathered totals) before anything is exchanged or
+    committed -- not from the one empty rank's pa_dist_finish after the others have committed"""
+    b = _binding()
+    from paper_2006_00561_b200 import dist
+    sh = dist.ShardedAnnealer(8, 6, seed=3, policy=b.PA_POLICY_NONE, emulate=2, flags=b.PA_KEEP_COUNTS)
+    refused = committed = 0
+    for k in range(1, 400):  # (a refused step keeps its ordinal, hence its random numbers: the retries mostly fail again)
+        if refused >= 3:
+            break
+        before, Rb, lz, bs = sh.gather_spins(), sh.R_local, sh.log_Z(), [s_.beta_steps() for s_ in sh.shards]
+        try:
+            sh.step(0.002 * k, 1)
+            committed += 1
+            assert len(set(s_.beta_steps() for s_ in sh.shards)) == 1           # same beta and step ordinal on all ranks
+        except b.PaError as e:
+            assert e.code in (b.PA_EEXTINCT, b.PA_ECAPACITY)
+            refused += 1
+            assert sh.R_local == Rb and np.array_equal(sh.gather_spins(), before) and sh.log_Z() == lz
+            assert [s_.beta_steps() for s_ in sh.shards] == bs
+            for s_ in sh.shards:                                                 # the dropped attempt's arrays are not served
+                with pytest.raises(b.PaError):
+                    s_.counts()
+    assert refused > 0 and committed > 0
+
+
 # ---------------------------------------------------------------------------------------------------
 # boundary behaviour
 # ---------------------------------------------------------------------------------------------------

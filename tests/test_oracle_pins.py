@@ -437,6 +437,16 @@ def test_policy_main_by_hand():
     assert cnt.tolist() == [3, 2, 1] and moves == 2  # r=(2,2,2), e=(3,-1,-2): 0->2, (4,1,1) e=(2,-1,-1): 0->1, (3,2,1) e=(1,0,-1): stop
 
 
+def test_policy_main_ties_on_the_excess_side_by_hand():
+    """reading G21 says "ties: lowest index" for the largest excess as well as for the largest shortage (PAPER.md:106
+    defines only excess and shortage): cases where equal excesses share an odd number of moves, so that taking the LAST
+    of the tied partitions instead ends with other counts"""
+    from main_by_hand import MAIN_BY_HAND
+    for born, B, maxexc, want, moves in MAIN_BY_HAND:
+        cnt, mv = orc.policy_counts(born, orc.POLICY_MAIN, B, maxexc)
+        assert cnt.tolist() == want and mv == moves, born
+
+
 @pytest.mark.parametrize("P,B,maxexc", [(8, 1024, 1), (8, 1024, 2), (148, 1024, 1), (5, 1, 1), (16, 256, 3)])
 def test_policy_main_invariants(P, B, maxexc):
     rng = np.random.default_rng(P * 7 + maxexc)
