@@ -26,23 +26,19 @@ if ROOT not in sys.path:
 
 from paper_2006_00561_b200 import inputs  # noqa: E402
 
-# Roofline of the sweep kernel: bound by the integer ALU pipe, 16 lanes/clk/SMSP
-# (B300_MICROARCH.md "alu-pipe ... rt_SMSP=2"; LOP3 measured at 2.02 cycles per warp instruction on B200).
-# Algorithmic ALU lane-operations per flip attempt of the bit-sliced lazy comparator (reading G20), per plane word of
-# 32 sites:  E_BLK Philox blocks x (19 LOP3 of Philox4x32-10 with the loop-invariant first round hoisted + the LOP3 of
-# the comparator) + the neighbour classes and the flip;  E_BLK = 2 + sum_{c>=2} [1 - (1 - 2^-4c)^32] = 2.126 blocks that a
-# (lane, word) pair needs when every site of the word needs a uniform.
-#   round 2 (current algorithm): comparator specialised on the threshold bits = 2 LOP3 per bit = 8 per block; neighbour
-#   classes 7 + flip mask 1 + flip 1 = 9 per word          -> 2.075 per attempt  (`roofline.frac`)
-#   round 1 (the ceiling VERDICT r1 set its target against): generic comparator 3 per bit = 12 per block; 12 per word
-#                                                           -> 2.435 per attempt  (`roofline.frac_r1_ceiling`)
-# The 16 IMAD.WIDE.U32 per Philox block run on the FMA-heavy pipe and are NOT counted here, although a probe on B200
-# shows that they do not overlap with the ALU pipe: a warp's IMAD.WIDE and LOP3 together retire at one
-# per 2 cycles per SMSP (16 IMAD.WIDE + 32 LOP3: 97 cycles; + 48 LOP3: 130).  `roofline.frac_int_datapath_model` counts
-# them (per word E_BLK x (16 + 19 + 8) + 9 at 16 lanes/clk/SMSP): the ceiling this instruction mix can actually reach.
+# Roofline of the sweep kernel: bound by the integer datapath of an SMSP, which retires the
+# kernel's two instruction classes -- LOP3 (ALU pipe) and IMAD.WIDE.U32 (FMA-heavy pipe; Philox's 32 x 32 -> 64 multiplies)
+# -- TOGETHER at one warp instruction per 2 cycles = 16 lanes/clk/SMSP.  Evidence: profiles/r3_pipe_probe_ncu.md (mixes of
+# the two at the sweep kernel's occupancy: 16 IMAD.WIDE + 32 LOP3 take 98 cycles, not 64; under ncu the pipes' active
+# cycles ADD to 98-99 % while smsp__issue_active stays at 49-50 %).
+# Algorithmic lane-operations per flip attempt of the bit-sliced lazy comparator (reading G20), per plane word of 32 sites:
+# E_BLK Philox blocks x (16 IMAD.WIDE + 19 LOP3 of Philox4x32-10 with the loop-invariant first round hoisted + 8 LOP3 of the
+# comparator specialised on the threshold bits, 2 per bit) + 9 per word (neighbour classes 7, flip mask 1, flip 1);
+# E_BLK = 2 + sum_{c>=2} [1 - (1 - 2^-4c)^32] = 2.126 blocks that a (lane, word) pair needs when every site of the word
+# needs a uniform.  -> 3.138 per attempt: `roofline.frac`.  `roofline.frac_alu_pipe_only` leaves the IMAD.WIDE out (2.075 per
+# attempt against the same 16 lanes/clk: what the ALU pipe alone would allow if the multiplies were free -- they are not).
 E_BLK = 2.0 + sum(1.0 - (1.0 - 2.0 ** (-4 * c)) ** 32 for c in range(2, 8))
 ALU_OPS_PER_ATTEMPT = (E_BLK * (19 + 8) + 9) / 32.0
-ALU_OPS_PER_ATTEMPT_R1 = (E_BLK * (19 + 12) + 12) / 32.0
 INT_OPS_PER_ATTEMPT = (E_BLK * (16 + 19 + 8) + 9) / 32.0
 I_MIN_SURVEY = 12.0   # one 32-bit Philox word per attempt at 1 warp-instr/clk/SMSP (kept for continuity)
 SM_COUNT, SMSP, LANES, ALU_LANES = 148, 4, 32, 16
@@ -55,6 +51,9 @@ NCU_CAPTURE_COMMIT = "b3dc885"
 # config 3, one launch of k_sweep<64> = gather + theta sweeps of R' ~ 2^21 replicas (algorithmic S*(U + R') + 8R')
 NCU_TRAFFIC_BYTES = {("k_sweep<64>", 3): 0.652404e9 + 1.032230e9}
 NCU_TRAFFIC_SRC = {"file": "profiles/r2_sweep64_ncu.md", "commit": NCU_SWEEP_CAPTURE_COMMIT}
+# executed lane-instructions per flip attempt (smsp__inst_executed.sum x 32 / attempts of the captured launch): the
+# distance to the 3.138 algorithmic ones is the kernel's overhead (queue, shuffles, moves, branches)
+NCU_LANE_INSTR_PER_ATTEMPT = {("k_sweep<64>", 3): 4.26}
 # a1-a6 chain of config 5: q_reduce (+ level tables) + poisson_scan + copy, read + write
 NCU_RESAMPLE_TRAFFIC_BYTES = 67.15e6 + (67.25e6 + 20.55e6) + (604.61e6 + 2156.73e6)
 NCU_RESAMPLE_TRAFFIC_SRC = {"file": "profiles/r2_resample_ncu.md", "commit": NCU_CAPTURE_COMMIT}
@@ -381,8 +380,8 @@ def glass_leg(binding, torch, wl, peaks, steps=20, warmup=3):
     hq = torch.from_numpy(h.astype("float64"))
     out = {"workload": wl.name + " with a +-J sample (seed %d, %d of %d bonds negative)" % (wl.seed, int((Jx < 0).sum() + (Jy < 0).sum()), 2 * wl.N),
            "steps": steps, "attempts_per_s": attempts / sec, "kernel_attempts_per_s": sweep_rate,
-           "roofline_frac": sweep_rate * ALU_OPS_PER_ATTEMPT / 1e12 / peak,
-           "roofline_frac_r1_ceiling": sweep_rate * ALU_OPS_PER_ATTEMPT_R1 / 1e12 / peak, "ms_per_step": 1e3 * sec / steps,
+           "roofline_frac": sweep_rate * INT_OPS_PER_ATTEMPT / 1e12 / peak,
+           "roofline_frac_alu_pipe_only": sweep_rate * ALU_OPS_PER_ATTEMPT / 1e12 / peak, "ms_per_step": 1e3 * sec / steps,
            "overlap_hist": {"pairs": pairs, "seconds_call": ovl_s, "GBps": pa.R * wl.bytes_per_replica / ovl_s / 1e9,
                             "mean_abs_q": float((hq * q.abs()).sum() / max(pairs, 1)), "mean_q2": float((hq * q * q).sum() / max(pairs, 1))},
            "lnZ": pa.log_Z()["lnZ"], "beta": pa.beta_steps()[0], "mean_E_per_spin": pa.observables()["mean_E"] / wl.N}
@@ -517,23 +516,25 @@ def run_ours(args):
     if wl.theta > 0 and sweep_n > 0:
         attempts_per_launch = units / sweep_n
         sweep_rate = attempts_per_launch / (sweep_ms / sweep_n * 1e-3)  # attempts/s inside the kernel
-        achieved = sweep_rate * ALU_OPS_PER_ATTEMPT / 1e12
+        achieved = sweep_rate * INT_OPS_PER_ATTEMPT / 1e12
         peak = SM_COUNT * SMSP * ALU_LANES * peaks["sm_max_mhz"] * 1e6 / 1e12
+        kkey = ("k_sweep<%d>" % wl.L, args.config)
         roof = {"bound": "alu", "achieved": achieved, "peak": peak,
-                "unit": "T ALU-pipe lane-ops/s (%.3f algorithmic per flip attempt)" % ALU_OPS_PER_ATTEMPT,
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(("k_sweep<%d>" % wl.L, args.config)),
-                "traffic_src": NCU_TRAFFIC_SRC if ("k_sweep<%d>" % wl.L, args.config) in NCU_TRAFFIC_BYTES else None,
+                "unit": "T integer lane-ops/s (%.3f algorithmic per flip attempt: per 32-site word %.3f Philox blocks x "
+                        "(16 IMAD.WIDE + 19 + 8 LOP3) + 9 LOP3)" % (INT_OPS_PER_ATTEMPT, E_BLK),
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(kkey),
+                "traffic_src": NCU_TRAFFIC_SRC if kkey in NCU_TRAFFIC_BYTES else None,
                 "traffic_algorithmic": (2 * wl.bytes_per_replica + 8) * (replica_steps / sweep_n),  # upper bound: U = R'
                 "kernel": "k_sweep<%d>" % wl.L,
                 "kernel_attempts_per_s": sweep_rate, "kernel_ms_per_launch": sweep_ms / sweep_n,
                 "kernel_share_of_step": sweep_ms / step_kernel_ms,
-                "peak_src": "148 SM x 4 SMSP x 16 ALU lanes x %d MHz (clocks.max.sm)" % peaks["sm_max_mhz"],
-                "frac_r1_ceiling": sweep_rate * ALU_OPS_PER_ATTEMPT_R1 / 1e12 / peak,
-                "r1_ceiling_note": "round 1's algorithmic count (%.3f ALU lane-ops per attempt, generic comparator): the ceiling "
-                                   "VERDICT r1's >= 0.60 target was stated against" % ALU_OPS_PER_ATTEMPT_R1,
-                "frac_int_datapath_model": sweep_rate * INT_OPS_PER_ATTEMPT / 1e12 / peak,
-                "int_datapath_note": "IMAD.WIDE counted with the ALU ops (%.3f per attempt): measured on B200, the two do not "
-                                     "overlap (DESIGN.md 8.2 probe)" % INT_OPS_PER_ATTEMPT,
+                "peak_src": "148 SM x 4 SMSP x 16 lanes/clk (LOP3 and IMAD.WIDE.U32 retire together at one warp instruction "
+                            "per 2 cycles per SMSP: profiles/r3_pipe_probe_ncu.md) x %d MHz (clocks.max.sm)" % peaks["sm_max_mhz"],
+                "lane_instr_per_attempt": NCU_LANE_INSTR_PER_ATTEMPT.get(kkey),
+                "lane_instr_src": NCU_TRAFFIC_SRC if kkey in NCU_LANE_INSTR_PER_ATTEMPT else None,
+                "frac_alu_pipe_only": sweep_rate * ALU_OPS_PER_ATTEMPT / 1e12 / peak,
+                "alu_pipe_only_note": "LOP3 only (%.3f per attempt), IMAD.WIDE taken as free: lower than `frac` by construction, "
+                                      "kept because rounds 1-2 reported it" % ALU_OPS_PER_ATTEMPT,
                 "frac_survey_12_instr_per_attempt_at_issue_rate":
                     sweep_rate * I_MIN_SURVEY / (SM_COUNT * SMSP * LANES * peaks["sm_max_mhz"] * 1e6)}
         if clocks.get("sm_mhz"):
