@@ -135,7 +135,8 @@ int pa_init(const pa_config* cfg, pa_ctx** out);
  * and one 264-byte read-back of the device state per call; queue whole schedules with pa_run to avoid both. */
 int pa_step(pa_ctx* ctx, double beta_next, int32_t theta);
 
-/* K steps beta_k = betas[k] (HOST array of K doubles), all launched back to back with ONE synchronisation at the
+/* The asynchronous form of the step that SURVEY.md 8(b) describes (pa_step is its K = 1 case with a synchronisation).
+ * K steps beta_k = betas[k] (HOST array of K doubles), all launched back to back with ONE synchronisation at the
  * end; stops committing at the first failing step (later steps are no-ops) and reports it.  *steps_done (may be
  * NULL) receives the number of committed steps. */
 int pa_run(pa_ctx* ctx, const double* betas, int32_t K, int32_t theta, int32_t* steps_done);

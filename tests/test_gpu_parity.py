@@ -89,8 +89,10 @@ def lockstep(gpu, ora, betas, theta, sweep_slots=None):
         else:
             # a1-a6 on the full population: children are exact copies of their parents, in parent order.
             # Sweeps: hash-selected slots, each swept alone by the oracle (depends only on lattice, slot, seed, step)
+            # plus, always, the edges of the sweep kernels' blocks (16 / 64 replicas per block) and the partly filled last one
             rng = np.random.default_rng(1000 + k)
-            slots = np.unique(rng.integers(0, ora.R, sweep_slots)).astype(np.uint32)
+            edges = [s_ for s_ in (0, 15, 16, 63, 64) if s_ < ora.R] + list(range(max(0, ora.R - 17), ora.R))
+            slots = np.unique(np.concatenate([rng.integers(0, ora.R, sweep_slots), np.asarray(edges, np.int64)])).astype(np.uint32)
             before = ora.spins[slots].copy()
             parent = orc.parent_of(info["n"], info["off"], info["Rnew"])
             assert np.array_equal(before, spins_before[parent[slots]])
@@ -245,6 +247,46 @@ def test_config2_full_size_first_steps():
     gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
     compare_population(gpu, ora, "init")
     lockstep(gpu, ora, [wl.beta(k) for k in range(1, 4)], wl.theta)
+
+
+def test_config2_full_size_whole_schedule_in_three_stretches():
+    """SURVEY.md 8(c) parity protocol, config 2: the FULL population (65 536 replicas: the launch shape of
+    k_sweep_small<32,.,8> that bench.py times) compared after every step of three stretches of its own 200-step schedule --
+    the first 20 steps, 15 steps across beta_c (0.405 -> 0.475), and the last 30 down to beta = 1.0, where nearly every
+    site asks for a uniform and rejects.  Between the stretches the schedule is run with pa_run and the oracle adopts the
+    population (its E, M recomputed and compared).  65 lock-step steps ~ 110 s of oracle time on 16 cores."""
+    wl = inputs.CONFIGS[2]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
+    lockstep(gpu, ora, [wl.beta(k) for k in range(1, 21)], wl.theta)
+    for k_from, k_to in ((80, 95), (170, 200)):
+        done = gpu.beta_steps()[1]
+        assert gpu.run([wl.beta(k) for k in range(done + 1, k_from + 1)], wl.theta) == k_from - done
+        adopt(gpu, ora)
+        lockstep(gpu, ora, [wl.beta(k) for k in range(k_from + 1, k_to + 1)], wl.theta)
+    beta, steps = gpu.beta_steps()
+    assert steps == wl.K == 200 and abs(beta - 1.0) < 1e-12
+    assert gpu.observables()["mean_E"] / wl.N < -1.99           # ordered phase reached
+    assert abs(gpu.log_Z()["lnZ"] / wl.N - inputs_exact_lnz_per_spin(32, 1.0)) < 2e-4
+
+
+def inputs_exact_lnz_per_spin(L, beta):
+    """ln Z / N of the L x L torus from the golden file written by tests/golden/make_ising_exact.py (Kaufman's formula)"""
+    import json
+    data = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "ising_exact.json")))
+    return float(data["lnZ"]["L%d_beta%g" % (L, beta)]) / (L * L)
+
+
+def test_config3_full_population_step_near_beta_c():
+    """SURVEY.md 8(c) parity protocol, config 3: ONE step of its own dbeta = 0.005 schedule with the WHOLE population of
+    2^21 replicas swept by the oracle and compared (spins, E, M, sums) -- step 88 (beta 0.435 -> 0.44, the critical region,
+    where the population fluctuates most): every one of the 131 072 blocks of the k_sweep<64> launch that
+    bench.py times, not a sample of slots.  ~ 215 s of oracle time on 16 cores."""
+    wl = inputs.CONFIGS[3]
+    gpu, ora = make_pair(wl.L, wl.R0, wl.P, wl.seed)
+    assert gpu.run([wl.beta(k) for k in range(1, 88)], wl.theta) == 87
+    adopt(gpu, ora)
+    lockstep(gpu, ora, [wl.beta(88)], wl.theta)
+    assert abs(gpu.beta_steps()[0] - 0.44) < 1e-12
 
 
 def test_config3_full_size_sampled():
