@@ -116,17 +116,31 @@ def exchange_slices(g, send, recv, counts, unit):
     if W == 1:
         return
     import torch.distributed as dist
-    ops = []
+    # gloo moves host memory only: device slices are staged through the host (the slices that cross a rank boundary,
+    # nothing else).  This is the path for several ranks on ONE GPU and for machines without NCCL; with NCCL the device
+    # buffers are handed over as they are.
+    staged = g.backend == "gloo" and send.is_cuda
+    ops, landing = [], []
     for p in range(W):
         if p == me:
             continue
         if counts[me][p]:
-            ops.append(dist.P2POp(dist.isend, send[s_off[p]:s_off[p + 1]], p))
+            out = send[s_off[p]:s_off[p + 1]]
+            ops.append(dist.P2POp(dist.isend, out.cpu() if staged else out, p))
         if counts[p][me]:
-            ops.append(dist.P2POp(dist.irecv, recv[r_off[p]:r_off[p + 1]], p))
+            dst = recv[r_off[p]:r_off[p + 1]]
+            if staged:
+                import torch
+                host = torch.empty(dst.shape, dtype=dst.dtype, device="cpu")
+                landing.append((dst, host))
+                ops.append(dist.P2POp(dist.irecv, host, p))
+            else:
+                ops.append(dist.P2POp(dist.irecv, dst, p))
     if ops:
         for req in dist.batch_isend_irecv(ops):
             req.wait()
+    for dst, host in landing:
+        dst.copy_(host)
 
 
 class ShardedAnnealer:

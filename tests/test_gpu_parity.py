@@ -658,6 +658,62 @@ def test_sharded_driver_with_one_rank_equals_the_single_context():
         assert rel(sh.log_Z()["lnZ"], single.log_Z()["lnZ"]) <= RTOL  # Q's rounding depends on the reduction grid (capacity)
 
 
+def _two_process_rank(rank, world, port, q, L, R0, seed, betas, theta, policy):
+    """one REAL rank of the multi-process driver: its own process, its own CUDA context on cuda:0, torch.distributed over
+    gloo with host-staged slices.  Kernels of different ranks never wait on one another (the ranks meet on the host)."""
+    os.environ.update({"RANK": str(rank), "WORLD_SIZE": str(world), "LOCAL_RANK": "0",
+                       "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    import torch
+    from paper_2006_00561_b200 import dist
+    g = dist.init_from_env(backend="gloo", device_kind="cuda")
+    sh = dist.ShardedAnnealer(L, R0, seed=seed, policy=policy, block=64, maxexc=1, group=g)
+    Rs = []
+    for beta in betas:
+        sh.step(beta, theta)
+        Rs.append(sh.R_local[0])
+    torch.cuda.synchronize()
+    q.put((rank, sh.shards[0].spins(), sh.shards[0].energies()[0], sh.log_Z()["lnZ"], Rs, int(sh.last_new_start[rank])))
+    dist.barrier(g)
+    dist.shutdown(g)
+
+
+@pytest.mark.parametrize("world,policy", [(2, 0), (3, 1)])
+def test_sharded_real_processes_on_one_gpu_equal_the_single_context(world, policy):
+    """the multi-process driver path (dist.init_from_env, all_gather_doubles, exchange_slices, ShardedAnnealer(group=...))
+    executed with world > 1: `world` spawned processes share cuda:0, exchange over gloo; the concatenation of their
+    populations equals the single-context run bit for bit, step counts and ln Z agree on every rank"""
+    import socket
+    import torch.multiprocessing as mp
+    b = _binding()
+    L, R0, seed, theta = 32, 3000, 31, 2
+    betas = [0.08 * k for k in range(1, 7)]
+    s_ = socket.socket()
+    s_.bind(("127.0.0.1", 0))
+    port = s_.getsockname()[1]
+    s_.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_two_process_rank, args=(r, world, port, q, L, R0, seed, betas, theta, policy)) for r in range(world)]
+    for p_ in procs:
+        p_.start()
+    res = sorted((q.get(timeout=300) for _ in procs), key=lambda t: t[0])
+    for p_ in procs:
+        p_.join(timeout=120)
+        assert p_.exitcode == 0
+    single = b.PopulationAnnealer(L, R0, P=1, seed=seed)
+    Rs = []
+    for beta in betas:
+        single.step(beta, theta)
+        Rs.append(single.R)
+    assert np.array_equal(np.concatenate([r[1] for r in res], axis=0), single.spins())
+    assert np.array_equal(np.concatenate([r[2] for r in res]), single.energies()[0])
+    assert [sum(r[4][k] for r in res) for k in range(len(betas))] == Rs
+    starts = [r[5] for r in res]
+    assert starts[0] == 0 and starts == sorted(starts)
+    for r in res:
+        assert rel(r[3], single.log_Z()["lnZ"]) <= RTOL
+
+
 def test_sharded_capacity_failure_is_consistent_and_leaves_the_population_unchanged():
     b = _binding()
     from paper_2006_00561_b200 import dist
