@@ -240,8 +240,10 @@ const char* pa_static_last_error(void);
  *                                                                           -> all-gather of the offspring totals T_r
  *   pa_dist_exchange_plan  (pure host function) global child offsets, new partition table under cfg.policy with
  *                     born_p = T_p (the paper's per-node offspring count), and the slice every rank sends to every other
+ *   pa_dist_plan_check     (pure host function) every rank's share fits / is not empty, judged alike on every rank
+ *   pa_dist_pack      theta > 0: gather the children that leave the rank into the send buffer
  *                                                                           -> all-to-all-v of lattices (contiguous slices)
- *   pa_dist_finish    theta sweeps of the new local population in place, E, M, local sums, commit
+ *   pa_dist_finish    theta sweeps of the new local population (theta > 0: gathered by the sweep's load), E, M, sums, commit
  *
  * Because global child order is source-rank order, the slices a rank receives are contiguous in its new buffer in source
  * order: the all-to-all-v writes straight into the population buffer (pa_dist_buffers), nothing is unpacked. */
@@ -270,12 +272,25 @@ int pa_dist_exchange_plan(int32_t world, const int64_t* T, int32_t policy, uint3
  * replicas above its balanced count) or the population outgrows 32-bit slot indices; PA_EEXTINCT if some rank's new share
  * is empty (policy none with a rank without offspring, or fewer children than ranks): a shard cannot be empty.  Every
  * rank evaluates this on the same gathered numbers BEFORE the exchange, so all ranks refuse the step or none does;
- * after a refusal every rank calls pa_dist_abort. */
-int pa_dist_plan_check(int32_t world, const int64_t* new_start, const int64_t* cap);
+ * after a refusal every rank calls pa_dist_abort.  base (as written by the plan) and R_cur (the ranks' current populations,
+ * known from the first all-gather) are given for a step with theta > 0 (both NULL for theta = 0): such a step lands what a
+ * rank receives behind its parents, so R_cur[r] + (new share - children that stay) must fit cap[r] too. */
+int pa_dist_plan_check(int32_t world, const int64_t* new_start, const int64_t* cap, const int64_t* base, const int64_t* R_cur);
 /* slots per buffer of this rank (cfg.capacity as resolved by pa_dist_init) */
 int pa_dist_capacity(pa_ctx* ctx, int64_t* cap);
-/* DEVICE pointers of the step in flight: children = the rank's offspring in child order (send side), population = where
- * the rank's new population must be written (receive side); valid between pa_dist_resample and pa_dist_finish. */
+/* Between the plan and the exchange.  theta > 0 (the lean step): nothing was expanded by pa_dist_resample; the rank's own
+ * children that stay on the rank are gathered straight from their parents by the sweep's load in pa_dist_finish (as in
+ * the one-GPU step), and this call gathers ONLY the children that leave the rank (a prefix for lower ranks, a suffix for
+ * higher ranks; a few per cent near beta_c) into the send buffer, in destination order, and writes the gather map of the
+ * new population.  *self_in_exchange = 0: the rank's own share is NOT part of the send and receive buffers.
+ * theta = 0: no-op, *self_in_exchange = 1 (pa_dist_resample has expanded all offspring; the own share is copied by the
+ * caller like any other slice).  The two small kernels are ENQUEUED on cfg.stream, not waited for: an exchange issued on
+ * another stream (or by another library) must be ordered after cfg.stream by the caller (stream wait, event, or a
+ * synchronisation).  PA_ECAPACITY if the plan does not fit (pa_dist_plan_check says so on every rank beforehand). */
+int pa_dist_pack(pa_ctx* ctx, const int64_t* T_all, int32_t* self_in_exchange);
+/* DEVICE pointers of the step in flight, valid between pa_dist_pack and pa_dist_finish: children = send side (slices in
+ * destination order), population = receive side (slices in source order).  theta = 0: all offspring in child order / the
+ * whole new population.  theta > 0: only what leaves the rank / only what arrives (own share absent on both sides). */
 int pa_dist_buffers(pa_ctx* ctx, void** children, void** population);
 /* T_all as given to the plan.  PA_ECAPACITY / PA_EEXTINCT if the rank's new share exceeds its capacity / is empty: check
  * BEFORE exchanging, on every rank for every rank, with pa_dist_plan_check -- a refusal here comes after the other ranks

@@ -19,7 +19,7 @@ KERNELS = ["levels_w", "q_reduce", "levels_tau", "poisson_scan", "balance", "cop
 EXPORTS = ["pa_workspace_bytes", "pa_init", "pa_step", "pa_run", "pa_adaptive_beta", "pa_population", "pa_beta", "pa_totals", "pa_energies", "pa_log_Z",
            "pa_observables", "pa_spins", "pa_tau", "pa_counts", "pa_parents", "pa_partitions", "pa_thresholds",
            "pa_set_spins", "pa_debug_set_thresholds", "pa_set_bonds", "pa_overlap_hist", "pa_overlap_hist_static", "pa_static_last_error", "pa_dist_init", "pa_dist_workspace_bytes", "pa_dist_begin",
-           "pa_dist_resample", "pa_dist_exchange_plan", "pa_dist_plan_check", "pa_dist_capacity", "pa_dist_buffers", "pa_dist_finish", "pa_dist_new_count",
+           "pa_dist_resample", "pa_dist_exchange_plan", "pa_dist_plan_check", "pa_dist_capacity", "pa_dist_pack", "pa_dist_buffers", "pa_dist_finish", "pa_dist_new_count",
            "pa_dist_abort", "pa_profile_read", "pa_launch_count", "pa_last_error", "pa_destroy"]
 
 
@@ -89,7 +89,8 @@ def load_library():
         "pa_dist_begin": (C.c_int, [vp, C.c_double, C.c_int32, C.POINTER(PaDistPartial)]),
         "pa_dist_resample": (C.c_int, [vp, C.POINTER(PaDistPartial), i64p]),
         "pa_dist_exchange_plan": (C.c_int, [C.c_int32, i64p, C.c_int32, C.c_uint32, C.c_uint32, i64p, i64p, i64p]),
-        "pa_dist_plan_check": (C.c_int, [C.c_int32, i64p, i64p]),
+        "pa_dist_plan_check": (C.c_int, [C.c_int32, i64p, i64p, i64p, i64p]),
+        "pa_dist_pack": (C.c_int, [vp, i64p, i32p]),
         "pa_dist_capacity": (C.c_int, [vp, i64p]),
         "pa_dist_buffers": (C.c_int, [vp, C.POINTER(vp), C.POINTER(vp)]),
         "pa_dist_finish": (C.c_int, [vp, i64p, C.POINTER(PaObs)]),
@@ -157,19 +158,23 @@ def overlap_hist_static(spins, L, R=None, out=None, stream=None):
     return h
 
 
-def plan_check(new_start, caps=None):
+def plan_check(new_start, caps=None, base=None, R_cur=None):
     """pa_dist_plan_check (pure host function): raises PaError(PA_ECAPACITY) if some rank's new share exceeds that rank's
-    capacity, PaError(PA_EEXTINCT) if some rank's new share is empty.  Same verdict on every rank (same inputs)."""
+    capacity, PaError(PA_EEXTINCT) if some rank's new share is empty.  Same verdict on every rank (same inputs).  base
+    (from exchange_plan) and R_cur (current populations in rank order): the step has theta > 0 and lands what a rank
+    receives behind its parents."""
     lib = load_library()
     ns = np.ascontiguousarray(new_start, np.int64)
     W = ns.shape[0] - 1
-    p64 = lambda a: a.ctypes.data_as(C.POINTER(C.c_int64))
-    cp = None
-    if caps is not None:
-        cp = np.ascontiguousarray(caps, np.int64)
-        if cp.shape[0] != W:
-            raise PaError(PA_EINVAL, "plan_check: one capacity per rank")
-    rc = lib.pa_dist_plan_check(W, p64(ns), p64(cp) if cp is not None else None)
+    p64 = lambda a: a.ctypes.data_as(C.POINTER(C.c_int64)) if a is not None else None
+    arrs = []
+    for a, n in ((caps, W), (base, W + 1), (R_cur, W)):
+        if a is not None:
+            a = np.ascontiguousarray(a, np.int64)
+            if a.shape[0] != n:
+                raise PaError(PA_EINVAL, "plan_check: array length does not match the number of ranks")
+        arrs.append(a)
+    rc = lib.pa_dist_plan_check(W, p64(ns), p64(arrs[0]), p64(arrs[1]), p64(arrs[2]))
     if rc != PA_OK:
         raise PaError(rc, {PA_ECAPACITY: "a rank's share of the new population exceeds its capacity",
                            PA_EEXTINCT: "a rank's share of the new population is empty"}.get(rc, "bad plan"))
@@ -394,6 +399,13 @@ class PopulationAnnealer:
         r = C.c_int64(0)
         self._check(self._lib.pa_dist_capacity(self._ctx, C.byref(r)))
         return int(r.value)
+
+    def dist_pack(self, T_all):
+        """pa_dist_pack; returns True when the rank's own share travels through the exchange buffers (theta = 0)"""
+        t = np.ascontiguousarray(T_all, np.int64)
+        f = C.c_int32(1)
+        self._check(self._lib.pa_dist_pack(self._ctx, t.ctypes.data_as(C.POINTER(C.c_int64)), C.byref(f)))
+        return bool(f.value)
 
     def dist_buffers(self):
         """(children, population) as uint8 views of the workspace tensor: send side / receive side of the exchange"""

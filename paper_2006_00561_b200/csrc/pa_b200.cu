@@ -8,6 +8,7 @@
 #include <new>
 #include <optional>
 #include <string>
+#include <algorithm>
 #include <vector>
 
 #include "pa_common.cuh"
@@ -28,7 +29,7 @@ constexpr int OBS_GRID = 148 * 4;
 
 struct Layout {
   uint64_t state, params, spins[2], EM[2], off, n, tau, tile_desc, tile_parent, parent_of, red_partial, obs_partial,
-      lev_tau, lev_mu, lev_m, lev_cdf, lev_hist, part[2], part_stats, bond_mask, ovl_hist, sys_tiles, total;
+      lev_tau, lev_mu, lev_m, lev_cdf, lev_hist, part[2], part_stats, bond_mask, ovl_hist, sys_tiles, dist_map, total;
 };
 
 inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
@@ -60,7 +61,7 @@ int64_t default_capacity(int64_t R0) {
   return (R0 + slack + 1023) / 1024 * 1024;
 }
 
-bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
+bool make_layout(const pa_config* c, int64_t cap, Layout* lo, bool shard = false) {
   if (!c || !valid_L(c->L) || c->P < 1 || c->R0 < 1 || c->R0 >= (1ll << 31) || cap < c->R0 || cap >= (1ll << 32) - 4096)
     return false;
   if (c->policy > PA_POLICY_NONE || (c->policy != PA_POLICY_BALANCED && c->P > BAL_PMAX)) return false;
@@ -94,6 +95,9 @@ bool make_layout(const pa_config* c, int64_t cap, Layout* lo) {
   lo->bond_mask = take(N / 2);        // +-J model: negative-bond masks, 2 colours x N/64 plane words x 4 bonds (pa_sweep.cuh)
   lo->ovl_hist = take(nlev * 8);      // overlap histogram (pa_overlap_hist)
   lo->sys_tiles = take(((ucap + SCAN_TILE - 1) / SCAN_TILE + 1) * 8);  // systematic resampling: tile sums / prefixes of Lam
+  // a multi-GPU shard: the scan's child -> parent map of the rank's own offspring (parent_of then holds the map of the NEW
+  // local population: own children + received lattices)
+  lo->dist_map = shard ? take(ucap * 4) : 0;
   lo->total = o;
   return true;
 }
@@ -129,6 +133,10 @@ struct pa_ctx {
   int64_t g_R0;             // target population of the WHOLE run (= cfg.R0 unless this is a shard)
   int dist_phase;           // 0 idle, 1 after pa_dist_begin, 2 after pa_dist_resample
   int dist_theta;
+  bool dist_lean;           // theta > 0: own children are gathered by the sweep's load, only crossing slices are packed
+  int64_t dist_T;           // the rank's offspring of the step in flight
+  int64_t dist_recv;        // lattices the rank receives (landed behind its parents in the current buffer)
+  bool dist_packed;
   double dist_beta_next;
   bool dbg_thresholds;  // test hook: pa_debug_set_thresholds
   uint32_t dbg_T4, dbg_T8;
@@ -282,13 +290,16 @@ void launch_copy(pa_ctx* c) {
 }
 
 // mode 0: sums of the new population, a5 (partition table + diagnostics) and the commit of the step; mode 1: sums only
-void launch_observe(pa_ctx* c, const StepParams* sp, int mode) {
+void launch_observe(pa_ctx* c, const StepParams* sp, int mode, bool shard_table = false) {
   Prof p(c, PA_K_OBSERVE);
   launch(c, "k_observe", k_observe, c->obs_grid, OBS_THREADS, c->dev<DevState>(c->lo.state), sp, c->dev<int32_t>(c->lo.EM[0]),
          c->dev<int32_t>(c->lo.EM[1]),
          c->dev<unsigned long long>(c->lo.obs_partial), mode, c->N, c->dev<uint32_t>(c->lo.off),
          c->dev<uint32_t>(c->lo.part[0]), c->dev<uint32_t>(c->lo.part[1]), c->dev<uint32_t>(c->lo.part_stats),
-         BalanceArgs{c->cfg.P, (int)c->cfg.policy, c->cfg.block ? c->cfg.block : 1024u, c->cfg.maxexc ? c->cfg.maxexc : 1u});
+         // a shard keeps ONE local partition (cfg.policy acts between the ranks, on the host): its table is [0, R'] and
+         // the offsets of the rank's own offspring do not add up to R', so the block-moving policies must not run on it
+         shard_table ? BalanceArgs{1, PA_POLICY_BALANCED, 1024u, 1u}
+                     : BalanceArgs{c->cfg.P, (int)c->cfg.policy, c->cfg.block ? c->cfg.block : 1024u, c->cfg.maxexc ? c->cfg.maxexc : 1u});
 }
 
 // persistent grid of k_poisson_scan: blocks per SM (occupancy of the variant) x SMs
@@ -408,6 +419,38 @@ __global__ void k_dist_set_new(DevState* st, unsigned long long count, unsigned 
   st->Rnew = count;
   st->slot0_new = slot0_new;
 }
+// Lean shard step (theta > 0).  The rank's T offspring are children j = 0..T-1 in child order with parents map[j].  Of
+// these, [a, b) stay on the rank; [0, a) go to lower ranks and [b, T) to higher ranks: k_dist_pack gathers exactly those
+// into the spare buffer in child order (= destination order), the send side of the exchange.
+__global__ void __launch_bounds__(256)
+k_dist_pack(const DevState* __restrict__ st, uint32_t* spins0, uint32_t* spins1, const uint32_t* __restrict__ map,
+            const unsigned long long a, const unsigned long long b, const unsigned long long T, const int wrep) {
+  const uint32_t* __restrict__ src = st->cur ? spins1 : spins0;
+  uint32_t* __restrict__ dst = st->cur ? spins0 : spins1;
+  const unsigned long long words = (a + (T - b)) * (unsigned long long)wrep;
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < words; i += stride) {
+    const unsigned long long k = i / (unsigned)wrep, w = i % (unsigned)wrep;
+    const unsigned long long j = k < a ? k : b + (k - a);
+    dst[i] = src[(unsigned long long)map[j] * wrep + w];
+  }
+}
+// ... and the gather map of the rank's NEW population for the sweep's load (mode 2), which reads the CURRENT buffer:
+// slots [0, n_lo) came from lower ranks and were landed behind the R parents, slots [n_lo, n_lo + b - a) are the rank's own
+// children (parents map[a ..]), the rest came from higher ranks.
+__global__ void __launch_bounds__(256)
+k_dist_compose(const uint32_t* __restrict__ map, uint32_t* __restrict__ parent_of, const unsigned long long n_new,
+               const unsigned long long n_lo, const unsigned long long n_stay, const unsigned long long a,
+               const unsigned long long R_old) {
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_new; i += stride) {
+    uint32_t v;
+    if (i < n_lo) v = (uint32_t)(R_old + i);
+    else if (i < n_lo + n_stay) v = map[a + (i - n_lo)];
+    else v = (uint32_t)(R_old + n_lo + (i - n_lo - n_stay));
+    parent_of[i] = v;
+  }
+}
 __global__ void k_set_e_off(DevState* st, int e_off) {
   st->e_off = e_off;
   st->obs_done = 0u;  // the population sums are taken again (k_observe's last-block counter)
@@ -515,7 +558,7 @@ int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t
   if (!c) return PA_ENOMEM;
   c->cfg = *cfg;
   c->cap = cfg->capacity > 0 ? cfg->capacity : (cfg->R0 >= 1 ? default_capacity(cfg->R0) : 0);
-  if (!make_layout(cfg, c->cap, &c->lo) || !(cfg->beta0 == cfg->beta0)) {
+  if (!make_layout(cfg, c->cap, &c->lo, world > 0) || !(cfg->beta0 == cfg->beta0)) {
     delete c;
     return PA_EINVAL;
   }
@@ -542,6 +585,10 @@ int init_common(const pa_config* cfg, pa_ctx** out, int rank, int world, int64_t
   c->rank = 0;
   c->world = 0;
   c->dist_phase = 0;
+  c->dist_lean = false;
+  c->dist_packed = false;
+  c->dist_T = 0;
+  c->dist_recv = 0;
   c->dbg_thresholds = false;
   c->dbg_T4 = c->dbg_T8 = 0u;
   c->scan_grid_max[0] = c->scan_grid_max[1] = 0;
@@ -921,14 +968,20 @@ int pa_dist_exchange_plan(int32_t world, const int64_t* T, int32_t policy, uint3
   return PA_OK;
 }
 
-int pa_dist_plan_check(int32_t world, const int64_t* new_start, const int64_t* cap) {
-  if (world < 1 || !new_start) return PA_EINVAL;
+int pa_dist_plan_check(int32_t world, const int64_t* new_start, const int64_t* cap, const int64_t* base, const int64_t* R_cur) {
+  if (world < 1 || !new_start || ((base == nullptr) != (R_cur == nullptr))) return PA_EINVAL;
   if (new_start[world] >= (1ll << 32) - 4096) return PA_ECAPACITY;  // global slot indices are 32-bit
   int rc = PA_OK;
   for (int r = 0; r < world; ++r) {
     const int64_t n = new_start[r + 1] - new_start[r];
     if (n < 0) return PA_EINVAL;
     if (cap && n > cap[r]) return PA_ECAPACITY;  // capacity first: the same answer on every rank whatever the order of the defects
+    if (cap && base) {  // theta > 0: what a rank receives is landed behind its R_cur parents in the current buffer
+      const int64_t lo = base[r] > new_start[r] ? base[r] : new_start[r];
+      const int64_t hi = base[r + 1] < new_start[r + 1] ? base[r + 1] : new_start[r + 1];
+      const int64_t stay = hi > lo ? hi - lo : 0;
+      if (R_cur[r] + (n - stay) > cap[r]) return PA_ECAPACITY;
+    }
     if (n == 0) rc = PA_EEXTINCT;
   }
   return rc;
@@ -967,7 +1020,9 @@ uint64_t pa_dist_workspace_bytes(const pa_config* cfg, int32_t world) {
   local.P = 1;
   local.policy = PA_POLICY_BALANCED;
   if (local.capacity == 0) local.capacity = (2 * ((cfg->R0 + world - 1) / world) + 4096 + 1023) / 1024 * 1024;
-  return pa_workspace_bytes(&local);
+  Layout lo;
+  if (!make_layout(&local, local.capacity, &lo, true)) return 0;
+  return lo.total;
 }
 
 int pa_dist_begin(pa_ctx* c, double beta_next, int32_t theta, pa_dist_partial* mine) {
@@ -1027,11 +1082,16 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
     out.tile_parent = c->dev<uint32_t>(c->lo.tile_parent);
     const int shift = copy_shift_for(c->cfg.L);
     const unsigned long long cap = (unsigned long long)c->cap;
-    const unsigned grid = scan_grid(c, false);
+    c->dist_lean = c->dist_theta > 0;
+    c->dist_packed = false;
+    if (c->dist_lean) out.parent_of = c->dev<uint32_t>(c->lo.dist_map);  // child -> parent map of the rank's own offspring
+    const unsigned grid = scan_grid(c, c->dist_lean);
     Prof p(c, PA_K_POISSON_SCAN);
-    launch_scan(c, keep, false, grid, st, E0, E1, tb, out, shift, cap);
+    launch_scan(c, keep, c->dist_lean, grid, st, E0, E1, tb, out, shift, cap);
   }
-  launch_copy(c);  // the rank's offspring, expanded in child order, into the spare buffer: the send side of the exchange
+  // theta = 0: the rank's offspring, expanded in child order, into the spare buffer: the send side of the exchange.
+  // theta > 0: nothing is expanded here; pa_dist_pack gathers only the slices that leave the rank, the sweep's load the rest.
+  if (!c->dist_lean) launch_copy(c);
   CK(cudaMemcpyAsync(c->h_state, st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   CK(cudaGetLastError());
@@ -1044,7 +1104,44 @@ int pa_dist_resample(pa_ctx* c, const pa_dist_partial* all, int64_t* offspring) 
   // a rank without offspring is fine here (extinction is a property of the whole population: the plan reports it)
   if (hs.status == ST_CAPACITY) *offspring = -1;
   else *offspring = (int64_t)hs.Rnew;
+  c->dist_T = (int64_t)hs.Rnew;
   c->dist_phase = 2;
+  return PA_OK;
+}
+
+int pa_dist_pack(pa_ctx* c, const int64_t* T_all, int32_t* self_in_exchange) {
+  if (!c || !T_all) return PA_EINVAL;
+  if (c->world < 1 || c->dist_phase != 2) return fail(c, PA_EINVAL, "pa_dist_pack: call pa_dist_resample first");
+  if (self_in_exchange) *self_in_exchange = c->dist_lean ? 0 : 1;
+  if (!c->dist_lean) return PA_OK;  // theta = 0: pa_dist_resample has expanded everything, own share included
+  if (int rc = bind_device(c)) return rc;
+  const int W = c->world, me = c->rank;
+  std::vector<int64_t> ns(W + 1), base(W + 1), counts((size_t)W * W);
+  const int rc = pa_dist_exchange_plan(W, T_all, (int)c->cfg.policy, c->cfg.block, c->cfg.maxexc, ns.data(), base.data(), counts.data());
+  if (rc != PA_OK) return fail(c, rc, rc == PA_EEXTINCT ? "population extinct (sum of offspring = 0)" : "a rank's offspring exceed its capacity");
+  const int64_t T = base[me + 1] - base[me], n_new = ns[me + 1] - ns[me];
+  if (T != c->dist_T) return fail(c, PA_EINVAL, "pa_dist_pack: T_all[rank] is not this rank's offspring total");
+  auto clamp = [](int64_t x, int64_t lo, int64_t hi) { return x < lo ? lo : (x > hi ? hi : x); };
+  const int64_t a = clamp(ns[me] - base[me], 0, T), b = clamp(ns[me + 1] - base[me], a, T);  // [a, b) stay
+  const int64_t n_lo = clamp(base[me] - ns[me], 0, n_new), n_stay = b - a, n_recv = n_new - n_stay;
+  if (n_new > c->cap || c->R + n_recv > c->cap)
+    return fail(c, PA_ECAPACITY, "the rank's new share, or its parents plus what it receives, exceed its capacity (pa_dist_plan_check refuses this on all ranks)");
+  const int64_t n_out = a + (T - b);
+  if (n_out > 0) {
+    const uint64_t words = (uint64_t)n_out * c->wrep;
+    const unsigned grid = (unsigned)std::min<uint64_t>((words + 255) / 256, 148 * 16);
+    launch(c, "k_dist_pack", k_dist_pack, grid, 256u, (const DevState*)c->dev<DevState>(c->lo.state), c->dev<uint32_t>(c->lo.spins[0]),
+           c->dev<uint32_t>(c->lo.spins[1]), (const uint32_t*)c->dev<uint32_t>(c->lo.dist_map), (unsigned long long)a,
+           (unsigned long long)b, (unsigned long long)T, c->wrep);
+  }
+  {
+    const unsigned grid = (unsigned)std::min<uint64_t>(((uint64_t)n_new + 255) / 256, 148 * 8);
+    launch(c, "k_dist_compose", k_dist_compose, grid ? grid : 1u, 256u, (const uint32_t*)c->dev<uint32_t>(c->lo.dist_map), c->dev<uint32_t>(c->lo.parent_of),
+           (unsigned long long)n_new, (unsigned long long)n_lo, (unsigned long long)n_stay, (unsigned long long)a, (unsigned long long)c->R);
+  }
+  CK(cudaGetLastError());  // enqueued, not synchronised: the caller orders its exchange after cfg.stream
+  c->dist_recv = n_recv;
+  c->dist_packed = true;
   return PA_OK;
 }
 
@@ -1052,8 +1149,10 @@ int pa_dist_buffers(pa_ctx* c, void** children, void** population) {
   if (!c) return PA_EINVAL;
   if (c->world < 1 || c->dist_phase != 2) return fail(c, PA_EINVAL, "pa_dist_buffers: no step in flight");
   const unsigned cur = c->h_state->cur;
+  if (c->dist_lean && !c->dist_packed) return fail(c, PA_EINVAL, "pa_dist_buffers: call pa_dist_pack first (theta > 0)");
   if (children) *children = c->dev<char>(c->lo.spins[cur ^ 1u]);
-  if (population) *population = c->dev<char>(c->lo.spins[cur]);
+  // theta = 0: the new population replaces the parents; theta > 0: what arrives is landed behind the R parents
+  if (population) *population = c->dev<char>(c->lo.spins[cur]) + (c->dist_lean ? (size_t)c->R * (size_t)(c->N / 8) : 0);
   return PA_OK;
 }
 
@@ -1103,8 +1202,19 @@ int pa_dist_finish(pa_ctx* c, const int64_t* T_all, pa_obs* local) {
   k_dist_set_new<<<1, 1, 0, c->stream>>>(st, (unsigned long long)n, (unsigned)first);
   c->launches += 2;
   const StepParams& hp = c->h_params[0];
-  launch_sweep(c, c->dist_theta, hp.T4, hp.T8, 3);  // theta sweeps in place (theta = 0: E, M only)
-  launch_observe(c, c->dev<StepParams>(c->lo.params), 2);
+  if (c->dist_lean) {
+    if (!c->dist_packed) {
+      c->attempt_failed = true;
+      return fail(c, PA_EINVAL, "pa_dist_finish: pa_dist_pack was not called for this step (theta > 0)");
+    }
+    // the sweep's load gathers the new population from the current buffer (own children from their parents, received
+    // lattices from behind the parents) into the spare one, as in the one-GPU step; the commit flips the buffers
+    launch_sweep(c, c->dist_theta, hp.T4, hp.T8, 2);
+    launch_observe(c, c->dev<StepParams>(c->lo.params), 0, true);
+  } else {
+    launch_sweep(c, c->dist_theta, hp.T4, hp.T8, 3);  // in place: E, M only
+    launch_observe(c, c->dev<StepParams>(c->lo.params), 2);
+  }
   c->dist_phase = 0;
   if (int rc = sync_state(c)) {
     c->attempt_failed = true;

@@ -100,18 +100,20 @@ def all_gather_doubles(g, values):
     return [[float(x) for x in t.tolist()] for t in out]
 
 
-def exchange_slices(g, send, recv, counts, unit):
+def exchange_slices(g, send, recv, counts, unit, with_self=True):
     """all-to-all-v of contiguous slices.  send / recv: 1-D tensors (uint8 bytes or int32 words) on this rank; counts[src][dst]
     = items src sends to dst; one item = `unit` tensor elements.  Rank r's slices leave `send` in destination order and
     arrive in `recv` in source order (global child order is source-rank order, so `recv` ends up in global order).
-    Point-to-point operations in one batch: the same code runs on NCCL (one group call) and on gloo."""
+    Point-to-point operations in one batch: the same code runs on NCCL (one group call) and on gloo.
+    with_self = False (a step with theta > 0 after pa_dist_pack): counts[me][me] items are skipped on both sides."""
     me, W = g.rank, g.world
     s_off = [0] * (W + 1)
     r_off = [0] * (W + 1)
-    for p in range(W):
-        s_off[p + 1] = s_off[p] + int(counts[me][p]) * unit
-        r_off[p + 1] = r_off[p] + int(counts[p][me]) * unit
-    if counts[me][me]:
+    for p in range(W):  # with_self = False: the rank's own share is in neither buffer (the sweep's load gathers it)
+        own = p == me and not with_self
+        s_off[p + 1] = s_off[p] + (0 if own else int(counts[me][p]) * unit)
+        r_off[p + 1] = r_off[p] + (0 if own else int(counts[p][me]) * unit)
+    if counts[me][me] and with_self:
         recv[r_off[me]:r_off[me + 1]].copy_(send[s_off[me]:s_off[me + 1]])
     if W == 1:
         return
@@ -190,11 +192,18 @@ class ShardedAnnealer:
         else:  # the offspring total travels with the rank's capacity: every rank can judge every rank's share
             rows = all_gather_doubles(self.g, [float(T_local[0]), float(caps_local[0])])
             T_all, caps = [int(r[0]) for r in rows], [int(r[1]) for r in rows]
+        R_all = [int(p[1]) for p in all_partials]
         try:
             # Every rank evaluates the same plan and the same check of EVERY rank's share (capacity of that rank, empty
             # share) on the same gathered numbers, before anything is exchanged: all ranks refuse the step or none does.
             ns, base, counts = b.exchange_plan(T_all, self.policy, self.block, self.maxexc)
-            b.plan_check(ns, caps)
+            if theta > 0:
+                b.plan_check(ns, caps, base, R_all)
+            else:
+                b.plan_check(ns, caps)
+            # theta > 0: only the children that leave a rank are gathered into its send buffer; the rest of the new
+            # population is gathered from the parents by the sweep's load in dist_finish, as in the one-GPU step
+            with_self = [s.dist_pack(T_all) for s in self.shards][0]
         except b.PaError:
             for s in self.shards:
                 s.dist_abort()
@@ -206,22 +215,26 @@ class ShardedAnnealer:
                 s_off = 0
                 for dst in range(self.world):
                     n = int(counts[src][dst])
+                    if src == dst and not with_self:
+                        continue
                     if n:
-                        r_off = int(sum(counts[q][dst] for q in range(src)))
+                        r_off = int(sum(counts[q][dst] for q in range(src) if with_self or q != dst))
                         bufs[dst][1][r_off * S:(r_off + n) * S].copy_(bufs[src][0][s_off * S:(s_off + n) * S])
                     s_off += n
         else:
             children, population = self.shards[0].dist_buffers()
             # The exchange is issued on torch's current stream (the local copy directly, NCCL through req.wait()); the
             # library works on the shard's own stream.  When the two differ, order them explicitly in both directions:
-            # dist_resample has already synchronised the library stream, dist_finish must not start before the receives.
+            # the exchange must see what dist_pack enqueued, dist_finish must not start before the receives have landed.
             lib_stream, cur = self.shards[0].stream, None
             if population.is_cuda:
                 import torch
                 cur = torch.cuda.current_stream(population.device)
                 if cur != lib_stream:
                     cur.wait_stream(lib_stream)
-            exchange_slices(self.g, children, population, counts, S)
+                if self.g.backend == "nccl" and self.world > 1:
+                    lib_stream.synchronize()  # NCCL runs on its own stream: hand it finished buffers
+            exchange_slices(self.g, children, population, counts, S, with_self=with_self)
             if cur is not None and cur != lib_stream:
                 lib_stream.wait_stream(cur)
         self.last_T, self.last_counts, self.last_new_start = T_all, counts, ns
