@@ -341,6 +341,20 @@ def theta1_leg(binding, torch, wl, steps=20, warmup=3):
            "share_sweep_incl_gather": prof["sweep"][0] / total}
     del pa
     torch.cuda.empty_cache()
+    # the same steps through the multi-GPU driver with ONE rank (rank = partition protocol: four library calls, plan, pack,
+    # exchange of nothing): what the sharded step costs on top of the queued one-GPU step where it matters most
+    from paper_2006_00561_b200 import dist
+    sh = dist.ShardedAnnealer(wl.L, wl.R0, seed=wl.seed, beta0=wl.beta0, group=dist.Group())
+    for b_ in schedule(wl, 1, warmup):
+        sh.step(b_, 1)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()  # host clock: the sharded step synchronises four times per step by construction
+    for b_ in schedule(wl, warmup + 1, steps):
+        sh.step(b_, 1)
+    torch.cuda.synchronize()
+    out["sharded_one_rank_ms_per_step"] = 1e3 * (time.perf_counter() - t0) / steps
+    del sh
+    torch.cuda.empty_cache()
     return out
 
 
